@@ -1,0 +1,345 @@
+"""CPU oracle for one PULSE skip-local (collocated) UNet stage.  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this file.  It shares no code with the CUDA path and never imports
+it.  Plain PyTorch CPU ops, fp64 by default (fp32 selectable for the two largest
+configs).
+
+What it follows
+  * PAPER.md:L91 (sec. III): "we allocate local buffers for skip activations and their
+    gradients.  Skip activations are stored locally during the forward pass, and
+    these values are retrieved for gradient computation in the backward pass."
+  * PAPER.md:L142 (sec. IV-B): the model is a linear sequence of operations whose
+    I/O carries "an additional field for storing skip connections".
+  * PAPER.md:L49 (sec. II-A): "Each block contains Attention and ResNet layers"; the
+    inside of a ResNet layer is not in the paper; BASELINE.json north_star fixes it
+    (GroupNorm, SiLU, timestep-embedding add, 3x3 conv, residual add, concat with the
+    cached skip) and SURVEY.md 8c items 1-7 / readings R1-R20 give the formulas.
+Because the stage is an exact reformulation (fusion, virtual concat, caching), the
+oracle is the plain definition: materialise the concat, run ops one at a time on
+[N,C,H,W] tensors, keep every intermediate, back-propagate by the chain rule written
+out below (no autograd anywhere in this file).
+
+Library primitives used as single steps: conv2d / conv_transpose2d / conv2d_weight
+(cross-correlation, its adjoint in the input and in the weight), matmul.  They are
+pinned in tests/test_oracle_pins.py against brute-force direct sums, adjoint
+identities, closed forms and fp64 central differences.  Parity status: pinned (no
+function here is "parity unpinned").
+"""
+from __future__ import annotations
+
+import math
+import torch
+import torch.nn.functional as F
+
+DT = torch.float64
+
+
+# --------------------------------------------------------------------------- elementary pieces
+
+def sigmoid(y):
+    return 1.0 / (1.0 + torch.exp(-y))
+
+
+def silu(y):
+    """SiLU(y) = y * s(y), s = logistic."""
+    return y * sigmoid(y)
+
+
+def silu_grad(y):
+    """d SiLU / dy = s(y) (1 + y (1 - s(y)))."""
+    s = sigmoid(y)
+    return s * (1.0 + y * (1.0 - s))
+
+
+def gn_silu_fwd(x, gamma, beta, groups, eps):
+    """a = SiLU(gamma * xhat + beta), xhat = (x - mu) r, per (n, group) biased variance,
+    r = 1/sqrt(var + eps)  (reading R5)."""
+    n, c, h, w = x.shape
+    xg = x.reshape(n, groups, -1)
+    mu = xg.mean(dim=2, keepdim=True)
+    var = ((xg - mu) ** 2).mean(dim=2, keepdim=True)
+    r = 1.0 / torch.sqrt(var + eps)
+    xhat = ((xg - mu) * r).reshape(n, c, h, w)
+    y = gamma.view(1, c, 1, 1) * xhat + beta.view(1, c, 1, 1)
+    return silu(y), {"xhat": xhat, "r": r, "y": y, "groups": groups}
+
+
+def gn_silu_bwd(g_a, ctx, gamma):
+    """g_y = g_a SiLU'(y); dgamma = sum g_y xhat; dbeta = sum g_y; q = g_y gamma;
+    A = mean_S q; B = mean_S q xhat; g_x = r (q - A - xhat B)."""
+    xhat, r, y, groups = ctx["xhat"], ctx["r"], ctx["y"], ctx["groups"]
+    n, c, h, w = xhat.shape
+    g_y = g_a * silu_grad(y)
+    dgamma = (g_y * xhat).sum(dim=(0, 2, 3))
+    dbeta = g_y.sum(dim=(0, 2, 3))
+    q = (g_y * gamma.view(1, c, 1, 1)).reshape(n, groups, -1)
+    xh = xhat.reshape(n, groups, -1)
+    A = q.mean(dim=2, keepdim=True)
+    B = (q * xh).mean(dim=2, keepdim=True)
+    g_x = (r * (q - A - xh * B)).reshape(n, c, h, w)
+    return g_x, dgamma, dbeta
+
+
+def conv_fwd(x, w, b, stride=1):
+    """out[n,co,y,x] = b[co] + sum_{ci,r,s} W[co,ci,r,s] in[n,ci,y st+r-pad,x st+s-pad],
+    zero outside, pad = (k-1)/2."""
+    return F.conv2d(x, w, b, stride=stride, padding=(w.shape[-1] - 1) // 2)
+
+
+def conv_dgrad(g, w, in_hw, stride=1):
+    """Adjoint of conv_fwd in its input (scatter of the same sum)."""
+    pad = (w.shape[-1] - 1) // 2
+    k = w.shape[-1]
+    oph = in_hw[0] - ((g.shape[2] - 1) * stride - 2 * pad + k)
+    opw = in_hw[1] - ((g.shape[3] - 1) * stride - 2 * pad + k)
+    return F.conv_transpose2d(g, w, None, stride=stride, padding=pad, output_padding=(oph, opw))
+
+
+def conv_wgrad(x, g, w_shape, stride=1):
+    """dW[co,ci,r,s] = sum_{n,y,x} g[n,co,y,x] in[n,ci,y st+r-pad,x st+s-pad]; db = sum g."""
+    pad = (w_shape[-1] - 1) // 2
+    dw = torch.nn.grad.conv2d_weight(x, w_shape, g, stride=stride, padding=pad)
+    return dw, g.sum(dim=(0, 2, 3))
+
+
+def upsample2(d):
+    """u[n,c,Y,X] = d[n,c,Y//2,X//2]."""
+    return d.repeat_interleave(2, dim=2).repeat_interleave(2, dim=3)
+
+
+def upsample2_bwd(g_u):
+    """g_d[y,x] = sum_{i,j in {0,1}} g_u[2y+i, 2x+j]."""
+    n, c, h, w = g_u.shape
+    return g_u.reshape(n, c, h // 2, 2, w // 2, 2).sum(dim=(3, 5))
+
+
+# --------------------------------------------------------------------------- time embedding
+
+def sinusoidal(t, d, dtype=DT):
+    """emb0[n,i] = cos(t_n f_i), emb0[n,half+i] = sin(t_n f_i), f_i = exp(-ln(10000) i/half)
+    (reading R15)."""
+    half = d // 2
+    f = torch.exp(-math.log(10000.0) * torch.arange(half, dtype=dtype) / half)
+    a = t.to(dtype).view(-1, 1) * f.view(1, -1)
+    return torch.cat([torch.cos(a), torch.sin(a)], dim=1)
+
+
+def temb_fwd(desc, P, t, dtype=DT):
+    """emb = emb0 (config 1) or W2 SiLU(W1 emb0 + b1) + b2 (configs 2-5)."""
+    emb0 = sinusoidal(t, desc["temb"]["d0"], dtype)
+    if desc["temb"]["kind"] == "sinusoidal":
+        return emb0, {"emb0": emb0}
+    z1 = emb0 @ P["temb.w1"].T + P["temb.b1"]
+    emb = silu(z1) @ P["temb.w2"].T + P["temb.b2"]
+    return emb, {"emb0": emb0, "z1": z1}
+
+
+def temb_bwd(desc, P, ctx, g_emb):
+    grads = {}
+    if desc["temb"]["kind"] == "sinusoidal":
+        return grads
+    a1 = silu(ctx["z1"])
+    grads["temb.w2"] = g_emb.T @ a1
+    grads["temb.b2"] = g_emb.sum(0)
+    g_z1 = (g_emb @ P["temb.w2"]) * silu_grad(ctx["z1"])
+    grads["temb.w1"] = g_z1.T @ ctx["emb0"]
+    grads["temb.b1"] = g_z1.sum(0)
+    return grads
+
+
+# --------------------------------------------------------------------------- ResBlock
+
+def resblock_fwd(P, p, x, emb, groups, eps):
+    """a1 = SiLU(GN1(x)); h1 = conv1(a1) + pr[n,c]; a2 = SiLU(GN2(h1));
+    out = conv2(a2) + sc(x); pr = Wt SiLU(emb) + bt; sc = identity if Cin == Cout else 1x1 conv
+    (readings R1, R2)."""
+    a1, c1 = gn_silu_fwd(x, P[p + "gn1.gamma"], P[p + "gn1.beta"], groups, eps)
+    pr = silu(emb) @ P[p + "temb.w"].T + P[p + "temb.b"]
+    h1 = conv_fwd(a1, P[p + "conv1.w"], P[p + "conv1.b"]) + pr[:, :, None, None]
+    a2, c2 = gn_silu_fwd(h1, P[p + "gn2.gamma"], P[p + "gn2.beta"], groups, eps)
+    out = conv_fwd(a2, P[p + "conv2.w"], P[p + "conv2.b"])
+    if (p + "sc.w") in P:
+        out = out + conv_fwd(x, P[p + "sc.w"], P[p + "sc.b"])
+    else:
+        out = out + x
+    return out, {"x": x, "a1": a1, "c1": c1, "h1": h1, "a2": a2, "c2": c2, "emb": emb}
+
+
+def resblock_bwd(P, p, ctx, g_out, G):
+    """Chain rule of resblock_fwd.  Adds parameter grads into G,
+    returns (g_x, g_emb contribution)."""
+    x, emb = ctx["x"], ctx["emb"]
+    hw = x.shape[2:]
+    G[p + "conv2.w"], G[p + "conv2.b"] = conv_wgrad(ctx["a2"], g_out, P[p + "conv2.w"].shape)
+    g_a2 = conv_dgrad(g_out, P[p + "conv2.w"], hw)
+    g_h1, G[p + "gn2.gamma"], G[p + "gn2.beta"] = gn_silu_bwd(g_a2, ctx["c2"], P[p + "gn2.gamma"])
+    g_p = g_h1.sum(dim=(2, 3))
+    G[p + "temb.w"] = g_p.T @ silu(emb)
+    G[p + "temb.b"] = g_p.sum(0)
+    g_emb = (g_p @ P[p + "temb.w"]) * silu_grad(emb)
+    G[p + "conv1.w"], G[p + "conv1.b"] = conv_wgrad(ctx["a1"], g_h1, P[p + "conv1.w"].shape)
+    g_a1 = conv_dgrad(g_h1, P[p + "conv1.w"], hw)
+    g_x, G[p + "gn1.gamma"], G[p + "gn1.beta"] = gn_silu_bwd(g_a1, ctx["c1"], P[p + "gn1.gamma"])
+    if (p + "sc.w") in P:
+        G[p + "sc.w"], G[p + "sc.b"] = conv_wgrad(x, g_out, P[p + "sc.w"].shape)
+        g_x = g_x + conv_dgrad(g_out, P[p + "sc.w"], hw)
+    else:
+        g_x = g_x + g_out
+    return g_x, g_emb
+
+
+# --------------------------------------------------------------------------- the collocated stage
+
+def stage_forward(desc, P, x_in, h_in, emb):
+    """Encoder ops then (closed: mid ops) then decoder ops of one collocated stage.
+    Pushed encoder outputs go to the local skip buffers `skips`; each
+    decoder ResBlock pops the most recent one (LIFO, reading R7) and runs on the
+    materialised concat [h, skip] along C, h first (reading R6)."""
+    G_, eps = desc["groups"], desc["eps"]
+    skips, tape = [], {"enc": [], "mid": [], "dec": []}
+    x = x_in
+    if desc["x_in_is_skip"]:
+        skips.append((0, x))
+    n_push = len(skips)
+    for i, op in enumerate(desc["enc_ops"]):
+        p = f"enc{i}."
+        if op["kind"] == "resblock":
+            x, c = resblock_fwd(P, p, x, emb, G_, eps)
+        elif op["kind"] in ("conv_in", "down"):
+            st = 2 if op["kind"] == "down" else 1
+            c = {"x": x, "stride": st}
+            x = conv_fwd(x, P[p + "conv.w"], P[p + "conv.b"], stride=st)
+        else:
+            raise ValueError(op["kind"])
+        c["push"] = None
+        if op["push"]:
+            c["push"] = n_push
+            skips.append((n_push, x))
+            n_push += 1
+        tape["enc"].append(c)
+    skip_list = [s for _, s in skips]          # what the skip cache holds, in push order
+    outs = {}
+    if desc["link"] == "closed":
+        h = x
+        for i, op in enumerate(desc["mid_ops"]):
+            h, c = resblock_fwd(P, f"mid{i}.", h, emb, G_, eps)
+            tape["mid"].append(c)
+    else:
+        outs["e_out"] = x
+        h = h_in
+    for i, op in enumerate(desc["dec_ops"]):
+        p = f"dec{i}."
+        if op["kind"] == "resblock":
+            k, s = skips.pop()
+            assert s.shape[1] == op["skip"] and h.shape[1] == op["cin"], (p, s.shape, h.shape)
+            h, c = resblock_fwd(P, p, torch.cat([h, s], dim=1), emb, G_, eps)
+            c["pop"], c["ch"] = k, op["cin"]
+        elif op["kind"] == "up":
+            u = upsample2(h)
+            c = {"u": u}
+            h = conv_fwd(u, P[p + "conv.w"], P[p + "conv.b"])
+        elif op["kind"] == "head":
+            a, cg = gn_silu_fwd(h, P[p + "gn.gamma"], P[p + "gn.beta"], G_, eps)
+            c = {"a": a, "cg": cg}
+            h = conv_fwd(a, P[p + "conv.w"], P[p + "conv.b"])
+        else:
+            raise ValueError(op["kind"])
+        tape["dec"].append(c)
+    assert not skips, "every cached skip is consumed exactly once"
+    outs["d_out"] = h
+    return outs, {"tape": tape, "skips": skip_list, "n_push": n_push}
+
+
+def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
+    """Reverse of stage_forward.  Each decoder ResBlock's input gradient is split into
+    g_h and g_skip; g_skip goes to that skip's local gradient buffer, and each pushed
+    tensor's gradient is (gradient from its encoder-chain consumer) + (its skip-gradient
+    buffer)  ("buffers for skip activations and their gradients";
+    SURVEY 8c item 5)."""
+    tape = ctx["tape"]
+    G, g_emb = {}, None
+    skip_grad = [None] * ctx["n_push"]
+    g = g_d_out
+    for i in reversed(range(len(desc["dec_ops"]))):
+        op, c, p = desc["dec_ops"][i], tape["dec"][i], f"dec{i}."
+        if op["kind"] == "resblock":
+            g_x, ge = resblock_bwd(P, p, c, g, G)
+            g_emb = ge if g_emb is None else g_emb + ge
+            g, skip_grad[c["pop"]] = g_x[:, :c["ch"]], g_x[:, c["ch"]:]
+        elif op["kind"] == "up":
+            G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["u"], g, P[p + "conv.w"].shape)
+            g = upsample2_bwd(conv_dgrad(g, P[p + "conv.w"], c["u"].shape[2:]))
+        elif op["kind"] == "head":
+            G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["a"], g, P[p + "conv.w"].shape)
+            g_a = conv_dgrad(g, P[p + "conv.w"], c["a"].shape[2:])
+            g, G[p + "gn.gamma"], G[p + "gn.beta"] = gn_silu_bwd(g_a, c["cg"], P[p + "gn.gamma"])
+    grads_out = {}
+    if desc["link"] == "closed":
+        for i in reversed(range(len(desc["mid_ops"]))):
+            g, ge = resblock_bwd(P, f"mid{i}.", tape["mid"][i], g, G)
+            g_emb = ge if g_emb is None else g_emb + ge
+    else:
+        grads_out["g_h_in"] = g
+        g = g_e_out          # may be None == zeros
+    for i in reversed(range(len(desc["enc_ops"]))):
+        op, c, p = desc["enc_ops"][i], tape["enc"][i], f"enc{i}."
+        if c["push"] is not None:
+            sg = skip_grad[c["push"]]
+            g = sg if g is None else g + sg
+        if g is None:
+            g = torch.zeros_like(conv_fwd(c["x"], P[p + "conv.w"], None, c["stride"])) \
+                if op["kind"] != "resblock" else torch.zeros_like(c["h1"])
+        if op["kind"] == "resblock":
+            g, ge = resblock_bwd(P, p, c, g, G)
+            g_emb = ge if g_emb is None else g_emb + ge
+        else:
+            G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["x"], g, P[p + "conv.w"].shape, c["stride"])
+            g = conv_dgrad(g, P[p + "conv.w"], c["x"].shape[2:], c["stride"])
+    if desc["x_in_is_skip"]:
+        g = g + skip_grad[0]
+    grads_out["g_x_in"] = g
+    grads_out["g_emb"] = g_emb
+    return grads_out, G
+
+
+def mse(d, target, scale=1.0):
+    """L = scale * mean((d - T)^2); g_d = scale * 2 (d - T) / numel."""
+    diff = d - target
+    return scale * (diff ** 2).mean(), scale * 2.0 * diff / diff.numel()
+
+
+def _to(x, dtype):
+    return None if x is None else torch.as_tensor(x).to(dtype)
+
+
+def run_stage(desc, params, mb, loss_scale=1.0, dtype=DT):
+    """One microbatch: temb -> stage forward -> MSE(d_out, target) -> stage backward ->
+    temb backward.  `params`, `mb` as produced by workloads.draw (numpy / tensors)."""
+    P = {k: _to(v, dtype) for k, v in params.items()}
+    x_in, h_in = _to(mb["x_in"], dtype), _to(mb.get("h_in"), dtype)
+    emb, tctx = temb_fwd(desc, P, torch.as_tensor(mb["t"]), dtype)
+    outs, ctx = stage_forward(desc, P, x_in, h_in, emb)
+    loss, g_d = mse(outs["d_out"], _to(mb["target"], dtype), loss_scale)
+    gi, G = stage_backward(desc, P, ctx, g_d, _to(mb.get("g_e_out"), dtype))
+    G.update(temb_bwd(desc, P, tctx, gi["g_emb"]))
+    res = {"loss": loss, "emb": emb, "skips": ctx["skips"], "param_grads": G}
+    res.update(outs)
+    res.update(gi)
+    return res
+
+
+def run_wave(desc, params, mbs, dtype=DT):
+    """configs[4]: forwards F0..F{M-1} then backwards B{M-1}..B0; L_total = mean over
+    microbatches, weight grads summed (reading R16).  The oracle has no notion of
+    time, so the wave order only matters for which skip sets are alive; it reports
+    the peak number of bytes the skip buffers would hold."""
+    M = len(mbs)
+    results = [run_stage(desc, params, mb, 1.0 / M, dtype) for mb in mbs]
+    total = {}
+    for r in results:
+        for k, v in r["param_grads"].items():
+            total[k] = v if k not in total else total[k] + v
+    elem = sum(s.numel() for s in results[0]["skips"])
+    return {"per_mb": results, "param_grads": total, "loss": sum(r["loss"] for r in results),
+            "skip_elements_per_mb": elem, "peak_skip_elements": elem * M}
