@@ -1,0 +1,167 @@
+/* pulse.h - C-ABI of the B200-native PULSE skip-local pipeline stage.
+ *
+ * What a "stage" is: PAPER.md:L91 (sec. III) "we allocate local buffers for skip
+ * activations and their gradients. Skip activations are stored locally during the
+ * forward pass, and these values are retrieved for gradient computation in the
+ * backward pass"; PAPER.md:L142 (sec. IV-B) the model is a linear sequence of
+ * operations whose I/O carries "an additional field for storing skip connections";
+ * PAPER.md:L144 a stage pair = encoder-side ops plus the decoder-side ops that
+ * consume their skips, on one device; PAPER.md:L255 (sec. VI) activations (and so the
+ * skips) of every in-flight microbatch stay resident until its backward.
+ * Block math (GroupNorm, SiLU, temb add, 3x3 conv, residual, concat with the cached
+ * skip) is fixed by BASELINE.json north_star; formulas in SURVEY.md 8c / DESIGN.md.
+ *
+ * Conventions
+ *  - Every call returns pulse_status_t (0 = OK), never throws/aborts/prints;
+ *    pulse_last_error() gives a thread-local message.  Out-params are written only
+ *    on success.
+ *  - "d_" pointers are DEVICE pointers, owned by the caller (the library never
+ *    allocates device memory); all must be 256-byte aligned.  Other pointers are host.
+ *  - Work is enqueued on the caller's stream (a cudaStream_t passed as void*); forward
+ *    and backward never synchronise the host.
+ *  - Activations are NHWC in the stage dtype (fp32 or bf16).  Conv weights are
+ *    [Cout][kh][kw][Cin], linear weights [out][in], all parameters in the stage dtype,
+ *    packed into one buffer at the offsets pulse_stage_param_info reports.  Parameter
+ *    gradients are always fp32, packed likewise.
+ *  - A handle is not thread-safe; distinct handles are independent.
+ */
+#ifndef PULSE_H_
+#define PULSE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  PULSE_OK = 0,
+  PULSE_ERR_INVALID_ARG = 1,      /* null / misaligned pointer, bad enum value */
+  PULSE_ERR_SHAPE = 2,            /* descriptor inconsistent (pops more than pushed, C % groups != 0 ...) */
+  PULSE_ERR_UNSUPPORTED = 3,
+  PULSE_ERR_BUFFER_TOO_SMALL = 4,
+  PULSE_ERR_CACHE = 5,            /* slot busy / unknown microbatch / cache full */
+  PULSE_ERR_STATE = 6,            /* params / workspace not bound, backward without forward */
+  PULSE_ERR_CUDA = 7
+} pulse_status_t;
+
+enum { PULSE_F32 = 0, PULSE_BF16 = 1 };
+enum { PULSE_OP_CONV_IN = 0, PULSE_OP_RESBLOCK = 1, PULSE_OP_DOWN = 2, PULSE_OP_UP = 3, PULSE_OP_HEAD = 4 };
+enum { PULSE_LINK_OPEN = 0, PULSE_LINK_CLOSED = 1 };
+enum { PULSE_TEMB_SINUSOIDAL = 0, PULSE_TEMB_MLP = 1 };
+/* flags */
+enum { PULSE_FLAG_FORCE_SIMT = 1  /* debug: CUDA-core fp32-accumulate convs even for bf16 */ };
+
+/* One operation of the linearised model.  cin excludes the popped skip:
+ * a decoder ResBlock runs on concat_C(h[cin], skip[skip_channels]), h first. */
+typedef struct {
+  int kind;           /* PULSE_OP_* */
+  int cin, cout;
+  int skip_channels;  /* decoder ResBlock: channels of the skip it pops (LIFO); else 0 */
+  int push_skip;      /* encoder op: 1 = its output goes to the skip cache */
+} pulse_op_desc;
+
+typedef struct {
+  int dtype;                         /* PULSE_F32 | PULSE_BF16 */
+  int n, h, w, c_in;                 /* x_in is [n,h,w,c_in] */
+  int groups; float eps;             /* GroupNorm */
+  int temb_kind, temb_d0, temb_dim;  /* sinusoidal(d0) [-> MLP d0->dim->dim]; dim = T */
+  int link;                          /* OPEN: h_in/e_out cross the boundary; CLOSED: h := mid(enc output) */
+  int x_in_is_skip;                  /* 1 = x_in itself is pushed first */
+  int n_enc_ops; const pulse_op_desc* enc_ops;
+  int n_mid_ops; const pulse_op_desc* mid_ops;   /* ResBlocks only; CLOSED only */
+  int n_dec_ops; const pulse_op_desc* dec_ops;
+  int max_inflight;                  /* microbatches forwarded but not yet backwarded */
+  unsigned flags;
+} pulse_stage_desc;
+
+typedef struct pulse_stage pulse_stage_t;
+typedef struct pulse_skip_cache pulse_skip_cache_t;
+
+/* ---- stage life cycle ----------------------------------------------------------- */
+/* Validates the op lists (every skip pushed is popped exactly once, channel counts
+ * chain, C % groups == 0 ...) -> PULSE_ERR_SHAPE otherwise.  The descriptor is copied. */
+pulse_status_t pulse_stage_create(const pulse_stage_desc* desc, pulse_stage_t** out);
+pulse_status_t pulse_stage_destroy(pulse_stage_t* stage);
+
+/* Parameters, in the fixed order temb MLP (w1,b1,w2,b2), then per op of enc, mid, dec:
+ * ResBlock: gn1.gamma gn1.beta conv1.w conv1.b temb.w temb.b gn2.gamma gn2.beta conv2.w
+ * conv2.b [sc.w sc.b if cin+skip != cout]; conv_in/down/up: conv.w conv.b; head: gn.gamma
+ * gn.beta conv.w conv.b.  name points into the handle (valid until destroy). */
+pulse_status_t pulse_stage_param_count(const pulse_stage_t* stage, int* count);
+pulse_status_t pulse_stage_param_info(const pulse_stage_t* stage, int index, const char** name, int* rank,
+                                      int shape[4], size_t* offset_bytes, size_t* grad_offset_bytes);
+pulse_status_t pulse_stage_param_bytes(const pulse_stage_t* stage, size_t* param_bytes, size_t* grad_bytes);
+/* d_params: param_bytes in the stage dtype; d_grads: grad_bytes of fp32.  Both stay
+ * caller-owned and must outlive the calls that use them. */
+pulse_status_t pulse_stage_bind_params(pulse_stage_t* stage, const void* d_params, float* d_grads);
+
+/* Scratch: per_stage bytes (gradient temporaries, skip-gradient buffers, reduction
+ * scratch) + max_inflight * per_inflight_stash bytes (forward intermediates kept for
+ * the backward of each in-flight microbatch).  Bind one buffer of at least that sum. */
+pulse_status_t pulse_stage_workspace_bytes(const pulse_stage_t* stage, size_t* per_stage, size_t* per_inflight_stash);
+pulse_status_t pulse_stage_bind_workspace(pulse_stage_t* stage, void* d_workspace, size_t bytes);
+
+/* ---- skip cache (PAPER.md:L91 local skip buffers; L255 one set per in-flight microbatch) */
+pulse_status_t pulse_skip_cache_bytes(const pulse_stage_t* stage, size_t* bytes_per_slot);
+/* d_mem: slots * bytes_per_slot bytes.  slots must be <= desc.max_inflight. */
+pulse_status_t pulse_skip_cache_create(pulse_stage_t* stage, void* d_mem, size_t bytes, int slots,
+                                       pulse_skip_cache_t** out);
+/* Skip k (push order) of live microbatch mb_id: device pointer and NHWC shape. */
+pulse_status_t pulse_skip_cache_get(const pulse_skip_cache_t* cache, int64_t mb_id, int k, void** d_ptr, int shape[4]);
+pulse_status_t pulse_skip_cache_count(const pulse_skip_cache_t* cache, int* skips_per_slot);
+/* Normally implicit at the end of pulse_stage_backward. */
+pulse_status_t pulse_skip_cache_release(pulse_skip_cache_t* cache, int64_t mb_id);
+pulse_status_t pulse_skip_cache_stats(const pulse_skip_cache_t* cache, int* live_slots, size_t* live_bytes,
+                                      size_t* peak_bytes);
+pulse_status_t pulse_skip_cache_destroy(pulse_skip_cache_t* cache);
+
+/* ---- the hot path ----------------------------------------------------------------- */
+/* Forward of microbatch mb_id: acquires a free slot
+ * (PULSE_ERR_CACHE if mb_id is already live or no slot is free).
+ *  d_x_in  [n,h,w,c_in]                     stage dtype
+ *  d_h_in  OPEN: input of the first decoder op; CLOSED: NULL
+ *  d_temb  [n,temb_dim] fp32 (the embedding after the MLP; see pulse_temb_forward)
+ *  d_e_out OPEN: last encoder output (written); CLOSED: NULL
+ *  d_d_out last decoder output (written) */
+pulse_status_t pulse_stage_forward(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id,
+                                   const void* d_x_in, const void* d_h_in, const float* d_temb,
+                                   void* d_e_out, void* d_d_out, void* stream);
+/* Backward of a live microbatch (rows a8-a11); releases its slot.
+ *  d_g_d_out  gradient of d_out (stage dtype)
+ *  d_g_e_out  OPEN: gradient of e_out or NULL (= zeros); CLOSED: NULL
+ *  d_g_x_in   written if non-NULL
+ *  d_g_h_in   OPEN: written; CLOSED: NULL
+ *  d_g_temb   [n,temb_dim] fp32, accumulated (+=) if non-NULL
+ *  accumulate_wgrad 0: parameter gradients overwritten, 1: += (fp32, row a11) */
+pulse_status_t pulse_stage_backward(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id,
+                                    const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
+                                    void* d_g_h_in, float* d_g_temb, int accumulate_wgrad, void* stream);
+
+/* ---- helpers on the path (row a1, a7) ----------------------------------------------- */
+/* emb0 = [cos(t f_i), sin(t f_i)], f_i = exp(-ln(1e4) i/half); MLP kind: emb = W2 SiLU(W1 emb0 + b1) + b2
+ * using the bound temb.* parameters.  d_t: int64 [n].  d_emb: fp32 [n,temb_dim].
+ * d_stash: fp32 scratch of pulse_temb_stash_elems floats kept by the caller until
+ * pulse_temb_backward of the same microbatch. */
+pulse_status_t pulse_temb_stash_elems(const pulse_stage_t* stage, size_t* elems);
+pulse_status_t pulse_temb_forward(pulse_stage_t* stage, const int64_t* d_t, float* d_emb, float* d_stash, void* stream);
+/* Gradients of temb.w1/b1/w2/b2 from d_g_emb [n,temb_dim] (no-op for the sinusoidal kind). */
+pulse_status_t pulse_temb_backward(pulse_stage_t* stage, const float* d_g_emb, const float* d_stash,
+                                   int accumulate_wgrad, void* stream);
+/* L = scale * mean((d - target)^2) added into *d_loss (fp32, caller zeroes it);
+ * g_d = scale * 2 (d - target) / numel in dtype. */
+pulse_status_t pulse_mse_fwd_bwd(int dtype, const void* d_d, const void* d_target, size_t numel, float scale,
+                                 float* d_loss, void* d_g_d, void* stream);
+
+/* Number of kernels this handle has launched so far (bench.py "gpu_launches"). */
+pulse_status_t pulse_stage_launch_count(const pulse_stage_t* stage, uint64_t* launches);
+
+int pulse_version(void);
+const char* pulse_status_string(pulse_status_t s);
+const char* pulse_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PULSE_H_ */

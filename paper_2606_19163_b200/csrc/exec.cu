@@ -1,0 +1,343 @@
+// exec.cu - pulse_stage_forward / pulse_stage_backward / temb and loss helpers:
+// walks the op plan and enqueues kernels.  Rows a1-a11 of SURVEY.md 8a.
+#include "stage.h"
+
+using namespace pulse;
+
+namespace {
+
+struct Ctx {
+  pulse_stage* s;
+  char* skip;     // base of this microbatch's skip-cache slot
+  char* stash;    // base of this microbatch's stash
+  char* work;     // per-stage workspace
+  cudaStream_t st;
+  int dt;
+  char* fwd(int t) const {
+    const TRef& r = s->tensors[t].ref;
+    return (r.region == R_SKIP ? skip : r.region == R_STASH ? stash : work) + r.off;
+  }
+  char* grad(int t) const { return work + s->tensors[t].goff; }
+  const char* par(int p) const { return s->d_params + s->params[p].off; }
+  float* pgrad(int p) const { return (float*)((char*)s->d_grads + s->params[p].goff); }
+  size_t bytes(int t) const {
+    const TRef& r = s->tensors[t].ref;
+    return (size_t)s->d.n * r.h * r.w * r.c * s->esz();
+  }
+  bool tc() const { return dt == DT_BF16 && !(s->d.flags & PULSE_FLAG_FORCE_SIMT); }
+};
+
+void run_conv(Ctx& c, const ConvArgs& a) {
+  if (c.tc() && conv_tc_supported(a)) c.s->launches += conv_tc(a, c.st);
+  else c.s->launches += conv_simt(a, c.st);
+}
+void run_wgrad(Ctx& c, const WgradArgs& a) {
+  if (c.tc() && wgrad_tc_supported(a)) c.s->launches += wgrad_tc(a, c.st);
+  else c.s->launches += wgrad_simt(a, c.st);
+}
+
+ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, int k, int stride, const void* w,
+                   int cout, const void* bias, const float* pn, const void* res, void* out) {
+  ConvArgs a;
+  a.dt = c.dt; a.src = src; a.n = c.s->d.n; a.hin = hin; a.win = win; a.hout = hout; a.wout = wout;
+  a.ksize = k; a.stride = stride; a.mode = CONV_FPROP; a.w = w; a.cout = cout; a.bias = bias; a.pn = pn;
+  a.residual = res; a.out = out; a.accumulate = 0;
+  return a;
+}
+
+// dgrad of a stride-1 conv == fprop with flipped/transposed weights
+void run_dgrad(Ctx& c, const void* g, int h, int w, int cout, const void* wts, int k, int cin, void* g_in,
+               int accumulate, int stride, int hin, int win) {
+  char* wt = c.work + c.s->w_wt;
+  c.s->launches += flip_transpose(c.dt, wts, cout, k, cin, wt, c.st);
+  Cat src{g, cout, nullptr, 0};
+  ConvArgs a = conv_args(c, src, h, w, hin, win, k, 1, wt, cin, nullptr, nullptr, nullptr, g_in);
+  a.accumulate = accumulate;
+  if (stride == 2) a.mode = CONV_DGRAD_S2;
+  run_conv(c, a);
+}
+
+void resblock_forward(Ctx& c, const OpPlan& op, const float* emb) {
+  pulse_stage* s = c.s;
+  const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip, T = s->d.temb_dim;
+  Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
+  float* partial = (float*)(c.work + s->w_partial);
+  float* stats1 = (float*)(c.stash + op.stats1);
+  float* stats2 = (float*)(c.stash + op.stats2);
+  float* pn = (float*)(c.stash + op.pn);
+  s->launches += gn_silu_fwd(c.dt, x, n, hw, s->d.groups, s->d.eps, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]),
+                             c.fwd(op.a1), stats1, partial, c.st);
+  s->launches += linear_fwd(c.dt, emb, n, T, op.cout, c.par(op.p[P_TW]), c.par(op.p[P_TB]), 1, pn, c.st);
+  Cat a1{c.fwd(op.a1), ctot, nullptr, 0};
+  run_conv(c, conv_args(c, a1, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C1W]), op.cout,
+                        c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)));
+  Cat h1{c.fwd(op.h1), op.cout, nullptr, 0};
+  s->launches += gn_silu_fwd(c.dt, h1, n, hw, s->d.groups, s->d.eps, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
+                             c.fwd(op.a2), stats2, partial, c.st);
+  const void* res = c.fwd(op.x0);
+  if (op.p[P_SCW] >= 0) {
+    run_conv(c, conv_args(c, x, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_SCW]), op.cout,
+                          c.par(op.p[P_SCB]), nullptr, nullptr, c.fwd(op.out)));
+    res = c.fwd(op.out);
+  }
+  Cat a2{c.fwd(op.a2), op.cout, nullptr, 0};
+  run_conv(c, conv_args(c, a2, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C2W]), op.cout,
+                        c.par(op.p[P_C2B]), nullptr, res, c.fwd(op.out)));
+  (void)ctot;
+}
+
+void resblock_backward(Ctx& c, const OpPlan& op, const float* emb, float* g_temb) {
+  pulse_stage* s = c.s;
+  const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip, T = s->d.temb_dim;
+  Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
+  float* partial = (float*)(c.work + s->w_partial);
+  float* coef = (float*)(c.work + s->w_coef);
+  float* gp = (float*)(c.work + s->w_gp);
+  char* g_out = c.grad(op.out);
+  char* g_a2 = c.work + s->w_ga2;
+  char* g_h1 = c.work + s->w_gh1;
+  char* g_a1 = c.work + s->w_ga1;
+  char* g_sc = c.work + s->w_gsc;
+  // conv2: bias grad, wgrad, dgrad
+  s->launches += colsum(c.dt, g_out, n, hw, op.cout, nullptr, c.pgrad(op.p[P_C2B]), partial, c.st);
+  if (op.p[P_SCB] >= 0) s->launches += colsum(c.dt, g_out, n, hw, op.cout, nullptr, c.pgrad(op.p[P_SCB]), partial, c.st);
+  WgradArgs w2{c.dt, Cat{c.fwd(op.a2), op.cout, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
+               c.pgrad(op.p[P_C2W])};
+  run_wgrad(c, w2);
+  run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C2W]), 3, op.cout, g_a2, 0, 1, op.hin, op.win);
+  // GN2 + SiLU backward -> g_h1
+  s->launches += gn_silu_bwd(c.dt, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, n, hw, s->d.groups,
+                             c.par(op.p[P_GN2G]), (const float*)(c.stash + op.stats2), nullptr, g_h1, op.cout, 0,
+                             nullptr, 0, c.pgrad(op.p[P_GN2G]), c.pgrad(op.p[P_GN2B]), partial, coef, c.st);
+  // temb projection: g_p[n,c] = sum_hw g_h1; conv1 bias grad = sum_n g_p
+  s->launches += colsum(c.dt, g_h1, n, hw, op.cout, gp, c.pgrad(op.p[P_C1B]), partial, c.st);
+  s->launches += linear_bwd(c.dt, emb, gp, n, T, op.cout, c.par(op.p[P_TW]), 1, c.pgrad(op.p[P_TW]),
+                            c.pgrad(op.p[P_TB]), g_temb, 1, c.st);
+  // conv1: wgrad, dgrad
+  WgradArgs w1{c.dt, Cat{c.fwd(op.a1), ctot, nullptr, 0}, n, op.hin, op.win, g_h1, op.hin, op.win, op.cout, 3, 1,
+               c.pgrad(op.p[P_C1W])};
+  run_wgrad(c, w1);
+  run_dgrad(c, g_h1, op.hin, op.win, op.cout, c.par(op.p[P_C1W]), 3, ctot, g_a1, 0, 1, op.hin, op.win);
+  // shortcut
+  const void* add = g_out;
+  if (op.p[P_SCW] >= 0) {
+    WgradArgs ws{c.dt, x, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 1, 1, c.pgrad(op.p[P_SCW])};
+    run_wgrad(c, ws);
+    run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_SCW]), 1, ctot, g_sc, 0, 1, op.hin, op.win);
+    add = g_sc;
+  }
+  // GN1 + SiLU backward, split into g_h and g_skip (skip gradient accumulated locally)
+  s->launches += gn_silu_bwd(c.dt, g_a1, x, n, hw, s->d.groups, c.par(op.p[P_GN1G]),
+                             (const float*)(c.stash + op.stats1), add, c.grad(op.x0), op.cin, op.acc_x0,
+                             op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]),
+                             c.pgrad(op.p[P_GN1B]), partial, coef, c.st);
+}
+
+pulse_status_t check_bound(pulse_stage* s, pulse_skip_cache* cache) {
+  if (!s || !cache) return fail(PULSE_ERR_INVALID_ARG, "null stage / cache");
+  if (cache->stage != s) return fail(PULSE_ERR_INVALID_ARG, "cache belongs to another stage");
+  if (!s->d_params || !s->d_grads) return fail(PULSE_ERR_STATE, "parameters not bound");
+  if (!s->d_work) return fail(PULSE_ERR_STATE, "workspace not bound");
+  return PULSE_OK;
+}
+
+}  // namespace
+
+extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
+                                              const void* d_x_in, const void* d_h_in, const float* d_temb,
+                                              void* d_e_out, void* d_d_out, void* stream) {
+  pulse_status_t stt = check_bound(s, cache);
+  if (stt) return stt;
+  const bool open = s->d.link == PULSE_LINK_OPEN;
+  if (!d_x_in || !d_temb || !d_d_out || mb < 0) return fail(PULSE_ERR_INVALID_ARG, "null x_in / temb / d_out or negative mb_id");
+  if (open && (!d_h_in || !d_e_out)) return fail(PULSE_ERR_INVALID_ARG, "OPEN stage needs h_in and e_out");
+  if (!open && (d_h_in || d_e_out)) return fail(PULSE_ERR_INVALID_ARG, "CLOSED stage takes no h_in / e_out");
+  int slot = -1;
+  for (int i = 0; i < cache->slots; ++i) {
+    if (cache->mb[i] == mb) return fail(PULSE_ERR_CACHE, "microbatch %lld is already live", (long long)mb);
+    if (cache->mb[i] < 0 && slot < 0) slot = i;
+  }
+  if (slot < 0) return fail(PULSE_ERR_CACHE, "skip cache full (%d slots)", cache->slots);
+  Ctx c;
+  c.s = s; c.st = (cudaStream_t)stream; c.dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
+  c.skip = cache->base + (size_t)slot * cache->bytes_per_slot;
+  c.work = s->d_work;
+  c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
+  float* emb = (float*)(c.stash + s->emb_off);
+  CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
+  CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
+  if (open) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
+  for (size_t i = 0; i < s->ops.size(); ++i) {
+    const OpPlan& op = s->ops[i];
+    if (open && (int)i == s->n_enc)   // decoder starts: the first decoder op reads h_in
+      ;
+    switch (op.kind) {
+      case PULSE_OP_RESBLOCK: resblock_forward(c, op, emb); break;
+      case PULSE_OP_CONV_IN:
+      case PULSE_OP_DOWN: {
+        const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
+        run_conv(c, conv_args(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin, op.win, op.hout, op.wout, 3, stride,
+                              c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
+        break;
+      }
+      case PULSE_OP_UP: {
+        s->launches += upsample2(c.dt, c.fwd(op.x0), s->d.n, op.hin, op.win, op.cin, c.fwd(op.u), c.st);
+        run_conv(c, conv_args(c, Cat{c.fwd(op.u), op.cin, nullptr, 0}, op.hout, op.wout, op.hout, op.wout, 3, 1,
+                              c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
+        break;
+      }
+      case PULSE_OP_HEAD: {
+        s->launches += gn_silu_fwd(c.dt, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, s->d.n, op.hin * op.win, s->d.groups,
+                                   s->d.eps, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1),
+                                   (float*)(c.stash + op.stats1), (float*)(c.work + s->w_partial), c.st);
+        run_conv(c, conv_args(c, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, op.hin, op.win, op.hin, op.win, 3, 1,
+                              c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
+        break;
+      }
+    }
+  }
+  if (open) CK_CUDA(cudaMemcpyAsync(d_e_out, c.fwd(s->t_eout), c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
+  CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+  CK_CUDA(cudaGetLastError());
+  cache->mb[slot] = mb;
+  cache->live++;
+  const size_t lb = (size_t)cache->live * cache->bytes_per_slot;
+  if (lb > cache->peak_bytes) cache->peak_bytes = lb;
+  return PULSE_OK;
+}
+
+extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
+                                               const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
+                                               void* d_g_h_in, float* d_g_temb, int accumulate_wgrad, void* stream) {
+  pulse_status_t stt = check_bound(s, cache);
+  if (stt) return stt;
+  const bool open = s->d.link == PULSE_LINK_OPEN;
+  if (!d_g_d_out || mb < 0) return fail(PULSE_ERR_INVALID_ARG, "null g_d_out or negative mb_id");
+  if (open && !d_g_h_in) return fail(PULSE_ERR_INVALID_ARG, "OPEN stage needs g_h_in");
+  if (!open && (d_g_h_in || d_g_e_out)) return fail(PULSE_ERR_INVALID_ARG, "CLOSED stage takes no g_h_in / g_e_out");
+  int slot = -1;
+  for (int i = 0; i < cache->slots; ++i) if (cache->mb[i] == mb) slot = i;
+  if (slot < 0) return fail(PULSE_ERR_STATE, "backward of microbatch %lld without a live forward", (long long)mb);
+  Ctx c;
+  c.s = s; c.st = (cudaStream_t)stream; c.dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
+  c.skip = cache->base + (size_t)slot * cache->bytes_per_slot;
+  c.work = s->d_work;
+  c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
+  const float* emb = (const float*)(c.stash + s->emb_off);
+  if (!accumulate_wgrad)
+    CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
+  CK_CUDA(cudaMemcpyAsync(c.grad(s->t_dout), d_g_d_out, c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+  if (open) {
+    if (d_g_e_out) CK_CUDA(cudaMemcpyAsync(c.grad(s->t_eout), d_g_e_out, c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
+    else CK_CUDA(cudaMemsetAsync(c.grad(s->t_eout), 0, c.bytes(s->t_eout), c.st));
+  }
+  float* partial = (float*)(c.work + s->w_partial);
+  for (int i = (int)s->ops.size() - 1; i >= 0; --i) {
+    const OpPlan& op = s->ops[i];
+    const int n = s->d.n;
+    switch (op.kind) {
+      case PULSE_OP_RESBLOCK: resblock_backward(c, op, emb, d_g_temb); break;
+      case PULSE_OP_CONV_IN:
+      case PULSE_OP_DOWN: {
+        const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
+        char* g_out = c.grad(op.out);
+        s->launches += colsum(c.dt, g_out, n, op.hout * op.wout, op.cout, nullptr, c.pgrad(op.p[P_C1B]), partial, c.st);
+        WgradArgs w{c.dt, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, n, op.hin, op.win, g_out, op.hout, op.wout, op.cout, 3,
+                    stride, c.pgrad(op.p[P_C1W])};
+        run_wgrad(c, w);
+        const bool need_gx = !(op.x0 == s->t_xin && !d_g_x_in);
+        if (need_gx)
+          run_dgrad(c, g_out, op.hout, op.wout, op.cout, c.par(op.p[P_C1W]), 3, op.cin, c.grad(op.x0), op.acc_x0,
+                    stride, op.hin, op.win);
+        break;
+      }
+      case PULSE_OP_UP: {
+        char* g_out = c.grad(op.out);
+        char* g_u = c.work + s->w_gu;
+        s->launches += colsum(c.dt, g_out, n, op.hout * op.wout, op.cout, nullptr, c.pgrad(op.p[P_C1B]), partial, c.st);
+        WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
+                    1, c.pgrad(op.p[P_C1W])};
+        run_wgrad(c, w);
+        run_dgrad(c, g_out, op.hout, op.wout, op.cout, c.par(op.p[P_C1W]), 3, op.cin, g_u, 0, 1, op.hout, op.wout);
+        s->launches += upsample2_bwd(c.dt, g_u, n, op.hin, op.win, op.cin, c.grad(op.x0), c.st);
+        break;
+      }
+      case PULSE_OP_HEAD: {
+        char* g_out = c.grad(op.out);
+        char* g_a = c.work + s->w_ga1;
+        s->launches += colsum(c.dt, g_out, n, op.hin * op.win, op.cout, nullptr, c.pgrad(op.p[P_C1B]), partial, c.st);
+        WgradArgs w{c.dt, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
+                    c.pgrad(op.p[P_C1W])};
+        run_wgrad(c, w);
+        run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C1W]), 3, op.cin, g_a, 0, 1, op.hin, op.win);
+        s->launches += gn_silu_bwd(c.dt, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, n, op.hin * op.win, s->d.groups,
+                                   c.par(op.p[P_GN1G]), (const float*)(c.stash + op.stats1), nullptr, c.grad(op.x0),
+                                   op.cin, 0, nullptr, 0, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]), partial,
+                                   (float*)(c.work + s->w_coef), c.st);
+        break;
+      }
+    }
+  }
+  if (open) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
+  if (d_g_x_in) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
+  CK_CUDA(cudaGetLastError());
+  cache->mb[slot] = -1;
+  cache->live--;
+  return PULSE_OK;
+}
+
+// ------------------------------------------------------------------------------ temb, loss
+extern "C" pulse_status_t pulse_temb_stash_elems(const pulse_stage_t* s, size_t* elems) {
+  if (!s || !elems) return fail(PULSE_ERR_INVALID_ARG, "null argument");
+  *elems = (size_t)s->d.n * (s->d.temb_d0 + s->d.temb_dim);
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_temb_forward(pulse_stage_t* s, const int64_t* d_t, float* d_emb, float* d_stash,
+                                             void* stream) {
+  if (!s || !d_t || !d_emb || !d_stash) return fail(PULSE_ERR_INVALID_ARG, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n = s->d.n, d0 = s->d.temb_d0, T = s->d.temb_dim;
+  const int dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
+  if (s->d.temb_kind == PULSE_TEMB_SINUSOIDAL) {
+    s->launches += sinusoidal(d_t, n, d0, d_emb, st);
+  } else {
+    if (!s->d_params) return fail(PULSE_ERR_STATE, "parameters not bound");
+    float* emb0 = d_stash;
+    float* z1 = d_stash + (size_t)n * d0;
+    s->launches += sinusoidal(d_t, n, d0, emb0, st);
+    s->launches += linear_fwd(dt, emb0, n, d0, T, s->d_params + s->params[0].off, s->d_params + s->params[1].off, 0, z1, st);
+    s->launches += linear_fwd(dt, z1, n, T, T, s->d_params + s->params[2].off, s->d_params + s->params[3].off, 1, d_emb, st);
+  }
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_temb_backward(pulse_stage_t* s, const float* d_g_emb, const float* d_stash,
+                                              int accumulate_wgrad, void* stream) {
+  if (!s || !d_g_emb || !d_stash) return fail(PULSE_ERR_INVALID_ARG, "null argument");
+  if (s->d.temb_kind == PULSE_TEMB_SINUSOIDAL) return PULSE_OK;
+  if (!s->d_params || !s->d_grads || !s->d_work) return fail(PULSE_ERR_STATE, "parameters / workspace not bound");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n = s->d.n, d0 = s->d.temb_d0, T = s->d.temb_dim;
+  const int dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
+  if (!accumulate_wgrad) CK_CUDA(cudaMemsetAsync(s->d_grads, 0, s->temb_grad_bytes, st));
+  const float* emb0 = d_stash;
+  const float* z1 = d_stash + (size_t)n * d0;
+  float* g_z1 = (float*)(s->d_work + s->w_tmpf);     // [n,T] fp32
+  auto G = [&](int p) { return (float*)((char*)s->d_grads + s->params[p].goff); };
+  // emb = W2 silu(z1) + b2
+  s->launches += linear_bwd(dt, z1, d_g_emb, n, T, T, s->d_params + s->params[2].off, 1, G(2), G(3), g_z1, 0, st);
+  // z1 = W1 emb0 + b1
+  s->launches += linear_bwd(dt, emb0, g_z1, n, d0, T, s->d_params + s->params[0].off, 0, G(0), G(1), nullptr, 0, st);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_mse_fwd_bwd(int dtype, const void* d_d, const void* d_target, size_t numel, float scale,
+                                            float* d_loss, void* d_g_d, void* stream) {
+  if (!d_d || !d_target || !d_loss || !d_g_d) return fail(PULSE_ERR_INVALID_ARG, "null argument");
+  if (dtype != PULSE_F32 && dtype != PULSE_BF16) return fail(PULSE_ERR_INVALID_ARG, "dtype");
+  const int V = dtype == PULSE_F32 ? 4 : 8;
+  if (numel == 0 || numel % V) return fail(PULSE_ERR_SHAPE, "numel must be a positive multiple of %d", V);
+  mse_fwd_bwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_d, d_target, numel, scale, d_loss, d_g_d, (cudaStream_t)stream);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}

@@ -1,0 +1,87 @@
+// kernels.h - host launchers of the CUDA kernels (internal to libpulse.so).
+// Every launcher enqueues on `st`, returns the number of kernels it launched.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace pulse {
+
+enum { DT_F32 = 0, DT_BF16 = 1 };
+static inline size_t dt_size(int dt) { return dt == DT_F32 ? 4 : 2; }
+
+// Channel concat of two NHWC tensors with equal N,H,W (the "virtual concat": PAPER.md
+// L91 skip buffer read in place, north_star "concat fused into the operand loader").
+struct Cat {
+  const void* p0; int c0;
+  const void* p1; int c1;     // p1 == nullptr, c1 == 0 for a single source
+  int c() const { return c0 + c1; }
+};
+
+// ---- GroupNorm + SiLU -------------------------------------------
+struct GnPlan { int nchunks, tpr, rows; };
+GnPlan gn_plan(int dt, int hw, int c, int n);
+size_t gn_partial_elems(const GnPlan& p, int n, int c);   // floats of scratch for partial sums
+// stats: [N][4][C] fp32 = {scale = r*gamma, shift = beta - mu*r*gamma, r, mu*r}
+int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
+                void* a_out, float* stats, float* partial, cudaStream_t st);
+// g_x = r(gamma g_y - A - xhat B) [+ add]; channels [0,dc0) -> dst0, rest -> dst1; accX: += instead of =
+// dgamma/dbeta: fp32, atomically accumulated.  coef: [N][2][C] fp32 scratch.
+int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, const void* gamma,
+                const float* stats, const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1,
+                float* dgamma, float* dbeta, float* partial, float* coef, cudaStream_t st);
+
+// ---- small ops -----------------------------------------------------------------------
+// s[n][c] = sum over pixels of g[n][hw][c];  out_n[n][c] = s (if non-null);
+// out_tot[c] += sum_n s (if non-null)
+int colsum(int dt, const void* g, int n, int hw, int c, float* out_n, float* out_tot, float* partial,
+           cudaStream_t st);
+size_t colsum_partial_elems(int dt, int n, int hw, int c);
+// out[n][o] = sum_i W[o][i] f(in[n][i]) + b[o]; f = SiLU if silu_in.  W,b in dtype dt; in/out fp32
+int linear_fwd(int dt, const float* in, int n, int din, int dout, const void* w, const void* b, int silu_in,
+               float* out, cudaStream_t st);
+// dW[o][i] += sum_n g[n][o] f(in[n][i]); db[o] += sum_n g[n][o];
+// g_in[n][i] (+)= (sum_o g[n][o] W[o][i]) f'(in[n][i])   (g_in may be null)
+int linear_bwd(int dt, const float* in, const float* g, int n, int din, int dout, const void* w, int silu_in,
+               float* dw, float* db, float* g_in, int acc_g_in, cudaStream_t st);
+int sinusoidal(const int64_t* t, int n, int d, float* out, cudaStream_t st);
+int mse_fwd_bwd(int dt, const void* d, const void* target, size_t numel, float scale, float* loss, void* g,
+                cudaStream_t st);
+int upsample2(int dt, const void* in, int n, int h, int w, int c, void* out, cudaStream_t st);
+int upsample2_bwd(int dt, const void* g_u, int n, int h, int w, int c, void* g_out, cudaStream_t st);  // h,w: low-res
+int add_inplace(int dt, void* dst, const void* src, size_t numel, cudaStream_t st);
+// Wt[ci][k-1-r][k-1-s][co] = W[co][r][s][ci]
+int flip_transpose(int dt, const void* w, int cout, int k, int cin, void* wt, cudaStream_t st);
+
+// ---- convolution ---------------------------------------------------
+enum { CONV_FPROP = 0, CONV_DGRAD_S2 = 1 };
+struct ConvArgs {
+  int dt;
+  Cat src; int n, hin, win;       // source tensor(s) [n,hin,win,c]
+  int hout, wout;                 // output pixels
+  int ksize, stride, mode;        // mode CONV_DGRAD_S2: src pixel = (y + r - pad)/2 when even (stride ignored)
+  const void* w;                  // [cout][k][k][src.c()]
+  int cout;
+  const void* bias;               // [cout] dtype, or null
+  const float* pn;                // [n][cout] fp32 per-sample bias (temb projection), or null
+  const void* residual;           // [n,hout,wout,cout] dtype, added, or null (may alias out)
+  void* out; int accumulate;      // out (+)= result
+};
+int conv_simt(const ConvArgs& a, cudaStream_t st);
+struct WgradArgs {
+  int dt;
+  Cat src; int n, hin, win;       // forward input
+  const void* g; int hout, wout, cout;   // forward output gradient [n,hout,wout,cout]
+  int ksize, stride;
+  float* dw;                      // [cout][k][k][src.c()] fp32, atomically accumulated
+};
+int wgrad_simt(const WgradArgs& a, cudaStream_t st);
+
+// tcgen05 / TMA path (bf16 only).  *_supported say whether the shape maps onto the tiles.
+bool conv_tc_supported(const ConvArgs& a);
+int conv_tc(const ConvArgs& a, cudaStream_t st);
+bool wgrad_tc_supported(const WgradArgs& a);
+int wgrad_tc(const WgradArgs& a, cudaStream_t st);
+const char* tc_last_error();
+
+}  // namespace pulse

@@ -1,0 +1,377 @@
+// misc.cu - the small, HBM- or latency-bound ops of the stage: per-channel pixel sums
+// (bias / temb-projection gradients), the [N<=16, <=1280] linears of the timestep path,
+// sinusoidal embedding, MSE loss+gradient, nearest-2x upsample and its adjoint, in-place
+// add, and the weight flip/transpose that turns dgrad into fprop.
+#include "common.cuh"
+#include "kernels.h"
+
+namespace pulse {
+
+// ------------------------------------------------------------------ column sums over pixels
+static void colsum_plan(int dt, int n, int hw, int c, int& tpr, int& rows, int& nchunks) {
+  const int vec = dt == DT_F32 ? 4 : 8;
+  tpr = c / vec;
+  rows = tpr >= 256 ? 1 : 256 / tpr;
+  if (rows > hw) rows = hw;
+  int maxc = hw / (rows * 4);
+  if (maxc < 1) maxc = 1;
+  int want = (592 + n - 1) / n;
+  nchunks = want < maxc ? want : maxc;
+}
+size_t colsum_partial_elems(int dt, int n, int hw, int c) {
+  int tpr, rows, nchunks;
+  colsum_plan(dt, n, hw, c, tpr, rows, nchunks);
+  return (size_t)n * nchunks * c;
+}
+
+template <typename T>
+__global__ void colsum_partial_k(const T* __restrict__ g, int hw, int C, float* __restrict__ partial) {
+  constexpr int V = Vec<T>::N;
+  extern __shared__ float sm[];
+  const int n = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x;
+  const int ppc = (hw + nchunks - 1) / nchunks;
+  const int pb = chunk * ppc, pe = min(hw, pb + ppc);
+  const int ch = threadIdx.x * V, rows = blockDim.y, ty = threadIdx.y;
+  float s[V];
+#pragma unroll
+  for (int i = 0; i < V; ++i) s[i] = 0.f;
+  for (int p = pb + ty; p < pe; p += rows) {
+    float v[V];
+    ldv(g + ((size_t)n * hw + p) * C + ch, v);
+#pragma unroll
+    for (int i = 0; i < V; ++i) s[i] += v[i];
+  }
+  if (rows > 1) {
+#pragma unroll
+    for (int i = 0; i < V; ++i) sm[ty * C + ch + i] = s[i];
+    __syncthreads();
+    if (ty == 0) {
+#pragma unroll
+      for (int i = 0; i < V; ++i) {
+        float u = 0.f;
+        for (int r = 0; r < rows; ++r) u += sm[r * C + ch + i];
+        s[i] = u;
+      }
+    }
+  }
+  if (ty == 0) {
+    float* o = partial + ((size_t)n * nchunks + chunk) * C + ch;
+#pragma unroll
+    for (int i = 0; i < V; ++i) o[i] = s[i];
+  }
+}
+
+__global__ void colsum_finalize_k(const float* __restrict__ partial, int n, int nchunks, int C, float* out_n,
+                                  float* out_tot) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= C) return;
+  float tot = 0.f;
+  for (int nn = 0; nn < n; ++nn) {
+    float s = 0.f;
+    for (int k = 0; k < nchunks; ++k) s += partial[((size_t)nn * nchunks + k) * C + c];
+    if (out_n) out_n[(size_t)nn * C + c] = s;
+    tot += s;
+  }
+  if (out_tot) out_tot[c] += tot;
+}
+
+// any C (used for Cout = 4): one block per channel
+template <typename T>
+__global__ void colsum_scalar_k(const T* __restrict__ g, int n, int hw, int C, float* out_n, float* out_tot) {
+  const int c = blockIdx.x;
+  __shared__ float sh[32];
+  float tot = 0.f;
+  for (int nn = 0; nn < n; ++nn) {
+    float s = 0.f;
+    for (int p = threadIdx.x; p < hw; p += blockDim.x) s += to_f(g[((size_t)nn * hw + p) * C + c]);
+    s = warp_sum(s);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      float v = 0.f;
+      for (int i = 0; i < (int)(blockDim.x >> 5); ++i) v += sh[i];
+      if (out_n) out_n[(size_t)nn * C + c] = v;
+      tot += v;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0 && out_tot) out_tot[c] += tot;
+}
+
+int colsum(int dt, const void* g, int n, int hw, int c, float* out_n, float* out_tot, float* partial,
+           cudaStream_t st) {
+  const int vec = dt == DT_F32 ? 4 : 8;
+  if (c % vec) {
+    if (dt == DT_F32) colsum_scalar_k<float><<<c, 256, 0, st>>>((const float*)g, n, hw, c, out_n, out_tot);
+    else colsum_scalar_k<bf16><<<c, 256, 0, st>>>((const bf16*)g, n, hw, c, out_n, out_tot);
+    return 1;
+  }
+  int tpr, rows, nchunks;
+  colsum_plan(dt, n, hw, c, tpr, rows, nchunks);
+  dim3 grid(nchunks, n), block(tpr, rows);
+  const size_t smem = rows > 1 ? (size_t)rows * c * sizeof(float) : 0;
+  if (dt == DT_F32) colsum_partial_k<float><<<grid, block, smem, st>>>((const float*)g, hw, c, partial);
+  else colsum_partial_k<bf16><<<grid, block, smem, st>>>((const bf16*)g, hw, c, partial);
+  colsum_finalize_k<<<(c + 127) / 128, 128, 0, st>>>(partial, n, nchunks, c, out_n, out_tot);
+  return 2;
+}
+
+// ------------------------------------------------------------------ tiny linears (timestep path)
+// one warp per output feature o; lanes stride over the input dimension; all n rows at once
+template <typename T, int MAXN>
+__global__ void linear_fwd_k(const float* __restrict__ in, int n, int din, int dout, const T* __restrict__ w,
+                             const T* __restrict__ b, int silu_in, float* __restrict__ out) {
+  const int o = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (o >= dout) return;
+  float acc[MAXN];
+#pragma unroll
+  for (int j = 0; j < MAXN; ++j) acc[j] = 0.f;
+  for (int i = lane; i < din; i += 32) {
+    const float wv = to_f(w[(size_t)o * din + i]);
+#pragma unroll
+    for (int j = 0; j < MAXN; ++j)
+      if (j < n) {
+        float x = in[(size_t)j * din + i];
+        if (silu_in) x = siluf_(x);
+        acc[j] = fmaf(wv, x, acc[j]);
+      }
+  }
+#pragma unroll
+  for (int j = 0; j < MAXN; ++j) {
+    if (j < n) {
+      const float s = warp_sum(acc[j]);
+      if (lane == 0) out[(size_t)j * dout + o] = s + (b ? to_f(b[o]) : 0.f);
+    }
+  }
+}
+
+int linear_fwd(int dt, const float* in, int n, int din, int dout, const void* w, const void* b, int silu_in,
+               float* out, cudaStream_t st) {
+  int launches = 0;
+  for (int n0 = 0; n0 < n; n0 += 8) {       // N <= 8 in every config; larger N handled in slabs
+    const int nn = n - n0 < 8 ? n - n0 : 8;
+    const int blocks = (dout * 32 + 255) / 256;
+    if (dt == DT_F32)
+      linear_fwd_k<float, 8><<<blocks, 256, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const float*)w,
+                                                      (const float*)b, silu_in, out + (size_t)n0 * dout);
+    else
+      linear_fwd_k<bf16, 8><<<blocks, 256, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const bf16*)w,
+                                                     (const bf16*)b, silu_in, out + (size_t)n0 * dout);
+    ++launches;
+  }
+  return launches;
+}
+
+// dW[o][i] += sum_n g[n][o] f(in[n][i]); db[o] += sum_n g[n][o]
+__global__ void linear_bwd_w_k(const float* __restrict__ in, const float* __restrict__ g, int n, int din, int dout,
+                               int silu_in, float* __restrict__ dw, float* __restrict__ db) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)din * dout) return;
+  const int o = idx / din, i = idx % din;
+  float s = 0.f, sb = 0.f;
+  for (int j = 0; j < n; ++j) {
+    float x = in[(size_t)j * din + i];
+    if (silu_in) x = siluf_(x);
+    const float gv = g[(size_t)j * dout + o];
+    s = fmaf(gv, x, s);
+    sb += gv;
+  }
+  dw[idx] += s;
+  if (i == 0 && db) db[o] += sb;
+}
+
+// g_in[n][i] (+)= (sum_o g[n][o] W[o][i]) f'(in[n][i])
+template <typename T>
+__global__ void linear_bwd_in_k(const float* __restrict__ in, const float* __restrict__ g, int n, int din, int dout,
+                                const T* __restrict__ w, int silu_in, float* __restrict__ g_in, int acc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= din) return;
+  float s = 0.f;
+  for (int o = 0; o < dout; ++o) s = fmaf(g[(size_t)j * dout + o], to_f(w[(size_t)o * din + i]), s);
+  if (silu_in) s *= silu_gradf_(in[(size_t)j * din + i]);
+  float* d = g_in + (size_t)j * din + i;
+  *d = acc ? *d + s : s;
+}
+
+int linear_bwd(int dt, const float* in, const float* g, int n, int din, int dout, const void* w, int silu_in,
+               float* dw, float* db, float* g_in, int acc_g_in, cudaStream_t st) {
+  int launches = 1;
+  const size_t tot = (size_t)din * dout;
+  linear_bwd_w_k<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(in, g, n, din, dout, silu_in, dw, db);
+  if (g_in) {
+    dim3 grid((din + 127) / 128, n);
+    if (dt == DT_F32)
+      linear_bwd_in_k<float><<<grid, 128, 0, st>>>(in, g, n, din, dout, (const float*)w, silu_in, g_in, acc_g_in);
+    else
+      linear_bwd_in_k<bf16><<<grid, 128, 0, st>>>(in, g, n, din, dout, (const bf16*)w, silu_in, g_in, acc_g_in);
+    ++launches;
+  }
+  return launches;
+}
+
+// ------------------------------------------------------------------ sinusoidal embedding
+__global__ void sinusoidal_k(const int64_t* __restrict__ t, int n, int d, float* __restrict__ out) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x, half = d / 2;
+  if (idx >= n * half) return;
+  const int j = idx / half, i = idx % half;
+  // f_i = exp(-ln(10000) i / half); angle in double so that t up to 999 keeps fp32-exact phase
+  const double f = exp(-9.210340371976184 * (double)i / (double)half);
+  const double a = (double)t[j] * f;
+  out[(size_t)j * d + i] = (float)cos(a);
+  out[(size_t)j * d + half + i] = (float)sin(a);
+}
+int sinusoidal(const int64_t* t, int n, int d, float* out, cudaStream_t st) {
+  const int tot = n * (d / 2);
+  sinusoidal_k<<<(tot + 127) / 128, 128, 0, st>>>(t, n, d, out);
+  return 1;
+}
+
+// ------------------------------------------------------------------ MSE loss + gradient
+template <typename T>
+__global__ void mse_k(const T* __restrict__ d, const T* __restrict__ tg, size_t nvec, float scale, float inv_numel,
+                      float* loss, T* __restrict__ g) {
+  constexpr int V = Vec<T>::N;
+  float acc = 0.f;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    float a[V], b[V], o[V];
+    ldv(d + i * V, a);
+    ldv(tg + i * V, b);
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+      const float df = a[k] - b[k];
+      acc = fmaf(df, df, acc);
+      o[k] = 2.0f * scale * inv_numel * df;
+    }
+    stv(g + i * V, o);
+  }
+  acc = warp_sum(acc);
+  __shared__ float sh[32];
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float v = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.f;
+    v = warp_sum(v);
+    if (threadIdx.x == 0) atomicAdd(loss, v * scale * inv_numel);
+  }
+}
+int mse_fwd_bwd(int dt, const void* d, const void* target, size_t numel, float scale, float* loss, void* g,
+                cudaStream_t st) {
+  const int V = dt == DT_F32 ? 4 : 8;
+  const size_t nvec = numel / V;       // numel % V == 0 is checked by the caller
+  size_t blocks = (nvec + 255) / 256;
+  if (blocks > 1184) blocks = 1184;
+  if (blocks < 1) blocks = 1;
+  const float inv = (float)(1.0 / (double)numel);
+  if (dt == DT_F32)
+    mse_k<float><<<(unsigned)blocks, 256, 0, st>>>((const float*)d, (const float*)target, nvec, scale, inv, loss,
+                                                   (float*)g);
+  else
+    mse_k<bf16><<<(unsigned)blocks, 256, 0, st>>>((const bf16*)d, (const bf16*)target, nvec, scale, inv, loss,
+                                                  (bf16*)g);
+  return 1;
+}
+
+// ------------------------------------------------------------------ nearest 2x upsample and adjoint
+template <typename T>
+__global__ void upsample2_k(const T* __restrict__ in, int h, int w, int nvec, size_t total, T* __restrict__ out) {
+  constexpr int V = Vec<T>::N;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const int v = i % nvec;
+    size_t p = i / nvec;                       // output pixel index n*(2h)*(2w) + Y*(2w) + X
+    const int X = p % (2 * w); p /= (2 * w);
+    const int Y = p % (2 * h);
+    const size_t n = p / (2 * h);
+    const uint4 val = *reinterpret_cast<const uint4*>(in + (((n * h + (Y >> 1)) * w + (X >> 1)) * nvec + v) * V);
+    *reinterpret_cast<uint4*>(out + i * V) = val;
+  }
+}
+template <typename T>
+__global__ void upsample2_bwd_k(const T* __restrict__ gu, int h, int w, int nvec, size_t total, T* __restrict__ g) {
+  constexpr int V = Vec<T>::N;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const int v = i % nvec;
+    size_t p = i / nvec;                       // low-res pixel
+    const int x = p % w; p /= w;
+    const int y = p % h;
+    const size_t n = p / h;
+    float s[V];
+#pragma unroll
+    for (int k = 0; k < V; ++k) s[k] = 0.f;
+#pragma unroll
+    for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+      for (int dx = 0; dx < 2; ++dx) {
+        float a[V];
+        ldv(gu + (((n * 2 * h + 2 * y + dy) * 2 * w + 2 * x + dx) * nvec + v) * V, a);
+#pragma unroll
+        for (int k = 0; k < V; ++k) s[k] += a[k];
+      }
+    stv(g + i * V, s);
+  }
+}
+static unsigned ew_blocks(size_t total) {
+  size_t b = (total + 255) / 256;
+  if (b > 148 * 16) b = 148 * 16;
+  return (unsigned)(b < 1 ? 1 : b);
+}
+int upsample2(int dt, const void* in, int n, int h, int w, int c, void* out, cudaStream_t st) {
+  const int nvec = c / (dt == DT_F32 ? 4 : 8);
+  const size_t total = (size_t)n * 4 * h * w * nvec;
+  if (dt == DT_F32) upsample2_k<float><<<ew_blocks(total), 256, 0, st>>>((const float*)in, h, w, nvec, total, (float*)out);
+  else upsample2_k<bf16><<<ew_blocks(total), 256, 0, st>>>((const bf16*)in, h, w, nvec, total, (bf16*)out);
+  return 1;
+}
+int upsample2_bwd(int dt, const void* g_u, int n, int h, int w, int c, void* g_out, cudaStream_t st) {
+  const int nvec = c / (dt == DT_F32 ? 4 : 8);
+  const size_t total = (size_t)n * h * w * nvec;
+  if (dt == DT_F32) upsample2_bwd_k<float><<<ew_blocks(total), 256, 0, st>>>((const float*)g_u, h, w, nvec, total, (float*)g_out);
+  else upsample2_bwd_k<bf16><<<ew_blocks(total), 256, 0, st>>>((const bf16*)g_u, h, w, nvec, total, (bf16*)g_out);
+  return 1;
+}
+
+// ------------------------------------------------------------------ dst += src
+template <typename T>
+__global__ void add_inplace_k(T* __restrict__ dst, const T* __restrict__ src, size_t nvec) {
+  constexpr int V = Vec<T>::N;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    float a[V], b[V];
+    ldv(dst + i * V, a);
+    ldv(src + i * V, b);
+#pragma unroll
+    for (int k = 0; k < V; ++k) a[k] += b[k];
+    stv(dst + i * V, a);
+  }
+}
+int add_inplace(int dt, void* dst, const void* src, size_t numel, cudaStream_t st) {
+  const size_t nvec = numel / (dt == DT_F32 ? 4 : 8);
+  if (dt == DT_F32) add_inplace_k<float><<<ew_blocks(nvec), 256, 0, st>>>((float*)dst, (const float*)src, nvec);
+  else add_inplace_k<bf16><<<ew_blocks(nvec), 256, 0, st>>>((bf16*)dst, (const bf16*)src, nvec);
+  return 1;
+}
+
+// ------------------------------------------------------------------ Wt[ci][k-1-r][k-1-s][co] = W[co][r][s][ci]
+template <typename T>
+__global__ void flip_transpose_k(const T* __restrict__ w, int cout, int kk, int cin, T* __restrict__ wt) {
+  // tile transpose through shared memory: reads coalesced along ci, writes coalesced along co
+  __shared__ T tile[32][33];
+  const int tap = blockIdx.z;
+  const int ci0 = blockIdx.x * 32, co0 = blockIdx.y * 32;
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    const int co = co0 + j, ci = ci0 + threadIdx.x;
+    if (co < cout && ci < cin) tile[j][threadIdx.x] = w[((size_t)co * kk + tap) * cin + ci];
+  }
+  __syncthreads();
+  const int ftap = kk - 1 - tap;      // (k-1-r)*k + (k-1-s) == k*k-1 - (r*k+s)
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    const int ci = ci0 + j, co = co0 + threadIdx.x;
+    if (co < cout && ci < cin) wt[((size_t)ci * kk + ftap) * cout + co] = tile[threadIdx.x][j];
+  }
+}
+int flip_transpose(int dt, const void* w, int cout, int k, int cin, void* wt, cudaStream_t st) {
+  dim3 grid((cin + 31) / 32, (cout + 31) / 32, k * k), block(32, 8);
+  if (dt == DT_F32) flip_transpose_k<float><<<grid, block, 0, st>>>((const float*)w, cout, k * k, cin, (float*)wt);
+  else flip_transpose_k<bf16><<<grid, block, 0, st>>>((const bf16*)w, cout, k * k, cin, (bf16*)wt);
+  return 1;
+}
+
+}  // namespace pulse

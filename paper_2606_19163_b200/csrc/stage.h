@@ -1,0 +1,82 @@
+// stage.h - host-side plan of one collocated stage (internal).
+#pragma once
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/pulse.h"
+#include "kernels.h"
+
+namespace pulse {
+
+enum Region { R_NONE = 0, R_SKIP = 1, R_STASH = 2, R_WORK = 3 };
+
+struct TRef {               // an NHWC tensor [n,h,w,c] at a byte offset inside a region
+  int region = R_NONE;
+  size_t off = 0;
+  int h = 0, w = 0, c = 0;
+};
+
+struct ParamInfo {
+  std::string name;
+  int rank; int shape[4];
+  size_t numel, off, goff;  // byte offsets into the param (stage dtype) / grad (fp32) buffers
+};
+
+struct OpPlan {
+  int kind, cin, cskip, cout;
+  int hin, win, hout, wout;
+  int x0 = -1, x1 = -1, out = -1;           // indices into Stage::tensors (activations)
+  int a1 = -1, h1 = -1, a2 = -1, u = -1;    // stashed intermediates
+  size_t stats1 = 0, stats2 = 0, pn = 0;    // byte offsets in the slot stash (fp32 arrays)
+  int p[12];                                // parameter indices (see stage.cu)
+  int push = -1, pop = -1;
+  // backward write modes decided at plan time (0: '=', 1: '+=')
+  int acc_x0 = 0, acc_x1 = 0;
+};
+
+struct Tensor {
+  TRef ref;          // forward value
+  size_t goff = 0;   // gradient buffer (R_WORK), same shape/dtype
+};
+
+}  // namespace pulse
+
+pulse_status_t pulse_set_error(pulse_status_t s, const char* fmt, ...);
+#define fail pulse_set_error
+#define CK_CUDA(x)                                                                            \
+  do {                                                                                        \
+    cudaError_t e_ = (x);                                                                     \
+    if (e_ != cudaSuccess) return fail(PULSE_ERR_CUDA, "%s: %s", #x, cudaGetErrorString(e_)); \
+  } while (0)
+// parameter slots of OpPlan::p
+enum { P_GN1G = 0, P_GN1B, P_C1W, P_C1B, P_TW, P_TB, P_GN2G, P_GN2B, P_C2W, P_C2B, P_SCW, P_SCB };
+
+struct pulse_stage {
+  pulse_stage_desc d;
+  std::vector<pulse_op_desc> enc, mid, dec;
+  std::vector<pulse::ParamInfo> params;
+  std::map<std::string, int> pindex;
+  size_t param_bytes = 0, grad_bytes = 0, temb_grad_bytes = 0;
+  std::vector<pulse::Tensor> tensors;
+  std::vector<pulse::OpPlan> ops;           // enc, mid, dec concatenated
+  int n_enc = 0, n_mid = 0, n_dec = 0;
+  std::vector<int> skip_tensor;             // push order -> tensor index
+  int t_xin = -1, t_hin = -1, t_eout = -1, t_dout = -1;
+  size_t skip_bytes = 0, stash_bytes = 0, work_bytes = 0;
+  size_t emb_off = 0;                       // slot stash: copy of temb [n,T] fp32
+  // per-stage workspace offsets (bytes)
+  size_t w_ga2 = 0, w_gh1 = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_wt = 0, w_partial = 0, w_coef = 0, w_gp = 0,
+         w_tmpf = 0;
+  const char* d_params = nullptr; float* d_grads = nullptr;
+  char* d_work = nullptr; size_t work_bound = 0;
+  uint64_t launches = 0;
+  size_t esz() const { return d.dtype == PULSE_F32 ? 4 : 2; }
+};
+
+struct pulse_skip_cache {
+  pulse_stage* stage;
+  char* base; int slots; size_t bytes_per_slot;
+  std::vector<int64_t> mb;     // microbatch id per slot, -1 = free
+  int live = 0; size_t peak_bytes = 0;
+};

@@ -1,0 +1,233 @@
+"""GPU parity: libpulse.so (through the C-ABI binding) vs the CPU oracle, element by
+element on the same seeded inputs.  Bars (BASELINE.json north_star): fp32 debug path
+max|err| <= 1e-4 * RMS(ref); bf16 max|err| <= 2e-2 * RMS(ref), per tensor."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import pulse_oracle as O
+from paper_2606_19163_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"fp32": 1e-4, "bf16": 2e-2}
+
+
+def _binding():
+    from paper_2606_19163_b200 import binding
+    return binding
+
+
+def rel_err(got, ref):
+    ref = ref.to(torch.float64)
+    rms = float(ref.pow(2).mean().sqrt())
+    return float((got.to(torch.float64) - ref).abs().max()) / max(rms, 1e-30)
+
+
+def run_gpu(desc, data, flags=0, with_g_e_out=False):
+    B = _binding()
+    st = B.Stage(desc, flags=flags)
+    st.load_params(data["params"])
+    M = desc["microbatches"]
+    outs = []
+    devs = [st.to_device(mb) for mb in data["microbatches"]]
+    if M == 1:
+        r = st.step(0, devs[0], 1.0, accumulate=False)
+        outs.append(r)
+    else:       # wave: F0..F{M-1}, B{M-1}..B0 (configs[4])
+        fw = []
+        for m, dev in enumerate(devs):
+            emb, tst = st.temb_forward(dev["t"])
+            e_out, d_out = st.forward(m, dev["x_in"], dev.get("h_in"), emb)
+            fw.append((emb, tst, e_out, d_out))
+        peak = st.cache_stats()
+        assert peak["live_slots"] == M and peak["peak_bytes"] == M * st.skip_bytes
+        for m in reversed(range(M)):
+            emb, tst, e_out, d_out = fw[m]
+            loss, g_d = st.mse(d_out, devs[m]["target"], 1.0 / M)
+            g_temb = torch.zeros_like(emb)
+            first = m == M - 1
+            g_x_in, g_h_in = st.backward(m, g_d, None, True, g_temb, accumulate=not first)
+            st.temb_backward(g_temb, tst, accumulate=not first)
+            outs.append({"loss": loss, "e_out": e_out, "d_out": d_out, "g_x_in": g_x_in, "g_h_in": g_h_in,
+                         "g_emb": g_temb, "emb": emb})
+        outs.reverse()
+        assert st.cache_stats()["live_slots"] == 0
+    torch.cuda.synchronize()
+    res = {"per_mb": [], "param_grads": st.grads(), "stage": st}
+    for r in outs:
+        o = {}
+        for k, v in r.items():
+            if v is None:
+                continue
+            o[k] = B.nchw(v) if v.dim() == 4 else v.to(torch.float64).cpu()
+        res["per_mb"].append(o)
+    return res
+
+
+def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, report=None):
+    data = W.draw(desc, seed, with_g_e_out=with_g_e_out)
+    got = run_gpu(desc, data, flags, with_g_e_out)
+    M = desc["microbatches"]
+    if M == 1:
+        ref_mbs = [O.run_stage(desc, data["params"], data["microbatches"][0], 1.0, oracle_dtype)]
+        ref_grads = ref_mbs[0]["param_grads"]
+    else:
+        wave = O.run_wave(desc, data["params"], data["microbatches"], oracle_dtype)
+        ref_mbs, ref_grads = wave["per_mb"], wave["param_grads"]
+    tol = tol or TOL[desc["dtype"]]
+    worst = {}
+    for m in range(M):
+        for k in ["d_out", "e_out", "g_x_in", "g_h_in", "emb", "g_emb"]:
+            if k in ref_mbs[m] and ref_mbs[m][k] is not None and k in got["per_mb"][m]:
+                worst[f"mb{m}.{k}"] = rel_err(got["per_mb"][m][k], ref_mbs[m][k])
+        lg, lr = float(got["per_mb"][m]["loss"]), float(ref_mbs[m]["loss"])
+        worst[f"mb{m}.loss"] = abs(lg - lr) / abs(lr)
+    for k, v in ref_grads.items():
+        worst["grad." + k] = rel_err(got["param_grads"][k], v)
+    bad = {k: v for k, v in worst.items() if not (v <= tol)}
+    top = sorted(worst.items(), key=lambda kv: -kv[1])[:5]
+    print(f"[parity] {desc['name']} flags={flags} tol={tol:g} worst: " + ", ".join(f"{k}={v:.2e}" for k, v in top))
+    if report is not None:
+        report.update(worst)
+    assert not bad, f"{desc['name']}: {len(bad)} tensors above {tol:g}: {sorted(bad.items(), key=lambda kv: -kv[1])[:8]}"
+    return got
+
+
+# ------------------------------------------------------------------ fp32 debug path
+@pytest.mark.parametrize("kind", ["pair", "level", "updown", "straddle", "unet", "wave"])
+def test_mini_fp32(kind):
+    check(W.mini(kind, "fp32"), seed=1, with_g_e_out=True)
+
+
+def test_config1_fp32():
+    check(W.config(1), seed=0)
+
+
+# ------------------------------------------------------------------ bf16, small shapes (CUDA-core convs)
+@pytest.mark.parametrize("kind", ["level", "updown", "unet", "wave"])
+def test_mini_bf16(kind):
+    # plumbing check only: 8-16 channel, 4x4 tensors give reductions of 32-100 terms that do not average
+    # bf16 store rounding (2^-9 per store, ~20 store points); the 2e-2 bar applies to the configs.
+    check(W.mini(kind, "bf16"), seed=1, with_g_e_out=True, tol=1e-1)
+
+
+# ------------------------------------------------------------------ bf16, tensor-core shapes with ragged tiles
+@pytest.mark.parametrize("kind", ["level", "updown", "unet"])
+def test_mid_bf16(kind):
+    check(W.gpu_mid(kind), seed=2, with_g_e_out=(kind != "unet"))
+
+
+@pytest.mark.parametrize("kind", ["level", "updown"])
+def test_mid_bf16_simt_crosscheck(kind):
+    """Same shapes through the CUDA-core convs (PULSE_FLAG_FORCE_SIMT): isolates tensor-core bugs."""
+    check(W.gpu_mid(kind), seed=2, flags=1, with_g_e_out=True)
+
+
+# ------------------------------------------------------------------ full configs
+def test_config2_bf16():
+    check(W.config(2), seed=0)
+
+
+def test_config3_bf16():
+    check(W.config(3), seed=0, oracle_dtype=torch.float32)
+
+
+@pytest.mark.skipif(os.environ.get("PULSE_SKIP_BIG") == "1", reason="PULSE_SKIP_BIG=1")
+def test_config4_bf16():
+    check(W.config(4), seed=0, oracle_dtype=torch.float32)
+
+
+@pytest.mark.skipif(os.environ.get("PULSE_BIG_WAVE") != "1", reason="config 5's full wave costs the oracle ~80 TFLOP; "
+                    "set PULSE_BIG_WAVE=1 (test_config5_wave_reduced covers the same path at 2 microbatches)")
+def test_config5_wave_full():
+    got = check(W.config(5), seed=0, oracle_dtype=torch.float32)
+    assert got["stage"].cache_stats()["peak_bytes"] == 780 * 2 ** 20
+
+
+def test_config5_wave_reduced():
+    """configs[4] shapes (N=2, 4x128x128, 9 skips) with a wave of 2 microbatches for the oracle comparison,
+    plus the full 8-slot peak-bytes accounting without the oracle."""
+    desc = W.scaled(W.config(5), microbatches=2, name="config5_wave2")
+    got = check(desc, seed=0, oracle_dtype=torch.float32)
+    assert got["stage"].skip_bytes == int(97.5 * 2 ** 20)
+    del got
+    torch.cuda.empty_cache()
+    B = _binding()
+    full = W.config(5)
+    st = B.Stage(full)
+    data = W.draw(W.scaled(full, microbatches=1), 0)
+    st.load_params(data["params"])
+    dev = st.to_device(data["microbatches"][0])
+    fw = []
+    for m in range(8):
+        emb, tst = st.temb_forward(dev["t"])
+        fw.append((emb, tst) + st.forward(m, dev["x_in"], None, emb))
+    stats = st.cache_stats()
+    assert stats["live_slots"] == 8 and stats["peak_bytes"] == 780 * 2 ** 20
+    with pytest.raises(B.PulseError) as ei:                                         # 9th forward with 8 slots
+        st.forward(8, dev["x_in"], None, fw[0][0])
+    assert ei.value.status == 5
+    for m in reversed(range(8)):
+        loss, g_d = st.mse(fw[m][3], dev["target"], 1.0 / 8)
+        st.backward(m, g_d, None, True, torch.zeros_like(fw[m][0]), accumulate=(m != 7))
+    torch.cuda.synchronize()
+    assert st.cache_stats()["live_slots"] == 0
+    # identical microbatches: summed weight gradient == 8 x (1/8-scaled single) -> equals the 1-microbatch gradient
+    g8 = st.grads()
+    st.step(0, dev, 1.0, accumulate=False)
+    torch.cuda.synchronize()
+    g1 = st.grads()
+    for k in g1:
+        if k.startswith("temb.w") or k.startswith("temb.b1") or k.startswith("temb.b2"):
+            continue
+        assert rel_err(g8[k], g1[k]) < 1e-2, k
+
+
+# ------------------------------------------------------------------ cache / error behaviour (paper-faithful cases)
+def test_cache_errors_and_skip_locality():
+    B = _binding()
+    desc = W.mini("level", "fp32")
+    data = W.draw(desc, 5)
+    st = B.Stage(desc, max_inflight=2)
+    st.load_params(data["params"])
+    dev = st.to_device(data["microbatches"][0])
+    emb, _ = st.temb_forward(dev["t"])
+    with pytest.raises(B.PulseError) as ei:          # backward on unknown microbatch
+        st.backward(7, dev["target"], None, True, None)
+    assert ei.value.status == 6
+    e_out, d_out = st.forward(0, dev["x_in"], dev["h_in"], emb)
+    with pytest.raises(B.PulseError) as ei:          # same microbatch forwarded twice
+        st.forward(0, dev["x_in"], dev["h_in"], emb)
+    assert ei.value.status == 5
+    st.forward(1, dev["x_in"], dev["h_in"], emb)
+    with pytest.raises(B.PulseError) as ei:          # third forward with 2 slots
+        st.forward(2, dev["x_in"], dev["h_in"], emb)
+    assert ei.value.status == 5
+    # the cached skips are the encoder outputs (zero-copy put): skip 0 = x_in, last = e_out
+    torch.cuda.synchronize()
+    assert st.skip_count() == 3
+    assert torch.equal(st.skip(0, 0), dev["x_in"]) and torch.equal(st.skip(0, 2), e_out)
+    ref = O.run_stage(desc, data["params"], data["microbatches"][0])
+    for k in range(3):
+        assert rel_err(B.nchw(st.skip(1, k)), ref["skips"][k]) < 1e-4
+    assert st.cache_stats() == {"live_slots": 2, "live_bytes": 2 * st.skip_bytes, "peak_bytes": 2 * st.skip_bytes}
+    st.backward(1, dev["target"], None, True, None)       # FIFO/LIFO free list: release 1 first, then reuse
+    st.forward(5, dev["x_in"], dev["h_in"], emb)
+    assert st.cache_stats()["live_slots"] == 2
+
+
+def test_descriptor_validation():
+    B = _binding()
+    bad = W.mini("level", "fp32")
+    bad["dec_ops"] = bad["dec_ops"] + [W.rb(8, 8, skip=8)]     # pops more than pushed
+    with pytest.raises(B.PulseError) as ei:
+        B.Stage(bad, allocate=False)
+    assert ei.value.status == 2
+    bad2 = W.mini("level", "fp32")
+    bad2["dec_ops"] = bad2["dec_ops"][:2]                       # a cached skip never consumed
+    with pytest.raises(B.PulseError) as ei:
+        B.Stage(bad2, allocate=False)
+    assert ei.value.status == 2
