@@ -154,6 +154,25 @@ pulse_status_t pulse_temb_backward(pulse_stage_t* stage, const float* d_g_emb, c
 pulse_status_t pulse_mse_fwd_bwd(int dtype, const void* d_d, const void* d_target, size_t numel, float scale,
                                  float* d_loss, void* d_g_d, void* stream);
 
+/* ---- single operators (the kernels of rows a2/a4/a5/a6/a8-a10 in isolation; used by the
+ * kernel-level parity tests and microbenchmarks).  NHWC activations, weights [cout][k][k][cin],
+ * k in {1,3}, pad (k-1)/2, stride in {1,2}; dtype as above.  force_simt != 0 selects the CUDA-core
+ * kernel even where the tcgen05 kernel applies.  SURVEY.md 8c item 2. */
+/* out[n,y,x,co] = bias[co] + pn[n,co] + residual[n,y,x,co] + sum W[co][r][s][c] in[n, y st+r-pad, x st+s-pad, c],
+ * in = concat_C(src0[c0], src1[c1]) (src1 may be NULL with c1 = 0); bias/pn/residual may be NULL. */
+pulse_status_t pulse_conv2d(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1, int c1,
+                            int n, int h, int w, int ksize, int stride, const void* d_w, int cout,
+                            const void* d_bias, const float* d_pn, const void* d_residual, void* d_out, void* stream);
+/* g_in[n,h,w,cin] (+)= adjoint of the conv in its input, from g [n,hout,wout,cout].
+ * d_wt_scratch: cout*k*k*cin elements of dtype (holds the flipped/transposed weights). */
+pulse_status_t pulse_conv2d_dgrad(int dtype, int force_simt, const void* d_g, int n, int h, int w, int cin,
+                                  int ksize, int stride, const void* d_w, int cout, void* d_wt_scratch,
+                                  void* d_g_in, int accumulate, void* stream);
+/* dw[cout][k][k][c0+c1] += sum_{n,y,x} g[n,y,x,co] in[n, y st+r-pad, x st+s-pad, c]  (fp32, accumulated) */
+pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1, int c1,
+                                  int n, int h, int w, int ksize, int stride, const void* d_g, int cout,
+                                  float* d_dw, void* stream);
+
 /* Number of kernels this handle has launched so far (bench.py "gpu_launches"). */
 pulse_status_t pulse_stage_launch_count(const pulse_stage_t* stage, uint64_t* launches);
 

@@ -64,6 +64,12 @@ _SIG = {
     "pulse_temb_backward": [_vp, _vp, _vp, C.c_int, _vp],
     "pulse_mse_fwd_bwd": [C.c_int, _vp, _vp, _sz, C.c_float, _vp, _vp, _vp],
     "pulse_stage_launch_count": [_vp, C.POINTER(C.c_uint64)],
+    "pulse_conv2d": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp,
+                     C.c_int, _vp, _vp, _vp, _vp, _vp],
+    "pulse_conv2d_dgrad": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int,
+                           _vp, _vp, C.c_int, _vp],
+    "pulse_conv2d_wgrad": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                           _vp, C.c_int, _vp, _vp],
 }
 for _name, _args in _SIG.items():
     _f = getattr(lib, _name)
@@ -294,3 +300,39 @@ class Stage:
             else:
                 dev[k] = nhwc(v, self.tdtype, self.device)
         return dev
+
+
+# ---- single operators (NHWC device tensors) ---------------------------------------------------------
+def _cd(t):
+    return BF16 if t.dtype == torch.bfloat16 else F32
+
+
+def conv2d(src0, w, src1=None, bias=None, pn=None, residual=None, stride=1, force_simt=False):
+    n, h, wd, c0 = src0.shape
+    cout, k = w.shape[0], w.shape[1]
+    out = torch.empty((n, h // stride, wd // stride, cout), dtype=src0.dtype, device=src0.device)
+    _ck(lib.pulse_conv2d(_cd(src0), int(force_simt), _ptr(src0), c0, _ptr(src1), 0 if src1 is None else src1.shape[3],
+                         n, h, wd, k, stride, _ptr(w), cout, _ptr(bias), _ptr(pn), _ptr(residual), _ptr(out), _stream()))
+    return out
+
+
+def conv2d_dgrad(g, w, in_hw, stride=1, force_simt=False, g_in=None):
+    n, cout = g.shape[0], g.shape[3]
+    k, cin = w.shape[1], w.shape[3]
+    acc = g_in is not None
+    if g_in is None:
+        g_in = torch.empty((n, in_hw[0], in_hw[1], cin), dtype=g.dtype, device=g.device)
+    wt = torch.empty(w.numel(), dtype=w.dtype, device=w.device)
+    _ck(lib.pulse_conv2d_dgrad(_cd(g), int(force_simt), _ptr(g), n, in_hw[0], in_hw[1], cin, k, stride, _ptr(w), cout,
+                               _ptr(wt), _ptr(g_in), int(acc), _stream()))
+    return g_in
+
+
+def conv2d_wgrad(src0, g, ksize, src1=None, stride=1, force_simt=False):
+    n, h, wd, c0 = src0.shape
+    c1 = 0 if src1 is None else src1.shape[3]
+    cout = g.shape[3]
+    dw = torch.zeros((cout, ksize, ksize, c0 + c1), dtype=torch.float32, device=g.device)
+    _ck(lib.pulse_conv2d_wgrad(_cd(src0), int(force_simt), _ptr(src0), c0, _ptr(src1), c1, n, h, wd, ksize, stride,
+                               _ptr(g), cout, _ptr(dw), _stream()))
+    return dw

@@ -1,10 +1,411 @@
-// conv_tc.cu - tcgen05 / TMEM / TMA implicit-GEMM convolutions (placeholder until the
-// tensor-core kernels land: reports "unsupported" so the executor uses conv_simt).
+// conv_tc.cu - tcgen05 / TMEM / TMA implicit-GEMM convolution for sm_100a (bf16 in, fp32
+// accumulate).  One kernel serves 3x3 / 1x1 fprop on a single or dual source (the channel
+// concat with the cached skip is fused into the operand loader: K blocks below c0 come from
+// h's tensor map, the rest from the skip's - PAPER.md:L91, north_star), stride-1 dgrad (fprop
+// with flipped/transposed weights), stride-2 fprop (5-D parity view of the input) and
+// stride-2 dgrad (4 output-parity phases, each a sub-pixel conv with 1/2/2/4 taps).
+//
+// GEMM view: D[pixel, co] = sum_{tap, c} A[pixel shifted by tap, c] * W[co][tap][c]
+//   M tile = 128 output pixels = a (bn x bh x bw) box of the NHWC tensor, loaded per tap by
+//            ONE tiled TMA with shifted coordinates; out-of-bounds rows/cols are zero-filled
+//            by TMA, which implements pad = 1 for free,
+//   N tile = BN output channels (160: every channel count of the configs is 320 k),
+//   K block = 64 channels of one tap (128-byte swizzled rows, K-major for both operands).
+// Warp roles (192 threads): warp 0 TMA producer, warp 1 MMA issuer (one elected thread;
+// owns TMEM alloc), warps 2-5 epilogue (tcgen05.ld -> +bias +temb/residual -> bf16 ->
+// global).  Persistent over tiles with two TMEM accumulators so the epilogue of tile i
+// overlaps the main loop of tile i+1.
+#include <cuda.h>
+
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
 #include "kernels.h"
+#include "sm100.cuh"
+
 namespace pulse {
-bool conv_tc_supported(const ConvArgs&) { return false; }
-int conv_tc(const ConvArgs&, cudaStream_t) { return 0; }
+
+namespace {
+
+using namespace sm100;
+
+constexpr int BM = 128, BK = 64;
+constexpr int A_BYTES = BM * BK * 2;           // 16 KB
+
+struct Tap { int dx, dy, px, py, widx; };
+
+struct TcParams {
+  int c0_blocks, c_blocks, ntaps, ctot, c0;
+  int s2;                         // 1: stride-2 fprop through the 5-D parity view
+  Tap taps[9];
+  int bw, bh, bn, tiles_h, tiles_mn, n_tiles;
+  int GH, GN;                     // pixel grid (rows, images); columns == bw
+  const bf16* bias; const float* pn; const bf16* residual; bf16* out; int accumulate;
+  int OH, OW, osy, osx, ooy, oox, cout_total;
+};
+
+template <int BN> struct Cfg {
+  static constexpr int B_BYTES = BN * BK * 2;
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int STAGES = (220 * 1024) / STAGE_BYTES > 8 ? 8 : (220 * 1024) / STAGE_BYTES;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024;
+  static constexpr int TMEM_COLS = 2 * BN <= 256 ? 256 : 512;
+};
+
+template <int BN>
+__global__ void __launch_bounds__(192, 1)
+conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
+          const __grid_constant__ CUtensorMap mapB, const TcParams p) {
+  using C = Cfg<BN>;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t full_bar[C::STAGES], empty_bar[C::STAGES], tfull_bar[2], tempty_bar[2];
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int num_kb = p.ntaps * p.c_blocks;
+  const int total_tiles = p.tiles_mn * p.n_tiles;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB);
+    for (int i = 0; i < C::STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull_bar[i], 1); mbar_init(&tempty_bar[i], 4); }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(&tmem_base_s, C::TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // ===== TMA producer =====
+      int stage = 0; uint32_t phase = 0;
+      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        const int mt = tile / p.n_tiles, nt = tile - mt * p.n_tiles;
+        const int n0 = (mt / p.tiles_h) * p.bn, y0 = (mt % p.tiles_h) * p.bh;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          const int ti = kb / p.c_blocks, cb = kb - ti * p.c_blocks;
+          const Tap t = p.taps[ti];
+          mbar_wait(&empty_bar[stage], phase ^ 1);
+          mbar_expect_tx(&full_bar[stage], C::STAGE_BYTES);
+          uint8_t* sa = smem + stage * C::STAGE_BYTES;
+          const bool first = cb < p.c0_blocks;
+          const CUtensorMap* ma = first ? &mapA0 : &mapA1;
+          const int cch = (first ? cb : cb - p.c0_blocks) * BK;
+          if (!p.s2) tma_load_4d(sa, ma, &full_bar[stage], cch, t.dx, y0 + t.dy, n0);
+          else tma_load_5d(sa, ma, &full_bar[stage], t.px * p.c0 + cch, t.dx, t.py, y0 + t.dy, n0);
+          tma_load_2d(sa + A_BYTES, &mapB, &full_bar[stage], t.widx * p.ctot + cb * BK, nt * BN);
+          if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      // ===== MMA issuer =====
+      constexpr uint32_t idesc = idesc_bf16(BM, BN, 0, 0);
+      constexpr uint64_t dbase = smem_desc_sw128(16, 1024);
+      int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
+      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        mbar_wait(&tempty_bar[acc], acc_phase ^ 1);
+        tc_fence_after();
+        const uint32_t tmem_d = tmem_base + acc * BN;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          mbar_wait(&full_bar[stage], phase);
+          tc_fence_after();
+          const uint32_t a_addr = smem_u32(smem + stage * C::STAGE_BYTES), b_addr = a_addr + A_BYTES;
+#pragma unroll
+          for (int k = 0; k < BK / 16; ++k)
+            umma_bf16(tmem_d, desc_with_addr(dbase, a_addr + k * 32), desc_with_addr(dbase, b_addr + k * 32), idesc,
+                      (kb | k) != 0);
+          umma_commit(&empty_bar[stage]);
+          if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
+        }
+        umma_commit(&tfull_bar[acc]);
+        acc ^= 1;
+        if (acc == 0) acc_phase ^= 1;
+      }
+    }
+  } else {
+    // ===== epilogue: warps 2..5 own TMEM lane quadrants (warp % 4) =====
+    const int q = warp & 3;
+    const int row = q * 32 + lane;
+    const int n_l = row / (p.bh * p.bw), rem = row - n_l * (p.bh * p.bw);
+    const int y_l = rem / p.bw, x = rem - y_l * p.bw;
+    int acc = 0; uint32_t acc_phase = 0;
+    for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+      const int mt = tile / p.n_tiles, nt = tile - mt * p.n_tiles;
+      const int n = (mt / p.tiles_h) * p.bn + n_l, y = (mt % p.tiles_h) * p.bh + y_l;
+      const bool valid = n < p.GN && y < p.GH;
+      const size_t off = (((size_t)n * p.OH + (size_t)y * p.osy + p.ooy) * p.OW + (size_t)x * p.osx + p.oox) *
+                             p.cout_total + (size_t)nt * BN;
+      mbar_wait(&tfull_bar[acc], acc_phase);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
+#pragma unroll 1
+      for (int ch = 0; ch < BN / 32; ++ch) {
+        uint32_t r[32];
+        tmem_ld32(taddr + ch * 32, r);
+        tmem_ld_wait();
+        if (ch == BN / 32 - 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&tempty_bar[acc]);
+        }
+        if (valid) {
+          const int co = nt * BN + ch * 32;
+          float v[32];
+#pragma unroll
+          for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+          if (p.bias) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              float b[8];
+              ldv(p.bias + co + i * 8, b);
+#pragma unroll
+              for (int j = 0; j < 8; ++j) v[i * 8 + j] += b[j];
+            }
+          }
+          if (p.pn) {
+            const float4* pp = reinterpret_cast<const float4*>(p.pn + (size_t)n * p.cout_total + co);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const float4 t = pp[i];
+              v[i * 4] += t.x; v[i * 4 + 1] += t.y; v[i * 4 + 2] += t.z; v[i * 4 + 3] += t.w;
+            }
+          }
+          if (p.residual) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              float b[8];
+              ldv(p.residual + off + ch * 32 + i * 8, b);
+#pragma unroll
+              for (int j = 0; j < 8; ++j) v[i * 8 + j] += b[j];
+            }
+          }
+          if (p.accumulate) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              float b[8];
+              ldv(p.out + off + ch * 32 + i * 8, b);
+#pragma unroll
+              for (int j = 0; j < 8; ++j) v[i * 8 + j] += b[j];
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            float o[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) o[j] = v[i * 8 + j];
+            stv(p.out + off + ch * 32 + i * 8, o);
+          }
+        }
+      }
+      acc ^= 1;
+      if (acc == 0) acc_phase ^= 1;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, C::TMEM_COLS);
+  }
+}
+
+// ------------------------------------------------------------------------------ host: tensor maps
+typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                             const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                             CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+std::string g_tc_err;
+EncodeFn g_encode = nullptr;
+std::mutex g_mu;
+std::map<std::vector<uint64_t>, CUtensorMap> g_maps;
+int g_sms = 0;
+
+bool init_driver() {
+  if (g_encode) return true;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+    g_tc_err = "cuTensorMapEncodeTiled not available";
+    return false;
+  }
+  g_encode = (EncodeFn)fn;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
+  return true;
+}
+
+// bf16 tensor map, 128-byte swizzle; dims/box innermost first; strides (bytes) for dims 1..rank-1
+bool get_map(const void* ptr, int rank, const uint64_t* dims, const uint64_t* strides, const uint32_t* box,
+             CUtensorMap* out) {
+  std::vector<uint64_t> key;
+  key.push_back((uint64_t)ptr); key.push_back(rank);
+  for (int i = 0; i < rank; ++i) { key.push_back(dims[i]); key.push_back(box[i]); if (i) key.push_back(strides[i - 1]); }
+  std::lock_guard<std::mutex> lk(g_mu);
+  auto it = g_maps.find(key);
+  if (it != g_maps.end()) { *out = it->second; return true; }
+  if (!init_driver()) return false;
+  cuuint64_t gd[5], gs[4]; cuuint32_t bx[5], es[5];
+  for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; es[i] = 1; if (i) gs[i - 1] = strides[i - 1]; }
+  CUtensorMap m;
+  CUresult r = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void*>(ptr), gd, gs, bx, es,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    g_tc_err = "cuTensorMapEncodeTiled failed with " + std::to_string((int)r);
+    return false;
+  }
+  if (g_maps.size() > 4096) g_maps.clear();
+  g_maps[key] = m;
+  *out = m;
+  return true;
+}
+
+// NHWC activation [n,h,w,c] as a 4-D map (c, w, h, n) with box (64, bw, bh, bn)
+bool act_map(const void* ptr, int n, int h, int w, int c, int bw, int bh, int bn, CUtensorMap* out) {
+  uint64_t dims[4] = {(uint64_t)c, (uint64_t)w, (uint64_t)h, (uint64_t)n};
+  uint64_t str[3] = {(uint64_t)c * 2, (uint64_t)w * c * 2, (uint64_t)h * w * c * 2};
+  uint32_t box[4] = {64, (uint32_t)bw, (uint32_t)bh, (uint32_t)bn};
+  return get_map(ptr, 4, dims, str, box, out);
+}
+// stride-2 parity view (px*c + ch, x', py, y', n) of [n,h,w,c], box (64, bw, 1, bh, bn)
+bool act_map_s2(const void* ptr, int n, int h, int w, int c, int bw, int bh, int bn, CUtensorMap* out) {
+  uint64_t dims[5] = {(uint64_t)2 * c, (uint64_t)w / 2, 2, (uint64_t)h / 2, (uint64_t)n};
+  uint64_t str[4] = {(uint64_t)2 * c * 2, (uint64_t)w * c * 2, (uint64_t)2 * w * c * 2, (uint64_t)h * w * c * 2};
+  uint32_t box[5] = {64, (uint32_t)bw, 1, (uint32_t)bh, (uint32_t)bn};
+  return get_map(ptr, 5, dims, str, box, out);
+}
+// row-major [rows][k] matrix, box (64, brows)
+bool mat_map(const void* ptr, uint64_t rows, uint64_t k, int brows, CUtensorMap* out) {
+  uint64_t dims[2] = {k, rows};
+  uint64_t str[1] = {k * 2};
+  uint32_t box[2] = {64, (uint32_t)brows};
+  return get_map(ptr, 2, dims, str, box, out);
+}
+
+// pixel-grid tiling: bw = W (W | 128), then rows, then images
+bool tile_geometry(int gh, int gw, int& bw, int& bh, int& bn) {
+  if (gw < 8 || gw > 128 || (gw & (gw - 1))) return false;
+  bw = gw;
+  const int rows = BM / gw;
+  if (rows <= gh) { bh = rows; bn = 1; return true; }
+  if ((gh & (gh - 1)) || BM % (gh * gw)) return false;
+  bh = gh; bn = BM / (gh * gw);
+  return true;
+}
+
+int pick_bn(int cout) { return cout % 160 == 0 ? 160 : (cout % 128 == 0 ? 128 : 0); }
+
+template <int BN>
+bool launch(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const TcParams& p, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(conv_tc_k<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<BN>::SMEM) != cudaSuccess) {
+      g_tc_err = "cudaFuncSetAttribute(max dynamic smem) failed";
+      return false;
+    }
+    attr_set = true;
+  }
+  const int tiles = p.tiles_mn * p.n_tiles;
+  const int grid = tiles < g_sms ? tiles : g_sms;
+  conv_tc_k<BN><<<grid, 192, Cfg<BN>::SMEM, st>>>(a0, a1, b, p);
+  return true;
+}
+
+}  // namespace
+
+const char* tc_last_error() { return g_tc_err.c_str(); }
+
+bool conv_tc_supported(const ConvArgs& a) {
+  if (a.dt != DT_BF16) return false;
+  if (a.src.c0 % 64 || a.src.c1 % 64 || a.src.c0 == 0) return false;
+  if (!pick_bn(a.cout)) return false;
+  if (a.ksize != 1 && a.ksize != 3) return false;
+  int bw, bh, bn;
+  if (a.mode == CONV_DGRAD_S2) {
+    if (a.ksize != 3 || a.src.c1) return false;
+    if (a.hout != 2 * a.hin || a.wout != 2 * a.win) return false;
+    return tile_geometry(a.hin, a.win, bw, bh, bn);
+  }
+  if (a.stride == 2) {
+    if (a.ksize != 3 || a.src.c1 || (a.hin & 1) || (a.win & 1) || a.hout * 2 != a.hin || a.wout * 2 != a.win) return false;
+  } else if (a.stride != 1 || a.hout != a.hin || a.wout != a.win) {
+    return false;
+  }
+  return tile_geometry(a.hout, a.wout, bw, bh, bn);
+}
+
+int conv_tc(const ConvArgs& a, cudaStream_t st) {
+  TcParams p;
+  memset(&p, 0, sizeof p);
+  const int bnn = pick_bn(a.cout);
+  const bool s2d = a.mode == CONV_DGRAD_S2, s2f = !s2d && a.stride == 2;
+  const int gh = s2d ? a.hin : a.hout, gw = s2d ? a.win : a.wout;
+  tile_geometry(gh, gw, p.bw, p.bh, p.bn);
+  p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64;
+  p.s2 = s2f;
+  p.tiles_h = (gh + p.bh - 1) / p.bh;
+  p.tiles_mn = p.tiles_h * ((a.n + p.bn - 1) / p.bn);
+  p.n_tiles = a.cout / bnn;
+  p.GH = gh; p.GN = a.n;
+  p.bias = (const bf16*)a.bias; p.pn = a.pn; p.residual = (const bf16*)a.residual; p.out = (bf16*)a.out;
+  p.accumulate = a.accumulate;
+  p.OH = a.hout; p.OW = a.wout; p.osy = p.osx = 1; p.ooy = p.oox = 0; p.cout_total = a.cout;
+  CUtensorMap m0, m1, mb;
+  bool ok = true;
+  if (s2f) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  m1 = m0;
+  if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
+  if (ok) ok = mat_map(a.w, a.cout, (uint64_t)a.ksize * a.ksize * p.ctot, bnn, &mb);
+  if (!ok) return -1;
+  int launches = 0;
+  auto go = [&]() {
+    bool r = bnn == 160 ? launch<160>(m0, m1, mb, p, st) : launch<128>(m0, m1, mb, p, st);
+    if (r) ++launches;
+    return r;
+  };
+  if (s2d) {
+    // output pixel (2y'+py, 2x'+px) <- taps r' with (py + r' - 1) even: py=0: r'=1 (dy 0); py=1: r'=0 (dy 0), r'=2 (dy +1)
+    p.osy = p.osx = 2;
+    for (int py = 0; py < 2; ++py)
+      for (int px = 0; px < 2; ++px) {
+        p.ooy = py; p.oox = px; p.ntaps = 0;
+        for (int r = 0; r < 3; ++r) {
+          if ((py + r - 1) & 1) continue;
+          for (int s = 0; s < 3; ++s) {
+            if ((px + s - 1) & 1) continue;
+            Tap t; t.dy = (py + r - 1) >> 1; t.dx = (px + s - 1) >> 1; t.px = t.py = 0; t.widx = r * 3 + s;
+            p.taps[p.ntaps++] = t;
+          }
+        }
+        if (!go()) return -1;
+      }
+    return launches;
+  }
+  const int pad = (a.ksize - 1) / 2;
+  p.ntaps = a.ksize * a.ksize;
+  for (int r = 0; r < a.ksize; ++r)
+    for (int s = 0; s < a.ksize; ++s) {
+      Tap t; t.widx = r * a.ksize + s; t.px = t.py = 0;
+      if (!s2f) { t.dy = r - pad; t.dx = s - pad; }
+      else {   // input row 2y + r - 1 = 2(y + dy) + py
+        t.dy = r == 0 ? -1 : 0; t.py = r == 1 ? 0 : 1;
+        t.dx = s == 0 ? -1 : 0; t.px = s == 1 ? 0 : 1;
+      }
+      p.taps[t.widx] = t;
+    }
+  if (!go()) return -1;
+  return launches;
+}
+
 bool wgrad_tc_supported(const WgradArgs&) { return false; }
 int wgrad_tc(const WgradArgs&, cudaStream_t) { return 0; }
-const char* tc_last_error() { return ""; }
+
 }  // namespace pulse

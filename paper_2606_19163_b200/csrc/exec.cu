@@ -13,6 +13,7 @@ struct Ctx {
   char* work;     // per-stage workspace
   cudaStream_t st;
   int dt;
+  bool err = false;
   char* fwd(int t) const {
     const TRef& r = s->tensors[t].ref;
     return (r.region == R_SKIP ? skip : r.region == R_STASH ? stash : work) + r.off;
@@ -28,12 +29,12 @@ struct Ctx {
 };
 
 void run_conv(Ctx& c, const ConvArgs& a) {
-  if (c.tc() && conv_tc_supported(a)) c.s->launches += conv_tc(a, c.st);
-  else c.s->launches += conv_simt(a, c.st);
+  const int r = (c.tc() && conv_tc_supported(a)) ? conv_tc(a, c.st) : conv_simt(a, c.st);
+  if (r < 0) c.err = true; else c.s->launches += r;
 }
 void run_wgrad(Ctx& c, const WgradArgs& a) {
-  if (c.tc() && wgrad_tc_supported(a)) c.s->launches += wgrad_tc(a, c.st);
-  else c.s->launches += wgrad_simt(a, c.st);
+  const int r = (c.tc() && wgrad_tc_supported(a)) ? wgrad_tc(a, c.st) : wgrad_simt(a, c.st);
+  if (r < 0) c.err = true; else c.s->launches += r;
 }
 
 ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, int k, int stride, const void* w,
@@ -198,6 +199,7 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   }
   if (open) CK_CUDA(cudaMemcpyAsync(d_e_out, c.fwd(s->t_eout), c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
   CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+  if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   cache->mb[slot] = mb;
   cache->live++;
@@ -280,6 +282,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   }
   if (open) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   if (d_g_x_in) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
+  if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   cache->mb[slot] = -1;
   cache->live--;
@@ -338,6 +341,63 @@ extern "C" pulse_status_t pulse_mse_fwd_bwd(int dtype, const void* d_d, const vo
   const int V = dtype == PULSE_F32 ? 4 : 8;
   if (numel == 0 || numel % V) return fail(PULSE_ERR_SHAPE, "numel must be a positive multiple of %d", V);
   mse_fwd_bwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_d, d_target, numel, scale, d_loss, d_g_d, (cudaStream_t)stream);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+
+// ------------------------------------------------------------------------------ single operators
+static pulse_status_t check_conv(int dtype, int c0, int c1, int n, int h, int w, int ksize, int stride, int cout) {
+  if (dtype != PULSE_F32 && dtype != PULSE_BF16) return fail(PULSE_ERR_INVALID_ARG, "dtype");
+  if (n <= 0 || h <= 0 || w <= 0 || c0 <= 0 || c1 < 0 || cout <= 0) return fail(PULSE_ERR_INVALID_ARG, "non-positive size");
+  if (ksize != 1 && ksize != 3) return fail(PULSE_ERR_UNSUPPORTED, "ksize must be 1 or 3");
+  if (stride != 1 && stride != 2) return fail(PULSE_ERR_UNSUPPORTED, "stride must be 1 or 2");
+  if (stride == 2 && ((h | w) & 1)) return fail(PULSE_ERR_SHAPE, "stride 2 needs even H, W");
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_conv2d(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1, int c1,
+                                       int n, int h, int w, int ksize, int stride, const void* d_w, int cout,
+                                       const void* d_bias, const float* d_pn, const void* d_residual, void* d_out,
+                                       void* stream) {
+  pulse_status_t s = check_conv(dtype, c0, c1, n, h, w, ksize, stride, cout);
+  if (s) return s;
+  if (!d_src0 || !d_w || !d_out || (c1 && !d_src1)) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  ConvArgs a;
+  a.dt = dtype == PULSE_F32 ? DT_F32 : DT_BF16; a.src = Cat{d_src0, c0, d_src1, c1}; a.n = n; a.hin = h; a.win = w;
+  a.hout = h / stride; a.wout = w / stride; a.ksize = ksize; a.stride = stride; a.mode = CONV_FPROP; a.w = d_w;
+  a.cout = cout; a.bias = d_bias; a.pn = d_pn; a.residual = d_residual; a.out = d_out; a.accumulate = 0;
+  const int r = (!force_simt && conv_tc_supported(a)) ? conv_tc(a, (cudaStream_t)stream) : conv_simt(a, (cudaStream_t)stream);
+  if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_conv2d_dgrad(int dtype, int force_simt, const void* d_g, int n, int h, int w, int cin,
+                                             int ksize, int stride, const void* d_w, int cout, void* d_wt, void* d_g_in,
+                                             int accumulate, void* stream) {
+  pulse_status_t s = check_conv(dtype, cin, 0, n, h, w, ksize, stride, cout);
+  if (s) return s;
+  if (!d_g || !d_w || !d_wt || !d_g_in) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  const int dt = dtype == PULSE_F32 ? DT_F32 : DT_BF16;
+  cudaStream_t st = (cudaStream_t)stream;
+  flip_transpose(dt, d_w, cout, ksize, cin, d_wt, st);
+  ConvArgs a;
+  a.dt = dt; a.src = Cat{d_g, cout, nullptr, 0}; a.n = n; a.hin = h / stride; a.win = w / stride; a.hout = h; a.wout = w;
+  a.ksize = ksize; a.stride = 1; a.mode = stride == 2 ? CONV_DGRAD_S2 : CONV_FPROP; a.w = d_wt; a.cout = cin;
+  a.bias = nullptr; a.pn = nullptr; a.residual = nullptr; a.out = d_g_in; a.accumulate = accumulate;
+  const int r = (!force_simt && conv_tc_supported(a)) ? conv_tc(a, st) : conv_simt(a, st);
+  if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1,
+                                             int c1, int n, int h, int w, int ksize, int stride, const void* d_g, int cout,
+                                             float* d_dw, void* stream) {
+  pulse_status_t s = check_conv(dtype, c0, c1, n, h, w, ksize, stride, cout);
+  if (s) return s;
+  if (!d_src0 || !d_g || !d_dw || (c1 && !d_src1)) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  WgradArgs a{dtype == PULSE_F32 ? DT_F32 : DT_BF16, Cat{d_src0, c0, d_src1, c1}, n, h, w, d_g, h / stride, w / stride,
+              cout, ksize, stride, d_dw};
+  const int r = (!force_simt && wgrad_tc_supported(a)) ? wgrad_tc(a, (cudaStream_t)stream) : wgrad_simt(a, (cudaStream_t)stream);
+  if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core wgrad launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }
