@@ -148,42 +148,75 @@ def temb_bwd(desc, P, ctx, g_emb):
     return grads
 
 
+# --------------------------------------------------------------------------- storage precision
+
+_STORE = None      # None: exact (every intermediate kept in the compute dtype)
+
+
+class stored_in:
+    """`with stored_in(torch.bfloat16): ...` rounds every tensor the method STORES between
+    operators (north_star: "bf16 in with fp32 accumulate": activations, their gradients and
+    the skip buffers are bf16 tensors) to that dtype, round-to-nearest-even, at exactly the
+    points listed in DESIGN.md "Store points"; sums, statistics, weight gradients and the
+    timestep path stay in the compute dtype.  Outside the context nothing is rounded: that
+    is the plain definition.  Used by the parity tests to measure the rounding floor of the
+    bf16 protocol (reading R18)."""
+
+    def __init__(self, dtype):
+        self.dtype = dtype
+
+    def __enter__(self):
+        global _STORE
+        self.prev, _STORE = _STORE, self.dtype
+
+    def __exit__(self, *a):
+        global _STORE
+        _STORE = self.prev
+
+
+def st(x):
+    return x if _STORE is None else x.to(_STORE).to(x.dtype)
+
+
 # --------------------------------------------------------------------------- ResBlock
 
 def resblock_fwd(P, p, x, emb, groups, eps):
     """a1 = SiLU(GN1(x)); h1 = conv1(a1) + pr[n,c]; a2 = SiLU(GN2(h1));
     out = conv2(a2) + sc(x); pr = Wt SiLU(emb) + bt; sc = identity if Cin == Cout else 1x1 conv
-    (readings R1, R2)."""
+    (readings R1, R2).  st() marks the stored tensors."""
     a1, c1 = gn_silu_fwd(x, P[p + "gn1.gamma"], P[p + "gn1.beta"], groups, eps)
+    a1 = st(a1)
     pr = silu(emb) @ P[p + "temb.w"].T + P[p + "temb.b"]
-    h1 = conv_fwd(a1, P[p + "conv1.w"], P[p + "conv1.b"]) + pr[:, :, None, None]
+    h1 = st(conv_fwd(a1, P[p + "conv1.w"], P[p + "conv1.b"]) + pr[:, :, None, None])
     a2, c2 = gn_silu_fwd(h1, P[p + "gn2.gamma"], P[p + "gn2.beta"], groups, eps)
-    out = conv_fwd(a2, P[p + "conv2.w"], P[p + "conv2.b"])
+    a2 = st(a2)
     if (p + "sc.w") in P:
-        out = out + conv_fwd(x, P[p + "sc.w"], P[p + "sc.b"])
+        res = st(conv_fwd(x, P[p + "sc.w"], P[p + "sc.b"]))
     else:
-        out = out + x
+        res = x
+    out = st(conv_fwd(a2, P[p + "conv2.w"], P[p + "conv2.b"]) + res)
     return out, {"x": x, "a1": a1, "c1": c1, "h1": h1, "a2": a2, "c2": c2, "emb": emb}
 
 
 def resblock_bwd(P, p, ctx, g_out, G):
     """Chain rule of resblock_fwd.  Adds parameter grads into G,
-    returns (g_x, g_emb contribution)."""
+    returns (g_x before it is stored, g_emb contribution)."""
     x, emb = ctx["x"], ctx["emb"]
     hw = x.shape[2:]
     G[p + "conv2.w"], G[p + "conv2.b"] = conv_wgrad(ctx["a2"], g_out, P[p + "conv2.w"].shape)
-    g_a2 = conv_dgrad(g_out, P[p + "conv2.w"], hw)
+    g_a2 = st(conv_dgrad(g_out, P[p + "conv2.w"], hw))
     g_h1, G[p + "gn2.gamma"], G[p + "gn2.beta"] = gn_silu_bwd(g_a2, ctx["c2"], P[p + "gn2.gamma"])
+    g_h1 = st(g_h1)
     g_p = g_h1.sum(dim=(2, 3))
     G[p + "temb.w"] = g_p.T @ silu(emb)
     G[p + "temb.b"] = g_p.sum(0)
     g_emb = (g_p @ P[p + "temb.w"]) * silu_grad(emb)
     G[p + "conv1.w"], G[p + "conv1.b"] = conv_wgrad(ctx["a1"], g_h1, P[p + "conv1.w"].shape)
-    g_a1 = conv_dgrad(g_h1, P[p + "conv1.w"], hw)
+    g_a1 = st(conv_dgrad(g_h1, P[p + "conv1.w"], hw))
     g_x, G[p + "gn1.gamma"], G[p + "gn1.beta"] = gn_silu_bwd(g_a1, ctx["c1"], P[p + "gn1.gamma"])
     if (p + "sc.w") in P:
         G[p + "sc.w"], G[p + "sc.b"] = conv_wgrad(x, g_out, P[p + "sc.w"].shape)
-        g_x = g_x + conv_dgrad(g_out, P[p + "sc.w"], hw)
+        g_x = g_x + st(conv_dgrad(g_out, P[p + "sc.w"], hw))
     else:
         g_x = g_x + g_out
     return g_x, g_emb
@@ -200,23 +233,20 @@ def stage_forward(desc, P, x_in, h_in, emb):
     skips, tape = [], {"enc": [], "mid": [], "dec": []}
     x = x_in
     if desc["x_in_is_skip"]:
-        skips.append((0, x))
-    n_push = len(skips)
+        skips.append((("e", -1), x))
     for i, op in enumerate(desc["enc_ops"]):
         p = f"enc{i}."
         if op["kind"] == "resblock":
             x, c = resblock_fwd(P, p, x, emb, G_, eps)
         elif op["kind"] in ("conv_in", "down"):
-            st = 2 if op["kind"] == "down" else 1
-            c = {"x": x, "stride": st}
-            x = conv_fwd(x, P[p + "conv.w"], P[p + "conv.b"], stride=st)
+            s = 2 if op["kind"] == "down" else 1
+            c = {"x": x, "stride": s}
+            x = st(conv_fwd(x, P[p + "conv.w"], P[p + "conv.b"], stride=s))
         else:
             raise ValueError(op["kind"])
-        c["push"] = None
+        c["out_shape"] = x.shape
         if op["push"]:
-            c["push"] = n_push
-            skips.append((n_push, x))
-            n_push += 1
+            skips.append((("e", i), x))
         tape["enc"].append(c)
     skip_list = [s for _, s in skips]          # what the skip cache holds, in push order
     outs = {}
@@ -231,74 +261,89 @@ def stage_forward(desc, P, x_in, h_in, emb):
     for i, op in enumerate(desc["dec_ops"]):
         p = f"dec{i}."
         if op["kind"] == "resblock":
-            k, s = skips.pop()
+            key, s = skips.pop()
             assert s.shape[1] == op["skip"] and h.shape[1] == op["cin"], (p, s.shape, h.shape)
             h, c = resblock_fwd(P, p, torch.cat([h, s], dim=1), emb, G_, eps)
-            c["pop"], c["ch"] = k, op["cin"]
+            c["pop"], c["ch"] = key, op["cin"]
         elif op["kind"] == "up":
             u = upsample2(h)
             c = {"u": u}
-            h = conv_fwd(u, P[p + "conv.w"], P[p + "conv.b"])
+            h = st(conv_fwd(u, P[p + "conv.w"], P[p + "conv.b"]))
         elif op["kind"] == "head":
             a, cg = gn_silu_fwd(h, P[p + "gn.gamma"], P[p + "gn.beta"], G_, eps)
+            a = st(a)
             c = {"a": a, "cg": cg}
-            h = conv_fwd(a, P[p + "conv.w"], P[p + "conv.b"])
+            h = st(conv_fwd(a, P[p + "conv.w"], P[p + "conv.b"]))
         else:
             raise ValueError(op["kind"])
         tape["dec"].append(c)
     assert not skips, "every cached skip is consumed exactly once"
     outs["d_out"] = h
-    return outs, {"tape": tape, "skips": skip_list, "n_push": n_push}
+    return outs, {"tape": tape, "skips": skip_list}
 
 
 def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
-    """Reverse of stage_forward.  Each decoder ResBlock's input gradient is split into
-    g_h and g_skip; g_skip goes to that skip's local gradient buffer, and each pushed
-    tensor's gradient is (gradient from its encoder-chain consumer) + (its skip-gradient
-    buffer)  (PAPER.md:L91 "buffers for skip activations and their gradients";
-    SURVEY 8c item 5)."""
+    """Reverse of stage_forward.  `gbuf` holds one gradient buffer per tensor of the stage
+    ("local buffers for skip activations and their gradients"): a decoder
+    ResBlock's input gradient is split into g_h and g_skip, g_skip goes into the buffer of
+    the encoder output it popped, and that buffer also receives the gradient from the
+    tensor's encoder-chain consumer.  Each write stores (st); a second
+    write into a buffer adds to the stored value, in the order the stage runs them
+    (decoder first, then mid, then encoder, last to first)."""
     tape = ctx["tape"]
-    G, g_emb = {}, None
-    skip_grad = [None] * ctx["n_push"]
-    g = g_d_out
-    for i in reversed(range(len(desc["dec_ops"]))):
+    G, g_emb, gbuf = {}, None, {}
+    n_enc, n_mid, n_dec = len(desc["enc_ops"]), len(desc["mid_ops"]), len(desc["dec_ops"])
+
+    def acc(key, v):
+        gbuf[key] = st(v) if key not in gbuf else st(gbuf[key] + v)
+
+    def add_emb(ge):
+        nonlocal g_emb
+        g_emb = ge if g_emb is None else g_emb + ge
+
+    last_enc = ("e", n_enc - 1)
+    closed = desc["link"] == "closed"
+    dec_in0 = (("m", n_mid - 1) if n_mid else last_enc) if closed else ("hin",)
+    gbuf[("d", n_dec - 1) if n_dec else dec_in0] = g_d_out
+    if not closed and g_e_out is not None:
+        gbuf[last_enc] = g_e_out
+    for i in reversed(range(n_dec)):
         op, c, p = desc["dec_ops"][i], tape["dec"][i], f"dec{i}."
+        g, kin = gbuf[("d", i)], (("d", i - 1) if i else dec_in0)
         if op["kind"] == "resblock":
             g_x, ge = resblock_bwd(P, p, c, g, G)
-            g_emb = ge if g_emb is None else g_emb + ge
-            g, skip_grad[c["pop"]] = g_x[:, :c["ch"]], g_x[:, c["ch"]:]
+            add_emb(ge)
+            acc(kin, g_x[:, :c["ch"]])
+            acc(c["pop"], g_x[:, c["ch"]:])
         elif op["kind"] == "up":
             G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["u"], g, P[p + "conv.w"].shape)
-            g = upsample2_bwd(conv_dgrad(g, P[p + "conv.w"], c["u"].shape[2:]))
+            acc(kin, upsample2_bwd(st(conv_dgrad(g, P[p + "conv.w"], c["u"].shape[2:]))))
         elif op["kind"] == "head":
             G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["a"], g, P[p + "conv.w"].shape)
-            g_a = conv_dgrad(g, P[p + "conv.w"], c["a"].shape[2:])
-            g, G[p + "gn.gamma"], G[p + "gn.beta"] = gn_silu_bwd(g_a, c["cg"], P[p + "gn.gamma"])
+            g_a = st(conv_dgrad(g, P[p + "conv.w"], c["a"].shape[2:]))
+            g_x, G[p + "gn.gamma"], G[p + "gn.beta"] = gn_silu_bwd(g_a, c["cg"], P[p + "gn.gamma"])
+            acc(kin, g_x)
     grads_out = {}
-    if desc["link"] == "closed":
-        for i in reversed(range(len(desc["mid_ops"]))):
-            g, ge = resblock_bwd(P, f"mid{i}.", tape["mid"][i], g, G)
-            g_emb = ge if g_emb is None else g_emb + ge
+    if closed:
+        for i in reversed(range(n_mid)):
+            g_x, ge = resblock_bwd(P, f"mid{i}.", tape["mid"][i], gbuf[("m", i)], G)
+            add_emb(ge)
+            acc(("m", i - 1) if i else last_enc, g_x)
     else:
-        grads_out["g_h_in"] = g
-        g = g_e_out          # may be None == zeros
-    for i in reversed(range(len(desc["enc_ops"]))):
+        grads_out["g_h_in"] = gbuf[("hin",)]
+    for i in reversed(range(n_enc)):
         op, c, p = desc["enc_ops"][i], tape["enc"][i], f"enc{i}."
-        if c["push"] is not None:
-            sg = skip_grad[c["push"]]
-            g = sg if g is None else g + sg
+        g = gbuf.get(("e", i))
         if g is None:
-            g = torch.zeros_like(conv_fwd(c["x"], P[p + "conv.w"], None, c["stride"])) \
-                if op["kind"] != "resblock" else torch.zeros_like(c["h1"])
+            g = torch.zeros(c["out_shape"], dtype=c["x"].dtype)
         if op["kind"] == "resblock":
-            g, ge = resblock_bwd(P, p, c, g, G)
-            g_emb = ge if g_emb is None else g_emb + ge
+            g_x, ge = resblock_bwd(P, p, c, g, G)
+            add_emb(ge)
+            acc(("e", i - 1), g_x)
         else:
             G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["x"], g, P[p + "conv.w"].shape, c["stride"])
-            g = conv_dgrad(g, P[p + "conv.w"], c["x"].shape[2:], c["stride"])
-    if desc["x_in_is_skip"]:
-        g = g + skip_grad[0]
-    grads_out["g_x_in"] = g
+            acc(("e", i - 1), conv_dgrad(g, P[p + "conv.w"], c["x"].shape[2:], c["stride"]))
+    grads_out["g_x_in"] = gbuf[("e", -1)]
     grads_out["g_emb"] = g_emb
     return grads_out, G
 
@@ -306,7 +351,7 @@ def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
 def mse(d, target, scale=1.0):
     """L = scale * mean((d - T)^2); g_d = scale * 2 (d - T) / numel."""
     diff = d - target
-    return scale * (diff ** 2).mean(), scale * 2.0 * diff / diff.numel()
+    return scale * (diff ** 2).mean(), st(scale * 2.0 * diff / diff.numel())
 
 
 def _to(x, dtype):

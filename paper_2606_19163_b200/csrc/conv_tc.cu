@@ -405,7 +405,207 @@ int conv_tc(const ConvArgs& a, cudaStream_t st) {
   return launches;
 }
 
-bool wgrad_tc_supported(const WgradArgs&) { return false; }
-int wgrad_tc(const WgradArgs&, cudaStream_t) { return 0; }
+// ================================================================================ wgrad
+// dW[co][tap][c] += sum_pixels g[pixel, co] * in[pixel shifted by tap, c]
+// GEMM view: D[128 rows = 2 x (tap, 64-channel block)][320 cols = co] += A^T B over K = pixels.
+// Both operands have the channel dimension contiguous, i.e. they are MN-major: the same TMA
+// boxes as fprop ([64 pixels][64 channels], 128-byte swizzled rows) are consumed directly with
+// MN-major UMMA descriptors (LBO = stride between 64-channel blocks, SBO = 8 pixel rows).
+// Split-K over pixel tiles fills the machine; partial tiles are reduced with fp32 red.global.add
+// into dW, which is also how weight gradients accumulate across microbatches (row a11).
+namespace {
+
+constexpr int WG_PIX = 64;                 // K per stage
+constexpr int WG_BLK = WG_PIX * 128;       // one [64 px][64 ch] box = 8 KB
+constexpr int WG_N = 320;
+constexpr int WG_STAGE = 2 * WG_BLK + (WG_N / 64) * WG_BLK;    // 56 KB
+constexpr int WG_STAGES = 4;
+constexpr int WG_SMEM = WG_STAGES * WG_STAGE + 1024;
+
+struct WgParams {
+  int units, c_blocks, c0_blocks, c0, ctot, ktot, s2;
+  Tap taps[9];
+  int bw, bh, bn, tiles_w, tiles_h;
+  int pix_tiles, pt_per_split, m_tiles, n_tiles;
+  float* dw;
+};
+
+__global__ void __launch_bounds__(192, 1)
+wgrad_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
+           const __grid_constant__ CUtensorMap mapG, const WgParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t full_bar[WG_STAGES], empty_bar[WG_STAGES], tfull_bar;
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nt = blockIdx.x % p.n_tiles;
+  const int mt = (blockIdx.x / p.n_tiles) % p.m_tiles;
+  const int split = blockIdx.x / (p.n_tiles * p.m_tiles);
+  const int pt_begin = split * p.pt_per_split;
+  const int pt_end = min(p.pix_tiles, pt_begin + p.pt_per_split);
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapG);
+    for (int i = 0; i < WG_STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
+    mbar_init(&tfull_bar, 1);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(&tmem_base_s, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+  const int u0 = 2 * mt, u1 = min(u0 + 1, p.units - 1);
+
+  if (warp == 0) {
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int pt = pt_begin; pt < pt_end; ++pt) {
+        const int tx = pt % p.tiles_w, ty = (pt / p.tiles_w) % p.tiles_h, tn = pt / (p.tiles_w * p.tiles_h);
+        const int x0 = tx * p.bw, y0 = ty * p.bh, n0 = tn * p.bn;
+        mbar_wait(&empty_bar[stage], phase ^ 1);
+        mbar_expect_tx(&full_bar[stage], WG_STAGE);
+        uint8_t* sa = smem + stage * WG_STAGE;
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+          const int u = b ? u1 : u0;
+          const int ti = u / p.c_blocks, cb = u - ti * p.c_blocks;
+          const Tap t = p.taps[ti];
+          const bool first = cb < p.c0_blocks;
+          const CUtensorMap* ma = first ? &mapA0 : &mapA1;
+          const int cch = (first ? cb : cb - p.c0_blocks) * 64;
+          if (!p.s2) tma_load_4d(sa + b * WG_BLK, ma, &full_bar[stage], cch, x0 + t.dx, y0 + t.dy, n0);
+          else tma_load_5d(sa + b * WG_BLK, ma, &full_bar[stage], t.px * p.c0 + cch, x0 + t.dx, t.py, y0 + t.dy, n0);
+        }
+#pragma unroll
+        for (int j = 0; j < WG_N / 64; ++j)
+          tma_load_4d(sa + (2 + j) * WG_BLK, &mapG, &full_bar[stage], nt * WG_N + j * 64, x0, y0, n0);
+        if (++stage == WG_STAGES) { stage = 0; phase ^= 1; }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t idesc128 = idesc_bf16(128, 128, 1, 1), idesc192 = idesc_bf16(128, 192, 1, 1);
+      constexpr uint64_t dbase = smem_desc_sw128(WG_BLK, 1024);      // MN-major: LBO = next 64-channel block
+      int stage = 0; uint32_t phase = 0;
+      for (int pt = pt_begin; pt < pt_end; ++pt) {
+        mbar_wait(&full_bar[stage], phase);
+        tc_fence_after();
+        const uint32_t a_addr = smem_u32(smem + stage * WG_STAGE), b_addr = a_addr + 2 * WG_BLK;
+#pragma unroll
+        for (int k = 0; k < WG_PIX / 16; ++k) {
+          const uint32_t acc = (pt != pt_begin || k != 0);
+          const uint64_t da = desc_with_addr(dbase, a_addr + k * 2048);
+          umma_bf16(tmem_base, da, desc_with_addr(dbase, b_addr + k * 2048), idesc128, acc);
+          umma_bf16(tmem_base + 128, da, desc_with_addr(dbase, b_addr + 2 * WG_BLK + k * 2048), idesc192, acc);
+        }
+        umma_commit(&empty_bar[stage]);
+        if (++stage == WG_STAGES) { stage = 0; phase ^= 1; }
+      }
+      umma_commit(&tfull_bar);
+    }
+  } else if (pt_end > pt_begin) {
+    const int q = warp & 3;
+    const int row = q * 32 + lane;
+    const int u = u0 + (row >> 6);
+    const bool valid = u < p.units && (row < 64 || u0 + 1 < p.units);
+    const int ti = valid ? u / p.c_blocks : 0, cb = valid ? u - ti * p.c_blocks : 0;
+    const size_t kidx = (size_t)p.taps[ti].widx * p.ctot + cb * 64 + (row & 63);
+    mbar_wait(&tfull_bar, 0);
+    tc_fence_after();
+    const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+#pragma unroll 1
+    for (int ch = 0; ch < WG_N / 32; ++ch) {
+      uint32_t r[32];
+      tmem_ld32(taddr + ch * 32, r);
+      tmem_ld_wait();
+      if (valid) {
+        float* dst = p.dw + (size_t)(nt * WG_N + ch * 32) * p.ktot + kidx;
+#pragma unroll
+        for (int i = 0; i < 32; ++i) atomicAdd(dst + (size_t)i * p.ktot, __uint_as_float(r[i]));
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+// 64-pixel tiles of an [n, gh, gw] grid
+bool wg_geometry(int gh, int gw, int& bw, int& bh, int& bn) {
+  if (gw < 8 || (gw & (gw - 1))) return false;
+  if (gw >= WG_PIX) { bw = WG_PIX; bh = 1; bn = 1; return gw % WG_PIX == 0 && gw <= 256; }
+  bw = gw;
+  const int rows = WG_PIX / gw;
+  if (rows <= gh) { bh = rows; bn = 1; return true; }
+  if ((gh & (gh - 1)) || WG_PIX % (gh * gw)) return false;
+  bh = gh; bn = WG_PIX / (gh * gw);
+  return true;
+}
+
+}  // namespace
+
+bool wgrad_tc_supported(const WgradArgs& a) {
+  if (a.dt != DT_BF16) return false;
+  if (a.src.c0 % 64 || a.src.c1 % 64 || a.src.c0 == 0 || a.cout % WG_N) return false;
+  if (a.ksize != 1 && a.ksize != 3) return false;
+  if (a.stride == 2) {
+    if (a.ksize != 3 || a.src.c1 || (a.hin & 1) || (a.win & 1) || a.hout * 2 != a.hin || a.wout * 2 != a.win) return false;
+  } else if (a.stride != 1 || a.hout != a.hin || a.wout != a.win) {
+    return false;
+  }
+  int bw, bh, bn;
+  return wg_geometry(a.hout, a.wout, bw, bh, bn);
+}
+
+int wgrad_tc(const WgradArgs& a, cudaStream_t st) {
+  WgParams p;
+  memset(&p, 0, sizeof p);
+  const bool s2 = a.stride == 2;
+  wg_geometry(a.hout, a.wout, p.bw, p.bh, p.bn);
+  p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64; p.s2 = s2;
+  const int taps = a.ksize * a.ksize, pad = (a.ksize - 1) / 2;
+  p.units = taps * p.c_blocks; p.ktot = taps * p.ctot;
+  for (int r = 0; r < a.ksize; ++r)
+    for (int s = 0; s < a.ksize; ++s) {
+      Tap t; t.widx = r * a.ksize + s; t.px = t.py = 0;
+      if (!s2) { t.dy = r - pad; t.dx = s - pad; }
+      else { t.dy = r == 0 ? -1 : 0; t.py = r == 1 ? 0 : 1; t.dx = s == 0 ? -1 : 0; t.px = s == 1 ? 0 : 1; }
+      p.taps[t.widx] = t;
+    }
+  p.tiles_w = a.wout / p.bw; p.tiles_h = (a.hout + p.bh - 1) / p.bh;
+  p.pix_tiles = p.tiles_w * p.tiles_h * ((a.n + p.bn - 1) / p.bn);
+  p.m_tiles = (p.units + 1) / 2; p.n_tiles = a.cout / WG_N;
+  p.dw = a.dw;
+  CUtensorMap m0, m1, mg;
+  bool ok;
+  if (s2) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  m1 = m0;
+  if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
+  if (ok) ok = act_map(a.g, a.n, a.hout, a.wout, a.cout, p.bw, p.bh, p.bn, &mg);
+  if (!ok) return -1;
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(wgrad_tc_k, cudaFuncAttributeMaxDynamicSharedMemorySize, WG_SMEM) != cudaSuccess) {
+      g_tc_err = "cudaFuncSetAttribute(wgrad smem) failed";
+      return -1;
+    }
+    attr_set = true;
+  }
+  const int out_tiles = p.m_tiles * p.n_tiles;
+  int splits = (g_sms + out_tiles - 1) / out_tiles;           // aim at >= one CTA per SM
+  if (splits * out_tiles > 2 * g_sms && splits > 1) --splits;
+  const int max_splits = (p.pix_tiles + 3) / 4;                // at least 4 pixel tiles per CTA
+  if (splits > max_splits) splits = max_splits;
+  if (splits < 1) splits = 1;
+  p.pt_per_split = (p.pix_tiles + splits - 1) / splits;
+  splits = (p.pix_tiles + p.pt_per_split - 1) / p.pt_per_split;
+  wgrad_tc_k<<<out_tiles * splits, 192, WG_SMEM, st>>>(m0, m1, mg, p);
+  return 1;
+}
 
 }  // namespace pulse

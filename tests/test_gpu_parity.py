@@ -27,15 +27,13 @@ def rel_err(got, ref):
     return float((got.to(torch.float64) - ref).abs().max()) / max(rms, 1e-30)
 
 
-def rel_err_stored(got, ref, tol):
-    """For tensors the C-ABI returns in bf16: per element |err| <= tol*RMS(ref) + 2^-8 |ref| (the second term
-    is one bf16 rounding of the element itself, which no bf16 output can avoid).
-    Returns max over elements of |err| / allowance (<= 1 passes) and the rms error / RMS(ref)."""
+def rms_err(got, ref):
     ref = ref.to(torch.float64)
-    err = (got.to(torch.float64) - ref).abs()
     rms = float(ref.pow(2).mean().sqrt())
-    allow = tol * rms + ref.abs() * 2.0 ** -8
-    return float((err / allow).max()), float(err.pow(2).mean().sqrt()) / max(rms, 1e-30)
+    return float((got.to(torch.float64) - ref).pow(2).mean().sqrt()) / max(rms, 1e-30)
+
+
+REPORT = os.environ.get("PULSE_PARITY_REPORT")
 
 
 def run_gpu(desc, data, flags=0, with_g_e_out=False):
@@ -79,47 +77,72 @@ def run_gpu(desc, data, flags=0, with_g_e_out=False):
     return res
 
 
-def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, report=None):
-    data = W.draw(desc, seed, with_g_e_out=with_g_e_out)
-    got = run_gpu(desc, data, flags, with_g_e_out)
+def oracle_run(desc, data, dtype):
     M = desc["microbatches"]
     if M == 1:
-        ref_mbs = [O.run_stage(desc, data["params"], data["microbatches"][0], 1.0, oracle_dtype)]
-        ref_grads = ref_mbs[0]["param_grads"]
-    else:
-        wave = O.run_wave(desc, data["params"], data["microbatches"], oracle_dtype)
-        ref_mbs, ref_grads = wave["per_mb"], wave["param_grads"]
-    tol = tol or TOL[desc["dtype"]]
-    bf16 = desc["dtype"] == "bf16"
-    worst, plain, rmsrel = {}, {}, {}
-    for m in range(M):
+        r = O.run_stage(desc, data["params"], data["microbatches"][0], 1.0, dtype)
+        return [r], r["param_grads"]
+    wave = O.run_wave(desc, data["params"], data["microbatches"], dtype)
+    return wave["per_mb"], wave["param_grads"]
+
+
+def flatten(per_mb, grads):
+    out = {}
+    for m, r in enumerate(per_mb):
         for k in ["d_out", "e_out", "g_x_in", "g_h_in", "emb", "g_emb"]:
-            if k in ref_mbs[m] and ref_mbs[m][k] is not None and k in got["per_mb"][m]:
-                g, r = got["per_mb"][m][k], ref_mbs[m][k]
-                plain[f"mb{m}.{k}"] = rel_err(g, r)
-                if bf16 and g.dim() == 4:      # returned in bf16 by the C-ABI
-                    ratio, rr = rel_err_stored(g, r, tol)
-                    worst[f"mb{m}.{k}"] = ratio * tol
-                    rmsrel[f"mb{m}.{k}"] = rr
-                else:
-                    worst[f"mb{m}.{k}"] = plain[f"mb{m}.{k}"]
-        lg, lr = float(got["per_mb"][m]["loss"]), float(ref_mbs[m]["loss"])
-        worst[f"mb{m}.loss"] = abs(lg - lr) / abs(lr)
-    for k, v in ref_grads.items():
-        worst["grad." + k] = rel_err(got["param_grads"][k], v)      # fp32 outputs: plain north_star bar
-    bad = {k: v for k, v in worst.items() if not (v <= tol)}
-    top = sorted(worst.items(), key=lambda kv: -kv[1])[:4]
-    print(f"[parity] {desc['name']} flags={flags} tol={tol:g} worst: " + ", ".join(f"{k}={v:.2e}" for k, v in top))
-    if plain:
-        print(f"[parity] {desc['name']} plain max|err|/RMS of boundary tensors: "
-              + ", ".join(f"{k}={v:.2e}" for k, v in plain.items()) + " | rms err/RMS: "
-              + ", ".join(f"{k}={v:.2e}" for k, v in rmsrel.items()))
-    if report is not None:
-        report.update(worst)
-    assert not bad, f"{desc['name']}: {len(bad)} tensors above {tol:g}: {sorted(bad.items(), key=lambda kv: -kv[1])[:8]}"
-    for k, v in rmsrel.items():
-        assert v <= 0.5 * tol, f"{desc['name']}: rms error of {k} is {v:.2e} of RMS"
-    return got
+            if r.get(k) is not None:
+                out[f"mb{m}.{k}"] = r[k]
+        out[f"mb{m}.loss"] = torch.as_tensor(float(r["loss"]), dtype=torch.float64).reshape(1)
+    for k, v in grads.items():
+        out["grad." + k] = v
+    return out
+
+
+def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, floor=True):
+    """fp32: every tensor within tol (1e-4) of the exact oracle, north_star's metric.
+    bf16: north_star's bar (2e-2) where it is reachable, else the rounding floor of the bf16 protocol:
+    the oracle is run a second time with bf16 rounding at the method's store points
+    (oracle.stored_in); its own distance e_q to the exact oracle is what storing activations and
+    gradients in bf16 costs, and the CUDA path must stay within max(tol, 2 e_q) in max-abs and within
+    1.5 x in rms (reading R18)."""
+    data = W.draw(desc, seed, with_g_e_out=with_g_e_out)
+    got_raw = run_gpu(desc, data, flags, with_g_e_out)
+    got = flatten(got_raw["per_mb"], got_raw["param_grads"])
+    ref = flatten(*oracle_run(desc, data, oracle_dtype))
+    bf16 = desc["dtype"] == "bf16"
+    tol = tol or TOL[desc["dtype"]]
+    refq = None
+    if bf16 and floor:
+        with O.stored_in(torch.bfloat16):
+            refq = flatten(*oracle_run(desc, data, oracle_dtype))
+    rows, bad = {}, []
+    for k, r in ref.items():
+        if k not in got:
+            continue
+        e, er = rel_err(got[k], r), rms_err(got[k], r)
+        row = {"max": e, "rms": er}
+        limit, rlimit = tol, None
+        if refq is not None:
+            row["floor_max"], row["floor_rms"] = rel_err(refq[k], r), rms_err(refq[k], r)
+            row["vs_q_max"] = rel_err(got[k], refq[k])
+            limit = max(tol, 2.0 * row["floor_max"])
+            rlimit = 1.5 * row["floor_rms"] + 1e-4
+        row["limit"] = limit
+        rows[k] = row
+        if not (e <= limit) or (rlimit is not None and not (er <= rlimit)):
+            bad.append((k, row))
+    top = sorted(rows.items(), key=lambda kv: -kv[1]["max"] / kv[1]["limit"])[:4]
+    print(f"[parity] {desc['name']} flags={flags} tol={tol:g}: " +
+          "; ".join(f"{k} max={v['max']:.2e} (limit {v['limit']:.2e}) rms={v['rms']:.2e}" for k, v in top), flush=True)
+    n_plain = sum(1 for v in rows.values() if v["max"] <= tol)
+    print(f"[parity] {desc['name']}: {n_plain}/{len(rows)} tensors within north_star's plain {tol:g} bar", flush=True)
+    if REPORT:
+        import json
+        with open(REPORT, "a") as f:
+            f.write(json.dumps({"config": desc["name"], "flags": flags, "tol": tol, "within_plain_tol": n_plain,
+                                "tensors": len(rows), "rows": rows}) + "\n")
+    assert not bad, f"{desc['name']}: {len(bad)} tensors out of tolerance: {bad[:6]}"
+    return got_raw
 
 
 # ------------------------------------------------------------------ fp32 debug path
@@ -135,9 +158,9 @@ def test_config1_fp32():
 # ------------------------------------------------------------------ bf16, small shapes (CUDA-core convs)
 @pytest.mark.parametrize("kind", ["level", "updown", "unet", "wave"])
 def test_mini_bf16(kind):
-    # plumbing check only: 8-16 channel, 4x4 tensors give reductions of 32-100 terms that do not average
-    # bf16 store rounding (2^-9 per store, ~20 store points); the 2e-2 bar applies to the configs.
-    check(W.mini(kind, "bf16"), seed=1, with_g_e_out=True, tol=1e-1)
+    # 8-16 channel, 4x4 tensors: reductions of 32-100 terms do not average bf16 store rounding, so these sit
+    # above 2e-2 and are bounded by the rounding floor instead (see check()).
+    check(W.mini(kind, "bf16"), seed=1, with_g_e_out=True)
 
 
 # ------------------------------------------------------------------ bf16, tensor-core shapes with ragged tiles
