@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py - one "step" = the whole hot path (temb -> stage forward -> MSE -> stage backward
+-> temb backward; for configs[4] the wave F0..F7,B7..B0) over one batch of synthetic input.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+Prints ONE JSON line (contract in the task statement / DESIGN.md "Measurement").  N > 1 runs
+N independent replicas (the path has no exchange step - "replicas only").
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+import torch  # noqa: E402
+
+from paper_2606_19163_b200 import workloads as W  # noqa: E402
+
+METRIC = "stage fwd+bwd samples/s"
+WORKLOADS = {1: "configs[0]: tiny collocated pair, fp32 debug path", 2: "configs[1]: SD1.5-shaped level-1 stage, "
+             "2 enc + 3 dec ResBlocks 320ch, microbatch 4, 64x64", 3: "configs[2]: level-2 stage with down/up, "
+             "microbatch 8, 32x32", 4: "configs[3]: full conv-only SD1.5-shaped UNet, microbatch 8, 4x64x64",
+             5: "configs[4]: SDXL-shaped stage, wave of 8 microbatches of 2, 4x128x128"}
+
+
+def conv_flops_fwd(desc) -> float:
+    """Algorithmic forward FLOPs of the convs + linears of one microbatch: 2 N Ho Wo Cout Cin k^2
+    (SURVEY.md 8d); the nominal 9-tap count for the up conv."""
+    n, h, w = desc["n"], desc["h"], desc["w"]
+    T = desc["temb"]["dim"]
+    fl = 0.0
+    if desc["temb"]["kind"] == "mlp":
+        fl += 2.0 * n * T * (desc["temb"]["d0"] + T)
+    sk = W.skip_channels_pushed(desc)
+    hh, ww = h, w
+    for op in desc["enc_ops"] + desc["mid_ops"]:
+        if op["kind"] == "down":
+            hh, ww = hh // 2, ww // 2
+        fl += _op_flops(op, n, hh, ww, T)
+    if desc["link"] == "open" and sk:
+        hh, ww = sk[-1][1], sk[-1][2]
+    for op in desc["dec_ops"]:
+        if op["kind"] == "up":
+            hh, ww = 2 * hh, 2 * ww
+        fl += _op_flops(op, n, hh, ww, T)
+    return fl
+
+
+def _op_flops(op, n, h, w, T):
+    ci, co = op["cin"] + op["skip"], op["cout"]
+    pix = 2.0 * n * h * w
+    if op["kind"] == "resblock":
+        f = pix * co * ci * 9 + pix * co * co * 9 + 2.0 * n * co * T
+        if ci != co:
+            f += pix * co * ci
+        return f
+    return pix * co * ci * 9
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        rows = [l.split(",") for t, l in self.lines if t0 <= t <= t1] or [l.split(",") for _, l in self.lines[-3:]]
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.strip().lower() == "active":
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def max_over_ranks(x: float, dist, device="cuda") -> float:
+    """Replicas only: the job's time is the slowest replica's (max over ranks)."""
+    if dist is None:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(samples_per_rank: int, world: int, seconds_max: float) -> float:
+    """Whole-job samples/s of `world` independent replicas (weak scaling)."""
+    return world * samples_per_rank / seconds_max
+
+
+def oracle_time(desc, data, budget_note):
+    from oracle import pulse_oracle as O
+    t0 = time.perf_counter()
+    if desc["microbatches"] == 1:
+        O.run_stage(desc, data["params"], data["microbatches"][0])
+    else:
+        O.run_wave(desc, data["params"], data["microbatches"])
+    dt = time.perf_counter() - t0
+    samples = desc["n"] * desc["microbatches"]
+    return {"value": samples / dt, "unit": "samples/s", "cores": torch.get_num_threads(), "kind": "oracle",
+            "sample": budget_note, "seconds": dt}
+
+
+def reference_sample(desc, full=False):
+    """Bounded sample of the workload for the CPU oracle: the stage structure and spatial size of the
+    config with the microbatch cut to 1 sample (GroupNorm and every conv are per-sample, so cost
+    scales linearly with N) and, for the wave, one microbatch."""
+    n = desc["n"] if (full and desc["name"] in ("config1", "config2")) else 1
+    d = W.scaled(desc, n=n, microbatches=1)
+    return d, f"{desc['name']} structure at N={n} sample(s), 1 microbatch, fp64 oracle as it stands"
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    desc = W.config(args.config)
+    d1, note = reference_sample(desc)
+    data = W.draw(d1, 0)
+    for _ in range(min(args.warmup, 1)):
+        oracle_time(d1, data, note)
+    ts = []
+    for _ in range(args.steps):
+        r = oracle_time(d1, data, note)
+        ts.append(r["seconds"])
+    dt = float(np.mean(ts))
+    val = d1["n"] / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "samples/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded N(0,1), DESIGN.md)",
+            "config": {"workload": WORKLOADS[args.config], "sample": note},
+            "cpu_baseline": {"value": val, "unit": "samples/s", "cores": torch.get_num_threads(), "kind": "oracle",
+                             "sample": note},
+            "e2e": {"value": val, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 3)
+
+    from paper_2606_19163_b200 import binding as B
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    desc = W.config(args.config)
+    M = desc["microbatches"]
+    data = W.draw(desc, 0)
+    st = B.Stage(desc)
+    st.load_params(data["params"])
+    devs = [st.to_device(mb) for mb in data["microbatches"]]
+    samples = desc["n"] * M
+    flops_step = 3.0 * conv_flops_fwd(desc) * M
+    loss = torch.zeros(1, dtype=torch.float32, device="cuda")
+
+    def step():
+        loss.zero_()
+        if M == 1:
+            return st.step(0, devs[0], 1.0, accumulate=False, loss=loss)
+        fw = []
+        for m, dev in enumerate(devs):                      # wave: F0..F{M-1}
+            emb, tst = st.temb_forward(dev["t"])
+            fw.append((emb, tst) + st.forward(m, dev["x_in"], dev.get("h_in"), emb))
+        for m in reversed(range(M)):                        # B{M-1}..B0
+            emb, tst, e_out, d_out = fw[m]
+            _, g_d = st.mse(d_out, devs[m]["target"], 1.0 / M, loss)
+            g_temb = torch.zeros_like(emb)
+            st.backward(m, g_d, None, True, g_temb, accumulate=(m != M - 1))
+            st.temb_backward(g_temb, tst, accumulate=(m != M - 1))
+        return None
+
+    # eager warm-up (first launches set function attributes, build tensor maps)
+    for _ in range(2):
+        step()
+    torch.cuda.synchronize()
+    l0 = st.launches()
+    step()
+    torch.cuda.synchronize()
+    launches_per_step = st.launches() - l0 + M       # + the MSE kernel(s), which take no stage handle
+
+    graph = None
+    if not args.no_graph:
+        try:
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                step()
+        except Exception as e:      # keep measuring eagerly, say so
+            graph = None
+            sys.stderr.write(f"bench: CUDA graph capture failed ({e}); timing eager launches\n")
+            torch.cuda.synchronize()
+    run = graph.replay if graph is not None else step
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        run()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        run()
+    e1.record()
+    barrier()
+    t1 = time.perf_counter()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist)
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    ms_per_step = ms / args.steps
+    value = job_throughput(samples, world, ms_per_step * 1e-3)
+
+    # ---- per-kernel-class times, live, same K steps launched eagerly with event brackets -----------------
+    st.profile(True)
+    torch.cuda.synchronize()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    for _ in range(args.steps):
+        step()
+    p1.record()
+    torch.cuda.synchronize()
+    prof = st.profile_read()
+    st.profile(False)
+    eager_ms = p0.elapsed_time(p1) / args.steps
+
+    # ---- end to end through the public API with HOST buffers -----------------------------------------------
+    host = []
+    for mb in data["microbatches"]:
+        h = {}
+        for k, v in mb.items():
+            if k == "t":
+                h[k] = torch.as_tensor(v).pin_memory()
+            else:       # NHWC in the stage dtype, pinned
+                h[k] = torch.as_tensor(np.ascontiguousarray(np.transpose(v, (0, 2, 3, 1)))).to(st.tdtype).pin_memory()
+        host.append(h)
+    h2d = sum(v.numel() * v.element_size() for h in host for v in h.values())
+    loss_host = torch.zeros(1, dtype=torch.float32).pin_memory()
+
+    def e2e_step():
+        for m in range(M):
+            for k, v in host[m].items():
+                devs[m][k].copy_(v, non_blocking=True)
+        run()
+        loss_host.copy_(loss, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        return float(loss_host[0])
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(args.steps):
+        last_loss = e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - w0) / args.steps
+    e2e_s = max_over_ranks(e2e_s, dist)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    tf_peak = peaks.get("bf16_tflops_sustained") or 1400.0
+    hbm_peak = peaks.get("hbm_gbs") or 6650.0
+    peak_src = "measured (MEASURED_PEAKS.json, sustained bf16 / copy)" if peaks else "fallback (B200_PROFILING.md)"
+    K = args.steps
+    kern = {}
+    for k, v in prof.items():
+        if v["launches"] == 0:
+            continue
+        row = {"ms_per_step": v["ms"] / K, "launches_per_step": v["launches"] / K}
+        if v["flops"]:
+            row["tflops"] = v["flops"] / (v["ms"] * 1e-3) / 1e12
+            row["frac_of_peak"] = row["tflops"] / tf_peak
+        if v["bytes"]:
+            row["gbs"] = v["bytes"] / (v["ms"] * 1e-3) / 1e9
+            row["frac_of_peak"] = row["gbs"] / hbm_peak
+        kern[k] = row
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"config{args.config}.conv_tc")
+    except Exception:
+        pass
+    dom = kern.get("conv_tc") or kern.get("conv_simt") or {}
+    roofline = {"kernel": "conv_tc_k (tcgen05 implicit-GEMM fprop+dgrad)" if "conv_tc" in kern else "conv_simt_k",
+                "bound": "tensor", "achieved": dom.get("tflops"), "peak": tf_peak, "unit": "TFLOP/s",
+                "frac": (dom.get("tflops") or 0.0) / tf_peak, "traffic": traffic, "peak_source": peak_src,
+                "share_of_step": (dom.get("ms_per_step") or 0.0) / eager_ms}
+    line = {"metric": METRIC, "value": value, "unit": "samples/s", "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16" if desc["dtype"] == "bf16" else "f32", "data": "synthetic (seeded N(0,1), DESIGN.md)",
+            "config": {"workload": WORKLOADS[args.config], "samples_per_step": samples, "microbatches": M,
+                       "l2": f"no flush: per-step working set {(st.stash_bytes * M + st.work_bytes + st.skip_bytes * M + st.param_bytes + st.grad_bytes) / 2**20:.0f} MiB > 126 MiB L2",
+                       "launch": "CUDA graph replay" if graph is not None else "eager launches",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "tflops": world * flops_step / (ms_per_step * 1e-3) / 1e12,
+            "frac_of_bf16_peak_nominal_2250": world * flops_step / (ms_per_step * 1e-3) / 1e12 / 2250.0 / world,
+            "frac_of_bf16_peak_measured": flops_step / (ms_per_step * 1e-3) / 1e12 / tf_peak,
+            "clocks": clocks, "gpu_launches": int(launches_per_step * K), "roofline": roofline,
+            "kernels": kern, "eager_ms_per_step": eager_ms, "loss": last_loss,
+            "e2e": {"value": world * samples / e2e_s, "unit": "samples/s", "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": 4, "ms_per_step": e2e_s * 1e3},
+            "peak_skip_cache_bytes": st.cache_stats()["peak_bytes"]}
+    if world == 1 and not args.no_cpu_baseline:
+        d1, note = reference_sample(desc, full=True)
+        line["cpu_baseline"] = {k: v for k, v in oracle_time(d1, W.draw(d1, 0), note).items() if k != "seconds"}
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

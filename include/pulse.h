@@ -173,6 +173,18 @@ pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const void* d_src0,
                                   int n, int h, int w, int ksize, int stride, const void* d_g, int cout,
                                   float* d_dw, void* stream);
 
+/* ---- per-kernel-class timing (row d: measurement) -------------------------------------------
+ * With profiling enabled, forward/backward bracket every kernel of these classes with CUDA events
+ * on the caller's stream: 0 tcgen05 conv (fprop+dgrad), 1 tcgen05 wgrad, 2 CUDA-core conv/wgrad,
+ * 3 GroupNorm+SiLU forward, 4 GroupNorm+SiLU backward, 5 everything else.  pulse_stage_profile_read
+ * synchronises those events and returns, per class, total milliseconds, launches, algorithmic FLOPs
+ * (2*M*N*K of the convs) and algorithmic bytes, then clears the records. */
+enum { PULSE_KCLASS_CONV_TC = 0, PULSE_KCLASS_WGRAD_TC = 1, PULSE_KCLASS_CONV_SIMT = 2, PULSE_KCLASS_GN_FWD = 3,
+       PULSE_KCLASS_GN_BWD = 4, PULSE_KCLASS_OTHER = 5, PULSE_KCLASS_COUNT = 6 };
+pulse_status_t pulse_stage_profile(pulse_stage_t* stage, int enable);
+pulse_status_t pulse_stage_profile_read(pulse_stage_t* stage, double ms[6], uint64_t launches[6], double flops[6],
+                                        double bytes[6]);
+
 /* Number of kernels this handle has launched so far (bench.py "gpu_launches"). */
 pulse_status_t pulse_stage_launch_count(const pulse_stage_t* stage, uint64_t* launches);
 

@@ -64,6 +64,9 @@ _SIG = {
     "pulse_temb_backward": [_vp, _vp, _vp, C.c_int, _vp],
     "pulse_mse_fwd_bwd": [C.c_int, _vp, _vp, _sz, C.c_float, _vp, _vp, _vp],
     "pulse_stage_launch_count": [_vp, C.POINTER(C.c_uint64)],
+    "pulse_stage_profile": [_vp, C.c_int],
+    "pulse_stage_profile_read": [_vp, C.POINTER(C.c_double * 6), C.POINTER(C.c_uint64 * 6), C.POINTER(C.c_double * 6),
+                                 C.POINTER(C.c_double * 6)],
     "pulse_conv2d": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp,
                      C.c_int, _vp, _vp, _vp, _vp, _vp],
     "pulse_conv2d_dgrad": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int,
@@ -276,6 +279,16 @@ class Stage:
         n = C.c_uint64()
         _ck(lib.pulse_stage_launch_count(self.h, C.byref(n)))
         return n.value
+
+    KCLASSES = ["conv_tc", "wgrad_tc", "conv_simt", "gn_fwd", "gn_bwd", "other"]
+
+    def profile(self, enable: bool):
+        _ck(lib.pulse_stage_profile(self.h, int(enable)))
+
+    def profile_read(self) -> dict:
+        ms, ln, fl, by = (C.c_double * 6)(), (C.c_uint64 * 6)(), (C.c_double * 6)(), (C.c_double * 6)()
+        _ck(lib.pulse_stage_profile_read(self.h, C.byref(ms), C.byref(ln), C.byref(fl), C.byref(by)))
+        return {k: {"ms": ms[i], "launches": ln[i], "flops": fl[i], "bytes": by[i]} for i, k in enumerate(self.KCLASSES)}
 
     # ---- one microbatch, device-resident inputs (what bench.py times) -------------------------
     def step(self, mb_id, dev, loss_scale=1.0, accumulate=False, loss=None, g_temb=None):

@@ -28,13 +28,57 @@ struct Ctx {
   bool tc() const { return dt == DT_BF16 && !(s->d.flags & PULSE_FLAG_FORCE_SIMT); }
 };
 
+// profiling span around a group of launches of one kernel class
+struct Prof {
+  pulse_stage* s; cudaStream_t st; int idx = -1; uint64_t l0;
+  Prof(pulse_stage* s_, cudaStream_t st_, int klass, double flops, double bytes) : s(s_), st(st_), l0(s_->launches) {
+    if (!s->profiling) return;
+    cudaEvent_t ev[2];
+    for (int i = 0; i < 2; ++i) {
+      if (!s->event_pool.empty()) { ev[i] = s->event_pool.back(); s->event_pool.pop_back(); }
+      else if (cudaEventCreate(&ev[i]) != cudaSuccess) return;
+    }
+    cudaEventRecord(ev[0], st);
+    s->spans.push_back({klass, ev[0], ev[1], flops, bytes, 0});
+    idx = (int)s->spans.size() - 1;
+  }
+  ~Prof() {
+    if (idx < 0) return;
+    cudaEventRecord(s->spans[idx].e1, st);
+    s->spans[idx].launches = (int)(s->launches - l0);
+  }
+};
+
+double conv_flops(const ConvArgs& a) {
+  const double mpix = a.mode == CONV_DGRAD_S2 ? (double)a.n * a.hin * a.win : (double)a.n * a.hout * a.wout;
+  return 2.0 * mpix * a.cout * a.src.c() * a.ksize * a.ksize;     // the s2 dgrad phases execute exactly 9/4 taps per output
+}
 void run_conv(Ctx& c, const ConvArgs& a) {
-  const int r = (c.tc() && conv_tc_supported(a)) ? conv_tc(a, c.st) : conv_simt(a, c.st);
+  const bool tc = c.tc() && conv_tc_supported(a);
+  Prof pr(c.s, c.st, tc ? PULSE_KCLASS_CONV_TC : PULSE_KCLASS_CONV_SIMT, conv_flops(a), 0.0);
+  const int r = tc ? conv_tc(a, c.st) : conv_simt(a, c.st);
   if (r < 0) c.err = true; else c.s->launches += r;
 }
 void run_wgrad(Ctx& c, const WgradArgs& a) {
-  const int r = (c.tc() && wgrad_tc_supported(a)) ? wgrad_tc(a, c.st) : wgrad_simt(a, c.st);
+  const bool tc = c.tc() && wgrad_tc_supported(a);
+  Prof pr(c.s, c.st, tc ? PULSE_KCLASS_WGRAD_TC : PULSE_KCLASS_CONV_SIMT,
+          2.0 * a.n * a.hout * a.wout * a.cout * a.src.c() * a.ksize * a.ksize, 0.0);
+  const int r = tc ? wgrad_tc(a, c.st) : wgrad_simt(a, c.st);
   if (r < 0) c.err = true; else c.s->launches += r;
+}
+// GroupNorm+SiLU wrappers: algorithmic bytes 2 x esz per element forward, 3 x esz backward
+void run_gn_fwd(Ctx& c, Cat x, int hw, const void* gamma, const void* beta, void* a_out, float* stats) {
+  pulse_stage* s = c.s;
+  Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 2.0 * s->esz() * s->d.n * hw * x.c());
+  s->launches += gn_silu_fwd(c.dt, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, a_out, stats,
+                             (float*)(c.work + s->w_partial), c.st);
+}
+void run_gn_bwd(Ctx& c, const void* g_a, Cat x, int hw, const void* gamma, const float* stats, const void* add,
+                void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta) {
+  pulse_stage* s = c.s;
+  Prof pr(s, c.st, PULSE_KCLASS_GN_BWD, 0.0, (3.0 + (add ? 1.0 : 0.0)) * s->esz() * s->d.n * hw * x.c());
+  s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, gamma, stats, add, dst0, dc0, acc0, dst1, acc1,
+                             dgamma, dbeta, (float*)(c.work + s->w_partial), (float*)(c.work + s->w_coef), c.st);
 }
 
 ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, int k, int stride, const void* w,
@@ -66,15 +110,13 @@ void resblock_forward(Ctx& c, const OpPlan& op, const float* emb) {
   float* stats1 = (float*)(c.stash + op.stats1);
   float* stats2 = (float*)(c.stash + op.stats2);
   float* pn = (float*)(c.stash + op.pn);
-  s->launches += gn_silu_fwd(c.dt, x, n, hw, s->d.groups, s->d.eps, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]),
-                             c.fwd(op.a1), stats1, partial, c.st);
+  run_gn_fwd(c, x, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1), stats1);
   s->launches += linear_fwd(c.dt, emb, n, T, op.cout, c.par(op.p[P_TW]), c.par(op.p[P_TB]), 1, pn, c.st);
   Cat a1{c.fwd(op.a1), ctot, nullptr, 0};
   run_conv(c, conv_args(c, a1, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C1W]), op.cout,
                         c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)));
   Cat h1{c.fwd(op.h1), op.cout, nullptr, 0};
-  s->launches += gn_silu_fwd(c.dt, h1, n, hw, s->d.groups, s->d.eps, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
-                             c.fwd(op.a2), stats2, partial, c.st);
+  run_gn_fwd(c, h1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2), stats2);
   const void* res = c.fwd(op.x0);
   if (op.p[P_SCW] >= 0) {
     run_conv(c, conv_args(c, x, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_SCW]), op.cout,
@@ -107,9 +149,9 @@ void resblock_backward(Ctx& c, const OpPlan& op, const float* emb, float* g_temb
   run_wgrad(c, w2);
   run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C2W]), 3, op.cout, g_a2, 0, 1, op.hin, op.win);
   // GN2 + SiLU backward -> g_h1
-  s->launches += gn_silu_bwd(c.dt, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, n, hw, s->d.groups,
-                             c.par(op.p[P_GN2G]), (const float*)(c.stash + op.stats2), nullptr, g_h1, op.cout, 0,
-                             nullptr, 0, c.pgrad(op.p[P_GN2G]), c.pgrad(op.p[P_GN2B]), partial, coef, c.st);
+  run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, hw, c.par(op.p[P_GN2G]),
+             (const float*)(c.stash + op.stats2), nullptr, g_h1, op.cout, 0, nullptr, 0, c.pgrad(op.p[P_GN2G]),
+             c.pgrad(op.p[P_GN2B]));
   // temb projection: g_p[n,c] = sum_hw g_h1; conv1 bias grad = sum_n g_p
   s->launches += colsum(c.dt, g_h1, n, hw, op.cout, gp, c.pgrad(op.p[P_C1B]), partial, c.st);
   s->launches += linear_bwd(c.dt, emb, gp, n, T, op.cout, c.par(op.p[P_TW]), 1, c.pgrad(op.p[P_TW]),
@@ -128,10 +170,8 @@ void resblock_backward(Ctx& c, const OpPlan& op, const float* emb, float* g_temb
     add = g_sc;
   }
   // GN1 + SiLU backward, split into g_h and g_skip (skip gradient accumulated locally)
-  s->launches += gn_silu_bwd(c.dt, g_a1, x, n, hw, s->d.groups, c.par(op.p[P_GN1G]),
-                             (const float*)(c.stash + op.stats1), add, c.grad(op.x0), op.cin, op.acc_x0,
-                             op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]),
-                             c.pgrad(op.p[P_GN1B]), partial, coef, c.st);
+  run_gn_bwd(c, g_a1, x, hw, c.par(op.p[P_GN1G]), (const float*)(c.stash + op.stats1), add, c.grad(op.x0), op.cin,
+             op.acc_x0, op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]));
 }
 
 pulse_status_t check_bound(pulse_stage* s, pulse_skip_cache* cache) {
@@ -188,9 +228,8 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
         break;
       }
       case PULSE_OP_HEAD: {
-        s->launches += gn_silu_fwd(c.dt, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, s->d.n, op.hin * op.win, s->d.groups,
-                                   s->d.eps, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1),
-                                   (float*)(c.stash + op.stats1), (float*)(c.work + s->w_partial), c.st);
+        run_gn_fwd(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin * op.win, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]),
+                   c.fwd(op.a1), (float*)(c.stash + op.stats1));
         run_conv(c, conv_args(c, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, op.hin, op.win, op.hin, op.win, 3, 1,
                               c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
         break;
@@ -272,10 +311,9 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
                     c.pgrad(op.p[P_C1W])};
         run_wgrad(c, w);
         run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C1W]), 3, op.cin, g_a, 0, 1, op.hin, op.win);
-        s->launches += gn_silu_bwd(c.dt, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, n, op.hin * op.win, s->d.groups,
-                                   c.par(op.p[P_GN1G]), (const float*)(c.stash + op.stats1), nullptr, c.grad(op.x0),
-                                   op.cin, 0, nullptr, 0, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]), partial,
-                                   (float*)(c.work + s->w_coef), c.st);
+        run_gn_bwd(c, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin * op.win, c.par(op.p[P_GN1G]),
+                   (const float*)(c.stash + op.stats1), nullptr, c.grad(op.x0), op.cin, 0, nullptr, 0,
+                   c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]));
         break;
       }
     }
@@ -342,6 +380,27 @@ extern "C" pulse_status_t pulse_mse_fwd_bwd(int dtype, const void* d_d, const vo
   if (numel == 0 || numel % V) return fail(PULSE_ERR_SHAPE, "numel must be a positive multiple of %d", V);
   mse_fwd_bwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_d, d_target, numel, scale, d_loss, d_g_d, (cudaStream_t)stream);
   CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+
+// ------------------------------------------------------------------------------ profiling
+extern "C" pulse_status_t pulse_stage_profile(pulse_stage_t* s, int enable) {
+  if (!s) return fail(PULSE_ERR_INVALID_ARG, "null stage");
+  s->profiling = enable != 0;
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_stage_profile_read(pulse_stage_t* s, double ms[6], uint64_t launches[6], double flops[6],
+                                                   double bytes[6]) {
+  if (!s || !ms || !launches || !flops || !bytes) return fail(PULSE_ERR_INVALID_ARG, "null argument");
+  for (int i = 0; i < PULSE_KCLASS_COUNT; ++i) { ms[i] = 0; launches[i] = 0; flops[i] = 0; bytes[i] = 0; }
+  for (auto& sp : s->spans) {
+    CK_CUDA(cudaEventSynchronize(sp.e1));
+    float t = 0.f;
+    CK_CUDA(cudaEventElapsedTime(&t, sp.e0, sp.e1));
+    ms[sp.klass] += t; launches[sp.klass] += sp.launches; flops[sp.klass] += sp.flops; bytes[sp.klass] += sp.bytes;
+    s->event_pool.push_back(sp.e0); s->event_pool.push_back(sp.e1);
+  }
+  s->spans.clear();
   return PULSE_OK;
 }
 

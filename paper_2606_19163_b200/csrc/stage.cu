@@ -255,6 +255,10 @@ extern "C" pulse_status_t pulse_stage_create(const pulse_stage_desc* desc, pulse
   return PULSE_OK;
 }
 extern "C" pulse_status_t pulse_stage_destroy(pulse_stage_t* s) {
+  if (s) {
+    for (auto& sp : s->spans) { cudaEventDestroy(sp.e0); cudaEventDestroy(sp.e1); }
+    for (auto ev : s->event_pool) cudaEventDestroy(ev);
+  }
   delete s;
   return PULSE_OK;
 }

@@ -71,6 +71,11 @@ struct pulse_stage {
   const char* d_params = nullptr; float* d_grads = nullptr;
   char* d_work = nullptr; size_t work_bound = 0;
   uint64_t launches = 0;
+  // profiling (pulse_stage_profile): event pairs per kernel-class span
+  struct Span { int klass; cudaEvent_t e0, e1; double flops, bytes; int launches; };
+  bool profiling = false;
+  std::vector<Span> spans;
+  std::vector<cudaEvent_t> event_pool;
   size_t esz() const { return d.dtype == PULSE_F32 ? 4 : 2; }
 };
 
