@@ -67,18 +67,19 @@ void run_wgrad(Ctx& c, const WgradArgs& a) {
   if (r < 0) c.err = true; else c.s->launches += r;
 }
 // GroupNorm+SiLU wrappers: algorithmic bytes 2 x esz per element forward, 3 x esz backward
-void run_gn_fwd(Ctx& c, Cat x, int hw, const void* gamma, const void* beta, void* a_out, float* stats) {
+void run_gn_fwd(Ctx& c, Cat x, int hw, const void* gamma, const void* beta, void* a_out, size_t site) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 2.0 * s->esz() * s->d.n * hw * x.c());
-  s->launches += gn_silu_fwd(c.dt, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, a_out, stats,
-                             (float*)(c.work + s->w_partial), c.st);
+  s->launches += gn_silu_fwd(c.dt, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, a_out,
+                             (double*)(c.stash + s->gn_off + site), (float*)(c.work + s->w_partial), c.st);
 }
-void run_gn_bwd(Ctx& c, const void* g_a, Cat x, int hw, const void* gamma, const float* stats, const void* add,
-                void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta) {
+void run_gn_bwd(Ctx& c, const void* g_a, Cat x, int hw, const void* gamma, const void* beta, size_t site,
+                const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_BWD, 0.0, (3.0 + (add ? 1.0 : 0.0)) * s->esz() * s->d.n * hw * x.c());
-  s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, gamma, stats, add, dst0, dc0, acc0, dst1, acc1,
-                             dgamma, dbeta, (float*)(c.work + s->w_partial), (float*)(c.work + s->w_coef), c.st);
+  s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta,
+                             (const double*)(c.stash + s->gn_off + site), add, dst0, dc0, acc0, dst1, acc1, dgamma,
+                             dbeta, (float*)(c.work + s->w_partial), c.st);
 }
 
 ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, int k, int stride, const void* w,
@@ -107,16 +108,14 @@ void resblock_forward(Ctx& c, const OpPlan& op, const float* emb) {
   const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip, T = s->d.temb_dim;
   Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
   float* partial = (float*)(c.work + s->w_partial);
-  float* stats1 = (float*)(c.stash + op.stats1);
-  float* stats2 = (float*)(c.stash + op.stats2);
   float* pn = (float*)(c.stash + op.pn);
-  run_gn_fwd(c, x, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1), stats1);
+  run_gn_fwd(c, x, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1), op.stats1);
   s->launches += linear_fwd(c.dt, emb, n, T, op.cout, c.par(op.p[P_TW]), c.par(op.p[P_TB]), 1, pn, c.st);
   Cat a1{c.fwd(op.a1), ctot, nullptr, 0};
   run_conv(c, conv_args(c, a1, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C1W]), op.cout,
                         c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)));
   Cat h1{c.fwd(op.h1), op.cout, nullptr, 0};
-  run_gn_fwd(c, h1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2), stats2);
+  run_gn_fwd(c, h1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2), op.stats2);
   const void* res = c.fwd(op.x0);
   if (op.p[P_SCW] >= 0) {
     run_conv(c, conv_args(c, x, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_SCW]), op.cout,
@@ -134,7 +133,6 @@ void resblock_backward(Ctx& c, const OpPlan& op, const float* emb, float* g_temb
   const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip, T = s->d.temb_dim;
   Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
   float* partial = (float*)(c.work + s->w_partial);
-  float* coef = (float*)(c.work + s->w_coef);
   float* gp = (float*)(c.work + s->w_gp);
   char* g_out = c.grad(op.out);
   char* g_a2 = c.work + s->w_ga2;
@@ -142,15 +140,15 @@ void resblock_backward(Ctx& c, const OpPlan& op, const float* emb, float* g_temb
   char* g_a1 = c.work + s->w_ga1;
   char* g_sc = c.work + s->w_gsc;
   // conv2: bias grad, wgrad, dgrad
-  s->launches += colsum(c.dt, g_out, n, hw, op.cout, nullptr, c.pgrad(op.p[P_C2B]), partial, c.st);
-  if (op.p[P_SCB] >= 0) s->launches += colsum(c.dt, g_out, n, hw, op.cout, nullptr, c.pgrad(op.p[P_SCB]), partial, c.st);
+  s->launches += colsum(c.dt, g_out, n, hw, op.cout, nullptr, c.pgrad(op.p[P_C2B]), partial, c.st,
+                        op.p[P_SCB] >= 0 ? c.pgrad(op.p[P_SCB]) : nullptr);
   WgradArgs w2{c.dt, Cat{c.fwd(op.a2), op.cout, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
                c.pgrad(op.p[P_C2W])};
   run_wgrad(c, w2);
   run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C2W]), 3, op.cout, g_a2, 0, 1, op.hin, op.win);
   // GN2 + SiLU backward -> g_h1
-  run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, hw, c.par(op.p[P_GN2G]),
-             (const float*)(c.stash + op.stats2), nullptr, g_h1, op.cout, 0, nullptr, 0, c.pgrad(op.p[P_GN2G]),
+  run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
+             op.stats2, nullptr, g_h1, op.cout, 0, nullptr, 0, c.pgrad(op.p[P_GN2G]),
              c.pgrad(op.p[P_GN2B]));
   // temb projection: g_p[n,c] = sum_hw g_h1; conv1 bias grad = sum_n g_p
   s->launches += colsum(c.dt, g_h1, n, hw, op.cout, gp, c.pgrad(op.p[P_C1B]), partial, c.st);
@@ -170,7 +168,7 @@ void resblock_backward(Ctx& c, const OpPlan& op, const float* emb, float* g_temb
     add = g_sc;
   }
   // GN1 + SiLU backward, split into g_h and g_skip (skip gradient accumulated locally)
-  run_gn_bwd(c, g_a1, x, hw, c.par(op.p[P_GN1G]), (const float*)(c.stash + op.stats1), add, c.grad(op.x0), op.cin,
+  run_gn_bwd(c, g_a1, x, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.stats1, add, c.grad(op.x0), op.cin,
              op.acc_x0, op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]));
 }
 
@@ -229,7 +227,7 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
       }
       case PULSE_OP_HEAD: {
         run_gn_fwd(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin * op.win, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]),
-                   c.fwd(op.a1), (float*)(c.stash + op.stats1));
+                   c.fwd(op.a1), op.stats1);
         run_conv(c, conv_args(c, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, op.hin, op.win, op.hin, op.win, 3, 1,
                               c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
         break;
@@ -312,7 +310,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
         run_wgrad(c, w);
         run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C1W]), 3, op.cin, g_a, 0, 1, op.hin, op.win);
         run_gn_bwd(c, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin * op.win, c.par(op.p[P_GN1G]),
-                   (const float*)(c.stash + op.stats1), nullptr, c.grad(op.x0), op.cin, 0, nullptr, 0,
+                   c.par(op.p[P_GN1B]), op.stats1, nullptr, c.grad(op.x0), op.cin, 0, nullptr, 0,
                    c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]));
         break;
       }

@@ -22,20 +22,21 @@ struct Cat {
 struct GnPlan { int nchunks, tpr, rows; };
 GnPlan gn_plan(int dt, int hw, int c, int n);
 size_t gn_partial_elems(const GnPlan& p, int n, int c);   // floats of scratch for partial sums
-// stats: [N][4][C] fp32 = {scale = r*gamma, shift = beta - mu*r*gamma, r, mu*r}
+// gsum: [N][G][2] doubles (sum, sum of squares per group), written by the forward, read by the backward.
+// partial: gn_partial_elems() floats of scratch (per-CTA partial sums; no atomics, no zeroing needed).
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                void* a_out, float* stats, float* partial, cudaStream_t st);
+                void* a_out, double* gsum, float* partial, cudaStream_t st);
 // g_x = r(gamma g_y - A - xhat B) [+ add]; channels [0,dc0) -> dst0, rest -> dst1; accX: += instead of =
-// dgamma/dbeta: fp32, atomically accumulated.  coef: [N][2][C] fp32 scratch.
-int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, const void* gamma,
-                const float* stats, const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1,
-                float* dgamma, float* dbeta, float* partial, float* coef, cudaStream_t st);
+// dgamma/dbeta: fp32, += (each channel owned by one CTA).  groups <= 64.
+int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
+                const void* beta, const double* gsum, const void* add, void* dst0, int dc0, int acc0, void* dst1,
+                int acc1, float* dgamma, float* dbeta, float* partial, cudaStream_t st);
 
 // ---- small ops -----------------------------------------------------------------------
 // s[n][c] = sum over pixels of g[n][hw][c];  out_n[n][c] = s (if non-null);
 // out_tot[c] += sum_n s (if non-null)
 int colsum(int dt, const void* g, int n, int hw, int c, float* out_n, float* out_tot, float* partial,
-           cudaStream_t st);
+           cudaStream_t st, float* out_tot2 = nullptr);
 size_t colsum_partial_elems(int dt, int n, int hw, int c);
 // out[n][o] = sum_i W[o][i] f(in[n][i]) + b[o]; f = SiLU if silu_in.  W,b in dtype dt; in/out fp32
 int linear_fwd(int dt, const float* in, int n, int din, int dout, const void* w, const void* b, int silu_in,

@@ -13,9 +13,9 @@ static void colsum_plan(int dt, int n, int hw, int c, int& tpr, int& rows, int& 
   tpr = c / vec;
   rows = tpr >= 256 ? 1 : 256 / tpr;
   if (rows > hw) rows = hw;
-  int maxc = hw / (rows * 4);
+  int maxc = hw / (rows * 8);
   if (maxc < 1) maxc = 1;
-  int want = (592 + n - 1) / n;
+  int want = (296 + n - 1) / n;
   nchunks = want < maxc ? want : maxc;
 }
 size_t colsum_partial_elems(int dt, int n, int hw, int c) {
@@ -24,8 +24,9 @@ size_t colsum_partial_elems(int dt, int n, int hw, int c) {
   return (size_t)n * nchunks * c;
 }
 
+// per-CTA partial column sums partial[n][chunk][C] (no same-address atomics across hundreds of CTAs)
 template <typename T>
-__global__ void colsum_partial_k(const T* __restrict__ g, int hw, int C, float* __restrict__ partial) {
+__global__ void __launch_bounds__(512) colsum_k(const T* __restrict__ g, int hw, int C, float* __restrict__ partial) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm[];
   const int n = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x;
@@ -35,11 +36,20 @@ __global__ void colsum_partial_k(const T* __restrict__ g, int hw, int C, float* 
   float s[V];
 #pragma unroll
   for (int i = 0; i < V; ++i) s[i] = 0.f;
-  for (int p = pb + ty; p < pe; p += rows) {
-    float v[V];
-    ldv(g + ((size_t)n * hw + p) * C + ch, v);
+  for (int p = pb + ty; p < pe; p += 4 * rows) {
+    float v[4][V];
 #pragma unroll
-    for (int i = 0; i < V; ++i) s[i] += v[i];
+    for (int u = 0; u < 4; ++u) {
+      if (p + u * rows < pe) ldv(g + ((size_t)n * hw + p + u * rows) * C + ch, v[u]);
+      else {
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[u][i] = 0.f;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int i = 0; i < V; ++i) s[i] += v[u][i];
   }
   if (rows > 1) {
 #pragma unroll
@@ -61,23 +71,30 @@ __global__ void colsum_partial_k(const T* __restrict__ g, int hw, int C, float* 
   }
 }
 
-__global__ void colsum_finalize_k(const float* __restrict__ partial, int n, int nchunks, int C, float* out_n,
-                                  float* out_tot) {
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= C) return;
-  float tot = 0.f;
-  for (int nn = 0; nn < n; ++nn) {
-    float s = 0.f;
-    for (int k = 0; k < nchunks; ++k) s += partial[((size_t)nn * nchunks + k) * C + c];
-    if (out_n) out_n[(size_t)nn * C + c] = s;
-    tot += s;
+// block (32 channels x 8 row slices) per (channel tile, image): out_n[n][c] = sum over chunks; out_tot[c] += it
+__global__ void colsum_finalize_k(const float* __restrict__ partial, int nchunks, int C, float* out_n, float* out_tot,
+                                  float* out_tot2) {
+  __shared__ float sm[8][33];
+  const int c = blockIdx.x * 32 + threadIdx.x, n = blockIdx.y;
+  float s = 0.f;
+  if (c < C)
+    for (int k = threadIdx.y; k < nchunks; k += 8) s += partial[((size_t)n * nchunks + k) * C + c];
+  sm[threadIdx.y][threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.y == 0 && c < C) {
+    float t = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t += sm[k][threadIdx.x];
+    if (out_n) out_n[(size_t)n * C + c] = t;
+    if (out_tot) atomicAdd(out_tot + c, t);      // <= N-way
+    if (out_tot2) atomicAdd(out_tot2 + c, t);
   }
-  if (out_tot) out_tot[c] += tot;
 }
 
 // any C (used for Cout = 4): one block per channel
 template <typename T>
-__global__ void colsum_scalar_k(const T* __restrict__ g, int n, int hw, int C, float* out_n, float* out_tot) {
+__global__ void colsum_scalar_k(const T* __restrict__ g, int n, int hw, int C, float* out_n, float* out_tot,
+                                float* out_tot2) {
   const int c = blockIdx.x;
   __shared__ float sh[32];
   float tot = 0.f;
@@ -96,28 +113,29 @@ __global__ void colsum_scalar_k(const T* __restrict__ g, int n, int hw, int C, f
     __syncthreads();
   }
   if (threadIdx.x == 0 && out_tot) out_tot[c] += tot;
+  if (threadIdx.x == 0 && out_tot2) out_tot2[c] += tot;
 }
 
 int colsum(int dt, const void* g, int n, int hw, int c, float* out_n, float* out_tot, float* partial,
-           cudaStream_t st) {
+           cudaStream_t st, float* out_tot2) {
   const int vec = dt == DT_F32 ? 4 : 8;
-  if (c % vec) {
-    if (dt == DT_F32) colsum_scalar_k<float><<<c, 256, 0, st>>>((const float*)g, n, hw, c, out_n, out_tot);
-    else colsum_scalar_k<bf16><<<c, 256, 0, st>>>((const bf16*)g, n, hw, c, out_n, out_tot);
+  if (c % vec || c / vec > 512) {
+    if (dt == DT_F32) colsum_scalar_k<float><<<c, 256, 0, st>>>((const float*)g, n, hw, c, out_n, out_tot, out_tot2);
+    else colsum_scalar_k<bf16><<<c, 256, 0, st>>>((const bf16*)g, n, hw, c, out_n, out_tot, out_tot2);
     return 1;
   }
   int tpr, rows, nchunks;
   colsum_plan(dt, n, hw, c, tpr, rows, nchunks);
   dim3 grid(nchunks, n), block(tpr, rows);
   const size_t smem = rows > 1 ? (size_t)rows * c * sizeof(float) : 0;
-  if (dt == DT_F32) colsum_partial_k<float><<<grid, block, smem, st>>>((const float*)g, hw, c, partial);
-  else colsum_partial_k<bf16><<<grid, block, smem, st>>>((const bf16*)g, hw, c, partial);
-  colsum_finalize_k<<<(c + 127) / 128, 128, 0, st>>>(partial, n, nchunks, c, out_n, out_tot);
+  if (dt == DT_F32) colsum_k<float><<<grid, block, smem, st>>>((const float*)g, hw, c, partial);
+  else colsum_k<bf16><<<grid, block, smem, st>>>((const bf16*)g, hw, c, partial);
+  colsum_finalize_k<<<dim3((c + 31) / 32, n), dim3(32, 8), 0, st>>>(partial, nchunks, c, out_n, out_tot, out_tot2);
   return 2;
 }
 
 // ------------------------------------------------------------------ tiny linears (timestep path)
-// one warp per output feature o; lanes stride over the input dimension; all n rows at once
+// one warp per output feature o; each lane takes 8 consecutive inputs per step; all n (<= 8) rows at once
 template <typename T, int MAXN>
 __global__ void linear_fwd_k(const float* __restrict__ in, int n, int din, int dout, const T* __restrict__ w,
                              const T* __restrict__ b, int silu_in, float* __restrict__ out) {
@@ -126,15 +144,33 @@ __global__ void linear_fwd_k(const float* __restrict__ in, int n, int din, int d
   float acc[MAXN];
 #pragma unroll
   for (int j = 0; j < MAXN; ++j) acc[j] = 0.f;
-  for (int i = lane; i < din; i += 32) {
-    const float wv = to_f(w[(size_t)o * din + i]);
+  const T* wr = w + (size_t)o * din;
+  if (din % 8 == 0) {
+    for (int i = lane * 8; i < din; i += 256) {
+      float wv[8];
 #pragma unroll
-    for (int j = 0; j < MAXN; ++j)
-      if (j < n) {
-        float x = in[(size_t)j * din + i];
-        if (silu_in) x = siluf_(x);
-        acc[j] = fmaf(wv, x, acc[j]);
-      }
+      for (int k = 0; k < 8; ++k) wv[k] = to_f(wr[i + k]);
+#pragma unroll
+      for (int j = 0; j < MAXN; ++j)
+        if (j < n) {
+          const float4 x0 = *reinterpret_cast<const float4*>(in + (size_t)j * din + i);
+          const float4 x1 = *reinterpret_cast<const float4*>(in + (size_t)j * din + i + 4);
+          float x[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+#pragma unroll
+          for (int k = 0; k < 8; ++k) acc[j] = fmaf(wv[k], silu_in ? siluf_(x[k]) : x[k], acc[j]);
+        }
+    }
+  } else {
+    for (int i = lane; i < din; i += 32) {
+      const float wv = to_f(wr[i]);
+#pragma unroll
+      for (int j = 0; j < MAXN; ++j)
+        if (j < n) {
+          float x = in[(size_t)j * din + i];
+          if (silu_in) x = siluf_(x);
+          acc[j] = fmaf(wv, x, acc[j]);
+        }
+    }
   }
 #pragma unroll
   for (int j = 0; j < MAXN; ++j) {
@@ -150,12 +186,12 @@ int linear_fwd(int dt, const float* in, int n, int din, int dout, const void* w,
   int launches = 0;
   for (int n0 = 0; n0 < n; n0 += 8) {       // N <= 8 in every config; larger N handled in slabs
     const int nn = n - n0 < 8 ? n - n0 : 8;
-    const int blocks = (dout * 32 + 255) / 256;
+    const int blocks = (dout * 32 + 127) / 128;
     if (dt == DT_F32)
-      linear_fwd_k<float, 8><<<blocks, 256, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const float*)w,
+      linear_fwd_k<float, 8><<<blocks, 128, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const float*)w,
                                                       (const float*)b, silu_in, out + (size_t)n0 * dout);
     else
-      linear_fwd_k<bf16, 8><<<blocks, 256, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const bf16*)w,
+      linear_fwd_k<bf16, 8><<<blocks, 128, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const bf16*)w,
                                                      (const bf16*)b, silu_in, out + (size_t)n0 * dout);
     ++launches;
   }
@@ -180,17 +216,25 @@ __global__ void linear_bwd_w_k(const float* __restrict__ in, const float* __rest
   if (i == 0 && db) db[o] += sb;
 }
 
-// g_in[n][i] (+)= (sum_o g[n][o] W[o][i]) f'(in[n][i])
+// g_in[n][i] += (sum_{o in chunk} g[n][o] W[o][i]) f'(in[n][i])   (atomic; caller zeroes g_in when it must not accumulate)
 template <typename T>
 __global__ void linear_bwd_in_k(const float* __restrict__ in, const float* __restrict__ g, int n, int din, int dout,
-                                const T* __restrict__ w, int silu_in, float* __restrict__ g_in, int acc) {
+                                const T* __restrict__ w, int silu_in, float* __restrict__ g_in, int ochunk) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= din) return;
-  float s = 0.f;
-  for (int o = 0; o < dout; ++o) s = fmaf(g[(size_t)j * dout + o], to_f(w[(size_t)o * din + i]), s);
+  const int o0 = blockIdx.z * ochunk, o1 = min(dout, o0 + ochunk);
+  float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+  int o = o0;
+  for (; o + 4 <= o1; o += 4) {
+    s0 = fmaf(g[(size_t)j * dout + o], to_f(w[(size_t)o * din + i]), s0);
+    s1 = fmaf(g[(size_t)j * dout + o + 1], to_f(w[(size_t)(o + 1) * din + i]), s1);
+    s2 = fmaf(g[(size_t)j * dout + o + 2], to_f(w[(size_t)(o + 2) * din + i]), s2);
+    s3 = fmaf(g[(size_t)j * dout + o + 3], to_f(w[(size_t)(o + 3) * din + i]), s3);
+  }
+  for (; o < o1; ++o) s0 = fmaf(g[(size_t)j * dout + o], to_f(w[(size_t)o * din + i]), s0);
+  float s = (s0 + s1) + (s2 + s3);
   if (silu_in) s *= silu_gradf_(in[(size_t)j * din + i]);
-  float* d = g_in + (size_t)j * din + i;
-  *d = acc ? *d + s : s;
+  atomicAdd(g_in + (size_t)j * din + i, s);
 }
 
 int linear_bwd(int dt, const float* in, const float* g, int n, int din, int dout, const void* w, int silu_in,
@@ -199,11 +243,13 @@ int linear_bwd(int dt, const float* in, const float* g, int n, int din, int dout
   const size_t tot = (size_t)din * dout;
   linear_bwd_w_k<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(in, g, n, din, dout, silu_in, dw, db);
   if (g_in) {
-    dim3 grid((din + 127) / 128, n);
+    if (!acc_g_in) cudaMemsetAsync(g_in, 0, (size_t)n * din * sizeof(float), st);
+    const int ochunk = 32;
+    dim3 grid((din + 127) / 128, n, (dout + ochunk - 1) / ochunk);
     if (dt == DT_F32)
-      linear_bwd_in_k<float><<<grid, 128, 0, st>>>(in, g, n, din, dout, (const float*)w, silu_in, g_in, acc_g_in);
+      linear_bwd_in_k<float><<<grid, 128, 0, st>>>(in, g, n, din, dout, (const float*)w, silu_in, g_in, ochunk);
     else
-      linear_bwd_in_k<bf16><<<grid, 128, 0, st>>>(in, g, n, din, dout, (const bf16*)w, silu_in, g_in, acc_g_in);
+      linear_bwd_in_k<bf16><<<grid, 128, 0, st>>>(in, g, n, din, dout, (const bf16*)w, silu_in, g_in, ochunk);
     ++launches;
   }
   return launches;

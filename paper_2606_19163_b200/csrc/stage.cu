@@ -76,7 +76,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
   const pulse_stage_desc& d = s->d;
   Planner pl; pl.s = s;
   const int G = d.groups, T = d.temb_dim, vec = d.dtype == PULSE_F32 ? 4 : 8;
-  auto chk_c = [&](int c, const char* what) -> bool { return c > 0 && c % G == 0 && c % vec == 0 && c / vec <= 1024; };
+  auto chk_c = [&](int c, const char* what) -> bool { return c > 0 && c % G == 0 && c % vec == 0 && c / vec <= 512; };
   if (d.temb_kind == PULSE_TEMB_MLP) {
     pl.param("temb.w1", 2, T, d.temb_d0); pl.param("temb.b1", 1, T);
     pl.param("temb.w2", 2, T, T); pl.param("temb.b2", 1, T);
@@ -85,6 +85,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
   }
   s->temb_grad_bytes = s->grad_bytes;
   if (d.temb_d0 % 2) return fail(PULSE_ERR_SHAPE, "temb_d0 must be even");
+  if (G > 64) return fail(PULSE_ERR_UNSUPPORTED, "at most 64 GroupNorm groups");
 
   std::vector<int> stack;
   int cur = pl.tensor(d.x_in_is_skip ? R_SKIP : R_STASH, d.c_in, d.h, d.w);
@@ -92,6 +93,8 @@ static pulse_status_t build_plan(pulse_stage* s) {
   if (d.x_in_is_skip) { s->skip_tensor.push_back(cur); stack.push_back(cur); }
   s->emb_off = pl.bump(R_STASH, (size_t)d.n * T * 4);
 
+  const size_t gsz = align256((size_t)d.n * G * 2 * sizeof(double));   // one GroupNorm site: [n][G][2] doubles
+  s->gn_site_bytes = gsz;
   size_t m_out = 0, m_cat = 0, m_gu = 0, m_w = 0, m_partial = 0, m_coef = 0, m_gp = 0;
   auto upd = [](size_t& m, size_t v) { if (v > m) m = v; };
   auto gn_site = [&](int c, int hw) {
@@ -141,8 +144,8 @@ static pulse_status_t build_plan(pulse_stage* s) {
         op.a1 = pl.tensor(R_STASH, ctot, op.hin, op.win, false);
         op.h1 = pl.tensor(R_STASH, o.cout, op.hin, op.win, false);
         op.a2 = pl.tensor(R_STASH, o.cout, op.hin, op.win, false);
-        op.stats1 = pl.bump(R_STASH, (size_t)d.n * 4 * ctot * 4);
-        op.stats2 = pl.bump(R_STASH, (size_t)d.n * 4 * o.cout * 4);
+        op.stats1 = (size_t)(s->gn_sites++) * gsz;
+        op.stats2 = (size_t)(s->gn_sites++) * gsz;
         op.pn = pl.bump(R_STASH, (size_t)d.n * o.cout * 4);
         upd(m_out, pix * o.cout * s->esz()); upd(m_cat, pix * ctot * s->esz());
         upd(m_w, (size_t)o.cout * 9 * (ctot > o.cout ? ctot : o.cout) * s->esz());
@@ -169,7 +172,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
         op.p[P_GN1G] = pl.param(pre + "gn.gamma", 1, o.cin); op.p[P_GN1B] = pl.param(pre + "gn.beta", 1, o.cin);
         op.p[P_C1W] = pl.param(pre + "conv.w", 4, o.cout, 3, 3, o.cin); op.p[P_C1B] = pl.param(pre + "conv.b", 1, o.cout);
         op.a1 = pl.tensor(R_STASH, o.cin, op.hin, op.win, false);
-        op.stats1 = pl.bump(R_STASH, (size_t)d.n * 4 * o.cin * 4);
+        op.stats1 = (size_t)(s->gn_sites++) * gsz;
         upd(m_cat, pix * o.cin * s->esz()); upd(m_w, (size_t)o.cout * 9 * o.cin * s->esz());
         gn_site(o.cin, op.hin * op.win); cs_site(o.cout, op.hin * op.win);
       } else {
@@ -221,6 +224,8 @@ static pulse_status_t build_plan(pulse_stage* s) {
       return fail(PULSE_ERR_UNSUPPORTED, "up/head input with a second consumer");
   }
 
+  s->gn_off = pl.bump(R_STASH, (size_t)s->gn_sites * gsz);
+  s->w_gb = pl.bump(R_WORK, (size_t)s->gn_sites * gsz);
   s->skip_bytes = pl.top[R_SKIP];
   s->stash_bytes = pl.top[R_STASH];
   s->w_ga2 = pl.bump(R_WORK, m_out); s->w_gh1 = pl.bump(R_WORK, m_out);

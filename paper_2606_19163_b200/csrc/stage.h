@@ -28,7 +28,8 @@ struct OpPlan {
   int hin, win, hout, wout;
   int x0 = -1, x1 = -1, out = -1;           // indices into Stage::tensors (activations)
   int a1 = -1, h1 = -1, a2 = -1, u = -1;    // stashed intermediates
-  size_t stats1 = 0, stats2 = 0, pn = 0;    // byte offsets in the slot stash (fp32 arrays)
+  size_t stats1 = 0, stats2 = 0;            // byte offsets of the GroupNorm sites inside the gn regions
+  size_t pn = 0;                            // byte offset in the slot stash ([n,cout] fp32)
   int p[12];                                // parameter indices (see stage.cu)
   int push = -1, pop = -1;
   // backward write modes decided at plan time (0: '=', 1: '+=')
@@ -65,6 +66,7 @@ struct pulse_stage {
   int t_xin = -1, t_hin = -1, t_eout = -1, t_dout = -1;
   size_t skip_bytes = 0, stash_bytes = 0, work_bytes = 0;
   size_t emb_off = 0;                       // slot stash: copy of temb [n,T] fp32
+  int gn_sites = 0; size_t gn_site_bytes = 0, gn_off = 0, w_gb = 0;   // GroupNorm group sums (stash) / backward sums (work)
   // per-stage workspace offsets (bytes)
   size_t w_ga2 = 0, w_gh1 = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_wt = 0, w_partial = 0, w_coef = 0, w_gp = 0,
          w_tmpf = 0;
