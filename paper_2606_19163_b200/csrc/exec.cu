@@ -2,6 +2,8 @@
 // walks the op plan and enqueues kernels.  Rows a1-a11 of SURVEY.md 8a.
 #include "stage.h"
 
+#include <cstring>
+
 using namespace pulse;
 
 namespace {
@@ -66,20 +68,35 @@ void run_wgrad(Ctx& c, const WgradArgs& a) {
   const int r = tc ? wgrad_tc(a, c.st) : wgrad_simt(a, c.st);
   if (r < 0) c.err = true; else c.s->launches += r;
 }
-// GroupNorm+SiLU wrappers: algorithmic bytes 2 x esz per element forward, 3 x esz backward (DESIGN.md)
-void run_gn_fwd(Ctx& c, Cat x, int hw, const void* gamma, const void* beta, void* a_out, size_t site) {
+// GroupNorm+SiLU wrappers: algorithmic bytes 2 x esz per element forward, 3 x esz backward (DESIGN.md sec. 5)
+float* cst_of(const Ctx& c, int t) { return t < 0 ? nullptr : (float*)(c.stash + c.s->tensors[t].cst); }
+float* cs_of(const Ctx& c, int t) {      // fused pixel sums of the gradient of tensor t, if its writers emit them
+  const Tensor& T = c.s->tensors[t];
+  return (T.is_out && T.cs_fused) ? (float*)(c.work + T.cs) : nullptr;
+}
+// channel stats of a freshly written tensor that a GroupNorm will read
+void run_stats(Ctx& c, int t) {
+  pulse_stage* s = c.s;
+  const Tensor& T = s->tensors[t];
+  if (!T.gn_input) return;
+  const int hw = T.ref.h * T.ref.w;
+  Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 0.0);      // its bytes are not algorithmic: counted as GroupNorm-forward time
+  s->launches += chan_stats(c.dt, c.fwd(t), s->d.n, hw, T.ref.c, cst_of(c, t), c.st);
+}
+void run_gn_fwd(Ctx& c, Cat x, int t0, int t1, int hw, const void* gamma, const void* beta, void* a_out) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 2.0 * s->esz() * s->d.n * hw * x.c());
-  s->launches += gn_silu_fwd(c.dt, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, a_out,
-                             (double*)(c.stash + s->gn_off + site), (float*)(c.work + s->w_partial), c.st);
+  s->launches += gn_silu_fwd(c.dt, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, cst_of(c, t0), cst_of(c, t1),
+                             a_out, c.st);
 }
-void run_gn_bwd(Ctx& c, const void* g_a, Cat x, int hw, const void* gamma, const void* beta, size_t site,
-                const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta) {
+void run_gn_bwd(Ctx& c, const void* g_a, Cat x, int t0, int t1, int hw, const void* gamma, const void* beta,
+                size_t bst, const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma,
+                float* dbeta, float* cs0, float* cs1) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_BWD, 0.0, (3.0 + (add ? 1.0 : 0.0)) * s->esz() * s->d.n * hw * x.c());
-  s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta,
-                             (const double*)(c.stash + s->gn_off + site), add, dst0, dc0, acc0, dst1, acc1, dgamma,
-                             dbeta, (float*)(c.work + s->w_partial), c.st);
+  s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, cst_of(c, t0),
+                             cst_of(c, t1), (float*)(c.work + bst), add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
+                             cs0, cs1, c.st);
 }
 
 ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, int k, int stride, const void* w,
@@ -91,31 +108,49 @@ ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, 
   return a;
 }
 
-// dgrad of a stride-1 conv == fprop with flipped/transposed weights
-void run_dgrad(Ctx& c, const void* g, int h, int w, int cout, const void* wts, int k, int cin, void* g_in,
+// dgrad of a conv == fprop with the flipped/transposed weights `wt`, which
+// prepare_weights() keeps in the workspace
+void run_dgrad(Ctx& c, const void* g, int h, int w, int cout, size_t wt_off, int k, int cin, void* g_in,
                int accumulate, int stride, int hin, int win) {
-  char* wt = c.work + c.s->w_wt;
-  c.s->launches += flip_transpose(c.dt, wts, cout, k, cin, wt, c.st);
   Cat src{g, cout, nullptr, 0};
-  ConvArgs a = conv_args(c, src, h, w, hin, win, k, 1, wt, cin, nullptr, nullptr, nullptr, g_in);
+  ConvArgs a = conv_args(c, src, h, w, hin, win, k, 1, c.work + wt_off, cin, nullptr, nullptr, nullptr, g_in);
   a.accumulate = accumulate;
   if (stride == 2) a.mode = CONV_DGRAD_S2;
   run_conv(c, a);
 }
 
-void resblock_forward(Ctx& c, const OpPlan& op, const float* emb) {
+// Wt[ci][k-1-r][k-1-s][co] = W[co][r][s][ci] for every conv of the stage, in one batched launch.  Redone at the
+// first backward of a step (accumulate_wgrad == 0), reused by the accumulating backwards of a wave (R21).
+void prepare_weights(Ctx& c) {
   pulse_stage* s = c.s;
-  const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip, T = s->d.temb_dim;
+  std::vector<TransposeEntry> e;
+  for (const OpPlan& op : s->ops) {
+    const int ctot = op.cin + op.cskip;
+    if (op.kind == PULSE_OP_RESBLOCK) {
+      e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, op.cout, 3, ctot});
+      e.push_back({c.par(op.p[P_C2W]), c.work + op.wt2, op.cout, 3, op.cout});
+      if (op.p[P_SCW] >= 0) e.push_back({c.par(op.p[P_SCW]), c.work + op.wtsc, op.cout, 1, ctot});
+    } else {
+      e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, op.cout, 3, op.cin});
+    }
+  }
+  Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
+  s->launches += flip_transpose_batch(c.dt, e.data(), (int)e.size(), c.st);
+  s->wt_valid = true;
+}
+
+void resblock_forward(Ctx& c, const OpPlan& op) {
+  pulse_stage* s = c.s;
+  const int hw = op.hin * op.win, ctot = op.cin + op.cskip;
   Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
-  float* partial = (float*)(c.work + s->w_partial);
   float* pn = (float*)(c.stash + op.pn);
-  run_gn_fwd(c, x, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1), op.stats1);
-  s->launches += linear_fwd(c.dt, emb, n, T, op.cout, c.par(op.p[P_TW]), c.par(op.p[P_TB]), 1, pn, c.st);
+  run_gn_fwd(c, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1));
   Cat a1{c.fwd(op.a1), ctot, nullptr, 0};
   run_conv(c, conv_args(c, a1, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C1W]), op.cout,
                         c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)));
+  run_stats(c, op.h1);
   Cat h1{c.fwd(op.h1), op.cout, nullptr, 0};
-  run_gn_fwd(c, h1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2), op.stats2);
+  run_gn_fwd(c, h1, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2));
   const void* res = c.fwd(op.x0);
   if (op.p[P_SCW] >= 0) {
     run_conv(c, conv_args(c, x, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_SCW]), op.cout,
@@ -125,51 +160,77 @@ void resblock_forward(Ctx& c, const OpPlan& op, const float* emb) {
   Cat a2{c.fwd(op.a2), op.cout, nullptr, 0};
   run_conv(c, conv_args(c, a2, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C2W]), op.cout,
                         c.par(op.p[P_C2B]), nullptr, res, c.fwd(op.out)));
-  (void)ctot;
+  run_stats(c, op.out);
 }
 
-void resblock_backward(Ctx& c, const OpPlan& op, const float* emb, float* g_temb) {
+// pixel sums of the gradient of an op's output, for its bias gradient: fused by the writers or one colsum pass
+void ensure_colsum(Ctx& c, int t) {
   pulse_stage* s = c.s;
-  const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip, T = s->d.temb_dim;
+  const Tensor& T = s->tensors[t];
+  if (T.cs_fused) return;
+  Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
+  s->launches += colsum(c.dt, c.grad(t), s->d.n, T.ref.h * T.ref.w, T.ref.c, (float*)(c.work + T.cs), c.st);
+}
+
+void resblock_backward(Ctx& c, const OpPlan& op) {
+  pulse_stage* s = c.s;
+  const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip;
   Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
-  float* partial = (float*)(c.work + s->w_partial);
-  float* gp = (float*)(c.work + s->w_gp);
   char* g_out = c.grad(op.out);
   char* g_a2 = c.work + s->w_ga2;
   char* g_h1 = c.work + s->w_gh1;
   char* g_a1 = c.work + s->w_ga1;
   char* g_sc = c.work + s->w_gsc;
-  // conv2: bias grad, wgrad, dgrad
-  s->launches += colsum(c.dt, g_out, n, hw, op.cout, nullptr, c.pgrad(op.p[P_C2B]), partial, c.st,
-                        op.p[P_SCB] >= 0 ? c.pgrad(op.p[P_SCB]) : nullptr);
+  ensure_colsum(c, op.out);
+  // conv2: wgrad, dgrad
   WgradArgs w2{c.dt, Cat{c.fwd(op.a2), op.cout, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
                c.pgrad(op.p[P_C2W])};
   run_wgrad(c, w2);
-  run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C2W]), 3, op.cout, g_a2, 0, 1, op.hin, op.win);
-  // GN2 + SiLU backward -> g_h1
-  run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
-             op.stats2, nullptr, g_h1, op.cout, 0, nullptr, 0, c.pgrad(op.p[P_GN2G]),
-             c.pgrad(op.p[P_GN2B]));
-  // temb projection: g_p[n,c] = sum_hw g_h1; conv1 bias grad = sum_n g_p
-  s->launches += colsum(c.dt, g_h1, n, hw, op.cout, gp, c.pgrad(op.p[P_C1B]), partial, c.st);
-  s->launches += linear_bwd(c.dt, emb, gp, n, T, op.cout, c.par(op.p[P_TW]), 1, c.pgrad(op.p[P_TW]),
-                            c.pgrad(op.p[P_TB]), g_temb, 1, c.st);
+  run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wt2, 3, op.cout, g_a2, 0, 1, op.hin, op.win);
+  // GN2 + SiLU backward -> g_h1, and its pixel sums g_p[n,c] (temb projection / conv1 bias gradients)
+  run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
+             op.bst2, nullptr, g_h1, op.cout, 0, nullptr, 0, c.pgrad(op.p[P_GN2G]), c.pgrad(op.p[P_GN2B]),
+             (float*)(c.work + op.gp), nullptr);
   // conv1: wgrad, dgrad
   WgradArgs w1{c.dt, Cat{c.fwd(op.a1), ctot, nullptr, 0}, n, op.hin, op.win, g_h1, op.hin, op.win, op.cout, 3, 1,
                c.pgrad(op.p[P_C1W])};
   run_wgrad(c, w1);
-  run_dgrad(c, g_h1, op.hin, op.win, op.cout, c.par(op.p[P_C1W]), 3, ctot, g_a1, 0, 1, op.hin, op.win);
+  run_dgrad(c, g_h1, op.hin, op.win, op.cout, op.wt1, 3, ctot, g_a1, 0, 1, op.hin, op.win);
   // shortcut
   const void* add = g_out;
   if (op.p[P_SCW] >= 0) {
     WgradArgs ws{c.dt, x, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 1, 1, c.pgrad(op.p[P_SCW])};
     run_wgrad(c, ws);
-    run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_SCW]), 1, ctot, g_sc, 0, 1, op.hin, op.win);
+    run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wtsc, 1, ctot, g_sc, 0, 1, op.hin, op.win);
     add = g_sc;
   }
   // GN1 + SiLU backward, split into g_h and g_skip (skip gradient accumulated locally)
-  run_gn_bwd(c, g_a1, x, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.stats1, add, c.grad(op.x0), op.cin,
-             op.acc_x0, op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]));
+  run_gn_bwd(c, g_a1, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.bst1, add, c.grad(op.x0), op.cin,
+             op.acc_x0, op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]),
+             cs_of(c, op.x0), op.x1 >= 0 ? cs_of(c, op.x1) : nullptr);
+}
+
+// bias / temb-projection gradients of every op from the pixel sums, in one batched launch (row a8-a10)
+void small_grads(Ctx& c, const float* emb, float* g_temb) {
+  pulse_stage* s = c.s;
+  std::vector<SmallGradEntry> e;
+  for (const OpPlan& op : s->ops) {
+    SmallGradEntry g;
+    memset(&g, 0, sizeof g);
+    g.cs_out = (const float*)(c.work + s->tensors[op.out].cs);
+    g.cout = op.cout;
+    if (op.kind == PULSE_OP_RESBLOCK) {
+      g.db_out = c.pgrad(op.p[P_C2B]);
+      g.db_out2 = op.p[P_SCB] >= 0 ? c.pgrad(op.p[P_SCB]) : nullptr;
+      g.gp = (const float*)(c.work + op.gp);
+      g.db1 = c.pgrad(op.p[P_C1B]); g.dtb = c.pgrad(op.p[P_TB]); g.dtw = c.pgrad(op.p[P_TW]); g.tw = c.par(op.p[P_TW]);
+    } else {
+      g.db_out = c.pgrad(op.p[P_C1B]);
+    }
+    e.push_back(g);
+  }
+  Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
+  s->launches += small_grads_batch(c.dt, emb, g_temb, s->d.n, s->d.temb_dim, e.data(), (int)e.size(), c.st);
 }
 
 pulse_status_t check_bound(pulse_stage* s, pulse_skip_cache* cache) {
@@ -203,31 +264,44 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
   float* emb = (float*)(c.stash + s->emb_off);
+  if (s->cst_end > s->cst_begin) CK_CUDA(cudaMemsetAsync(c.stash + s->cst_begin, 0, s->cst_end - s->cst_begin, c.st));
   CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
   if (open) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
+  run_stats(c, s->t_xin);
+  if (open) run_stats(c, s->t_hin);
+  {   // p[n,c] = Wt SiLU(emb) + bt of every ResBlock in one launch (row a1)
+    std::vector<ProjEntry> pe;
+    for (const OpPlan& op : s->ops)
+      if (op.kind == PULSE_OP_RESBLOCK)
+        pe.push_back({c.par(op.p[P_TW]), c.par(op.p[P_TB]), (float*)(c.stash + op.pn), op.cout});
+    if (!pe.empty()) {
+      Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
+      s->launches += temb_proj_batch(c.dt, emb, s->d.n, s->d.temb_dim, pe.data(), (int)pe.size(), c.st);
+    }
+  }
   for (size_t i = 0; i < s->ops.size(); ++i) {
     const OpPlan& op = s->ops[i];
-    if (open && (int)i == s->n_enc)   // decoder starts: the first decoder op reads h_in
-      ;
     switch (op.kind) {
-      case PULSE_OP_RESBLOCK: resblock_forward(c, op, emb); break;
+      case PULSE_OP_RESBLOCK: resblock_forward(c, op); break;
       case PULSE_OP_CONV_IN:
       case PULSE_OP_DOWN: {
         const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
         run_conv(c, conv_args(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin, op.win, op.hout, op.wout, 3, stride,
                               c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
+        run_stats(c, op.out);
         break;
       }
       case PULSE_OP_UP: {
         s->launches += upsample2(c.dt, c.fwd(op.x0), s->d.n, op.hin, op.win, op.cin, c.fwd(op.u), c.st);
         run_conv(c, conv_args(c, Cat{c.fwd(op.u), op.cin, nullptr, 0}, op.hout, op.wout, op.hout, op.wout, 3, 1,
                               c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
+        run_stats(c, op.out);
         break;
       }
       case PULSE_OP_HEAD: {
-        run_gn_fwd(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin * op.win, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]),
-                   c.fwd(op.a1), op.stats1);
+        run_gn_fwd(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.x0, -1, op.hin * op.win, c.par(op.p[P_GN1G]),
+                   c.par(op.p[P_GN1B]), c.fwd(op.a1));
         run_conv(c, conv_args(c, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, op.hin, op.win, op.hin, op.win, 3, 1,
                               c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
         break;
@@ -265,57 +339,59 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   const float* emb = (const float*)(c.stash + s->emb_off);
   if (!accumulate_wgrad)
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
+  if (!accumulate_wgrad || !s->wt_valid) prepare_weights(c);
+  CK_CUDA(cudaMemsetAsync(c.work + s->zero_begin, 0, s->zero_end - s->zero_begin, c.st));
   CK_CUDA(cudaMemcpyAsync(c.grad(s->t_dout), d_g_d_out, c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
   if (open) {
     if (d_g_e_out) CK_CUDA(cudaMemcpyAsync(c.grad(s->t_eout), d_g_e_out, c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
     else CK_CUDA(cudaMemsetAsync(c.grad(s->t_eout), 0, c.bytes(s->t_eout), c.st));
   }
-  float* partial = (float*)(c.work + s->w_partial);
   for (int i = (int)s->ops.size() - 1; i >= 0; --i) {
     const OpPlan& op = s->ops[i];
     const int n = s->d.n;
     switch (op.kind) {
-      case PULSE_OP_RESBLOCK: resblock_backward(c, op, emb, d_g_temb); break;
+      case PULSE_OP_RESBLOCK: resblock_backward(c, op); break;
       case PULSE_OP_CONV_IN:
       case PULSE_OP_DOWN: {
         const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
         char* g_out = c.grad(op.out);
-        s->launches += colsum(c.dt, g_out, n, op.hout * op.wout, op.cout, nullptr, c.pgrad(op.p[P_C1B]), partial, c.st);
+        ensure_colsum(c, op.out);
         WgradArgs w{c.dt, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, n, op.hin, op.win, g_out, op.hout, op.wout, op.cout, 3,
                     stride, c.pgrad(op.p[P_C1W])};
         run_wgrad(c, w);
         const bool need_gx = !(op.x0 == s->t_xin && !d_g_x_in);
         if (need_gx)
-          run_dgrad(c, g_out, op.hout, op.wout, op.cout, c.par(op.p[P_C1W]), 3, op.cin, c.grad(op.x0), op.acc_x0,
-                    stride, op.hin, op.win);
+          run_dgrad(c, g_out, op.hout, op.wout, op.cout, op.wt1, 3, op.cin, c.grad(op.x0), op.acc_x0, stride, op.hin,
+                    op.win);
         break;
       }
       case PULSE_OP_UP: {
         char* g_out = c.grad(op.out);
         char* g_u = c.work + s->w_gu;
-        s->launches += colsum(c.dt, g_out, n, op.hout * op.wout, op.cout, nullptr, c.pgrad(op.p[P_C1B]), partial, c.st);
+        ensure_colsum(c, op.out);
         WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
                     1, c.pgrad(op.p[P_C1W])};
         run_wgrad(c, w);
-        run_dgrad(c, g_out, op.hout, op.wout, op.cout, c.par(op.p[P_C1W]), 3, op.cin, g_u, 0, 1, op.hout, op.wout);
+        run_dgrad(c, g_out, op.hout, op.wout, op.cout, op.wt1, 3, op.cin, g_u, 0, 1, op.hout, op.wout);
         s->launches += upsample2_bwd(c.dt, g_u, n, op.hin, op.win, op.cin, c.grad(op.x0), c.st);
         break;
       }
       case PULSE_OP_HEAD: {
         char* g_out = c.grad(op.out);
         char* g_a = c.work + s->w_ga1;
-        s->launches += colsum(c.dt, g_out, n, op.hin * op.win, op.cout, nullptr, c.pgrad(op.p[P_C1B]), partial, c.st);
+        ensure_colsum(c, op.out);
         WgradArgs w{c.dt, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
                     c.pgrad(op.p[P_C1W])};
         run_wgrad(c, w);
-        run_dgrad(c, g_out, op.hin, op.win, op.cout, c.par(op.p[P_C1W]), 3, op.cin, g_a, 0, 1, op.hin, op.win);
-        run_gn_bwd(c, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin * op.win, c.par(op.p[P_GN1G]),
-                   c.par(op.p[P_GN1B]), op.stats1, nullptr, c.grad(op.x0), op.cin, 0, nullptr, 0,
-                   c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]));
+        run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wt1, 3, op.cin, g_a, 0, 1, op.hin, op.win);
+        run_gn_bwd(c, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.x0, -1, op.hin * op.win, c.par(op.p[P_GN1G]),
+                   c.par(op.p[P_GN1B]), op.bst1, nullptr, c.grad(op.x0), op.cin, 0, nullptr, 0,
+                   c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]), cs_of(c, op.x0), nullptr);
         break;
       }
     }
   }
+  small_grads(c, emb, d_g_temb);
   if (open) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   if (d_g_x_in) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());

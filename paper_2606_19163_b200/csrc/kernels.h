@@ -19,25 +19,27 @@ struct Cat {
 };
 
 // ---- GroupNorm + SiLU -------------------------------------------
-struct GnPlan { int nchunks, tpr, rows; };
-GnPlan gn_plan(int dt, int hw, int c, int n);
-size_t gn_partial_elems(const GnPlan& p, int n, int c);   // floats of scratch for partial sums
-// gsum: [N][G][2] doubles (sum, sum of squares per group), written by the forward, read by the backward.
-// partial: gn_partial_elems() floats of scratch (per-CTA partial sums; no atomics, no zeroing needed).
+// Statistics interface: "channel stats" cst[n][2][c] fp32 = per-(image, channel) sum and sum of squares over
+// the pixels of ONE tensor, accumulated with atomics (zero them first).  Produced by chan_stats (or, later, by
+// the conv epilogue that writes the tensor), consumed by every GroupNorm site that reads the tensor; a dual-
+// source site takes one cst per source.
+struct RowPlan { int tpr, rows, nchunks; };
+RowPlan row_plan(int dt, int hw, int c, int n, int max_threads);
+int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st);
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                void* a_out, double* gsum, float* partial, cudaStream_t st);
+                const float* cst0, const float* cst1, void* a_out, cudaStream_t st);
 // g_x = r(gamma g_y - A - xhat B) [+ add]; channels [0,dc0) -> dst0, rest -> dst1; accX: += instead of =
-// dgamma/dbeta: fp32, += (each channel owned by one CTA).  groups <= 64.
+// bst: [n][2][C] fp32 scratch, zeroed by the caller (per-(image, channel) sums of g_y and g_y xhat).
+// dgamma/dbeta: fp32, +=.  cs0/cs1 (nullable): [n][dc0] / [n][C-dc0] fp32, += the per-(image, channel) pixel
+// sums of what this call adds to dst0 / dst1 (bias and temb-projection gradients are made of these).
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
-                const void* beta, const double* gsum, const void* add, void* dst0, int dc0, int acc0, void* dst1,
-                int acc1, float* dgamma, float* dbeta, float* partial, cudaStream_t st);
+                const void* beta, const float* cst0, const float* cst1, float* bst, const void* add, void* dst0,
+                int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
+                cudaStream_t st);
 
 // ---- small ops -----------------------------------------------------------------------
-// s[n][c] = sum over pixels of g[n][hw][c];  out_n[n][c] = s (if non-null);
-// out_tot[c] += sum_n s (if non-null)
-int colsum(int dt, const void* g, int n, int hw, int c, float* out_n, float* out_tot, float* partial,
-           cudaStream_t st, float* out_tot2 = nullptr);
-size_t colsum_partial_elems(int dt, int n, int hw, int c);
+// cs[n][c] += sum over pixels of g[n][hw][c]   (tensors whose writers could not emit their column sums)
+int colsum(int dt, const void* g, int n, int hw, int c, float* cs, cudaStream_t st);
 // out[n][o] = sum_i W[o][i] f(in[n][i]) + b[o]; f = SiLU if silu_in.  W,b in dtype dt; in/out fp32
 int linear_fwd(int dt, const float* in, int n, int din, int dout, const void* w, const void* b, int silu_in,
                float* out, cudaStream_t st);
@@ -45,6 +47,21 @@ int linear_fwd(int dt, const float* in, int n, int din, int dout, const void* w,
 // g_in[n][i] (+)= (sum_o g[n][o] W[o][i]) f'(in[n][i])   (g_in may be null)
 int linear_bwd(int dt, const float* in, const float* g, int n, int din, int dout, const void* w, int silu_in,
                float* dw, float* db, float* g_in, int acc_g_in, cudaStream_t st);
+// Batched over the ops of a stage (one launch per 16 entries instead of one per op):
+struct ProjEntry { const void* w; const void* b; float* out; int cout; };          // out[n][cout] = W silu(emb) + b
+int temb_proj_batch(int dt, const float* emb, int n, int T, const ProjEntry* e, int count, cudaStream_t st);
+// Everything an op's small gradients need, from the column sums the big kernels emitted:
+//   db_out (+ db_out2) += sum_n cs_out[n][c];  with gp (ResBlocks): db1 += sum_n gp, dtb += sum_n gp,
+//   dtw[c][j] += sum_n gp[n][c] silu(emb[n][j]),  g_emb[n][j] += sum_c gp[n][c] tw[c][j] silu'(emb[n][j])
+struct SmallGradEntry {
+  const float* cs_out; float* db_out; float* db_out2;
+  const float* gp; float* db1; float* dtb; float* dtw; const void* tw;
+  int cout;
+};
+int small_grads_batch(int dt, const float* emb, float* g_emb, int n, int T, const SmallGradEntry* e, int count,
+                      cudaStream_t st);
+struct TransposeEntry { const void* w; void* wt; int cout, k, cin; };
+int flip_transpose_batch(int dt, const TransposeEntry* e, int count, cudaStream_t st);
 int sinusoidal(const int64_t* t, int n, int d, float* out, cudaStream_t st);
 int mse_fwd_bwd(int dt, const void* d, const void* target, size_t numel, float scale, float* loss, void* g,
                 cudaStream_t st);

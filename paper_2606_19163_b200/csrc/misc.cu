@@ -8,30 +8,16 @@
 namespace pulse {
 
 // ------------------------------------------------------------------ column sums over pixels
-static void colsum_plan(int dt, int n, int hw, int c, int& tpr, int& rows, int& nchunks) {
-  const int vec = dt == DT_F32 ? 4 : 8;
-  tpr = c / vec;
-  rows = tpr >= 256 ? 1 : 256 / tpr;
-  if (rows > hw) rows = hw;
-  int maxc = hw / (rows * 8);
-  if (maxc < 1) maxc = 1;
-  int want = (296 + n - 1) / n;
-  nchunks = want < maxc ? want : maxc;
-}
-size_t colsum_partial_elems(int dt, int n, int hw, int c) {
-  int tpr, rows, nchunks;
-  colsum_plan(dt, n, hw, c, tpr, rows, nchunks);
-  return (size_t)n * nchunks * c;
-}
-
-// per-CTA partial column sums partial[n][chunk][C] (no same-address atomics across hundreds of CTAs)
+// cs[n][c] += sum_pix g[n][pix][c].  Only for gradient tensors whose writers could not emit their own column
+// sums (the loss gradient that enters from outside, conv-dgrad outputs); everything written by the GroupNorm
+// backward carries its sums already (norm.cu).  One fp32 atomic per channel per CTA.
 template <typename T>
-__global__ void __launch_bounds__(512) colsum_k(const T* __restrict__ g, int hw, int C, float* __restrict__ partial) {
+__global__ void __launch_bounds__(512, 2) colsum_k(const T* __restrict__ g, int hw, int C, float* __restrict__ cs) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm[];
-  const int n = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x;
+  const int n = blockIdx.y, nchunks = gridDim.x;
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = chunk * ppc, pe = min(hw, pb + ppc);
+  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
   const int ch = threadIdx.x * V, rows = blockDim.y, ty = threadIdx.y;
   float s[V];
 #pragma unroll
@@ -51,87 +37,179 @@ __global__ void __launch_bounds__(512) colsum_k(const T* __restrict__ g, int hw,
 #pragma unroll
       for (int i = 0; i < V; ++i) s[i] += v[u][i];
   }
-  if (rows > 1) {
+  if (rows == 1) {
 #pragma unroll
-    for (int i = 0; i < V; ++i) sm[ty * C + ch + i] = s[i];
-    __syncthreads();
-    if (ty == 0) {
-#pragma unroll
-      for (int i = 0; i < V; ++i) {
-        float u = 0.f;
-        for (int r = 0; r < rows; ++r) u += sm[r * C + ch + i];
-        s[i] = u;
-      }
-    }
+    for (int i = 0; i < V; ++i) atomicAdd(cs + (size_t)n * C + ch + i, s[i]);
+    return;
   }
-  if (ty == 0) {
-    float* o = partial + ((size_t)n * nchunks + chunk) * C + ch;
 #pragma unroll
-    for (int i = 0; i < V; ++i) o[i] = s[i];
-  }
-}
-
-// block (32 channels x 8 row slices) per (channel tile, image): out_n[n][c] = sum over chunks; out_tot[c] += it
-__global__ void colsum_finalize_k(const float* __restrict__ partial, int nchunks, int C, float* out_n, float* out_tot,
-                                  float* out_tot2) {
-  __shared__ float sm[8][33];
-  const int c = blockIdx.x * 32 + threadIdx.x, n = blockIdx.y;
-  float s = 0.f;
-  if (c < C)
-    for (int k = threadIdx.y; k < nchunks; k += 8) s += partial[((size_t)n * nchunks + k) * C + c];
-  sm[threadIdx.y][threadIdx.x] = s;
+  for (int i = 0; i < V; ++i) sm[ty * C + ch + i] = s[i];
   __syncthreads();
-  if (threadIdx.y == 0 && c < C) {
+  for (int c = ty * blockDim.x + threadIdx.x; c < C; c += blockDim.x * blockDim.y) {
     float t = 0.f;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) t += sm[k][threadIdx.x];
-    if (out_n) out_n[(size_t)n * C + c] = t;
-    if (out_tot) atomicAdd(out_tot + c, t);      // <= N-way
-    if (out_tot2) atomicAdd(out_tot2 + c, t);
+    for (int r = 0; r < rows; ++r) t += sm[r * C + c];
+    atomicAdd(cs + (size_t)n * C + c, t);
   }
 }
 
-// any C (used for Cout = 4): one block per channel
+// any C (used for Cout = 4): one block per (channel, image)
 template <typename T>
-__global__ void colsum_scalar_k(const T* __restrict__ g, int n, int hw, int C, float* out_n, float* out_tot,
-                                float* out_tot2) {
-  const int c = blockIdx.x;
+__global__ void colsum_scalar_k(const T* __restrict__ g, int hw, int C, float* cs) {
+  const int c = blockIdx.x, n = blockIdx.y;
   __shared__ float sh[32];
-  float tot = 0.f;
-  for (int nn = 0; nn < n; ++nn) {
-    float s = 0.f;
-    for (int p = threadIdx.x; p < hw; p += blockDim.x) s += to_f(g[((size_t)nn * hw + p) * C + c]);
-    s = warp_sum(s);
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      float v = 0.f;
-      for (int i = 0; i < (int)(blockDim.x >> 5); ++i) v += sh[i];
-      if (out_n) out_n[(size_t)nn * C + c] = v;
-      tot += v;
-    }
-    __syncthreads();
+  float s = 0.f;
+  for (int p = threadIdx.x; p < hw; p += blockDim.x) s += to_f(g[((size_t)n * hw + p) * C + c]);
+  s = warp_sum(s);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float v = 0.f;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) v += sh[i];
+    atomicAdd(cs + (size_t)n * C + c, v);
   }
-  if (threadIdx.x == 0 && out_tot) out_tot[c] += tot;
-  if (threadIdx.x == 0 && out_tot2) out_tot2[c] += tot;
 }
 
-int colsum(int dt, const void* g, int n, int hw, int c, float* out_n, float* out_tot, float* partial,
-           cudaStream_t st, float* out_tot2) {
+int colsum(int dt, const void* g, int n, int hw, int c, float* cs, cudaStream_t st) {
   const int vec = dt == DT_F32 ? 4 : 8;
   if (c % vec || c / vec > 512) {
-    if (dt == DT_F32) colsum_scalar_k<float><<<c, 256, 0, st>>>((const float*)g, n, hw, c, out_n, out_tot, out_tot2);
-    else colsum_scalar_k<bf16><<<c, 256, 0, st>>>((const bf16*)g, n, hw, c, out_n, out_tot, out_tot2);
+    if (dt == DT_F32) colsum_scalar_k<float><<<dim3(c, n), 256, 0, st>>>((const float*)g, hw, c, cs);
+    else colsum_scalar_k<bf16><<<dim3(c, n), 256, 0, st>>>((const bf16*)g, hw, c, cs);
     return 1;
   }
-  int tpr, rows, nchunks;
-  colsum_plan(dt, n, hw, c, tpr, rows, nchunks);
-  dim3 grid(nchunks, n), block(tpr, rows);
-  const size_t smem = rows > 1 ? (size_t)rows * c * sizeof(float) : 0;
-  if (dt == DT_F32) colsum_k<float><<<grid, block, smem, st>>>((const float*)g, hw, c, partial);
-  else colsum_k<bf16><<<grid, block, smem, st>>>((const bf16*)g, hw, c, partial);
-  colsum_finalize_k<<<dim3((c + 31) / 32, n), dim3(32, 8), 0, st>>>(partial, nchunks, c, out_n, out_tot, out_tot2);
-  return 2;
+  const RowPlan pl = row_plan(dt, hw, c, n, 512);
+  dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
+  const size_t smem = pl.rows > 1 ? (size_t)pl.rows * c * sizeof(float) : 0;
+  if (dt == DT_F32) colsum_k<float><<<grid, block, smem, st>>>((const float*)g, hw, c, cs);
+  else colsum_k<bf16><<<grid, block, smem, st>>>((const bf16*)g, hw, c, cs);
+  return 1;
+}
+
+// ------------------------------------------------------------------ batched per-op small kernels
+constexpr int BATCH = 16;
+struct ProjBatch { int count; ProjEntry e[BATCH]; };
+struct SmallGradBatch { int count; SmallGradEntry e[BATCH]; };
+struct TransposeBatch { int count; TransposeEntry e[BATCH]; };
+
+// p[n][o] = sum_j W[o][j] silu(emb[n][j]) + b[o] for every ResBlock of the stage in one launch.
+// Block: 8 warps x 4 outputs; silu(emb) is staged once per block in shared memory ([n <= 8][T] floats).
+template <typename T>
+__global__ void __launch_bounds__(256) temb_proj_k(const float* __restrict__ emb, int n0, int nn, int Tdim,
+                                                   const __grid_constant__ ProjBatch b) {
+  extern __shared__ float se[];        // [nn][Tdim]
+  const ProjEntry& e = b.e[blockIdx.y];
+  const int o0 = blockIdx.x * 32;
+  if (o0 >= e.cout) return;
+  for (int i = threadIdx.x; i < nn * Tdim; i += blockDim.x) se[i] = siluf_(emb[(size_t)n0 * Tdim + i]);
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const T* w = (const T*)e.w;
+  const T* bias = (const T*)e.b;
+  for (int q = 0; q < 4; ++q) {
+    const int o = o0 + warp * 4 + q;
+    if (o >= e.cout) break;
+    float acc[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+    for (int i = lane; i < Tdim; i += 32) {
+      const float wv = to_f(w[(size_t)o * Tdim + i]);
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        if (j < nn) acc[j] = fmaf(wv, se[j * Tdim + i], acc[j]);
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      if (j < nn) {
+        const float t = warp_sum(acc[j]);
+        if (lane == 0) e.out[(size_t)(n0 + j) * e.cout + o] = t + to_f(bias[o]);
+      }
+  }
+}
+
+int temb_proj_batch(int dt, const float* emb, int n, int T, const ProjEntry* e, int count, cudaStream_t st) {
+  int launches = 0;
+  for (int i0 = 0; i0 < count; i0 += BATCH) {
+    ProjBatch b;
+    b.count = count - i0 < BATCH ? count - i0 : BATCH;
+    int maxc = 0;
+    for (int i = 0; i < b.count; ++i) { b.e[i] = e[i0 + i]; if (e[i0 + i].cout > maxc) maxc = e[i0 + i].cout; }
+    for (int n0 = 0; n0 < n; n0 += 8) {
+      const int nn = n - n0 < 8 ? n - n0 : 8;
+      dim3 grid((maxc + 31) / 32, b.count);
+      const size_t smem = (size_t)nn * T * sizeof(float);
+      if (dt == DT_F32) temb_proj_k<float><<<grid, 256, smem, st>>>(emb, n0, nn, T, b);
+      else temb_proj_k<bf16><<<grid, 256, smem, st>>>(emb, n0, nn, T, b);
+      ++launches;
+    }
+  }
+  return launches;
+}
+
+// Per op (blockIdx.z), channel chunk of 32 (blockIdx.y), 256 columns j of the temb dimension (blockIdx.x):
+//   dtw[c][j] += sum_n gp[n][c] silu(emb[n][j]);  g_emb[n][j] += silu'(emb[n][j]) sum_c gp[n][c] tw[c][j];
+//   blockIdx.x == 0 also folds the bias gradients: db_out (+ db_out2) += sum_n cs_out, db1 / dtb += sum_n gp.
+template <typename T>
+__global__ void __launch_bounds__(256) small_grads_k(const float* __restrict__ emb, float* g_emb, int n, int Tdim,
+                                                     const __grid_constant__ SmallGradBatch b) {
+  const SmallGradEntry& e = b.e[blockIdx.z];
+  const int c0 = blockIdx.y * 32;
+  if (c0 >= e.cout) return;
+  const int cn = min(32, e.cout - c0);
+  __shared__ float sgp[8][32];
+  if (blockIdx.x == 0 && threadIdx.x < cn) {
+    const int c = c0 + threadIdx.x;
+    float s = 0.f, t = 0.f;
+    for (int j = 0; j < n; ++j) {
+      s += e.cs_out[(size_t)j * e.cout + c];
+      if (e.gp) t += e.gp[(size_t)j * e.cout + c];
+    }
+    e.db_out[c] += s;
+    if (e.db_out2) e.db_out2[c] += s;
+    if (e.gp) { e.db1[c] += t; e.dtb[c] += t; }
+  }
+  if (!e.gp) return;
+  const int j = blockIdx.x * 256 + threadIdx.x;
+  const T* tw = (const T*)e.tw;
+  for (int n0 = 0; n0 < n; n0 += 8) {
+    const int nn = min(8, n - n0);
+    __syncthreads();
+    if (threadIdx.x < 32 * nn) {
+      const int r = threadIdx.x >> 5, c = threadIdx.x & 31;
+      sgp[r][c] = c < cn ? e.gp[(size_t)(n0 + r) * e.cout + c0 + c] : 0.f;
+    }
+    __syncthreads();
+    if (j < Tdim) {
+      float se[8], ge[8];
+#pragma unroll
+      for (int r = 0; r < 8; ++r) { se[r] = r < nn ? siluf_(emb[(size_t)(n0 + r) * Tdim + j]) : 0.f; ge[r] = 0.f; }
+      for (int c = 0; c < cn; ++c) {
+        const float w = to_f(tw[(size_t)(c0 + c) * Tdim + j]);
+        float d = 0.f;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) { d = fmaf(sgp[r][c], se[r], d); ge[r] = fmaf(sgp[r][c], w, ge[r]); }
+        e.dtw[(size_t)(c0 + c) * Tdim + j] += d;
+      }
+      if (g_emb)
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+          if (r < nn) atomicAdd(g_emb + (size_t)(n0 + r) * Tdim + j, ge[r] * silu_gradf_(emb[(size_t)(n0 + r) * Tdim + j]));
+    }
+  }
+}
+
+int small_grads_batch(int dt, const float* emb, float* g_emb, int n, int T, const SmallGradEntry* e, int count,
+                      cudaStream_t st) {
+  int launches = 0;
+  for (int i0 = 0; i0 < count; i0 += BATCH) {
+    SmallGradBatch b;
+    b.count = count - i0 < BATCH ? count - i0 : BATCH;
+    int maxc = 0;
+    for (int i = 0; i < b.count; ++i) { b.e[i] = e[i0 + i]; if (e[i0 + i].cout > maxc) maxc = e[i0 + i].cout; }
+    dim3 grid((T + 255) / 256, (maxc + 31) / 32, b.count);
+    if (dt == DT_F32) small_grads_k<float><<<grid, 256, 0, st>>>(emb, g_emb, n, T, b);
+    else small_grads_k<bf16><<<grid, 256, 0, st>>>(emb, g_emb, n, T, b);
+    ++launches;
+  }
+  return launches;
 }
 
 // ------------------------------------------------------------------ tiny linears (timestep path)
@@ -412,6 +490,47 @@ __global__ void flip_transpose_k(const T* __restrict__ w, int cout, int kk, int 
     const int ci = ci0 + j, co = co0 + threadIdx.x;
     if (co < cout && ci < cin) wt[((size_t)ci * kk + ftap) * cout + co] = tile[threadIdx.x][j];
   }
+}
+// all conv weights of a stage in one launch per 16 tensors (blockIdx.z = entry; taps looped inside)
+template <typename T>
+__global__ void flip_transpose_batch_k(const __grid_constant__ TransposeBatch b) {
+  __shared__ T tile[32][33];
+  const TransposeEntry& e = b.e[blockIdx.z];
+  const int ci0 = blockIdx.x * 32, co0 = blockIdx.y * 32, kk = e.k * e.k;
+  if (ci0 >= e.cin || co0 >= e.cout) return;
+  const T* w = (const T*)e.w;
+  T* wt = (T*)e.wt;
+  for (int tap = 0; tap < kk; ++tap) {
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+      const int co = co0 + j, ci = ci0 + threadIdx.x;
+      if (co < e.cout && ci < e.cin) tile[j][threadIdx.x] = w[((size_t)co * kk + tap) * e.cin + ci];
+    }
+    __syncthreads();
+    const int ftap = kk - 1 - tap;
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+      const int ci = ci0 + j, co = co0 + threadIdx.x;
+      if (co < e.cout && ci < e.cin) wt[((size_t)ci * kk + ftap) * e.cout + co] = tile[threadIdx.x][j];
+    }
+    __syncthreads();
+  }
+}
+int flip_transpose_batch(int dt, const TransposeEntry* e, int count, cudaStream_t st) {
+  int launches = 0;
+  for (int i0 = 0; i0 < count; i0 += BATCH) {
+    TransposeBatch b;
+    b.count = count - i0 < BATCH ? count - i0 : BATCH;
+    int mci = 0, mco = 0;
+    for (int i = 0; i < b.count; ++i) {
+      b.e[i] = e[i0 + i];
+      if (b.e[i].cin > mci) mci = b.e[i].cin;
+      if (b.e[i].cout > mco) mco = b.e[i].cout;
+    }
+    dim3 grid((mci + 31) / 32, (mco + 31) / 32, b.count), block(32, 8);
+    if (dt == DT_F32) flip_transpose_batch_k<float><<<grid, block, 0, st>>>(b);
+    else flip_transpose_batch_k<bf16><<<grid, block, 0, st>>>(b);
+    ++launches;
+  }
+  return launches;
 }
 int flip_transpose(int dt, const void* w, int cout, int k, int cin, void* wt, cudaStream_t st) {
   dim3 grid((cin + 31) / 32, (cout + 31) / 32, k * k), block(32, 8);

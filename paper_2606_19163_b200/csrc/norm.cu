@@ -1,14 +1,24 @@
-// norm.cu - fused GroupNorm + SiLU forward / backward on NHWC tensors, single or
-// dual source (virtual concat).  SURVEY.md 8c item 1:
+// norm.cu - fused GroupNorm + SiLU forward / backward on NHWC tensors, single or dual
+// source (virtual concat).  SURVEY.md 8c item 1:
 //   fwd: mu, var per (n,group) (biased), r = rsqrt(var+eps), xhat = (x-mu) r,
 //        y = gamma xhat + beta, a = y sigmoid(y)
 //   bwd: g_y = g_a SiLU'(y); dgamma = sum g_y xhat; dbeta = sum g_y; q = g_y gamma;
 //        A = mean_S q; B = mean_S q xhat; g_x = r (q - A - xhat B)
-// Layout choice for NHWC: a thread owns one 16-byte channel vector and walks pixels, so
-// every warp-wide access is contiguous and per-channel partial sums live in registers;
-// group statistics are then formed from per-channel sums in a tiny finalize kernel
-// (groups of 10/20/30/60 channels are not 16-byte aligned and may straddle the h|skip
-// boundary - per-channel partials make both irrelevant).
+// HBM-bound, so the design is about passes over memory:
+//  * Statistics travel as PER-(image, channel) sums [n][2][C] fp32 ("channel stats").  Group
+//    sums are formed from them in a few hundred cycles of kernel prologue, which makes groups
+//    that are not 16-byte aligned (10/20/30/60 channels) or that straddle the h|skip boundary
+//    (960 = 640|320) irrelevant, and lets the PRODUCER of a tensor (a conv epilogue, or
+//    chan_stats_k for tensors that enter from outside) supply them: the forward is then a
+//    single read + write pass, and a tensor consumed by two GroupNorm sites (an encoder output
+//    that is also a cached skip) has its statistics computed once.
+//  * The backward needs per-(image, channel) sums of g_y and g_y xhat: one reduction pass
+//    (gn_bwd_stats_k), then one apply pass that also emits the per-(image, channel) sums of the
+//    gradient it writes (bias / temb-projection gradients need exactly those: no separate
+//    column-sum pass over the tensor).
+//  * Thread layout: a thread owns one 16-byte channel vector and walks pixels, so a CTA reads
+//    whole contiguous pixel rows (fully coalesced), per-channel partials live in registers,
+//    cross-CTA reduction is one fp32 atomic per channel per CTA (<= ~74-way per address).
 #include "common.cuh"
 #include "kernels.h"
 
@@ -25,146 +35,159 @@ static int num_sms() {
   return g_num_sms;
 }
 
-GnPlan gn_plan(int dt, int hw, int c, int n) {
-  GnPlan p;
+RowPlan row_plan(int dt, int hw, int c, int n, int max_threads) {
+  RowPlan p;
   const int vec = dt == DT_F32 ? 4 : 8;
   p.tpr = c / vec;
-  p.rows = p.tpr >= 256 ? 1 : 256 / p.tpr;
+  p.rows = p.tpr >= max_threads ? 1 : max_threads / p.tpr;
   if (p.rows > hw) p.rows = hw;
-  // ~2 CTAs per SM, at least 8 pixels per thread row (4 loads in flight x 2)
+  // ~2 CTAs per SM over the whole grid, at least 4 pixels per thread row (one unrolled batch of loads)
   int want = (2 * num_sms() + n - 1) / n;
-  int maxc = hw / (p.rows * 8);
+  int maxc = hw / (p.rows * 4);
   if (maxc < 1) maxc = 1;
   p.nchunks = want < maxc ? want : maxc;
   return p;
 }
-// scratch floats: per-CTA group partials [n][chunk][G][2] + per-CTA channel partials [n][chunk][2][C]
-size_t gn_partial_elems(const GnPlan& p, int n, int c) { return (size_t)n * p.nchunks * (2 * (size_t)c + 2 * 64) + 1024; }
+
+namespace {
 
 template <typename T>
 __device__ __forceinline__ const T* cat_ptr(const T* p0, int c0, const T* p1, int c1, size_t pix, int ch) {
   return ch < c0 ? p0 + pix * c0 + ch : p1 + pix * c1 + (ch - c0);
 }
 
-// Cross-CTA reductions avoid same-address atomics (hundreds of CTAs adding into C addresses serialise
-// in L2, measured 30 us for a 10 MB tensor): every CTA writes its partials, and the consuming kernel
-// finalises them in its prologue - group sums redundantly per CTA (2G values x nchunks loads), channel
-// sums with each channel owned by exactly one CTA.
+// dynamic shared memory layout of every kernel here: [2C] channel sums | [2G] group values | reduction scratch
+struct Smem {
+  float* cs;     // [2][C]
+  float* grp;    // [2][G]
+  float* red;    // [rows][k][C]
+  __device__ Smem(float* base, int C, int G) : cs(base), grp(base + 2 * C), red(base + 2 * C + 2 * G) {}
+};
+size_t smem_bytes(int C, int G, int rows, int k) {
+  return ((size_t)2 * C + 2 * G + (rows > 1 ? (size_t)rows * k * C : 0)) * sizeof(float);
+}
 
-// sm_g[2G] doubles <- sum over chunks of pg[n][chunk][2G]
-__device__ __forceinline__ void group_sums_to_smem(const float* __restrict__ pg, int n, int nchunks, int G, double* sm_g) {
-  const int tid = threadIdx.y * blockDim.x + threadIdx.x, nthr = blockDim.x * blockDim.y;
-  for (int i = tid; i < 2 * G; i += nthr) {
-    const float* p = pg + (size_t)n * nchunks * 2 * G + i;
-    double s = 0.0;
-    for (int k = 0; k < nchunks; ++k) s += (double)p[(size_t)k * 2 * G];
-    sm_g[i] = s;
+__device__ __forceinline__ int tid_() { return threadIdx.y * blockDim.x + threadIdx.x; }
+__device__ __forceinline__ int nthr_() { return blockDim.x * blockDim.y; }
+
+// grp[g] = mean, grp[G+g] = rstd of group g of image n, from the channel stats of the two sources
+__device__ __forceinline__ void group_mean_rstd(const float* __restrict__ cst0, int c0, const float* __restrict__ cst1,
+                                                int c1, int n, int hw, int G, float eps, Smem& s) {
+  const int C = c0 + c1, tid = tid_(), nthr = nthr_(), cpg = C / G;
+  for (int i = tid; i < 2 * C; i += nthr) {
+    const int which = i / C, c = i - which * C;
+    s.cs[i] = c < c0 ? cst0[((size_t)n * 2 + which) * c0 + c] : cst1[((size_t)n * 2 + which) * c1 + (c - c0)];
+  }
+  __syncthreads();
+  // combined in double (R22); 4 threads per group when the CTA has that many whole warps
+  const bool quad = nthr >= ((4 * G + 31) & ~31);
+  const int L = quad ? 4 : 1;
+  for (int g0 = 0; g0 < G; g0 += quad ? G : nthr) {
+    const int g = g0 + tid / L, l = tid % L;
+    double a = 0.0, b = 0.0;
+    if (g < G)
+      for (int c = g * cpg + l; c < (g + 1) * cpg; c += L) { a += (double)s.cs[c]; b += (double)s.cs[C + c]; }
+    if (quad && tid < ((4 * G + 31) & ~31)) {
+      a += __shfl_xor_sync(0xffffffffu, a, 1); b += __shfl_xor_sync(0xffffffffu, b, 1);
+      a += __shfl_xor_sync(0xffffffffu, a, 2); b += __shfl_xor_sync(0xffffffffu, b, 2);
+    }
+    if (g < G && l == 0) {
+      const double m = (double)cpg * hw, mu = a / m;
+      double var = b / m - mu * mu;
+      if (var < 0.0) var = 0.0;
+      s.grp[g] = (float)mu;
+      s.grp[G + g] = (float)(1.0 / sqrt(var + (double)eps));
+    }
   }
   __syncthreads();
 }
 
-// per-thread normalisation coefficients of V consecutive channels from the group sums (sum, sum of squares)
+// per-thread normalisation coefficients of V consecutive channels: y = x sc + sh, xhat = x rr - mr
 template <typename T, int V>
-__device__ __forceinline__ void gn_coefs(const double* gsum_n, int cpg, int hw, float eps, const T* __restrict__ gamma,
+__device__ __forceinline__ void gn_coefs(const Smem& s, int G, int cpg, const T* __restrict__ gamma,
                                          const T* __restrict__ beta, int ch, float (&sc)[V], float (&sh)[V],
                                          float (&rr)[V], float (&mr)[V]) {
-  const double m = (double)cpg * hw;
 #pragma unroll
   for (int i = 0; i < V; ++i) {
     const int g = (ch + i) / cpg;
-    const double mu = gsum_n[2 * g] / m;
-    double var = gsum_n[2 * g + 1] / m - mu * mu;
-    if (var < 0.0) var = 0.0;
-    const float r = (float)(1.0 / sqrt(var + (double)eps));
+    const float mu = s.grp[g], r = s.grp[G + g];
     const float ga = to_f(gamma[ch + i]), be = to_f(beta[ch + i]);
-    rr[i] = r; mr[i] = (float)mu * r;
+    rr[i] = r; mr[i] = mu * r;
     sc[i] = r * ga; sh[i] = be - mr[i] * ga;
   }
 }
 
-// block-reduce per-channel partials over rows; write per-group partials pg_out[2G] (weighted by wgt) and,
-// if pc_out, the per-channel sums pc_out[0..C) = s1, pc_out[C..2C) = s2
-template <int V, typename T>
-__device__ __forceinline__ void reduce_block(float (&s1)[V], float (&s2)[V], int C, int G, int cpg, const T* wgt,
-                                             float* pg_out, float* pc_out) {
-  extern __shared__ float sm[];
-  const int rows = blockDim.y, tx = threadIdx.x, ty = threadIdx.y, ch = tx * V;
-  float* a = sm;                  // [rows][C]
-  float* b = sm + rows * C;       // [rows][C]
-  float* gs = sm + 2 * rows * C;  // [G][2]
-  const int tid = ty * blockDim.x + tx, nthr = blockDim.x * blockDim.y;
-  for (int i = tid; i < 2 * G; i += nthr) gs[i] = 0.f;
-  if (rows > 1) {
+// sum the per-thread partials v[2][V] over the rows of the CTA and add them into dst[2][C] (global, one atomic
+// per channel per CTA)
+template <int V>
+__device__ __forceinline__ void reduce_rows_atomic(float (&v)[2][V], int C, Smem& s, float* dst) {
+  const int rows = blockDim.y, ch = threadIdx.x * V;
+  if (rows == 1) {
 #pragma unroll
-    for (int i = 0; i < V; ++i) { a[ty * C + ch + i] = s1[i]; b[ty * C + ch + i] = s2[i]; }
-  }
-  __syncthreads();
-  if (ty == 0) {
+    for (int k = 0; k < 2; ++k)
 #pragma unroll
-    for (int i = 0; i < V; ++i) {
-      float u = s1[i], v = s2[i];
-      if (rows > 1) {
-        u = 0.f; v = 0.f;
-        for (int r = 0; r < rows; ++r) { u += a[r * C + ch + i]; v += b[r * C + ch + i]; }
-      }
-      if (pc_out) { pc_out[ch + i] = u; pc_out[C + ch + i] = v; }
-      const float w = wgt ? to_f(wgt[ch + i]) : 1.f;
-      const int g = (ch + i) / cpg;
-      atomicAdd(&gs[2 * g], w * u);        // shared-memory atomics, <= cpg-way
-      atomicAdd(&gs[2 * g + 1], w * v);
-    }
+      for (int i = 0; i < V; ++i) atomicAdd(dst + k * C + ch + i, v[k][i]);
+    return;
   }
+#pragma unroll
+  for (int k = 0; k < 2; ++k)
+#pragma unroll
+    for (int i = 0; i < V; ++i) s.red[((size_t)threadIdx.y * 2 + k) * C + ch + i] = v[k][i];
   __syncthreads();
-  for (int i = tid; i < 2 * G; i += nthr) pg_out[i] = gs[i];
+  for (int j = tid_(); j < 2 * C; j += nthr_()) {
+    float t = 0.f;
+    for (int r = 0; r < rows; ++r) t += s.red[(size_t)r * 2 * C + j];
+    atomicAdd(dst + j, t);
+  }
 }
 
+// ------------------------------------------------------------------------------ channel stats of one tensor
 template <typename T>
-__global__ void __launch_bounds__(512) gn_stats_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1,
-                                                  int hw, int G, float* __restrict__ pg) {
+__global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, int C, int hw, float* __restrict__ cst) {
   constexpr int V = Vec<T>::N;
-  const int C = c0 + c1, n = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x;
+  extern __shared__ float sm_[];
+  Smem s(sm_, C, 0);
+  const int n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y;
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = chunk * ppc, pe = min(hw, pb + ppc);
-  const int ch = threadIdx.x * V, rows = blockDim.y;
-  float s1[V], s2[V];
+  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
+  const int ch = threadIdx.x * V;
+  float v[2][V];
 #pragma unroll
-  for (int i = 0; i < V; ++i) s1[i] = s2[i] = 0.f;
+  for (int i = 0; i < V; ++i) v[0][i] = v[1][i] = 0.f;
   for (int p = pb + threadIdx.y; p < pe; p += 4 * rows) {
-    float v[4][V];
+    float t[4][V];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      if (p + u * rows < pe) ldv(cat_ptr(p0, c0, p1, c1, (size_t)n * hw + p + u * rows, ch), v[u]);
+      if (p + u * rows < pe) ldv(x + ((size_t)n * hw + p + u * rows) * C + ch, t[u]);
       else {
 #pragma unroll
-        for (int i = 0; i < V; ++i) v[u][i] = 0.f;
+        for (int i = 0; i < V; ++i) t[u][i] = 0.f;
       }
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u)
 #pragma unroll
-      for (int i = 0; i < V; ++i) { s1[i] += v[u][i]; s2[i] = fmaf(v[u][i], v[u][i], s2[i]); }
+      for (int i = 0; i < V; ++i) { v[0][i] += t[u][i]; v[1][i] = fmaf(t[u][i], t[u][i], v[1][i]); }
   }
-  reduce_block<V, T>(s1, s2, C, G, C / G, nullptr, pg + ((size_t)n * nchunks + chunk) * 2 * G, nullptr);
+  reduce_rows_atomic<V>(v, C, s, cst + (size_t)n * 2 * C);
 }
 
+// ------------------------------------------------------------------------------ forward apply (one pass)
 template <typename T>
-__global__ void __launch_bounds__(512) gn_silu_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1,
-                                                       int hw, int G, float eps, const T* __restrict__ gamma,
-                                                       const T* __restrict__ beta, const float* __restrict__ pg,
-                                                       double* __restrict__ gsum, T* __restrict__ out) {
+__global__ void __launch_bounds__(512, 2)
+gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw, int G, float eps,
+           const T* __restrict__ gamma, const T* __restrict__ beta, const float* __restrict__ cst0,
+           const float* __restrict__ cst1, T* __restrict__ out) {
   constexpr int V = Vec<T>::N;
-  __shared__ double sm_g[128];
-  const int C = c0 + c1, n = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x;
+  extern __shared__ float sm_[];
+  const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y;
+  Smem s(sm_, C, G);
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = chunk * ppc, pe = min(hw, pb + ppc);
-  const int ch = threadIdx.x * V, rows = blockDim.y;
-  group_sums_to_smem(pg, n, nchunks, G, sm_g);
-  if (chunk == 0) {     // keep the group sums for the backward pass
-    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
-    for (int i = tid; i < 2 * G; i += blockDim.x * blockDim.y) gsum[(size_t)n * 2 * G + i] = sm_g[i];
-  }
+  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
+  const int ch = threadIdx.x * V;
+  group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
   float sc[V], sh[V], rr[V], mr[V];
-  gn_coefs<T, V>(sm_g, C / G, hw, eps, gamma, beta, ch, sc, sh, rr, mr);
+  gn_coefs<T, V>(s, G, C / G, gamma, beta, ch, sc, sh, rr, mr);
   for (int p = pb + threadIdx.y; p < pe; p += 4 * rows) {
     float v[4][V];
 #pragma unroll
@@ -180,43 +203,25 @@ __global__ void __launch_bounds__(512) gn_silu_apply_k(const T* __restrict__ p0,
   }
 }
 
-static size_t gn_smem(const GnPlan& pl, int C, int G) { return ((size_t)2 * pl.rows * C + 2 * G) * sizeof(float); }
-
+// ------------------------------------------------------------------------------ backward: reduction pass
+// bst[n][0][c] += sum_pix g_y, bst[n][1][c] += sum_pix g_y xhat
 template <typename T>
-static int gn_fwd_t(Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta, void* a_out,
-                    double* gsum, float* partial, const GnPlan& pl, cudaStream_t st) {
-  const int C = x.c();
-  dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
-  gn_stats_k<T><<<grid, block, gn_smem(pl, C, groups), st>>>((const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, partial);
-  gn_silu_apply_k<T><<<grid, block, 0, st>>>((const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps,
-                                             (const T*)gamma, (const T*)beta, partial, gsum, (T*)a_out);
-  return 2;
-}
-
-int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                void* a_out, double* gsum, float* partial, cudaStream_t st) {
-  GnPlan pl = gn_plan(dt, hw, x.c(), n);
-  return dt == DT_F32 ? gn_fwd_t<float>(x, n, hw, groups, eps, gamma, beta, a_out, gsum, partial, pl, st)
-                      : gn_fwd_t<bf16>(x, n, hw, groups, eps, gamma, beta, a_out, gsum, partial, pl, st);
-}
-
-// ------------------------------------------------------------------------------ backward
-
-template <typename T>
-__global__ void __launch_bounds__(512) gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0,
-                                                      const T* __restrict__ p1, int c1, int hw, int G, float eps,
-                                                      const T* __restrict__ gamma, const T* __restrict__ beta,
-                                                      const double* __restrict__ gsum, float* __restrict__ pg,
-                                                      float* __restrict__ pc) {
+__global__ void __launch_bounds__(512, 1)
+gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
+               int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
+               const float* __restrict__ cst0, const float* __restrict__ cst1, float* __restrict__ bst) {
   constexpr int V = Vec<T>::N;
-  const int C = c0 + c1, n = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x;
+  extern __shared__ float sm_[];
+  const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y;
+  Smem s(sm_, C, G);
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = chunk * ppc, pe = min(hw, pb + ppc);
-  const int ch = threadIdx.x * V, rows = blockDim.y;
-  float sc[V], sh[V], rr[V], mr[V], s1[V], s2[V];
-  gn_coefs<T, V>(gsum + (size_t)n * 2 * G, C / G, hw, eps, gamma, beta, ch, sc, sh, rr, mr);
+  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
+  const int ch = threadIdx.x * V;
+  group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
+  float sc[V], sh[V], rr[V], mr[V], v[2][V];
+  gn_coefs<T, V>(s, G, C / G, gamma, beta, ch, sc, sh, rr, mr);
 #pragma unroll
-  for (int i = 0; i < V; ++i) s1[i] = s2[i] = 0.f;
+  for (int i = 0; i < V; ++i) v[0][i] = v[1][i] = 0.f;
   for (int p = pb + threadIdx.y; p < pe; p += 2 * rows) {
     float x[2][V], g[2][V];
 #pragma unroll
@@ -235,62 +240,77 @@ __global__ void __launch_bounds__(512) gn_bwd_stats_k(const T* __restrict__ ga, 
 #pragma unroll
       for (int i = 0; i < V; ++i) {
         const float gy = g[u][i] * silu_gradf_(fmaf(x[u][i], sc[i], sh[i]));
-        s1[i] += gy;
-        s2[i] = fmaf(gy, fmaf(x[u][i], rr[i], -mr[i]), s2[i]);
+        v[0][i] += gy;
+        v[1][i] = fmaf(gy, fmaf(x[u][i], rr[i], -mr[i]), v[1][i]);
       }
   }
-  // channel partials: s1 -> dbeta, s2 -> dgamma; group partials weighted by gamma: A m = sum gamma s1, B m = sum gamma s2
-  const size_t cta = (size_t)n * nchunks + chunk;
-  reduce_block<V, T>(s1, s2, C, G, C / G, gamma, pg + cta * 2 * G, pc + cta * 2 * C);
+  reduce_rows_atomic<V>(v, C, s, bst + (size_t)n * 2 * C);
 }
 
+// ------------------------------------------------------------------------------ backward: apply pass
+// g_x = r (gamma g_y - A - xhat B) [+ add]; channels [0,dc0) -> dst0, the rest -> dst1 (skip gradient,
+// PAPER.md:L91); acc: += instead of =.  cs0/cs1: per-(image, channel) sums of what this launch ADDS to
+// dst0/dst1 (before bf16 rounding), accumulated.  dgamma/dbeta: += sum_n bst (CTA chunk 0 of each image).
 template <typename T>
-__global__ void __launch_bounds__(512) gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0,
-                                                      const T* __restrict__ p1, int c1, int hw, int G, float eps,
-                                                      const T* __restrict__ gamma, const T* __restrict__ beta,
-                                                      const double* __restrict__ gsum, const float* __restrict__ pg,
-                                                      const float* __restrict__ pc, float* dgamma, float* dbeta,
-                                                      const T* __restrict__ add, T* dst0, int dc0, int acc0, T* dst1,
-                                                      int acc1) {
+__global__ void __launch_bounds__(512, 1)
+gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
+               int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
+               const float* __restrict__ cst0, const float* __restrict__ cst1, const float* __restrict__ bst,
+               float* dgamma, float* dbeta, const T* __restrict__ add, T* dst0, int dc0, int acc0, T* dst1, int acc1,
+               float* cs0, float* cs1) {
   constexpr int V = Vec<T>::N;
-  __shared__ double sm_g[128];
-  const int C = c0 + c1, n = blockIdx.y, chunk = blockIdx.x, nchunks = gridDim.x, cpg = C / G;
+  extern __shared__ float sm_[];
+  const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y, cpg = C / G;
+  Smem s(sm_, C, G);
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = chunk * ppc, pe = min(hw, pb + ppc);
-  const int ch = threadIdx.x * V, rows = blockDim.y;
-  group_sums_to_smem(pg, n, nchunks, G, sm_g);
-  {  // dgamma / dbeta: (channel, which) pair j is owned by CTA j % T; one warp sums its T partial rows
-    const int T_ = gridDim.x * gridDim.y, cta = blockIdx.y * gridDim.x + blockIdx.x;
-    const int tid = threadIdx.y * blockDim.x + threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nthr = blockDim.x * blockDim.y, nwarps = (nthr + 31) >> 5;
-    const bool full = (warp + 1) * 32 <= nthr;      // a partial last warp sums serially on its lane 0
-    for (int j = cta + warp * T_; j < 2 * C; j += nwarps * T_) {
-      const int which = j / C, c = j - which * C;
-      float s = 0.f;
-      if (full) {
-        for (int r = lane; r < T_; r += 32) s += pc[(size_t)r * 2 * C + which * C + c];
-        s = warp_sum(s);
-      } else if (lane == 0) {
-        for (int r = 0; r < T_; ++r) s += pc[(size_t)r * 2 * C + which * C + c];
-      }
-      if (lane == 0) {
-        if (which) dgamma[c] += s; else dbeta[c] += s;
-      }
+  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
+  const int ch = threadIdx.x * V, tid = tid_(), nthr = nthr_();
+  group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
+  float sc[V], sh[V], rr[V], mr[V], k2[V], k3[V];
+  gn_coefs<T, V>(s, G, cpg, gamma, beta, ch, sc, sh, rr, mr);
+  // group sums A m = sum_c gamma_c S1[c], B m = sum_c gamma_c S2[c]  (s.cs is free again: reuse it for S1|S2)
+  __syncthreads();
+  for (int i = tid; i < 2 * C; i += nthr) {
+    const float t = bst[(size_t)n * 2 * C + i];
+    s.cs[i] = t;
+    if (blockIdx.x == 0) {
+      if (i < C) atomicAdd(dbeta + i, t); else atomicAdd(dgamma + (i - C), t);
     }
   }
-  float sc[V], sh[V], rr[V], mr[V], k2[V], k3[V];
-  gn_coefs<T, V>(gsum + (size_t)n * 2 * G, cpg, hw, eps, gamma, beta, ch, sc, sh, rr, mr);
-  const double m = (double)cpg * hw;
+  __syncthreads();
+  {   // everyone has read s.grp (mean, rstd) through gn_coefs and synchronised since: overwrite it with A/m, B/m
+    const bool quad = nthr >= ((4 * G + 31) & ~31);
+    const int L = quad ? 4 : 1;
+    const float inv = 1.0f / ((float)cpg * (float)hw);
+    for (int g0 = 0; g0 < G; g0 += quad ? G : nthr) {
+      const int g = g0 + tid / L, l = tid % L;
+      float a = 0.f, b = 0.f;
+      if (g < G)
+        for (int c = g * cpg + l; c < (g + 1) * cpg; c += L) {
+          const float ga_ = to_f(gamma[c]);
+          a = fmaf(ga_, s.cs[c], a); b = fmaf(ga_, s.cs[C + c], b);
+        }
+      if (quad && tid < ((4 * G + 31) & ~31)) {
+        a += __shfl_xor_sync(0xffffffffu, a, 1); b += __shfl_xor_sync(0xffffffffu, b, 1);
+        a += __shfl_xor_sync(0xffffffffu, a, 2); b += __shfl_xor_sync(0xffffffffu, b, 2);
+      }
+      if (g < G && l == 0) { s.grp[g] = a * inv; s.grp[G + g] = b * inv; }
+    }
+    __syncthreads();
+  }
 #pragma unroll
   for (int i = 0; i < V; ++i) {
     const int g = (ch + i) / cpg;
-    k2[i] = (float)(sm_g[2 * g] / m) * rr[i];
-    k3[i] = (float)(sm_g[2 * g + 1] / m) * rr[i];
+    k2[i] = s.grp[g] * rr[i];
+    k3[i] = s.grp[G + g] * rr[i];
   }
   const bool first = ch < dc0;
   T* dst = first ? dst0 : dst1;
   const int dC = first ? dc0 : C - dc0, dch = first ? ch : ch - dc0;
   const int acc = first ? acc0 : acc1;
+  float sum[V];
+#pragma unroll
+  for (int i = 0; i < V; ++i) sum[i] = 0.f;
   for (int p = pb + threadIdx.y; p < pe; p += 2 * rows) {
     float x[2][V], g[2][V], e[2][V], f[2][V];
 #pragma unroll
@@ -313,37 +333,92 @@ __global__ void __launch_bounds__(512) gn_bwd_apply_k(const T* __restrict__ ga, 
           const float xh = fmaf(x[u][i], rr[i], -mr[i]);
           o[i] = sc[i] * gy - k2[i] - xh * k3[i];
           if (add) o[i] += e[u][i];
+          sum[i] += o[i];
           if (acc) o[i] += f[u][i];
         }
         stv(dst + pix * dC + dch, o);
       }
   }
+  if (cs0 || cs1) {      // channels below dc0 -> cs0[n][dc0], the rest -> cs1[n][C - dc0]
+    if (rows == 1) {
+#pragma unroll
+      for (int i = 0; i < V; ++i) {
+        const int c = ch + i;
+        if (c < dc0) { if (cs0) atomicAdd(cs0 + (size_t)n * dc0 + c, sum[i]); }
+        else if (cs1) atomicAdd(cs1 + (size_t)n * (C - dc0) + (c - dc0), sum[i]);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < V; ++i) s.red[(size_t)threadIdx.y * C + ch + i] = sum[i];
+      __syncthreads();
+      for (int c = tid; c < C; c += nthr) {
+        float t = 0.f;
+        for (int r = 0; r < rows; ++r) t += s.red[(size_t)r * C + c];
+        if (c < dc0) { if (cs0) atomicAdd(cs0 + (size_t)n * dc0 + c, t); }
+        else if (cs1) atomicAdd(cs1 + (size_t)n * (C - dc0) + (c - dc0), t);
+      }
+    }
+  }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------ host launchers
+int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st) {
+  const RowPlan pl = row_plan(dt, hw, c, n, 512);
+  dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
+  const size_t sm = smem_bytes(c, 0, pl.rows, 2);
+  if (dt == DT_F32) chan_stats_k<float><<<grid, block, sm, st>>>((const float*)x, c, hw, cst);
+  else chan_stats_k<bf16><<<grid, block, sm, st>>>((const bf16*)x, c, hw, cst);
+  return 1;
+}
+
+int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
+                const float* cst0, const float* cst1, void* a_out, cudaStream_t st) {
+  const int C = x.c();
+  const RowPlan pl = row_plan(dt, hw, C, n, 512);
+  dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
+  const size_t sm = smem_bytes(C, groups, 1, 0);
+  if (dt == DT_F32)
+    gn_apply_k<float><<<grid, block, sm, st>>>((const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw, groups, eps,
+                                               (const float*)gamma, (const float*)beta, cst0, cst1, (float*)a_out);
+  else
+    gn_apply_k<bf16><<<grid, block, sm, st>>>((const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw, groups, eps,
+                                              (const bf16*)gamma, (const bf16*)beta, cst0, cst1, (bf16*)a_out);
+  return 1;
 }
 
 template <typename T>
 static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                    const double* gsum, const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1,
-                    float* dgamma, float* dbeta, float* partial, const GnPlan& pl, cudaStream_t st) {
+                    const float* cst0, const float* cst1, float* bst, const void* add, void* dst0, int dc0, int acc0,
+                    void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st) {
   const int C = x.c();
+  const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
+  const RowPlan pl = row_plan(dt, hw, C, n, 256);
   dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
-  float* pg = partial;
-  float* pc = partial + (size_t)n * pl.nchunks * 2 * groups;
-  gn_bwd_stats_k<T><<<grid, block, gn_smem(pl, C, groups), st>>>((const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1,
-                                                                  hw, groups, eps, (const T*)gamma, (const T*)beta, gsum, pg, pc);
-  gn_bwd_apply_k<T><<<grid, block, 0, st>>>((const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps,
-                                            (const T*)gamma, (const T*)beta, gsum, pg, pc, dgamma, dbeta, (const T*)add,
-                                            (T*)dst0, dc0, acc0, (T*)dst1, acc1);
+  static bool attr = false;
+  if (!attr) {
+    cudaFuncSetAttribute(gn_bwd_stats_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    cudaFuncSetAttribute(gn_bwd_apply_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    attr = true;
+  }
+  gn_bwd_stats_k<T><<<grid, block, smem_bytes(C, groups, pl.rows, 2), st>>>(
+      (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0,
+      cst1, bst);
+  gn_bwd_apply_k<T><<<grid, block, smem_bytes(C, groups, pl.rows, 1), st>>>(
+      (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0,
+      cst1, bst, dgamma, dbeta, (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1);
   return 2;
 }
 
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
-                const void* beta, const double* gsum, const void* add, void* dst0, int dc0, int acc0, void* dst1,
-                int acc1, float* dgamma, float* dbeta, float* partial, cudaStream_t st) {
-  GnPlan pl = gn_plan(dt, hw, x.c(), n);
-  return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, gsum, add, dst0, dc0, acc0, dst1, acc1,
-                                        dgamma, dbeta, partial, pl, st)
-                      : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, gsum, add, dst0, dc0, acc0, dst1, acc1,
-                                       dgamma, dbeta, partial, pl, st);
+                const void* beta, const float* cst0, const float* cst1, float* bst, const void* add, void* dst0,
+                int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
+                cudaStream_t st) {
+  return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, cst0, cst1, bst, add, dst0, dc0, acc0,
+                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st)
+                      : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, cst0, cst1, bst, add, dst0, dc0, acc0,
+                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st);
 }
 
 }  // namespace pulse

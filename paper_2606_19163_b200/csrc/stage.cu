@@ -93,18 +93,8 @@ static pulse_status_t build_plan(pulse_stage* s) {
   if (d.x_in_is_skip) { s->skip_tensor.push_back(cur); stack.push_back(cur); }
   s->emb_off = pl.bump(R_STASH, (size_t)d.n * T * 4);
 
-  const size_t gsz = align256((size_t)d.n * G * 2 * sizeof(double));   // one GroupNorm site: [n][G][2] doubles
-  s->gn_site_bytes = gsz;
-  size_t m_out = 0, m_cat = 0, m_gu = 0, m_w = 0, m_partial = 0, m_coef = 0, m_gp = 0;
+  size_t m_out = 0, m_cat = 0, m_gu = 0;
   auto upd = [](size_t& m, size_t v) { if (v > m) m = v; };
-  auto gn_site = [&](int c, int hw) {
-    GnPlan gp = gn_plan(d.dtype, hw, c, d.n);
-    upd(m_partial, gn_partial_elems(gp, d.n, c) * 4);
-    upd(m_coef, (size_t)d.n * 2 * c * 4);
-  };
-  auto cs_site = [&](int c, int hw) {
-    if (c % vec == 0) upd(m_partial, colsum_partial_elems(d.dtype, d.n, hw, c) * 4);
-  };
 
   auto plan_ops = [&](const std::vector<pulse_op_desc>& list, const char* phase, bool is_dec) -> pulse_status_t {
     for (size_t i = 0; i < list.size(); ++i) {
@@ -144,13 +134,14 @@ static pulse_status_t build_plan(pulse_stage* s) {
         op.a1 = pl.tensor(R_STASH, ctot, op.hin, op.win, false);
         op.h1 = pl.tensor(R_STASH, o.cout, op.hin, op.win, false);
         op.a2 = pl.tensor(R_STASH, o.cout, op.hin, op.win, false);
-        op.stats1 = (size_t)(s->gn_sites++) * gsz;
-        op.stats2 = (size_t)(s->gn_sites++) * gsz;
+        s->tensors[op.x0].gn_input = true;
+        if (op.x1 >= 0) s->tensors[op.x1].gn_input = true;
+        s->tensors[op.h1].gn_input = true;
         op.pn = pl.bump(R_STASH, (size_t)d.n * o.cout * 4);
         upd(m_out, pix * o.cout * s->esz()); upd(m_cat, pix * ctot * s->esz());
-        upd(m_w, (size_t)o.cout * 9 * (ctot > o.cout ? ctot : o.cout) * s->esz());
-        upd(m_gp, (size_t)d.n * o.cout * 4);
-        gn_site(ctot, op.hin * op.win); gn_site(o.cout, op.hin * op.win); cs_site(o.cout, op.hin * op.win);
+        op.wt1 = pl.bump(R_WORK, (size_t)o.cout * 9 * ctot * s->esz());
+        op.wt2 = pl.bump(R_WORK, (size_t)o.cout * 9 * o.cout * s->esz());
+        if (ctot != o.cout) op.wtsc = pl.bump(R_WORK, (size_t)o.cout * ctot * s->esz());
       } else if (o.kind == PULSE_OP_CONV_IN || o.kind == PULSE_OP_DOWN || o.kind == PULSE_OP_UP) {
         if (o.skip_channels) return fail(PULSE_ERR_SHAPE, "%s%zu: only ResBlocks pop skips", phase, i);
         if (o.kind == PULSE_OP_DOWN) {
@@ -165,22 +156,22 @@ static pulse_status_t build_plan(pulse_stage* s) {
         }
         if (o.kind == PULSE_OP_CONV_IN && is_dec) return fail(PULSE_ERR_SHAPE, "%s%zu: conv_in belongs to the encoder", phase, i);
         op.p[P_C1W] = pl.param(pre + "conv.w", 4, o.cout, 3, 3, o.cin); op.p[P_C1B] = pl.param(pre + "conv.b", 1, o.cout);
-        upd(m_w, (size_t)o.cout * 9 * o.cin * s->esz());
-        cs_site(o.cout, op.hout * op.wout);
+        op.wt1 = pl.bump(R_WORK, (size_t)o.cout * 9 * o.cin * s->esz());
       } else if (o.kind == PULSE_OP_HEAD) {
         if (!is_dec || o.skip_channels || !chk_c(o.cin, "cin")) return fail(PULSE_ERR_SHAPE, "%s%zu: bad head", phase, i);
         op.p[P_GN1G] = pl.param(pre + "gn.gamma", 1, o.cin); op.p[P_GN1B] = pl.param(pre + "gn.beta", 1, o.cin);
         op.p[P_C1W] = pl.param(pre + "conv.w", 4, o.cout, 3, 3, o.cin); op.p[P_C1B] = pl.param(pre + "conv.b", 1, o.cout);
         op.a1 = pl.tensor(R_STASH, o.cin, op.hin, op.win, false);
-        op.stats1 = (size_t)(s->gn_sites++) * gsz;
-        upd(m_cat, pix * o.cin * s->esz()); upd(m_w, (size_t)o.cout * 9 * o.cin * s->esz());
-        gn_site(o.cin, op.hin * op.win); cs_site(o.cout, op.hin * op.win);
+        s->tensors[op.x0].gn_input = true;
+        upd(m_cat, pix * o.cin * s->esz());
+        op.wt1 = pl.bump(R_WORK, (size_t)o.cout * 9 * o.cin * s->esz());
       } else {
         return fail(PULSE_ERR_INVALID_ARG, "%s%zu: unknown op kind %d", phase, i, o.kind);
       }
       const bool push = !is_dec && o.push_skip;
       if (o.push_skip && (is_dec || phase[0] == 'm')) return fail(PULSE_ERR_SHAPE, "%s%zu: only encoder ops push skips", phase, i);
       op.out = pl.tensor(push ? R_SKIP : R_STASH, o.cout, op.hout, op.wout);
+      s->tensors[op.out].is_out = true;
       if (push) { op.push = (int)s->skip_tensor.size(); s->skip_tensor.push_back(op.out); stack.push_back(op.out); }
       cur = op.out;
       s->ops.push_back(op);
@@ -212,27 +203,47 @@ static pulse_status_t build_plan(pulse_stage* s) {
   if (!stack.empty()) return fail(PULSE_ERR_SHAPE, "%zu cached skips are never popped", stack.size());
   s->t_dout = cur;
 
-  // backward write modes: first writer of a gradient buffer stores, later writers add
+  // backward write modes: first writer of a gradient buffer stores, later writers add.  A gradient's pixel
+  // sums come fused from its writers when ALL of them are GroupNorm-backward launches (norm.cu); a gradient
+  // that enters from outside or is written by a conv / upsample adjoint gets a colsum pass instead.
   std::vector<char> written(s->tensors.size(), 0);
-  written[s->t_dout] = 1;
-  if (s->t_eout >= 0) written[s->t_eout] = 1;
+  written[s->t_dout] = 1; s->tensors[s->t_dout].cs_fused = false;
+  if (s->t_eout >= 0) { written[s->t_eout] = 1; s->tensors[s->t_eout].cs_fused = false; }
   for (int i = (int)s->ops.size() - 1; i >= 0; --i) {
     OpPlan& op = s->ops[i];
     op.acc_x0 = written[op.x0]; written[op.x0] = 1;
     if (op.x1 >= 0) { op.acc_x1 = written[op.x1]; written[op.x1] = 1; }
+    if (op.kind == PULSE_OP_CONV_IN || op.kind == PULSE_OP_DOWN || op.kind == PULSE_OP_UP)
+      s->tensors[op.x0].cs_fused = false;
     if ((op.kind == PULSE_OP_UP || op.kind == PULSE_OP_HEAD) && op.acc_x0)
       return fail(PULSE_ERR_UNSUPPORTED, "up/head input with a second consumer");
   }
 
-  s->gn_off = pl.bump(R_STASH, (size_t)s->gn_sites * gsz);
-  s->w_gb = pl.bump(R_WORK, (size_t)s->gn_sites * gsz);
+  // slot stash: channel stats of every tensor a GroupNorm reads, one contiguous area (zeroed per forward)
+  s->cst_begin = pl.bump(R_STASH, 0);
+  for (auto& t : s->tensors)
+    if (t.gn_input) t.cst = pl.bump(R_STASH, (size_t)d.n * 2 * t.ref.c * 4);
+  s->cst_end = pl.bump(R_STASH, 0);
   s->skip_bytes = pl.top[R_SKIP];
   s->stash_bytes = pl.top[R_STASH];
+  // workspace: backward sums, one contiguous area (zeroed per backward)
+  s->zero_begin = pl.bump(R_WORK, 0);
+  for (auto& t : s->tensors)
+    if (t.is_out) t.cs = pl.bump(R_WORK, (size_t)d.n * t.ref.c * 4);
+  for (auto& op : s->ops) {
+    if (op.kind == PULSE_OP_RESBLOCK) {
+      op.bst1 = pl.bump(R_WORK, (size_t)d.n * 2 * (op.cin + op.cskip) * 4);
+      op.bst2 = pl.bump(R_WORK, (size_t)d.n * 2 * op.cout * 4);
+      op.gp = pl.bump(R_WORK, (size_t)d.n * op.cout * 4);
+    } else if (op.kind == PULSE_OP_HEAD) {
+      op.bst1 = pl.bump(R_WORK, (size_t)d.n * 2 * op.cin * 4);
+    }
+  }
+  s->zero_end = pl.bump(R_WORK, 0);
   s->w_ga2 = pl.bump(R_WORK, m_out); s->w_gh1 = pl.bump(R_WORK, m_out);
   s->w_ga1 = pl.bump(R_WORK, m_cat); s->w_gsc = pl.bump(R_WORK, m_cat);
-  s->w_gu = pl.bump(R_WORK, m_gu); s->w_wt = pl.bump(R_WORK, m_w);
-  s->w_partial = pl.bump(R_WORK, m_partial + 1024); s->w_coef = pl.bump(R_WORK, m_coef + 256);
-  s->w_gp = pl.bump(R_WORK, m_gp + 256); s->w_tmpf = pl.bump(R_WORK, (size_t)d.n * T * 4 + 256);
+  s->w_gu = pl.bump(R_WORK, m_gu);
+  s->w_tmpf = pl.bump(R_WORK, (size_t)d.n * T * 4 + 256);
   s->work_bytes = pl.top[R_WORK];
   return PULSE_OK;
 }
@@ -294,6 +305,7 @@ extern "C" pulse_status_t pulse_stage_bind_params(pulse_stage_t* s, const void* 
   if (!s || !d_params || !d_grads) return fail(PULSE_ERR_INVALID_ARG, "null argument");
   if (!aligned256(d_params) || !aligned256(d_grads)) return fail(PULSE_ERR_INVALID_ARG, "buffers must be 256-byte aligned");
   s->d_params = (const char*)d_params; s->d_grads = d_grads;
+  s->wt_valid = false;
   return PULSE_OK;
 }
 extern "C" pulse_status_t pulse_stage_workspace_bytes(const pulse_stage_t* s, size_t* per_stage, size_t* per_inflight) {
@@ -308,6 +320,7 @@ extern "C" pulse_status_t pulse_stage_bind_workspace(pulse_stage_t* s, void* d, 
   const size_t need = s->work_bytes + (size_t)s->d.max_inflight * s->stash_bytes;
   if (bytes < need) return fail(PULSE_ERR_BUFFER_TOO_SMALL, "workspace %zu < %zu bytes", bytes, need);
   s->d_work = (char*)d; s->work_bound = bytes;
+  s->wt_valid = false;
   return PULSE_OK;
 }
 extern "C" pulse_status_t pulse_stage_launch_count(const pulse_stage_t* s, uint64_t* n) {

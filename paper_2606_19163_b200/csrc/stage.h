@@ -23,13 +23,17 @@ struct ParamInfo {
   size_t numel, off, goff;  // byte offsets into the param (stage dtype) / grad (fp32) buffers
 };
 
+constexpr size_t NO_OFF = (size_t)-1;
+
 struct OpPlan {
   int kind, cin, cskip, cout;
   int hin, win, hout, wout;
   int x0 = -1, x1 = -1, out = -1;           // indices into Stage::tensors (activations)
   int a1 = -1, h1 = -1, a2 = -1, u = -1;    // stashed intermediates
-  size_t stats1 = 0, stats2 = 0;            // byte offsets of the GroupNorm sites inside the gn regions
+  size_t bst1 = 0, bst2 = 0;                // R_WORK (zeroed area): GroupNorm backward sums [n][2][C] fp32 per site
+  size_t gp = 0;                            // R_WORK (zeroed area): [n][cout] fp32 pixel sums of g_h1
   size_t pn = 0;                            // byte offset in the slot stash ([n,cout] fp32)
+  size_t wt1 = 0, wt2 = 0, wtsc = 0;        // R_WORK: flipped/transposed conv weights (kept across a wave)
   int p[12];                                // parameter indices (see stage.cu)
   int push = -1, pop = -1;
   // backward write modes decided at plan time (0: '=', 1: '+=')
@@ -37,8 +41,13 @@ struct OpPlan {
 };
 
 struct Tensor {
-  TRef ref;          // forward value
-  size_t goff = 0;   // gradient buffer (R_WORK), same shape/dtype
+  TRef ref;              // forward value
+  size_t goff = 0;       // gradient buffer (R_WORK), same shape/dtype
+  bool gn_input = false; // read by a GroupNorm site: carries channel stats
+  size_t cst = NO_OFF;   // R_STASH (zeroed area): channel stats [n][2][c] fp32 of the forward value
+  bool is_out = false;   // output of an op with a bias: its gradient's pixel sums are needed
+  size_t cs = NO_OFF;    // R_WORK (zeroed area): [n][c] fp32 pixel sums of the gradient
+  bool cs_fused = true;  // every writer of the gradient emits its sums (else a colsum pass runs)
 };
 
 }  // namespace pulse
@@ -66,10 +75,11 @@ struct pulse_stage {
   int t_xin = -1, t_hin = -1, t_eout = -1, t_dout = -1;
   size_t skip_bytes = 0, stash_bytes = 0, work_bytes = 0;
   size_t emb_off = 0;                       // slot stash: copy of temb [n,T] fp32
-  int gn_sites = 0; size_t gn_site_bytes = 0, gn_off = 0, w_gb = 0;   // GroupNorm group sums (stash) / backward sums (work)
+  size_t cst_begin = 0, cst_end = 0;        // slot stash: channel-stats area, zeroed at the start of forward
+  size_t zero_begin = 0, zero_end = 0;      // workspace: backward sums area, zeroed at the start of backward
+  bool wt_valid = false;                    // transposed weights match the bound parameters
   // per-stage workspace offsets (bytes)
-  size_t w_ga2 = 0, w_gh1 = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_wt = 0, w_partial = 0, w_coef = 0, w_gp = 0,
-         w_tmpf = 0;
+  size_t w_ga2 = 0, w_gh1 = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0;
   const char* d_params = nullptr; float* d_grads = nullptr;
   char* d_work = nullptr; size_t work_bound = 0;
   uint64_t launches = 0;
