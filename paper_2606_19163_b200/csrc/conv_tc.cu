@@ -25,17 +25,17 @@
 #include "common.cuh"
 #include "kernels.h"
 #include "sm100.cuh"
+#include "tmap.h"
 
 namespace pulse {
 
 namespace {
 
 using namespace sm100;
+using namespace tmap;
 
 constexpr int BM = 128, BK = 64;
 constexpr int A_BYTES = BM * BK * 2;           // 16 KB
-
-struct Tap { int dx, dy, px, py, widx; };
 
 struct TcParams {
   int c0_blocks, c_blocks, ntaps, ctot, c0;
@@ -216,7 +216,11 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
   }
 }
 
+}  // namespace
+
 // ------------------------------------------------------------------------------ host: tensor maps
+namespace tmap {
+namespace {
 typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                              const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                              CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -235,17 +239,25 @@ bool init_driver() {
     return false;
   }
   g_encode = (EncodeFn)fn;
-  int dev = 0;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
   return true;
 }
+}  // namespace
 
-// bf16 tensor map, 128-byte swizzle; dims/box innermost first; strides (bytes) for dims 1..rank-1
+void set_error(const std::string& e) { g_tc_err = e; }
+int sm_count() {
+  if (!g_sms) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (g_sms <= 0) g_sms = 148;
+  }
+  return g_sms;
+}
+
 bool get_map(const void* ptr, int rank, const uint64_t* dims, const uint64_t* strides, const uint32_t* box,
-             CUtensorMap* out) {
+             CUtensorMap* out, int swizzle_bytes) {
   std::vector<uint64_t> key;
-  key.push_back((uint64_t)ptr); key.push_back(rank);
+  key.push_back((uint64_t)ptr); key.push_back(rank + 16 * (uint64_t)swizzle_bytes);
   for (int i = 0; i < rank; ++i) { key.push_back(dims[i]); key.push_back(box[i]); if (i) key.push_back(strides[i - 1]); }
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_maps.find(key);
@@ -255,7 +267,10 @@ bool get_map(const void* ptr, int rank, const uint64_t* dims, const uint64_t* st
   for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; es[i] = 1; if (i) gs[i - 1] = strides[i - 1]; }
   CUtensorMap m;
   CUresult r = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void*>(ptr), gd, gs, bx, es,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        swizzle_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
+                                             : (swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE),
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     g_tc_err = "cuTensorMapEncodeTiled failed with " + std::to_string((int)r);
@@ -267,39 +282,37 @@ bool get_map(const void* ptr, int rank, const uint64_t* dims, const uint64_t* st
   return true;
 }
 
-// NHWC activation [n,h,w,c] as a 4-D map (c, w, h, n) with box (64, bw, bh, bn)
 bool act_map(const void* ptr, int n, int h, int w, int c, int bw, int bh, int bn, CUtensorMap* out) {
   uint64_t dims[4] = {(uint64_t)c, (uint64_t)w, (uint64_t)h, (uint64_t)n};
   uint64_t str[3] = {(uint64_t)c * 2, (uint64_t)w * c * 2, (uint64_t)h * w * c * 2};
   uint32_t box[4] = {64, (uint32_t)bw, (uint32_t)bh, (uint32_t)bn};
   return get_map(ptr, 4, dims, str, box, out);
 }
-// stride-2 parity view (px*c + ch, x', py, y', n) of [n,h,w,c], box (64, bw, 1, bh, bn)
 bool act_map_s2(const void* ptr, int n, int h, int w, int c, int bw, int bh, int bn, CUtensorMap* out) {
   uint64_t dims[5] = {(uint64_t)2 * c, (uint64_t)w / 2, 2, (uint64_t)h / 2, (uint64_t)n};
   uint64_t str[4] = {(uint64_t)2 * c * 2, (uint64_t)w * c * 2, (uint64_t)2 * w * c * 2, (uint64_t)h * w * c * 2};
   uint32_t box[5] = {64, (uint32_t)bw, 1, (uint32_t)bh, (uint32_t)bn};
   return get_map(ptr, 5, dims, str, box, out);
 }
-// row-major [rows][k] matrix, box (64, brows)
 bool mat_map(const void* ptr, uint64_t rows, uint64_t k, int brows, CUtensorMap* out) {
   uint64_t dims[2] = {k, rows};
   uint64_t str[1] = {k * 2};
   uint32_t box[2] = {64, (uint32_t)brows};
   return get_map(ptr, 2, dims, str, box, out);
 }
-
-// pixel-grid tiling: bw = W (W | 128), then rows, then images
 bool tile_geometry(int gh, int gw, int& bw, int& bh, int& bn) {
   if (gw < 8 || gw > 128 || (gw & (gw - 1))) return false;
   bw = gw;
-  const int rows = BM / gw;
+  const int rows = 128 / gw;
   if (rows <= gh) { bh = rows; bn = 1; return true; }
-  if ((gh & (gh - 1)) || BM % (gh * gw)) return false;
-  bh = gh; bn = BM / (gh * gw);
+  if ((gh & (gh - 1)) || 128 % (gh * gw)) return false;
+  bh = gh; bn = 128 / (gh * gw);
   return true;
 }
+const std::string& last_error() { return g_tc_err; }
+}  // namespace tmap
 
+namespace {
 int pick_bn(int cout) { return cout % 160 == 0 ? 160 : (cout % 128 == 0 ? 128 : 0); }
 
 template <int BN>
@@ -307,20 +320,20 @@ bool launch(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, 
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(conv_tc_k<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<BN>::SMEM) != cudaSuccess) {
-      g_tc_err = "cudaFuncSetAttribute(max dynamic smem) failed";
+      tmap::set_error("cudaFuncSetAttribute(max dynamic smem) failed");
       return false;
     }
     attr_set = true;
   }
   const int tiles = p.tiles_mn * p.n_tiles;
-  const int grid = tiles < g_sms ? tiles : g_sms;
+  const int grid = tiles < sm_count() ? tiles : sm_count();
   conv_tc_k<BN><<<grid, 192, Cfg<BN>::SMEM, st>>>(a0, a1, b, p);
   return true;
 }
 
 }  // namespace
 
-const char* tc_last_error() { return g_tc_err.c_str(); }
+const char* tc_last_error() { return tmap::last_error().c_str(); }
 
 bool conv_tc_supported(const ConvArgs& a) {
   if (a.dt != DT_BF16) return false;
@@ -591,12 +604,13 @@ int wgrad_tc(const WgradArgs& a, cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(wgrad_tc_k, cudaFuncAttributeMaxDynamicSharedMemorySize, WG_SMEM) != cudaSuccess) {
-      g_tc_err = "cudaFuncSetAttribute(wgrad smem) failed";
+      tmap::set_error("cudaFuncSetAttribute(wgrad smem) failed");
       return -1;
     }
     attr_set = true;
   }
   const int out_tiles = p.m_tiles * p.n_tiles;
+  const int g_sms = sm_count();
   int splits = (g_sms + out_tiles - 1) / out_tiles;           // aim at >= one CTA per SM
   if (splits * out_tiles > 2 * g_sms && splits > 1) --splits;
   const int max_splits = (p.pix_tiles + 3) / 4;                // at least 4 pixel tiles per CTA

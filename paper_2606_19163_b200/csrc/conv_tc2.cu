@@ -1,0 +1,420 @@
+// conv_tc2.cu - CTA-pair (tcgen05 cta_group::2) implicit-GEMM convolution for sm_100a.
+//
+// Same GEMM view as conv_tc.cu (D[pixel, co] = sum_{tap, c} A[pixel shifted by tap, c] W[co][tap][c], TMA im2col
+// by coordinate shift with hardware zero fill, virtual concat by switching tensor maps inside the K loop), but the
+// tile is computed by TWO CTAs of a cluster on neighbouring SMs:
+//   pair tile   = 256 pixels x (NJ x UN) output channels; each CTA owns 128 of the pixels (its TMEM lanes),
+//   per K block = each CTA loads ITS 128 pixel rows of A and HALF of the weight rows of every UN-wide N slice;
+//                 one thread of the leader CTA issues tcgen05.mma.cta_group::2 (M = 256, N = UN), which reads A and
+//                 B from both CTAs' shared memory and accumulates into both CTAs' TMEM.
+// Why: the 128 x 160 single-CTA tile fetches 36.9 KB of operands per 2.6 MFLOP (71 FLOP/B) and its main loop is
+// bound by that operand feed (profiles/r01a_*: tensor pipe 51 % active).  The 256 x 320 pair tile fetches the same
+// 36.9 KB per CTA for twice the math (142 FLOP/B) and halves each CTA's shared-memory read traffic per MMA.
+//
+// Synchronisation (barriers live at the same shared-memory offsets in both CTAs):
+//   full[s]   (leader's copy)  1 arrival: the leader's producer arrive.expect_tx(bytes of BOTH CTAs); the TMA loads
+//                              of both CTAs complete_tx on it (cp.async.bulk.tensor ... cta_group::2),
+//   empty[s]  (own copy)       tcgen05.commit multicast to both CTAs when the MMAs reading stage s are done,
+//   tfull[a]  (own copy)       tcgen05.commit multicast when a tile's accumulator is complete,
+//   tempty[a] (leader's copy)  8 arrivals: the 4 epilogue warps of both CTAs (remote arrive from the peer).
+#include <cuda.h>
+
+#include <cstdlib>
+#include <cstring>
+
+#include "common.cuh"
+#include "kernels.h"
+#include "sm100.cuh"
+#include "tmap.h"
+
+namespace pulse {
+
+namespace {
+
+using namespace sm100;
+using namespace tmap;
+
+constexpr int BM = 128, BK = 64;
+constexpr int A_BYTES = BM * BK * 2;           // 16 KB
+
+struct Tc2Params {
+  int c0_blocks, c_blocks, ntaps, ctot, c0;
+  int s2;                         // 1: stride-2 fprop through the 5-D parity view
+  Tap taps[9];
+  int bw, bh, bn, tiles_h, tiles_m, pair_tiles_m, n_tiles;
+  int GH, GN;                     // pixel grid (rows, images); columns == bw
+  const bf16* bias; const float* pn; const bf16* residual; bf16* out; int accumulate;
+  int OH, OW, osy, osx, ooy, oox, cout_total;
+  int dbg;                        // microbenchmark modes (only compiled with -DPULSE_MB): 1 no MMA, 2 no TMA, 4 no stores
+};
+#ifdef PULSE_MB
+#define DBG(p) ((p).dbg)
+__device__ unsigned long long g_tl[64];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TL(i) do { if (blockIdx.x == 0) g_tl[i] = gtime(); } while (0)
+#else
+#define DBG(p) 0
+#define TL(i) do {} while (0)
+#endif
+
+template <int UN, int NJ> struct Cfg2 {
+  static constexpr int BN = UN * NJ;                       // output channels per pair tile
+  static constexpr int B_SLICE = (UN / 2) * BK * 2;        // this CTA's half of one UN-wide weight slice
+  static constexpr int STAGE_BYTES = A_BYTES + NJ * B_SLICE;
+  static constexpr int CW = BN % 64 == 0 ? 64 : 32;        // channels per epilogue chunk / TMA store box
+  static constexpr int BOX_BYTES = 32 * CW * 2;            // one warp's [32 pixels][CW channels] bf16
+  static constexpr int EPI_BYTES = 4 * (2 * BOX_BYTES + 2048);   // per epilogue warp: 2 boxes + column vector [BN] fp32
+  static constexpr int RING = 227 * 1024 - 256 - EPI_BYTES - 1024;       // what is left of the 227 KB for the operand ring
+  static constexpr int STAGES = RING / STAGE_BYTES > 8 ? 8 : RING / STAGE_BYTES;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_BYTES + 1024;
+  static constexpr int ACC = 2 * BN <= 512 ? 2 : 1;        // TMEM accumulator stages
+  static constexpr int TMEM_COLS = ACC * BN <= 256 ? 256 : 512;
+  static_assert(B_SLICE % 1024 == 0, "weight slices must keep the 1024-byte swizzle-atom alignment");
+  static_assert(UN % 16 == 0 && UN <= 256, "UMMA N for M = 256");
+};
+
+template <int UN, int NJ>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
+           const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CUtensorMap mapO, const Tc2Params p) {
+  using C = Cfg2<UN, NJ>;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t full_bar[C::STAGES], empty_bar[C::STAGES], tfull_bar[2], tempty_bar[2];
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int num_kb = p.ntaps * p.c_blocks;
+  const int total_tiles = p.pair_tiles_m * p.n_tiles;
+  const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+
+  if (threadIdx.x == 0) TL(0);
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB); prefetch_tmap(&mapO);
+    for (int i = 0; i < C::STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull_bar[i], 1); mbar_init(&tempty_bar[i], 8); }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc2(&tmem_base_s, C::TMEM_COLS);
+  tc_fence_before();
+  cluster_sync_all();          // the peer's barriers are initialised and its TMEM allocated before anyone signals
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+  if (threadIdx.x == 0) TL(1);
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // ===== TMA producer (both CTAs): own 128 pixel rows of A, own half of every weight slice =====
+      int stage = 0; uint32_t phase = 0;
+      for (int tile = pair; tile < total_tiles; tile += npairs) {
+        const int mp = tile / p.n_tiles, nt = tile - mp * p.n_tiles;
+        const int mt = 2 * mp + (int)rank;
+        const int n0 = (mt / p.tiles_h) * p.bn, y0 = (mt % p.tiles_h) * p.bh;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          const int ti = kb / p.c_blocks, cb = kb - ti * p.c_blocks;
+          const Tap t = p.taps[ti];
+          mbar_wait(&empty_bar[stage], phase ^ 1);
+          if (DBG(p) & 2) {
+            if (rank == 0) mbar_arrive(&full_bar[stage]);
+            if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
+            continue;
+          }
+          if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * C::STAGE_BYTES);
+          const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
+          uint8_t* sa = smem + stage * C::STAGE_BYTES;
+          const bool first = cb < p.c0_blocks;
+          const CUtensorMap* ma = first ? &mapA0 : &mapA1;
+          const int cch = (first ? cb : cb - p.c0_blocks) * BK;
+          if (!p.s2) tma2_load_4d(sa, ma, fb, cch, t.dx, y0 + t.dy, n0);
+          else tma2_load_5d(sa, ma, fb, t.px * p.c0 + cch, t.dx, t.py, y0 + t.dy, n0);
+          const int kcol = t.widx * p.ctot + cb * BK;
+#pragma unroll
+          for (int j = 0; j < NJ; ++j)
+            tma2_load_2d(sa + A_BYTES + j * C::B_SLICE, &mapB, fb, kcol, nt * C::BN + j * UN + (int)rank * (UN / 2));
+          if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (rank == 0 && lane == 0) {
+      // ===== MMA issuer (leader CTA only) =====
+      constexpr uint32_t idesc = idesc_bf16(2 * BM, UN, 0, 0);
+      constexpr uint64_t dbase = smem_desc_sw128(16, 1024);
+      int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
+      for (int tile = pair; tile < total_tiles; tile += npairs) {
+        mbar_wait(&tempty_bar[acc], acc_phase ^ 1);
+        tc_fence_after();
+        const uint32_t tmem_d = tmem_base + acc * C::BN;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          mbar_wait(&full_bar[stage], phase);
+          tc_fence_after();
+          if (kb == 0) TL(2);
+          if (kb == num_kb - 1) TL(3);
+          const uint32_t a_addr = smem_u32(smem + stage * C::STAGE_BYTES), b_addr = a_addr + A_BYTES;
+          if (!(DBG(p) & 1))
+#pragma unroll
+          for (int k = 0; k < BK / 16; ++k)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j)
+              umma2_bf16(tmem_d + j * UN, desc_with_addr(dbase, a_addr + k * 32),
+                         desc_with_addr(dbase, b_addr + j * C::B_SLICE + k * 32), idesc, (kb | k) != 0);
+          umma2_commit_mc(&empty_bar[stage], 3);
+          if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
+        }
+        umma2_commit_mc(&tfull_bar[acc], 3);
+        if (C::ACC == 2) { acc ^= 1; if (acc == 0) acc_phase ^= 1; }
+        else acc_phase ^= 1;
+      }
+    }
+  } else {
+    // ===== epilogue (both CTAs): warps 2..5 own TMEM lane quadrants (warp % 4) = 32 of this CTA's 128 pixels.
+    // Per 32-channel chunk: tcgen05.ld -> +bias +temb/residual -> bf16 -> this warp's staging buffer (64-byte
+    // swizzle, conflict-free) -> one TMA store of the [32 pixels][32 channels] box.  The store clips rows that fall
+    // outside the tensor (ragged tiles) and keeps the global writes as full 64-byte segments.
+    constexpr int CW = C::CW;
+    const int q = warp & 3;
+    const int row = q * 32 + lane;
+    const int n_l = row / (p.bh * p.bw), rem = row - n_l * (p.bh * p.bw);
+    const int y_l = rem / p.bw, x = rem - y_l * p.bw;
+    // box origin of this warp inside the tile (lane 0's pixel)
+    const int row0 = q * 32, n_w = row0 / (p.bh * p.bw), rem0 = row0 - n_w * (p.bh * p.bw);
+    const int y_w = rem0 / p.bw, x_w = rem0 - y_w * p.bw;
+    uint8_t* stg = smem + C::STAGES * C::STAGE_BYTES + q * (2 * C::BOX_BYTES + 2048);
+    float* colv = reinterpret_cast<float*>(stg + 2 * C::BOX_BYTES);      // [BN] bias (+ temb projection of this image)
+    const uint32_t stg_lane = smem_u32(stg) + lane * (CW * 2);
+    const int sw = CW == 64 ? (lane & 7) : ((lane >> 1) & 3);            // 128-byte / 64-byte swizzle of 16-byte pieces
+    int acc = 0, buf = 0; uint32_t acc_phase = 0;
+    for (int tile = pair; tile < total_tiles; tile += npairs) {
+      const int mp = tile / p.n_tiles, nt = tile - mp * p.n_tiles;
+      const int mt = 2 * mp + (int)rank;
+      const int n_t = (mt / p.tiles_h) * p.bn, y_t = (mt % p.tiles_h) * p.bh;
+      const int n = n_t + n_l, y = y_t + y_l;
+      const bool valid = mt < p.tiles_m && n < p.GN && y < p.GH;
+      const size_t off = (((size_t)n * p.OH + (size_t)y * p.osy + p.ooy) * p.OW + (size_t)x * p.osx + p.oox) *
+                             p.cout_total + (size_t)nt * C::BN;
+      const bf16* addend = p.residual ? p.residual : (p.accumulate ? p.out : nullptr);
+      {   // column vector of this warp's image, staged while the main loop runs
+        const int nw = min(n_t + n_w, p.GN - 1);
+        __syncwarp();
+        for (int c = lane; c < C::BN; c += 32) {
+          float t = p.bias ? to_f(p.bias[nt * C::BN + c]) : 0.f;
+          if (p.pn) t += p.pn[(size_t)nw * p.cout_total + nt * C::BN + c];
+          colv[c] = t;
+        }
+        __syncwarp();
+      }
+      mbar_wait(&tfull_bar[acc], acc_phase);
+      tc_fence_after();
+      if (warp == 2 && lane == 0) TL(4);
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * C::BN;
+#pragma unroll 1
+      for (int ch = 0; ch < C::BN / CW; ++ch) {
+        uint32_t r[CW];
+        tmem_ld32(taddr + ch * CW, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+        if (CW == 64) tmem_ld32(taddr + ch * CW + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[CW - 32]));
+        const int co = nt * C::BN + ch * CW;
+        tmem_ld_wait();
+        if (ch == C::BN / CW - 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&tempty_bar[acc]), 0));
+        }
+        if (!(DBG(p) & 4)) {
+          if (lane == 0) bulk_wait_read<1>();        // the store issued from this buffer two chunks ago has read it
+          __syncwarp();
+          const uint32_t dst = stg_lane + buf * C::BOX_BYTES;
+#pragma unroll
+          for (int i = 0; i < CW / 8; ++i) {
+            const float4 c0 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8);
+            const float4 c1 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8 + 4);
+            float v[8] = {__uint_as_float(r[i * 8]) + c0.x,     __uint_as_float(r[i * 8 + 1]) + c0.y,
+                          __uint_as_float(r[i * 8 + 2]) + c0.z, __uint_as_float(r[i * 8 + 3]) + c0.w,
+                          __uint_as_float(r[i * 8 + 4]) + c1.x, __uint_as_float(r[i * 8 + 5]) + c1.y,
+                          __uint_as_float(r[i * 8 + 6]) + c1.z, __uint_as_float(r[i * 8 + 7]) + c1.w};
+            if (addend && valid) {
+              float a8[8];
+              ldv(addend + off + ch * CW + i * 8, a8);
+#pragma unroll
+              for (int j = 0; j < 8; ++j) v[j] += a8[j];
+            }
+            st_shared_v4(dst + ((i ^ sw) << 4), pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
+                         pack_bf16(v[6], v[7]));
+          }
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            tma_store_4d(&mapO, stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
+            bulk_commit();
+          }
+          buf ^= 1;
+        }
+      }
+      if (C::ACC == 2) { acc ^= 1; if (acc == 0) acc_phase ^= 1; }
+      else acc_phase ^= 1;
+    }
+    if (lane == 0) bulk_wait<0>();
+  }
+  if (warp == 2 && lane == 0) TL(5);
+  tc_fence_before();
+  cluster_sync_all();          // nobody leaves (or frees TMEM) while the peer may still read its shared memory / TMEM
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc2(tmem_base, C::TMEM_COLS);
+  }
+  if (threadIdx.x == 32) TL(6);
+}
+#ifdef PULSE_MB
+}  // namespace
+void mb_timeline(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tl, sizeof(unsigned long long) * 8); }
+namespace {
+#endif
+
+template <int UN, int NJ>
+bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const CUtensorMap& o, const Tc2Params& p,
+             cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(conv_tc2_k<UN, NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg2<UN, NJ>::SMEM) !=
+        cudaSuccess) {
+      tmap::set_error("cudaFuncSetAttribute(max dynamic smem) failed for conv_tc2_k");
+      return false;
+    }
+    attr_set = true;
+  }
+  const int tiles = p.pair_tiles_m * p.n_tiles;
+  const int max_pairs = sm_count() / 2;
+  const int pairs = tiles < max_pairs ? tiles : max_pairs;
+  conv_tc2_k<UN, NJ><<<2 * pairs, 192, Cfg2<UN, NJ>::SMEM, st>>>(a0, a1, b, o, p);
+  return true;
+}
+
+// (UN, NJ) for a channel count: 320 k -> 2 x 160; 160 k -> 1 x 160; 256 k -> 2 x 128; 128 k -> 1 x 128
+void pick_tile(int cout, int& un, int& nj) {
+  un = nj = 0;
+#ifdef PULSE_MB
+  if (getenv("PULSE_NJ1") && cout % 160 == 0) { un = 160; nj = 1; return; }
+#endif
+  if (cout % 320 == 0) { un = 160; nj = 2; }
+  else if (cout % 160 == 0) { un = 160; nj = 1; }
+  else if (cout % 256 == 0) { un = 128; nj = 2; }
+  else if (cout % 128 == 0) { un = 128; nj = 1; }
+}
+
+}  // namespace
+
+bool conv_tc2_supported(const ConvArgs& a) {
+  if (a.dt != DT_BF16) return false;
+  if (a.src.c0 % 64 || a.src.c1 % 64 || a.src.c0 == 0) return false;
+  int un, nj;
+  pick_tile(a.cout, un, nj);
+  if (!un) return false;
+  if (a.ksize != 1 && a.ksize != 3) return false;
+  int bw, bh, bn;
+  if (a.mode == CONV_DGRAD_S2) {
+    if (a.ksize != 3 || a.src.c1) return false;
+    if (a.hout != 2 * a.hin || a.wout != 2 * a.win) return false;
+    return tile_geometry(a.hin, a.win, bw, bh, bn) && bw * bh >= 32;
+  }
+  if (a.stride == 2) {
+    if (a.ksize != 3 || a.src.c1 || (a.hin & 1) || (a.win & 1) || a.hout * 2 != a.hin || a.wout * 2 != a.win) return false;
+  } else if (a.stride != 1 || a.hout != a.hin || a.wout != a.win) {
+    return false;
+  }
+  return tile_geometry(a.hout, a.wout, bw, bh, bn) && bw * bh >= 32;      // a warp's 32 pixels lie inside one image
+}
+
+int conv_tc2(const ConvArgs& a, cudaStream_t st) {
+  Tc2Params p;
+  memset(&p, 0, sizeof p);
+  int un, nj;
+  pick_tile(a.cout, un, nj);
+  const bool s2d = a.mode == CONV_DGRAD_S2, s2f = !s2d && a.stride == 2;
+  const int gh = s2d ? a.hin : a.hout, gw = s2d ? a.win : a.wout;
+  tile_geometry(gh, gw, p.bw, p.bh, p.bn);
+  p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64;
+  p.s2 = s2f;
+  p.tiles_h = (gh + p.bh - 1) / p.bh;
+  p.tiles_m = p.tiles_h * ((a.n + p.bn - 1) / p.bn);
+  p.pair_tiles_m = (p.tiles_m + 1) / 2;
+  p.n_tiles = a.cout / (un * nj);
+  p.GH = gh; p.GN = a.n;
+  p.bias = (const bf16*)a.bias; p.pn = a.pn; p.residual = (const bf16*)a.residual; p.out = (bf16*)a.out;
+  p.accumulate = a.accumulate;
+#ifdef PULSE_MB
+  { const char* e = getenv("PULSE_DBG"); p.dbg = e ? atoi(e) : 0; }
+#endif
+  p.OH = a.hout; p.OW = a.wout; p.osy = p.osx = 1; p.ooy = p.oox = 0; p.cout_total = a.cout;
+  CUtensorMap m0, m1, mb;
+  bool ok = true;
+  if (s2f) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  m1 = m0;
+  if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
+  if (ok) ok = mat_map(a.w, a.cout, (uint64_t)a.ksize * a.ksize * p.ctot, un / 2, &mb);
+  if (!ok) return -1;
+  int launches = 0;
+  auto go = [&]() {
+    // output view of this launch: (c, x, y, n) with pixel strides osx/osy from pixel (ooy, oox); box = one warp's
+    // [32 pixels][32 channels], 64-byte swizzle
+    CUtensorMap mo;
+    {
+      const int bwb = p.bw < 32 ? p.bw : 32, bhb = 32 / bwb;
+      const size_t C2 = (size_t)a.cout * 2;
+      uint64_t dims[4] = {(uint64_t)a.cout, (uint64_t)gw, (uint64_t)gh, (uint64_t)a.n};
+      uint64_t str[3] = {(uint64_t)p.osx * C2, (uint64_t)p.osy * a.wout * C2, (uint64_t)a.hout * a.wout * C2};
+      const uint32_t cw = (un * nj) % 64 == 0 ? 64 : 32;
+      uint32_t box[4] = {cw, (uint32_t)bwb, (uint32_t)bhb, 1};
+      const char* base = (const char*)a.out + ((size_t)p.ooy * a.wout + p.oox) * C2;
+      if (!get_map(base, 4, dims, str, box, &mo, 2 * (int)cw)) return false;
+    }
+    bool r = un == 160 ? (nj == 2 ? launch2<160, 2>(m0, m1, mb, mo, p, st) : launch2<160, 1>(m0, m1, mb, mo, p, st))
+                       : (nj == 2 ? launch2<128, 2>(m0, m1, mb, mo, p, st) : launch2<128, 1>(m0, m1, mb, mo, p, st));
+    if (r) ++launches;
+    return r;
+  };
+  if (s2d) {
+    // output pixel (2y'+py, 2x'+px) <- taps r' with (py + r' - 1) even: py=0: r'=1 (dy 0); py=1: r'=0 (dy 0), r'=2 (dy +1)
+    p.osy = p.osx = 2;
+    for (int py = 0; py < 2; ++py)
+      for (int px = 0; px < 2; ++px) {
+        p.ooy = py; p.oox = px; p.ntaps = 0;
+        for (int r = 0; r < 3; ++r) {
+          if ((py + r - 1) & 1) continue;
+          for (int s = 0; s < 3; ++s) {
+            if ((px + s - 1) & 1) continue;
+            Tap t; t.dy = (py + r - 1) >> 1; t.dx = (px + s - 1) >> 1; t.px = t.py = 0; t.widx = r * 3 + s;
+            p.taps[p.ntaps++] = t;
+          }
+        }
+        if (!go()) return -1;
+      }
+    return launches;
+  }
+  const int pad = (a.ksize - 1) / 2;
+  p.ntaps = a.ksize * a.ksize;
+  for (int r = 0; r < a.ksize; ++r)
+    for (int s = 0; s < a.ksize; ++s) {
+      Tap t; t.widx = r * a.ksize + s; t.px = t.py = 0;
+      if (!s2f) { t.dy = r - pad; t.dx = s - pad; }
+      else {   // input row 2y + r - 1 = 2(y + dy) + py
+        t.dy = r == 0 ? -1 : 0; t.py = r == 1 ? 0 : 1;
+        t.dx = s == 0 ? -1 : 0; t.px = s == 1 ? 0 : 1;
+      }
+      p.taps[t.widx] = t;
+    }
+  if (!go()) return -1;
+  return launches;
+}
+
+static bool force_1cta() {
+  static int v = -1;
+  if (v < 0) { const char* e = getenv("PULSE_CONV_1CTA"); v = (e && e[0] == '1') ? 1 : 0; }
+  return v == 1;
+}
+bool conv_tc_any_supported(const ConvArgs& a) { return conv_tc2_supported(a) || conv_tc_supported(a); }
+int conv_tc_any(const ConvArgs& a, cudaStream_t st) {
+  if (!force_1cta() && conv_tc2_supported(a)) return conv_tc2(a, st);
+  return conv_tc(a, st);
+}
+
+}  // namespace pulse

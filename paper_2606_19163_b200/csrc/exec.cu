@@ -56,9 +56,9 @@ double conv_flops(const ConvArgs& a) {
   return 2.0 * mpix * a.cout * a.src.c() * a.ksize * a.ksize;     // the s2 dgrad phases execute exactly 9/4 taps per output
 }
 void run_conv(Ctx& c, const ConvArgs& a) {
-  const bool tc = c.tc() && conv_tc_supported(a);
+  const bool tc = c.tc() && conv_tc_any_supported(a);
   Prof pr(c.s, c.st, tc ? PULSE_KCLASS_CONV_TC : PULSE_KCLASS_CONV_SIMT, conv_flops(a), 0.0);
-  const int r = tc ? conv_tc(a, c.st) : conv_simt(a, c.st);
+  const int r = tc ? conv_tc_any(a, c.st) : conv_simt(a, c.st);
   if (r < 0) c.err = true; else c.s->launches += r;
 }
 void run_wgrad(Ctx& c, const WgradArgs& a) {
@@ -498,7 +498,7 @@ extern "C" pulse_status_t pulse_conv2d(int dtype, int force_simt, const void* d_
   a.dt = dtype == PULSE_F32 ? DT_F32 : DT_BF16; a.src = Cat{d_src0, c0, d_src1, c1}; a.n = n; a.hin = h; a.win = w;
   a.hout = h / stride; a.wout = w / stride; a.ksize = ksize; a.stride = stride; a.mode = CONV_FPROP; a.w = d_w;
   a.cout = cout; a.bias = d_bias; a.pn = d_pn; a.residual = d_residual; a.out = d_out; a.accumulate = 0;
-  const int r = (!force_simt && conv_tc_supported(a)) ? conv_tc(a, (cudaStream_t)stream) : conv_simt(a, (cudaStream_t)stream);
+  const int r = (!force_simt && conv_tc_any_supported(a)) ? conv_tc_any(a, (cudaStream_t)stream) : conv_simt(a, (cudaStream_t)stream);
   if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
@@ -516,7 +516,7 @@ extern "C" pulse_status_t pulse_conv2d_dgrad(int dtype, int force_simt, const vo
   a.dt = dt; a.src = Cat{d_g, cout, nullptr, 0}; a.n = n; a.hin = h / stride; a.win = w / stride; a.hout = h; a.wout = w;
   a.ksize = ksize; a.stride = 1; a.mode = stride == 2 ? CONV_DGRAD_S2 : CONV_FPROP; a.w = d_wt; a.cout = cin;
   a.bias = nullptr; a.pn = nullptr; a.residual = nullptr; a.out = d_g_in; a.accumulate = accumulate;
-  const int r = (!force_simt && conv_tc_supported(a)) ? conv_tc(a, st) : conv_simt(a, st);
+  const int r = (!force_simt && conv_tc_any_supported(a)) ? conv_tc_any(a, st) : conv_simt(a, st);
   if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;

@@ -98,6 +98,12 @@ int wgrad_simt(const WgradArgs& a, cudaStream_t st);
 // tcgen05 / TMA path (bf16 only).  *_supported say whether the shape maps onto the tiles.
 bool conv_tc_supported(const ConvArgs& a);
 int conv_tc(const ConvArgs& a, cudaStream_t st);
+// CTA-pair (cta_group::2) variant, 256-pixel x 320-channel tiles (conv_tc2.cu); preferred where it applies
+bool conv_tc2_supported(const ConvArgs& a);
+int conv_tc2(const ConvArgs& a, cudaStream_t st);
+// picks conv_tc2, else conv_tc; returns false if neither applies.  PULSE_CONV_1CTA=1 forces the single-CTA kernel.
+bool conv_tc_any_supported(const ConvArgs& a);
+int conv_tc_any(const ConvArgs& a, cudaStream_t st);
 bool wgrad_tc_supported(const WgradArgs& a);
 int wgrad_tc(const WgradArgs& a, cudaStream_t st);
 const char* tc_last_error();
