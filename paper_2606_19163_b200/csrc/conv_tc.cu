@@ -310,6 +310,24 @@ bool tile_geometry(int gh, int gw, int& bw, int& bh, int& bn) {
   return true;
 }
 const std::string& last_error() { return g_tc_err; }
+// 64-pixel tiles of an [n, gh, gw] grid (wgrad K blocks)
+bool tile_geometry64(int gh, int gw, int& bw, int& bh, int& bn) {
+  if (gw < 8 || (gw & (gw - 1))) return false;
+  if (gw >= 64) { bw = 64; bh = 1; bn = 1; return gw % 64 == 0 && gw <= 256; }
+  bw = gw;
+  const int rows = 64 / gw;
+  if (rows <= gh) { bh = rows; bn = 1; return true; }
+  if ((gh & (gh - 1)) || 64 % (gh * gw)) return false;
+  bh = gh; bn = 64 / (gh * gw);
+  return true;
+}
+// NHWC activation as (c, w, h, n) with a (cbox, bw, bh, bn) box; swizzle = 2 * cbox bytes
+bool act_map_c(const void* ptr, int n, int h, int w, int c, int cbox, int bw, int bh, int bn, CUtensorMap* out) {
+  uint64_t dims[4] = {(uint64_t)c, (uint64_t)w, (uint64_t)h, (uint64_t)n};
+  uint64_t str[3] = {(uint64_t)c * 2, (uint64_t)w * c * 2, (uint64_t)h * w * c * 2};
+  uint32_t box[4] = {(uint32_t)cbox, (uint32_t)bw, (uint32_t)bh, (uint32_t)bn};
+  return get_map(ptr, 4, dims, str, box, out, 2 * cbox);
+}
 }  // namespace tmap
 
 namespace {
@@ -439,28 +457,29 @@ struct WgParams {
   int units, c_blocks, c0_blocks, c0, ctot, ktot, s2;
   Tap taps[9];
   int bw, bh, bn, tiles_w, tiles_h;
-  int pix_tiles, pt_per_split, m_tiles, n_tiles;
+  int pix_tiles, m_tiles, n_tiles;
+  long long work;          // m_tiles * n_tiles * pix_tiles work items of (128 rows x 320 cols x 64 pixels)
   float* dw;
 };
 
+// Work distribution ("stream-K"): the work items, ordered (output tile, pixel tile), are cut into gridDim.x equal
+// contiguous ranges, so every SM gets the same number of MMAs whatever the number of output tiles is (23 or 45 for
+// the config-2 shapes: any whole-tile split leaves a ragged second wave).  A range that crosses an output-tile
+// boundary flushes its accumulator (fp32 red.add into dW) and starts the next tile.
 __global__ void __launch_bounds__(192, 1)
 wgrad_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
            const __grid_constant__ CUtensorMap mapG, const WgParams p) {
   extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t full_bar[WG_STAGES], empty_bar[WG_STAGES], tfull_bar;
+  __shared__ uint64_t full_bar[WG_STAGES], empty_bar[WG_STAGES], tfull_bar, tempty_bar;
   __shared__ uint32_t tmem_base_s;
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int nt = blockIdx.x % p.n_tiles;
-  const int mt = (blockIdx.x / p.n_tiles) % p.m_tiles;
-  const int split = blockIdx.x / (p.n_tiles * p.m_tiles);
-  const int pt_begin = split * p.pt_per_split;
-  const int pt_end = min(p.pix_tiles, pt_begin + p.pt_per_split);
+  const long long wb = p.work * blockIdx.x / gridDim.x, we = p.work * (blockIdx.x + 1) / gridDim.x;
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapG);
     for (int i = 0; i < WG_STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
-    mbar_init(&tfull_bar, 1);
+    mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 4);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(&tmem_base_s, 512);
@@ -468,12 +487,14 @@ wgrad_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
-  const int u0 = 2 * mt, u1 = min(u0 + 1, p.units - 1);
 
   if (warp == 0) {
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      for (int pt = pt_begin; pt < pt_end; ++pt) {
+      for (long long w = wb; w < we; ++w) {
+        const int ot = (int)(w / p.pix_tiles), pt = (int)(w - (long long)ot * p.pix_tiles);
+        const int nt = ot % p.n_tiles, mt = ot / p.n_tiles;
+        const int u0 = 2 * mt, u1 = min(u0 + 1, p.units - 1);
         const int tx = pt % p.tiles_w, ty = (pt / p.tiles_w) % p.tiles_h, tn = pt / (p.tiles_w * p.tiles_h);
         const int x0 = tx * p.bw, y0 = ty * p.bh, n0 = tn * p.bn;
         mbar_wait(&empty_bar[stage], phase ^ 1);
@@ -500,43 +521,69 @@ wgrad_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
     if (lane == 0) {
       constexpr uint32_t idesc128 = idesc_bf16(128, 128, 1, 1), idesc192 = idesc_bf16(128, 192, 1, 1);
       constexpr uint64_t dbase = smem_desc_sw128(WG_BLK, 1024);      // MN-major: LBO = next 64-channel block
-      int stage = 0; uint32_t phase = 0;
-      for (int pt = pt_begin; pt < pt_end; ++pt) {
+      int stage = 0; uint32_t phase = 0, tphase = 0;
+      bool fresh = true;
+      for (long long w = wb; w < we; ++w) {
+        const int pt = (int)(w % p.pix_tiles);
+        if (fresh) {                       // new output tile: the epilogue must have drained the accumulator
+          mbar_wait(&tempty_bar, tphase ^ 1);
+          tc_fence_after();
+        }
         mbar_wait(&full_bar[stage], phase);
         tc_fence_after();
         const uint32_t a_addr = smem_u32(smem + stage * WG_STAGE), b_addr = a_addr + 2 * WG_BLK;
 #pragma unroll
         for (int k = 0; k < WG_PIX / 16; ++k) {
-          const uint32_t acc = (pt != pt_begin || k != 0);
+          const uint32_t acc = (!fresh || k != 0);
           const uint64_t da = desc_with_addr(dbase, a_addr + k * 2048);
           umma_bf16(tmem_base, da, desc_with_addr(dbase, b_addr + k * 2048), idesc128, acc);
           umma_bf16(tmem_base + 128, da, desc_with_addr(dbase, b_addr + 2 * WG_BLK + k * 2048), idesc192, acc);
         }
         umma_commit(&empty_bar[stage]);
         if (++stage == WG_STAGES) { stage = 0; phase ^= 1; }
+        fresh = false;
+        if (pt == p.pix_tiles - 1 || w == we - 1) {      // end of this CTA's share of the output tile
+          umma_commit(&tfull_bar);
+          tphase ^= 1;
+          fresh = true;
+        }
       }
-      umma_commit(&tfull_bar);
     }
-  } else if (pt_end > pt_begin) {
+  } else {
     const int q = warp & 3;
     const int row = q * 32 + lane;
-    const int u = u0 + (row >> 6);
-    const bool valid = u < p.units && (row < 64 || u0 + 1 < p.units);
-    const int ti = valid ? u / p.c_blocks : 0, cb = valid ? u - ti * p.c_blocks : 0;
-    const size_t kidx = (size_t)p.taps[ti].widx * p.ctot + cb * 64 + (row & 63);
-    mbar_wait(&tfull_bar, 0);
-    tc_fence_after();
-    const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+    uint32_t tphase = 0;
+    long long w = wb;
+    while (w < we) {
+      const int ot = (int)(w / p.pix_tiles);
+      const long long seg_end = min(we, (long long)(ot + 1) * p.pix_tiles);
+      const int nt = ot % p.n_tiles, mt = ot / p.n_tiles;
+      const int u0 = 2 * mt;
+      const int u = u0 + (row >> 6);
+      const bool valid = u < p.units;
+      const int ti = valid ? u / p.c_blocks : 0, cb = valid ? u - ti * p.c_blocks : 0;
+      const size_t kidx = (size_t)p.taps[ti].widx * p.ctot + cb * 64 + (row & 63);
+      mbar_wait(&tfull_bar, tphase);
+      tphase ^= 1;
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
 #pragma unroll 1
-    for (int ch = 0; ch < WG_N / 32; ++ch) {
-      uint32_t r[32];
-      tmem_ld32(taddr + ch * 32, r);
-      tmem_ld_wait();
-      if (valid) {
-        float* dst = p.dw + (size_t)(nt * WG_N + ch * 32) * p.ktot + kidx;
+      for (int ch = 0; ch < WG_N / 32; ++ch) {
+        uint32_t r[32];
+        tmem_ld32(taddr + ch * 32, r);
+        tmem_ld_wait();
+        if (ch == WG_N / 32 - 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&tempty_bar);
+        }
+        if (valid) {
+          float* dst = p.dw + (size_t)(nt * WG_N + ch * 32) * p.ktot + kidx;
 #pragma unroll
-        for (int i = 0; i < 32; ++i) atomicAdd(dst + (size_t)i * p.ktot, __uint_as_float(r[i]));
+          for (int i = 0; i < 32; ++i) atomicAdd(dst + (size_t)i * p.ktot, __uint_as_float(r[i]));
+        }
       }
+      w = seg_end;
     }
   }
   tc_fence_before();
@@ -545,18 +592,6 @@ wgrad_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
     tc_fence_after();
     tmem_dealloc(tmem_base, 512);
   }
-}
-
-// 64-pixel tiles of an [n, gh, gw] grid
-bool wg_geometry(int gh, int gw, int& bw, int& bh, int& bn) {
-  if (gw < 8 || (gw & (gw - 1))) return false;
-  if (gw >= WG_PIX) { bw = WG_PIX; bh = 1; bn = 1; return gw % WG_PIX == 0 && gw <= 256; }
-  bw = gw;
-  const int rows = WG_PIX / gw;
-  if (rows <= gh) { bh = rows; bn = 1; return true; }
-  if ((gh & (gh - 1)) || WG_PIX % (gh * gw)) return false;
-  bh = gh; bn = WG_PIX / (gh * gw);
-  return true;
 }
 
 }  // namespace
@@ -571,14 +606,14 @@ bool wgrad_tc_supported(const WgradArgs& a) {
     return false;
   }
   int bw, bh, bn;
-  return wg_geometry(a.hout, a.wout, bw, bh, bn);
+  return tile_geometry64(a.hout, a.wout, bw, bh, bn);
 }
 
 int wgrad_tc(const WgradArgs& a, cudaStream_t st) {
   WgParams p;
   memset(&p, 0, sizeof p);
   const bool s2 = a.stride == 2;
-  wg_geometry(a.hout, a.wout, p.bw, p.bh, p.bn);
+  tile_geometry64(a.hout, a.wout, p.bw, p.bh, p.bn);
   p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64; p.s2 = s2;
   const int taps = a.ksize * a.ksize, pad = (a.ksize - 1) / 2;
   p.units = taps * p.c_blocks; p.ktot = taps * p.ctot;
@@ -609,16 +644,11 @@ int wgrad_tc(const WgradArgs& a, cudaStream_t st) {
     }
     attr_set = true;
   }
-  const int out_tiles = p.m_tiles * p.n_tiles;
-  const int g_sms = sm_count();
-  int splits = (g_sms + out_tiles - 1) / out_tiles;           // aim at >= one CTA per SM
-  if (splits * out_tiles > 2 * g_sms && splits > 1) --splits;
-  const int max_splits = (p.pix_tiles + 3) / 4;                // at least 4 pixel tiles per CTA
-  if (splits > max_splits) splits = max_splits;
-  if (splits < 1) splits = 1;
-  p.pt_per_split = (p.pix_tiles + splits - 1) / splits;
-  splits = (p.pix_tiles + p.pt_per_split - 1) / p.pt_per_split;
-  wgrad_tc_k<<<out_tiles * splits, 192, WG_SMEM, st>>>(m0, m1, mg, p);
+  p.work = (long long)p.m_tiles * p.n_tiles * p.pix_tiles;
+  // one CTA per SM, each with an equal share of the work items (at least 4 per CTA)
+  long long ctas = sm_count();
+  if (p.work / 4 < ctas) ctas = p.work / 4 > 0 ? p.work / 4 : 1;
+  wgrad_tc_k<<<(unsigned)ctas, 192, WG_SMEM, st>>>(m0, m1, mg, p);
   return 1;
 }
 

@@ -51,7 +51,7 @@ struct Tc2Params {
 #define DBG(p) ((p).dbg)
 __device__ unsigned long long g_tl[64];
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TL(i) do { if (blockIdx.x == 0) g_tl[i] = gtime(); } while (0)
+#define TL(i) do { if (blockIdx.x == 0) { g_tl[i] = gtime(); g_tl[32 + i] = clock64(); } } while (0)
 #else
 #define DBG(p) 0
 #define TL(i) do {} while (0)
@@ -136,10 +136,12 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       }
     }
   } else if (warp == 1) {
-    if (rank == 0 && lane == 0) {
-      // ===== MMA issuer (leader CTA only) =====
+    if (rank == 0) {
+      // ===== MMA issuer (leader CTA only): the whole warp runs the loop, one elected lane issues =====
       constexpr uint32_t idesc = idesc_bf16(2 * BM, UN, 0, 0);
       constexpr uint64_t dbase = smem_desc_sw128(16, 1024);
+      constexpr uint32_t desc_hi = (uint32_t)(dbase >> 32);
+      const uint32_t desc_lo0 = (uint32_t)dbase | ((smem_u32(smem) >> 4) & 0x3FFF);     // smem is 1024-aligned: no carry
       int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
       for (int tile = pair; tile < total_tiles; tile += npairs) {
         mbar_wait(&tempty_bar[acc], acc_phase ^ 1);
@@ -150,18 +152,22 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           tc_fence_after();
           if (kb == 0) TL(2);
           if (kb == num_kb - 1) TL(3);
-          const uint32_t a_addr = smem_u32(smem + stage * C::STAGE_BYTES), b_addr = a_addr + A_BYTES;
-          if (!(DBG(p) & 1))
+          const uint32_t a_lo = desc_lo0 + stage * (C::STAGE_BYTES >> 4), b_lo = a_lo + (A_BYTES >> 4);
+          if (elect_one_sync()) {
+            if (!(DBG(p) & 1)) {
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k)
+              for (int k = 0; k < BK / 16; ++k)
 #pragma unroll
-            for (int j = 0; j < NJ; ++j)
-              umma2_bf16(tmem_d + j * UN, desc_with_addr(dbase, a_addr + k * 32),
-                         desc_with_addr(dbase, b_addr + j * C::B_SLICE + k * 32), idesc, (kb | k) != 0);
-          umma2_commit_mc(&empty_bar[stage], 3);
+                for (int j = 0; j < NJ; ++j)
+                  umma2_bf16(tmem_d + j * UN, ((uint64_t)desc_hi << 32) | (a_lo + 2 * k),
+                             ((uint64_t)desc_hi << 32) | (b_lo + j * (C::B_SLICE >> 4) + 2 * k), idesc, (kb | k) != 0);
+            }
+            umma2_commit_mc(&empty_bar[stage], 3);
+            if (kb == num_kb - 1) umma2_commit_mc(&tfull_bar[acc], 3);
+          }
+          __syncwarp();
           if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
         }
-        umma2_commit_mc(&tfull_bar[acc], 3);
         if (C::ACC == 2) { acc ^= 1; if (acc == 0) acc_phase ^= 1; }
         else acc_phase ^= 1;
       }
@@ -265,7 +271,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
 }
 #ifdef PULSE_MB
 }  // namespace
-void mb_timeline(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tl, sizeof(unsigned long long) * 8); }
+void mb_timeline(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tl, sizeof(unsigned long long) * 64); }
 namespace {
 #endif
 
@@ -293,6 +299,7 @@ void pick_tile(int cout, int& un, int& nj) {
   un = nj = 0;
 #ifdef PULSE_MB
   if (getenv("PULSE_NJ1") && cout % 160 == 0) { un = 160; nj = 1; return; }
+  if (getenv("PULSE_UN256") && cout % 256 == 0) { un = 256; nj = 1; return; }
 #endif
   if (cout % 320 == 0) { un = 160; nj = 2; }
   else if (cout % 160 == 0) { un = 160; nj = 1; }
@@ -367,6 +374,9 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
       const char* base = (const char*)a.out + ((size_t)p.ooy * a.wout + p.oox) * C2;
       if (!get_map(base, 4, dims, str, box, &mo, 2 * (int)cw)) return false;
     }
+#ifdef PULSE_MB
+    if (un == 256) { bool r2 = launch2<256, 1>(m0, m1, mb, mo, p, st); if (r2) ++launches; return r2; }
+#endif
     bool r = un == 160 ? (nj == 2 ? launch2<160, 2>(m0, m1, mb, mo, p, st) : launch2<160, 1>(m0, m1, mb, mo, p, st))
                        : (nj == 2 ? launch2<128, 2>(m0, m1, mb, mo, p, st) : launch2<128, 1>(m0, m1, mb, mo, p, st));
     if (r) ++launches;

@@ -62,10 +62,10 @@ void run_conv(Ctx& c, const ConvArgs& a) {
   if (r < 0) c.err = true; else c.s->launches += r;
 }
 void run_wgrad(Ctx& c, const WgradArgs& a) {
-  const bool tc = c.tc() && wgrad_tc_supported(a);
+  const bool tc = c.tc() && wgrad_tc_any_supported(a);
   Prof pr(c.s, c.st, tc ? PULSE_KCLASS_WGRAD_TC : PULSE_KCLASS_CONV_SIMT,
           2.0 * a.n * a.hout * a.wout * a.cout * a.src.c() * a.ksize * a.ksize, 0.0);
-  const int r = tc ? wgrad_tc(a, c.st) : wgrad_simt(a, c.st);
+  const int r = tc ? wgrad_tc_any(a, c.st) : wgrad_simt(a, c.st);
   if (r < 0) c.err = true; else c.s->launches += r;
 }
 // GroupNorm+SiLU wrappers: algorithmic bytes 2 x esz per element forward, 3 x esz backward
@@ -529,7 +529,7 @@ extern "C" pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const vo
   if (!d_src0 || !d_g || !d_dw || (c1 && !d_src1)) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
   WgradArgs a{dtype == PULSE_F32 ? DT_F32 : DT_BF16, Cat{d_src0, c0, d_src1, c1}, n, h, w, d_g, h / stride, w / stride,
               cout, ksize, stride, d_dw};
-  const int r = (!force_simt && wgrad_tc_supported(a)) ? wgrad_tc(a, (cudaStream_t)stream) : wgrad_simt(a, (cudaStream_t)stream);
+  const int r = (!force_simt && wgrad_tc_any_supported(a)) ? wgrad_tc_any(a, (cudaStream_t)stream) : wgrad_simt(a, (cudaStream_t)stream);
   if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core wgrad launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;

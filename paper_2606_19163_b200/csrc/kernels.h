@@ -106,6 +106,10 @@ bool conv_tc_any_supported(const ConvArgs& a);
 int conv_tc_any(const ConvArgs& a, cudaStream_t st);
 bool wgrad_tc_supported(const WgradArgs& a);
 int wgrad_tc(const WgradArgs& a, cudaStream_t st);
+bool wgrad_tc2_supported(const WgradArgs& a);      // CTA-pair variant (wgrad_tc2.cu), preferred where it applies
+int wgrad_tc2(const WgradArgs& a, cudaStream_t st);
+bool wgrad_tc_any_supported(const WgradArgs& a);   // PULSE_WGRAD_1CTA=1 forces the single-CTA kernel
+int wgrad_tc_any(const WgradArgs& a, cudaStream_t st);
 const char* tc_last_error();
 
 }  // namespace pulse

@@ -21,6 +21,8 @@ bool act_map_s2(const void* ptr, int n, int h, int w, int c, int bw, int bh, int
 bool mat_map(const void* ptr, uint64_t rows, uint64_t k, int brows, CUtensorMap* out);
 // pixel-grid tiling of 128 pixels: bw = W (W | 128), then rows, then images
 bool tile_geometry(int gh, int gw, int& bw, int& bh, int& bn);
+bool tile_geometry64(int gh, int gw, int& bw, int& bh, int& bn);
+bool act_map_c(const void* ptr, int n, int h, int w, int c, int cbox, int bw, int bh, int bn, CUtensorMap* out);
 int sm_count();
 void set_error(const std::string& e);
 const std::string& last_error();

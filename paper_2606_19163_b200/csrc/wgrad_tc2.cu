@@ -1,0 +1,299 @@
+// wgrad_tc2.cu - CTA-pair (tcgen05 cta_group::2) weight-gradient kernel for sm_100a.
+//   dW[co][tap][c] += sum_pixels g[pixel, co] * in[pixel shifted by tap, c]
+// GEMM view: D[256 rows = 4 x (tap, 64-channel block)][320 cols = co] += A^T B over K = pixels.  Both operands
+// have the channel dimension contiguous (MN-major), so the fprop TMA boxes ([64 pixels][64 channels], 128-byte
+// swizzled rows) are consumed directly by MN-major UMMA descriptors.
+// Pair tile: each CTA loads ITS two (tap, channel-block) units of the activations (16 KB) and HALF of the
+// gradient columns (co): 128 of the first 256 (two 64-wide boxes) and 32 of the last 64 (one 64-byte-swizzled
+// box) = 20 KB, and the leader issues M = 256 MMAs with N = 256 and N = 64.  Per CTA that is 36 KB of operands
+// per 640 MMA cycles (the single-CTA kernel moves 56 KB for the same math and is bound by shared-memory
+// bandwidth: TMA writes + MMA reads > 128 B/cycle/SM).
+// Work distribution ("stream-K"): items (output tile, 64-pixel tile) are cut into equal contiguous ranges, one
+// per CTA pair; a range that crosses an output-tile boundary flushes its accumulator with fp32 red.add into dW
+// (which is also how weight gradients accumulate across microbatches, row a11) and starts the next tile.
+#include <cuda.h>
+
+#include <cstdlib>
+#include <cstring>
+
+#include "common.cuh"
+#include "kernels.h"
+#include "sm100.cuh"
+#include "tmap.h"
+
+namespace pulse {
+
+namespace {
+
+using namespace sm100;
+using namespace tmap;
+
+constexpr int PIX = 64;                       // K per stage
+constexpr int BLK = PIX * 128;                // one [64 px][64 ch] box = 8 KB
+constexpr int BLK32 = PIX * 64;               // one [64 px][32 ch] box = 4 KB
+constexpr int N_TOT = 320;
+constexpr int STAGE = 2 * BLK + 2 * BLK + BLK32;      // 36 KB per CTA
+constexpr int STAGES = 6;
+constexpr int SMEM = STAGES * STAGE + 1024;
+
+#ifdef PULSE_MB
+__device__ unsigned long long g_tlw[64];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TL(i) do { if (blockIdx.x == 0) { g_tlw[i] = gtime(); g_tlw[32 + i] = clock64(); } } while (0)
+#define DBGW(p) ((p).dbg)
+#else
+#define TL(i) do {} while (0)
+#define DBGW(p) 0
+#endif
+
+struct Wg2Params {
+  int dbg;
+  int units, c_blocks, c0_blocks, c0, ctot, ktot, s2;
+  Tap taps[9];
+  int bw, bh, bn, tiles_w, tiles_h;
+  int pix_tiles, m_tiles, n_tiles;       // m_tiles: pair tiles of 4 units
+  long long work;
+  float* dw;
+};
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
+            const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapG32, const Wg2Params p) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tfull_bar, tempty_bar;
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+  const long long wb = p.work * pair / npairs, we = p.work * (pair + 1) / npairs;
+
+  if (threadIdx.x == 0) TL(0);
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapG); prefetch_tmap(&mapG32);
+    for (int i = 0; i < STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
+    mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 8);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc2(&tmem_base_s, 512);
+  tc_fence_before();
+  cluster_sync_all();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // ===== TMA producer (both CTAs) =====
+      // indices advance incrementally: a 64-bit division per work item would cost more than the item's MMAs
+      int stage = 0; uint32_t phase = 0;
+      int ot = (int)(wb / p.pix_tiles), pt = (int)(wb - (long long)ot * p.pix_tiles);
+      int tx = pt % p.tiles_w, ty = (pt / p.tiles_w) % p.tiles_h, tn = pt / (p.tiles_w * p.tiles_h);
+      const int n_items = (int)(we - wb);
+      const CUtensorMap* ma[2]; int cch[2], adx[2], ady[2], apx[2], apy[2], co = 0;
+      bool new_tile = true;
+      for (int it = 0; it < n_items; ++it) {
+        if (new_tile) {
+          const int nt = ot % p.n_tiles, mt = ot / p.n_tiles;
+#pragma unroll
+          for (int b = 0; b < 2; ++b) {
+            const int u = min(4 * mt + 2 * (int)rank + b, p.units - 1);
+            const int ti = u / p.c_blocks, cb = u - ti * p.c_blocks;
+            const Tap t = p.taps[ti];
+            const bool first = cb < p.c0_blocks;
+            ma[b] = first ? &mapA0 : &mapA1;
+            cch[b] = (first ? cb : cb - p.c0_blocks) * 64;
+            adx[b] = t.dx; ady[b] = t.dy; apx[b] = t.px; apy[b] = t.py;
+          }
+          co = nt * N_TOT;
+          new_tile = false;
+        }
+        const int x0 = tx * p.bw, y0 = ty * p.bh, n0 = tn * p.bn;
+        mbar_wait(&empty_bar[stage], phase ^ 1);
+        if (DBGW(p) & 2) {
+          if (rank == 0) mbar_arrive(&full_bar[stage]);
+        } else {
+          if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * STAGE);
+          const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
+          uint8_t* sa = smem + stage * STAGE;
+#pragma unroll
+          for (int b = 0; b < 2; ++b) {
+            if (!p.s2) tma2_load_4d(sa + b * BLK, ma[b], fb, cch[b], x0 + adx[b], y0 + ady[b], n0);
+            else tma2_load_5d(sa + b * BLK, ma[b], fb, apx[b] * p.c0 + cch[b], x0 + adx[b], apy[b], y0 + ady[b], n0);
+          }
+          tma2_load_4d(sa + 2 * BLK, &mapG, fb, co + (int)rank * 128, x0, y0, n0);
+          tma2_load_4d(sa + 3 * BLK, &mapG, fb, co + (int)rank * 128 + 64, x0, y0, n0);
+          tma2_load_4d(sa + 4 * BLK, &mapG32, fb, co + 256 + (int)rank * 32, x0, y0, n0);
+        }
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        if (++tx == p.tiles_w) { tx = 0; if (++ty == p.tiles_h) { ty = 0; ++tn; } }
+        if (++pt == p.pix_tiles) { pt = 0; tx = ty = tn = 0; ++ot; new_tile = true; }
+      }
+    }
+  } else if (warp == 1) {
+    if (rank == 0) {
+      // ===== MMA issuer (leader): the whole warp runs the loop, one elected lane issues (see elect_one_sync) =====
+      constexpr uint32_t idesc256 = idesc_bf16(256, 256, 1, 1), idesc64 = idesc_bf16(256, 64, 1, 1);
+      constexpr uint64_t d128 = smem_desc_sw128(BLK, 1024);      // MN-major: LBO = next 64-channel block, SBO = 8 pixels
+      constexpr uint64_t d64 = smem_desc_sw64(BLK32, 512);
+      constexpr uint32_t hi128 = (uint32_t)(d128 >> 32), hi64 = (uint32_t)(d64 >> 32);
+      const uint32_t base16 = (smem_u32(smem) >> 4) & 0x3FFF;
+      int stage = 0; uint32_t phase = 0, tphase = 0;
+      bool fresh = true;
+      int pt = (int)(wb % p.pix_tiles);
+      const int n_items = (int)(we - wb);
+      for (int it = 0; it < n_items; ++it) {
+        if (fresh) {
+          mbar_wait(&tempty_bar, tphase ^ 1);
+          tc_fence_after();
+        }
+        mbar_wait(&full_bar[stage], phase);
+        tc_fence_after();
+        if (it == 0) TL(2);
+        if (it == n_items - 1) TL(3);
+        const uint32_t a16 = base16 + stage * (STAGE >> 4);
+        const bool last = (++pt == p.pix_tiles || it == n_items - 1);
+        if (elect_one_sync()) {
+          if (!(DBGW(p) & 1)) {
+#pragma unroll
+            for (int k = 0; k < PIX / 16; ++k) {
+              const uint32_t acc = (!fresh || k != 0);
+              const uint64_t da = ((uint64_t)hi128 << 32) | ((uint32_t)d128 | (a16 + k * 128));
+              umma2_bf16(tmem_base, da, ((uint64_t)hi128 << 32) | ((uint32_t)d128 | (a16 + (2 * BLK >> 4) + k * 128)),
+                         idesc256, acc);
+              umma2_bf16(tmem_base + 256, da, ((uint64_t)hi64 << 32) | ((uint32_t)d64 | (a16 + (4 * BLK >> 4) + k * 64)),
+                         idesc64, acc);
+            }
+          }
+          umma2_commit_mc(&empty_bar[stage], 3);
+          if (last) umma2_commit_mc(&tfull_bar, 3);
+        }
+        __syncwarp();
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        fresh = false;
+        if (last) { pt = 0; tphase ^= 1; fresh = true; }
+      }
+    }
+  } else {
+    // ===== epilogue (both CTAs): fp32 red.add of this CTA's 128 rows x 320 columns =====
+    const int q = warp & 3;
+    const int row = q * 32 + lane;
+    uint32_t tphase = 0;
+    long long w = wb;
+    while (w < we) {
+      const int ot = (int)(w / p.pix_tiles);
+      const long long seg_end = min(we, (long long)(ot + 1) * p.pix_tiles);
+      const int nt = ot % p.n_tiles, mt = ot / p.n_tiles;
+      const int u = 4 * mt + 2 * (int)rank + (row >> 6);
+      const bool valid = u < p.units;
+      const int ti = valid ? u / p.c_blocks : 0, cb = valid ? u - ti * p.c_blocks : 0;
+      const size_t kidx = (size_t)p.taps[ti].widx * p.ctot + cb * 64 + (row & 63);
+      mbar_wait(&tfull_bar, tphase);
+      tphase ^= 1;
+      tc_fence_after();
+      if (warp == 2 && lane == 0 && seg_end == we) TL(4);
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+#pragma unroll 1
+      for (int ch = 0; ch < N_TOT / 32; ++ch) {
+        uint32_t r[32];
+        tmem_ld32(taddr + ch * 32, r);
+        tmem_ld_wait();
+        if (ch == N_TOT / 32 - 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&tempty_bar), 0));
+        }
+        if (valid && !(DBGW(p) & 4)) {
+          float* dst = p.dw + (size_t)(nt * N_TOT + ch * 32) * p.ktot + kidx;
+#pragma unroll
+          for (int i = 0; i < 32; ++i) atomicAdd(dst + (size_t)i * p.ktot, __uint_as_float(r[i]));
+        }
+      }
+      w = seg_end;
+    }
+  }
+  if (warp == 2 && lane == 0) TL(5);
+  tc_fence_before();
+  cluster_sync_all();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc2(tmem_base, 512);
+  }
+  if (threadIdx.x == 32) TL(6);
+}
+
+}  // namespace
+#ifdef PULSE_MB
+void mb_timeline_w(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tlw, sizeof(unsigned long long) * 64); }
+#endif
+
+bool wgrad_tc2_supported(const WgradArgs& a) {
+  if (a.dt != DT_BF16) return false;
+  if (a.src.c0 % 64 || a.src.c1 % 64 || a.src.c0 == 0 || a.cout % N_TOT) return false;
+  if (a.ksize != 1 && a.ksize != 3) return false;
+  if (a.stride == 2) {
+    if (a.ksize != 3 || a.src.c1 || (a.hin & 1) || (a.win & 1) || a.hout * 2 != a.hin || a.wout * 2 != a.win) return false;
+  } else if (a.stride != 1 || a.hout != a.hin || a.wout != a.win) {
+    return false;
+  }
+  int bw, bh, bn;
+  return tile_geometry64(a.hout, a.wout, bw, bh, bn);
+}
+
+int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
+  Wg2Params p;
+  memset(&p, 0, sizeof p);
+  const bool s2 = a.stride == 2;
+  tile_geometry64(a.hout, a.wout, p.bw, p.bh, p.bn);
+  p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64; p.s2 = s2;
+  const int taps = a.ksize * a.ksize, pad = (a.ksize - 1) / 2;
+  p.units = taps * p.c_blocks; p.ktot = taps * p.ctot;
+  for (int r = 0; r < a.ksize; ++r)
+    for (int s = 0; s < a.ksize; ++s) {
+      Tap t; t.widx = r * a.ksize + s; t.px = t.py = 0;
+      if (!s2) { t.dy = r - pad; t.dx = s - pad; }
+      else { t.dy = r == 0 ? -1 : 0; t.py = r == 1 ? 0 : 1; t.dx = s == 0 ? -1 : 0; t.px = s == 1 ? 0 : 1; }
+      p.taps[t.widx] = t;
+    }
+  p.tiles_w = a.wout / p.bw; p.tiles_h = (a.hout + p.bh - 1) / p.bh;
+  p.pix_tiles = p.tiles_w * p.tiles_h * ((a.n + p.bn - 1) / p.bn);
+  p.m_tiles = (p.units + 3) / 4; p.n_tiles = a.cout / N_TOT;
+  p.dw = a.dw;
+#ifdef PULSE_MB
+  { const char* e = getenv("PULSE_DBG"); p.dbg = e ? atoi(e) : 0; }
+#endif
+  CUtensorMap m0, m1, mg, mg32;
+  bool ok;
+  if (s2) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
+  m1 = m0;
+  if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
+  if (ok) ok = act_map(a.g, a.n, a.hout, a.wout, a.cout, p.bw, p.bh, p.bn, &mg);
+  if (ok) ok = act_map_c(a.g, a.n, a.hout, a.wout, a.cout, 32, p.bw, p.bh, p.bn, &mg32);
+  if (!ok) return -1;
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(wgrad_tc2_k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM) != cudaSuccess) {
+      tmap::set_error("cudaFuncSetAttribute(wgrad2 smem) failed");
+      return -1;
+    }
+    attr_set = true;
+  }
+  p.work = (long long)p.m_tiles * p.n_tiles * p.pix_tiles;
+  long long pairs = sm_count() / 2;                       // one CTA pair per SM pair, equal shares, >= 4 items each
+  if (p.work / 4 < pairs) pairs = p.work / 4 > 0 ? p.work / 4 : 1;
+  wgrad_tc2_k<<<(unsigned)(2 * pairs), 192, SMEM, st>>>(m0, m1, mg, mg32, p);
+  return 1;
+}
+
+static bool force_1cta_wgrad() {
+  static int v = -1;
+  if (v < 0) { const char* e = getenv("PULSE_WGRAD_1CTA"); v = (e && e[0] == '1') ? 1 : 0; }
+  return v == 1;
+}
+bool wgrad_tc_any_supported(const WgradArgs& a) { return wgrad_tc2_supported(a) || wgrad_tc_supported(a); }
+int wgrad_tc_any(const WgradArgs& a, cudaStream_t st) {
+  if (!force_1cta_wgrad() && wgrad_tc2_supported(a)) return wgrad_tc2(a, st);
+  return wgrad_tc(a, st);
+}
+
+}  // namespace pulse
