@@ -45,6 +45,7 @@ struct Tc2Params {
   int GH, GN;                     // pixel grid (rows, images); columns == bw
   const bf16* bias; const float* pn; const bf16* residual; bf16* out; int accumulate;
   int OH, OW, osy, osx, ooy, oox, cout_total;
+  float* cst;                     // channel stats [n][2][cout] of the stored output, accumulated (or null)
   int dbg;                        // microbenchmark modes (only compiled with -DPULSE_MB): 1 no MMA, 2 no TMA, 4 no stores
 };
 #ifdef PULSE_MB
@@ -199,6 +200,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       const size_t off = (((size_t)n * p.OH + (size_t)y * p.osy + p.ooy) * p.OW + (size_t)x * p.osx + p.oox) *
                              p.cout_total + (size_t)nt * C::BN;
       const bf16* addend = p.residual ? p.residual : (p.accumulate ? p.out : nullptr);
+      const unsigned vmask = __ballot_sync(0xffffffffu, valid);
       {   // column vector of this warp's image, staged while the main loop runs
         const int nw = min(n_t + n_w, p.GN - 1);
         __syncwarp();
@@ -251,6 +253,24 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           if (lane == 0) {
             tma_store_4d(&mapO, stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
             bulk_commit();
+          }
+          if (p.cst && vmask && lane < CW / 2) {
+            // channel stats of the STORED (bf16) values for the GroupNorm that reads this tensor: each lane sums two
+            // columns of the staged box over the warp's valid pixel rows (conflict-free: a row is one 128/64-byte line)
+            float s0 = 0.f, s1 = 0.f, q0 = 0.f, q1 = 0.f;
+            const uint32_t base = smem_u32(stg) + buf * C::BOX_BYTES + (lane & 3) * 4;
+#pragma unroll 8
+            for (int r = 0; r < 32; ++r) {
+              if (!((vmask >> r) & 1)) continue;
+              const uint32_t swr = CW == 64 ? (r & 7) : ((r >> 1) & 3);
+              uint32_t wv;
+              asm volatile("ld.shared.b32 %0, [%1];" : "=r"(wv) : "r"(base + r * (CW * 2) + (((lane >> 2) ^ swr) << 4)));
+              const float a = __uint_as_float(wv << 16), b = __uint_as_float(wv & 0xffff0000u);
+              s0 += a; q0 = fmaf(a, a, q0); s1 += b; q1 = fmaf(b, b, q1);
+            }
+            float* dst = p.cst + (size_t)(n_t + n_w) * 2 * p.cout_total + co + 2 * lane;
+            atomicAdd(dst, s0); atomicAdd(dst + 1, s1);
+            atomicAdd(dst + p.cout_total, q0); atomicAdd(dst + p.cout_total + 1, q1);
           }
           buf ^= 1;
         }
@@ -347,6 +367,7 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
   p.GH = gh; p.GN = a.n;
   p.bias = (const bf16*)a.bias; p.pn = a.pn; p.residual = (const bf16*)a.residual; p.out = (bf16*)a.out;
   p.accumulate = a.accumulate;
+  p.cst = a.cst;
 #ifdef PULSE_MB
   { const char* e = getenv("PULSE_DBG"); p.dbg = e ? atoi(e) : 0; }
 #endif
@@ -420,6 +441,9 @@ static bool force_1cta() {
   static int v = -1;
   if (v < 0) { const char* e = getenv("PULSE_CONV_1CTA"); v = (e && e[0] == '1') ? 1 : 0; }
   return v == 1;
+}
+bool conv_emits_stats(const ConvArgs& a) {
+  return !force_1cta() && conv_tc2_supported(a) && a.mode == CONV_FPROP && !a.accumulate;
 }
 bool conv_tc_any_supported(const ConvArgs& a) { return conv_tc2_supported(a) || conv_tc_supported(a); }
 int conv_tc_any(const ConvArgs& a, cudaStream_t st) {

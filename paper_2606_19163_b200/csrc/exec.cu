@@ -55,11 +55,23 @@ double conv_flops(const ConvArgs& a) {
   const double mpix = a.mode == CONV_DGRAD_S2 ? (double)a.n * a.hin * a.win : (double)a.n * a.hout * a.wout;
   return 2.0 * mpix * a.cout * a.src.c() * a.ksize * a.ksize;     // the s2 dgrad phases execute exactly 9/4 taps per output
 }
-void run_conv(Ctx& c, const ConvArgs& a) {
+void run_stats(Ctx& c, int t);
+// stats_t >= 0: the conv writes tensor stats_t, which a GroupNorm will read: its channel stats come from the conv
+// epilogue where the kernel supports it, else from a chan_stats pass
+void run_conv(Ctx& c, ConvArgs a, int stats_t = -1) {
   const bool tc = c.tc() && conv_tc_any_supported(a);
-  Prof pr(c.s, c.st, tc ? PULSE_KCLASS_CONV_TC : PULSE_KCLASS_CONV_SIMT, conv_flops(a), 0.0);
-  const int r = tc ? conv_tc_any(a, c.st) : conv_simt(a, c.st);
-  if (r < 0) c.err = true; else c.s->launches += r;
+  bool fused = false;
+  if (stats_t >= 0 && c.s->tensors[stats_t].gn_input) {
+    a.cst = (float*)(c.stash + c.s->tensors[stats_t].cst);
+    fused = tc && conv_emits_stats(a);
+    if (!fused) a.cst = nullptr;
+  }
+  {
+    Prof pr(c.s, c.st, tc ? PULSE_KCLASS_CONV_TC : PULSE_KCLASS_CONV_SIMT, conv_flops(a), 0.0);
+    const int r = tc ? conv_tc_any(a, c.st) : conv_simt(a, c.st);
+    if (r < 0) c.err = true; else c.s->launches += r;
+  }
+  if (stats_t >= 0 && !fused) run_stats(c, stats_t);
 }
 void run_wgrad(Ctx& c, const WgradArgs& a) {
   const bool tc = c.tc() && wgrad_tc_any_supported(a);
@@ -147,8 +159,7 @@ void resblock_forward(Ctx& c, const OpPlan& op) {
   run_gn_fwd(c, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1));
   Cat a1{c.fwd(op.a1), ctot, nullptr, 0};
   run_conv(c, conv_args(c, a1, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C1W]), op.cout,
-                        c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)));
-  run_stats(c, op.h1);
+                        c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)), op.h1);
   Cat h1{c.fwd(op.h1), op.cout, nullptr, 0};
   run_gn_fwd(c, h1, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2));
   const void* res = c.fwd(op.x0);
@@ -159,8 +170,7 @@ void resblock_forward(Ctx& c, const OpPlan& op) {
   }
   Cat a2{c.fwd(op.a2), op.cout, nullptr, 0};
   run_conv(c, conv_args(c, a2, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C2W]), op.cout,
-                        c.par(op.p[P_C2B]), nullptr, res, c.fwd(op.out)));
-  run_stats(c, op.out);
+                        c.par(op.p[P_C2B]), nullptr, res, c.fwd(op.out)), op.out);
 }
 
 // pixel sums of the gradient of an op's output, for its bias gradient: fused by the writers or one colsum pass
@@ -288,15 +298,13 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
       case PULSE_OP_DOWN: {
         const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
         run_conv(c, conv_args(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin, op.win, op.hout, op.wout, 3, stride,
-                              c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
-        run_stats(c, op.out);
+                              c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)), op.out);
         break;
       }
       case PULSE_OP_UP: {
         s->launches += upsample2(c.dt, c.fwd(op.x0), s->d.n, op.hin, op.win, op.cin, c.fwd(op.u), c.st);
         run_conv(c, conv_args(c, Cat{c.fwd(op.u), op.cin, nullptr, 0}, op.hout, op.wout, op.hout, op.wout, 3, 1,
-                              c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
-        run_stats(c, op.out);
+                              c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)), op.out);
         break;
       }
       case PULSE_OP_HEAD: {

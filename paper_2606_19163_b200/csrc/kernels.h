@@ -84,7 +84,10 @@ struct ConvArgs {
   const float* pn;                // [n][cout] fp32 per-sample bias (temb projection), or null
   const void* residual;           // [n,hout,wout,cout] dtype, added, or null (may alias out)
   void* out; int accumulate;      // out (+)= result
+  float* cst = nullptr;           // if non-null and the kernel can (conv_emits_stats): channel stats [n][2][cout] of
+                                  // the stored output are accumulated here by the epilogue (norm.cu interface)
 };
+bool conv_emits_stats(const ConvArgs& a);   // true: conv_tc_any(a) fills a.cst itself; false: run chan_stats after it
 int conv_simt(const ConvArgs& a, cudaStream_t st);
 struct WgradArgs {
   int dt;

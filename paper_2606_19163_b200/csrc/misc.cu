@@ -491,27 +491,47 @@ __global__ void flip_transpose_k(const T* __restrict__ w, int cout, int kk, int 
     if (co < cout && ci < cin) wt[((size_t)ci * kk + ftap) * cout + co] = tile[threadIdx.x][j];
   }
 }
-// all conv weights of a stage in one launch per 16 tensors (blockIdx.z = entry; taps looped inside)
+// all conv weights of a stage in one launch per 16 tensors: blockIdx.z = entry * 9 + tap, 64 x 64 tiles, both the
+// reads (along ci) and the writes (along co) are 128 contiguous bytes per warp row (bf16; 32-bit accesses of pairs)
 template <typename T>
-__global__ void flip_transpose_batch_k(const __grid_constant__ TransposeBatch b) {
-  __shared__ T tile[32][33];
-  const TransposeEntry& e = b.e[blockIdx.z];
-  const int ci0 = blockIdx.x * 32, co0 = blockIdx.y * 32, kk = e.k * e.k;
-  if (ci0 >= e.cin || co0 >= e.cout) return;
-  const T* w = (const T*)e.w;
-  T* wt = (T*)e.wt;
-  for (int tap = 0; tap < kk; ++tap) {
-    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
-      const int co = co0 + j, ci = ci0 + threadIdx.x;
-      if (co < e.cout && ci < e.cin) tile[j][threadIdx.x] = w[((size_t)co * kk + tap) * e.cin + ci];
+__global__ void __launch_bounds__(256) flip_transpose_batch_k(const __grid_constant__ TransposeBatch b) {
+  const TransposeEntry& e = b.e[blockIdx.z / 9];
+  const int tap = blockIdx.z % 9, kk = e.k * e.k;
+  const int ci0 = blockIdx.x * 64, co0 = blockIdx.y * 64;
+  if (tap >= kk || ci0 >= e.cin || co0 >= e.cout) return;
+  const int ftap = kk - 1 - tap, tx = threadIdx.x, ty = threadIdx.y;
+  if (sizeof(T) == 2 && !(e.cin & 1) && !(e.cout & 1)) {
+    __shared__ uint16_t tile[64][66];
+    const uint16_t* w = (const uint16_t*)e.w;
+    uint16_t* wt = (uint16_t*)e.wt;
+    for (int j = ty; j < 64; j += 8) {
+      const int co = co0 + j, ci = ci0 + 2 * tx;
+      uint32_t v = 0;
+      if (co < e.cout && ci < e.cin) v = *reinterpret_cast<const uint32_t*>(w + ((size_t)co * kk + tap) * e.cin + ci);
+      tile[j][2 * tx] = (uint16_t)v; tile[j][2 * tx + 1] = (uint16_t)(v >> 16);
     }
     __syncthreads();
-    const int ftap = kk - 1 - tap;
-    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
-      const int ci = ci0 + j, co = co0 + threadIdx.x;
-      if (co < e.cout && ci < e.cin) wt[((size_t)ci * kk + ftap) * e.cout + co] = tile[threadIdx.x][j];
+    for (int j = ty; j < 64; j += 8) {
+      const int ci = ci0 + j, co = co0 + 2 * tx;
+      if (ci < e.cin && co < e.cout)
+        *reinterpret_cast<uint32_t*>(wt + ((size_t)ci * kk + ftap) * e.cout + co) =
+            (uint32_t)tile[2 * tx][j] | ((uint32_t)tile[2 * tx + 1][j] << 16);
     }
+  } else {
+    __shared__ T tile[64][65];
+    const T* w = (const T*)e.w;
+    T* wt = (T*)e.wt;
+    for (int j = ty; j < 64; j += 8)
+      for (int i = tx; i < 64; i += 32) {
+        const int co = co0 + j, ci = ci0 + i;
+        if (co < e.cout && ci < e.cin) tile[j][i] = w[((size_t)co * kk + tap) * e.cin + ci];
+      }
     __syncthreads();
+    for (int j = ty; j < 64; j += 8)
+      for (int i = tx; i < 64; i += 32) {
+        const int ci = ci0 + j, co = co0 + i;
+        if (co < e.cout && ci < e.cin) wt[((size_t)ci * kk + ftap) * e.cout + co] = tile[i][j];
+      }
   }
 }
 int flip_transpose_batch(int dt, const TransposeEntry* e, int count, cudaStream_t st) {
@@ -525,7 +545,7 @@ int flip_transpose_batch(int dt, const TransposeEntry* e, int count, cudaStream_
       if (b.e[i].cin > mci) mci = b.e[i].cin;
       if (b.e[i].cout > mco) mco = b.e[i].cout;
     }
-    dim3 grid((mci + 31) / 32, (mco + 31) / 32, b.count), block(32, 8);
+    dim3 grid((mci + 63) / 64, (mco + 63) / 64, b.count * 9), block(32, 8);
     if (dt == DT_F32) flip_transpose_batch_k<float><<<grid, block, 0, st>>>(b);
     else flip_transpose_batch_k<bf16><<<grid, block, 0, st>>>(b);
     ++launches;

@@ -19,8 +19,13 @@
 //  * Thread layout: a thread owns one 16-byte channel vector and walks pixels, so a CTA reads
 //    whole contiguous pixel rows (fully coalesced), per-channel partials live in registers,
 //    cross-CTA reduction is one fp32 atomic per channel per CTA (<= ~74-way per address).
+//  * Memory-level parallelism without registers: the apply / backward kernels stream their inputs through a
+//    shared-memory ring filled by bulk asynchronous copies (cp.async.bulk + mbarrier, one elected thread issues).
+//    The first stages are requested at kernel entry, BEFORE the statistics prologue, so DRAM latency overlaps
+//    the prologue, and a 10 MB tensor spread over 148 CTAs is entirely in flight at once.
 #include "common.cuh"
 #include "kernels.h"
+#include "sm100.cuh"
 
 namespace pulse {
 
@@ -141,6 +146,55 @@ __device__ __forceinline__ void reduce_rows_atomic(float (&v)[2][V], int C, Smem
   }
 }
 
+
+// ---- shared-memory ring fed by bulk asynchronous copies -----------------------------------------------------
+constexpr int RS = 3;        // ring stages
+constexpr int MAXS = 4;      // input streams per kernel
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(sm100::smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(sm100::smem_u32(bar)) : "memory");
+}
+struct Ring {
+  uint64_t* full;            // [RS]
+  uint8_t* buf;
+  int ns = 0;
+  const char* g[MAXS]; int ppb[MAXS]; int soff[MAXS];    // global base (pixel 0 of this image), bytes per pixel, offset in a stage
+  int stage_bytes, P, pb, pe, nch;
+  // stream i of every stage holds P pixels of `bytes_per_pixel` bytes
+  __device__ __forceinline__ int add(const void* base, int bytes_per_pixel) {
+    g[ns] = (const char*)base; ppb[ns] = bytes_per_pixel; soff[ns] = ns ? soff[ns - 1] + P * ppb[ns - 1] : 0;
+    return ns++;
+  }
+  __device__ __forceinline__ void issue(int c) {            // one thread
+    const int s = c % RS, p0 = pb + c * P, np = min(P, pe - p0);
+    uint32_t bytes = 0;
+    for (int i = 0; i < ns; ++i) bytes += (uint32_t)np * ppb[i];
+    sm100::mbar_expect_tx(&full[s], bytes);
+    for (int i = 0; i < ns; ++i)
+      bulk_g2s(buf + (size_t)s * stage_bytes + soff[i], g[i] + (size_t)p0 * ppb[i], (uint32_t)np * ppb[i], &full[s]);
+  }
+  __device__ __forceinline__ void start(int tid) {          // whole CTA; barriers are initialised here
+    if (tid == 0) {
+      for (int i = 0; i < RS; ++i) sm100::mbar_init(&full[i], 1);
+      sm100::fence_barrier_init();
+      for (int c = 0; c < RS && c < nch; ++c) issue(c);
+    }
+    __syncthreads();
+  }
+  __device__ __forceinline__ const uint8_t* wait(int c) {
+    sm100::mbar_wait(&full[c % RS], (c / RS) & 1);
+    return buf + (size_t)(c % RS) * stage_bytes;
+  }
+  __device__ __forceinline__ void release(int c, int tid) { // whole CTA: everyone is done reading stage c % RS
+    __syncthreads();
+    if (tid == 0 && c + RS < nch) issue(c + RS);
+  }
+};
+// load Vec<T>::N consecutive elements from shared memory (generic pointer) into floats
+template <typename T> __device__ __forceinline__ void lds(const uint8_t* p, float (&o)[Vec<T>::N]) {
+  ldv(reinterpret_cast<const T*>(p), o);
+}
+
 // ------------------------------------------------------------------------------ channel stats of one tensor
 template <typename T>
 __global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, int C, int hw, float* __restrict__ cst) {
@@ -172,34 +226,64 @@ __global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, 
   reduce_rows_atomic<V>(v, C, s, cst + (size_t)n * 2 * C);
 }
 
+// SiLU pieces: sigmoid = 1 / (1 + 2^(-y log2 e)): one MUFU.EX2 and one MUFU.RCP per element.  (The single-MUFU
+// tanh.approx form, sigmoid = 0.5 tanh(y/2) + 0.5, was measured and rejected: its 2^-11 relative error is a smooth
+// function of y, so it does not average out in the bias / gamma / beta sums and pushed small-tensor gradients past
+// the 2e-2 bar.)
+template <typename T> __device__ __forceinline__ float sigmoid_t(float y) { return sigmoidf_(y); }
+template <typename T> __device__ __forceinline__ float silu_t(float y) { return y * sigmoid_t<T>(y); }
+template <typename T> __device__ __forceinline__ float silu_grad_t(float y) {
+  const float s = sigmoid_t<T>(y);
+  return fmaf(y * s, 1.0f - s, s);
+}
+
+// dynamic smem: [prologue floats (Smem)] | pad to 128 | ring.  `pro_floats` = size of the first part.
+__device__ __forceinline__ uint8_t* ring_base(float* sm, int pro_floats) {
+  return reinterpret_cast<uint8_t*>(sm) + (((size_t)pro_floats * 4 + 127) & ~(size_t)127);
+}
+
 // ------------------------------------------------------------------------------ forward apply (one pass)
 template <typename T>
 __global__ void __launch_bounds__(512, 2)
 gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw, int G, float eps,
            const T* __restrict__ gamma, const T* __restrict__ beta, const float* __restrict__ cst0,
-           const float* __restrict__ cst1, T* __restrict__ out) {
+           const float* __restrict__ cst1, T* __restrict__ out, int P, int stage_bytes, int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
-  const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y;
+  __shared__ uint64_t full[RS];
+  const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y, tid = tid_();
   Smem s(sm_, C, G);
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
   const int ch = threadIdx.x * V;
+  Ring r;
+  r.full = full; r.buf = ring_base(sm_, pro_floats); r.P = P; r.stage_bytes = stage_bytes;
+  r.pb = blockIdx.x * ppc; r.pe = min(hw, r.pb + ppc); r.nch = r.pe > r.pb ? (r.pe - r.pb + P - 1) / P : 0;
+  const int i0 = r.add(p0 + (size_t)n * hw * c0, c0 * (int)sizeof(T));
+  const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
+  r.start(tid);
   group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
   float sc[V], sh[V], rr[V], mr[V];
   gn_coefs<T, V>(s, G, C / G, gamma, beta, ch, sc, sh, rr, mr);
-  for (int p = pb + threadIdx.y; p < pe; p += 4 * rows) {
-    float v[4][V];
+  const bool lo = ch < c0;
+  const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
+  const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
+  for (int c = 0; c < r.nch; ++c) {
+    const uint8_t* st = r.wait(c);
+    const int pbase = r.pb + c * P, np = min(P, r.pe - pbase);
+    for (int pl = threadIdx.y; pl < np; pl += 2 * rows) {      // two independent pixels per iteration (ILP)
+      float v[2][V];
+      const bool two = pl + rows < np;
+      lds<T>(st + xoff + pl * xpp, v[0]);
+      if (two) lds<T>(st + xoff + (pl + rows) * xpp, v[1]);
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (p + u * rows < pe) ldv(cat_ptr(p0, c0, p1, c1, (size_t)n * hw + p + u * rows, ch), v[u]);
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (p + u * rows < pe) {
-#pragma unroll
-        for (int i = 0; i < V; ++i) v[u][i] = siluf_(fmaf(v[u][i], sc[i], sh[i]));
-        stv(out + ((size_t)n * hw + p + u * rows) * C + ch, v[u]);
+      for (int i = 0; i < V; ++i) {
+        v[0][i] = silu_t<T>(fmaf(v[0][i], sc[i], sh[i]));
+        v[1][i] = silu_t<T>(fmaf(v[1][i], sc[i], sh[i]));
       }
+      stv(out + ((size_t)n * hw + pbase + pl) * C + ch, v[0]);
+      if (two) stv(out + ((size_t)n * hw + pbase + pl + rows) * C + ch, v[1]);
+    }
+    r.release(c, tid);
   }
 }
 
@@ -209,40 +293,46 @@ template <typename T>
 __global__ void __launch_bounds__(512, 1)
 gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
-               const float* __restrict__ cst0, const float* __restrict__ cst1, float* __restrict__ bst) {
+               const float* __restrict__ cst0, const float* __restrict__ cst1, float* __restrict__ bst, int P,
+               int stage_bytes, int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
-  const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y;
+  __shared__ uint64_t full[RS];
+  const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y, tid = tid_();
   Smem s(sm_, C, G);
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
   const int ch = threadIdx.x * V;
+  Ring r;
+  r.full = full; r.buf = ring_base(sm_, pro_floats); r.P = P; r.stage_bytes = stage_bytes;
+  r.pb = blockIdx.x * ppc; r.pe = min(hw, r.pb + ppc); r.nch = r.pe > r.pb ? (r.pe - r.pb + P - 1) / P : 0;
+  const int i0 = r.add(p0 + (size_t)n * hw * c0, c0 * (int)sizeof(T));
+  const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
+  const int ig = r.add(ga + (size_t)n * hw * C, C * (int)sizeof(T));
+  r.start(tid);
   group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
   float sc[V], sh[V], rr[V], mr[V], v[2][V];
   gn_coefs<T, V>(s, G, C / G, gamma, beta, ch, sc, sh, rr, mr);
 #pragma unroll
   for (int i = 0; i < V; ++i) v[0][i] = v[1][i] = 0.f;
-  for (int p = pb + threadIdx.y; p < pe; p += 2 * rows) {
-    float x[2][V], g[2][V];
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      if (p + u * rows < pe) {
-        const size_t pix = (size_t)n * hw + p + u * rows;
-        ldv(cat_ptr(p0, c0, p1, c1, pix, ch), x[u]);
-        ldv(ga + pix * C + ch, g[u]);
-      } else {
-#pragma unroll
-        for (int i = 0; i < V; ++i) { x[u][i] = 0.f; g[u][i] = 0.f; }
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < 2; ++u)
+  const bool lo = ch < c0;
+  const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
+  const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
+  const int goff = r.soff[ig] + ch * (int)sizeof(T), gpp = r.ppb[ig];
+  for (int c = 0; c < r.nch; ++c) {
+    const uint8_t* st = r.wait(c);
+    const int np = min(P, r.pe - (r.pb + c * P));
+    for (int pl = threadIdx.y; pl < np; pl += rows) {
+      float x[V], g[V];
+      lds<T>(st + xoff + pl * xpp, x);
+      lds<T>(st + goff + pl * gpp, g);
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        const float gy = g[u][i] * silu_gradf_(fmaf(x[u][i], sc[i], sh[i]));
+        const float gy = g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i]));
         v[0][i] += gy;
-        v[1][i] = fmaf(gy, fmaf(x[u][i], rr[i], -mr[i]), v[1][i]);
+        v[1][i] = fmaf(gy, fmaf(x[i], rr[i], -mr[i]), v[1][i]);
       }
+    }
+    r.release(c, tid);
   }
   reduce_rows_atomic<V>(v, C, s, bst + (size_t)n * 2 * C);
 }
@@ -257,14 +347,22 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
                const float* __restrict__ cst0, const float* __restrict__ cst1, const float* __restrict__ bst,
                float* dgamma, float* dbeta, const T* __restrict__ add, T* dst0, int dc0, int acc0, T* dst1, int acc1,
-               float* cs0, float* cs1) {
+               float* cs0, float* cs1, int P, int stage_bytes, int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
+  __shared__ uint64_t full[RS];
   const int C = c0 + c1, n = blockIdx.y, nchunks = gridDim.x, rows = blockDim.y, cpg = C / G;
   Smem s(sm_, C, G);
   const int ppc = (hw + nchunks - 1) / nchunks;
-  const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
   const int ch = threadIdx.x * V, tid = tid_(), nthr = nthr_();
+  Ring r;
+  r.full = full; r.buf = ring_base(sm_, pro_floats); r.P = P; r.stage_bytes = stage_bytes;
+  r.pb = blockIdx.x * ppc; r.pe = min(hw, r.pb + ppc); r.nch = r.pe > r.pb ? (r.pe - r.pb + P - 1) / P : 0;
+  const int i0 = r.add(p0 + (size_t)n * hw * c0, c0 * (int)sizeof(T));
+  const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
+  const int ig = r.add(ga + (size_t)n * hw * C, C * (int)sizeof(T));
+  const int ie = add ? r.add(add + (size_t)n * hw * C, C * (int)sizeof(T)) : ig;
+  r.start(tid);
   group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
   float sc[V], sh[V], rr[V], mr[V], k2[V], k3[V];
   gn_coefs<T, V>(s, G, cpg, gamma, beta, ch, sc, sh, rr, mr);
@@ -311,33 +409,32 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   float sum[V];
 #pragma unroll
   for (int i = 0; i < V; ++i) sum[i] = 0.f;
-  for (int p = pb + threadIdx.y; p < pe; p += 2 * rows) {
-    float x[2][V], g[2][V], e[2][V], f[2][V];
+  const bool lo = ch < c0;
+  const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
+  const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
+  const int goff = r.soff[ig] + ch * (int)sizeof(T), eoff = r.soff[ie] + ch * (int)sizeof(T), gpp = C * (int)sizeof(T);
+  for (int c = 0; c < r.nch; ++c) {
+    const uint8_t* st = r.wait(c);
+    const int pbase = r.pb + c * P, np = min(P, r.pe - pbase);
+    for (int pl = threadIdx.y; pl < np; pl += rows) {
+      const size_t pix = (size_t)n * hw + pbase + pl;
+      float x[V], g[V], e[V], f[V], o[V];
+      if (acc) ldv(dst + pix * dC + dch, f);          // the only non-streamed input (second writer of a gradient)
+      lds<T>(st + xoff + pl * xpp, x);
+      lds<T>(st + goff + pl * gpp, g);
+      if (add) lds<T>(st + eoff + pl * gpp, e);
 #pragma unroll
-    for (int u = 0; u < 2; ++u)
-      if (p + u * rows < pe) {
-        const size_t pix = (size_t)n * hw + p + u * rows;
-        ldv(cat_ptr(p0, c0, p1, c1, pix, ch), x[u]);
-        ldv(ga + pix * C + ch, g[u]);
-        if (add) ldv(add + pix * C + ch, e[u]);
-        if (acc) ldv(dst + pix * dC + dch, f[u]);
+      for (int i = 0; i < V; ++i) {
+        const float gy = g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i]));
+        const float xh = fmaf(x[i], rr[i], -mr[i]);
+        o[i] = sc[i] * gy - k2[i] - xh * k3[i];
+        if (add) o[i] += e[i];
+        sum[i] += o[i];
+        if (acc) o[i] += f[i];
       }
-#pragma unroll
-    for (int u = 0; u < 2; ++u)
-      if (p + u * rows < pe) {
-        const size_t pix = (size_t)n * hw + p + u * rows;
-        float o[V];
-#pragma unroll
-        for (int i = 0; i < V; ++i) {
-          const float gy = g[u][i] * silu_gradf_(fmaf(x[u][i], sc[i], sh[i]));
-          const float xh = fmaf(x[u][i], rr[i], -mr[i]);
-          o[i] = sc[i] * gy - k2[i] - xh * k3[i];
-          if (add) o[i] += e[u][i];
-          sum[i] += o[i];
-          if (acc) o[i] += f[u][i];
-        }
-        stv(dst + pix * dC + dch, o);
-      }
+      stv(dst + pix * dC + dch, o);
+    }
+    r.release(c, tid);
   }
   if (cs0 || cs1) {      // channels below dc0 -> cs0[n][dc0], the rest -> cs1[n][C - dc0]
     if (rows == 1) {
@@ -373,18 +470,47 @@ int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStre
   return 1;
 }
 
+// launch geometry of the streaming kernels: one CTA per SM over the whole grid, <= 512 threads; P pixels per ring
+// stage so that a stage is <= 56 KB (3 stages + prologue stay under the 227 KB of shared memory)
+struct StreamPlan { dim3 grid, block; int P, stage_bytes, pro_floats; size_t smem; };
+static StreamPlan stream_plan(int dt, int n, int hw, int C, int G, int red_k, int bytes_per_pixel, int ctas_per_sm = 1) {
+  StreamPlan sp;
+  const int vec = dt == DT_F32 ? 4 : 8;
+  const int tpr = C / vec;
+  int rows = tpr >= 512 ? 1 : 512 / tpr;
+  if (rows > hw) rows = hw;
+  int ppt = (56 * 1024 / ctas_per_sm) / (rows * bytes_per_pixel);
+  if (ppt < 1) ppt = 1;
+  if (ppt > 8) ppt = 8;
+  sp.P = rows * ppt;
+  sp.stage_bytes = (sp.P * bytes_per_pixel + 127) & ~127;
+  int nchunks = (ctas_per_sm * num_sms() + n - 1) / n;
+  const int maxc = (hw + rows - 1) / rows;        // at least one pixel per thread row
+  if (nchunks > maxc) nchunks = maxc;
+  if (nchunks < 1) nchunks = 1;
+  sp.grid = dim3(nchunks, n); sp.block = dim3(tpr, rows);
+  sp.pro_floats = 2 * C + 2 * G + (rows > 1 ? rows * red_k * C : 0);
+  sp.smem = (((size_t)sp.pro_floats * 4 + 127) & ~(size_t)127) + (size_t)RS * sp.stage_bytes;
+  return sp;
+}
+template <typename K> static void allow_big_smem(K kernel) {
+  cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
+}
+
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
                 const float* cst0, const float* cst1, void* a_out, cudaStream_t st) {
   const int C = x.c();
-  const RowPlan pl = row_plan(dt, hw, C, n, 512);
-  dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
-  const size_t sm = smem_bytes(C, groups, 1, 0);
+  const StreamPlan sp = stream_plan(dt, n, hw, C, groups, 0, C * (int)dt_size(dt), 2);
+  static bool attr = false;
+  if (!attr) { allow_big_smem(gn_apply_k<float>); allow_big_smem(gn_apply_k<bf16>); attr = true; }
   if (dt == DT_F32)
-    gn_apply_k<float><<<grid, block, sm, st>>>((const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw, groups, eps,
-                                               (const float*)gamma, (const float*)beta, cst0, cst1, (float*)a_out);
+    gn_apply_k<float><<<sp.grid, sp.block, sp.smem, st>>>((const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw, groups,
+                                                          eps, (const float*)gamma, (const float*)beta, cst0, cst1,
+                                                          (float*)a_out, sp.P, sp.stage_bytes, sp.pro_floats);
   else
-    gn_apply_k<bf16><<<grid, block, sm, st>>>((const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw, groups, eps,
-                                              (const bf16*)gamma, (const bf16*)beta, cst0, cst1, (bf16*)a_out);
+    gn_apply_k<bf16><<<sp.grid, sp.block, sp.smem, st>>>((const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw, groups, eps,
+                                                         (const bf16*)gamma, (const bf16*)beta, cst0, cst1, (bf16*)a_out,
+                                                         sp.P, sp.stage_bytes, sp.pro_floats);
   return 1;
 }
 
@@ -394,20 +520,17 @@ static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps
                     void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st) {
   const int C = x.c();
   const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
-  const RowPlan pl = row_plan(dt, hw, C, n, 256);
-  dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
   static bool attr = false;
-  if (!attr) {
-    cudaFuncSetAttribute(gn_bwd_stats_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-    cudaFuncSetAttribute(gn_bwd_apply_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-    attr = true;
-  }
-  gn_bwd_stats_k<T><<<grid, block, smem_bytes(C, groups, pl.rows, 2), st>>>(
+  if (!attr) { allow_big_smem(gn_bwd_stats_k<T>); allow_big_smem(gn_bwd_apply_k<T>); attr = true; }
+  const StreamPlan s1 = stream_plan(dt, n, hw, C, groups, 2, 2 * C * (int)sizeof(T));
+  gn_bwd_stats_k<T><<<s1.grid, s1.block, s1.smem, st>>>(
       (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0,
-      cst1, bst);
-  gn_bwd_apply_k<T><<<grid, block, smem_bytes(C, groups, pl.rows, 1), st>>>(
+      cst1, bst, s1.P, s1.stage_bytes, s1.pro_floats);
+  const StreamPlan s2 = stream_plan(dt, n, hw, C, groups, 1, (add ? 3 : 2) * C * (int)sizeof(T));
+  gn_bwd_apply_k<T><<<s2.grid, s2.block, s2.smem, st>>>(
       (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0,
-      cst1, bst, dgamma, dbeta, (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1);
+      cst1, bst, dgamma, dbeta, (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes,
+      s2.pro_floats);
   return 2;
 }
 
