@@ -4,9 +4,37 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cstdlib>
+#include <utility>
+
 namespace pulse {
 
 typedef __nv_bfloat16 bf16;
+
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------------------
+// Kernels launched through launch_pdl may start while the previous kernel of the stream is still draining: their
+// CTAs are scheduled as SMs free up and run their prologue (barrier init, TMEM allocation, tensor-map prefetch),
+// then block in pdl_wait() until the previous grid has completed and its writes are visible.  Every such kernel
+// calls pdl_wait() before its first global-memory access and pdl_launch_dependents() right after it.
+// PULSE_NO_PDL=1 launches them as ordinary stream-ordered kernels (both calls are then no-ops).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+inline bool pdl_enabled() {
+  static int v = -1;
+  if (v < 0) { const char* e = getenv("PULSE_NO_PDL"); v = (e && e[0] == '1') ? 0 : 1; }
+  return v == 1;
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                              Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = pdl_enabled() ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 
 template <typename T> struct Vec;                 // 16-byte vector of T
 template <> struct Vec<float> { static constexpr int N = 4; };

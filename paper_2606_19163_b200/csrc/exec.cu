@@ -2,6 +2,7 @@
 // walks the op plan and enqueues kernels.  Rows a1-a11 of SURVEY.md 8a.
 #include "stage.h"
 
+#include <cstdlib>
 #include <cstring>
 
 using namespace pulse;
@@ -14,8 +15,34 @@ struct Ctx {
   char* stash;    // base of this microbatch's stash
   char* work;     // per-stage workspace
   cudaStream_t st;
+  cudaStream_t side = nullptr;   // non-null: weight-gradient kernels go here (backward only)
+  int n_ev = 0;                  // events of s->sync_events used by this call
+  int rb_count = 0;              // ResBlocks processed so far in this backward (g_h1 double buffer / hazard events)
+  int ev_rb[2] = {-1, -1};       // event recorded on the side stream after the wgrads of the last ResBlock of each parity
   int dt;
   bool err = false;
+  cudaEvent_t new_event() {
+    if (n_ev == (int)s->sync_events.size()) {
+      cudaEvent_t e;
+      cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+      s->sync_events.push_back(e);
+    }
+    return s->sync_events[n_ev++];
+  }
+  // side stream continues after everything enqueued on the main stream so far
+  void fork() {
+    if (!side) return;
+    cudaEvent_t e = new_event();
+    cudaEventRecord(e, st);
+    cudaStreamWaitEvent(side, e, 0);
+  }
+  int mark_side() {              // returns the index of an event recorded on the side stream now
+    cudaEvent_t e = new_event();
+    cudaEventRecord(e, side);
+    return n_ev - 1;
+  }
+  void wait_side(int ev) { if (side && ev >= 0) cudaStreamWaitEvent(st, s->sync_events[ev], 0); }
+  cudaStream_t wst() const { return side ? side : st; }
   char* fwd(int t) const {
     const TRef& r = s->tensors[t].ref;
     return (r.region == R_SKIP ? skip : r.region == R_STASH ? stash : work) + r.off;
@@ -75,9 +102,9 @@ void run_conv(Ctx& c, ConvArgs a, int stats_t = -1) {
 }
 void run_wgrad(Ctx& c, const WgradArgs& a) {
   const bool tc = c.tc() && wgrad_tc_any_supported(a);
-  Prof pr(c.s, c.st, tc ? PULSE_KCLASS_WGRAD_TC : PULSE_KCLASS_CONV_SIMT,
+  Prof pr(c.s, c.wst(), tc ? PULSE_KCLASS_WGRAD_TC : PULSE_KCLASS_CONV_SIMT,
           2.0 * a.n * a.hout * a.wout * a.cout * a.src.c() * a.ksize * a.ksize, 0.0);
-  const int r = tc ? wgrad_tc_any(a, c.st) : wgrad_simt(a, c.st);
+  const int r = tc ? wgrad_tc_any(a, c.wst()) : wgrad_simt(a, c.wst());
   if (r < 0) c.err = true; else c.s->launches += r;
 }
 // GroupNorm+SiLU wrappers: algorithmic bytes 2 x esz per element forward, 3 x esz backward
@@ -186,31 +213,39 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
   pulse_stage* s = c.s;
   const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip;
   Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
+  const int par = c.rb_count & 1;
   char* g_out = c.grad(op.out);
   char* g_a2 = c.work + s->w_ga2;
-  char* g_h1 = c.work + s->w_gh1;
+  char* g_h1 = c.work + (par ? s->w_gh1b : s->w_gh1);     // double-buffered: the side stream's wgrad1 reads it late
   char* g_a1 = c.work + s->w_ga1;
   char* g_sc = c.work + s->w_gsc;
   ensure_colsum(c, op.out);
-  // conv2: wgrad, dgrad
+  // conv2 (and shortcut) weight gradients need only g_out: fork them off now
+  c.fork();
   WgradArgs w2{c.dt, Cat{c.fwd(op.a2), op.cout, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
                c.pgrad(op.p[P_C2W])};
   run_wgrad(c, w2);
+  if (op.p[P_SCW] >= 0) {
+    WgradArgs ws{c.dt, x, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 1, 1, c.pgrad(op.p[P_SCW])};
+    run_wgrad(c, ws);
+  }
   run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wt2, 3, op.cout, g_a2, 0, 1, op.hin, op.win);
-  // GN2 + SiLU backward -> g_h1, and its pixel sums g_p[n,c] (temb projection / conv1 bias gradients)
+  // GN2 + SiLU backward -> g_h1, and its pixel sums g_p[n,c] (temb projection / conv1 bias gradients).
+  // g_h1 of this parity was last read by the wgrad1 of the ResBlock two back: wait for it.
+  c.wait_side(c.ev_rb[par]);
   run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
              op.bst2, nullptr, g_h1, op.cout, 0, nullptr, 0, c.pgrad(op.p[P_GN2G]), c.pgrad(op.p[P_GN2B]),
              (float*)(c.work + op.gp), nullptr);
-  // conv1: wgrad, dgrad
+  // conv1: wgrad (side stream), dgrad
+  c.fork();
   WgradArgs w1{c.dt, Cat{c.fwd(op.a1), ctot, nullptr, 0}, n, op.hin, op.win, g_h1, op.hin, op.win, op.cout, 3, 1,
                c.pgrad(op.p[P_C1W])};
   run_wgrad(c, w1);
+  if (c.side) c.ev_rb[par] = c.mark_side();
   run_dgrad(c, g_h1, op.hin, op.win, op.cout, op.wt1, 3, ctot, g_a1, 0, 1, op.hin, op.win);
   // shortcut
   const void* add = g_out;
   if (op.p[P_SCW] >= 0) {
-    WgradArgs ws{c.dt, x, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 1, 1, c.pgrad(op.p[P_SCW])};
-    run_wgrad(c, ws);
     run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wtsc, 1, ctot, g_sc, 0, 1, op.hin, op.win);
     add = g_sc;
   }
@@ -218,6 +253,7 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
   run_gn_bwd(c, g_a1, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.bst1, add, c.grad(op.x0), op.cin,
              op.acc_x0, op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]),
              cs_of(c, op.x0), op.x1 >= 0 ? cs_of(c, op.x1) : nullptr);
+  ++c.rb_count;
 }
 
 // bias / temb-projection gradients of every op from the pixel sums, in one batched launch (row a8-a10)
@@ -345,6 +381,14 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
   const float* emb = (const float*)(c.stash + s->emb_off);
+  if (s->side_mode < 0) {
+    const char* e = getenv("PULSE_NO_SIDE_STREAM");
+    s->side_mode = (e && e[0] == '1') ? 0 : 1;
+  }
+  if (s->side_mode == 1 && !s->profiling) {
+    if (!s->side) CK_CUDA(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
+    c.side = s->side;
+  }
   if (!accumulate_wgrad)
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
   if (!accumulate_wgrad || !s->wt_valid) prepare_weights(c);
@@ -366,6 +410,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
         ensure_colsum(c, op.out);
         WgradArgs w{c.dt, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, n, op.hin, op.win, g_out, op.hout, op.wout, op.cout, 3,
                     stride, c.pgrad(op.p[P_C1W])};
+        c.fork();
         run_wgrad(c, w);
         const bool need_gx = !(op.x0 == s->t_xin && !d_g_x_in);
         if (need_gx)
@@ -379,6 +424,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
         ensure_colsum(c, op.out);
         WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
                     1, c.pgrad(op.p[P_C1W])};
+        c.fork();
         run_wgrad(c, w);
         run_dgrad(c, g_out, op.hout, op.wout, op.cout, op.wt1, 3, op.cin, g_u, 0, 1, op.hout, op.wout);
         s->launches += upsample2_bwd(c.dt, g_u, n, op.hin, op.win, op.cin, c.grad(op.x0), c.st);
@@ -390,6 +436,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
         ensure_colsum(c, op.out);
         WgradArgs w{c.dt, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
                     c.pgrad(op.p[P_C1W])};
+        c.fork();
         run_wgrad(c, w);
         run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wt1, 3, op.cin, g_a, 0, 1, op.hin, op.win);
         run_gn_bwd(c, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.x0, -1, op.hin * op.win, c.par(op.p[P_GN1G]),
@@ -400,6 +447,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
     }
   }
   small_grads(c, emb, d_g_temb);
+  if (c.side) c.wait_side(c.mark_side());      // join: the caller's stream sees every weight gradient complete
   if (open) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   if (d_g_x_in) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());

@@ -260,6 +260,8 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
   r.pb = blockIdx.x * ppc; r.pe = min(hw, r.pb + ppc); r.nch = r.pe > r.pb ? (r.pe - r.pb + P - 1) / P : 0;
   const int i0 = r.add(p0 + (size_t)n * hw * c0, c0 * (int)sizeof(T));
   const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
+  pdl_wait();
+  pdl_launch_dependents();
   r.start(tid);
   group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
   float sc[V], sh[V], rr[V], mr[V];
@@ -308,6 +310,8 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   const int i0 = r.add(p0 + (size_t)n * hw * c0, c0 * (int)sizeof(T));
   const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
   const int ig = r.add(ga + (size_t)n * hw * C, C * (int)sizeof(T));
+  pdl_wait();
+  pdl_launch_dependents();
   r.start(tid);
   group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
   float sc[V], sh[V], rr[V], mr[V], v[2][V];
@@ -362,6 +366,8 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
   const int ig = r.add(ga + (size_t)n * hw * C, C * (int)sizeof(T));
   const int ie = add ? r.add(add + (size_t)n * hw * C, C * (int)sizeof(T)) : ig;
+  pdl_wait();
+  pdl_launch_dependents();
   r.start(tid);
   group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
   float sc[V], sh[V], rr[V], mr[V], k2[V], k3[V];
@@ -504,13 +510,13 @@ int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void*
   static bool attr = false;
   if (!attr) { allow_big_smem(gn_apply_k<float>); allow_big_smem(gn_apply_k<bf16>); attr = true; }
   if (dt == DT_F32)
-    gn_apply_k<float><<<sp.grid, sp.block, sp.smem, st>>>((const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw, groups,
-                                                          eps, (const float*)gamma, (const float*)beta, cst0, cst1,
-                                                          (float*)a_out, sp.P, sp.stage_bytes, sp.pro_floats);
+    launch_pdl(gn_apply_k<float>, sp.grid, sp.block, sp.smem, st, (const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw,
+               groups, eps, (const float*)gamma, (const float*)beta, cst0, cst1, (float*)a_out, sp.P, sp.stage_bytes,
+               sp.pro_floats);
   else
-    gn_apply_k<bf16><<<sp.grid, sp.block, sp.smem, st>>>((const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw, groups, eps,
-                                                         (const bf16*)gamma, (const bf16*)beta, cst0, cst1, (bf16*)a_out,
-                                                         sp.P, sp.stage_bytes, sp.pro_floats);
+    launch_pdl(gn_apply_k<bf16>, sp.grid, sp.block, sp.smem, st, (const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw,
+               groups, eps, (const bf16*)gamma, (const bf16*)beta, cst0, cst1, (bf16*)a_out, sp.P, sp.stage_bytes,
+               sp.pro_floats);
   return 1;
 }
 
@@ -523,14 +529,12 @@ static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps
   static bool attr = false;
   if (!attr) { allow_big_smem(gn_bwd_stats_k<T>); allow_big_smem(gn_bwd_apply_k<T>); attr = true; }
   const StreamPlan s1 = stream_plan(dt, n, hw, C, groups, 2, 2 * C * (int)sizeof(T));
-  gn_bwd_stats_k<T><<<s1.grid, s1.block, s1.smem, st>>>(
-      (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0,
-      cst1, bst, s1.P, s1.stage_bytes, s1.pro_floats);
+  launch_pdl(gn_bwd_stats_k<T>, s1.grid, s1.block, s1.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
+             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0, cst1, bst, s1.P, s1.stage_bytes, s1.pro_floats);
   const StreamPlan s2 = stream_plan(dt, n, hw, C, groups, 1, (add ? 3 : 2) * C * (int)sizeof(T));
-  gn_bwd_apply_k<T><<<s2.grid, s2.block, s2.smem, st>>>(
-      (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0,
-      cst1, bst, dgamma, dbeta, (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes,
-      s2.pro_floats);
+  launch_pdl(gn_bwd_apply_k<T>, s2.grid, s2.block, s2.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
+             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0, cst1, (const float*)bst, dgamma, dbeta,
+             (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes, s2.pro_floats);
   return 2;
 }
 

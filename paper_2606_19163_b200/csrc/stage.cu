@@ -240,7 +240,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
     }
   }
   s->zero_end = pl.bump(R_WORK, 0);
-  s->w_ga2 = pl.bump(R_WORK, m_out); s->w_gh1 = pl.bump(R_WORK, m_out);
+  s->w_ga2 = pl.bump(R_WORK, m_out); s->w_gh1 = pl.bump(R_WORK, m_out); s->w_gh1b = pl.bump(R_WORK, m_out);
   s->w_ga1 = pl.bump(R_WORK, m_cat); s->w_gsc = pl.bump(R_WORK, m_cat);
   s->w_gu = pl.bump(R_WORK, m_gu);
   s->w_tmpf = pl.bump(R_WORK, (size_t)d.n * T * 4 + 256);
@@ -274,6 +274,8 @@ extern "C" pulse_status_t pulse_stage_destroy(pulse_stage_t* s) {
   if (s) {
     for (auto& sp : s->spans) { cudaEventDestroy(sp.e0); cudaEventDestroy(sp.e1); }
     for (auto ev : s->event_pool) cudaEventDestroy(ev);
+    for (auto ev : s->sync_events) cudaEventDestroy(ev);
+    if (s->side) cudaStreamDestroy(s->side);
   }
   delete s;
   return PULSE_OK;

@@ -79,7 +79,12 @@ struct pulse_stage {
   size_t zero_begin = 0, zero_end = 0;      // workspace: backward sums area, zeroed at the start of backward
   bool wt_valid = false;                    // transposed weights match the bound parameters
   // per-stage workspace offsets (bytes)
-  size_t w_ga2 = 0, w_gh1 = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0;
+  size_t w_ga2 = 0, w_gh1 = 0, w_gh1b = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0;
+  // weight-gradient kernels run on a side stream, concurrently with the dgrad / GroupNorm chain of the backward
+  // (fork / join with events; legal inside CUDA-graph capture).  PULSE_NO_SIDE_STREAM=1 disables it.
+  cudaStream_t side = nullptr;
+  std::vector<cudaEvent_t> sync_events;
+  int side_mode = -1;                       // -1 unknown, 0 off, 1 on
   const char* d_params = nullptr; float* d_grads = nullptr;
   char* d_work = nullptr; size_t work_bound = 0;
   uint64_t launches = 0;

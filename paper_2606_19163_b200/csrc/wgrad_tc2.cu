@@ -80,6 +80,8 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
   cluster_sync_all();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
+  pdl_wait();
+  pdl_launch_dependents();
 
   if (warp == 0) {
     if (lane == 0) {
@@ -281,7 +283,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   p.work = (long long)p.m_tiles * p.n_tiles * p.pix_tiles;
   long long pairs = sm_count() / 2;                       // one CTA pair per SM pair, equal shares, >= 4 items each
   if (p.work / 4 < pairs) pairs = p.work / 4 > 0 ? p.work / 4 : 1;
-  wgrad_tc2_k<<<(unsigned)(2 * pairs), 192, SMEM, st>>>(m0, m1, mg, mg32, p);
+  launch_pdl(wgrad_tc2_k, dim3((unsigned)(2 * pairs)), dim3(192), SMEM, st, m0, m1, mg, mg32, p);
   return 1;
 }
 
