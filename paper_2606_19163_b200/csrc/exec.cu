@@ -42,7 +42,9 @@ struct Ctx {
     return n_ev - 1;
   }
   void wait_side(int ev) { if (side && ev >= 0) cudaStreamWaitEvent(st, s->sync_events[ev], 0); }
-  cudaStream_t wst() const { return side ? side : st; }
+  int side_mask = 3;             // debug (PULSE_SIDE_MASK): 1 ResBlock wgrads, 2 other ops' wgrads
+  bool in_rb = false;
+  cudaStream_t wst() const { return (side && (side_mask & (in_rb ? 1 : 2))) ? side : st; }
   char* fwd(int t) const {
     const TRef& r = s->tensors[t].ref;
     return (r.region == R_SKIP ? skip : r.region == R_STASH ? stash : work) + r.off;
@@ -214,6 +216,7 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
   const int n = s->d.n, hw = op.hin * op.win, ctot = op.cin + op.cskip;
   Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
   const int par = c.rb_count & 1;
+  c.in_rb = true;
   char* g_out = c.grad(op.out);
   char* g_a2 = c.work + s->w_ga2;
   char* g_h1 = c.work + (par ? s->w_gh1b : s->w_gh1);     // double-buffered: the side stream's wgrad1 reads it late
@@ -254,6 +257,7 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
              op.acc_x0, op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]),
              cs_of(c, op.x0), op.x1 >= 0 ? cs_of(c, op.x1) : nullptr);
   ++c.rb_count;
+  c.in_rb = false;
 }
 
 // bias / temb-projection gradients of every op from the pixel sums, in one batched launch (row a8-a10)
@@ -388,6 +392,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   if (s->side_mode == 1 && !s->profiling) {
     if (!s->side) CK_CUDA(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
     c.side = s->side;
+    if (const char* m = getenv("PULSE_SIDE_MASK")) c.side_mask = atoi(m);
   }
   if (!accumulate_wgrad)
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));

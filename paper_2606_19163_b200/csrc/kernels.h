@@ -97,6 +97,11 @@ struct WgradArgs {
   float* dw;                      // [cout][k][k][src.c()] fp32, atomically accumulated
 };
 int wgrad_simt(const WgradArgs& a, cudaStream_t st);
+// 4 channels on one side (conv_in, head; conv_thin.cu): conv_simt / wgrad_simt route to these when they apply
+bool conv_thin_supported(const ConvArgs& a);
+int conv_thin(const ConvArgs& a, cudaStream_t st);
+bool wgrad_thin_supported(const WgradArgs& a);
+int wgrad_thin(const WgradArgs& a, cudaStream_t st);
 
 // tcgen05 / TMA path (bf16 only).  *_supported say whether the shape maps onto the tiles.
 bool conv_tc_supported(const ConvArgs& a);

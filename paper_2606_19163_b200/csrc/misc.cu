@@ -172,9 +172,9 @@ __global__ void __launch_bounds__(256) small_grads_k(const float* __restrict__ e
   for (int n0 = 0; n0 < n; n0 += 8) {
     const int nn = min(8, n - n0);
     __syncthreads();
-    if (threadIdx.x < 32 * nn) {
+    {   // all 8 x 32 entries are written: rows >= nn must be 0, not stale shared memory (0 x NaN = NaN)
       const int r = threadIdx.x >> 5, c = threadIdx.x & 31;
-      sgp[r][c] = c < cn ? e.gp[(size_t)(n0 + r) * e.cout + c0 + c] : 0.f;
+      sgp[r][c] = (r < nn && c < cn) ? e.gp[(size_t)(n0 + r) * e.cout + c0 + c] : 0.f;
     }
     __syncthreads();
     if (j < Tdim) {
