@@ -99,16 +99,23 @@ __global__ void __launch_bounds__(256) thin_in_wgrad_k(const T* __restrict__ in,
     for (int c = 0; c < TC; ++c) acc[t][c] = 0.f;
   const int rows = min(R, h - y0);
   for (int ry = 0; ry < rows; ++ry)
-    for (int x = 0; x < wd; ++x) {
-      const float gv = to_f(g[(((size_t)img * h + y0 + ry) * wd + x) * cout + co]);
+    for (int x0 = 0; x0 < wd; x0 += 4) {            // 4 pixels per iteration: their g loads are independent
+      float gv[4];
 #pragma unroll
-      for (int r = 0; r < 3; ++r)
+      for (int u = 0; u < 4; ++u)
+        gv[u] = x0 + u < wd ? to_f(g[(((size_t)img * h + y0 + ry) * wd + x0 + u) * cout + co]) : 0.f;
 #pragma unroll
-        for (int s = 0; s < 3; ++s) {
-          const float4 v = patch[(ry + r) * pw + x + s];
-          acc[r * 3 + s][0] = fmaf(gv, v.x, acc[r * 3 + s][0]); acc[r * 3 + s][1] = fmaf(gv, v.y, acc[r * 3 + s][1]);
-          acc[r * 3 + s][2] = fmaf(gv, v.z, acc[r * 3 + s][2]); acc[r * 3 + s][3] = fmaf(gv, v.w, acc[r * 3 + s][3]);
-        }
+      for (int u = 0; u < 4; ++u) {
+        const int x = min(x0 + u, wd - 1);
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+          for (int s = 0; s < 3; ++s) {
+            const float4 v = patch[(ry + r) * pw + x + s];
+            acc[r * 3 + s][0] = fmaf(gv[u], v.x, acc[r * 3 + s][0]); acc[r * 3 + s][1] = fmaf(gv[u], v.y, acc[r * 3 + s][1]);
+            acc[r * 3 + s][2] = fmaf(gv[u], v.z, acc[r * 3 + s][2]); acc[r * 3 + s][3] = fmaf(gv[u], v.w, acc[r * 3 + s][3]);
+          }
+      }
     }
 #pragma unroll
   for (int t = 0; t < 9; ++t)
@@ -125,10 +132,16 @@ __global__ void __launch_bounds__(512) thin_out_k(const T* __restrict__ in, cons
                                                   const T* __restrict__ bias, T* __restrict__ out, int n, int h, int wd,
                                                   int C, int PB, int accumulate) {
   constexpr int V = Vec<T>::N;
-  extern __shared__ float sw[];                  // [4][9][C] weights, then [PB][tpp][4] partials
+  extern __shared__ float sw[];                  // weights [9][tpp][4 co][V] (+4 floats of padding per thread slot:
+                                                 // 16-byte reads at a 144-byte lane stride are bank-conflict free),
+                                                 // then [PB][tpp][4] partials
   const int tpp = C / V;                          // threads per pixel
-  float* red = sw + TC * 9 * C;
-  for (int i = threadIdx.x; i < TC * 9 * C; i += blockDim.x) sw[i] = to_f(w[i]);
+  constexpr int SLOT = TC * V + 4;
+  float* red = sw + 9 * tpp * SLOT;
+  for (int i = threadIdx.x; i < TC * 9 * C; i += blockDim.x) {
+    const int co = i / (9 * C), rem = i - co * 9 * C, tap = rem / C, c = rem - tap * C;
+    sw[(tap * tpp + c / V) * SLOT + co * V + (c % V)] = to_f(w[i]);
+  }
   __syncthreads();
   const int pl = threadIdx.x / tpp, cv = threadIdx.x - pl * tpp, ch = cv * V;
   const long long M = (long long)n * h * wd;
@@ -148,12 +161,15 @@ __global__ void __launch_bounds__(512) thin_out_k(const T* __restrict__ in, cons
           if (iy < 0 || iy >= h || ix < 0 || ix >= wd) continue;
           float v[V];
           ldv(in + ((img * h + iy) * wd + ix) * C + ch, v);
+          const float4* wp = reinterpret_cast<const float4*>(sw + ((r * 3 + s) * tpp + cv) * SLOT);
 #pragma unroll
-          for (int co = 0; co < TC; ++co) {
-            const float* wp = sw + (co * 9 + r * 3 + s) * C + ch;
+          for (int co = 0; co < TC; ++co)
 #pragma unroll
-            for (int i = 0; i < V; ++i) acc[co] = fmaf(wp[i], v[i], acc[co]);
-          }
+            for (int q = 0; q < V / 4; ++q) {
+              const float4 wv = wp[co * (V / 4) + q];
+              acc[co] = fmaf(wv.x, v[4 * q], acc[co]); acc[co] = fmaf(wv.y, v[4 * q + 1], acc[co]);
+              acc[co] = fmaf(wv.z, v[4 * q + 2], acc[co]); acc[co] = fmaf(wv.w, v[4 * q + 3], acc[co]);
+            }
         }
     }
     *reinterpret_cast<float4*>(red + ((size_t)pl * tpp + cv) * TC) = make_float4(acc[0], acc[1], acc[2], acc[3]);
@@ -198,19 +214,26 @@ __global__ void __launch_bounds__(512) thin_out_wgrad_k(const T* __restrict__ in
   long long t = pb / wd;
   int y = (int)(t % h);
   long long img = t / h;
-  for (long long p = pb; p < pe; ++p) {
-    const int iy = y + r - 1, ix = x + s - 1;
-    if (iy >= 0 && iy < h && ix >= 0 && ix < wd) {
-      float v[V];
-      ldv(in + ((img * h + iy) * wd + ix) * C + ch, v);
-      const float4 gv = *reinterpret_cast<const float4*>(sg + (p - pb) * TC);
+  for (long long p = pb; p < pe; p += 4) {          // 4 pixels per iteration: their loads are independent
+    float v[4][V];
+    bool ok[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int iy = y + r - 1, ix = x + s - 1;
+      ok[u] = p + u < pe && iy >= 0 && iy < h && ix >= 0 && ix < wd;
+      if (ok[u]) ldv(in + ((img * h + iy) * wd + ix) * C + ch, v[u]);
+      if (++x == wd) { x = 0; if (++y == h) { y = 0; ++img; } }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (!ok[u]) continue;
+      const float4 gv = *reinterpret_cast<const float4*>(sg + (p + u - pb) * TC);
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        acc[0][i] = fmaf(gv.x, v[i], acc[0][i]); acc[1][i] = fmaf(gv.y, v[i], acc[1][i]);
-        acc[2][i] = fmaf(gv.z, v[i], acc[2][i]); acc[3][i] = fmaf(gv.w, v[i], acc[3][i]);
+        acc[0][i] = fmaf(gv.x, v[u][i], acc[0][i]); acc[1][i] = fmaf(gv.y, v[u][i], acc[1][i]);
+        acc[2][i] = fmaf(gv.z, v[u][i], acc[2][i]); acc[3][i] = fmaf(gv.w, v[u][i], acc[3][i]);
       }
     }
-    if (++x == wd) { x = 0; if (++y == h) { y = 0; ++img; } }
   }
 #pragma unroll
   for (int co = 0; co < TC; ++co)
@@ -259,7 +282,7 @@ int conv_thin(const ConvArgs& a, cudaStream_t st) {
   const long long M = (long long)a.n * a.hin * a.win;
   long long blocks = (M + PB - 1) / PB;
   if (blocks > 296) blocks = 296;
-  const size_t sm = ((size_t)TC * 9 * C + (size_t)PB * tpp * TC) * sizeof(float);
+  const size_t sm = ((size_t)9 * tpp * (TC * vec + 4) + (size_t)PB * tpp * TC) * sizeof(float);
   if (a.dt == DT_F32) {
     big_smem(thin_out_k<float>, sm);
     thin_out_k<float><<<(unsigned)blocks, threads, sm, st>>>((const float*)a.src.p0, (const float*)a.w,
@@ -305,7 +328,7 @@ int wgrad_thin(const WgradArgs& a, cudaStream_t st) {
   const int vec = a.dt == DT_F32 ? 4 : 8, C = a.src.c0, tpp = C / vec;
   const int threads = (9 * tpp + 31) / 32 * 32;
   const long long M = (long long)a.n * a.hin * a.win;
-  int strip = (int)((M + 591) / 592);               // ~4 blocks per SM
+  int strip = (int)((M + 295) / 296);               // ~2 blocks per SM: fewer, longer strips = fewer atomics
   if (strip < 16) strip = 16;
   if (strip > 2048) strip = 2048;
   const long long blocks = (M + strip - 1) / strip;
