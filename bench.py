@@ -275,6 +275,35 @@ def main():
     st.profile(False)
     eager_ms = p0.elapsed_time(p1) / args.steps
 
+    # ---- the same kernel classes inside the CUDA-graph replays (CUPTI kernel records through torch.profiler) ----
+    in_graph = None
+    if graph is not None and rank == 0:
+        try:
+            from torch.profiler import profile, ProfilerActivity
+            reps = 3
+            with profile(activities=[ProfilerActivity.CUDA]) as tp:
+                for _ in range(reps):
+                    graph.replay()
+                torch.cuda.synchronize()
+            in_graph = {}
+            for e in tp.events():
+                if e.device_type != torch.autograd.DeviceType.CUDA:
+                    continue
+                nm = e.name
+                if "wgrad_tc" in nm: k = "wgrad_tc"
+                elif "conv_tc" in nm: k = "conv_tc"
+                elif "conv_simt" in nm or "wgrad_simt" in nm or "thin_" in nm: k = "conv_simt"
+                elif "gn_bwd" in nm: k = "gn_bwd"
+                elif "gn_apply" in nm or "chan_stats" in nm: k = "gn_fwd"
+                else: k = "other"
+                a = in_graph.setdefault(k, [0, 0.0])
+                a[0] += 1
+                a[1] += (e.time_range.end - e.time_range.start) / 1e3
+            in_graph = {k: {"launches_per_step": v[0] / reps, "ms_per_step": v[1] / reps} for k, v in in_graph.items()}
+        except Exception as ex:      # the event-bracket numbers above remain
+            sys.stderr.write(f"bench: CUPTI kernel timing unavailable ({ex})\n")
+            in_graph = None
+
     # ---- end to end through the public API with HOST buffers -----------------------------------------------
     host = []
     for mb in data["microbatches"]:
@@ -331,6 +360,13 @@ def main():
         if v["bytes"]:
             row["gbs"] = v["bytes"] / (v["ms"] * 1e-3) / 1e9
             row["frac_of_peak"] = row["gbs"] / hbm_peak
+        if in_graph and k in in_graph:      # same class inside the graph replays
+            g = in_graph[k]
+            row["in_graph_ms_per_step"] = g["ms_per_step"]
+            if v["flops"]:
+                row["in_graph_tflops"] = v["flops"] / K / (g["ms_per_step"] * 1e-3) / 1e12
+            if v["bytes"]:
+                row["in_graph_gbs"] = v["bytes"] / K / (g["ms_per_step"] * 1e-3) / 1e9
         kern[k] = row
     traffic = None
     try:
@@ -338,7 +374,11 @@ def main():
     except Exception:
         pass
     dom = kern.get("conv_tc") or kern.get("conv_simt") or {}
-    roofline = {"kernel": "conv_tc_k (tcgen05 implicit-GEMM fprop+dgrad)" if "conv_tc" in kern else "conv_simt_k",
+    gnk = [kern[k] for k in ("gn_fwd", "gn_bwd") if k in kern]
+    roofline = {"kernel": "conv_tc2_k (tcgen05 cta_group::2 implicit-GEMM conv, fprop + dgrad)" if "conv_tc" in kern else "conv_simt_k",
+                "timing": "CUDA-event brackets around every launch of the class, K eager steps on the launch stream",
+                "achieved_in_graph": dom.get("in_graph_tflops"),
+                "frac_in_graph": (dom.get("in_graph_tflops") or 0.0) / tf_peak,
                 "bound": "tensor", "achieved": dom.get("tflops"), "peak": tf_peak, "unit": "TFLOP/s",
                 "frac": (dom.get("tflops") or 0.0) / tf_peak, "traffic": traffic, "peak_source": peak_src,
                 "share_of_step": (dom.get("ms_per_step") or 0.0) / eager_ms}

@@ -95,34 +95,52 @@ struct TransposeBatch { int count; TransposeEntry e[BATCH]; };
 template <typename T>
 __global__ void __launch_bounds__(256) temb_proj_k(const float* __restrict__ emb, int n0, int nn, int Tdim,
                                                    const __grid_constant__ ProjBatch b) {
+  constexpr int V = Vec<T>::N;
   extern __shared__ float se[];        // [nn][Tdim]
   const ProjEntry& e = b.e[blockIdx.y];
-  const int o0 = blockIdx.x * 32;
+  const int o0 = blockIdx.x * 8;
   if (o0 >= e.cout) return;
   for (int i = threadIdx.x; i < nn * Tdim; i += blockDim.x) se[i] = siluf_(emb[(size_t)n0 * Tdim + i]);
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const T* w = (const T*)e.w;
-  const T* bias = (const T*)e.b;
-  for (int q = 0; q < 4; ++q) {
-    const int o = o0 + warp * 4 + q;
-    if (o >= e.cout) break;
-    float acc[8];
+  const int o = o0 + warp;
+  if (o >= e.cout) return;
+  const T* w = (const T*)e.w + (size_t)o * Tdim;
+  float acc[8];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+  for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+  if (Tdim % (32 * V) == 0) {
+    for (int i0 = 0; i0 < Tdim; i0 += 4 * 32 * V) {     // up to 4 vector loads per lane in flight
+      float wv[4][V];
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (i0 + u * 32 * V < Tdim) ldv(w + i0 + u * 32 * V + lane * V, wv[u]);
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (i0 + u * 32 * V < Tdim) {
+          const int i = i0 + u * 32 * V + lane * V;
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            if (j < nn)
+#pragma unroll
+              for (int k = 0; k < V; ++k) acc[j] = fmaf(wv[u][k], se[j * Tdim + i + k], acc[j]);
+        }
+    }
+  } else {
     for (int i = lane; i < Tdim; i += 32) {
-      const float wv = to_f(w[(size_t)o * Tdim + i]);
+      const float wv = to_f(w[i]);
 #pragma unroll
       for (int j = 0; j < 8; ++j)
         if (j < nn) acc[j] = fmaf(wv, se[j * Tdim + i], acc[j]);
     }
-#pragma unroll
-    for (int j = 0; j < 8; ++j)
-      if (j < nn) {
-        const float t = warp_sum(acc[j]);
-        if (lane == 0) e.out[(size_t)(n0 + j) * e.cout + o] = t + to_f(bias[o]);
-      }
   }
+  const T* bias = (const T*)e.b;
+#pragma unroll
+  for (int j = 0; j < 8; ++j)
+    if (j < nn) {
+      const float t = warp_sum(acc[j]);
+      if (lane == 0) e.out[(size_t)(n0 + j) * e.cout + o] = t + to_f(bias[o]);
+    }
 }
 
 int temb_proj_batch(int dt, const float* emb, int n, int T, const ProjEntry* e, int count, cudaStream_t st) {
@@ -134,7 +152,7 @@ int temb_proj_batch(int dt, const float* emb, int n, int T, const ProjEntry* e, 
     for (int i = 0; i < b.count; ++i) { b.e[i] = e[i0 + i]; if (e[i0 + i].cout > maxc) maxc = e[i0 + i].cout; }
     for (int n0 = 0; n0 < n; n0 += 8) {
       const int nn = n - n0 < 8 ? n - n0 : 8;
-      dim3 grid((maxc + 31) / 32, b.count);
+      dim3 grid((maxc + 7) / 8, b.count);
       const size_t smem = (size_t)nn * T * sizeof(float);
       if (dt == DT_F32) temb_proj_k<float><<<grid, 256, smem, st>>>(emb, n0, nn, T, b);
       else temb_proj_k<bf16><<<grid, 256, smem, st>>>(emb, n0, nn, T, b);
@@ -181,12 +199,23 @@ __global__ void __launch_bounds__(256) small_grads_k(const float* __restrict__ e
       float se[8], ge[8];
 #pragma unroll
       for (int r = 0; r < 8; ++r) { se[r] = r < nn ? siluf_(emb[(size_t)(n0 + r) * Tdim + j]) : 0.f; ge[r] = 0.f; }
-      for (int c = 0; c < cn; ++c) {
-        const float w = to_f(tw[(size_t)(c0 + c) * Tdim + j]);
-        float d = 0.f;
+      for (int cb = 0; cb < cn; cb += 8) {            // 8 channels per batch: 16 independent loads in flight
+        float w[8], old[8];
 #pragma unroll
-        for (int r = 0; r < 8; ++r) { d = fmaf(sgp[r][c], se[r], d); ge[r] = fmaf(sgp[r][c], w, ge[r]); }
-        e.dtw[(size_t)(c0 + c) * Tdim + j] += d;
+        for (int u = 0; u < 8; ++u)
+          if (cb + u < cn) {
+            w[u] = to_f(tw[(size_t)(c0 + cb + u) * Tdim + j]);
+            old[u] = e.dtw[(size_t)(c0 + cb + u) * Tdim + j];
+          }
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+          if (cb + u < cn) {
+            const int c = cb + u;
+            float d = old[u];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) { d = fmaf(sgp[r][c], se[r], d); ge[r] = fmaf(sgp[r][c], w[u], ge[r]); }
+            e.dtw[(size_t)(c0 + c) * Tdim + j] = d;
+          }
       }
       if (g_emb)
 #pragma unroll
