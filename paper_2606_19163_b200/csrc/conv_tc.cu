@@ -255,9 +255,9 @@ int sm_count() {
 }
 
 bool get_map(const void* ptr, int rank, const uint64_t* dims, const uint64_t* strides, const uint32_t* box,
-             CUtensorMap* out, int swizzle_bytes) {
+             CUtensorMap* out, int swizzle_bytes, int elem_bytes) {
   std::vector<uint64_t> key;
-  key.push_back((uint64_t)ptr); key.push_back(rank + 16 * (uint64_t)swizzle_bytes);
+  key.push_back((uint64_t)ptr); key.push_back(rank + 16 * (uint64_t)swizzle_bytes + 4096 * (uint64_t)elem_bytes);
   for (int i = 0; i < rank; ++i) { key.push_back(dims[i]); key.push_back(box[i]); if (i) key.push_back(strides[i - 1]); }
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_maps.find(key);
@@ -266,7 +266,7 @@ bool get_map(const void* ptr, int rank, const uint64_t* dims, const uint64_t* st
   cuuint64_t gd[5], gs[4]; cuuint32_t bx[5], es[5];
   for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; es[i] = 1; if (i) gs[i - 1] = strides[i - 1]; }
   CUtensorMap m;
-  CUresult r = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void*>(ptr), gd, gs, bx, es,
+  CUresult r = g_encode(&m, elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void*>(ptr), gd, gs, bx, es,
                         CU_TENSOR_MAP_INTERLEAVE_NONE,
                         swizzle_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
                                              : (swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE),
@@ -299,6 +299,12 @@ bool mat_map(const void* ptr, uint64_t rows, uint64_t k, int brows, CUtensorMap*
   uint64_t str[1] = {k * 2};
   uint32_t box[2] = {64, (uint32_t)brows};
   return get_map(ptr, 2, dims, str, box, out);
+}
+bool mat_map_f32(const void* ptr, uint64_t rows, uint64_t cols, int bcols, int brows, CUtensorMap* out) {
+  uint64_t dims[2] = {cols, rows};
+  uint64_t str[1] = {cols * 4};
+  uint32_t box[2] = {(uint32_t)bcols, (uint32_t)brows};
+  return get_map(ptr, 2, dims, str, box, out, 0, 4);
 }
 bool tile_geometry(int gh, int gw, int& bw, int& bh, int& bn) {
   if (gw < 8 || gw > 128 || (gw & (gw - 1))) return false;

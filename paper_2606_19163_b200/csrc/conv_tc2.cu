@@ -223,6 +223,9 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
         tmem_ld32(taddr + ch * CW, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
         if (CW == 64) tmem_ld32(taddr + ch * CW + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[CW - 32]));
         const int co = nt * C::BN + ch * CW;
+        float4 cvv[CW / 4];                          // column vector of the chunk: loaded while the TMEM load is in flight
+#pragma unroll
+        for (int i = 0; i < CW / 4; ++i) cvv[i] = *reinterpret_cast<const float4*>(colv + ch * CW + i * 4);
         tmem_ld_wait();
         if (ch == C::BN / CW - 1) {
           tc_fence_before();
@@ -230,13 +233,12 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&tempty_bar[acc]), 0));
         }
         if (!(DBG(p) & 4)) {
-          if (lane == 0) bulk_wait_read<1>();        // the store issued from this buffer two chunks ago has read it
+          if (lane == 0 && !(DBG(p) & 64)) bulk_wait_read<1>();        // the store issued from this buffer two chunks ago has read it
           __syncwarp();
           const uint32_t dst = stg_lane + buf * C::BOX_BYTES;
 #pragma unroll
           for (int i = 0; i < CW / 8; ++i) {
-            const float4 c0 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8);
-            const float4 c1 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8 + 4);
+            const float4 c0 = cvv[2 * i], c1 = cvv[2 * i + 1];
             float v[8] = {__uint_as_float(r[i * 8]) + c0.x,     __uint_as_float(r[i * 8 + 1]) + c0.y,
                           __uint_as_float(r[i * 8 + 2]) + c0.z, __uint_as_float(r[i * 8 + 3]) + c0.w,
                           __uint_as_float(r[i * 8 + 4]) + c1.x, __uint_as_float(r[i * 8 + 5]) + c1.y,
@@ -250,9 +252,9 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
             st_shared_v4(dst + ((i ^ sw) << 4), pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
                          pack_bf16(v[6], v[7]));
           }
-          fence_proxy_async_smem();
+          if (!(DBG(p) & 128)) fence_proxy_async_smem();
           __syncwarp();
-          if (lane == 0) {
+          if (lane == 0 && !(DBG(p) & 256)) {
             tma_store_4d(&mapO, stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
             bulk_commit();
           }

@@ -33,8 +33,9 @@ constexpr int BLK = PIX * 128;                // one [64 px][64 ch] box = 8 KB
 constexpr int BLK32 = PIX * 64;               // one [64 px][32 ch] box = 4 KB
 constexpr int N_TOT = 320;
 constexpr int STAGE = 2 * BLK + 2 * BLK + BLK32;      // 36 KB per CTA
-constexpr int STAGES = 6;
-constexpr int SMEM = STAGES * STAGE + 1024;
+constexpr int STAGES = 5;
+constexpr int FLUSH_BYTES = 4 * 2 * 4096;             // per epilogue warp: 2 x [32 co][32 c] fp32 boxes
+constexpr int SMEM = STAGES * STAGE + FLUSH_BYTES + 1024;
 
 #ifdef PULSE_MB
 __device__ unsigned long long g_tlw[64];
@@ -53,12 +54,14 @@ struct Wg2Params {
   int bw, bh, bn, tiles_w, tiles_h;
   int pix_tiles, m_tiles, n_tiles;       // m_tiles: pair tiles of 4 units
   long long work;
+  int ppt;                               // pairs per output tile (aligned split) or 0 (stream-K)
   float* dw;
 };
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
 wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
-            const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapG32, const Wg2Params p) {
+            const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapG32,
+            const __grid_constant__ CUtensorMap mapW, const Wg2Params p) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tfull_bar, tempty_bar;
   __shared__ uint32_t tmem_base_s;
@@ -66,11 +69,20 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
-  const long long wb = p.work * pair / npairs, we = p.work * (pair + 1) / npairs;
+  // ranges: aligned (ppt pairs per output tile, each a share of its pixel tiles: one flush per pair) when there are
+  // at least as many pairs as output tiles, else equal contiguous ranges over everything (stream-K)
+  long long wb, we;
+  if (p.ppt > 0) {
+    const int ot = pair / p.ppt, k = pair - ot * p.ppt;
+    wb = (long long)ot * p.pix_tiles + (long long)p.pix_tiles * k / p.ppt;
+    we = (long long)ot * p.pix_tiles + (long long)p.pix_tiles * (k + 1) / p.ppt;
+  } else {
+    wb = p.work * pair / npairs; we = p.work * (pair + 1) / npairs;
+  }
 
   if (threadIdx.x == 0) TL(0);
   if (warp == 0 && lane == 0) {
-    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapG); prefetch_tmap(&mapG32);
+    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapG); prefetch_tmap(&mapG32); prefetch_tmap(&mapW);
     for (int i = 0; i < STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
     mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 8);
     fence_barrier_init();
@@ -176,19 +188,24 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       }
     }
   } else {
-    // ===== epilogue (both CTAs): fp32 red.add of this CTA's 128 rows x 320 columns =====
+    // ===== epilogue (both CTAs): this CTA's 128 rows x 320 columns are ADDED into dW (fp32).  A warp owns 32
+    // consecutive channels c (its TMEM lanes); per 32 output channels it transposes its registers into a
+    // [32 co][32 c] fp32 box in shared memory (conflict-free: a row is one 128-byte line) and one TMA reduce-add
+    // instruction replaces 1024 scalar atomics.
     const int q = warp & 3;
-    const int row = q * 32 + lane;
+    uint8_t* stg = smem + STAGES * STAGE + q * 8192;
+    const uint32_t stg_lane = smem_u32(stg) + lane * 4;
     uint32_t tphase = 0;
+    int buf = 0;
     long long w = wb;
     while (w < we) {
       const int ot = (int)(w / p.pix_tiles);
       const long long seg_end = min(we, (long long)(ot + 1) * p.pix_tiles);
       const int nt = ot % p.n_tiles, mt = ot / p.n_tiles;
-      const int u = 4 * mt + 2 * (int)rank + (row >> 6);
+      const int u = 4 * mt + 2 * (int)rank + (q >> 1);
       const bool valid = u < p.units;
       const int ti = valid ? u / p.c_blocks : 0, cb = valid ? u - ti * p.c_blocks : 0;
-      const size_t kidx = (size_t)p.taps[ti].widx * p.ctot + cb * 64 + (row & 63);
+      const int kcol = p.taps[ti].widx * p.ctot + cb * 64 + (q & 1) * 32;
       mbar_wait(&tfull_bar, tphase);
       tphase ^= 1;
       tc_fence_after();
@@ -205,13 +222,23 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
           if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&tempty_bar), 0));
         }
         if (valid && !(DBGW(p) & 4)) {
-          float* dst = p.dw + (size_t)(nt * N_TOT + ch * 32) * p.ktot + kidx;
+          if (lane == 0) bulk_wait_read<1>();
+          __syncwarp();
+          const uint32_t dst = stg_lane + buf * 4096;
 #pragma unroll
-          for (int i = 0; i < 32; ++i) atomicAdd(dst + (size_t)i * p.ktot, __uint_as_float(r[i]));
+          for (int i = 0; i < 32; ++i) asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i * 128), "r"(r[i]) : "memory");
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            tma_reduce_add_2d(&mapW, stg + buf * 4096, kcol, nt * N_TOT + ch * 32);
+            bulk_commit();
+          }
+          buf ^= 1;
         }
       }
       w = seg_end;
     }
+    if (lane == 0) bulk_wait<0>();
   }
   if (warp == 2 && lane == 0) TL(5);
   tc_fence_before();
@@ -263,7 +290,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
 #ifdef PULSE_MB
   { const char* e = getenv("PULSE_DBG"); p.dbg = e ? atoi(e) : 0; }
 #endif
-  CUtensorMap m0, m1, mg, mg32;
+  CUtensorMap m0, m1, mg, mg32, mw;
   bool ok;
   if (s2) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
   else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
@@ -271,6 +298,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
   if (ok) ok = act_map(a.g, a.n, a.hout, a.wout, a.cout, p.bw, p.bh, p.bn, &mg);
   if (ok) ok = act_map_c(a.g, a.n, a.hout, a.wout, a.cout, 32, p.bw, p.bh, p.bn, &mg32);
+  if (ok) ok = mat_map_f32(a.dw, a.cout, p.ktot, 32, 32, &mw);
   if (!ok) return -1;
   static bool attr_set = false;
   if (!attr_set) {
@@ -283,7 +311,13 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   p.work = (long long)p.m_tiles * p.n_tiles * p.pix_tiles;
   long long pairs = sm_count() / 2;                       // one CTA pair per SM pair, equal shares, >= 4 items each
   if (p.work / 4 < pairs) pairs = p.work / 4 > 0 ? p.work / 4 : 1;
-  launch_pdl(wgrad_tc2_k, dim3((unsigned)(2 * pairs)), dim3(192), SMEM, st, m0, m1, mg, mg32, p);
+  const long long out_tiles = (long long)p.m_tiles * p.n_tiles;
+  p.ppt = 0;
+  if (out_tiles <= pairs && p.pix_tiles >= 4 * (pairs / out_tiles)) {       // aligned split: one flush per pair
+    p.ppt = (int)(pairs / out_tiles);
+    pairs = p.ppt * out_tiles;
+  }
+  launch_pdl(wgrad_tc2_k, dim3((unsigned)(2 * pairs)), dim3(192), SMEM, st, m0, m1, mg, mg32, mw, p);
   return 1;
 }
 
