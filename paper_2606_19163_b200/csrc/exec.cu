@@ -15,7 +15,8 @@ struct Ctx {
   char* stash;    // base of this microbatch's stash
   char* work;     // per-stage workspace
   cudaStream_t st;
-  cudaStream_t side = nullptr;   // non-null: weight-gradient kernels go here (backward only)
+  cudaStream_t side = nullptr;   // non-null: kernels off the critical chain go here (weight gradients, shortcut convs ...)
+  int ev_proj = -1;              // forward: side-stream event after the temb projections
   int n_ev = 0;                  // events of s->sync_events used by this call
   int rb_count = 0;              // ResBlocks processed so far in this backward (g_h1 double buffer / hazard events)
   int ev_rb[2] = {-1, -1};       // event recorded on the side stream after the wgrads of the last ResBlock of each parity
@@ -58,6 +59,24 @@ struct Ctx {
   }
   bool tc() const { return dt == DT_BF16 && !(s->d.flags & PULSE_FLAG_FORCE_SIMT); }
 };
+
+// launches inside the scope go to the side stream (if there is one)
+struct OnSide {
+  Ctx& c; cudaStream_t saved;
+  explicit OnSide(Ctx& c_) : c(c_), saved(c_.st) { if (c.side) c.st = c.side; }
+  ~OnSide() { c.st = saved; }
+};
+void setup_side(pulse_stage* s, Ctx& c) {
+  if (s->side_mode < 0) {
+    const char* e = getenv("PULSE_NO_SIDE_STREAM");
+    s->side_mode = (e && e[0] == '1') ? 0 : 1;
+  }
+  if (s->side_mode == 1 && !s->profiling) {
+    if (!s->side && cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking) != cudaSuccess) { s->side = nullptr; return; }
+    c.side = s->side;
+    if (const char* m = getenv("PULSE_SIDE_MASK")) c.side_mask = atoi(m);
+  }
+}
 
 // profiling span around a group of launches of one kernel class
 struct Prof {
@@ -185,18 +204,27 @@ void resblock_forward(Ctx& c, const OpPlan& op) {
   const int hw = op.hin * op.win, ctot = op.cin + op.cskip;
   Cat x{c.fwd(op.x0), op.cin, op.x1 >= 0 ? c.fwd(op.x1) : nullptr, op.cskip};
   float* pn = (float*)(c.stash + op.pn);
+  // the 1x1 shortcut needs only x: it runs beside the GN1 -> conv1 -> GN2 chain and is joined before conv2
+  const void* res = c.fwd(op.x0);
+  int ev_sc = -1;
+  if (op.p[P_SCW] >= 0) {
+    c.fork();
+    {
+      OnSide g(c);
+      run_conv(c, conv_args(c, x, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_SCW]), op.cout,
+                            c.par(op.p[P_SCB]), nullptr, nullptr, c.fwd(op.out)));
+    }
+    if (c.side) ev_sc = c.mark_side();
+    res = c.fwd(op.out);
+  }
   run_gn_fwd(c, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1));
+  if (c.ev_proj >= 0) { c.wait_side(c.ev_proj); c.ev_proj = -1; }      // temb projections (side stream) are ready
   Cat a1{c.fwd(op.a1), ctot, nullptr, 0};
   run_conv(c, conv_args(c, a1, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C1W]), op.cout,
                         c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)), op.h1);
   Cat h1{c.fwd(op.h1), op.cout, nullptr, 0};
   run_gn_fwd(c, h1, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2));
-  const void* res = c.fwd(op.x0);
-  if (op.p[P_SCW] >= 0) {
-    run_conv(c, conv_args(c, x, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_SCW]), op.cout,
-                          c.par(op.p[P_SCB]), nullptr, nullptr, c.fwd(op.out)));
-    res = c.fwd(op.out);
-  }
+  c.wait_side(ev_sc);
   Cat a2{c.fwd(op.a2), op.cout, nullptr, 0};
   run_conv(c, conv_args(c, a2, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C2W]), op.cout,
                         c.par(op.p[P_C2B]), nullptr, res, c.fwd(op.out)), op.out);
@@ -225,6 +253,14 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
   ensure_colsum(c, op.out);
   // conv2 (and shortcut) weight gradients need only g_out: fork them off now
   c.fork();
+  int ev_sc = -1;
+  if (op.p[P_SCW] >= 0 && c.side) {     // shortcut dgrad needs only g_out: side stream, joined before the GN1 backward
+    {
+      OnSide g(c);
+      run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wtsc, 1, ctot, g_sc, 0, 1, op.hin, op.win);
+    }
+    ev_sc = c.mark_side();
+  }
   WgradArgs w2{c.dt, Cat{c.fwd(op.a2), op.cout, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, op.cout, 3, 1,
                c.pgrad(op.p[P_C2W])};
   run_wgrad(c, w2);
@@ -249,7 +285,8 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
   // shortcut
   const void* add = g_out;
   if (op.p[P_SCW] >= 0) {
-    run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wtsc, 1, ctot, g_sc, 0, 1, op.hin, op.win);
+    if (c.side) c.wait_side(ev_sc);
+    else run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wtsc, 1, ctot, g_sc, 0, 1, op.hin, op.win);
     add = g_sc;
   }
   // GN1 + SiLU backward, split into g_h and g_skip (skip gradient accumulated locally)
@@ -318,9 +355,12 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
   if (open) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
-  run_stats(c, s->t_xin);
-  if (open) run_stats(c, s->t_hin);
-  {   // p[n,c] = Wt SiLU(emb) + bt of every ResBlock in one launch (row a1)
+  setup_side(s, c);
+  {   // beside the chain (side stream): p[n,c] = Wt SiLU(emb) + bt of every ResBlock in one launch (row a1), joined
+      // before the first conv1; and, on the first forward of a step, the flipped / transposed weights the backward
+      // needs (parameters may have changed since the last backward; R21), joined at the end of this call
+    c.fork();
+    OnSide g(c);
     std::vector<ProjEntry> pe;
     for (const OpPlan& op : s->ops)
       if (op.kind == PULSE_OP_RESBLOCK)
@@ -329,7 +369,11 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
       Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
       s->launches += temb_proj_batch(c.dt, emb, s->d.n, s->d.temb_dim, pe.data(), (int)pe.size(), c.st);
     }
+    if (c.side) c.ev_proj = c.mark_side();
+    if (!s->wt_valid || s->last_was_backward) prepare_weights(c);
   }
+  run_stats(c, s->t_xin);
+  if (open) run_stats(c, s->t_hin);
   for (size_t i = 0; i < s->ops.size(); ++i) {
     const OpPlan& op = s->ops[i];
     switch (op.kind) {
@@ -356,6 +400,8 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
       }
     }
   }
+  if (c.side) c.wait_side(c.mark_side());       // join
+  s->last_was_backward = false;
   if (open) CK_CUDA(cudaMemcpyAsync(d_e_out, c.fwd(s->t_eout), c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
   CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
@@ -385,18 +431,10 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
   const float* emb = (const float*)(c.stash + s->emb_off);
-  if (s->side_mode < 0) {
-    const char* e = getenv("PULSE_NO_SIDE_STREAM");
-    s->side_mode = (e && e[0] == '1') ? 0 : 1;
-  }
-  if (s->side_mode == 1 && !s->profiling) {
-    if (!s->side) CK_CUDA(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
-    c.side = s->side;
-    if (const char* m = getenv("PULSE_SIDE_MASK")) c.side_mask = atoi(m);
-  }
+  setup_side(s, c);
   if (!accumulate_wgrad)
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
-  if (!accumulate_wgrad || !s->wt_valid) prepare_weights(c);
+  if (!s->wt_valid) prepare_weights(c);        // normally done by the forward of this step (side stream)
   CK_CUDA(cudaMemsetAsync(c.work + s->zero_begin, 0, s->zero_end - s->zero_begin, c.st));
   CK_CUDA(cudaMemcpyAsync(c.grad(s->t_dout), d_g_d_out, c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
   if (open) {
@@ -459,6 +497,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   CK_CUDA(cudaGetLastError());
   cache->mb[slot] = -1;
   cache->live--;
+  s->last_was_backward = true;
   return PULSE_OK;
 }
 

@@ -85,6 +85,7 @@ struct pulse_stage {
   cudaStream_t side = nullptr;
   std::vector<cudaEvent_t> sync_events;
   int side_mode = -1;                       // -1 unknown, 0 off, 1 on
+  bool last_was_backward = true;            // a forward that follows a backward starts a new step: weights may have changed
   const char* d_params = nullptr; float* d_grads = nullptr;
   char* d_work = nullptr; size_t work_bound = 0;
   uint64_t launches = 0;
