@@ -143,19 +143,19 @@ void run_stats(Ctx& c, int t) {
   Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 0.0);      // its bytes are not algorithmic: counted as GroupNorm-forward time
   s->launches += chan_stats(c.dt, c.fwd(t), s->d.n, hw, T.ref.c, cst_of(c, t), c.st);
 }
-void run_gn_fwd(Ctx& c, Cat x, int t0, int t1, int hw, const void* gamma, const void* beta, void* a_out) {
+void run_gn_fwd(Ctx& c, Cat x, int t0, int t1, int hw, const void* gamma, const void* beta, size_t mr, void* a_out) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 2.0 * s->esz() * s->d.n * hw * x.c());
   s->launches += gn_silu_fwd(c.dt, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, cst_of(c, t0), cst_of(c, t1),
-                             a_out, c.st);
+                             (float*)(c.stash + mr), a_out, c.st);
 }
-void run_gn_bwd(Ctx& c, const void* g_a, Cat x, int t0, int t1, int hw, const void* gamma, const void* beta,
+void run_gn_bwd(Ctx& c, const void* g_a, Cat x, size_t mr, int hw, const void* gamma, const void* beta,
                 size_t bst, const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma,
                 float* dbeta, float* cs0, float* cs1) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_BWD, 0.0, (3.0 + (add ? 1.0 : 0.0)) * s->esz() * s->d.n * hw * x.c());
-  s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, cst_of(c, t0),
-                             cst_of(c, t1), (float*)(c.work + bst), add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
+  s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta,
+                             (const float*)(c.stash + mr), (float*)(c.work + bst), add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
                              cs0, cs1, c.st);
 }
 
@@ -217,13 +217,13 @@ void resblock_forward(Ctx& c, const OpPlan& op) {
     if (c.side) ev_sc = c.mark_side();
     res = c.fwd(op.out);
   }
-  run_gn_fwd(c, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), c.fwd(op.a1));
+  run_gn_fwd(c, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.mr1, c.fwd(op.a1));
   if (c.ev_proj >= 0) { c.wait_side(c.ev_proj); c.ev_proj = -1; }      // temb projections (side stream) are ready
   Cat a1{c.fwd(op.a1), ctot, nullptr, 0};
   run_conv(c, conv_args(c, a1, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C1W]), op.cout,
                         c.par(op.p[P_C1B]), pn, nullptr, c.fwd(op.h1)), op.h1);
   Cat h1{c.fwd(op.h1), op.cout, nullptr, 0};
-  run_gn_fwd(c, h1, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), c.fwd(op.a2));
+  run_gn_fwd(c, h1, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]), op.mr2, c.fwd(op.a2));
   c.wait_side(ev_sc);
   Cat a2{c.fwd(op.a2), op.cout, nullptr, 0};
   run_conv(c, conv_args(c, a2, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C2W]), op.cout,
@@ -272,7 +272,7 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
   // GN2 + SiLU backward -> g_h1, and its pixel sums g_p[n,c] (temb projection / conv1 bias gradients).
   // g_h1 of this parity was last read by the wgrad1 of the ResBlock two back: wait for it.
   c.wait_side(c.ev_rb[par]);
-  run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, op.h1, -1, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
+  run_gn_bwd(c, g_a2, Cat{c.fwd(op.h1), op.cout, nullptr, 0}, op.mr2, hw, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
              op.bst2, nullptr, g_h1, op.cout, 0, nullptr, 0, c.pgrad(op.p[P_GN2G]), c.pgrad(op.p[P_GN2B]),
              (float*)(c.work + op.gp), nullptr);
   // conv1: wgrad (side stream), dgrad
@@ -290,7 +290,7 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
     add = g_sc;
   }
   // GN1 + SiLU backward, split into g_h and g_skip (skip gradient accumulated locally)
-  run_gn_bwd(c, g_a1, x, op.x0, op.x1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.bst1, add, c.grad(op.x0), op.cin,
+  run_gn_bwd(c, g_a1, x, op.mr1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.bst1, add, c.grad(op.x0), op.cin,
              op.acc_x0, op.x1 >= 0 ? c.grad(op.x1) : nullptr, op.acc_x1, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]),
              cs_of(c, op.x0), op.x1 >= 0 ? cs_of(c, op.x1) : nullptr);
   ++c.rb_count;
@@ -393,7 +393,7 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
       }
       case PULSE_OP_HEAD: {
         run_gn_fwd(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.x0, -1, op.hin * op.win, c.par(op.p[P_GN1G]),
-                   c.par(op.p[P_GN1B]), c.fwd(op.a1));
+                   c.par(op.p[P_GN1B]), op.mr1, c.fwd(op.a1));
         run_conv(c, conv_args(c, Cat{c.fwd(op.a1), op.cin, nullptr, 0}, op.hin, op.win, op.hin, op.win, 3, 1,
                               c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)));
         break;
@@ -482,7 +482,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
         c.fork();
         run_wgrad(c, w);
         run_dgrad(c, g_out, op.hin, op.win, op.cout, op.wt1, 3, op.cin, g_a, 0, 1, op.hin, op.win);
-        run_gn_bwd(c, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.x0, -1, op.hin * op.win, c.par(op.p[P_GN1G]),
+        run_gn_bwd(c, g_a, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.mr1, op.hin * op.win, c.par(op.p[P_GN1G]),
                    c.par(op.p[P_GN1B]), op.bst1, nullptr, c.grad(op.x0), op.cin, 0, nullptr, 0,
                    c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]), cs_of(c, op.x0), nullptr);
         break;

@@ -26,14 +26,15 @@ struct Cat {
 struct RowPlan { int tpr, rows, nchunks; };
 RowPlan row_plan(int dt, int hw, int c, int n, int max_threads);
 int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st);
+// mr_out: [n][2][groups] fp32, the group means and reciprocal standard deviations, kept for the backward
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                const float* cst0, const float* cst1, void* a_out, cudaStream_t st);
+                const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st);
 // g_x = r(gamma g_y - A - xhat B) [+ add]; channels [0,dc0) -> dst0, rest -> dst1; accX: += instead of =
 // bst: [n][2][C] fp32 scratch, zeroed by the caller (per-(image, channel) sums of g_y and g_y xhat).
 // dgamma/dbeta: fp32, +=.  cs0/cs1 (nullable): [n][dc0] / [n][C-dc0] fp32, += the per-(image, channel) pixel
 // sums of what this call adds to dst0 / dst1 (bias and temb-projection gradients are made of these).
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
-                const void* beta, const float* cst0, const float* cst1, float* bst, const void* add, void* dst0,
+                const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
                 cudaStream_t st);
 

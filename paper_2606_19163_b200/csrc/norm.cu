@@ -23,6 +23,8 @@
 //    shared-memory ring filled by bulk asynchronous copies (cp.async.bulk + mbarrier, one elected thread issues).
 //    The first stages are requested at kernel entry, BEFORE the statistics prologue, so DRAM latency overlaps
 //    the prologue, and a 10 MB tensor spread over 148 CTAs is entirely in flight at once.
+#include <type_traits>
+
 #include "common.cuh"
 #include "kernels.h"
 #include "sm100.cuh"
@@ -56,6 +58,14 @@ RowPlan row_plan(int dt, int hw, int c, int n, int max_threads) {
 
 namespace {
 
+#ifdef PULSE_MB
+__device__ unsigned long long g_tlg[64];
+__device__ __forceinline__ unsigned long long gtime_() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TLG(k, i) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0) g_tlg[8 * (k) + (i)] = gtime_(); } while (0)
+#else
+#define TLG(k, i) do {} while (0)
+#endif
+
 template <typename T>
 __device__ __forceinline__ const T* cat_ptr(const T* p0, int c0, const T* p1, int c1, size_t pix, int ch) {
   return ch < c0 ? p0 + pix * c0 + ch : p1 + pix * c1 + (ch - c0);
@@ -76,6 +86,7 @@ __device__ __forceinline__ int tid_() { return threadIdx.y * blockDim.x + thread
 __device__ __forceinline__ int nthr_() { return blockDim.x * blockDim.y; }
 
 // grp[g] = mean, grp[G+g] = rstd of group g of image n, from the channel stats of the two sources
+template <typename ACC>
 __device__ __forceinline__ void group_mean_rstd(const float* __restrict__ cst0, int c0, const float* __restrict__ cst1,
                                                 int c1, int n, int hw, int G, float eps, Smem& s) {
   const int C = c0 + c1, tid = tid_(), nthr = nthr_(), cpg = C / G;
@@ -84,39 +95,45 @@ __device__ __forceinline__ void group_mean_rstd(const float* __restrict__ cst0, 
     s.cs[i] = c < c0 ? cst0[((size_t)n * 2 + which) * c0 + c] : cst1[((size_t)n * 2 + which) * c1 + (c - c0)];
   }
   __syncthreads();
-  // combined in double (R22); 4 threads per group when the CTA has that many whole warps
+  // combined in ACC (R22: double on the fp32 debug path; fp32 for bf16 tensors, where fp64 division / sqrt cost
+  // microseconds per kernel); 4 threads per group when the CTA has that many whole warps
   const bool quad = nthr >= ((4 * G + 31) & ~31);
   const int L = quad ? 4 : 1;
   for (int g0 = 0; g0 < G; g0 += quad ? G : nthr) {
     const int g = g0 + tid / L, l = tid % L;
-    double a = 0.0, b = 0.0;
+    ACC a = 0, b = 0;
     if (g < G)
-      for (int c = g * cpg + l; c < (g + 1) * cpg; c += L) { a += (double)s.cs[c]; b += (double)s.cs[C + c]; }
+      for (int c = g * cpg + l; c < (g + 1) * cpg; c += L) { a += (ACC)s.cs[c]; b += (ACC)s.cs[C + c]; }
     if (quad && tid < ((4 * G + 31) & ~31)) {
       a += __shfl_xor_sync(0xffffffffu, a, 1); b += __shfl_xor_sync(0xffffffffu, b, 1);
       a += __shfl_xor_sync(0xffffffffu, a, 2); b += __shfl_xor_sync(0xffffffffu, b, 2);
     }
     if (g < G && l == 0) {
-      const double m = (double)cpg * hw, mu = a / m;
-      double var = b / m - mu * mu;
-      if (var < 0.0) var = 0.0;
+      const ACC m = (ACC)cpg * (ACC)hw, mu = a / m;
+      ACC var = b / m - mu * mu;
+      if (var < 0) var = 0;
       s.grp[g] = (float)mu;
-      s.grp[G + g] = (float)(1.0 / sqrt(var + (double)eps));
+      s.grp[G + g] = (float)((ACC)1 / sqrt(var + (ACC)eps));
     }
   }
   __syncthreads();
 }
 
+// backward kernels: mean / rstd [n][2G] as the forward apply saved them (no statistics prologue)
+__device__ __forceinline__ void load_mean_rstd(const float* __restrict__ mr, int n, int G, Smem& s) {
+  for (int i = tid_(); i < 2 * G; i += nthr_()) s.grp[i] = mr[(size_t)n * 2 * G + i];
+  __syncthreads();
+}
+
 // per-thread normalisation coefficients of V consecutive channels: y = x sc + sh, xhat = x rr - mr
 template <typename T, int V>
-__device__ __forceinline__ void gn_coefs(const Smem& s, int G, int cpg, const T* __restrict__ gamma,
-                                         const T* __restrict__ beta, int ch, float (&sc)[V], float (&sh)[V],
-                                         float (&rr)[V], float (&mr)[V]) {
+__device__ __forceinline__ void gn_coefs(const Smem& s, int G, int cpg, const float (&gav)[V], const float (&bev)[V],
+                                         int ch, float (&sc)[V], float (&sh)[V], float (&rr)[V], float (&mr)[V]) {
 #pragma unroll
   for (int i = 0; i < V; ++i) {
     const int g = (ch + i) / cpg;
     const float mu = s.grp[g], r = s.grp[G + g];
-    const float ga = to_f(gamma[ch + i]), be = to_f(beta[ch + i]);
+    const float ga = gav[i], be = bev[i];
     rr[i] = r; mr[i] = mu * r;
     sc[i] = r * ga; sh[i] = be - mr[i] * ga;
   }
@@ -247,7 +264,8 @@ template <typename T>
 __global__ void __launch_bounds__(512, 2)
 gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw, int G, float eps,
            const T* __restrict__ gamma, const T* __restrict__ beta, const float* __restrict__ cst0,
-           const float* __restrict__ cst1, T* __restrict__ out, int P, int stage_bytes, int pro_floats) {
+           const float* __restrict__ cst1, float* __restrict__ mr_out, T* __restrict__ out, int P, int stage_bytes,
+           int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -260,17 +278,26 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
   r.pb = blockIdx.x * ppc; r.pe = min(hw, r.pb + ppc); r.nch = r.pe > r.pb ? (r.pe - r.pb + P - 1) / P : 0;
   const int i0 = r.add(p0 + (size_t)n * hw * c0, c0 * (int)sizeof(T));
   const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
+  float gav[V], bev[V];                 // parameters: loaded before the dependency wait
+#pragma unroll
+  for (int i = 0; i < V; ++i) { gav[i] = to_f(gamma[ch + i]); bev[i] = to_f(beta[ch + i]); }
+  TLG(0, 0);
   pdl_wait();
   pdl_launch_dependents();
   r.start(tid);
-  group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
+  TLG(0, 1);
+  group_mean_rstd<typename std::conditional<sizeof(T) == 4, double, float>::type>(cst0, c0, cst1, c1, n, hw, G, eps, s);
+  if (blockIdx.x == 0)        // mean / rstd for the backward kernels of this site
+    for (int i = tid; i < 2 * G; i += nthr_()) mr_out[(size_t)n * 2 * G + i] = s.grp[i];
   float sc[V], sh[V], rr[V], mr[V];
-  gn_coefs<T, V>(s, G, C / G, gamma, beta, ch, sc, sh, rr, mr);
+  gn_coefs<T, V>(s, G, C / G, gav, bev, ch, sc, sh, rr, mr);
   const bool lo = ch < c0;
   const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
   const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
+  TLG(0, 2);
   for (int c = 0; c < r.nch; ++c) {
     const uint8_t* st = r.wait(c);
+    if (c == 0) TLG(0, 3);
     const int pbase = r.pb + c * P, np = min(P, r.pe - pbase);
     for (int pl = threadIdx.y; pl < np; pl += 2 * rows) {      // two independent pixels per iteration (ILP)
       float v[2][V];
@@ -287,6 +314,7 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
     }
     r.release(c, tid);
   }
+  TLG(0, 4);
 }
 
 // ------------------------------------------------------------------------------ backward: reduction pass
@@ -295,8 +323,7 @@ template <typename T>
 __global__ void __launch_bounds__(512, 1)
 gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
-               const float* __restrict__ cst0, const float* __restrict__ cst1, float* __restrict__ bst, int P,
-               int stage_bytes, int pro_floats) {
+               const float* __restrict__ mrp, float* __restrict__ bst, int P, int stage_bytes, int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -310,20 +337,27 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   const int i0 = r.add(p0 + (size_t)n * hw * c0, c0 * (int)sizeof(T));
   const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
   const int ig = r.add(ga + (size_t)n * hw * C, C * (int)sizeof(T));
+  float gav[V], bev[V];                 // parameters: loaded before the dependency wait
+#pragma unroll
+  for (int i = 0; i < V; ++i) { gav[i] = to_f(gamma[ch + i]); bev[i] = to_f(beta[ch + i]); }
+  TLG(1, 0);
   pdl_wait();
   pdl_launch_dependents();
   r.start(tid);
-  group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
+  TLG(1, 1);
+  load_mean_rstd(mrp, n, G, s);
   float sc[V], sh[V], rr[V], mr[V], v[2][V];
-  gn_coefs<T, V>(s, G, C / G, gamma, beta, ch, sc, sh, rr, mr);
+  gn_coefs<T, V>(s, G, C / G, gav, bev, ch, sc, sh, rr, mr);
 #pragma unroll
   for (int i = 0; i < V; ++i) v[0][i] = v[1][i] = 0.f;
   const bool lo = ch < c0;
   const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
   const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
   const int goff = r.soff[ig] + ch * (int)sizeof(T), gpp = r.ppb[ig];
+  TLG(1, 2);
   for (int c = 0; c < r.nch; ++c) {
     const uint8_t* st = r.wait(c);
+    if (c == 0) TLG(1, 3);
     const int np = min(P, r.pe - (r.pb + c * P));
     for (int pl = threadIdx.y; pl < np; pl += rows) {
       float x[V], g[V];
@@ -338,7 +372,9 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
     }
     r.release(c, tid);
   }
+  TLG(1, 4);
   reduce_rows_atomic<V>(v, C, s, bst + (size_t)n * 2 * C);
+  TLG(1, 5);
 }
 
 // ------------------------------------------------------------------------------ backward: apply pass
@@ -349,8 +385,7 @@ template <typename T>
 __global__ void __launch_bounds__(512, 1)
 gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
-               const float* __restrict__ cst0, const float* __restrict__ cst1, const float* __restrict__ bst,
-               float* dgamma, float* dbeta, const T* __restrict__ add, T* dst0, int dc0, int acc0, T* dst1, int acc1,
+               const float* __restrict__ mrp, const float* __restrict__ bst, float* dgamma, float* dbeta, const T* __restrict__ add, T* dst0, int dc0, int acc0, T* dst1, int acc1,
                float* cs0, float* cs1, int P, int stage_bytes, int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
@@ -366,12 +401,17 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   const int i1 = c1 ? r.add(p1 + (size_t)n * hw * c1, c1 * (int)sizeof(T)) : i0;
   const int ig = r.add(ga + (size_t)n * hw * C, C * (int)sizeof(T));
   const int ie = add ? r.add(add + (size_t)n * hw * C, C * (int)sizeof(T)) : ig;
+  float gav[V], bev[V];                 // parameters: loaded before the dependency wait
+#pragma unroll
+  for (int i = 0; i < V; ++i) { gav[i] = to_f(gamma[ch + i]); bev[i] = to_f(beta[ch + i]); }
+  TLG(2, 0);
   pdl_wait();
   pdl_launch_dependents();
   r.start(tid);
-  group_mean_rstd(cst0, c0, cst1, c1, n, hw, G, eps, s);
+  TLG(2, 1);
+  load_mean_rstd(mrp, n, G, s);
   float sc[V], sh[V], rr[V], mr[V], k2[V], k3[V];
-  gn_coefs<T, V>(s, G, cpg, gamma, beta, ch, sc, sh, rr, mr);
+  gn_coefs<T, V>(s, G, cpg, gav, bev, ch, sc, sh, rr, mr);
   // group sums A m = sum_c gamma_c S1[c], B m = sum_c gamma_c S2[c]  (s.cs is free again: reuse it for S1|S2)
   __syncthreads();
   for (int i = tid; i < 2 * C; i += nthr) {
@@ -419,8 +459,10 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
   const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
   const int goff = r.soff[ig] + ch * (int)sizeof(T), eoff = r.soff[ie] + ch * (int)sizeof(T), gpp = C * (int)sizeof(T);
+  TLG(2, 2);
   for (int c = 0; c < r.nch; ++c) {
     const uint8_t* st = r.wait(c);
+    if (c == 0) TLG(2, 3);
     const int pbase = r.pb + c * P, np = min(P, r.pe - pbase);
     for (int pl = threadIdx.y; pl < np; pl += rows) {
       const size_t pix = (size_t)n * hw + pbase + pl;
@@ -442,6 +484,7 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
     }
     r.release(c, tid);
   }
+  TLG(2, 4);
   if (cs0 || cs1) {      // channels below dc0 -> cs0[n][dc0], the rest -> cs1[n][C - dc0]
     if (rows == 1) {
 #pragma unroll
@@ -465,6 +508,9 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
 }
 
 }  // namespace
+#ifdef PULSE_MB
+void mb_timeline_gn(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tlg, sizeof(unsigned long long) * 64); }
+#endif
 
 // ------------------------------------------------------------------------------ host launchers
 int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st) {
@@ -504,25 +550,25 @@ template <typename K> static void allow_big_smem(K kernel) {
 }
 
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                const float* cst0, const float* cst1, void* a_out, cudaStream_t st) {
+                const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st) {
   const int C = x.c();
   const StreamPlan sp = stream_plan(dt, n, hw, C, groups, 0, C * (int)dt_size(dt), 2);
   static bool attr = false;
   if (!attr) { allow_big_smem(gn_apply_k<float>); allow_big_smem(gn_apply_k<bf16>); attr = true; }
   if (dt == DT_F32)
     launch_pdl(gn_apply_k<float>, sp.grid, sp.block, sp.smem, st, (const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw,
-               groups, eps, (const float*)gamma, (const float*)beta, cst0, cst1, (float*)a_out, sp.P, sp.stage_bytes,
+               groups, eps, (const float*)gamma, (const float*)beta, cst0, cst1, mr_out, (float*)a_out, sp.P, sp.stage_bytes,
                sp.pro_floats);
   else
     launch_pdl(gn_apply_k<bf16>, sp.grid, sp.block, sp.smem, st, (const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw,
-               groups, eps, (const bf16*)gamma, (const bf16*)beta, cst0, cst1, (bf16*)a_out, sp.P, sp.stage_bytes,
+               groups, eps, (const bf16*)gamma, (const bf16*)beta, cst0, cst1, mr_out, (bf16*)a_out, sp.P, sp.stage_bytes,
                sp.pro_floats);
   return 1;
 }
 
 template <typename T>
 static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                    const float* cst0, const float* cst1, float* bst, const void* add, void* dst0, int dc0, int acc0,
+                    const float* mr, float* bst, const void* add, void* dst0, int dc0, int acc0,
                     void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st) {
   const int C = x.c();
   const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
@@ -530,21 +576,21 @@ static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps
   if (!attr) { allow_big_smem(gn_bwd_stats_k<T>); allow_big_smem(gn_bwd_apply_k<T>); attr = true; }
   const StreamPlan s1 = stream_plan(dt, n, hw, C, groups, 2, 2 * C * (int)sizeof(T));
   launch_pdl(gn_bwd_stats_k<T>, s1.grid, s1.block, s1.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
-             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0, cst1, bst, s1.P, s1.stage_bytes, s1.pro_floats);
+             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, bst, s1.P, s1.stage_bytes, s1.pro_floats);
   const StreamPlan s2 = stream_plan(dt, n, hw, C, groups, 1, (add ? 3 : 2) * C * (int)sizeof(T));
   launch_pdl(gn_bwd_apply_k<T>, s2.grid, s2.block, s2.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
-             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, cst0, cst1, (const float*)bst, dgamma, dbeta,
+             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, (const float*)bst, dgamma, dbeta,
              (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes, s2.pro_floats);
   return 2;
 }
 
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
-                const void* beta, const float* cst0, const float* cst1, float* bst, const void* add, void* dst0,
+                const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
                 cudaStream_t st) {
-  return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, cst0, cst1, bst, add, dst0, dc0, acc0,
+  return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
                                         dst1, acc1, dgamma, dbeta, cs0, cs1, st)
-                      : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, cst0, cst1, bst, add, dst0, dc0, acc0,
+                      : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st);
 }
 

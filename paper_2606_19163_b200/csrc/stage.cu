@@ -138,6 +138,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
         if (op.x1 >= 0) s->tensors[op.x1].gn_input = true;
         s->tensors[op.h1].gn_input = true;
         op.pn = pl.bump(R_STASH, (size_t)d.n * o.cout * 4);
+        op.mr1 = pl.bump(R_STASH, (size_t)d.n * 2 * G * 4); op.mr2 = pl.bump(R_STASH, (size_t)d.n * 2 * G * 4);
         upd(m_out, pix * o.cout * s->esz()); upd(m_cat, pix * ctot * s->esz());
         op.wt1 = pl.bump(R_WORK, (size_t)o.cout * 9 * ctot * s->esz());
         op.wt2 = pl.bump(R_WORK, (size_t)o.cout * 9 * o.cout * s->esz());
@@ -162,6 +163,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
         op.p[P_GN1G] = pl.param(pre + "gn.gamma", 1, o.cin); op.p[P_GN1B] = pl.param(pre + "gn.beta", 1, o.cin);
         op.p[P_C1W] = pl.param(pre + "conv.w", 4, o.cout, 3, 3, o.cin); op.p[P_C1B] = pl.param(pre + "conv.b", 1, o.cout);
         op.a1 = pl.tensor(R_STASH, o.cin, op.hin, op.win, false);
+        op.mr1 = pl.bump(R_STASH, (size_t)d.n * 2 * G * 4);
         s->tensors[op.x0].gn_input = true;
         upd(m_cat, pix * o.cin * s->esz());
         op.wt1 = pl.bump(R_WORK, (size_t)o.cout * 9 * o.cin * s->esz());

@@ -33,6 +33,7 @@ struct OpPlan {
   size_t bst1 = 0, bst2 = 0;                // R_WORK (zeroed area): GroupNorm backward sums [n][2][C] fp32 per site
   size_t gp = 0;                            // R_WORK (zeroed area): [n][cout] fp32 pixel sums of g_h1
   size_t pn = 0;                            // byte offset in the slot stash ([n,cout] fp32)
+  size_t mr1 = 0, mr2 = 0;                  // slot stash: [n][2][G] fp32 group mean / rstd of the GroupNorm sites
   size_t wt1 = 0, wt2 = 0, wtsc = 0;        // R_WORK: flipped/transposed conv weights (kept across a wave)
   int p[12];                                // parameter indices (see stage.cu)
   int push = -1, pop = -1;
