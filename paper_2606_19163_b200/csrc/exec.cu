@@ -46,11 +46,19 @@ struct Ctx {
   int side_mask = 3;             // debug (PULSE_SIDE_MASK): 1 ResBlock wgrads, 2 other ops' wgrads
   bool in_rb = false;
   cudaStream_t wst() const { return (side && (side_mask & (in_rb ? 1 : 2))) ? side : st; }
+  // boundary tensors that nothing reads after this call live directly in the caller's buffers (no copy):
+  // d_out (forward), g_d_out / g_h_in / g_x_in (backward)
+  int ov_ft = -1; char* ov_fp = nullptr;
+  int ov_gt[3] = {-1, -1, -1}; char* ov_gp[3] = {nullptr, nullptr, nullptr};
   char* fwd(int t) const {
+    if (t == ov_ft) return ov_fp;
     const TRef& r = s->tensors[t].ref;
     return (r.region == R_SKIP ? skip : r.region == R_STASH ? stash : work) + r.off;
   }
-  char* grad(int t) const { return work + s->tensors[t].goff; }
+  char* grad(int t) const {
+    for (int i = 0; i < 3; ++i) if (t == ov_gt[i]) return ov_gp[i];
+    return work + s->tensors[t].goff;
+  }
   const char* par(int p) const { return s->d_params + s->params[p].off; }
   float* pgrad(int p) const { return (float*)((char*)s->d_grads + s->params[p].goff); }
   size_t bytes(int t) const {
@@ -351,6 +359,7 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
   float* emb = (float*)(c.stash + s->emb_off);
+  if (s->tensors[s->t_dout].ref.region == R_STASH && ((uintptr_t)d_d_out & 255) == 0) { c.ov_ft = s->t_dout; c.ov_fp = (char*)d_d_out; }
   if (s->cst_end > s->cst_begin) CK_CUDA(cudaMemsetAsync(c.stash + s->cst_begin, 0, s->cst_end - s->cst_begin, c.st));
   CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
@@ -403,7 +412,7 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   if (c.side) c.wait_side(c.mark_side());       // join
   s->last_was_backward = false;
   if (open) CK_CUDA(cudaMemcpyAsync(d_e_out, c.fwd(s->t_eout), c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
-  CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+  if (c.ov_ft < 0) CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   cache->mb[slot] = mb;
@@ -436,7 +445,11 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
   if (!s->wt_valid) prepare_weights(c);        // normally done by the forward of this step (side stream)
   CK_CUDA(cudaMemsetAsync(c.work + s->zero_begin, 0, s->zero_end - s->zero_begin, c.st));
-  CK_CUDA(cudaMemcpyAsync(c.grad(s->t_dout), d_g_d_out, c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+  const bool al = (((uintptr_t)d_g_d_out | (uintptr_t)d_g_h_in | (uintptr_t)d_g_x_in) & 255) == 0;
+  if (al) { c.ov_gt[0] = s->t_dout; c.ov_gp[0] = (char*)const_cast<void*>(d_g_d_out); }       // read in place
+  else CK_CUDA(cudaMemcpyAsync(c.grad(s->t_dout), d_g_d_out, c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+  if (al && open && s->t_hin != s->t_dout) { c.ov_gt[1] = s->t_hin; c.ov_gp[1] = (char*)d_g_h_in; }
+  if (al && d_g_x_in && s->t_xin != s->t_dout && s->t_xin != s->t_eout) { c.ov_gt[2] = s->t_xin; c.ov_gp[2] = (char*)d_g_x_in; }
   if (open) {
     if (d_g_e_out) CK_CUDA(cudaMemcpyAsync(c.grad(s->t_eout), d_g_e_out, c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
     else CK_CUDA(cudaMemsetAsync(c.grad(s->t_eout), 0, c.bytes(s->t_eout), c.st));
@@ -491,8 +504,8 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   }
   small_grads(c, emb, d_g_temb);
   if (c.side) c.wait_side(c.mark_side());      // join: the caller's stream sees every weight gradient complete
-  if (open) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
-  if (d_g_x_in) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
+  if (open && c.ov_gt[1] < 0) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
+  if (d_g_x_in && c.ov_gt[2] < 0) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   cache->mb[slot] = -1;
