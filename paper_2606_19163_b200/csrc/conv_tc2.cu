@@ -75,7 +75,7 @@ template <int UN, int NJ> struct Cfg2 {
 };
 
 template <int UN, int NJ>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
 conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
            const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CUtensorMap mapO, const Tc2Params p) {
   using C = Cfg2<UN, NJ>;
@@ -93,7 +93,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB); prefetch_tmap(&mapO);
     for (int i = 0; i < C::STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&tfull_bar[i], 1); mbar_init(&tempty_bar[i], 8); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull_bar[i], 1); mbar_init(&tempty_bar[i], 16); }
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc2(&tmem_base_s, C::TMEM_COLS);
@@ -176,23 +176,27 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       }
     }
   } else {
-    // ===== epilogue (both CTAs): warps 2..5 own TMEM lane quadrants (warp % 4) = 32 of this CTA's 128 pixels.
+    // ===== epilogue (both CTAs): warps 2..9; TMEM lane quadrant warp % 4 = 32 of this CTA's 128 pixels, and the two
+    // warps of a quadrant (on the same scheduler) take alternate channel chunks: the epilogue is a chain of
+    // dependent TMEM load -> convert -> shared store -> TMA store steps, two warps per scheduler hide its latencies.
     // Per 32-channel chunk: tcgen05.ld -> +bias +temb/residual -> bf16 -> this warp's staging buffer (64-byte
     // swizzle, conflict-free) -> one TMA store of the [32 pixels][32 channels] box.  The store clips rows that fall
     // outside the tensor (ragged tiles) and keeps the global writes as full 64-byte segments.
     constexpr int CW = C::CW;
-    const int q = warp & 3;
+    const int q = warp & 3, grp = (warp - 2) >> 2;
     const int row = q * 32 + lane;
     const int n_l = row / (p.bh * p.bw), rem = row - n_l * (p.bh * p.bw);
     const int y_l = rem / p.bw, x = rem - y_l * p.bw;
     // box origin of this warp inside the tile (lane 0's pixel)
     const int row0 = q * 32, n_w = row0 / (p.bh * p.bw), rem0 = row0 - n_w * (p.bh * p.bw);
     const int y_w = rem0 / p.bw, x_w = rem0 - y_w * p.bw;
-    uint8_t* stg = smem + C::STAGES * C::STAGE_BYTES + q * (2 * C::BOX_BYTES + 2048);
-    float* colv = reinterpret_cast<float*>(stg + 2 * C::BOX_BYTES);      // [BN] bias (+ temb projection of this image)
+    uint8_t* stg_q = smem + C::STAGES * C::STAGE_BYTES + q * (2 * C::BOX_BYTES + 2048);
+    float* colv = reinterpret_cast<float*>(stg_q + 2 * C::BOX_BYTES);    // [BN] bias (+ temb projection of this image)
+    uint8_t* stg = stg_q + grp * C::BOX_BYTES;                           // this warp's staging box
     const uint32_t stg_lane = smem_u32(stg) + lane * (CW * 2);
     const int sw = CW == 64 ? (lane & 7) : ((lane >> 1) & 3);            // 128-byte / 64-byte swizzle of 16-byte pieces
-    int acc = 0, buf = 0; uint32_t acc_phase = 0;
+    int acc = 0; uint32_t acc_phase = 0;
+    constexpr int buf = 0;
     for (int tile = pair; tile < total_tiles; tile += npairs) {
       const int mp = tile / p.n_tiles, nt = tile - mp * p.n_tiles;
       const int mt = 2 * mp + (int)rank;
@@ -203,22 +207,24 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
                              p.cout_total + (size_t)nt * C::BN;
       const bf16* addend = p.residual ? p.residual : (p.accumulate ? p.out : nullptr);
       const unsigned vmask = __ballot_sync(0xffffffffu, valid);
-      {   // column vector of this warp's image, staged while the main loop runs
+      {   // column vector of this quadrant's image, staged while the main loop runs (by the first warp of the pair;
+          // named barrier 1 + q joins the quadrant's two warps before and after)
         const int nw = min(n_t + n_w, p.GN - 1);
-        __syncwarp();
-        for (int c = lane; c < C::BN; c += 32) {
-          float t = p.bias ? to_f(p.bias[nt * C::BN + c]) : 0.f;
-          if (p.pn) t += p.pn[(size_t)nw * p.cout_total + nt * C::BN + c];
-          colv[c] = t;
-        }
-        __syncwarp();
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + q) : "memory");
+        if (grp == 0)
+          for (int c = lane; c < C::BN; c += 32) {
+            float t = p.bias ? to_f(p.bias[nt * C::BN + c]) : 0.f;
+            if (p.pn) t += p.pn[(size_t)nw * p.cout_total + nt * C::BN + c];
+            colv[c] = t;
+          }
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + q) : "memory");
       }
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       if (warp == 2 && lane == 0) TL(4);
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * C::BN;
 #pragma unroll 1
-      for (int ch = 0; ch < C::BN / CW; ++ch) {
+      for (int ch = grp; ch < C::BN / CW; ch += 2) {
         uint32_t r[CW];
         tmem_ld32(taddr + ch * CW, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
         if (CW == 64) tmem_ld32(taddr + ch * CW + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[CW - 32]));
@@ -227,13 +233,13 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
 #pragma unroll
         for (int i = 0; i < CW / 4; ++i) cvv[i] = *reinterpret_cast<const float4*>(colv + ch * CW + i * 4);
         tmem_ld_wait();
-        if (ch == C::BN / CW - 1) {
+        if (ch + 2 >= C::BN / CW) {                 // this warp's last TMEM read of the tile
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&tempty_bar[acc]), 0));
         }
         if (!(DBG(p) & 4)) {
-          if (lane == 0 && !(DBG(p) & 64)) bulk_wait_read<1>();        // the store issued from this buffer two chunks ago has read it
+          if (lane == 0 && !(DBG(p) & 64)) bulk_wait_read<0>();        // this warp's previous store has read the box
           __syncwarp();
           const uint32_t dst = stg_lane + buf * C::BOX_BYTES;
 #pragma unroll
@@ -285,7 +291,6 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
             atomicAdd(dst + p.cout_total, q0); atomicAdd(dst + p.cout_total + 1, q1);
             } else if (s0 + s1 + q0 + q1 == 123.456f) dst[0] = s0;
           }
-          buf ^= 1;
         }
       }
       if (C::ACC == 2) { acc ^= 1; if (acc == 0) acc_phase ^= 1; }
@@ -323,7 +328,7 @@ bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b,
   const int tiles = p.pair_tiles_m * p.n_tiles;
   const int max_pairs = sm_count() / 2;
   const int pairs = tiles < max_pairs ? tiles : max_pairs;
-  launch_pdl(conv_tc2_k<UN, NJ>, dim3(2 * pairs), dim3(192), Cfg2<UN, NJ>::SMEM, st, a0, a1, b, o, p);
+  launch_pdl(conv_tc2_k<UN, NJ>, dim3(2 * pairs), dim3(320), Cfg2<UN, NJ>::SMEM, st, a0, a1, b, o, p);
   return true;
 }
 
