@@ -38,6 +38,11 @@ int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
                 cudaStream_t st);
 
+// the same in one launch (norm_fused.cu; bf16, mean / rstd from the forward); 0 = shape not covered, nothing launched
+int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* gamma, const void* beta, const float* mr,
+                 const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta,
+                 float* cs0, float* cs1, cudaStream_t st);
+
 // ---- small ops -----------------------------------------------------------------------
 // cs[n][c] += sum over pixels of g[n][hw][c]   (tensors whose writers could not emit their column sums)
 int colsum(int dt, const void* g, int n, int hw, int c, float* cs, cudaStream_t st);

@@ -572,6 +572,11 @@ static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps
                     void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st) {
   const int C = x.c();
   const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
+  if (dt == DT_BF16) {        // one pass with the tensors resident in shared memory where the shape allows (norm_fused.cu)
+    const int r = gn_bwd_fused(g_a, x, n, hw, groups, gamma, beta, mr, add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
+                               cs0, cs1, st);
+    if (r > 0) return r;
+  }
   static bool attr = false;
   if (!attr) { allow_big_smem(gn_bwd_stats_k<T>); allow_big_smem(gn_bwd_apply_k<T>); attr = true; }
   const StreamPlan s1 = stream_plan(dt, n, hw, C, groups, 2, 2 * C * (int)sizeof(T));

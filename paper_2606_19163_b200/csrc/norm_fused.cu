@@ -1,0 +1,352 @@
+// norm_fused.cu - GroupNorm + SiLU backward in ONE pass over memory (SURVEY.md 8c item 1, bf16 tensors).
+//   g_y = g_a SiLU'(y); S1[c] = sum_pix g_y; S2[c] = sum_pix g_y xhat; A = mean_S gamma g_y; B = mean_S gamma g_y xhat;
+//   g_x = r (gamma g_y - A - xhat B) [+ add];  dgamma += S2, dbeta += S1
+// The two-kernel form (norm.cu: gn_bwd_stats_k, then gn_bwd_apply_k) reads x and g_a twice and pays two launches
+// with their ramps; at 10 MB per tensor those ramps are most of the time.  GroupNorm groups are independent, so a
+// work item here is (image, slice of whole groups): Cs = lcm(channels per group, 8) channels, i.e. 16-byte
+// aligned channel vectors.  A CLUSTER of CL CTAs owns one item; each CTA keeps its 1/CL of the pixels of x and g_a
+// resident in shared memory (TMA boxes [BR pixels][Cs channels], no swizzle: a pixel's Cs channels are one row):
+//   phase 1  as the boxes land: the per-channel S1, S2; CTA reduction through shared memory, cluster reduction
+//            through distributed shared memory
+//   phase 2  g_x from the resident x and g_a: no second read (g_y is recomputed in fp32: keeping it in shared
+//            memory as bf16 would add a rounding the two-kernel form does not have); `add` (the shortcut
+//            gradient) streams in through a per-thread cp.async ring started before the reductions.
+// Falls back (returns 0) when a slice of one image does not fit into 8 CTAs' shared memory or the channel split
+// does not fall on slice boundaries; norm.cu then runs the two-kernel form.
+#include <cuda.h>
+
+#include <cstdlib>
+
+#include "common.cuh"
+#include "kernels.h"
+#include "sm100.cuh"
+#include "tmap.h"
+
+namespace pulse {
+
+namespace {
+
+using namespace sm100;
+
+constexpr int MAXBOX = 16;     // TMA boxes per tensor per CTA
+constexpr int ED = 2;          // depth of the per-thread cp.async ring for `add`
+constexpr int NP = 8;          // partial sums per value in the second stage of the CTA reduction
+constexpr int MAXCS = 120;     // widest slice (channels per group 30 -> lcm(30, 8))
+
+#ifdef PULSE_MB
+__device__ unsigned long long g_tlf[16];
+__device__ __forceinline__ unsigned long long gtimef_() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TLF(i) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) g_tlf[i] = gtimef_(); } while (0)
+#else
+#define TLF(i) do {} while (0)
+#endif
+
+struct GnfParams {
+  int c0, c1, hw, G, Cs, CL, ppc, BR, nbox, nrow;
+  const bf16* gamma; const bf16* beta; const float* mr;
+  float* dgamma; float* dbeta;
+  const bf16* add; bf16* dst0; bf16* dst1; int dc0, acc0, acc1;
+  float* cs0; float* cs1;
+  int data_bytes, red_floats;
+};
+
+__device__ __forceinline__ void lds8(const uint8_t* p, float (&o)[8]) { ldv(reinterpret_cast<const bf16*>(p), o); }
+
+// sum v[K] over the `nrow` threads that share a channel vector; result[j], j < K * tpp (layout [k][Cs]) is returned
+// to every thread through `out` (shared memory, K * Cs floats).  Whole CTA; `red` holds nrow * K * Cs + NP * K * Cs floats.
+template <int K>
+__device__ __forceinline__ void cta_reduce(const float (&v)[K][8], bool active, int row, int vec, int nrow, int Cs,
+                                           float* red, float* out) {
+  const int W = K * Cs, tid = threadIdx.x;
+  if (active) {
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      float4* d = reinterpret_cast<float4*>(red + (size_t)row * W + k * Cs + vec * 8);
+      d[0] = make_float4(v[k][0], v[k][1], v[k][2], v[k][3]);
+      d[1] = make_float4(v[k][4], v[k][5], v[k][6], v[k][7]);
+    }
+  }
+  __syncthreads();
+  float* red2 = red + (size_t)nrow * W;
+  for (int u = tid; u < NP * W; u += blockDim.x) {
+    const int part = u / W, j = u - part * W;
+    float t = 0.f;
+    for (int r = part; r < nrow; r += NP) t += red[(size_t)r * W + j];
+    red2[u] = t;
+  }
+  __syncthreads();
+  if (tid < W) {
+    float t = 0.f;
+#pragma unroll
+    for (int q = 0; q < NP; ++q) t += red2[q * W + tid];
+    out[tid] = t;
+  }
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(512, 1)
+gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant__ CUtensorMap mapX1,
+               const __grid_constant__ CUtensorMap mapG, const GnfParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t fullx[MAXBOX], fullg[MAXBOX];
+  __shared__ float tot[2 * MAXCS];          // S1 | S2 of the slice: this CTA, then the whole cluster
+  __shared__ float grpAB[2][MAXCS / 8];     // A, B per group of the slice
+  uint8_t* base = smem_raw + ((128 - (smem_u32(smem_raw) & 127)) & 127);
+  uint8_t* xs = base;
+  uint8_t* gs = xs + p.data_bytes;
+  float* red = reinterpret_cast<float*>(gs + p.data_bytes);
+  float* cl = red + p.red_floats;                                  // [CL][2 Cs]: every CTA's S1 | S2
+  uint8_t* ering = reinterpret_cast<uint8_t*>(cl + p.CL * 2 * p.Cs);
+
+  const int tid = threadIdx.x, Cs = p.Cs, tpp = Cs >> 3, nrow = p.nrow, nthr = nrow * tpp;
+  const uint32_t rank = cluster_ctarank();
+  const int slice = blockIdx.x / p.CL, n = blockIdx.y;
+  const int C = p.c0 + p.c1, chs = slice * Cs, cpg = C / p.G, rb = Cs * 2;
+  const bool active = tid < nthr;
+  const int row = active ? tid / tpp : 0, vec = active ? tid - row * tpp : 0, ch = chs + vec * 8;
+  const int prow = n * p.hw + (int)rank * p.ppc;       // first pixel (row of the [n hw][C] matrices) of this CTA
+
+  TLF(0);
+  if (tid == 0) {
+    prefetch_tmap(&mapX0); prefetch_tmap(&mapX1); prefetch_tmap(&mapG);
+    for (int b = 0; b < p.nbox; ++b) { mbar_init(&fullx[b], 1); mbar_init(&fullg[b], 1); }
+    fence_barrier_init();
+    // x is a tensor of the FORWARD pass: not written by the previous kernel, so its boxes are requested before the
+    // dependency wait and stream in while that kernel drains
+    const bool lo = chs < p.c0;
+    for (int b = 0; b < p.nbox; ++b) {
+      mbar_expect_tx(&fullx[b], (uint32_t)(p.BR * rb));
+      tma_load_2d(xs + (size_t)b * p.BR * rb, lo ? &mapX0 : &mapX1, &fullx[b], lo ? chs : chs - p.c0, prow + b * p.BR);
+    }
+  }
+  cluster_arrive();                          // #1: waited on before the first remote shared-memory write
+  float sc[8], sh[8], rr[8], mr[8];
+  {
+    float gav[8], bev[8];
+    ldv(p.gamma + ch, gav); ldv(p.beta + ch, bev);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int g = (ch + i) / cpg;
+      const float mu = p.mr[(size_t)n * 2 * p.G + g], r = p.mr[(size_t)n * 2 * p.G + p.G + g];
+      rr[i] = r; mr[i] = mu * r;
+      sc[i] = r * gav[i]; sh[i] = bev[i] - mr[i] * gav[i];
+    }
+  }
+  TLF(1);
+  pdl_wait();
+  pdl_launch_dependents();
+  TLF(2);
+  if (tid == 0)
+    for (int b = 0; b < p.nbox; ++b) {
+      mbar_expect_tx(&fullg[b], (uint32_t)(p.BR * rb));
+      tma_load_2d(gs + (size_t)b * p.BR * rb, &mapG, &fullg[b], chs, prow + b * p.BR);
+    }
+  __syncthreads();                           // barrier initialisation is visible to every thread
+
+  // ---- phase 1 ------------------------------------------------------------------------------------------
+  float S[2][8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) S[0][i] = S[1][i] = 0.f;
+  if (active) {
+    int waited = 0;
+    for (int pl = row; pl < p.ppc; pl += nrow) {
+      const int b = pl / p.BR;
+      while (waited <= b) { mbar_wait(&fullx[waited], 0); mbar_wait(&fullg[waited], 0); ++waited; }
+      const int off = pl * rb + vec * 16;
+      float x[8], g[8];
+      lds8(xs + off, x); lds8(gs + off, g);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float y = fmaf(x[i], sc[i], sh[i]);
+        const float s = sigmoidf_(y);
+        const float gy = g[i] * fmaf(y * s, 1.0f - s, s);
+        S[0][i] += gy;
+        S[1][i] = fmaf(gy, fmaf(x[i], rr[i], -mr[i]), S[1][i]);
+      }
+    }
+  }
+  TLF(3);
+  // `add` ring: the first ED pixels of this thread are requested now, their latency hides behind the reductions
+  const size_t gpix0 = (size_t)prow;
+  const uint32_t eslot = smem_u32(ering) + (uint32_t)tid * 16;
+  if (p.add) {
+#pragma unroll
+    for (int d = 0; d < ED; ++d) {
+      const int pl = row + d * nrow;
+      if (active && pl < p.ppc) cp_async16(eslot + (uint32_t)d * nthr * 16, p.add + (gpix0 + pl) * C + ch);
+      cp_async_commit();
+    }
+  }
+  cta_reduce<2>(S, active, row, vec, nrow, Cs, red, tot);
+  TLF(4);
+  // cluster reduction: every CTA writes its 2 Cs sums into slot [rank] of every CTA of the cluster
+  cluster_wait();                            // #1: every CTA of the cluster is running
+  if (tid < 2 * Cs) {
+    const float v = tot[tid];
+    const uint32_t a = smem_u32(cl + (size_t)rank * 2 * Cs + tid);
+    for (int q = 0; q < p.CL; ++q) st_cluster_f32(mapa_u32(a, (uint32_t)q), v);
+  }
+  cluster_arrive();                          // #2 (release): the remote writes above ...
+  cluster_wait();                            //    (acquire): ... are visible to everyone
+  if (tid < 2 * Cs) {
+    float t = 0.f;
+    for (int q = 0; q < p.CL; ++q) t += cl[(size_t)q * 2 * Cs + tid];
+    tot[tid] = t;
+    if (rank == 0) atomicAdd((tid < Cs ? p.dbeta + chs + tid : p.dgamma + chs + (tid - Cs)), t);
+  }
+  __syncthreads();
+  if (tid < Cs / cpg) {                      // A, B of the groups of this slice
+    float a = 0.f, b = 0.f;
+    for (int c = tid * cpg; c < (tid + 1) * cpg; ++c) {
+      const float ga = to_f(p.gamma[chs + c]);
+      a = fmaf(ga, tot[c], a); b = fmaf(ga, tot[Cs + c], b);
+    }
+    const float inv = 1.0f / ((float)cpg * (float)p.hw);
+    grpAB[0][tid] = a * inv; grpAB[1][tid] = b * inv;
+  }
+  __syncthreads();
+
+  TLF(5);
+  // ---- phase 2 ------------------------------------------------------------------------------------------
+  float k2[8], k3[8], sum[1][8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int g = (vec * 8 + i) / cpg;
+    k2[i] = grpAB[0][g] * rr[i];
+    k3[i] = grpAB[1][g] * rr[i];
+    sum[0][i] = 0.f;
+  }
+  const bool first = ch < p.dc0;
+  bf16* dst = first ? p.dst0 : p.dst1;
+  const int dC = first ? p.dc0 : C - p.dc0, dch = first ? ch : ch - p.dc0;
+  const int acc = first ? p.acc0 : p.acc1;
+  if (active) {
+    int it = 0;
+    for (int pl = row; pl < p.ppc; pl += nrow, ++it) {
+      const int off = pl * rb + vec * 16;
+      float x[8], g[8], o[8];
+      lds8(xs + off, x); lds8(gs + off, g);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {          // g_y again, in fp32 (keeping it in shared memory would round it to bf16)
+        const float y = fmaf(x[i], sc[i], sh[i]);
+        const float s = sigmoidf_(y);
+        const float gy = g[i] * fmaf(y * s, 1.0f - s, s);
+        o[i] = sc[i] * gy - k2[i] - fmaf(x[i], rr[i], -mr[i]) * k3[i];
+      }
+      if (p.add) {
+        cp_async_wait<ED - 1>();             // the oldest outstanding request (this pixel's) has landed
+        float e[8];
+        const uint32_t slot = eslot + (uint32_t)(it % ED) * nthr * 16;
+        lds8(ering + (slot - smem_u32(ering)), e);
+        const int pn = pl + ED * nrow;       // refill the slot just read
+        if (pn < p.ppc) cp_async16(slot, p.add + (gpix0 + pn) * C + ch);
+        cp_async_commit();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) o[i] += e[i];
+      }
+#pragma unroll
+      for (int i = 0; i < 8; ++i) sum[0][i] += o[i];
+      bf16* d = dst + (gpix0 + pl) * dC + dch;
+      if (acc) {
+        float f[8];
+        ldv(d, f);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) o[i] += f[i];
+      }
+      stv(d, o);
+    }
+  }
+  TLF(6);
+  if (p.cs0 || p.cs1) {        // per-(image, channel) sums of what this launch adds to dst0 / dst1
+    cta_reduce<1>(sum, active, row, vec, nrow, Cs, red, tot);
+    if (tid < Cs) {
+      const int c = chs + tid;
+      if (c < p.dc0) { if (p.cs0) atomicAdd(p.cs0 + (size_t)n * p.dc0 + c, tot[tid]); }
+      else if (p.cs1) atomicAdd(p.cs1 + (size_t)n * (C - p.dc0) + (c - p.dc0), tot[tid]);
+    }
+  }
+  TLF(7);
+}
+
+}  // namespace
+#ifdef PULSE_MB
+void mb_timeline_gnf(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tlf, sizeof(unsigned long long) * 16); }
+#endif
+
+static int gcd_(int a, int b) { while (b) { const int t = a % b; a = b; b = t; } return a; }
+
+// One launch, or 0 when the shape is not covered (the caller then runs the two-kernel form).
+int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* gamma, const void* beta, const float* mr,
+                 const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta,
+                 float* cs0, float* cs1, cudaStream_t st) {
+  static int enabled = -1;
+  if (enabled < 0) { const char* e = getenv("PULSE_NO_GN_FUSED"); enabled = (e && e[0] == '1') ? 0 : 1; }
+  if (!enabled) return 0;
+  const int C = x.c();
+  if (groups <= 0 || C % groups) return 0;
+  const int cpg = C / groups;
+  const int Cs = cpg / gcd_(cpg, 8) * 8;               // lcm(cpg, 8)
+  if (Cs > MAXCS || C % Cs || x.c0 % Cs || dc0 % Cs || (x.c1 && x.c1 % 8) || x.c0 % 8) return 0;
+  if ((long long)n * hw >= (1LL << 31) / Cs) return 0;
+  const int tpp = Cs / 8, rb = Cs * 2;
+  const int slices = C / Cs;
+  const int budget = 227 * 1024 - 128 - 2048;          // dynamic shared memory: alignment slack, static arrays
+  GnfParams p;
+  int CL = 0, smem = 0;
+  for (int cl = 1; cl <= 8; cl *= 2) {
+    if (hw % cl) break;
+    const int ppc = hw / cl;
+    int nrow = 512 / tpp;
+    if (nrow > ppc) nrow = ppc;
+    int BR = ppc;
+    while (BR > 128 && BR % 2 == 0) BR /= 2;
+    while (ppc / BR > MAXBOX && BR * 2 <= 256 && ppc % (BR * 2) == 0) BR *= 2;
+    if (BR > 256 || ppc % BR || ppc / BR > MAXBOX || (BR * rb) % 128) continue;
+    const int data = ppc * rb;
+    const int red = nrow * 2 * Cs + NP * 2 * Cs;
+    const int need = 2 * data + (red + cl * 2 * Cs) * 4 + (add ? ED * nrow * tpp * 16 : 0);
+    if (need > budget) continue;
+    // the smallest cluster that fits; a larger one only while the grid would leave most SMs idle
+    const long long ctas = (long long)n * slices * cl;
+    CL = cl; smem = need + 128;
+    p.ppc = ppc; p.BR = BR; p.nbox = ppc / BR; p.nrow = nrow; p.data_bytes = data; p.red_floats = red;
+    if (ctas * 4 >= 3LL * tmap::sm_count() || ppc / 2 < 4 * nrow) break;
+  }
+  if (!CL) return 0;
+  p.c0 = x.c0; p.c1 = x.c1; p.hw = hw; p.G = groups; p.Cs = Cs; p.CL = CL;
+  p.gamma = (const bf16*)gamma; p.beta = (const bf16*)beta; p.mr = mr; p.dgamma = dgamma; p.dbeta = dbeta;
+  p.add = (const bf16*)add; p.dst0 = (bf16*)dst0; p.dst1 = (bf16*)dst1; p.dc0 = dc0; p.acc0 = acc0; p.acc1 = acc1;
+  p.cs0 = cs0; p.cs1 = cs1;
+  CUtensorMap mx0, mx1, mg;
+  const uint64_t rows = (uint64_t)n * hw;
+  auto mk = [&](const void* ptr, int c, CUtensorMap* m) {
+    const uint64_t dims[2] = {(uint64_t)c, rows}, str[1] = {(uint64_t)c * 2};
+    const uint32_t box[2] = {(uint32_t)Cs, (uint32_t)p.BR};
+    return tmap::get_map(ptr, 2, dims, str, box, m, 0);
+  };
+  if (!mk(x.p0, x.c0, &mx0)) return 0;
+  if (x.c1) { if (!mk(x.p1, x.c1, &mx1)) return 0; } else mx1 = mx0;
+  if (!mk(g_a, C, &mg)) return 0;
+  static bool attr = false;
+  if (!attr) {
+    if (cudaFuncSetAttribute(gn_bwd_fused_k, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048) != cudaSuccess) {
+      cudaGetLastError();
+      enabled = 0;
+      return 0;
+    }
+    attr = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(slices * CL, n); cfg.blockDim = dim3((p.nrow * tpp + 31) & ~31);
+  cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[1].val.programmaticStreamSerializationAllowed = pdl_enabled() ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = 2;
+  if (cudaLaunchKernelEx(&cfg, gn_bwd_fused_k, mx0, mx1, mg, p) != cudaSuccess) { cudaGetLastError(); return 0; }
+  return 1;
+}
+
+}  // namespace pulse
