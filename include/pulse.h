@@ -51,7 +51,11 @@ enum { PULSE_OP_CONV_IN = 0, PULSE_OP_RESBLOCK = 1, PULSE_OP_DOWN = 2, PULSE_OP_
 enum { PULSE_LINK_OPEN = 0, PULSE_LINK_CLOSED = 1 };
 enum { PULSE_TEMB_SINUSOIDAL = 0, PULSE_TEMB_MLP = 1 };
 /* flags */
-enum { PULSE_FLAG_FORCE_SIMT = 1  /* debug: CUDA-core fp32-accumulate convs even for bf16 */ };
+enum {
+  PULSE_FLAG_FORCE_SIMT = 1,    /* debug: CUDA-core fp32-accumulate convs even for bf16 */
+  PULSE_FLAG_GN_TWO_PASS = 2    /* debug: GroupNorm backward always as reduction pass + apply pass (never the
+                                   one-pass cluster kernel); same arithmetic, different summation order */
+};
 
 /* One operation of the linearised model.  cin excludes the popped skip:
  * a decoder ResBlock runs on concat_C(h[cin], skip[skip_channels]), h first. */

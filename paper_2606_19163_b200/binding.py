@@ -21,6 +21,7 @@ lib = C.CDLL(LIB_PATH)
 F32, BF16 = 0, 1
 OP_KIND = {"conv_in": 0, "resblock": 1, "down": 2, "up": 3, "head": 4}
 FLAG_FORCE_SIMT = 1
+FLAG_GN_TWO_PASS = 2
 
 
 class OpDesc(C.Structure):

@@ -164,7 +164,7 @@ void run_gn_bwd(Ctx& c, const void* g_a, Cat x, size_t mr, int hw, const void* g
   Prof pr(s, c.st, PULSE_KCLASS_GN_BWD, 0.0, (3.0 + (add ? 1.0 : 0.0)) * s->esz() * s->d.n * hw * x.c());
   s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta,
                              (const float*)(c.stash + mr), (float*)(c.work + bst), add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
-                             cs0, cs1, c.st);
+                             cs0, cs1, c.st, !(s->d.flags & PULSE_FLAG_GN_TWO_PASS));
 }
 
 ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, int k, int stride, const void* w,

@@ -36,7 +36,7 @@ int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void*
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
                 const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
-                cudaStream_t st);
+                cudaStream_t st, bool allow_fused = true);
 
 // the same in one launch (norm_fused.cu; bf16, mean / rstd from the forward); 0 = shape not covered, nothing launched
 int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* gamma, const void* beta, const float* mr,

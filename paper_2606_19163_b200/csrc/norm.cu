@@ -569,10 +569,11 @@ int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void*
 template <typename T>
 static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
                     const float* mr, float* bst, const void* add, void* dst0, int dc0, int acc0,
-                    void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st) {
+                    void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st,
+                    bool allow_fused) {
   const int C = x.c();
   const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
-  if (dt == DT_BF16) {        // one pass with the tensors resident in shared memory where the shape allows (norm_fused.cu)
+  if (dt == DT_BF16 && allow_fused) {        // one pass with the tensors resident in shared memory where the shape allows (norm_fused.cu)
     const int r = gn_bwd_fused(g_a, x, n, hw, groups, gamma, beta, mr, add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
                                cs0, cs1, st);
     if (r > 0) return r;
@@ -592,11 +593,11 @@ static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
                 const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
-                cudaStream_t st) {
+                cudaStream_t st, bool allow_fused) {
   return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st)
+                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st, false)
                       : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st);
+                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st, allow_fused);
 }
 
 }  // namespace pulse

@@ -176,6 +176,14 @@ def test_mid_bf16_simt_crosscheck(kind):
     check(W.gpu_mid(kind), seed=2, flags=1, with_g_e_out=True)
 
 
+@pytest.mark.parametrize("kind", ["mini_updown", "mid_level", "mid_unet"])
+def test_bf16_gn_two_pass_crosscheck(kind):
+    """GroupNorm backward as reduction pass + apply pass (PULSE_FLAG_GN_TWO_PASS): the form that runs where a
+    slice of an image does not fit a cluster's shared memory; the default runs cover the one-pass cluster kernel."""
+    desc = W.mini("updown", "bf16") if kind == "mini_updown" else W.gpu_mid(kind[4:])
+    check(desc, seed=2, flags=2, with_g_e_out=(kind != "mid_unet"))
+
+
 # ------------------------------------------------------------------ full configs
 def test_config2_bf16():
     check(W.config(2), seed=0)
