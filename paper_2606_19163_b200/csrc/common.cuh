@@ -46,13 +46,11 @@ template <typename T> __device__ __forceinline__ T from_f(float v);
 template <> __device__ __forceinline__ float from_f<float>(float v) { return v; }
 template <> __device__ __forceinline__ bf16 from_f<bf16>(float v) { return __float2bfloat16_rn(v); }
 
-// load Vec<T>::N consecutive elements (16-byte aligned) into floats
-__device__ __forceinline__ void ldv(const float* p, float (&o)[4]) {
-  float4 v = *reinterpret_cast<const float4*>(p);
-  o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+// 16 raw bytes -> 4 floats (fp32 tensor) or 8 floats (bf16 tensor)
+__device__ __forceinline__ void unpack(const uint4& v, float (&o)[4]) {
+  o[0] = __uint_as_float(v.x); o[1] = __uint_as_float(v.y); o[2] = __uint_as_float(v.z); o[3] = __uint_as_float(v.w);
 }
-__device__ __forceinline__ void ldv(const bf16* p, float (&o)[8]) {
-  uint4 v = *reinterpret_cast<const uint4*>(p);
+__device__ __forceinline__ void unpack(const uint4& v, float (&o)[8]) {
   const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -60,6 +58,9 @@ __device__ __forceinline__ void ldv(const bf16* p, float (&o)[8]) {
     o[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
   }
 }
+// load Vec<T>::N consecutive elements (16-byte aligned) into floats
+__device__ __forceinline__ void ldv(const float* p, float (&o)[4]) { unpack(*reinterpret_cast<const uint4*>(p), o); }
+__device__ __forceinline__ void ldv(const bf16* p, float (&o)[8]) { unpack(*reinterpret_cast<const uint4*>(p), o); }
 __device__ __forceinline__ void stv(float* p, const float (&o)[4]) {
   *reinterpret_cast<float4*>(p) = make_float4(o[0], o[1], o[2], o[3]);
 }

@@ -86,6 +86,7 @@ void setup_side(pulse_stage* s, Ctx& c) {
   }
 }
 
+
 // profiling span around a group of launches of one kernel class
 struct Prof {
   pulse_stage* s; cudaStream_t st; int idx = -1; uint64_t l0;
@@ -361,9 +362,11 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   float* emb = (float*)(c.stash + s->emb_off);
   if (s->tensors[s->t_dout].ref.region == R_STASH && ((uintptr_t)d_d_out & 255) == 0) { c.ov_ft = s->t_dout; c.ov_fp = (char*)d_d_out; }
   if (s->cst_end > s->cst_begin) CK_CUDA(cudaMemsetAsync(c.stash + s->cst_begin, 0, s->cst_end - s->cst_begin, c.st));
-  CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
+  // a boundary tensor that a GroupNorm reads is stashed and measured in one pass (stash_in below); the rest are copies
+  const bool fuse_x = s->tensors[s->t_xin].gn_input, fuse_h = open && s->tensors[s->t_hin].gn_input;
+  if (!fuse_x) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
-  if (open) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
+  if (open && !fuse_h) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   setup_side(s, c);
   {   // beside the chain (side stream): p[n,c] = Wt SiLU(emb) + bt of every ResBlock in one launch (row a1), joined
       // before the first conv1; and, on the first forward of a step, the flipped / transposed weights the backward
@@ -381,8 +384,13 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
     if (c.side) c.ev_proj = c.mark_side();
     if (!s->wt_valid || s->last_was_backward) prepare_weights(c);
   }
-  run_stats(c, s->t_xin);
-  if (open) run_stats(c, s->t_hin);
+  auto stash_in = [&](int t, const void* src) {      // channel stats of `src` + its copy into the stage's tensor t
+    const Tensor& T = s->tensors[t];
+    Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 0.0);
+    s->launches += chan_stats(c.dt, src, s->d.n, T.ref.h * T.ref.w, T.ref.c, cst_of(c, t), c.st, c.fwd(t));
+  };
+  if (fuse_x) stash_in(s->t_xin, d_x_in);
+  if (fuse_h) stash_in(s->t_hin, d_h_in);
   for (size_t i = 0; i < s->ops.size(); ++i) {
     const OpPlan& op = s->ops[i];
     switch (op.kind) {

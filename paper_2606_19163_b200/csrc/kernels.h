@@ -25,7 +25,8 @@ struct Cat {
 // source site takes one cst per source.
 struct RowPlan { int tpr, rows, nchunks; };
 RowPlan row_plan(int dt, int hw, int c, int n, int max_threads);
-int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st);
+// copy (nullable): the same pass also copies x there (a tensor that enters the stage is stashed and measured at once)
+int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st, void* copy = nullptr);
 // mr_out: [n][2][groups] fp32, the group means and reciprocal standard deviations, kept for the backward
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
                 const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st);

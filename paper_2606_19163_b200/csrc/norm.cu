@@ -214,7 +214,8 @@ template <typename T> __device__ __forceinline__ void lds(const uint8_t* p, floa
 
 // ------------------------------------------------------------------------------ channel stats of one tensor
 template <typename T>
-__global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, int C, int hw, float* __restrict__ cst) {
+__global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, int C, int hw, float* __restrict__ cst,
+                                                        T* __restrict__ copy) {     // copy (nullable): also copy x there
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   Smem s(sm_, C, 0);
@@ -229,8 +230,12 @@ __global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, 
     float t[4][V];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      if (p + u * rows < pe) ldv(x + ((size_t)n * hw + p + u * rows) * C + ch, t[u]);
-      else {
+      if (p + u * rows < pe) {
+        const size_t off = ((size_t)n * hw + p + u * rows) * C + ch;
+        const uint4 raw = *reinterpret_cast<const uint4*>(x + off);       // 16 bytes = V elements
+        if (copy) *reinterpret_cast<uint4*>(copy + off) = raw;
+        unpack(raw, t[u]);
+      } else {
 #pragma unroll
         for (int i = 0; i < V; ++i) t[u][i] = 0.f;
       }
@@ -513,12 +518,12 @@ void mb_timeline_gn(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tlg, 
 #endif
 
 // ------------------------------------------------------------------------------ host launchers
-int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st) {
+int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st, void* copy) {
   const RowPlan pl = row_plan(dt, hw, c, n, 512);
   dim3 grid(pl.nchunks, n), block(pl.tpr, pl.rows);
   const size_t sm = smem_bytes(c, 0, pl.rows, 2);
-  if (dt == DT_F32) chan_stats_k<float><<<grid, block, sm, st>>>((const float*)x, c, hw, cst);
-  else chan_stats_k<bf16><<<grid, block, sm, st>>>((const bf16*)x, c, hw, cst);
+  if (dt == DT_F32) chan_stats_k<float><<<grid, block, sm, st>>>((const float*)x, c, hw, cst, (float*)copy);
+  else chan_stats_k<bf16><<<grid, block, sm, st>>>((const bf16*)x, c, hw, cst, (bf16*)copy);
   return 1;
 }
 
