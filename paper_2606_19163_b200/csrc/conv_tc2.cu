@@ -62,9 +62,10 @@ template <int UN, int NJ> struct Cfg2 {
   static constexpr int BN = UN * NJ;                       // output channels per pair tile
   static constexpr int B_SLICE = (UN / 2) * BK * 2;        // this CTA's half of one UN-wide weight slice
   static constexpr int STAGE_BYTES = A_BYTES + NJ * B_SLICE;
-  static constexpr int CW = BN % 64 == 0 ? 64 : 32;        // channels per epilogue chunk / TMA store box
+  static constexpr int CW = 32;                            // channels per epilogue chunk / TMA store box
   static constexpr int BOX_BYTES = 32 * CW * 2;            // one warp's [32 pixels][CW channels] bf16
-  static constexpr int EPI_BYTES = 4 * (2 * BOX_BYTES + 2048);   // per epilogue warp: 2 boxes + column vector [BN] fp32
+  static constexpr int NBUF = 2;                           // staging boxes per warp: chunk c is written while the TMA store of c - 1 reads
+  static constexpr int EPI_BYTES = 4 * (2 * NBUF * BOX_BYTES + 2048);   // per quadrant: 2 warps x NBUF boxes + column vector [BN] fp32
   static constexpr int RING = 227 * 1024 - 256 - EPI_BYTES - 1024;       // what is left of the 227 KB for the operand ring
   static constexpr int STAGES = RING / STAGE_BYTES > 8 ? 8 : RING / STAGE_BYTES;
   static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_BYTES + 1024;
@@ -190,13 +191,13 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
     // box origin of this warp inside the tile (lane 0's pixel)
     const int row0 = q * 32, n_w = row0 / (p.bh * p.bw), rem0 = row0 - n_w * (p.bh * p.bw);
     const int y_w = rem0 / p.bw, x_w = rem0 - y_w * p.bw;
-    uint8_t* stg_q = smem + C::STAGES * C::STAGE_BYTES + q * (2 * C::BOX_BYTES + 2048);
-    float* colv = reinterpret_cast<float*>(stg_q + 2 * C::BOX_BYTES);    // [BN] bias (+ temb projection of this image)
-    uint8_t* stg = stg_q + grp * C::BOX_BYTES;                           // this warp's staging box
+    uint8_t* stg_q = smem + C::STAGES * C::STAGE_BYTES + q * (2 * C::NBUF * C::BOX_BYTES + 2048);
+    float* colv = reinterpret_cast<float*>(stg_q + 2 * C::NBUF * C::BOX_BYTES);    // [BN] bias (+ temb projection of this image)
+    uint8_t* stg = stg_q + grp * C::NBUF * C::BOX_BYTES;                 // this warp's staging boxes
     const uint32_t stg_lane = smem_u32(stg) + lane * (CW * 2);
     const int sw = CW == 64 ? (lane & 7) : ((lane >> 1) & 3);            // 128-byte / 64-byte swizzle of 16-byte pieces
     int acc = 0; uint32_t acc_phase = 0;
-    constexpr int buf = 0;
+    int buf = 0;
     for (int tile = pair; tile < total_tiles; tile += npairs) {
       const int mp = tile / p.n_tiles, nt = tile - mp * p.n_tiles;
       const int mt = 2 * mp + (int)rank;
@@ -223,28 +224,36 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       tc_fence_after();
       if (warp == 2 && lane == 0) TL(4);
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * C::BN;
-#pragma unroll 1
-      for (int ch = grp; ch < C::BN / CW; ch += 2) {
-        uint32_t r[CW];
-        tmem_ld32(taddr + ch * CW, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
-        if (CW == 64) tmem_ld32(taddr + ch * CW + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[CW - 32]));
-        const int co = nt * C::BN + ch * CW;
-        float4 cvv[CW / 4];                          // column vector of the chunk: loaded while the TMEM load is in flight
+      // software pipeline: the TMEM load of this warp's next chunk is issued before the current chunk is converted
+      // and stored (tcgen05.wait::ld waits for every outstanding load, so the next one is issued right after it)
+      constexpr int NCH = C::BN / CW, NIT = (NCH + 1) / 2;
+      uint32_t rr[2][32];
+      tmem_ld32(taddr + grp * CW, rr[0]);
 #pragma unroll
-        for (int i = 0; i < CW / 4; ++i) cvv[i] = *reinterpret_cast<const float4*>(colv + ch * CW + i * 4);
+      for (int it = 0; it < NIT; ++it) {
+        const int ch = grp + 2 * it;
+        if (ch >= NCH) break;
+        uint32_t (&r)[32] = rr[it & 1];
+        const int co = nt * C::BN + ch * CW;
         tmem_ld_wait();
-        if (ch + 2 >= C::BN / CW) {                 // this warp's last TMEM read of the tile
+        if (ch + 2 < NCH) {
+          tmem_ld32(taddr + (ch + 2) * CW, rr[(it + 1) & 1]);
+        } else {                                    // that was this warp's last TMEM read of the tile
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&tempty_bar[acc]), 0));
+          if (lane == 0) mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty_bar[acc]), 0));
         }
         if (!(DBG(p) & 4)) {
-          if (lane == 0 && !(DBG(p) & 64)) bulk_wait_read<0>();        // this warp's previous store has read the box
+          if (lane == 0 && !(DBG(p) & 64)) bulk_wait_read<C::NBUF - 1>();   // the store that last used this box has read it
           __syncwarp();
           const uint32_t dst = stg_lane + buf * C::BOX_BYTES;
 #pragma unroll
           for (int i = 0; i < CW / 8; ++i) {
-            const float4 c0 = cvv[2 * i], c1 = cvv[2 * i + 1];
+            float4 c0 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8);
+            float4 c1 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8 + 4);
+#ifdef PULSE_MB
+            if (DBG(p) & 2048) { c0 = make_float4(0.f, 0.f, 0.f, 0.f); c1 = c0; }
+#endif
             float v[8] = {__uint_as_float(r[i * 8]) + c0.x,     __uint_as_float(r[i * 8 + 1]) + c0.y,
                           __uint_as_float(r[i * 8 + 2]) + c0.z, __uint_as_float(r[i * 8 + 3]) + c0.w,
                           __uint_as_float(r[i * 8 + 4]) + c1.x, __uint_as_float(r[i * 8 + 5]) + c1.y,
@@ -255,6 +264,15 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
 #pragma unroll
               for (int j = 0; j < 8; ++j) v[j] += a8[j];
             }
+#ifdef PULSE_MB
+            if (DBG(p) & 4096) { if (v[0] + v[3] + v[5] == 123.4f) st_shared_v4(dst, 1, 2, 3, 4); }
+            else if (DBG(p) & 512)
+              st_shared_v4(dst + ((i ^ sw) << 4), __byte_perm(__float_as_uint(v[0]), __float_as_uint(v[1]), 0x7632),
+                           __byte_perm(__float_as_uint(v[2]), __float_as_uint(v[3]), 0x7632),
+                           __byte_perm(__float_as_uint(v[4]), __float_as_uint(v[5]), 0x7632),
+                           __byte_perm(__float_as_uint(v[6]), __float_as_uint(v[7]), 0x7632));
+            else
+#endif
             st_shared_v4(dst + ((i ^ sw) << 4), pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
                          pack_bf16(v[6], v[7]));
           }
@@ -291,6 +309,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
             atomicAdd(dst + p.cout_total, q0); atomicAdd(dst + p.cout_total + 1, q1);
             } else if (s0 + s1 + q0 + q1 == 123.456f) dst[0] = s0;
           }
+          buf ^= 1;
         }
       }
       if (C::ACC == 2) { acc ^= 1; if (acc == 0) acc_phase ^= 1; }
@@ -408,7 +427,7 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
       const size_t C2 = (size_t)a.cout * 2;
       uint64_t dims[4] = {(uint64_t)a.cout, (uint64_t)gw, (uint64_t)gh, (uint64_t)a.n};
       uint64_t str[3] = {(uint64_t)p.osx * C2, (uint64_t)p.osy * a.wout * C2, (uint64_t)a.hout * a.wout * C2};
-      const uint32_t cw = (un * nj) % 64 == 0 ? 64 : 32;
+      const uint32_t cw = 32;        // Cfg2::CW
       uint32_t box[4] = {cw, (uint32_t)bwb, (uint32_t)bhb, 1};
       const char* base = (const char*)a.out + ((size_t)p.ooy * a.wout + p.oox) * C2;
       if (!get_map(base, 4, dims, str, box, &mo, 2 * (int)cw)) return false;
