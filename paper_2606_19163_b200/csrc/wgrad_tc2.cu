@@ -34,7 +34,7 @@ constexpr int BLK32 = PIX * 64;               // one [64 px][32 ch] box = 4 KB
 constexpr int N_TOT = 320;
 constexpr int STAGE = 2 * BLK + 2 * BLK + BLK32;      // 36 KB per CTA
 constexpr int STAGES = 5;
-constexpr int FLUSH_BYTES = 4 * 2 * 4096;             // per epilogue warp: 2 x [32 co][32 c] fp32 boxes
+constexpr int FLUSH_BYTES = 8 * 2 * 2048;             // per epilogue warp: 2 x [16 co][32 c] fp32 boxes
 constexpr int SMEM = STAGES * STAGE + FLUSH_BYTES + 1024;
 
 #ifdef PULSE_MB
@@ -58,7 +58,7 @@ struct Wg2Params {
   float* dw;
 };
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
 wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
             const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapG32,
             const __grid_constant__ CUtensorMap mapW, const Wg2Params p) {
@@ -84,7 +84,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapG); prefetch_tmap(&mapG32); prefetch_tmap(&mapW);
     for (int i = 0; i < STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
-    mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 8);
+    mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 16);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc2(&tmem_base_s, 512);
@@ -188,12 +188,14 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       }
     }
   } else {
-    // ===== epilogue (both CTAs): this CTA's 128 rows x 320 columns are ADDED into dW (fp32).  A warp owns 32
-    // consecutive channels c (its TMEM lanes); per 32 output channels it transposes its registers into a
-    // [32 co][32 c] fp32 box in shared memory (conflict-free: a row is one 128-byte line) and one TMA reduce-add
-    // instruction replaces 1024 scalar atomics.
-    const int q = warp & 3;
-    uint8_t* stg = smem + STAGES * STAGE + q * 8192;
+    // ===== epilogue (both CTAs, warps 2..9): this CTA's 128 rows x 320 columns are ADDED into dW (fp32).  A warp
+    // reads 32 consecutive channels c (the TMEM lane quadrant warp % 4); the two warps of a quadrant take alternate
+    // 16-column chunks.  Per chunk a warp transposes its registers into a [16 co][32 c] fp32 box in shared memory
+    // (conflict-free: a row is one 128-byte line) and one TMA reduce-add instruction replaces 512 scalar atomics;
+    // boxes are double-buffered per warp and the TMEM load of the next chunk is issued before the current one is
+    // stored.
+    const int q = warp & 3, grp = (warp - 2) >> 2;
+    uint8_t* stg = smem + STAGES * STAGE + q * 8192 + grp * 4096;
     const uint32_t stg_lane = smem_u32(stg) + lane * 4;
     uint32_t tphase = 0;
     int buf = 0;
@@ -211,26 +213,31 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       tc_fence_after();
       if (warp == 2 && lane == 0 && seg_end == we) TL(4);
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
-#pragma unroll 1
-      for (int ch = 0; ch < N_TOT / 32; ++ch) {
-        uint32_t r[32];
-        tmem_ld32(taddr + ch * 32, r);
+      constexpr int NIT = N_TOT / 32;          // 20 chunks of 16 columns, 10 per warp
+      uint32_t rr[2][16];
+      tmem_ld16(taddr + grp * 16, rr[0]);
+#pragma unroll
+      for (int it = 0; it < NIT; ++it) {
+        const int ch = grp + 2 * it;
+        uint32_t (&r)[16] = rr[it & 1];
         tmem_ld_wait();
-        if (ch == N_TOT / 32 - 1) {
+        if (it + 1 < NIT) {
+          tmem_ld16(taddr + (ch + 2) * 16, rr[(it + 1) & 1]);
+        } else {                                 // that was this warp's last TMEM read of the tile
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&tempty_bar), 0));
+          if (lane == 0) mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty_bar), 0));
         }
         if (valid && !(DBGW(p) & 4)) {
           if (lane == 0) bulk_wait_read<1>();
           __syncwarp();
-          const uint32_t dst = stg_lane + buf * 4096;
+          const uint32_t dst = stg_lane + buf * 2048;
 #pragma unroll
-          for (int i = 0; i < 32; ++i) asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i * 128), "r"(r[i]) : "memory");
+          for (int i = 0; i < 16; ++i) asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i * 128), "r"(r[i]) : "memory");
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            tma_reduce_add_2d(&mapW, stg + buf * 4096, kcol, nt * N_TOT + ch * 32);
+            tma_reduce_add_2d(&mapW, stg + buf * 2048, kcol, nt * N_TOT + ch * 16);
             bulk_commit();
           }
           buf ^= 1;
@@ -298,7 +305,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
   if (ok) ok = act_map(a.g, a.n, a.hout, a.wout, a.cout, p.bw, p.bh, p.bn, &mg);
   if (ok) ok = act_map_c(a.g, a.n, a.hout, a.wout, a.cout, 32, p.bw, p.bh, p.bn, &mg32);
-  if (ok) ok = mat_map_f32(a.dw, a.cout, p.ktot, 32, 32, &mw);
+  if (ok) ok = mat_map_f32(a.dw, a.cout, p.ktot, 32, 16, &mw);
   if (!ok) return -1;
   static bool attr_set = false;
   if (!attr_set) {
@@ -317,7 +324,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
     p.ppt = (int)(pairs / out_tiles);
     pairs = p.ppt * out_tiles;
   }
-  launch_pdl(wgrad_tc2_k, dim3((unsigned)(2 * pairs)), dim3(192), SMEM, st, m0, m1, mg, mg32, mw, p);
+  launch_pdl(wgrad_tc2_k, dim3((unsigned)(2 * pairs)), dim3(320), SMEM, st, m0, m1, mg, mg32, mw, p);
   return 1;
 }
 
