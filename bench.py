@@ -206,14 +206,12 @@ def main():
             return st.step(0, devs[0], 1.0, accumulate=False, loss=loss)
         fw = []
         for m, dev in enumerate(devs):                      # wave: F0..F{M-1}
-            emb, tst = st.temb_forward(dev["t"])
-            fw.append((emb, tst) + st.forward(m, dev["x_in"], dev.get("h_in"), emb))
+            fw.append(st.forward_temb(m, dev["x_in"], dev.get("h_in"), dev["t"]))
         for m in reversed(range(M)):                        # B{M-1}..B0
             emb, tst, e_out, d_out = fw[m]
             _, g_d = st.mse(d_out, devs[m]["target"], 1.0 / M, loss)
             g_temb = torch.zeros_like(emb)
-            st.backward(m, g_d, None, True, g_temb, accumulate=(m != M - 1))
-            st.temb_backward(g_temb, tst, accumulate=(m != M - 1))
+            st.backward_temb(m, g_d, None, g_temb, tst, True, accumulate=(m != M - 1))
         return None
 
     # eager warm-up (first launches set function attributes, build tensor maps)

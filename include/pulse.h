@@ -143,6 +143,19 @@ pulse_status_t pulse_stage_backward(pulse_stage_t* stage, pulse_skip_cache_t* ca
                                     const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
                                     void* d_g_h_in, float* d_g_temb, int accumulate_wgrad, void* stream);
 
+/* The same two calls with the timestep path inside (rows a1, a7), so that it runs beside the chain instead of
+ * before / after it: forward = pulse_temb_forward(d_t -> d_emb, d_temb_stash) + pulse_stage_forward(d_temb = d_emb);
+ * backward = pulse_stage_backward + pulse_temb_backward(d_g_temb, d_temb_stash).  Same results as the separate
+ * calls.  d_emb [n,temb_dim] fp32 and d_temb_stash (pulse_temb_stash_elems floats) are written by the forward and
+ * kept by the caller until the backward of the microbatch; d_g_temb must be zeroed by the caller (it is +=). */
+pulse_status_t pulse_stage_forward_temb(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id,
+                                        const void* d_x_in, const void* d_h_in, const int64_t* d_t, float* d_emb,
+                                        float* d_temb_stash, void* d_e_out, void* d_d_out, void* stream);
+pulse_status_t pulse_stage_backward_temb(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id,
+                                         const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
+                                         void* d_g_h_in, float* d_g_temb, const float* d_temb_stash,
+                                         int accumulate_wgrad, void* stream);
+
 /* ---- helpers on the path (row a1, a7) ----------------------------------------------- */
 /* emb0 = [cos(t f_i), sin(t f_i)], f_i = exp(-ln(1e4) i/half); MLP kind: emb = W2 SiLU(W1 emb0 + b1) + b2
  * using the bound temb.* parameters.  d_t: int64 [n].  d_emb: fp32 [n,temb_dim].

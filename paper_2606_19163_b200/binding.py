@@ -60,6 +60,8 @@ _SIG = {
     "pulse_skip_cache_destroy": [_vp],
     "pulse_stage_forward": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp],
     "pulse_stage_backward": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_int, _vp],
+    "pulse_stage_forward_temb": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
+    "pulse_stage_backward_temb": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int, _vp],
     "pulse_temb_stash_elems": [_vp, C.POINTER(_sz)],
     "pulse_temb_forward": [_vp, _vp, _vp, _vp, _vp],
     "pulse_temb_backward": [_vp, _vp, _vp, C.c_int, _vp],
@@ -239,6 +241,28 @@ class Stage:
                                      _ptr(g_h_in), _ptr(g_temb), int(accumulate), _stream()))
         return g_x_in, g_h_in
 
+    def forward_temb(self, mb_id: int, x_in, h_in, t):
+        """temb_forward + forward in one call: the timestep path runs beside the stash of the boundary tensors."""
+        sh = self._shapes()
+        n = _sz()
+        _ck(lib.pulse_temb_stash_elems(self.h, C.byref(n)))
+        emb = torch.empty((self.desc["n"], self.desc["temb"]["dim"]), dtype=torch.float32, device=self.device)
+        stash = torch.empty(max(1, n.value), dtype=torch.float32, device=self.device)
+        d_out = torch.empty(sh["d_out"], dtype=self.tdtype, device=self.device)
+        e_out = torch.empty(sh["e_out"], dtype=self.tdtype, device=self.device) if "e_out" in sh else None
+        _ck(lib.pulse_stage_forward_temb(self.h, self.cache, mb_id, _ptr(x_in), _ptr(h_in), _ptr(t), _ptr(emb),
+                                         _ptr(stash), _ptr(e_out), _ptr(d_out), _stream()))
+        return emb, stash, e_out, d_out
+
+    def backward_temb(self, mb_id: int, g_d_out, g_e_out, g_temb, tstash, want_g_x_in=True, accumulate=False):
+        """backward + temb_backward in one call: the timestep-MLP backward runs beside the last operator."""
+        sh = self._shapes()
+        g_x_in = torch.empty(sh["x_in"], dtype=self.tdtype, device=self.device) if want_g_x_in else None
+        g_h_in = torch.empty(sh["h_in"], dtype=self.tdtype, device=self.device) if "h_in" in sh else None
+        _ck(lib.pulse_stage_backward_temb(self.h, self.cache, mb_id, _ptr(g_d_out), _ptr(g_e_out), _ptr(g_x_in),
+                                          _ptr(g_h_in), _ptr(g_temb), _ptr(tstash), int(accumulate), _stream()))
+        return g_x_in, g_h_in
+
     def temb_forward(self, t):
         n = _sz()
         _ck(lib.pulse_temb_stash_elems(self.h, C.byref(n)))
@@ -295,13 +319,11 @@ class Stage:
     def step(self, mb_id, dev, loss_scale=1.0, accumulate=False, loss=None, g_temb=None):
         """temb -> forward -> MSE -> backward -> temb backward for device-resident inputs
         `dev` = {x_in, h_in?, t, target, g_e_out?}.  Returns (outputs dict)."""
-        emb, tstash = self.temb_forward(dev["t"])
-        e_out, d_out = self.forward(mb_id, dev["x_in"], dev.get("h_in"), emb)
+        emb, tstash, e_out, d_out = self.forward_temb(mb_id, dev["x_in"], dev.get("h_in"), dev["t"])
         loss, g_d = self.mse(d_out, dev["target"], loss_scale, loss)
         if g_temb is None:
             g_temb = torch.zeros_like(emb)
-        g_x_in, g_h_in = self.backward(mb_id, g_d, dev.get("g_e_out"), True, g_temb, accumulate)
-        self.temb_backward(g_temb, tstash, accumulate)
+        g_x_in, g_h_in = self.backward_temb(mb_id, g_d, dev.get("g_e_out"), g_temb, tstash, True, accumulate)
         return {"loss": loss, "e_out": e_out, "d_out": d_out, "g_x_in": g_x_in, "g_h_in": g_h_in, "g_emb": g_temb,
                 "emb": emb}
 

@@ -16,11 +16,16 @@ struct Ctx {
   char* work;     // per-stage workspace
   cudaStream_t st;
   cudaStream_t side = nullptr;   // non-null: kernels off the critical chain go here (weight gradients, shortcut convs ...)
+  cudaStream_t side2 = nullptr;  // non-null (with side): the tail of the backward runs here, beside both
   int ev_proj = -1;              // forward: side-stream event after the temb projections
   int n_ev = 0;                  // events of s->sync_events used by this call
   int rb_count = 0;              // ResBlocks processed so far in this backward (g_h1 double buffer / hazard events)
   int ev_rb[2] = {-1, -1};       // event recorded on the side stream after the wgrads of the last ResBlock of each parity
   int dt;
+  // backward: what the tail (bias / temb-projection gradients of every op, then optionally the timestep-MLP
+  // backward) needs; it is enqueued beside the chain as soon as the last g_p is complete (tail_work)
+  const float* emb = nullptr; float* g_temb = nullptr; const float* temb_stash = nullptr;
+  int acc_w = 0; bool last_op = false, tail_done = false;
   bool err = false;
   cudaEvent_t new_event() {
     if (n_ev == (int)s->sync_events.size()) {
@@ -82,6 +87,8 @@ void setup_side(pulse_stage* s, Ctx& c) {
   if (s->side_mode == 1 && !s->profiling) {
     if (!s->side && cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking) != cudaSuccess) { s->side = nullptr; return; }
     c.side = s->side;
+    if (!s->side2 && cudaStreamCreateWithFlags(&s->side2, cudaStreamNonBlocking) != cudaSuccess) s->side2 = nullptr;
+    c.side2 = s->side2;
     if (const char* m = getenv("PULSE_SIDE_MASK")) c.side_mask = atoi(m);
   }
 }
@@ -113,6 +120,7 @@ double conv_flops(const ConvArgs& a) {
   return 2.0 * mpix * a.cout * a.src.c() * a.ksize * a.ksize;     // the s2 dgrad phases execute exactly 9/4 taps per output
 }
 void run_stats(Ctx& c, int t);
+void tail_work(Ctx& c);
 // stats_t >= 0: the conv writes tensor stats_t, which a GroupNorm will read: its channel stats come from the conv
 // epilogue where the kernel supports it, else from a chan_stats pass
 void run_conv(Ctx& c, ConvArgs a, int stats_t = -1) {
@@ -286,6 +294,7 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
              (float*)(c.work + op.gp), nullptr);
   // conv1: wgrad (side stream), dgrad
   c.fork();
+  if (c.last_op && c.side2) tail_work(c);      // every g_p is complete: the tail runs beside conv1 / GN1 of this block
   WgradArgs w1{c.dt, Cat{c.fwd(op.a1), ctot, nullptr, 0}, n, op.hin, op.win, g_h1, op.hin, op.win, op.cout, 3, 1,
                c.pgrad(op.p[P_C1W])};
   run_wgrad(c, w1);
@@ -307,7 +316,7 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
 }
 
 // bias / temb-projection gradients of every op from the pixel sums, in one batched launch (row a8-a10)
-void small_grads(Ctx& c, const float* emb, float* g_temb) {
+void small_grads(Ctx& c, const float* emb, float* g_temb, cudaStream_t st) {
   pulse_stage* s = c.s;
   std::vector<SmallGradEntry> e;
   for (const OpPlan& op : s->ops) {
@@ -325,8 +334,23 @@ void small_grads(Ctx& c, const float* emb, float* g_temb) {
     }
     e.push_back(g);
   }
-  Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
-  s->launches += small_grads_batch(c.dt, emb, g_temb, s->d.n, s->d.temb_dim, e.data(), (int)e.size(), c.st);
+  Prof pr(s, st, PULSE_KCLASS_OTHER, 0.0, 0.0);
+  s->launches += small_grads_batch(c.dt, emb, g_temb, s->d.n, s->d.temb_dim, e.data(), (int)e.size(), st);
+}
+pulse_status_t temb_backward_impl(pulse_stage* s, const float* d_g_emb, const float* d_stash, int accumulate_wgrad,
+                                  cudaStream_t st);
+// bias / temb-projection gradients of every op, then (pulse_stage_backward_temb) the timestep-MLP backward; on the
+// side stream when there is one (the caller has forked it), so that none of it is left for the end of the step
+void tail_work(Ctx& c) {
+  cudaStream_t st = c.side2 ? c.side2 : (c.side ? c.side : c.st);
+  if (c.side2) {                                   // side2 continues after everything enqueued on the main stream so far
+    cudaEvent_t e = c.new_event();
+    cudaEventRecord(e, c.st);
+    cudaStreamWaitEvent(c.side2, e, 0);
+  }
+  small_grads(c, c.emb, c.g_temb, st);
+  if (c.temb_stash && temb_backward_impl(c.s, c.g_temb, c.temb_stash, c.acc_w, st) != PULSE_OK) c.err = true;
+  c.tail_done = true;
 }
 
 pulse_status_t check_bound(pulse_stage* s, pulse_skip_cache* cache) {
@@ -339,9 +363,14 @@ pulse_status_t check_bound(pulse_stage* s, pulse_skip_cache* cache) {
 
 }  // namespace
 
-extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
-                                              const void* d_x_in, const void* d_h_in, const float* d_temb,
-                                              void* d_e_out, void* d_d_out, void* stream) {
+namespace {
+pulse_status_t temb_forward_impl(pulse_stage* s, const int64_t* d_t, float* d_emb, float* d_stash, cudaStream_t st);
+}
+// d_t != nullptr (pulse_stage_forward_temb): the embedding is computed here, beside the stash of the boundary tensors,
+// from the timesteps into d_temb (written) with its MLP stash in d_temb_stash
+static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_x_in,
+                                   const void* d_h_in, float* d_temb, const int64_t* d_t, float* d_temb_stash,
+                                   void* d_e_out, void* d_d_out, void* stream) {
   pulse_status_t stt = check_bound(s, cache);
   if (stt) return stt;
   const bool open = s->d.link == PULSE_LINK_OPEN;
@@ -365,7 +394,7 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   // a boundary tensor that a GroupNorm reads is stashed and measured in one pass (stash_in below); the rest are copies
   const bool fuse_x = s->tensors[s->t_xin].gn_input, fuse_h = open && s->tensors[s->t_hin].gn_input;
   if (!fuse_x) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
-  CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
+  if (!d_t) CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
   if (open && !fuse_h) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   setup_side(s, c);
   {   // beside the chain (side stream): p[n,c] = Wt SiLU(emb) + bt of every ResBlock in one launch (row a1), joined
@@ -373,6 +402,10 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
       // needs (parameters may have changed since the last backward; R21), joined at the end of this call
     c.fork();
     OnSide g(c);
+    if (d_t) {
+      if (temb_forward_impl(s, d_t, d_temb, d_temb_stash, c.st) != PULSE_OK) c.err = true;
+      CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
+    }
     std::vector<ProjEntry> pe;
     for (const OpPlan& op : s->ops)
       if (op.kind == PULSE_OP_RESBLOCK)
@@ -429,10 +462,22 @@ extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache
   if (lb > cache->peak_bytes) cache->peak_bytes = lb;
   return PULSE_OK;
 }
+extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
+                                              const void* d_x_in, const void* d_h_in, const float* d_temb,
+                                              void* d_e_out, void* d_d_out, void* stream) {
+  return forward_impl(s, cache, mb, d_x_in, d_h_in, const_cast<float*>(d_temb), nullptr, nullptr, d_e_out, d_d_out, stream);
+}
+extern "C" pulse_status_t pulse_stage_forward_temb(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
+                                                   const void* d_x_in, const void* d_h_in, const int64_t* d_t,
+                                                   float* d_emb, float* d_temb_stash, void* d_e_out, void* d_d_out,
+                                                   void* stream) {
+  if (!d_t || !d_emb || !d_temb_stash) return fail(PULSE_ERR_INVALID_ARG, "null t / emb / temb stash");
+  return forward_impl(s, cache, mb, d_x_in, d_h_in, d_emb, d_t, d_temb_stash, d_e_out, d_d_out, stream);
+}
 
-extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
-                                               const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
-                                               void* d_g_h_in, float* d_g_temb, int accumulate_wgrad, void* stream) {
+static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_g_d_out,
+                                    const void* d_g_e_out, void* d_g_x_in, void* d_g_h_in, float* d_g_temb,
+                                    const float* d_temb_stash, int accumulate_wgrad, void* stream) {
   pulse_status_t stt = check_bound(s, cache);
   if (stt) return stt;
   const bool open = s->d.link == PULSE_LINK_OPEN;
@@ -447,7 +492,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   c.skip = cache->base + (size_t)slot * cache->bytes_per_slot;
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
-  const float* emb = (const float*)(c.stash + s->emb_off);
+  c.emb = (const float*)(c.stash + s->emb_off); c.g_temb = d_g_temb; c.temb_stash = d_temb_stash; c.acc_w = accumulate_wgrad;
   setup_side(s, c);
   if (!accumulate_wgrad)
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
@@ -465,6 +510,7 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   for (int i = (int)s->ops.size() - 1; i >= 0; --i) {
     const OpPlan& op = s->ops[i];
     const int n = s->d.n;
+    c.last_op = i == 0;
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_backward(c, op); break;
       case PULSE_OP_CONV_IN:
@@ -510,7 +556,15 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
       }
     }
   }
-  small_grads(c, emb, d_g_temb);
+  if (!c.tail_done) {
+    if (!c.side2) c.fork();
+    tail_work(c);
+  }
+  if (c.side2) {                               // join the tail
+    cudaEvent_t e = c.new_event();
+    cudaEventRecord(e, c.side2);
+    cudaStreamWaitEvent(c.st, e, 0);
+  }
   if (c.side) c.wait_side(c.mark_side());      // join: the caller's stream sees every weight gradient complete
   if (open && c.ov_gt[1] < 0) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   if (d_g_x_in && c.ov_gt[2] < 0) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
@@ -520,6 +574,18 @@ extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cach
   cache->live--;
   s->last_was_backward = true;
   return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_stage_backward(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
+                                               const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
+                                               void* d_g_h_in, float* d_g_temb, int accumulate_wgrad, void* stream) {
+  return backward_impl(s, cache, mb, d_g_d_out, d_g_e_out, d_g_x_in, d_g_h_in, d_g_temb, nullptr, accumulate_wgrad, stream);
+}
+extern "C" pulse_status_t pulse_stage_backward_temb(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
+                                                    const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
+                                                    void* d_g_h_in, float* d_g_temb, const float* d_temb_stash,
+                                                    int accumulate_wgrad, void* stream) {
+  if (!d_g_temb || !d_temb_stash) return fail(PULSE_ERR_INVALID_ARG, "null g_temb / temb stash");
+  return backward_impl(s, cache, mb, d_g_d_out, d_g_e_out, d_g_x_in, d_g_h_in, d_g_temb, d_temb_stash, accumulate_wgrad, stream);
 }
 
 // ------------------------------------------------------------------------------ temb, loss
@@ -531,7 +597,10 @@ extern "C" pulse_status_t pulse_temb_stash_elems(const pulse_stage_t* s, size_t*
 extern "C" pulse_status_t pulse_temb_forward(pulse_stage_t* s, const int64_t* d_t, float* d_emb, float* d_stash,
                                              void* stream) {
   if (!s || !d_t || !d_emb || !d_stash) return fail(PULSE_ERR_INVALID_ARG, "null argument");
-  cudaStream_t st = (cudaStream_t)stream;
+  return temb_forward_impl(s, d_t, d_emb, d_stash, (cudaStream_t)stream);
+}
+namespace {
+pulse_status_t temb_forward_impl(pulse_stage* s, const int64_t* d_t, float* d_emb, float* d_stash, cudaStream_t st) {
   const int n = s->d.n, d0 = s->d.temb_d0, T = s->d.temb_dim;
   const int dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
   if (s->d.temb_kind == PULSE_TEMB_SINUSOIDAL) {
@@ -547,12 +616,17 @@ extern "C" pulse_status_t pulse_temb_forward(pulse_stage_t* s, const int64_t* d_
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }
+}  // namespace
 extern "C" pulse_status_t pulse_temb_backward(pulse_stage_t* s, const float* d_g_emb, const float* d_stash,
                                               int accumulate_wgrad, void* stream) {
   if (!s || !d_g_emb || !d_stash) return fail(PULSE_ERR_INVALID_ARG, "null argument");
+  return temb_backward_impl(s, d_g_emb, d_stash, accumulate_wgrad, (cudaStream_t)stream);
+}
+namespace {
+pulse_status_t temb_backward_impl(pulse_stage* s, const float* d_g_emb, const float* d_stash, int accumulate_wgrad,
+                                  cudaStream_t st) {
   if (s->d.temb_kind == PULSE_TEMB_SINUSOIDAL) return PULSE_OK;
   if (!s->d_params || !s->d_grads || !s->d_work) return fail(PULSE_ERR_STATE, "parameters / workspace not bound");
-  cudaStream_t st = (cudaStream_t)stream;
   const int n = s->d.n, d0 = s->d.temb_d0, T = s->d.temb_dim;
   const int dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
   if (!accumulate_wgrad) CK_CUDA(cudaMemsetAsync(s->d_grads, 0, s->temb_grad_bytes, st));
@@ -567,6 +641,7 @@ extern "C" pulse_status_t pulse_temb_backward(pulse_stage_t* s, const float* d_g
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }
+}  // namespace
 extern "C" pulse_status_t pulse_mse_fwd_bwd(int dtype, const void* d_d, const void* d_target, size_t numel, float scale,
                                             float* d_loss, void* d_g_d, void* stream) {
   if (!d_d || !d_target || !d_loss || !d_g_d) return fail(PULSE_ERR_INVALID_ARG, "null argument");

@@ -278,6 +278,7 @@ extern "C" pulse_status_t pulse_stage_destroy(pulse_stage_t* s) {
     for (auto ev : s->event_pool) cudaEventDestroy(ev);
     for (auto ev : s->sync_events) cudaEventDestroy(ev);
     if (s->side) cudaStreamDestroy(s->side);
+    if (s->side2) cudaStreamDestroy(s->side2);
   }
   delete s;
   return PULSE_OK;

@@ -84,6 +84,7 @@ struct pulse_stage {
   // weight-gradient kernels run on a side stream, concurrently with the dgrad / GroupNorm chain of the backward
   // (fork / join with events; legal inside CUDA-graph capture).  PULSE_NO_SIDE_STREAM=1 disables it.
   cudaStream_t side = nullptr;
+  cudaStream_t side2 = nullptr;             // the tail of the backward (bias / temb gradients, timestep-MLP backward)
   std::vector<cudaEvent_t> sync_events;
   int side_mode = -1;                       // -1 unknown, 0 off, 1 on
   bool last_was_backward = true;            // a forward that follows a backward starts a new step: weights may have changed
