@@ -246,6 +246,41 @@ def test_config5_wave_reduced():
         assert rel_err(g8[k], g1[k]) < 6e-2 and rms_err(g8[k], g1[k]) < 1e-2, k
 
 
+# ------------------------------------------------------------------ the one-call forms of the timestep path
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+def test_temb_fused_calls_match_separate_calls(dtype):
+    """pulse_stage_forward_temb / pulse_stage_backward_temb == pulse_temb_forward + pulse_stage_forward and
+    pulse_stage_backward + pulse_temb_backward (same kernels, the timestep path merely runs beside the chain)."""
+    B = _binding()
+    desc = W.mini("level", dtype)
+    data = W.draw(desc, 3)
+    res = []
+    for fused in (False, True):
+        st = B.Stage(desc)
+        st.load_params(data["params"])
+        dev = st.to_device(data["microbatches"][0])
+        if fused:
+            emb, tst, e_out, d_out = st.forward_temb(0, dev["x_in"], dev.get("h_in"), dev["t"])
+        else:
+            emb, tst = st.temb_forward(dev["t"])
+            e_out, d_out = st.forward(0, dev["x_in"], dev.get("h_in"), emb)
+        _, g_d = st.mse(d_out, dev["target"], 1.0)
+        g_temb = torch.zeros_like(emb)
+        if fused:
+            g_x, g_h = st.backward_temb(0, g_d, None, g_temb, tst, True, False)
+        else:
+            g_x, g_h = st.backward(0, g_d, None, True, g_temb, False)
+            st.temb_backward(g_temb, tst, False)
+        torch.cuda.synchronize()
+        res.append((emb.cpu(), d_out.float().cpu(), g_x.float().cpu(), g_temb.cpu(), st.grads()))
+    a, b = res
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])          # forward: same kernels, same order of sums
+    tol = 1e-5 if dtype == "fp32" else 3e-2                              # backward: atomics re-roll the last bits
+    assert rel_err(b[2], a[2]) < tol and rel_err(b[3], a[3]) < tol
+    for k in a[4]:
+        assert rel_err(b[4][k], a[4][k]) < tol, k
+
+
 # ------------------------------------------------------------------ cache / error behaviour (paper-faithful cases)
 def test_cache_errors_and_skip_locality():
     B = _binding()
