@@ -421,7 +421,9 @@ def main():
                 "frac_in_graph": (dom.get("in_graph_tflops") or 0.0) / tf_peak,
                 "bound": "tensor", "achieved": dom.get("tflops"), "peak": tf_peak, "unit": "TFLOP/s",
                 "frac": (dom.get("tflops") or 0.0) / tf_peak, "traffic": traffic, "peak_source": peak_src,
-                "share_of_step": (dom.get("ms_per_step") or 0.0) / eager_ms}
+                # share of the step's kernel time (same event brackets, all classes): comparable with the share in the
+                # ncu launch list under profiles/
+                "share_of_step": (dom.get("ms_per_step") or 0.0) / max(1e-9, sum(r["ms_per_step"] for r in kern.values()))}
     line = {"metric": METRIC, "value": value, "unit": "samples/s", "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16" if desc["dtype"] == "bf16" else "f32", "data": "synthetic (seeded N(0,1), DESIGN.md)",
