@@ -249,11 +249,8 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           const uint32_t dst = stg_lane + buf * C::BOX_BYTES;
 #pragma unroll
           for (int i = 0; i < CW / 8; ++i) {
-            float4 c0 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8);
-            float4 c1 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8 + 4);
-#ifdef PULSE_MB
-            if (DBG(p) & 2048) { c0 = make_float4(0.f, 0.f, 0.f, 0.f); c1 = c0; }
-#endif
+            const float4 c0 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8);
+            const float4 c1 = *reinterpret_cast<const float4*>(colv + ch * CW + i * 8 + 4);
             float v[8] = {__uint_as_float(r[i * 8]) + c0.x,     __uint_as_float(r[i * 8 + 1]) + c0.y,
                           __uint_as_float(r[i * 8 + 2]) + c0.z, __uint_as_float(r[i * 8 + 3]) + c0.w,
                           __uint_as_float(r[i * 8 + 4]) + c1.x, __uint_as_float(r[i * 8 + 5]) + c1.y,
@@ -264,15 +261,6 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
 #pragma unroll
               for (int j = 0; j < 8; ++j) v[j] += a8[j];
             }
-#ifdef PULSE_MB
-            if (DBG(p) & 4096) { if (v[0] + v[3] + v[5] == 123.4f) st_shared_v4(dst, 1, 2, 3, 4); }
-            else if (DBG(p) & 512)
-              st_shared_v4(dst + ((i ^ sw) << 4), __byte_perm(__float_as_uint(v[0]), __float_as_uint(v[1]), 0x7632),
-                           __byte_perm(__float_as_uint(v[2]), __float_as_uint(v[3]), 0x7632),
-                           __byte_perm(__float_as_uint(v[4]), __float_as_uint(v[5]), 0x7632),
-                           __byte_perm(__float_as_uint(v[6]), __float_as_uint(v[7]), 0x7632));
-            else
-#endif
             st_shared_v4(dst + ((i ^ sw) << 4), pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
                          pack_bf16(v[6], v[7]));
           }
@@ -315,7 +303,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       if (C::ACC == 2) { acc ^= 1; if (acc == 0) acc_phase ^= 1; }
       else acc_phase ^= 1;
     }
-    if (lane == 0) bulk_wait<0>();
+    if (lane == 0) bulk_wait_read<0>();       // the staging boxes have been read; the global writes complete before the grid does
   }
   if (warp == 2 && lane == 0) TL(5);
   tc_fence_before();

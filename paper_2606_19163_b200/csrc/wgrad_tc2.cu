@@ -245,7 +245,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       }
       w = seg_end;
     }
-    if (lane == 0) bulk_wait<0>();
+    if (lane == 0) bulk_wait_read<0>();       // the staging boxes have been read; the reductions complete before the grid does
   }
   if (warp == 2 && lane == 0) TL(5);
   tc_fence_before();
