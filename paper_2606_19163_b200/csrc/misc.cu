@@ -90,60 +90,105 @@ struct ProjBatch { int count; ProjEntry e[BATCH]; };
 struct SmallGradBatch { int count; SmallGradEntry e[BATCH]; };
 struct TransposeBatch { int count; TransposeEntry e[BATCH]; };
 
-// p[n][o] = sum_j W[o][j] silu(emb[n][j]) + b[o] for every ResBlock of the stage in one launch.
-// Block: 8 warps x 4 outputs; silu(emb) is staged once per block in shared memory ([n <= 8][T] floats).
+// out[n][o] = sum_j W[o][j] f(in[n][j]) + b[o], f = SiLU or identity, for up to 16 weight matrices in one launch
+// (the temb projections of every ResBlock; the two linears of the timestep MLP, row a1).
+// Latency-bound GEMVs (n <= 8 rows): a warp owns one output row and requests its first 5 weight vectors (16 bytes
+// each) BEFORE the block stages f(in) in shared memory ([n <= 8][din] floats), so that the two global round trips
+// overlap; then FMAs against shared memory, a warp reduction per row of in, one store.
+constexpr int RD_PRE = 5;         // weight vectors per lane in flight (din <= 1280 for bf16: the whole row)
 template <typename T>
-__global__ void __launch_bounds__(256) temb_proj_k(const float* __restrict__ emb, int n0, int nn, int Tdim,
-                                                   const __grid_constant__ ProjBatch b) {
+__global__ void __launch_bounds__(256) rowdot_k(const float* __restrict__ in, int n0, int nn, int din, int silu_in,
+                                                const __grid_constant__ ProjBatch b) {
   constexpr int V = Vec<T>::N;
-  extern __shared__ float se[];        // [nn][Tdim]
+  extern __shared__ float se[];        // [nn][din]
   const ProjEntry& e = b.e[blockIdx.y];
   const int o0 = blockIdx.x * 8;
   if (o0 >= e.cout) return;
-  for (int i = threadIdx.x; i < nn * Tdim; i += blockDim.x) se[i] = siluf_(emb[(size_t)n0 * Tdim + i]);
-  __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int o = o0 + warp;
-  if (o >= e.cout) return;
-  const T* w = (const T*)e.w + (size_t)o * Tdim;
-  float acc[8];
+  const bool vec_ok = din % V == 0;
+  const T* w = (const T*)e.w + (size_t)(o < e.cout ? o : o0) * din;
+  const int nvec = din / V;            // vectors per row (vec_ok)
+  uint4 pre[RD_PRE];
+  if (vec_ok) {
 #pragma unroll
-  for (int j = 0; j < 8; ++j) acc[j] = 0.f;
-  if (Tdim % (32 * V) == 0) {
-    for (int i0 = 0; i0 < Tdim; i0 += 4 * 32 * V) {     // up to 4 vector loads per lane in flight
-      float wv[4][V];
+    for (int u = 0; u < RD_PRE; ++u) {
+      const int v = lane + 32 * u;
+      pre[u] = v < nvec ? *reinterpret_cast<const uint4*>(w + (size_t)v * V) : make_uint4(0u, 0u, 0u, 0u);
+    }
+  }
+  if (din % 4 == 0) {                  // stage f(in): float4 loads, all of a thread's requests before the first use
+    const int n4 = nn * din / 4;
+    const float4* src = reinterpret_cast<const float4*>(in + (size_t)n0 * din);
+    for (int i0 = threadIdx.x; i0 < n4; i0 += 4 * 256) {
+      float4 t[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (i0 + u * 256 < n4) t[u] = src[i0 + u * 256];
 #pragma unroll
       for (int u = 0; u < 4; ++u)
-        if (i0 + u * 32 * V < Tdim) ldv(w + i0 + u * 32 * V + lane * V, wv[u]);
-#pragma unroll
-      for (int u = 0; u < 4; ++u)
-        if (i0 + u * 32 * V < Tdim) {
-          const int i = i0 + u * 32 * V + lane * V;
-#pragma unroll
-          for (int j = 0; j < 8; ++j)
-            if (j < nn)
-#pragma unroll
-              for (int k = 0; k < V; ++k) acc[j] = fmaf(wv[u][k], se[j * Tdim + i + k], acc[j]);
+        if (i0 + u * 256 < n4) {
+          if (silu_in) { t[u].x = siluf_(t[u].x); t[u].y = siluf_(t[u].y); t[u].z = siluf_(t[u].z); t[u].w = siluf_(t[u].w); }
+          reinterpret_cast<float4*>(se)[i0 + u * 256] = t[u];
         }
     }
   } else {
-    for (int i = lane; i < Tdim; i += 32) {
+    for (int i = threadIdx.x; i < nn * din; i += 256) {
+      const float t = in[(size_t)n0 * din + i];
+      se[i] = silu_in ? siluf_(t) : t;
+    }
+  }
+  __syncthreads();
+  if (o >= e.cout) return;
+  float acc[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+  if (vec_ok) {
+    for (int v0 = 0; v0 < nvec; v0 += 32 * RD_PRE) {
+      if (v0) {                          // rows longer than 32 * RD_PRE vectors: next batch
+#pragma unroll
+        for (int u = 0; u < RD_PRE; ++u) {
+          const int v = v0 + lane + 32 * u;
+          pre[u] = v < nvec ? *reinterpret_cast<const uint4*>(w + (size_t)v * V) : make_uint4(0u, 0u, 0u, 0u);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < RD_PRE; ++u) {
+        const int v = v0 + lane + 32 * u;
+        if (v < nvec) {
+          float wv[V];
+          unpack(pre[u], wv);
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            if (j < nn) {
+              const float* x = se + j * din + v * V;
+#pragma unroll
+              for (int k = 0; k < V; k += 4) {
+                const float4 xv = *reinterpret_cast<const float4*>(x + k);
+                acc[j] = fmaf(wv[k], xv.x, acc[j]); acc[j] = fmaf(wv[k + 1], xv.y, acc[j]);
+                acc[j] = fmaf(wv[k + 2], xv.z, acc[j]); acc[j] = fmaf(wv[k + 3], xv.w, acc[j]);
+              }
+            }
+        }
+      }
+    }
+  } else {
+    for (int i = lane; i < din; i += 32) {
       const float wv = to_f(w[i]);
 #pragma unroll
       for (int j = 0; j < 8; ++j)
-        if (j < nn) acc[j] = fmaf(wv, se[j * Tdim + i], acc[j]);
+        if (j < nn) acc[j] = fmaf(wv, se[j * din + i], acc[j]);
     }
   }
-  const T* bias = (const T*)e.b;
+  const float bo = e.b ? to_f(((const T*)e.b)[o]) : 0.f;
 #pragma unroll
   for (int j = 0; j < 8; ++j)
     if (j < nn) {
       const float t = warp_sum(acc[j]);
-      if (lane == 0) e.out[(size_t)(n0 + j) * e.cout + o] = t + to_f(bias[o]);
+      if (lane == 0) e.out[(size_t)(n0 + j) * e.cout + o] = t + bo;
     }
 }
 
-int temb_proj_batch(int dt, const float* emb, int n, int T, const ProjEntry* e, int count, cudaStream_t st) {
+static int rowdot_batch(int dt, const float* in, int n, int din, int silu_in, const ProjEntry* e, int count, cudaStream_t st) {
   int launches = 0;
   for (int i0 = 0; i0 < count; i0 += BATCH) {
     ProjBatch b;
@@ -153,13 +198,16 @@ int temb_proj_batch(int dt, const float* emb, int n, int T, const ProjEntry* e, 
     for (int n0 = 0; n0 < n; n0 += 8) {
       const int nn = n - n0 < 8 ? n - n0 : 8;
       dim3 grid((maxc + 7) / 8, b.count);
-      const size_t smem = (size_t)nn * T * sizeof(float);
-      if (dt == DT_F32) temb_proj_k<float><<<grid, 256, smem, st>>>(emb, n0, nn, T, b);
-      else temb_proj_k<bf16><<<grid, 256, smem, st>>>(emb, n0, nn, T, b);
+      const size_t smem = (size_t)nn * din * sizeof(float);
+      if (dt == DT_F32) rowdot_k<float><<<grid, 256, smem, st>>>(in, n0, nn, din, silu_in, b);
+      else rowdot_k<bf16><<<grid, 256, smem, st>>>(in, n0, nn, din, silu_in, b);
       ++launches;
     }
   }
   return launches;
+}
+int temb_proj_batch(int dt, const float* emb, int n, int T, const ProjEntry* e, int count, cudaStream_t st) {
+  return rowdot_batch(dt, emb, n, T, 1, e, count, st);
 }
 
 // Per op (blockIdx.z), channel chunk of 32 (blockIdx.y), 256 columns j of the temb dimension (blockIdx.x):
@@ -242,67 +290,10 @@ int small_grads_batch(int dt, const float* emb, float* g_emb, int n, int T, cons
 }
 
 // ------------------------------------------------------------------ tiny linears (timestep path)
-// one warp per output feature o; each lane takes 8 consecutive inputs per step; all n (<= 8) rows at once
-template <typename T, int MAXN>
-__global__ void linear_fwd_k(const float* __restrict__ in, int n, int din, int dout, const T* __restrict__ w,
-                             const T* __restrict__ b, int silu_in, float* __restrict__ out) {
-  const int o = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (o >= dout) return;
-  float acc[MAXN];
-#pragma unroll
-  for (int j = 0; j < MAXN; ++j) acc[j] = 0.f;
-  const T* wr = w + (size_t)o * din;
-  if (din % 8 == 0) {
-    for (int i = lane * 8; i < din; i += 256) {
-      float wv[8];
-#pragma unroll
-      for (int k = 0; k < 8; ++k) wv[k] = to_f(wr[i + k]);
-#pragma unroll
-      for (int j = 0; j < MAXN; ++j)
-        if (j < n) {
-          const float4 x0 = *reinterpret_cast<const float4*>(in + (size_t)j * din + i);
-          const float4 x1 = *reinterpret_cast<const float4*>(in + (size_t)j * din + i + 4);
-          float x[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-#pragma unroll
-          for (int k = 0; k < 8; ++k) acc[j] = fmaf(wv[k], silu_in ? siluf_(x[k]) : x[k], acc[j]);
-        }
-    }
-  } else {
-    for (int i = lane; i < din; i += 32) {
-      const float wv = to_f(wr[i]);
-#pragma unroll
-      for (int j = 0; j < MAXN; ++j)
-        if (j < n) {
-          float x = in[(size_t)j * din + i];
-          if (silu_in) x = siluf_(x);
-          acc[j] = fmaf(wv, x, acc[j]);
-        }
-    }
-  }
-#pragma unroll
-  for (int j = 0; j < MAXN; ++j) {
-    if (j < n) {
-      const float s = warp_sum(acc[j]);
-      if (lane == 0) out[(size_t)j * dout + o] = s + (b ? to_f(b[o]) : 0.f);
-    }
-  }
-}
-
 int linear_fwd(int dt, const float* in, int n, int din, int dout, const void* w, const void* b, int silu_in,
                float* out, cudaStream_t st) {
-  int launches = 0;
-  for (int n0 = 0; n0 < n; n0 += 8) {       // N <= 8 in every config; larger N handled in slabs
-    const int nn = n - n0 < 8 ? n - n0 : 8;
-    const int blocks = (dout * 32 + 127) / 128;
-    if (dt == DT_F32)
-      linear_fwd_k<float, 8><<<blocks, 128, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const float*)w,
-                                                      (const float*)b, silu_in, out + (size_t)n0 * dout);
-    else
-      linear_fwd_k<bf16, 8><<<blocks, 128, 0, st>>>(in + (size_t)n0 * din, nn, din, dout, (const bf16*)w,
-                                                     (const bf16*)b, silu_in, out + (size_t)n0 * dout);
-    ++launches;
-  }
-  return launches;
+  const ProjEntry e{w, b, out, dout};
+  return rowdot_batch(dt, in, n, din, silu_in, &e, 1, st);
 }
 
 // dW[o][i] += sum_n g[n][o] f(in[n][i]); db[o] += sum_n g[n][o]
