@@ -42,7 +42,7 @@ __device__ __forceinline__ unsigned long long gtimef_() { unsigned long long t; 
 #endif
 
 struct GnfParams {
-  int c0, c1, hw, G, Cs, CL, ppc, BR, nbox, nrow;
+  int c0, c1, hw, G, Cs, CL, ppc, BR, nbox, nrow, br_shift;   // BR = 1 << br_shift
   const bf16* gamma; const bf16* beta; const float* mr;
   float* dgamma; float* dbeta;
   const bf16* add; bf16* dst0; bf16* dst1; int dc0, acc0, acc1;
@@ -149,10 +149,11 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
   for (int i = 0; i < 8; ++i) S[0][i] = S[1][i] = 0.f;
   if (active) {
     int waited = 0;
-    for (int pl = row; pl < p.ppc; pl += nrow) {
-      const int b = pl / p.BR;
+    int off = row * rb + vec * 16;
+    const int step = nrow * rb;
+    for (int pl = row; pl < p.ppc; pl += nrow, off += step) {
+      const int b = pl >> p.br_shift;
       while (waited <= b) { mbar_wait(&fullx[waited], 0); mbar_wait(&fullg[waited], 0); ++waited; }
-      const int off = pl * rb + vec * 16;
       float x[8], g[8];
       lds8(xs + off, x); lds8(gs + off, g);
 #pragma unroll
@@ -222,8 +223,11 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
   const int acc = first ? p.acc0 : p.acc1;
   if (active) {
     int it = 0;
-    for (int pl = row; pl < p.ppc; pl += nrow, ++it) {
-      const int off = pl * rb + vec * 16;
+    int off = row * rb + vec * 16;
+    const int step = nrow * rb;
+    bf16* d = dst + (gpix0 + row) * dC + dch;
+    const size_t dstep = (size_t)nrow * dC;
+    for (int pl = row; pl < p.ppc; pl += nrow, ++it, off += step, d += dstep) {
       float x[8], g[8], o[8];
       lds8(xs + off, x); lds8(gs + off, g);
 #pragma unroll
@@ -246,7 +250,6 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
       }
 #pragma unroll
       for (int i = 0; i < 8; ++i) sum[0][i] += o[i];
-      bf16* d = dst + (gpix0 + pl) * dC + dch;
       if (acc) {
         float f[8];
         ldv(d, f);
@@ -301,7 +304,7 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
     int BR = ppc;
     while (BR > 128 && BR % 2 == 0) BR /= 2;
     while (ppc / BR > MAXBOX && BR * 2 <= 256 && ppc % (BR * 2) == 0) BR *= 2;
-    if (BR > 256 || ppc % BR || ppc / BR > MAXBOX || (BR * rb) % 128) continue;
+    if (BR > 256 || ppc % BR || ppc / BR > MAXBOX || (BR * rb) % 128 || (BR & (BR - 1))) continue;
     const int data = ppc * rb;
     const int red = nrow * 2 * Cs + NP * 2 * Cs;
     const int need = 2 * data + (red + cl * 2 * Cs) * 4 + (add ? ED * nrow * tpp * 16 : 0);
@@ -309,6 +312,8 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
     // the smallest cluster that fits; a larger one only while the grid would leave most SMs idle
     const long long ctas = (long long)n * slices * cl;
     CL = cl; smem = need + 128;
+    p.br_shift = 0;
+    while ((1 << p.br_shift) < BR) ++p.br_shift;
     p.ppc = ppc; p.BR = BR; p.nbox = ppc / BR; p.nrow = nrow; p.data_bytes = data; p.red_floats = red;
     if (ctas * 4 >= 3LL * tmap::sm_count() || ppc / 2 < 4 * nrow) break;
   }
