@@ -227,6 +227,8 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
     const int step = nrow * rb;
     bf16* d = dst + (gpix0 + row) * dC + dch;
     const size_t dstep = (size_t)nrow * dC;
+    const bf16* ap = p.add ? p.add + (gpix0 + row + ED * nrow) * C + ch : nullptr;      // the pixel ED passes ahead
+    const size_t astep = (size_t)nrow * C;
     for (int pl = row; pl < p.ppc; pl += nrow, ++it, off += step, d += dstep) {
       float x[8], g[8], o[8];
       lds8(xs + off, x); lds8(gs + off, g);
@@ -240,11 +242,11 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
       if (p.add) {
         cp_async_wait<ED - 1>();             // the oldest outstanding request (this pixel's) has landed
         float e[8];
-        const uint32_t slot = eslot + (uint32_t)(it % ED) * nthr * 16;
-        lds8(ering + (slot - smem_u32(ering)), e);
-        const int pn = pl + ED * nrow;       // refill the slot just read
-        if (pn < p.ppc) cp_async16(slot, p.add + (gpix0 + pn) * C + ch);
+        const uint32_t sidx = (uint32_t)(it & (ED - 1)) * nthr * 16;
+        lds8(ering + tid * 16 + sidx, e);
+        if (pl + ED * nrow < p.ppc) cp_async16(eslot + sidx, ap);        // refill the slot just read
         cp_async_commit();
+        ap += astep;
 #pragma unroll
         for (int i = 0; i < 8; ++i) o[i] += e[i];
       }
