@@ -90,9 +90,19 @@ template <typename ACC>
 __device__ __forceinline__ void group_mean_rstd(const float* __restrict__ cst0, int c0, const float* __restrict__ cst1,
                                                 int c1, int n, int hw, int G, float eps, Smem& s) {
   const int C = c0 + c1, tid = tid_(), nthr = nthr_(), cpg = C / G;
-  for (int i = tid; i < 2 * C; i += nthr) {
-    const int which = i / C, c = i - which * C;
-    s.cs[i] = c < c0 ? cst0[((size_t)n * 2 + which) * c0 + c] : cst1[((size_t)n * 2 + which) * c1 + (c - c0)];
+  for (int i0 = tid; i0 < 2 * C; i0 += 4 * nthr) {      // 4 independent loads per thread in flight: one L2 round trip
+    float v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * nthr;
+      if (i < 2 * C) {
+        const int which = i >= C ? 1 : 0, c = i - which * C;
+        v[u] = c < c0 ? cst0[((size_t)n * 2 + which) * c0 + c] : cst1[((size_t)n * 2 + which) * c1 + (c - c0)];
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (i0 + u * nthr < 2 * C) s.cs[i0 + u * nthr] = v[u];
   }
   __syncthreads();
   // combined in ACC (R22: double on the fp32 debug path; fp32 for bf16 tensors, where fp64 division / sqrt cost
@@ -129,13 +139,14 @@ __device__ __forceinline__ void load_mean_rstd(const float* __restrict__ mr, int
 template <typename T, int V>
 __device__ __forceinline__ void gn_coefs(const Smem& s, int G, int cpg, const float (&gav)[V], const float (&bev)[V],
                                          int ch, float (&sc)[V], float (&sh)[V], float (&rr)[V], float (&mr)[V]) {
+  int g = ch / cpg, rem = ch - g * cpg;          // one division; the V channels then walk the groups
 #pragma unroll
   for (int i = 0; i < V; ++i) {
-    const int g = (ch + i) / cpg;
     const float mu = s.grp[g], r = s.grp[G + g];
     const float ga = gav[i], be = bev[i];
     rr[i] = r; mr[i] = mu * r;
     sc[i] = r * ga; sh[i] = be - mr[i] * ga;
+    if (++rem == cpg) { rem = 0; ++g; }
   }
 }
 

@@ -124,12 +124,13 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
   {
     float gav[8], bev[8];
     ldv(p.gamma + ch, gav); ldv(p.beta + ch, bev);
+    int g = ch / cpg, rem = ch - g * cpg;        // one division; the 8 channels then walk the groups
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-      const int g = (ch + i) / cpg;
       const float mu = p.mr[(size_t)n * 2 * p.G + g], r = p.mr[(size_t)n * 2 * p.G + p.G + g];
       rr[i] = r; mr[i] = mu * r;
       sc[i] = r * gav[i]; sh[i] = bev[i] - mr[i] * gav[i];
+      if (++rem == cpg) { rem = 0; ++g; }
     }
   }
   TLF(1);
@@ -210,12 +211,15 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
   TLF(5);
   // ---- phase 2 ------------------------------------------------------------------------------------------
   float k2[8], k3[8], sum[1][8];
+  {
+    int g = (vec * 8) / cpg, rem = vec * 8 - g * cpg;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const int g = (vec * 8 + i) / cpg;
-    k2[i] = grpAB[0][g] * rr[i];
-    k3[i] = grpAB[1][g] * rr[i];
-    sum[0][i] = 0.f;
+    for (int i = 0; i < 8; ++i) {
+      k2[i] = grpAB[0][g] * rr[i];
+      k3[i] = grpAB[1][g] * rr[i];
+      sum[0][i] = 0.f;
+      if (++rem == cpg) { rem = 0; ++g; }
+    }
   }
   const bool first = ch < p.dc0;
   bf16* dst = first ? p.dst0 : p.dst1;
