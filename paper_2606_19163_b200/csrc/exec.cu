@@ -196,12 +196,14 @@ void run_dgrad(Ctx& c, const void* g, int h, int w, int cout, size_t wt_off, int
   run_conv(c, a);
 }
 
-// Wt[ci][k-1-r][k-1-s][co] = W[co][r][s][ci] for every conv of the stage, in one batched launch.  Redone at the
-// first backward of a step (accumulate_wgrad == 0), reused by the accumulating backwards of a wave (R21).
-void prepare_weights(Ctx& c) {
+// Wt[ci][k-1-r][k-1-s][co] = W[co][r][s][ci] for the convs of ops [lo, hi), one batched launch.  Redone by the first
+// backward after a forward that followed a backward (a new step: parameters may have changed), reused by the other
+// backwards of a wave (R21).
+void prepare_weights(Ctx& c, int lo, int hi) {
   pulse_stage* s = c.s;
   std::vector<TransposeEntry> e;
-  for (const OpPlan& op : s->ops) {
+  for (int oi = hi - 1; oi >= lo; --oi) {            // in the order the backward needs them
+    const OpPlan& op = s->ops[oi];
     const int ctot = op.cin + op.cskip;
     if (op.kind == PULSE_OP_RESBLOCK) {
       e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, op.cout, 3, ctot});
@@ -211,9 +213,9 @@ void prepare_weights(Ctx& c) {
       e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, op.cout, 3, op.cin});
     }
   }
+  if (e.empty()) return;
   Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
   s->launches += flip_transpose_batch(c.dt, e.data(), (int)e.size(), c.st);
-  s->wt_valid = true;
 }
 
 void resblock_forward(Ctx& c, const OpPlan& op) {
@@ -397,9 +399,8 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
   if (!d_t) CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
   if (open && !fuse_h) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   setup_side(s, c);
-  {   // beside the chain (side stream): p[n,c] = Wt SiLU(emb) + bt of every ResBlock in one launch (row a1), joined
-      // before the first conv1; and, on the first forward of a step, the flipped / transposed weights the backward
-      // needs (parameters may have changed since the last backward; R21), joined at the end of this call
+  {   // beside the chain (side stream): (one-call form) the timestep MLP, then p[n,c] = Wt SiLU(emb) + bt of every
+      // ResBlock in one launch (row a1), joined before the first conv1
     c.fork();
     OnSide g(c);
     if (d_t) {
@@ -415,7 +416,6 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
       s->launches += temb_proj_batch(c.dt, emb, s->d.n, s->d.temb_dim, pe.data(), (int)pe.size(), c.st);
     }
     if (c.side) c.ev_proj = c.mark_side();
-    if (!s->wt_valid || s->last_was_backward) prepare_weights(c);
   }
   auto stash_in = [&](int t, const void* src) {      // channel stats of `src` + its copy into the stage's tensor t
     const Tensor& T = s->tensors[t];
@@ -451,6 +451,7 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
     }
   }
   if (c.side) c.wait_side(c.mark_side());       // join
+  if (s->last_was_backward) s->wt_valid = false;      // a forward after a backward starts a new step: the parameters may have changed
   s->last_was_backward = false;
   if (open) CK_CUDA(cudaMemcpyAsync(d_e_out, c.fwd(s->t_eout), c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
   if (c.ov_ft < 0) CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
@@ -494,9 +495,23 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
   c.emb = (const float*)(c.stash + s->emb_off); c.g_temb = d_g_temb; c.temb_stash = d_temb_stash; c.acc_w = accumulate_wgrad;
   setup_side(s, c);
+  // flipped / transposed weights for the dgrad convs, beside the memsets / column sums that open the backward (side
+  // stream): first those of the last op (waited for before its dgrad), then the rest (waited for before the next op)
+  int ev_wt_first = -1, ev_wt_rest = -1;
+  const int nops = (int)s->ops.size();
+  if (!s->wt_valid) {
+    c.fork();
+    {
+      OnSide g(c);
+      prepare_weights(c, nops - 1, nops);
+      if (c.side) ev_wt_first = c.mark_side();
+      prepare_weights(c, 0, nops - 1);
+      if (c.side) ev_wt_rest = c.mark_side();
+    }
+    s->wt_valid = true;
+  }
   if (!accumulate_wgrad)
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
-  if (!s->wt_valid) prepare_weights(c);        // normally done by the forward of this step (side stream)
   CK_CUDA(cudaMemsetAsync(c.work + s->zero_begin, 0, s->zero_end - s->zero_begin, c.st));
   const bool al = (((uintptr_t)d_g_d_out | (uintptr_t)d_g_h_in | (uintptr_t)d_g_x_in) & 255) == 0;
   if (al) { c.ov_gt[0] = s->t_dout; c.ov_gp[0] = (char*)const_cast<void*>(d_g_d_out); }       // read in place
@@ -511,6 +526,8 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
     const OpPlan& op = s->ops[i];
     const int n = s->d.n;
     c.last_op = i == 0;
+    if (i == nops - 1) c.wait_side(ev_wt_first);
+    if (i == nops - 2) c.wait_side(ev_wt_rest);
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_backward(c, op); break;
       case PULSE_OP_CONV_IN:

@@ -511,31 +511,45 @@ __global__ void flip_transpose_k(const T* __restrict__ w, int cout, int kk, int 
     if (co < cout && ci < cin) wt[((size_t)ci * kk + ftap) * cout + co] = tile[threadIdx.x][j];
   }
 }
-// all conv weights of a stage in one launch per 16 tensors: blockIdx.z = entry * 9 + tap, 64 x 64 tiles, both the
-// reads (along ci) and the writes (along co) are 128 contiguous bytes per warp row (bf16; 32-bit accesses of pairs)
+// all conv weights of a stage in one launch per 16 tensors: blockIdx.z = entry * 9 + tap, 64 x 64 tiles.  bf16 with
+// channel counts that are multiples of 8: 16-byte global accesses both ways (a tile row is 128 contiguous bytes);
+// the tile is transposed on its way INTO shared memory (8 two-byte stores per 16-byte load, pitch 66 elements: a
+// column walk lands on 4 different banks, 2-way conflicts) and read back as 4-byte words.
 template <typename T>
 __global__ void __launch_bounds__(256) flip_transpose_batch_k(const __grid_constant__ TransposeBatch b) {
   const TransposeEntry& e = b.e[blockIdx.z / 9];
   const int tap = blockIdx.z % 9, kk = e.k * e.k;
   const int ci0 = blockIdx.x * 64, co0 = blockIdx.y * 64;
   if (tap >= kk || ci0 >= e.cin || co0 >= e.cout) return;
-  const int ftap = kk - 1 - tap, tx = threadIdx.x, ty = threadIdx.y;
-  if (sizeof(T) == 2 && !(e.cin & 1) && !(e.cout & 1)) {
-    __shared__ uint16_t tile[64][66];
+  const int ftap = kk - 1 - tap, tx = threadIdx.x, ty = threadIdx.y, t = ty * 32 + tx;
+  if (sizeof(T) == 2 && !(e.cin & 7) && !(e.cout & 7)) {
+    constexpr int PITCH = 66;
+    __shared__ __align__(16) uint16_t tileT[64 * PITCH];        // [ci][co]
     const uint16_t* w = (const uint16_t*)e.w;
     uint16_t* wt = (uint16_t*)e.wt;
-    for (int j = ty; j < 64; j += 8) {
-      const int co = co0 + j, ci = ci0 + 2 * tx;
-      uint32_t v = 0;
-      if (co < e.cout && ci < e.cin) v = *reinterpret_cast<const uint32_t*>(w + ((size_t)co * kk + tap) * e.cin + ci);
-      tile[j][2 * tx] = (uint16_t)v; tile[j][2 * tx + 1] = (uint16_t)(v >> 16);
+    const int v = t & 7, r = t >> 3;            // 16-byte vector within a row, row 0..31
+    uint4 in[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int co = co0 + r + 32 * h, ci = ci0 + v * 8;
+      in[h] = (co < e.cout && ci < e.cin) ? *reinterpret_cast<const uint4*>(w + ((size_t)co * kk + tap) * e.cin + ci)
+                                          : make_uint4(0u, 0u, 0u, 0u);
+    }
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const uint32_t wd[4] = {in[h].x, in[h].y, in[h].z, in[h].w};
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        tileT[(v * 8 + k) * PITCH + r + 32 * h] = (uint16_t)(wd[k >> 1] >> ((k & 1) * 16));
     }
     __syncthreads();
-    for (int j = ty; j < 64; j += 8) {
-      const int ci = ci0 + j, co = co0 + 2 * tx;
-      if (ci < e.cin && co < e.cout)
-        *reinterpret_cast<uint32_t*>(wt + ((size_t)ci * kk + ftap) * e.cout + co) =
-            (uint32_t)tile[2 * tx][j] | ((uint32_t)tile[2 * tx + 1][j] << 16);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int cil = r + 32 * h, ci = ci0 + cil, co = co0 + v * 8;
+      if (ci < e.cin && co < e.cout) {
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(tileT + cil * PITCH + v * 8);     // 4-byte aligned
+        *reinterpret_cast<uint4*>(wt + ((size_t)ci * kk + ftap) * e.cout + co) = make_uint4(src[0], src[1], src[2], src[3]);
+      }
     }
   } else {
     __shared__ T tile[64][65];
