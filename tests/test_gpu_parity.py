@@ -103,8 +103,8 @@ def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False,
     bf16: north_star's bar (2e-2) where it is reachable, else the rounding floor of the bf16 protocol:
     the oracle is run a second time with bf16 rounding at the method's store points
     (oracle.stored_in); its own distance e_q to the exact oracle is what storing activations and
-    gradients in bf16 costs, and the CUDA path must stay within max(tol, 2 e_q) in max-abs and within
-    1.5 x in rms (reading R18)."""
+    gradients in bf16 costs, and the CUDA path must stay within max(tol, 2 e_q) in max-abs and, where it uses
+    that allowance (max-abs above tol), within 1.5 x in rms (reading R18)."""
     data = W.draw(desc, seed, with_g_e_out=with_g_e_out)
     got_raw = run_gpu(desc, data, flags, with_g_e_out)
     got = flatten(got_raw["per_mb"], got_raw["param_grads"])
@@ -130,7 +130,9 @@ def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False,
             rlimit = 1.5 * row["floor_rms"] + 1e-4 if r.numel() >= 1024 else None
         row["limit"] = limit
         rows[k] = row
-        if not (e <= limit) or (rlimit is not None and not (er <= rlimit)):
+        # north_star's bar is the max bar: a tensor inside the plain tol has met it.  The rms bound guards the tensors
+        # that are admitted under the floor allowance (tol < e <= 2 x floor) against a systematic error hiding there.
+        if not (e <= limit) or (e > tol and rlimit is not None and not (er <= rlimit)):
             bad.append((k, row))
     top = sorted(rows.items(), key=lambda kv: -kv[1]["max"] / kv[1]["limit"])[:4]
     print(f"[parity] {desc['name']} flags={flags} tol={tol:g}: " +
