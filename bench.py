@@ -309,6 +309,36 @@ def main():
             sys.stderr.write(f"bench: CUPTI kernel timing unavailable ({ex})\n")
             in_graph = None
 
+    # ---- the dominant kernel alone: the commonest 3x3 conv shape of the config, launched back to back through the
+    # C-ABI (pulse_conv2d) between two events.  This is the kernel without the event-bracket overhead of the per-class
+    # numbers above; it is compared with the BURST peak (a kernel timed alone), the brackets with the sustained one.
+    alone = None
+    if rank == 0 and desc["dtype"] == "bf16":
+        try:
+            ops = [o for o in desc["enc_ops"] + desc.get("mid_ops", []) + desc["dec_ops"] if o["kind"] == "resblock"]
+            c = ops[0]["cout"]
+            hh, ww = devs[0]["x_in"].shape[1], devs[0]["x_in"].shape[2]
+            gen = torch.Generator(device="cuda").manual_seed(1)
+            xa = torch.randn((desc["n"], hh, ww, c), device="cuda", generator=gen).to(torch.bfloat16)
+            wa = (torch.randn((c, 3, 3, c), device="cuda", generator=gen) * 0.02).to(torch.bfloat16)
+            ba = torch.zeros(c, device="cuda", dtype=torch.bfloat16)
+            for _ in range(5):
+                B.conv2d(xa, wa, bias=ba)
+            reps = 50
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a0.record()
+            for _ in range(reps):
+                B.conv2d(xa, wa, bias=ba)
+            a1.record()
+            torch.cuda.synchronize()
+            us = a0.elapsed_time(a1) * 1e3 / reps
+            fl = 2.0 * desc["n"] * hh * ww * c * c * 9
+            alone = {"shape": f"M={desc['n'] * hh * ww}, N={c}, K={9 * c}", "us_per_launch": us,
+                     "tflops": fl / (us * 1e-6) / 1e12, "launches": reps}
+        except Exception as ex:
+            sys.stderr.write(f"bench: stand-alone conv timing skipped ({ex})\n")
+
     # ---- end to end through the public API with HOST buffers -----------------------------------------------
     host = []
     for mb in data["microbatches"]:
@@ -447,6 +477,8 @@ def main():
                 "frac_in_graph": (dom.get("in_graph_tflops") or 0.0) / tf_peak,
                 "bound": "tensor", "achieved": dom.get("tflops"), "peak": tf_peak, "unit": "TFLOP/s",
                 "frac": (dom.get("tflops") or 0.0) / tf_peak, "traffic": traffic, "peak_source": peak_src,
+                "alone": None if alone is None else dict(alone, peak_burst=(peaks.get("bf16_tflops") or 1650.0),
+                                                         frac_of_burst=alone["tflops"] / (peaks.get("bf16_tflops") or 1650.0)),
                 # share of the step's kernel time (same event brackets, all classes): comparable with the share in the
                 # ncu launch list under profiles/
                 "share_of_step": (dom.get("ms_per_step") or 0.0) / max(1e-9, sum(r["ms_per_step"] for r in kern.values()))}
