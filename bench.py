@@ -339,6 +339,67 @@ def main():
         except Exception as ex:
             sys.stderr.write(f"bench: stand-alone conv timing skipped ({ex})\n")
 
+    # ---- the GroupNorm + SiLU kernels alone (north_star "Reporting": achieved HBM GB/s of the norm kernels): the
+    # config's commonest site shapes launched back to back through the C-ABI, rotating over enough buffer sets that
+    # the working set exceeds the 126 MB L2 ("hbm") and on one set ("l2_hot": what the step sees, where the producer
+    # has just written the tensor).  Algorithmic bytes: forward read x + write a; backward read x, g_a (+ add),
+    # write g_x.
+    gn_alone = None
+    if rank == 0 and desc["dtype"] == "bf16":
+        try:
+            ops = [o for o in desc["enc_ops"] + desc.get("mid_ops", []) + desc["dec_ops"] if o["kind"] == "resblock"]
+            c = ops[0]["cout"]
+            n_, hh, ww = desc["n"], devs[0]["x_in"].shape[1], devs[0]["x_in"].shape[2]
+            gen = torch.Generator(device="cuda").manual_seed(2)
+            rnd = lambda ch: torch.randn((n_, hh, ww, ch), device="cuda", generator=gen).to(torch.bfloat16)
+            gn_alone = {}
+            for name, c1 in (("single", 0), ("concat", c)):
+                C_ = c + c1
+                elems = n_ * hh * ww * C_
+                nset = max(2, int(160e6 // (elems * 2 * 3)) + 1)
+                sets = []
+                for _ in range(nset):
+                    x0, x1, ga = rnd(c), (rnd(c1) if c1 else None), rnd(C_)
+                    sets.append({"x0": x0, "x1": x1, "g_a": ga, "a": torch.empty_like(ga), "g0": torch.empty_like(x0),
+                                 "g1": None if x1 is None else torch.empty_like(x1)})
+                gam = torch.ones(C_, device="cuda", dtype=torch.bfloat16)
+                bet = torch.zeros(C_, device="cuda", dtype=torch.bfloat16)
+                scr = torch.empty(n_ * 2 * C_, device="cuda", dtype=torch.float32)
+                dg, db = torch.zeros(C_, device="cuda"), torch.zeros(C_, device="cuda")
+                for q in sets:
+                    q["stats"] = B.groupnorm_silu(q["x0"], gam, bet, desc["groups"], desc["eps"], x1=q["x1"])[1]
+
+                def fwd(q):
+                    B.lib.pulse_groupnorm_silu(B.BF16, B._ptr(q["x0"]), c, B._ptr(q["x1"]), c1, n_, hh, ww, desc["groups"],
+                                               desc["eps"], B._ptr(gam), B._ptr(bet), B._ptr(q["stats"]), 1, B._ptr(q["a"]),
+                                               B._stream())
+
+                def bwd(q):
+                    B.lib.pulse_groupnorm_silu_backward(B.BF16, 0, B._ptr(q["g_a"]), B._ptr(q["x0"]), c, B._ptr(q["x1"]), c1,
+                                                        n_, hh, ww, desc["groups"], desc["eps"], B._ptr(gam), B._ptr(bet),
+                                                        B._ptr(q["stats"]), B._ptr(scr), None, B._ptr(q["g0"]), 0,
+                                                        B._ptr(q["g1"]), 0, B._ptr(dg), B._ptr(db), B._stream())
+
+                for kind, fn, nbytes in (("fwd", fwd, 2 * 2 * elems), ("bwd", bwd, 3 * 2 * elems)):
+                    row = {"shape": f"[{n_},{hh},{ww},{c}" + (f"|{c1}]" if c1 else "]"), "bytes": nbytes}
+                    for mode, use in (("hbm", sets), ("l2_hot", sets[:1])):
+                        reps = 10 * len(sets)
+                        for q in use:
+                            fn(q)
+                        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        torch.cuda.synchronize()
+                        a0.record()
+                        for i in range(reps):
+                            fn(use[i % len(use)])
+                        a1.record()
+                        torch.cuda.synchronize()
+                        us = a0.elapsed_time(a1) * 1e3 / reps
+                        row[mode] = {"us_per_call": us, "gbs": nbytes / (us * 1e-6) / 1e9, "buffer_sets": len(use)}
+                    gn_alone[f"{kind}_{name}"] = row
+        except Exception as ex:
+            sys.stderr.write(f"bench: stand-alone GroupNorm timing skipped ({ex})\n")
+            gn_alone = None
+
     # ---- end to end through the public API with HOST buffers -----------------------------------------------
     host = []
     for mb in data["microbatches"]:
@@ -443,6 +504,9 @@ def main():
         pass
     tf_peak = peaks.get("bf16_tflops_sustained") or 1400.0
     hbm_peak = peaks.get("hbm_gbs") or 6650.0
+    for row in (gn_alone or {}).values():
+        for mode in ("hbm", "l2_hot"):
+            row[mode]["frac_of_hbm_peak"] = row[mode]["gbs"] / hbm_peak
     peak_src = "measured (MEASURED_PEAKS.json, sustained bf16 / copy)" if peaks else "fallback (B200_PROFILING.md)"
     K = args.steps
     kern = {}
@@ -493,7 +557,7 @@ def main():
             "frac_of_bf16_peak_nominal_2250": world * flops_step / (ms_per_step * 1e-3) / 1e12 / 2250.0 / world,
             "frac_of_bf16_peak_measured": flops_step / (ms_per_step * 1e-3) / 1e12 / tf_peak,
             "clocks": clocks, "gpu_launches": int(launches_per_step * K), "roofline": roofline,
-            "kernels": kern, "eager_ms_per_step": eager_ms, "loss": last_loss,
+            "kernels": kern, "gn_alone": gn_alone, "eager_ms_per_step": eager_ms, "loss": last_loss,
             "e2e": {"value": world * samples / e2e_s, "unit": "samples/s", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": 4, "ms_per_step": e2e_s * 1e3,
                     "pipelining": "H2D of step i+1 (copy stream, into the second of two device input sets, one CUDA graph per set) overlaps the compute of step i; "

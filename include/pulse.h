@@ -190,6 +190,36 @@ pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const void* d_src0,
                                   int n, int h, int w, int ksize, int stride, const void* d_g, int cout,
                                   float* d_dw, void* stream);
 
+/* GroupNorm + SiLU in isolation (the kernels of rows a2/a5 and a8/a9), on
+ * x = concat_C(x0[c0], x1[c1]) (x1 may be NULL with c1 = 0), NHWC, C = c0 + c1 divisible by groups
+ * (a group may straddle the x0|x1 boundary):
+ *   mu, var per (image, group) over its C/groups channels and all pixels (biased variance),
+ *   r = 1/sqrt(var + eps), xhat = (x - mu) r, y = gamma xhat + beta, a = y sigmoid(y).
+ * d_stats: caller-owned fp32 scratch of pulse_groupnorm_stats_floats(n, C, groups) elements; the forward
+ * fills it (per-(image, channel) sums, then mean / r per (image, group)) and the backward of the same
+ * tensor reads it.  reuse_stats != 0: d_stats already holds the statistics of this x (an earlier forward
+ * call): only the normalise + SiLU pass runs (what a conv epilogue that emitted the sums leaves to do).
+ * gamma, beta: [C] in dtype.  d_a: [n,h,w,C].  Errors: PULSE_ERR_INVALID_ARG (null pointer, sizes <= 0,
+ * dtype), PULSE_ERR_SHAPE (C % groups, channel counts not a multiple of the 16-byte vector: 4 fp32 / 8 bf16). */
+size_t pulse_groupnorm_stats_floats(int n, int c, int groups);
+pulse_status_t pulse_groupnorm_silu(int dtype, const void* d_x0, int c0, const void* d_x1, int c1, int n, int h, int w,
+                                    int groups, float eps, const void* d_gamma, const void* d_beta, float* d_stats,
+                                    int reuse_stats, void* d_a, void* stream);
+/* Backward of the above from g_a [n,h,w,C]:
+ *   g_y = g_a SiLU'(y); dgamma += sum g_y xhat; dbeta += sum g_y (fp32 [C], accumulated: caller zeroes);
+ *   q = gamma g_y; A = mean_S q; B = mean_S q xhat; g_x = r (q - A - xhat B) + add,
+ * add: [n,h,w,C] in dtype or NULL.  g_x is split at c0: channels [0,c0) -> d_g_x0 [n,h,w,c0], the rest ->
+ * d_g_x1 [n,h,w,c1] (the skip-gradient buffer of PAPER.md:L91); accumulate0 / accumulate1 != 0: += into that
+ * destination.  d_stats: as the forward left it.  d_scratch: n*2*C fp32 (zeroed here; used by the two-kernel
+ * form).  two_pass != 0 forces the two-kernel form (reduction pass + apply pass) where the one-pass cluster
+ * kernel would apply (bf16 tensors whose per-image group slices fit a cluster's shared memory). */
+pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass, const void* d_g_a, const void* d_x0, int c0,
+                                             const void* d_x1, int c1, int n, int h, int w, int groups, float eps,
+                                             const void* d_gamma, const void* d_beta, const float* d_stats,
+                                             float* d_scratch, const void* d_add, void* d_g_x0, int accumulate0,
+                                             void* d_g_x1, int accumulate1, float* d_dgamma, float* d_dbeta,
+                                             void* stream);
+
 /* ---- per-kernel-class timing (row d: measurement) -------------------------------------------
  * With profiling enabled, forward/backward bracket every kernel of these classes with CUDA events
  * on the caller's stream: 0 tcgen05 conv (fprop+dgrad), 1 tcgen05 wgrad, 2 CUDA-core conv/wgrad,

@@ -76,6 +76,11 @@ _SIG = {
                            _vp, _vp, C.c_int, _vp],
     "pulse_conv2d_wgrad": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                            _vp, C.c_int, _vp, _vp],
+    "pulse_groupnorm_silu": [C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, _vp, _vp,
+                             _vp, C.c_int, _vp, _vp],
+    "pulse_groupnorm_silu_backward": [C.c_int, C.c_int, _vp, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int,
+                                      C.c_int, C.c_float, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int, _vp, C.c_int, _vp, _vp,
+                                      _vp],
 }
 for _name, _args in _SIG.items():
     _f = getattr(lib, _name)
@@ -85,7 +90,9 @@ lib.pulse_version.restype = C.c_int
 lib.pulse_status_string.restype = C.c_char_p
 lib.pulse_status_string.argtypes = [C.c_int]
 lib.pulse_last_error.restype = C.c_char_p
-EXPORTS = list(_SIG) + ["pulse_version", "pulse_status_string", "pulse_last_error"]
+lib.pulse_groupnorm_stats_floats.restype = _sz
+lib.pulse_groupnorm_stats_floats.argtypes = [C.c_int, C.c_int, C.c_int]
+EXPORTS = list(_SIG) + ["pulse_groupnorm_stats_floats", "pulse_version", "pulse_status_string", "pulse_last_error"]
 
 
 class PulseError(RuntimeError):
@@ -372,3 +379,39 @@ def conv2d_wgrad(src0, g, ksize, src1=None, stride=1, force_simt=False):
     _ck(lib.pulse_conv2d_wgrad(_cd(src0), int(force_simt), _ptr(src0), c0, _ptr(src1), c1, n, h, wd, ksize, stride,
                                _ptr(g), cout, _ptr(dw), _stream()))
     return dw
+
+
+def groupnorm_silu(x0, gamma, beta, groups, eps=1e-5, x1=None, stats=None):
+    """a = SiLU(GroupNorm(concat_C(x0, x1))); returns (a, stats).  stats from an earlier call on the same x: only the
+    normalise + SiLU pass runs."""
+    n, h, wd, c0 = x0.shape
+    c1 = 0 if x1 is None else x1.shape[3]
+    reuse = stats is not None
+    if stats is None:
+        stats = torch.empty(lib.pulse_groupnorm_stats_floats(n, c0 + c1, groups), dtype=torch.float32, device=x0.device)
+    a = torch.empty((n, h, wd, c0 + c1), dtype=x0.dtype, device=x0.device)
+    _ck(lib.pulse_groupnorm_silu(_cd(x0), _ptr(x0), c0, _ptr(x1), c1, n, h, wd, groups, eps, _ptr(gamma), _ptr(beta),
+                                 _ptr(stats), int(reuse), _ptr(a), _stream()))
+    return a, stats
+
+
+def groupnorm_silu_backward(g_a, x0, gamma, beta, groups, stats, eps=1e-5, x1=None, add=None, two_pass=False,
+                            g_x0=None, g_x1=None, scratch=None, dgamma=None, dbeta=None):
+    """Returns (g_x0, g_x1 or None, dgamma, dbeta); g_x0 / g_x1 given: accumulated into (+=)."""
+    n, h, wd, c0 = x0.shape
+    c1 = 0 if x1 is None else x1.shape[3]
+    C_ = c0 + c1
+    acc0, acc1 = g_x0 is not None, g_x1 is not None
+    if g_x0 is None:
+        g_x0 = torch.empty((n, h, wd, c0), dtype=x0.dtype, device=x0.device)
+    if g_x1 is None and c1:
+        g_x1 = torch.empty((n, h, wd, c1), dtype=x0.dtype, device=x0.device)
+    if scratch is None:
+        scratch = torch.empty(n * 2 * C_, dtype=torch.float32, device=x0.device)
+    if dgamma is None:
+        dgamma = torch.zeros(C_, dtype=torch.float32, device=x0.device)
+        dbeta = torch.zeros(C_, dtype=torch.float32, device=x0.device)
+    _ck(lib.pulse_groupnorm_silu_backward(_cd(x0), int(two_pass), _ptr(g_a), _ptr(x0), c0, _ptr(x1), c1, n, h, wd, groups,
+                                          eps, _ptr(gamma), _ptr(beta), _ptr(stats), _ptr(scratch), _ptr(add), _ptr(g_x0),
+                                          int(acc0), _ptr(g_x1), int(acc1), _ptr(dgamma), _ptr(dbeta), _stream()))
+    return g_x0, g_x1, dgamma, dbeta

@@ -747,3 +747,66 @@ extern "C" pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const vo
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }
+
+// d_stats layout: channel stats of x0 [n][2][c0] | channel stats of x1 [n][2][c1] | mean, r [n][2][groups]
+static pulse_status_t check_gn(int dtype, int c0, int c1, int n, int h, int w, int groups) {
+  if (dtype != PULSE_F32 && dtype != PULSE_BF16) return fail(PULSE_ERR_INVALID_ARG, "dtype");
+  if (n <= 0 || h <= 0 || w <= 0 || c0 <= 0 || c1 < 0 || groups <= 0) return fail(PULSE_ERR_INVALID_ARG, "non-positive size");
+  const int vec = dtype == PULSE_F32 ? 4 : 8;
+  if ((c0 + c1) % groups) return fail(PULSE_ERR_SHAPE, "channels %d not divisible by groups %d", c0 + c1, groups);
+  if (c0 % vec || c1 % vec) return fail(PULSE_ERR_SHAPE, "channel counts must be multiples of %d", vec);
+  if ((c0 + c1) / vec > 1024) return fail(PULSE_ERR_UNSUPPORTED, "more than %d channels", 1024 * vec);
+  return PULSE_OK;
+}
+extern "C" size_t pulse_groupnorm_stats_floats(int n, int c, int groups) {
+  if (n <= 0 || c <= 0 || groups <= 0) return 0;
+  return (size_t)n * 2 * ((size_t)c + (size_t)groups);
+}
+extern "C" pulse_status_t pulse_groupnorm_silu(int dtype, const void* d_x0, int c0, const void* d_x1, int c1, int n, int h,
+                                               int w, int groups, float eps, const void* d_gamma, const void* d_beta,
+                                               float* d_stats, int reuse_stats, void* d_a, void* stream) {
+  pulse_status_t s = check_gn(dtype, c0, c1, n, h, w, groups);
+  if (s) return s;
+  if (!d_x0 || !d_gamma || !d_beta || !d_stats || !d_a || (c1 && !d_x1)) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  const int dt = dtype == PULSE_F32 ? DT_F32 : DT_BF16, hw = h * w;
+  cudaStream_t st = (cudaStream_t)stream;
+  float* cst0 = d_stats;
+  float* cst1 = cst0 + (size_t)n * 2 * c0;
+  float* mr = cst1 + (size_t)n * 2 * c1;
+  if (!reuse_stats) {
+    CK_CUDA(cudaMemsetAsync(d_stats, 0, (size_t)n * 2 * (c0 + c1) * sizeof(float), st));
+    chan_stats(dt, d_x0, n, hw, c0, cst0, st);
+    if (c1) chan_stats(dt, d_x1, n, hw, c1, cst1, st);
+  }
+  gn_silu_fwd(dt, Cat{d_x0, c0, c1 ? d_x1 : nullptr, c1}, n, hw, groups, eps, d_gamma, d_beta, cst0, c1 ? cst1 : nullptr, mr,
+              d_a, st);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass, const void* d_g_a, const void* d_x0, int c0,
+                                                        const void* d_x1, int c1, int n, int h, int w, int groups, float eps,
+                                                        const void* d_gamma, const void* d_beta, const float* d_stats,
+                                                        float* d_scratch, const void* d_add, void* d_g_x0, int accumulate0,
+                                                        void* d_g_x1, int accumulate1, float* d_dgamma, float* d_dbeta,
+                                                        void* stream) {
+  pulse_status_t s = check_gn(dtype, c0, c1, n, h, w, groups);
+  if (s) return s;
+  if (!d_g_a || !d_x0 || !d_gamma || !d_beta || !d_stats || !d_scratch || !d_g_x0 || !d_dgamma || !d_dbeta ||
+      (c1 && (!d_x1 || !d_g_x1)))
+    return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  const int dt = dtype == PULSE_F32 ? DT_F32 : DT_BF16, hw = h * w, C = c0 + c1;
+  cudaStream_t st = (cudaStream_t)stream;
+  const float* mr = d_stats + (size_t)n * 2 * C;
+  const Cat x{d_x0, c0, c1 ? d_x1 : nullptr, c1};
+  if (dt == DT_BF16 && !two_pass &&
+      gn_bwd_fused(d_g_a, x, n, hw, groups, d_gamma, d_beta, mr, d_add, d_g_x0, c0, accumulate0, d_g_x1, accumulate1,
+                   d_dgamma, d_dbeta, nullptr, nullptr, st) > 0) {
+    CK_CUDA(cudaGetLastError());
+    return PULSE_OK;
+  }
+  CK_CUDA(cudaMemsetAsync(d_scratch, 0, (size_t)n * 2 * C * sizeof(float), st));
+  gn_silu_bwd(dt, d_g_a, x, n, hw, groups, eps, d_gamma, d_beta, mr, d_scratch, d_add, d_g_x0, c0, accumulate0, d_g_x1,
+              accumulate1, d_dgamma, d_dbeta, nullptr, nullptr, st, false);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}

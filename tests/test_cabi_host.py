@@ -99,3 +99,25 @@ def test_unbound_stage_refuses_to_run(B):
     assert B.lib.pulse_stage_forward(st.h, None, 0, None, None, None, None, None, None) == 1
     assert B.lib.pulse_stage_bind_params(st.h, C.c_void_p(1), C.c_void_p(256)) == 1   # misaligned
     assert B.lib.pulse_stage_bind_workspace(st.h, C.c_void_p(256), 8) == 4            # too small
+
+
+def test_groupnorm_entry_points_validate_before_any_launch(B):
+    """include/pulse.h: INVALID_ARG for null pointers / sizes, SHAPE for C % groups and channel counts off the
+    16-byte vector; the scratch size is the closed form n * 2 * (C + groups)."""
+    L = B.lib
+    assert L.pulse_groupnorm_stats_floats(4, 640, 32) == 4 * 2 * (640 + 32)
+    assert L.pulse_groupnorm_stats_floats(0, 640, 32) == 0
+    p = C.c_void_p(256)      # never dereferenced: validation comes first
+    fwd = lambda dt, x0, c0, x1, c1, n, g: L.pulse_groupnorm_silu(dt, x0, c0, x1, c1, n, 8, 8, g, 1e-5, p, p, p, 0, p, None)
+    INVALID, SHAPE = 1, 2
+    assert fwd(B.BF16, None, 64, None, 0, 2, 8) == INVALID
+    assert fwd(B.BF16, p, 64, None, 32, 2, 8) == INVALID              # c1 > 0 without x1
+    assert fwd(B.BF16, p, 64, None, 0, 0, 8) == INVALID
+    assert fwd(7, p, 64, None, 0, 2, 8) == INVALID
+    assert fwd(B.BF16, p, 64, None, 0, 2, 7) == SHAPE                 # 64 % 7
+    assert fwd(B.BF16, p, 60, None, 0, 2, 4) == SHAPE                 # 60 channels: not a multiple of 8 bf16
+    bwd = lambda g_a, c0, g: L.pulse_groupnorm_silu_backward(B.BF16, 0, g_a, p, c0, None, 0, 2, 8, 8, g, 1e-5, p, p, p, p,
+                                                             None, p, 0, None, 0, p, p, None)
+    assert bwd(None, 64, 8) == INVALID
+    assert bwd(p, 64, 7) == SHAPE
+    assert b"divisible" in L.pulse_last_error()
