@@ -52,6 +52,31 @@ struct GnfParams {
 
 __device__ __forceinline__ void lds8(const uint8_t* p, float (&o)[8]) { ldv(reinterpret_cast<const bf16*>(p), o); }
 
+// ---- packed fp32 pairs (sm_100 FFMA2 / FMUL2 / FADD2: one issue slot for two lanes of arithmetic).  The phase loops
+// are bound by instruction issue, not by the fp32 pipe; a pair is (lo, hi) = two neighbouring channels.
+typedef unsigned long long f2_t;
+__device__ __forceinline__ f2_t pk2(float lo, float hi) { f2_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(f2_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f2_t fma2(f2_t a, f2_t b, f2_t c) { f2_t r; asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ f2_t mul2(f2_t a, f2_t b) { f2_t r; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2_t add2(f2_t a, f2_t b) { f2_t r; asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ float ex2_(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rcp_(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+// two bf16 of one 32-bit word -> fp32 pair (element 2j in the low half)
+__device__ __forceinline__ f2_t bf2(uint32_t w) { return pk2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u)); }
+// SiLU'(y) = s + y s (1 - s), s = 1 / (1 + 2^(-y log2 e)), of the pair y = x sc + sh; also returns nothing else: the
+// MUFU work (ex2, rcp) is per lane, everything around it is packed
+__device__ __forceinline__ f2_t silu_grad2(f2_t y, f2_t nl2e, f2_t one, f2_t mone) {
+  const f2_t t = mul2(y, nl2e);
+  float t0, t1;
+  upk2(t, t0, t1);
+  const f2_t d = add2(pk2(ex2_(t0), ex2_(t1)), one);
+  float d0, d1;
+  upk2(d, d0, d1);
+  const f2_t sg = pk2(rcp_(d0), rcp_(d1));
+  return fma2(mul2(y, sg), fma2(sg, mone, one), sg);
+}
+
 // sum v[K] over the `nrow` threads that share a channel vector; result[j], j < K * tpp (layout [k][Cs]) is returned
 // to every thread through `out` (shared memory, K * Cs floats).  Whole CTA; `red` holds nrow * K * Cs + NP * K * Cs floats.
 template <int K>
@@ -146,8 +171,14 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
 
   // ---- phase 1 ------------------------------------------------------------------------------------------
   float S[2][8];
+  f2_t S2[2][4], sc2[4], sh2[4], rr2[4], nmr2[4];
+  const f2_t nl2e = pk2(-1.4426950408889634f, -1.4426950408889634f), one = pk2(1.0f, 1.0f), mone = pk2(-1.0f, -1.0f);
 #pragma unroll
-  for (int i = 0; i < 8; ++i) S[0][i] = S[1][i] = 0.f;
+  for (int j = 0; j < 4; ++j) {
+    S2[0][j] = S2[1][j] = pk2(0.f, 0.f);
+    sc2[j] = pk2(sc[2 * j], sc[2 * j + 1]); sh2[j] = pk2(sh[2 * j], sh[2 * j + 1]);
+    rr2[j] = pk2(rr[2 * j], rr[2 * j + 1]); nmr2[j] = pk2(-mr[2 * j], -mr[2 * j + 1]);
+  }
   if (active) {
     int waited = 0;
     int off = row * rb + vec * 16;
@@ -155,18 +186,19 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
     for (int pl = row; pl < p.ppc; pl += nrow, off += step) {
       const int b = pl >> p.br_shift;
       while (waited <= b) { mbar_wait(&fullx[waited], 0); mbar_wait(&fullg[waited], 0); ++waited; }
-      float x[8], g[8];
-      lds8(xs + off, x); lds8(gs + off, g);
+      const uint4 xw = *reinterpret_cast<const uint4*>(xs + off), gw = *reinterpret_cast<const uint4*>(gs + off);
+      const uint32_t xv[4] = {xw.x, xw.y, xw.z, xw.w}, gv[4] = {gw.x, gw.y, gw.z, gw.w};
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const float y = fmaf(x[i], sc[i], sh[i]);
-        const float s = sigmoidf_(y);
-        const float gy = g[i] * fmaf(y * s, 1.0f - s, s);
-        S[0][i] += gy;
-        S[1][i] = fmaf(gy, fmaf(x[i], rr[i], -mr[i]), S[1][i]);
+      for (int j = 0; j < 4; ++j) {
+        const f2_t x = bf2(xv[j]);
+        const f2_t gy = mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone));
+        S2[0][j] = add2(S2[0][j], gy);
+        S2[1][j] = fma2(gy, fma2(x, rr2[j], nmr2[j]), S2[1][j]);
       }
     }
   }
+#pragma unroll
+  for (int j = 0; j < 4; ++j) { upk2(S2[0][j], S[0][2 * j], S[0][2 * j + 1]); upk2(S2[1][j], S[1][2 * j], S[1][2 * j + 1]); }
   TLF(3);
   // `add` ring: the first ED pixels of this thread are requested now, their latency hides behind the reductions
   const size_t gpix0 = (size_t)prow;
@@ -210,15 +242,21 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
 
   TLF(5);
   // ---- phase 2 ------------------------------------------------------------------------------------------
-  float k2[8], k3[8], sum[1][8];
+  float sum[1][8];
+  f2_t nk2[4], nk3[4], sum2[4];        // -A r, -B r per channel pair
   {
+    float k2[8], k3[8];
     int g = (vec * 8) / cpg, rem = vec * 8 - g * cpg;
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       k2[i] = grpAB[0][g] * rr[i];
       k3[i] = grpAB[1][g] * rr[i];
-      sum[0][i] = 0.f;
       if (++rem == cpg) { rem = 0; ++g; }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      nk2[j] = pk2(-k2[2 * j], -k2[2 * j + 1]); nk3[j] = pk2(-k3[2 * j], -k3[2 * j + 1]);
+      sum2[j] = pk2(0.f, 0.f);
     }
   }
   const bool first = ch < p.dc0;
@@ -234,37 +272,43 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
     const bf16* ap = p.add ? p.add + (gpix0 + row + ED * nrow) * C + ch : nullptr;      // the pixel ED passes ahead
     const size_t astep = (size_t)nrow * C;
     for (int pl = row; pl < p.ppc; pl += nrow, ++it, off += step, d += dstep) {
-      float x[8], g[8], o[8];
-      lds8(xs + off, x); lds8(gs + off, g);
+      const uint4 xw = *reinterpret_cast<const uint4*>(xs + off), gw = *reinterpret_cast<const uint4*>(gs + off);
+      const uint32_t xv[4] = {xw.x, xw.y, xw.z, xw.w}, gv[4] = {gw.x, gw.y, gw.z, gw.w};
+      f2_t o[4];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {          // g_y again, in fp32 (keeping it in shared memory would round it to bf16)
-        const float y = fmaf(x[i], sc[i], sh[i]);
-        const float s = sigmoidf_(y);
-        const float gy = g[i] * fmaf(y * s, 1.0f - s, s);
-        o[i] = sc[i] * gy - k2[i] - fmaf(x[i], rr[i], -mr[i]) * k3[i];
+      for (int j = 0; j < 4; ++j) {          // g_y again, in fp32 (keeping it in shared memory would round it to bf16)
+        const f2_t x = bf2(xv[j]);
+        const f2_t gy = mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone));
+        o[j] = fma2(fma2(x, rr2[j], nmr2[j]), nk3[j], fma2(sc2[j], gy, nk2[j]));
       }
       if (p.add) {
         cp_async_wait<ED - 1>();             // the oldest outstanding request (this pixel's) has landed
-        float e[8];
         const uint32_t sidx = (uint32_t)(it & (ED - 1)) * nthr * 16;
-        lds8(ering + tid * 16 + sidx, e);
+        const uint4 ew = *reinterpret_cast<const uint4*>(ering + tid * 16 + sidx);
         if (pl + ED * nrow < p.ppc) cp_async16(eslot + sidx, ap);        // refill the slot just read
         cp_async_commit();
         ap += astep;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) o[i] += e[i];
+        o[0] = add2(o[0], bf2(ew.x)); o[1] = add2(o[1], bf2(ew.y));
+        o[2] = add2(o[2], bf2(ew.z)); o[3] = add2(o[3], bf2(ew.w));
       }
 #pragma unroll
-      for (int i = 0; i < 8; ++i) sum[0][i] += o[i];
+      for (int j = 0; j < 4; ++j) sum2[j] = add2(sum2[j], o[j]);
       if (acc) {
-        float f[8];
-        ldv(d, f);
-#pragma unroll
-        for (int i = 0; i < 8; ++i) o[i] += f[i];
+        const uint4 fw = *reinterpret_cast<const uint4*>(d);
+        o[0] = add2(o[0], bf2(fw.x)); o[1] = add2(o[1], bf2(fw.y));
+        o[2] = add2(o[2], bf2(fw.z)); o[3] = add2(o[3], bf2(fw.w));
       }
-      stv(d, o);
+      uint4 ov;
+      float a, b;
+      upk2(o[0], a, b); ov.x = pack_bf16(a, b);
+      upk2(o[1], a, b); ov.y = pack_bf16(a, b);
+      upk2(o[2], a, b); ov.z = pack_bf16(a, b);
+      upk2(o[3], a, b); ov.w = pack_bf16(a, b);
+      *reinterpret_cast<uint4*>(d) = ov;
     }
   }
+#pragma unroll
+  for (int j = 0; j < 4; ++j) upk2(sum2[j], sum[0][2 * j], sum[0][2 * j + 1]);
   TLF(6);
   if (p.cs0 || p.cs1) {        // per-(image, channel) sums of what this launch adds to dst0 / dst1
     cta_reduce<1>(sum, active, row, vec, nrow, Cs, red, tot);
