@@ -340,7 +340,8 @@ def main():
             sys.stderr.write(f"bench: stand-alone conv timing skipped ({ex})\n")
 
     # ---- the GroupNorm + SiLU kernels alone (north_star "Reporting": achieved HBM GB/s of the norm kernels): the
-    # config's commonest site shapes launched back to back through the C-ABI, rotating over enough buffer sets that
+    # config's commonest site shapes launched back to back through the C-ABI (captured in one CUDA graph per
+    # measurement, so that the CPU launch rate does not bound 10 us kernels), rotating over enough buffer sets that
     # the working set exceeds the 126 MB L2 ("hbm") and on one set ("l2_hot": what the step sees, where the producer
     # has just written the tensor).  Algorithmic bytes: forward read x + write a; backward read x, g_a (+ add),
     # write g_x.
@@ -383,17 +384,24 @@ def main():
                 for kind, fn, nbytes in (("fwd", fwd, 2 * 2 * elems), ("bwd", bwd, 3 * 2 * elems)):
                     row = {"shape": f"[{n_},{hh},{ww},{c}" + (f"|{c1}]" if c1 else "]"), "bytes": nbytes}
                     for mode, use in (("hbm", sets), ("l2_hot", sets[:1])):
-                        reps = 10 * len(sets)
+                        reps, replays = 10 * len(sets), 5
                         for q in use:
                             fn(q)
+                        torch.cuda.synchronize()
+                        gg = torch.cuda.CUDAGraph()      # one graph of `reps` launches: a 10 us kernel outruns ctypes calls
+                        with torch.cuda.graph(gg):
+                            for i in range(reps):
+                                fn(use[i % len(use)])
+                        gg.replay()
                         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                         torch.cuda.synchronize()
                         a0.record()
-                        for i in range(reps):
-                            fn(use[i % len(use)])
+                        for _ in range(replays):
+                            gg.replay()
                         a1.record()
                         torch.cuda.synchronize()
-                        us = a0.elapsed_time(a1) * 1e3 / reps
+                        us = a0.elapsed_time(a1) * 1e3 / (reps * replays)
+                        del gg
                         row[mode] = {"us_per_call": us, "gbs": nbytes / (us * 1e-6) / 1e9, "buffer_sets": len(use)}
                     gn_alone[f"{kind}_{name}"] = row
         except Exception as ex:
