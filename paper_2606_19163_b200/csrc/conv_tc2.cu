@@ -467,12 +467,31 @@ static bool force_1cta() {
   if (v < 0) { const char* e = getenv("PULSE_CONV_1CTA"); v = (e && e[0] == '1') ? 1 : 0; }
   return v == 1;
 }
-bool conv_emits_stats(const ConvArgs& a) {
-  return !force_1cta() && conv_tc2_supported(a) && a.mode == CONV_FPROP && !a.accumulate;
+// Few output tiles (deep UNet levels: 1280 channels on 8 x 8 or 16 x 16 pixels give 8 / 32 pair tiles for 74 CTA
+// pairs): every tile runs in one wave either way, so the step time is ONE tile's time, and the single-CTA 128 x 160
+// tile has a quarter of the pair tile's MMAs (at 57 % of the pair's MMA rate: 0.44 of its time).  The single-CTA
+// kernel is preferred while all of its tiles still fit one wave.  PULSE_CONV_1CTA_TILES overrides the bound
+// (single-CTA tiles; 0 = never).
+static int one_cta_tile_bound() {
+  static int v = -1;
+  if (v < 0) { const char* e = getenv("PULSE_CONV_1CTA_TILES"); v = e ? atoi(e) : sm_count(); }
+  return v;
 }
+static bool prefer_1cta(const ConvArgs& a) {
+  if (!conv_tc_supported(a)) return false;
+  const bool s2d = a.mode == CONV_DGRAD_S2;
+  int bw, bh, bn;
+  if (!tile_geometry(s2d ? a.hin : a.hout, s2d ? a.win : a.wout, bw, bh, bn)) return false;
+  const int gh = s2d ? a.hin : a.hout;
+  const long long tiles_m = (long long)((gh + bh - 1) / bh) * ((a.n + bn - 1) / bn);
+  const long long tiles = tiles_m * (a.cout / (a.cout % 160 == 0 ? 160 : 128));      // its N tiles are 160 (or 128) wide
+  return tiles <= one_cta_tile_bound();
+}
+static bool use_pair(const ConvArgs& a) { return !force_1cta() && conv_tc2_supported(a) && !prefer_1cta(a); }
+bool conv_emits_stats(const ConvArgs& a) { return use_pair(a) && a.mode == CONV_FPROP && !a.accumulate; }
 bool conv_tc_any_supported(const ConvArgs& a) { return conv_tc2_supported(a) || conv_tc_supported(a); }
 int conv_tc_any(const ConvArgs& a, cudaStream_t st) {
-  if (!force_1cta() && conv_tc2_supported(a)) return conv_tc2(a, st);
+  if (use_pair(a)) return conv_tc2(a, st);
   return conv_tc(a, st);
 }
 
