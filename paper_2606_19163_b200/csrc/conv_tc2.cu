@@ -270,32 +270,46 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
             tma_store_4d(&mapO, stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
             bulk_commit();
           }
-          if (p.cst && vmask && lane < CW / 2) {
-            // channel stats of the STORED (bf16) values for the GroupNorm that reads this tensor: each lane sums two
-            // columns of the staged box over the warp's valid pixel rows (conflict-free: a row is one 128/64-byte line)
-            float s0 = 0.f, s1 = 0.f, q0 = 0.f, q1 = 0.f;
-            const uint32_t base = smem_u32(stg) + buf * C::BOX_BYTES + (lane & 3) * 4;
+          static_assert(CW == 32, "the statistics pass reads 16 words per staged row");
+          if (p.cst && vmask) {
+            // channel stats of the STORED (bf16) values for the GroupNorm that reads this tensor: a lane sums two
+            // columns of the staged box (one 32-bit word per row) over 16 of the warp's 32 pixel rows - lanes 0-15 the
+            // even rows, 16-31 the odd rows: a row is one 64-byte line, so the two halves hit disjoint banks - in packed
+            // fp32 pairs; the halves are combined by one shuffle each
+            f2_t s2 = pk2(0.f, 0.f), q2 = s2;
+            const int half = lane >> 4, l16 = lane & 15;
+            const uint32_t base = smem_u32(stg) + buf * C::BOX_BYTES + (l16 & 3) * 4;
+            const bool full = vmask == 0xffffffffu;
 #pragma unroll
-            for (int r0 = 0; r0 < 32; r0 += 8) {       // 8 independent loads in flight, no branches
+            for (int r0 = 0; r0 < 16; r0 += 8) {       // 8 independent loads in flight, no branches
               uint32_t wv[8];
 #pragma unroll
               for (int j = 0; j < 8; ++j) {
-                const int r = r0 + j;
+                const int r = 2 * (r0 + j) + half;
                 const uint32_t swr = CW == 64 ? (r & 7) : ((r >> 1) & 3);
-                asm volatile("ld.shared.b32 %0, [%1];" : "=r"(wv[j]) : "r"(base + r * (CW * 2) + (((lane >> 2) ^ swr) << 4)));
+                asm volatile("ld.shared.b32 %0, [%1];" : "=r"(wv[j]) : "r"(base + r * (CW * 2) + (((l16 >> 2) ^ swr) << 4)));
               }
 #pragma unroll
               for (int j = 0; j < 8; ++j) {
-                const float m = ((vmask >> (r0 + j)) & 1) ? 1.f : 0.f;      // rows outside the tensor do not count
-                const float a = m * __uint_as_float(wv[j] << 16), b = m * __uint_as_float(wv[j] & 0xffff0000u);
-                s0 += a; q0 = fmaf(a, a, q0); s1 += b; q1 = fmaf(b, b, q1);
+                f2_t v = bf2(wv[j]);
+                if (!full) {                            // rows outside the tensor do not count (warp-uniform branch)
+                  const float m = ((vmask >> (2 * (r0 + j) + half)) & 1) ? 1.f : 0.f;
+                  v = mul2(v, pk2(m, m));
+                }
+                s2 = add2(s2, v); q2 = fma2(v, v, q2);
               }
             }
-            float* dst = p.cst + (size_t)(n_t + n_w) * 2 * p.cout_total + co + 2 * lane;
-            if (!(DBG(p) & 32)) {
-            atomicAdd(dst, s0); atomicAdd(dst + 1, s1);
-            atomicAdd(dst + p.cout_total, q0); atomicAdd(dst + p.cout_total + 1, q1);
-            } else if (s0 + s1 + q0 + q1 == 123.456f) dst[0] = s0;
+            float s0, s1, q0, q1;
+            upk2(s2, s0, s1); upk2(q2, q0, q1);
+            s0 += __shfl_xor_sync(0xffffffffu, s0, 16); s1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+            q0 += __shfl_xor_sync(0xffffffffu, q0, 16); q1 += __shfl_xor_sync(0xffffffffu, q1, 16);
+            float* dst = p.cst + (size_t)(n_t + n_w) * 2 * p.cout_total + co + 2 * l16;
+            if (half == 0) {
+              if (!(DBG(p) & 32)) {
+                atomicAdd(dst, s0); atomicAdd(dst + 1, s1);
+                atomicAdd(dst + p.cout_total, q0); atomicAdd(dst + p.cout_total + 1, q1);
+              } else if (s0 + s1 + q0 + q1 == 123.456f) dst[0] = s0;
+            }
           }
           buf ^= 1;
         }

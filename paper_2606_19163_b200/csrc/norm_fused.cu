@@ -52,18 +52,8 @@ struct GnfParams {
 
 __device__ __forceinline__ void lds8(const uint8_t* p, float (&o)[8]) { ldv(reinterpret_cast<const bf16*>(p), o); }
 
-// ---- packed fp32 pairs (sm_100 FFMA2 / FMUL2 / FADD2: one issue slot for two lanes of arithmetic).  The phase loops
-// are bound by instruction issue, not by the fp32 pipe; a pair is (lo, hi) = two neighbouring channels.
-typedef unsigned long long f2_t;
-__device__ __forceinline__ f2_t pk2(float lo, float hi) { f2_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ void upk2(f2_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ f2_t fma2(f2_t a, f2_t b, f2_t c) { f2_t r; asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-__device__ __forceinline__ f2_t mul2(f2_t a, f2_t b) { f2_t r; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f2_t add2(f2_t a, f2_t b) { f2_t r; asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ float ex2_(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float rcp_(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
-// two bf16 of one 32-bit word -> fp32 pair (element 2j in the low half)
-__device__ __forceinline__ f2_t bf2(uint32_t w) { return pk2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u)); }
 // SiLU'(y) = s + y s (1 - s), s = 1 / (1 + 2^(-y log2 e)), of the pair y = x sc + sh; also returns nothing else: the
 // MUFU work (ex2, rcp) is per lane, everything around it is packed
 __device__ __forceinline__ f2_t silu_grad2(f2_t y, f2_t nl2e, f2_t one, f2_t mone) {
