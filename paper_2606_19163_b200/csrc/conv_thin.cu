@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(256) thin_in_wgrad_k(const T* __restrict__ in,
 // weights [4][9][C] sit in shared memory as fp32; the PB x (C/8) partial sums are reduced through shared memory.
 // Blocks walk pixel groups with a grid stride so that the 46 KB of weights are staged once per block.
 template <typename T>
-__global__ void __launch_bounds__(512) thin_out_k(const T* __restrict__ in, const T* __restrict__ w,
+__global__ void __launch_bounds__(512, 2) thin_out_k(const T* __restrict__ in, const T* __restrict__ w,
                                                   const T* __restrict__ bias, T* __restrict__ out, int n, int h, int wd,
                                                   int C, int PB, int accumulate) {
   constexpr int V = Vec<T>::N;
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(512) thin_out_k(const T* __restrict__ in, cons
 // dW[co<4][tap][c] += sum_p g[p, co] in[p + tap, c]: a thread owns (tap, 8 channels) and 4 x 8 accumulators; the
 // block walks a contiguous strip of pixels; g of the strip is staged in shared memory.
 template <typename T>
-__global__ void __launch_bounds__(512) thin_out_wgrad_k(const T* __restrict__ in, const T* __restrict__ g,
+__global__ void __launch_bounds__(512, 2) thin_out_wgrad_k(const T* __restrict__ in, const T* __restrict__ g,
                                                         float* __restrict__ dw, int n, int h, int wd, int C,
                                                         int strip) {
   constexpr int V = Vec<T>::N;
