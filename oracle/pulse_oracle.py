@@ -23,8 +23,12 @@ out below (no autograd anywhere in this file).
 Library primitives used as single steps: conv2d / conv_transpose2d / conv2d_weight
 (cross-correlation, its adjoint in the input and in the weight), matmul.  They are
 pinned in tests/test_oracle_pins.py against brute-force direct sums, adjoint
-identities, closed forms and fp64 central differences.  Parity status: pinned (no
-function here is "parity unpinned").
+identities, closed forms and fp64 central differences.  The two further instantiations
+are pinned there as well: the float32 one (configs 3-5 on the GPU box) against the float64
+one, and the storage-precision mode `stored_in` / `st` (bit-identical to the exact mode
+when storing in the compute dtype, number of store points = the closed form of DESIGN.md
+"Store points", round-to-nearest-even, idempotent).  Parity status: pinned (no function
+here is "parity unpinned").
 """
 from __future__ import annotations
 
