@@ -141,13 +141,15 @@ def reference_sample(desc, full=False):
 
 
 def run_reference(args):
+    """The oracle as it stands on the host cores: configs 1-2 at the SAME microbatch as our arm, configs 3-5 on the
+    bounded sample (one sample of one microbatch); every step is one oracle forward + backward."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     desc = W.config(args.config)
-    d1, note = reference_sample(desc)
+    d1, note = reference_sample(desc, full=True)
     data = W.draw(d1, 0)
-    for _ in range(min(args.warmup, 1)):
+    for _ in range(args.warmup):
         oracle_time(d1, data, note)
     ts = []
     for _ in range(args.steps):
@@ -156,9 +158,10 @@ def run_reference(args):
     dt = float(np.mean(ts))
     val = d1["n"] / dt
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "samples/s", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded N(0,1), DESIGN.md)",
-            "config": {"workload": WORKLOADS[args.config], "sample": note},
+            "config": {"workload": WORKLOADS[args.config], "sample": note, "samples_per_step": d1["n"],
+                       "microbatches": 1},
             "cpu_baseline": {"value": val, "unit": "samples/s", "cores": torch.get_num_threads(), "kind": "oracle",
                              "sample": note},
             "e2e": {"value": val, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -175,6 +178,9 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--brief", action="store_true", help="device-timed step only: no per-class brackets, stand-alone "
+                    "kernels, e2e, CPU baseline or other configs (what the `configs` object of the full line runs)")
+    ap.add_argument("--no-other-configs", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -201,18 +207,22 @@ def main():
     loss = torch.zeros(1, dtype=torch.float32, device="cuda")
 
     def step(devs=devs):
+        """One pass of the whole hot path; returns the tensors that leave the stage (what a neighbouring stage or the
+        host receives: e_out, d_out, g_x_in, g_h_in of every microbatch)."""
         loss.zero_()
         if M == 1:
-            return st.step(0, devs[0], 1.0, accumulate=False, loss=loss)
-        fw = []
+            r = st.step(0, devs[0], 1.0, accumulate=False, loss=loss)
+            return [r[k] for k in ("e_out", "d_out", "g_x_in", "g_h_in") if r.get(k) is not None]
+        fw, outs = [], []
         for m, dev in enumerate(devs):                      # wave: F0..F{M-1}
             fw.append(st.forward_temb(m, dev["x_in"], dev.get("h_in"), dev["t"]))
         for m in reversed(range(M)):                        # B{M-1}..B0
             emb, tst, e_out, d_out = fw[m]
             _, g_d = st.mse(d_out, devs[m]["target"], 1.0 / M, loss)
             g_temb = torch.zeros_like(emb)
-            st.backward_temb(m, g_d, None, g_temb, tst, True, accumulate=(m != M - 1))
-        return None
+            g_x_in, g_h_in = st.backward_temb(m, g_d, None, g_temb, tst, True, accumulate=(m != M - 1))
+            outs += [t for t in (e_out, d_out, g_x_in, g_h_in) if t is not None]
+        return outs
 
     # eager warm-up (first launches set function attributes, build tensor maps)
     for _ in range(2):
@@ -224,11 +234,12 @@ def main():
     launches_per_step = st.launches() - l0 + M       # + the MSE kernel(s), which take no stage handle
 
     graph = None
+    graph_outs = [None, None]          # the step's outputs inside each captured graph (static addresses)
     if not args.no_graph:
         try:
             graph = torch.cuda.CUDAGraph()
             with torch.cuda.graph(graph):
-                step()
+                graph_outs[0] = step()
         except Exception as e:      # keep measuring eagerly, say so
             graph = None
             sys.stderr.write(f"bench: CUDA graph capture failed ({e}); timing eager launches\n")
@@ -259,6 +270,21 @@ def main():
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     ms_per_step = ms / args.steps
     value = job_throughput(samples, world, ms_per_step * 1e-3)
+
+    tflops = world * flops_step / (ms_per_step * 1e-3) / 1e12
+    if args.brief:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
+                              "warmup": args.warmup, "ms_per_step": ms_per_step, "tflops": tflops,
+                              "frac_of_bf16_peak_nominal_2250": tflops / world / 2250.0, "clocks": clocks,
+                              "gpu_launches": int(launches_per_step * args.steps),
+                              "config": {"workload": WORKLOADS[args.config], "samples_per_step": samples, "microbatches": M,
+                                         "launch": "CUDA graph replay" if graph is not None else "eager launches"},
+                              "peak_skip_cache_bytes": st.cache_stats()["peak_bytes"]}))
+        return
 
     # ---- per-kernel-class times, live, same K steps launched eagerly with event brackets -----------------
     # Eager launches are CPU-bound here (eager_ms > ms_per_step): a bracket would also count the time the GPU waits
@@ -376,7 +402,7 @@ def main():
                                                B._stream())
 
                 def bwd(q):
-                    B.lib.pulse_groupnorm_silu_backward(B.BF16, 0, B._ptr(q["g_a"]), B._ptr(q["x0"]), c, B._ptr(q["x1"]), c1,
+                    B.lib.pulse_groupnorm_silu_backward(B.BF16, 0, 1, B._ptr(q["g_a"]), B._ptr(q["x0"]), c, B._ptr(q["x1"]), c1,
                                                         n_, hh, ww, desc["groups"], desc["eps"], B._ptr(gam), B._ptr(bet),
                                                         B._ptr(q["stats"]), B._ptr(scr), None, B._ptr(q["g0"]), 0,
                                                         B._ptr(q["g1"]), 0, B._ptr(dg), B._ptr(db), B._stream())
@@ -426,6 +452,7 @@ def main():
     # graphs), so it reads the H2D destination directly; the loss of step i is read back asynchronously and consumed
     # one step later.
     copy_stream = torch.cuda.Stream()
+    d2h_stream = torch.cuda.Stream()
     main = torch.cuda.current_stream()
     stg = [devs, [{k: torch.empty_like(v) for k, v in devs[m].items()} for m in range(M)]]
     for m in range(M):
@@ -437,7 +464,7 @@ def main():
             step(stg[1]); torch.cuda.synchronize()          # eager once: tensor maps of the second input set
             g2 = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g2):
-                step(stg[1])
+                graph_outs[1] = step(stg[1])
             runs = [graph.replay, g2.replay]
         except Exception as e:
             sys.stderr.write(f"bench: second CUDA graph failed ({e}); e2e copies into one input set\n")
@@ -451,6 +478,12 @@ def main():
     loss_pin = [torch.zeros(1, dtype=torch.float32).pin_memory() for _ in range(2)]
     ev_loss = [torch.cuda.Event(), torch.cuda.Event()]
     ev_step = [torch.cuda.Event(), torch.cuda.Event()]
+    # the step's results go back to pinned host buffers every step (what leaves the stage: e_out, d_out, g_x_in, g_h_in
+    # of every microbatch, and the loss); the fp32 weight gradients stay on the device for the optimizer, as in training
+    shapes0 = graph_outs[0] if graph_outs[0] is not None else step()
+    torch.cuda.synchronize()
+    out_pin = [[torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in shapes0] for _ in range(2)]
+    d2h = sum(t.numel() * t.element_size() for t in shapes0) + 4
 
     def prefetch(i):
         b = i % 2
@@ -465,27 +498,31 @@ def main():
         losses = []
         for b in range(2):
             ev_free[b].record(main)
+            ev_loss[b].record(d2h_stream)
         prefetch(0)
         for i in range(nsteps):
             b = i % 2
             if i + 1 < nsteps:
                 prefetch(i + 1)
             main.wait_event(ev_ready[b])
+            main.wait_event(ev_loss[b])                      # the outputs of step i - 2 (same buffers) have been read back
             if runs is None:                                 # fallback: one graph, D2D from the staging set
                 if b == 1:
                     for m in range(M):
                         for k in host[m]:
                             devs[m][k].copy_(stg[1][m][k], non_blocking=True)
-                run()
+                outs = run() or graph_outs[0]
             else:
-                runs[b]()
+                outs = runs[b]() or graph_outs[b]
             ev_free[b].record(main)                          # input set b may be overwritten by the H2D of step i + 2
             loss_dev[b].copy_(loss, non_blocking=True)
             ev_step[b].record(main)
-            with torch.cuda.stream(copy_stream):             # the D2H read does not sit in the compute stream
-                copy_stream.wait_event(ev_step[b])
+            with torch.cuda.stream(d2h_stream):              # the D2H reads do not sit in the compute stream
+                d2h_stream.wait_event(ev_step[b])
+                for dst, src in zip(out_pin[b], outs):
+                    dst.copy_(src, non_blocking=True)
                 loss_pin[b].copy_(loss_dev[b], non_blocking=True)
-                ev_loss[b].record(copy_stream)
+                ev_loss[b].record(d2h_stream)
             if i >= 1:                                       # consume the previous step's loss
                 ev_loss[1 - b].synchronize()
                 losses.append(float(loss_pin[1 - b][0]))
@@ -510,12 +547,17 @@ def main():
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
-    tf_peak = peaks.get("bf16_tflops_sustained") or 1400.0
+    # Every tensor figure of this line is a BURST measurement (a kernel or a 30 ms timed region at full clocks, not a
+    # seconds-long loop under the power cap), so the denominator is the burst cuBLAS figure; the sustained figure and
+    # the nominal 2250 TFLOP/s that north_star's ">= 60 %" is stated on are reported beside it.
+    tf_burst = peaks.get("bf16_tflops") or 1590.0
+    tf_sustained = peaks.get("bf16_tflops_sustained") or 1400.0
     hbm_peak = peaks.get("hbm_gbs") or 6650.0
     for row in (gn_alone or {}).values():
         for mode in ("hbm", "l2_hot"):
             row[mode]["frac_of_hbm_peak"] = row[mode]["gbs"] / hbm_peak
-    peak_src = "measured (MEASURED_PEAKS.json, sustained bf16 / copy)" if peaks else "fallback (B200_PROFILING.md)"
+    peak_src = ("measured (MEASURED_PEAKS.json: bf16_tflops = cuBLAS burst, hbm_gbs = copy)" if peaks
+                else "fallback (B200_PROFILING.md: 1.59 PFLOP/s burst, 6.65 TB/s)")
     K = args.steps
     kern = {}
     for k, v in prof.items():
@@ -524,7 +566,7 @@ def main():
         row = {"ms_per_step": v["ms"] / K, "launches_per_step": v["launches"] / K}
         if v["flops"]:
             row["tflops"] = v["flops"] / (v["ms"] * 1e-3) / 1e12
-            row["frac_of_peak"] = row["tflops"] / tf_peak
+            row["frac_of_peak"] = row["tflops"] / tf_burst
         if v["bytes"]:
             row["gbs"] = v["bytes"] / (v["ms"] * 1e-3) / 1e9
             row["frac_of_peak"] = row["gbs"] / hbm_peak
@@ -536,21 +578,25 @@ def main():
             if v["bytes"]:
                 row["in_graph_gbs"] = v["bytes"] / K / (g["ms_per_step"] * 1e-3) / 1e9
         kern[k] = row
-    traffic = None
+    traffic, traffic_src = None, None
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"config{args.config}.conv_tc")
+        tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        traffic = tj.get(f"config{args.config}.conv_tc")
+        traffic_src = tj.get("source", "profiles/traffic.json") + " (an ncu --set full capture of an earlier run, NOT measured by this run)"
     except Exception:
         pass
     dom = kern.get("conv_tc") or kern.get("conv_simt") or {}
-    gnk = [kern[k] for k in ("gn_fwd", "gn_bwd") if k in kern]
+    ach = dom.get("tflops") or 0.0
     roofline = {"kernel": "conv_tc2_k (tcgen05 cta_group::2 implicit-GEMM conv, fprop + dgrad)" if "conv_tc" in kern else "conv_simt_k",
-                "timing": "CUDA-event brackets around every launch of the class, K eager steps on the launch stream, each step enqueued behind a device-side sleep so that the brackets hold no CPU launch time",
+                "timing": "CUDA-event brackets around every launch of the class, K eager steps on the launch stream, each step enqueued behind a device-side sleep so that the brackets hold no CPU launch time (burst clocks)",
+                "bound": "tensor", "achieved": dom.get("tflops"), "peak": tf_burst, "unit": "TFLOP/s",
+                "frac": ach / tf_burst, "peak_source": peak_src,
+                "frac_of_nominal_2250": ach / 2250.0, "frac_of_sustained": ach / tf_sustained, "peak_sustained": tf_sustained,
                 "achieved_in_graph": dom.get("in_graph_tflops"),
-                "frac_in_graph": (dom.get("in_graph_tflops") or 0.0) / tf_peak,
-                "bound": "tensor", "achieved": dom.get("tflops"), "peak": tf_peak, "unit": "TFLOP/s",
-                "frac": (dom.get("tflops") or 0.0) / tf_peak, "traffic": traffic, "peak_source": peak_src,
-                "alone": None if alone is None else dict(alone, peak_burst=(peaks.get("bf16_tflops") or 1650.0),
-                                                         frac_of_burst=alone["tflops"] / (peaks.get("bf16_tflops") or 1650.0)),
+                "frac_in_graph": (dom.get("in_graph_tflops") or 0.0) / tf_burst,
+                "traffic": traffic, "traffic_source": traffic_src,
+                "alone": None if alone is None else dict(alone, peak_burst=tf_burst, frac_of_burst=alone["tflops"] / tf_burst,
+                                                         frac_of_nominal_2250=alone["tflops"] / 2250.0),
                 # share of the step's kernel time (same event brackets, all classes): comparable with the share in the
                 # ncu launch list under profiles/
                 "share_of_step": (dom.get("ms_per_step") or 0.0) / max(1e-9, sum(r["ms_per_step"] for r in kern.values()))}
@@ -561,19 +607,34 @@ def main():
                        "l2": f"no flush: per-step working set {(st.stash_bytes * M + st.work_bytes + st.skip_bytes * M + st.param_bytes + st.grad_bytes) / 2**20:.0f} MiB > 126 MiB L2",
                        "launch": "CUDA graph replay" if graph is not None else "eager launches",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
-            "tflops": world * flops_step / (ms_per_step * 1e-3) / 1e12,
-            "frac_of_bf16_peak_nominal_2250": world * flops_step / (ms_per_step * 1e-3) / 1e12 / 2250.0 / world,
-            "frac_of_bf16_peak_measured": flops_step / (ms_per_step * 1e-3) / 1e12 / tf_peak,
+            "tflops": tflops,
+            "frac_of_bf16_peak_nominal_2250": tflops / world / 2250.0,
+            "frac_of_bf16_peak_measured": tflops / world / tf_burst, "peak_measured": tf_burst,
             "clocks": clocks, "gpu_launches": int(launches_per_step * K), "roofline": roofline,
             "kernels": kern, "gn_alone": gn_alone, "eager_ms_per_step": eager_ms, "loss": last_loss,
             "e2e": {"value": world * samples / e2e_s, "unit": "samples/s", "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": 4, "ms_per_step": e2e_s * 1e3,
-                    "pipelining": "H2D of step i+1 (copy stream, into the second of two device input sets, one CUDA graph per set) overlaps the compute of step i; "
-                                  "loss read back asynchronously, consumed one step later"},
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
+                    "d2h": "e_out, d_out, g_x_in, g_h_in of every microbatch and the loss, into pinned host buffers; the fp32 weight gradients stay on the device (optimizer state)",
+                    "pipelining": "H2D of step i+1 (copy stream, into the second of two device input sets, one CUDA graph per set) and the D2H of step i-1 (second copy stream) overlap the compute of step i; "
+                                  "results consumed one step later"},
             "peak_skip_cache_bytes": st.cache_stats()["peak_bytes"]}
     if world == 1 and not args.no_cpu_baseline:
         d1, note = reference_sample(desc, full=True)
         line["cpu_baseline"] = {k: v for k, v in oracle_time(d1, W.draw(d1, 0), note).items() if k != "seconds"}
+    # ---- the other tensor-core configs, driver-run: device-timed graph replays only (10 steps, no CPU leg), each in
+    # its own process (180 GB of HBM: the parent's ~2 GB stay allocated)
+    if world == 1 and args.config == 2 and not args.no_other_configs:
+        torch.cuda.empty_cache()
+        others = {}
+        for c in (3, 4, 5):
+            try:
+                r = subprocess.run([sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", "10", "--warmup", "3",
+                                    "--brief"], capture_output=True, text=True, timeout=900)
+                last = [l for l in r.stdout.splitlines() if l.startswith("{")]
+                others[f"config{c}"] = json.loads(last[-1]) if last else {"error": (r.stderr or "no output")[-300:]}
+            except Exception as ex:
+                others[f"config{c}"] = {"error": str(ex)[:300]}
+        line["configs"] = others
     print(json.dumps(line))
 
 

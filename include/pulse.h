@@ -50,12 +50,25 @@ enum { PULSE_F32 = 0, PULSE_BF16 = 1 };
 enum { PULSE_OP_CONV_IN = 0, PULSE_OP_RESBLOCK = 1, PULSE_OP_DOWN = 2, PULSE_OP_UP = 3, PULSE_OP_HEAD = 4 };
 enum { PULSE_LINK_OPEN = 0, PULSE_LINK_CLOSED = 1 };
 enum { PULSE_TEMB_SINUSOIDAL = 0, PULSE_TEMB_MLP = 1 };
-/* flags */
+/* stage flags (cross-checks: same arithmetic, different kernel / summation order) */
 enum {
-  PULSE_FLAG_FORCE_SIMT = 1,    /* debug: CUDA-core fp32-accumulate convs even for bf16 */
-  PULSE_FLAG_GN_TWO_PASS = 2    /* debug: GroupNorm backward always as reduction pass + apply pass (never the
-                                   one-pass cluster kernel); same arithmetic, different summation order */
+  PULSE_FLAG_FORCE_SIMT = 1,    /* CUDA-core fp32-accumulate convs even for bf16 */
+  PULSE_FLAG_GN_TWO_PASS = 2,   /* GroupNorm backward always as reduction pass + apply pass (never the one-pass
+                                   cluster kernel) */
+  PULSE_FLAG_CONV_PAIR = 4,     /* tcgen05 convs: the CTA-pair kernel (conv_tc2_k) wherever it covers the shape */
+  PULSE_FLAG_CONV_1CTA = 8      /* tcgen05 convs: the single-CTA kernel (conv_tc_k) wherever it covers the shape */
 };
+/* kernel selector of the single-operator conv calls */
+enum { PULSE_CONV_AUTO = 0, PULSE_CONV_SIMT = 1, PULSE_CONV_TC_PAIR = 2, PULSE_CONV_TC_1CTA = 3 };
+
+/* Environment toggles (part of the library's observable behaviour; read ONCE per process at first use; none changes
+ * results beyond the order of fp32 sums):
+ *   PULSE_NO_PDL=1           ordinary stream-ordered launches instead of programmatic dependent launch
+ *   PULSE_NO_SIDE_STREAM=1   weight gradients / shortcut convs / timestep path on the caller's stream (no fork / join)
+ *   PULSE_NO_GN_FUSED=1      as PULSE_FLAG_GN_TWO_PASS, for every stage of the process
+ *   PULSE_CONV_1CTA=1        as PULSE_FLAG_CONV_1CTA, for every conv of the process without an explicit selector
+ *   PULSE_CONV_1CTA_TILES=k  convs with at most k single-CTA tiles take the single-CTA kernel (default: the SM count)
+ *   PULSE_WGRAD_1CTA=1       single-CTA tcgen05 weight-gradient kernel everywhere */
 
 /* One operation of the linearised model.  cin excludes the popped skip:
  * a decoder ResBlock runs on concat_C(h[cin], skip[skip_channels]), h first. */
@@ -173,16 +186,24 @@ pulse_status_t pulse_mse_fwd_bwd(int dtype, const void* d_d, const void* d_targe
 
 /* ---- single operators (the kernels of rows a2/a4/a5/a6/a8-a10 in isolation; used by the
  * kernel-level parity tests and microbenchmarks).  NHWC activations, weights [cout][k][k][cin],
- * k in {1,3}, pad (k-1)/2, stride in {1,2}; dtype as above.  force_simt != 0 selects the CUDA-core
- * kernel even where the tcgen05 kernel applies.  SURVEY.md 8c item 2. */
+ * k in {1,3}, pad (k-1)/2, stride in {1,2}; dtype as above.  kernel: PULSE_CONV_AUTO (tcgen05 where the shape is
+ * covered - CTA-pair or single-CTA kernel by tile count - else CUDA cores), PULSE_CONV_SIMT (CUDA cores),
+ * PULSE_CONV_TC_PAIR / PULSE_CONV_TC_1CTA (that tcgen05 kernel; PULSE_ERR_UNSUPPORTED if it does not cover the
+ * shape / dtype).  SURVEY.md 8c item 2. */
 /* out[n,y,x,co] = bias[co] + pn[n,co] + residual[n,y,x,co] + sum W[co][r][s][c] in[n, y st+r-pad, x st+s-pad, c],
- * in = concat_C(src0[c0], src1[c1]) (src1 may be NULL with c1 = 0); bias/pn/residual may be NULL. */
-pulse_status_t pulse_conv2d(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1, int c1,
+ * in = concat_C(src0[c0], src1[c1]) (src1 may be NULL with c1 = 0); bias/pn/residual may be NULL.
+ * d_chan_stats (nullable): [n][2][cout] fp32, += the per-(image, channel) sum and sum of squares over the pixels of
+ * the STORED output - the statistics hand-off to the GroupNorm that reads this tensor (caller zeroes it).  The
+ * CTA-pair kernel emits them from its epilogue; for the other kernels a statistics pass follows the conv.  (For
+ * PULSE_F32 tensors the sums are taken about a pivot, x - x[n, pixel 0, c], reading R22; they are an
+ * opaque hand-off to pulse_groupnorm_silu either way.) */
+pulse_status_t pulse_conv2d(int dtype, int kernel, const void* d_src0, int c0, const void* d_src1, int c1,
                             int n, int h, int w, int ksize, int stride, const void* d_w, int cout,
-                            const void* d_bias, const float* d_pn, const void* d_residual, void* d_out, void* stream);
+                            const void* d_bias, const float* d_pn, const void* d_residual, void* d_out,
+                            float* d_chan_stats, void* stream);
 /* g_in[n,h,w,cin] (+)= adjoint of the conv in its input, from g [n,hout,wout,cout].
  * d_wt_scratch: cout*k*k*cin elements of dtype (holds the flipped/transposed weights). */
-pulse_status_t pulse_conv2d_dgrad(int dtype, int force_simt, const void* d_g, int n, int h, int w, int cin,
+pulse_status_t pulse_conv2d_dgrad(int dtype, int kernel, const void* d_g, int n, int h, int w, int cin,
                                   int ksize, int stride, const void* d_w, int cout, void* d_wt_scratch,
                                   void* d_g_in, int accumulate, void* stream);
 /* dw[cout][k][k][c0+c1] += sum_{n,y,x} g[n,y,x,co] in[n, y st+r-pad, x st+s-pad, c]  (fp32, accumulated) */
@@ -212,8 +233,12 @@ pulse_status_t pulse_groupnorm_silu(int dtype, const void* d_x0, int c0, const v
  * d_g_x1 [n,h,w,c1] (the skip-gradient buffer of PAPER.md:L91); accumulate0 / accumulate1 != 0: += into that
  * destination.  d_stats: as the forward left it.  d_scratch: n*2*C fp32 (zeroed here; used by the two-kernel
  * form).  two_pass != 0 forces the two-kernel form (reduction pass + apply pass) where the one-pass cluster
- * kernel would apply (bf16 tensors whose per-image group slices fit a cluster's shared memory). */
-pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass, const void* d_g_a, const void* d_x0, int c0,
+ * kernel would apply (bf16 tensors whose per-image group slices fit a cluster's shared memory).
+ * fwd_data_ready: 0 = the call is ordered after everything enqueued on the stream before it (it may directly follow
+ * the pulse_groupnorm_silu that writes d_stats); nonzero = the caller guarantees that x0 / x1 and d_stats were
+ * complete before the PREVIOUS kernel of the stream started (as inside a stage, where they are forward-pass data):
+ * the one-pass kernel is then launched with programmatic serialization and prefetches them during that kernel's tail. */
+pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass, int fwd_data_ready, const void* d_g_a, const void* d_x0, int c0,
                                              const void* d_x1, int c1, int n, int h, int w, int groups, float eps,
                                              const void* d_gamma, const void* d_beta, const float* d_stats,
                                              float* d_scratch, const void* d_add, void* d_g_x0, int accumulate0,

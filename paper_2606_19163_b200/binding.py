@@ -22,6 +22,8 @@ F32, BF16 = 0, 1
 OP_KIND = {"conv_in": 0, "resblock": 1, "down": 2, "up": 3, "head": 4}
 FLAG_FORCE_SIMT = 1
 FLAG_GN_TWO_PASS = 2
+FLAG_CONV_PAIR = 4
+FLAG_CONV_1CTA = 8
 
 
 class OpDesc(C.Structure):
@@ -71,14 +73,14 @@ _SIG = {
     "pulse_stage_profile_read": [_vp, C.POINTER(C.c_double * 6), C.POINTER(C.c_uint64 * 6), C.POINTER(C.c_double * 6),
                                  C.POINTER(C.c_double * 6)],
     "pulse_conv2d": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp,
-                     C.c_int, _vp, _vp, _vp, _vp, _vp],
+                     C.c_int, _vp, _vp, _vp, _vp, _vp, _vp],
     "pulse_conv2d_dgrad": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int,
                            _vp, _vp, C.c_int, _vp],
     "pulse_conv2d_wgrad": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                            _vp, C.c_int, _vp, _vp],
     "pulse_groupnorm_silu": [C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, _vp, _vp,
                              _vp, C.c_int, _vp, _vp],
-    "pulse_groupnorm_silu_backward": [C.c_int, C.c_int, _vp, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int,
+    "pulse_groupnorm_silu_backward": [C.c_int, C.c_int, C.c_int, _vp, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int,
                                       C.c_int, C.c_float, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int, _vp, C.c_int, _vp, _vp,
                                       _vp],
 }
@@ -350,23 +352,28 @@ def _cd(t):
     return BF16 if t.dtype == torch.bfloat16 else F32
 
 
-def conv2d(src0, w, src1=None, bias=None, pn=None, residual=None, stride=1, force_simt=False):
+CONV_KERNELS = {"auto": 0, "simt": 1, "pair": 2, "1cta": 3}     # include/pulse.h PULSE_CONV_*
+
+
+def conv2d(src0, w, src1=None, bias=None, pn=None, residual=None, stride=1, kernel="auto", chan_stats=None):
+    """chan_stats: zeroed fp32 [n, 2, cout]; receives the sum / sum of squares per (image, channel) of the stored output."""
     n, h, wd, c0 = src0.shape
     cout, k = w.shape[0], w.shape[1]
     out = torch.empty((n, h // stride, wd // stride, cout), dtype=src0.dtype, device=src0.device)
-    _ck(lib.pulse_conv2d(_cd(src0), int(force_simt), _ptr(src0), c0, _ptr(src1), 0 if src1 is None else src1.shape[3],
-                         n, h, wd, k, stride, _ptr(w), cout, _ptr(bias), _ptr(pn), _ptr(residual), _ptr(out), _stream()))
+    _ck(lib.pulse_conv2d(_cd(src0), CONV_KERNELS[kernel], _ptr(src0), c0, _ptr(src1), 0 if src1 is None else src1.shape[3],
+                         n, h, wd, k, stride, _ptr(w), cout, _ptr(bias), _ptr(pn), _ptr(residual), _ptr(out),
+                         _ptr(chan_stats), _stream()))
     return out
 
 
-def conv2d_dgrad(g, w, in_hw, stride=1, force_simt=False, g_in=None):
+def conv2d_dgrad(g, w, in_hw, stride=1, kernel="auto", g_in=None):
     n, cout = g.shape[0], g.shape[3]
     k, cin = w.shape[1], w.shape[3]
     acc = g_in is not None
     if g_in is None:
         g_in = torch.empty((n, in_hw[0], in_hw[1], cin), dtype=g.dtype, device=g.device)
     wt = torch.empty(w.numel(), dtype=w.dtype, device=w.device)
-    _ck(lib.pulse_conv2d_dgrad(_cd(g), int(force_simt), _ptr(g), n, in_hw[0], in_hw[1], cin, k, stride, _ptr(w), cout,
+    _ck(lib.pulse_conv2d_dgrad(_cd(g), CONV_KERNELS[kernel], _ptr(g), n, in_hw[0], in_hw[1], cin, k, stride, _ptr(w), cout,
                                _ptr(wt), _ptr(g_in), int(acc), _stream()))
     return g_in
 
@@ -396,7 +403,7 @@ def groupnorm_silu(x0, gamma, beta, groups, eps=1e-5, x1=None, stats=None):
 
 
 def groupnorm_silu_backward(g_a, x0, gamma, beta, groups, stats, eps=1e-5, x1=None, add=None, two_pass=False,
-                            g_x0=None, g_x1=None, scratch=None, dgamma=None, dbeta=None):
+                            g_x0=None, g_x1=None, scratch=None, dgamma=None, dbeta=None, fwd_data_ready=False):
     """Returns (g_x0, g_x1 or None, dgamma, dbeta); g_x0 / g_x1 given: accumulated into (+=)."""
     n, h, wd, c0 = x0.shape
     c1 = 0 if x1 is None else x1.shape[3]
@@ -411,7 +418,7 @@ def groupnorm_silu_backward(g_a, x0, gamma, beta, groups, stats, eps=1e-5, x1=No
     if dgamma is None:
         dgamma = torch.zeros(C_, dtype=torch.float32, device=x0.device)
         dbeta = torch.zeros(C_, dtype=torch.float32, device=x0.device)
-    _ck(lib.pulse_groupnorm_silu_backward(_cd(x0), int(two_pass), _ptr(g_a), _ptr(x0), c0, _ptr(x1), c1, n, h, wd, groups,
+    _ck(lib.pulse_groupnorm_silu_backward(_cd(x0), int(two_pass), int(fwd_data_ready), _ptr(g_a), _ptr(x0), c0, _ptr(x1), c1, n, h, wd, groups,
                                           eps, _ptr(gamma), _ptr(beta), _ptr(stats), _ptr(scratch), _ptr(add), _ptr(g_x0),
                                           int(acc0), _ptr(g_x1), int(acc1), _ptr(dgamma), _ptr(dbeta), _stream()))
     return g_x0, g_x1, dgamma, dbeta

@@ -7,6 +7,8 @@
 #include <cstdlib>
 #include <utility>
 
+#include "toggles.h"
+
 namespace pulse {
 
 typedef __nv_bfloat16 bf16;
@@ -19,11 +21,7 @@ typedef __nv_bfloat16 bf16;
 // PULSE_NO_PDL=1 launches them as ordinary stream-ordered kernels (both calls are then no-ops).
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-inline bool pdl_enabled() {
-  static int v = -1;
-  if (v < 0) { const char* e = getenv("PULSE_NO_PDL"); v = (e && e[0] == '1') ? 0 : 1; }
-  return v == 1;
-}
+inline bool pdl_enabled() { return !toggles().no_pdl; }
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
                               Args&&... args) {

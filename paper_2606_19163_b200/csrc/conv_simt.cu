@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(256) wgrad_simt_k(WgP a) {
 }  // namespace
 
 int conv_simt(const ConvArgs& a, cudaStream_t st) {
-  if (!getenv("PULSE_NO_THIN") && conv_thin_supported(a)) return conv_thin(a, st);
+  if (conv_thin_supported(a)) return conv_thin(a, st);
   SimtP p;
   p.p0 = a.src.p0; p.c0 = a.src.c0; p.p1 = a.src.p1; p.c1 = a.src.c1;
   p.n = a.n; p.hin = a.hin; p.win = a.win; p.hout = a.hout; p.wout = a.wout;
@@ -211,7 +211,7 @@ int conv_simt(const ConvArgs& a, cudaStream_t st) {
 }
 
 int wgrad_simt(const WgradArgs& a, cudaStream_t st) {
-  if (!getenv("PULSE_NO_THIN") && wgrad_thin_supported(a)) return wgrad_thin(a, st);
+  if (wgrad_thin_supported(a)) return wgrad_thin(a, st);
   WgP p;
   p.p0 = a.src.p0; p.c0 = a.src.c0; p.p1 = a.src.p1; p.c1 = a.src.c1;
   p.n = a.n; p.hin = a.hin; p.win = a.win; p.hout = a.hout; p.wout = a.wout;

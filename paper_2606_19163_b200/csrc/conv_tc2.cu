@@ -46,17 +46,7 @@ struct Tc2Params {
   const bf16* bias; const float* pn; const bf16* residual; bf16* out; int accumulate;
   int OH, OW, osy, osx, ooy, oox, cout_total;
   float* cst;                     // channel stats [n][2][cout] of the stored output, accumulated (or null)
-  int dbg;                        // microbenchmark modes (only compiled with -DPULSE_MB): 1 no MMA, 2 no TMA, 4 no stores
 };
-#ifdef PULSE_MB
-#define DBG(p) ((p).dbg)
-__device__ unsigned long long g_tl[64];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TL(i) do { if (blockIdx.x == 0) { g_tl[i] = gtime(); g_tl[32 + i] = clock64(); } } while (0)
-#else
-#define DBG(p) 0
-#define TL(i) do {} while (0)
-#endif
 
 template <int UN, int NJ> struct Cfg2 {
   static constexpr int BN = UN * NJ;                       // output channels per pair tile
@@ -90,7 +80,6 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   const int total_tiles = p.pair_tiles_m * p.n_tiles;
   const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
 
-  if (threadIdx.x == 0) TL(0);
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB); prefetch_tmap(&mapO);
     for (int i = 0; i < C::STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
@@ -104,7 +93,6 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   const uint32_t tmem_base = tmem_base_s;
   pdl_wait();                  // everything above overlapped the tail of the previous kernel
   pdl_launch_dependents();
-  if (threadIdx.x == 0) TL(1);
 
   if (warp == 0) {
     if (lane == 0) {
@@ -118,11 +106,6 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           const int ti = kb / p.c_blocks, cb = kb - ti * p.c_blocks;
           const Tap t = p.taps[ti];
           mbar_wait(&empty_bar[stage], phase ^ 1);
-          if (DBG(p) & 2) {
-            if (rank == 0) mbar_arrive(&full_bar[stage]);
-            if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
-            continue;
-          }
           if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * C::STAGE_BYTES);
           const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
           uint8_t* sa = smem + stage * C::STAGE_BYTES;
@@ -154,18 +137,14 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&full_bar[stage], phase);
           tc_fence_after();
-          if (kb == 0) TL(2);
-          if (kb == num_kb - 1) TL(3);
           const uint32_t a_lo = desc_lo0 + stage * (C::STAGE_BYTES >> 4), b_lo = a_lo + (A_BYTES >> 4);
           if (elect_one_sync()) {
-            if (!(DBG(p) & 1)) {
 #pragma unroll
-              for (int k = 0; k < BK / 16; ++k)
+            for (int k = 0; k < BK / 16; ++k)
 #pragma unroll
-                for (int j = 0; j < NJ; ++j)
-                  umma2_bf16(tmem_d + j * UN, ((uint64_t)desc_hi << 32) | (a_lo + 2 * k),
-                             ((uint64_t)desc_hi << 32) | (b_lo + j * (C::B_SLICE >> 4) + 2 * k), idesc, (kb | k) != 0);
-            }
+              for (int j = 0; j < NJ; ++j)
+                umma2_bf16(tmem_d + j * UN, ((uint64_t)desc_hi << 32) | (a_lo + 2 * k),
+                           ((uint64_t)desc_hi << 32) | (b_lo + j * (C::B_SLICE >> 4) + 2 * k), idesc, (kb | k) != 0);
             umma2_commit_mc(&empty_bar[stage], 3);
             if (kb == num_kb - 1) umma2_commit_mc(&tfull_bar[acc], 3);
           }
@@ -222,7 +201,6 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       }
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
-      if (warp == 2 && lane == 0) TL(4);
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * C::BN;
       // software pipeline: the TMEM load of this warp's next chunk is issued before the current chunk is converted
       // and stored (tcgen05.wait::ld waits for every outstanding load, so the next one is issued right after it)
@@ -243,8 +221,8 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty_bar[acc]), 0));
         }
-        if (!(DBG(p) & 4)) {
-          if (lane == 0 && !(DBG(p) & 64)) bulk_wait_read<C::NBUF - 1>();   // the store that last used this box has read it
+        {
+          if (lane == 0) bulk_wait_read<C::NBUF - 1>();   // the store that last used this box has read it
           __syncwarp();
           const uint32_t dst = stg_lane + buf * C::BOX_BYTES;
 #pragma unroll
@@ -264,9 +242,9 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
             st_shared_v4(dst + ((i ^ sw) << 4), pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
                          pack_bf16(v[6], v[7]));
           }
-          if (!(DBG(p) & 128)) fence_proxy_async_smem();
+          fence_proxy_async_smem();
           __syncwarp();
-          if (lane == 0 && !(DBG(p) & 256)) {
+          if (lane == 0) {
             tma_store_4d(&mapO, stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
             bulk_commit();
           }
@@ -305,10 +283,8 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
             q0 += __shfl_xor_sync(0xffffffffu, q0, 16); q1 += __shfl_xor_sync(0xffffffffu, q1, 16);
             float* dst = p.cst + (size_t)(n_t + n_w) * 2 * p.cout_total + co + 2 * l16;
             if (half == 0) {
-              if (!(DBG(p) & 32)) {
-                atomicAdd(dst, s0); atomicAdd(dst + 1, s1);
-                atomicAdd(dst + p.cout_total, q0); atomicAdd(dst + p.cout_total + 1, q1);
-              } else if (s0 + s1 + q0 + q1 == 123.456f) dst[0] = s0;
+              atomicAdd(dst, s0); atomicAdd(dst + 1, s1);
+              atomicAdd(dst + p.cout_total, q0); atomicAdd(dst + p.cout_total + 1, q1);
             }
           }
           buf ^= 1;
@@ -319,20 +295,13 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
     }
     if (lane == 0) bulk_wait_read<0>();       // the staging boxes have been read; the global writes complete before the grid does
   }
-  if (warp == 2 && lane == 0) TL(5);
   tc_fence_before();
   cluster_sync_all();          // nobody leaves (or frees TMEM) while the peer may still read its shared memory / TMEM
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc2(tmem_base, C::TMEM_COLS);
   }
-  if (threadIdx.x == 32) TL(6);
 }
-#ifdef PULSE_MB
-}  // namespace
-void mb_timeline(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tl, sizeof(unsigned long long) * 64); }
-namespace {
-#endif
 
 template <int UN, int NJ>
 bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const CUtensorMap& o, const Tc2Params& p,
@@ -356,10 +325,6 @@ bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b,
 // (UN, NJ) for a channel count: 320 k -> 2 x 160; 160 k -> 1 x 160; 256 k -> 2 x 128; 128 k -> 1 x 128
 void pick_tile(int cout, int& un, int& nj) {
   un = nj = 0;
-#ifdef PULSE_MB
-  if (getenv("PULSE_NJ1") && cout % 160 == 0) { un = 160; nj = 1; return; }
-  if (getenv("PULSE_UN256") && cout % 256 == 0) { un = 256; nj = 1; return; }
-#endif
   if (cout % 320 == 0) { un = 160; nj = 2; }
   else if (cout % 160 == 0) { un = 160; nj = 1; }
   else if (cout % 256 == 0) { un = 128; nj = 2; }
@@ -407,9 +372,6 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
   p.bias = (const bf16*)a.bias; p.pn = a.pn; p.residual = (const bf16*)a.residual; p.out = (bf16*)a.out;
   p.accumulate = a.accumulate;
   p.cst = a.cst;
-#ifdef PULSE_MB
-  { const char* e = getenv("PULSE_DBG"); p.dbg = e ? atoi(e) : 0; }
-#endif
   p.OH = a.hout; p.OW = a.wout; p.osy = p.osx = 1; p.ooy = p.oox = 0; p.cout_total = a.cout;
   CUtensorMap m0, m1, mb;
   bool ok = true;
@@ -434,9 +396,6 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
       const char* base = (const char*)a.out + ((size_t)p.ooy * a.wout + p.oox) * C2;
       if (!get_map(base, 4, dims, str, box, &mo, 2 * (int)cw)) return false;
     }
-#ifdef PULSE_MB
-    if (un == 256) { bool r2 = launch2<256, 1>(m0, m1, mb, mo, p, st); if (r2) ++launches; return r2; }
-#endif
     bool r = un == 160 ? (nj == 2 ? launch2<160, 2>(m0, m1, mb, mo, p, st) : launch2<160, 1>(m0, m1, mb, mo, p, st))
                        : (nj == 2 ? launch2<128, 2>(m0, m1, mb, mo, p, st) : launch2<128, 1>(m0, m1, mb, mo, p, st));
     if (r) ++launches;
@@ -476,21 +435,12 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
   return launches;
 }
 
-static bool force_1cta() {
-  static int v = -1;
-  if (v < 0) { const char* e = getenv("PULSE_CONV_1CTA"); v = (e && e[0] == '1') ? 1 : 0; }
-  return v == 1;
-}
 // Few output tiles (deep UNet levels: 1280 channels on 8 x 8 or 16 x 16 pixels give 8 / 32 pair tiles for 74 CTA
 // pairs): every tile runs in one wave either way, so the step time is ONE tile's time, and the single-CTA 128 x 160
 // tile has a quarter of the pair tile's MMAs (at 57 % of the pair's MMA rate: 0.44 of its time).  The single-CTA
 // kernel is preferred while all of its tiles still fit one wave.  PULSE_CONV_1CTA_TILES overrides the bound
 // (single-CTA tiles; 0 = never).
-static int one_cta_tile_bound() {
-  static int v = -1;
-  if (v < 0) { const char* e = getenv("PULSE_CONV_1CTA_TILES"); v = e ? atoi(e) : sm_count(); }
-  return v;
-}
+static int one_cta_tile_bound() { return toggles().conv_1cta_tiles >= 0 ? toggles().conv_1cta_tiles : sm_count(); }
 static bool prefer_1cta(const ConvArgs& a) {
   if (!conv_tc_supported(a)) return false;
   const bool s2d = a.mode == CONV_DGRAD_S2;
@@ -501,9 +451,19 @@ static bool prefer_1cta(const ConvArgs& a) {
   const long long tiles = tiles_m * (a.cout / (a.cout % 160 == 0 ? 160 : 128));      // its N tiles are 160 (or 128) wide
   return tiles <= one_cta_tile_bound();
 }
-static bool use_pair(const ConvArgs& a) { return !force_1cta() && conv_tc2_supported(a) && !prefer_1cta(a); }
+// a.kernel: CONV_K_AUTO picks by tile count (above); CONV_K_PAIR / CONV_K_1CTA force one kernel where it applies
+static bool use_pair(const ConvArgs& a) {
+  if (!conv_tc2_supported(a)) return false;
+  if (a.kernel == CONV_K_PAIR || !conv_tc_supported(a)) return true;
+  if (a.kernel == CONV_K_1CTA || toggles().conv_1cta) return false;
+  return !prefer_1cta(a);
+}
 bool conv_emits_stats(const ConvArgs& a) { return use_pair(a) && a.mode == CONV_FPROP && !a.accumulate; }
-bool conv_tc_any_supported(const ConvArgs& a) { return conv_tc2_supported(a) || conv_tc_supported(a); }
+bool conv_tc_any_supported(const ConvArgs& a) {
+  if (a.kernel == CONV_K_PAIR) return conv_tc2_supported(a);
+  if (a.kernel == CONV_K_1CTA) return conv_tc_supported(a);
+  return conv_tc2_supported(a) || conv_tc_supported(a);
+}
 int conv_tc_any(const ConvArgs& a, cudaStream_t st) {
   if (use_pair(a)) return conv_tc2(a, st);
   return conv_tc(a, st);

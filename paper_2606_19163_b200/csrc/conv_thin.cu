@@ -297,10 +297,6 @@ int conv_thin(const ConvArgs& a, cudaStream_t st) {
 }
 
 bool wgrad_thin_supported(const WgradArgs& a) {
-  if (const char* e = getenv("PULSE_THIN_W")) {      // debug: 1 = only the thin-input wgrad, 2 = only the thin-output one
-    if (e[0] == '1' && a.src.c0 != TC) return false;
-    if (e[0] == '2' && a.src.c0 == TC) return false;
-  }
   if (!thin_common(a.ksize, a.stride, CONV_FPROP, a.src, a.hin, a.win, a.hout, a.wout)) return false;
   const int vec = a.dt == DT_F32 ? 4 : 8;
   if (a.src.c0 == TC && a.cout >= 32) return (size_t)3 * (a.win + 2) * 16 <= 96 * 1024;

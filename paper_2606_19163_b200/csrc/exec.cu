@@ -1,6 +1,7 @@
 // exec.cu - pulse_stage_forward / pulse_stage_backward / temb and loss helpers:
 // walks the op plan and enqueues kernels.  Rows a1-a11 of SURVEY.md 8a.
 #include "stage.h"
+#include "toggles.h"
 
 #include <cstdlib>
 #include <cstring>
@@ -48,9 +49,8 @@ struct Ctx {
     return n_ev - 1;
   }
   void wait_side(int ev) { if (side && ev >= 0) cudaStreamWaitEvent(st, s->sync_events[ev], 0); }
-  int side_mask = 3;             // debug (PULSE_SIDE_MASK): 1 ResBlock wgrads, 2 other ops' wgrads
   bool in_rb = false;
-  cudaStream_t wst() const { return (side && (side_mask & (in_rb ? 1 : 2))) ? side : st; }
+  cudaStream_t wst() const { return side ? side : st; }      // weight gradients: beside the chain when there is a side stream
   // boundary tensors that nothing reads after this call live directly in the caller's buffers (no copy):
   // d_out (forward), g_d_out / g_h_in / g_x_in (backward)
   int ov_ft = -1; char* ov_fp = nullptr;
@@ -80,16 +80,12 @@ struct OnSide {
   ~OnSide() { c.st = saved; }
 };
 void setup_side(pulse_stage* s, Ctx& c) {
-  if (s->side_mode < 0) {
-    const char* e = getenv("PULSE_NO_SIDE_STREAM");
-    s->side_mode = (e && e[0] == '1') ? 0 : 1;
-  }
+  if (s->side_mode < 0) s->side_mode = toggles().no_side_stream ? 0 : 1;
   if (s->side_mode == 1 && !s->profiling) {
     if (!s->side && cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking) != cudaSuccess) { s->side = nullptr; return; }
     c.side = s->side;
     if (!s->side2 && cudaStreamCreateWithFlags(&s->side2, cudaStreamNonBlocking) != cudaSuccess) s->side2 = nullptr;
     c.side2 = s->side2;
-    if (const char* m = getenv("PULSE_SIDE_MASK")) c.side_mask = atoi(m);
   }
 }
 
@@ -182,6 +178,7 @@ ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, 
   a.dt = c.dt; a.src = src; a.n = c.s->d.n; a.hin = hin; a.win = win; a.hout = hout; a.wout = wout;
   a.ksize = k; a.stride = stride; a.mode = CONV_FPROP; a.w = w; a.cout = cout; a.bias = bias; a.pn = pn;
   a.residual = res; a.out = out; a.accumulate = 0;
+  a.kernel = (c.s->d.flags & PULSE_FLAG_CONV_PAIR) ? CONV_K_PAIR : (c.s->d.flags & PULSE_FLAG_CONV_1CTA) ? CONV_K_1CTA : CONV_K_AUTO;
   return a;
 }
 
@@ -700,10 +697,17 @@ static pulse_status_t check_conv(int dtype, int c0, int c1, int n, int h, int w,
   if (stride == 2 && ((h | w) & 1)) return fail(PULSE_ERR_SHAPE, "stride 2 needs even H, W");
   return PULSE_OK;
 }
-extern "C" pulse_status_t pulse_conv2d(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1, int c1,
+static int conv_kernel_of(int kernel) { return kernel == PULSE_CONV_TC_PAIR ? CONV_K_PAIR : kernel == PULSE_CONV_TC_1CTA ? CONV_K_1CTA : CONV_K_AUTO; }
+static pulse_status_t check_kernel(int kernel, const ConvArgs& a) {
+  if (kernel < PULSE_CONV_AUTO || kernel > PULSE_CONV_TC_1CTA) return fail(PULSE_ERR_INVALID_ARG, "kernel selector %d", kernel);
+  if ((kernel == PULSE_CONV_TC_PAIR || kernel == PULSE_CONV_TC_1CTA) && !conv_tc_any_supported(a))
+    return fail(PULSE_ERR_UNSUPPORTED, "the requested tcgen05 kernel does not cover this shape / dtype");
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_conv2d(int dtype, int kernel, const void* d_src0, int c0, const void* d_src1, int c1,
                                        int n, int h, int w, int ksize, int stride, const void* d_w, int cout,
                                        const void* d_bias, const float* d_pn, const void* d_residual, void* d_out,
-                                       void* stream) {
+                                       float* d_chan_stats, void* stream) {
   pulse_status_t s = check_conv(dtype, c0, c1, n, h, w, ksize, stride, cout);
   if (s) return s;
   if (!d_src0 || !d_w || !d_out || (c1 && !d_src1)) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
@@ -711,12 +715,18 @@ extern "C" pulse_status_t pulse_conv2d(int dtype, int force_simt, const void* d_
   a.dt = dtype == PULSE_F32 ? DT_F32 : DT_BF16; a.src = Cat{d_src0, c0, d_src1, c1}; a.n = n; a.hin = h; a.win = w;
   a.hout = h / stride; a.wout = w / stride; a.ksize = ksize; a.stride = stride; a.mode = CONV_FPROP; a.w = d_w;
   a.cout = cout; a.bias = d_bias; a.pn = d_pn; a.residual = d_residual; a.out = d_out; a.accumulate = 0;
-  const int r = (!force_simt && conv_tc_any_supported(a)) ? conv_tc_any(a, (cudaStream_t)stream) : conv_simt(a, (cudaStream_t)stream);
+  a.kernel = conv_kernel_of(kernel);
+  if ((s = check_kernel(kernel, a))) return s;
+  const bool tc = kernel != PULSE_CONV_SIMT && conv_tc_any_supported(a);
+  const bool fused = d_chan_stats && tc && (a.cst = d_chan_stats, conv_emits_stats(a));
+  if (!fused) a.cst = nullptr;
+  const int r = tc ? conv_tc_any(a, (cudaStream_t)stream) : conv_simt(a, (cudaStream_t)stream);
   if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
+  if (d_chan_stats && !fused) chan_stats(a.dt, d_out, n, a.hout * a.wout, cout, d_chan_stats, (cudaStream_t)stream);
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }
-extern "C" pulse_status_t pulse_conv2d_dgrad(int dtype, int force_simt, const void* d_g, int n, int h, int w, int cin,
+extern "C" pulse_status_t pulse_conv2d_dgrad(int dtype, int kernel, const void* d_g, int n, int h, int w, int cin,
                                              int ksize, int stride, const void* d_w, int cout, void* d_wt, void* d_g_in,
                                              int accumulate, void* stream) {
   pulse_status_t s = check_conv(dtype, cin, 0, n, h, w, ksize, stride, cout);
@@ -729,7 +739,9 @@ extern "C" pulse_status_t pulse_conv2d_dgrad(int dtype, int force_simt, const vo
   a.dt = dt; a.src = Cat{d_g, cout, nullptr, 0}; a.n = n; a.hin = h / stride; a.win = w / stride; a.hout = h; a.wout = w;
   a.ksize = ksize; a.stride = 1; a.mode = stride == 2 ? CONV_DGRAD_S2 : CONV_FPROP; a.w = d_wt; a.cout = cin;
   a.bias = nullptr; a.pn = nullptr; a.residual = nullptr; a.out = d_g_in; a.accumulate = accumulate;
-  const int r = (!force_simt && conv_tc_any_supported(a)) ? conv_tc_any(a, st) : conv_simt(a, st);
+  a.kernel = conv_kernel_of(kernel);
+  if ((s = check_kernel(kernel, a))) return s;
+  const int r = (kernel != PULSE_CONV_SIMT && conv_tc_any_supported(a)) ? conv_tc_any(a, st) : conv_simt(a, st);
   if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
@@ -783,7 +795,8 @@ extern "C" pulse_status_t pulse_groupnorm_silu(int dtype, const void* d_x0, int 
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }
-extern "C" pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass, const void* d_g_a, const void* d_x0, int c0,
+extern "C" pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass, int fwd_data_ready, const void* d_g_a,
+                                                        const void* d_x0, int c0,
                                                         const void* d_x1, int c1, int n, int h, int w, int groups, float eps,
                                                         const void* d_gamma, const void* d_beta, const float* d_stats,
                                                         float* d_scratch, const void* d_add, void* d_g_x0, int accumulate0,
@@ -800,7 +813,7 @@ extern "C" pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass,
   const Cat x{d_x0, c0, c1 ? d_x1 : nullptr, c1};
   if (dt == DT_BF16 && !two_pass &&
       gn_bwd_fused(d_g_a, x, n, hw, groups, d_gamma, d_beta, mr, d_add, d_g_x0, c0, accumulate0, d_g_x1, accumulate1,
-                   d_dgamma, d_dbeta, nullptr, nullptr, st) > 0) {
+                   d_dgamma, d_dbeta, nullptr, nullptr, st, fwd_data_ready != 0) > 0) {
     CK_CUDA(cudaGetLastError());
     return PULSE_OK;
   }

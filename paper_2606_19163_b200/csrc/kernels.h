@@ -37,12 +37,15 @@ int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void*
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
                 const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
-                cudaStream_t st, bool allow_fused = true);
+                cudaStream_t st, bool allow_fused = true, bool fwd_data_ready = true);
 
-// the same in one launch (norm_fused.cu; bf16, mean / rstd from the forward); 0 = shape not covered, nothing launched
+// the same in one launch (norm_fused.cu; bf16, mean / rstd from the forward); 0 = shape not covered, nothing launched.
+// fwd_data_ready: x and mr were complete before the PREVIOUS kernel of the stream started (true inside a stage: they
+// are forward-pass data), so the kernel may read them before its dependency wait; false: launched without
+// programmatic serialization (the single-operator entry point, where the forward may be the previous kernel).
 int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* gamma, const void* beta, const float* mr,
                  const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta,
-                 float* cs0, float* cs1, cudaStream_t st);
+                 float* cs0, float* cs1, cudaStream_t st, bool fwd_data_ready = true);
 
 // ---- small ops -----------------------------------------------------------------------
 // cs[n][c] += sum over pixels of g[n][hw][c]   (tensors whose writers could not emit their column sums)
@@ -80,6 +83,7 @@ int flip_transpose(int dt, const void* w, int cout, int k, int cin, void* wt, cu
 
 // ---- convolution ---------------------------------------------------
 enum { CONV_FPROP = 0, CONV_DGRAD_S2 = 1 };
+enum { CONV_K_AUTO = 0, CONV_K_PAIR = 1, CONV_K_1CTA = 2 };      // which tcgen05 conv kernel (ConvArgs::kernel)
 struct ConvArgs {
   int dt;
   Cat src; int n, hin, win;       // source tensor(s) [n,hin,win,c]
@@ -91,6 +95,7 @@ struct ConvArgs {
   const float* pn;                // [n][cout] fp32 per-sample bias (temb projection), or null
   const void* residual;           // [n,hout,wout,cout] dtype, added, or null (may alias out)
   void* out; int accumulate;      // out (+)= result
+  int kernel = CONV_K_AUTO;       // tcgen05 kernel choice (tests / stage flags); AUTO: by tile count
   float* cst = nullptr;           // if non-null and the kernel can (conv_emits_stats): channel stats [n][2][cout] of
                                   // the stored output are accumulated here by the epilogue (norm.cu interface)
 };
@@ -116,7 +121,7 @@ int conv_tc(const ConvArgs& a, cudaStream_t st);
 // CTA-pair (cta_group::2) variant, 256-pixel x 320-channel tiles (conv_tc2.cu); preferred where it applies
 bool conv_tc2_supported(const ConvArgs& a);
 int conv_tc2(const ConvArgs& a, cudaStream_t st);
-// picks conv_tc2, else conv_tc; returns false if neither applies.  PULSE_CONV_1CTA=1 forces the single-CTA kernel.
+// picks conv_tc2 or conv_tc (ConvArgs::kernel, toggles.h); *_supported: false if the chosen kernel(s) do not apply
 bool conv_tc_any_supported(const ConvArgs& a);
 int conv_tc_any(const ConvArgs& a, cudaStream_t st);
 bool wgrad_tc_supported(const WgradArgs& a);

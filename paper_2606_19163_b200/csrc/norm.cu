@@ -58,14 +58,6 @@ RowPlan row_plan(int dt, int hw, int c, int n, int max_threads) {
 
 namespace {
 
-#ifdef PULSE_MB
-__device__ unsigned long long g_tlg[64];
-__device__ __forceinline__ unsigned long long gtime_() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TLG(k, i) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0) g_tlg[8 * (k) + (i)] = gtime_(); } while (0)
-#else
-#define TLG(k, i) do {} while (0)
-#endif
-
 template <typename T>
 __device__ __forceinline__ const T* cat_ptr(const T* p0, int c0, const T* p1, int c1, size_t pix, int ch) {
   return ch < c0 ? p0 + pix * c0 + ch : p1 + pix * c1 + (ch - c0);
@@ -86,9 +78,12 @@ __device__ __forceinline__ int tid_() { return threadIdx.y * blockDim.x + thread
 __device__ __forceinline__ int nthr_() { return blockDim.x * blockDim.y; }
 
 // grp[g] = mean, grp[G+g] = rstd of group g of image n, from the channel stats of the two sources
-template <typename ACC>
+// PIV (fp32 tensors): the sums are of (x - pivot_c), pivot_c = x[n, pixel 0, c] (chan_stats_k); they are turned into
+// plain per-channel moments in ACC = double here, where the cancellation is harmless.
+template <typename ACC, bool PIV, typename T>
 __device__ __forceinline__ void group_mean_rstd(const float* __restrict__ cst0, int c0, const float* __restrict__ cst1,
-                                                int c1, int n, int hw, int G, float eps, Smem& s) {
+                                                int c1, int n, int hw, int G, float eps, Smem& s, const T* __restrict__ p0,
+                                                const T* __restrict__ p1) {
   const int C = c0 + c1, tid = tid_(), nthr = nthr_(), cpg = C / G;
   for (int i0 = tid; i0 < 2 * C; i0 += 4 * nthr) {      // 4 independent loads per thread in flight: one L2 round trip
     float v[4];
@@ -113,7 +108,15 @@ __device__ __forceinline__ void group_mean_rstd(const float* __restrict__ cst0, 
     const int g = g0 + tid / L, l = tid % L;
     ACC a = 0, b = 0;
     if (g < G)
-      for (int c = g * cpg + l; c < (g + 1) * cpg; c += L) { a += (ACC)s.cs[c]; b += (ACC)s.cs[C + c]; }
+      for (int c = g * cpg + l; c < (g + 1) * cpg; c += L) {
+        ACC s1 = (ACC)s.cs[c], s2 = (ACC)s.cs[C + c];
+        if (PIV) {      // sum x = s1 + hw p; sum x^2 = s2 + 2 p s1 + hw p^2
+          const ACC pv = (ACC)to_f(c < c0 ? p0[(size_t)n * hw * c0 + c] : p1[(size_t)n * hw * c1 + (c - c0)]);
+          s2 += (ACC)2 * pv * s1 + (ACC)hw * pv * pv;
+          s1 += (ACC)hw * pv;
+        }
+        a += s1; b += s2;
+      }
     if (quad && tid < ((4 * G + 31) & ~31)) {
       a += __shfl_xor_sync(0xffffffffu, a, 1); b += __shfl_xor_sync(0xffffffffu, b, 1);
       a += __shfl_xor_sync(0xffffffffu, a, 2); b += __shfl_xor_sync(0xffffffffu, b, 2);
@@ -234,9 +237,17 @@ __global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, 
   const int ppc = (hw + nchunks - 1) / nchunks;
   const int pb = blockIdx.x * ppc, pe = min(hw, pb + ppc);
   const int ch = threadIdx.x * V;
-  float v[2][V];
+  float v[2][V], piv[V];
 #pragma unroll
   for (int i = 0; i < V; ++i) v[0][i] = v[1][i] = 0.f;
+  // fp32 path (R22): sums of (x - pivot), pivot = the channel's value at pixel 0 of the image, so that a channel mean far
+  // from zero does not cancel in E[x^2] - E[x]^2; the consumer (group_mean_rstd) reads the same pivot from x itself.
+  // bf16 tensors (statistics also come from conv epilogues, which see one tile each) keep plain sums.
+  if (sizeof(T) == 4) ldv(x + (size_t)n * hw * C + ch, piv);
+  else {
+#pragma unroll
+    for (int i = 0; i < V; ++i) piv[i] = 0.f;
+  }
   for (int p = pb + threadIdx.y; p < pe; p += 4 * rows) {
     float t[4][V];
 #pragma unroll
@@ -246,6 +257,8 @@ __global__ void __launch_bounds__(512, 2) chan_stats_k(const T* __restrict__ x, 
         const uint4 raw = *reinterpret_cast<const uint4*>(x + off);       // 16 bytes = V elements
         if (copy) *reinterpret_cast<uint4*>(copy + off) = raw;
         unpack(raw, t[u]);
+#pragma unroll
+        for (int i = 0; i < V; ++i) t[u][i] -= piv[i];
       } else {
 #pragma unroll
         for (int i = 0; i < V; ++i) t[u][i] = 0.f;
@@ -297,12 +310,11 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
   float gav[V], bev[V];                 // parameters: loaded before the dependency wait
 #pragma unroll
   for (int i = 0; i < V; ++i) { gav[i] = to_f(gamma[ch + i]); bev[i] = to_f(beta[ch + i]); }
-  TLG(0, 0);
   pdl_wait();
   pdl_launch_dependents();
   r.start(tid);
-  TLG(0, 1);
-  group_mean_rstd<typename std::conditional<sizeof(T) == 4, double, float>::type>(cst0, c0, cst1, c1, n, hw, G, eps, s);
+  group_mean_rstd<typename std::conditional<sizeof(T) == 4, double, float>::type, sizeof(T) == 4, T>(cst0, c0, cst1, c1, n, hw,
+                                                                                                     G, eps, s, p0, p1);
   if (blockIdx.x == 0)        // mean / rstd for the backward kernels of this site
     for (int i = tid; i < 2 * G; i += nthr_()) mr_out[(size_t)n * 2 * G + i] = s.grp[i];
   float sc[V], sh[V], rr[V], mr[V];
@@ -310,10 +322,8 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
   const bool lo = ch < c0;
   const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
   const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
-  TLG(0, 2);
   for (int c = 0; c < r.nch; ++c) {
     const uint8_t* st = r.wait(c);
-    if (c == 0) TLG(0, 3);
     const int pbase = r.pb + c * P, np = min(P, r.pe - pbase);
     for (int pl = threadIdx.y; pl < np; pl += 2 * rows) {      // two independent pixels per iteration (ILP)
       float v[2][V];
@@ -330,7 +340,6 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
     }
     r.release(c, tid);
   }
-  TLG(0, 4);
 }
 
 // ------------------------------------------------------------------------------ backward: reduction pass
@@ -356,11 +365,9 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   float gav[V], bev[V];                 // parameters: loaded before the dependency wait
 #pragma unroll
   for (int i = 0; i < V; ++i) { gav[i] = to_f(gamma[ch + i]); bev[i] = to_f(beta[ch + i]); }
-  TLG(1, 0);
   pdl_wait();
   pdl_launch_dependents();
   r.start(tid);
-  TLG(1, 1);
   load_mean_rstd(mrp, n, G, s);
   float sc[V], sh[V], rr[V], mr[V], v[2][V];
   gn_coefs<T, V>(s, G, C / G, gav, bev, ch, sc, sh, rr, mr);
@@ -370,10 +377,8 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
   const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
   const int goff = r.soff[ig] + ch * (int)sizeof(T), gpp = r.ppb[ig];
-  TLG(1, 2);
   for (int c = 0; c < r.nch; ++c) {
     const uint8_t* st = r.wait(c);
-    if (c == 0) TLG(1, 3);
     const int np = min(P, r.pe - (r.pb + c * P));
     for (int pl = threadIdx.y; pl < np; pl += rows) {
       float x[V], g[V];
@@ -388,9 +393,7 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
     }
     r.release(c, tid);
   }
-  TLG(1, 4);
   reduce_rows_atomic<V>(v, C, s, bst + (size_t)n * 2 * C);
-  TLG(1, 5);
 }
 
 // ------------------------------------------------------------------------------ backward: apply pass
@@ -420,11 +423,9 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   float gav[V], bev[V];                 // parameters: loaded before the dependency wait
 #pragma unroll
   for (int i = 0; i < V; ++i) { gav[i] = to_f(gamma[ch + i]); bev[i] = to_f(beta[ch + i]); }
-  TLG(2, 0);
   pdl_wait();
   pdl_launch_dependents();
   r.start(tid);
-  TLG(2, 1);
   load_mean_rstd(mrp, n, G, s);
   float sc[V], sh[V], rr[V], mr[V], k2[V], k3[V];
   gn_coefs<T, V>(s, G, cpg, gav, bev, ch, sc, sh, rr, mr);
@@ -475,10 +476,8 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
   const int xoff = lo ? r.soff[i0] + ch * (int)sizeof(T) : r.soff[i1] + (ch - c0) * (int)sizeof(T);
   const int xpp = lo ? r.ppb[i0] : r.ppb[i1];
   const int goff = r.soff[ig] + ch * (int)sizeof(T), eoff = r.soff[ie] + ch * (int)sizeof(T), gpp = C * (int)sizeof(T);
-  TLG(2, 2);
   for (int c = 0; c < r.nch; ++c) {
     const uint8_t* st = r.wait(c);
-    if (c == 0) TLG(2, 3);
     const int pbase = r.pb + c * P, np = min(P, r.pe - pbase);
     for (int pl = threadIdx.y; pl < np; pl += rows) {
       const size_t pix = (size_t)n * hw + pbase + pl;
@@ -500,7 +499,6 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
     }
     r.release(c, tid);
   }
-  TLG(2, 4);
   if (cs0 || cs1) {      // channels below dc0 -> cs0[n][dc0], the rest -> cs1[n][C - dc0]
     if (rows == 1) {
 #pragma unroll
@@ -524,9 +522,6 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
 }
 
 }  // namespace
-#ifdef PULSE_MB
-void mb_timeline_gn(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tlg, sizeof(unsigned long long) * 64); }
-#endif
 
 // ------------------------------------------------------------------------------ host launchers
 int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st, void* copy) {
@@ -586,12 +581,12 @@ template <typename T>
 static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
                     const float* mr, float* bst, const void* add, void* dst0, int dc0, int acc0,
                     void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st,
-                    bool allow_fused) {
+                    bool allow_fused, bool fwd_data_ready) {
   const int C = x.c();
   const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
   if (dt == DT_BF16 && allow_fused) {        // one pass with the tensors resident in shared memory where the shape allows (norm_fused.cu)
     const int r = gn_bwd_fused(g_a, x, n, hw, groups, gamma, beta, mr, add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
-                               cs0, cs1, st);
+                               cs0, cs1, st, fwd_data_ready);
     if (r > 0) return r;
   }
   static bool attr = false;
@@ -609,11 +604,11 @@ static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
                 const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
-                cudaStream_t st, bool allow_fused) {
+                cudaStream_t st, bool allow_fused, bool fwd_data_ready) {
   return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st, false)
+                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st, false, fwd_data_ready)
                       : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st, allow_fused);
+                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st, allow_fused, fwd_data_ready);
 }
 
 }  // namespace pulse

@@ -33,14 +33,6 @@ constexpr int ED = 2;          // depth of the per-thread cp.async ring for `add
 constexpr int NP = 8;          // partial sums per value in the second stage of the CTA reduction
 constexpr int MAXCS = 120;     // widest slice (channels per group 30 -> lcm(30, 8))
 
-#ifdef PULSE_MB
-__device__ unsigned long long g_tlf[16];
-__device__ __forceinline__ unsigned long long gtimef_() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TLF(i) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) g_tlf[i] = gtimef_(); } while (0)
-#else
-#define TLF(i) do {} while (0)
-#endif
-
 struct GnfParams {
   int c0, c1, hw, G, Cs, CL, ppc, BR, nbox, nrow, br_shift;   // BR = 1 << br_shift
   const bf16* gamma; const bf16* beta; const float* mr;
@@ -120,8 +112,6 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
   const bool active = tid < nthr;
   const int row = active ? tid / tpp : 0, vec = active ? tid - row * tpp : 0, ch = chs + vec * 8;
   const int prow = n * p.hw + (int)rank * p.ppc;       // first pixel (row of the [n hw][C] matrices) of this CTA
-
-  TLF(0);
   if (tid == 0) {
     prefetch_tmap(&mapX0); prefetch_tmap(&mapX1); prefetch_tmap(&mapG);
     for (int b = 0; b < p.nbox; ++b) { mbar_init(&fullx[b], 1); mbar_init(&fullg[b], 1); }
@@ -148,10 +138,8 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
       if (++rem == cpg) { rem = 0; ++g; }
     }
   }
-  TLF(1);
   pdl_wait();
   pdl_launch_dependents();
-  TLF(2);
   if (tid == 0)
     for (int b = 0; b < p.nbox; ++b) {
       mbar_expect_tx(&fullg[b], (uint32_t)(p.BR * rb));
@@ -189,7 +177,6 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
   }
 #pragma unroll
   for (int j = 0; j < 4; ++j) { upk2(S2[0][j], S[0][2 * j], S[0][2 * j + 1]); upk2(S2[1][j], S[1][2 * j], S[1][2 * j + 1]); }
-  TLF(3);
   // `add` ring: the first ED pixels of this thread are requested now, their latency hides behind the reductions
   const size_t gpix0 = (size_t)prow;
   const uint32_t eslot = smem_u32(ering) + (uint32_t)tid * 16;
@@ -202,7 +189,6 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
     }
   }
   cta_reduce<2>(S, active, row, vec, nrow, Cs, red, tot);
-  TLF(4);
   // cluster reduction: every CTA writes its 2 Cs sums into slot [rank] of every CTA of the cluster
   cluster_wait();                            // #1: every CTA of the cluster is running
   if (tid < 2 * Cs) {
@@ -229,8 +215,6 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
     grpAB[0][tid] = a * inv; grpAB[1][tid] = b * inv;
   }
   __syncthreads();
-
-  TLF(5);
   // ---- phase 2 ------------------------------------------------------------------------------------------
   float sum[1][8];
   f2_t nk2[4], nk3[4], sum2[4];        // -A r, -B r per channel pair
@@ -299,7 +283,6 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
   }
 #pragma unroll
   for (int j = 0; j < 4; ++j) upk2(sum2[j], sum[0][2 * j], sum[0][2 * j + 1]);
-  TLF(6);
   if (p.cs0 || p.cs1) {        // per-(image, channel) sums of what this launch adds to dst0 / dst1
     cta_reduce<1>(sum, active, row, vec, nrow, Cs, red, tot);
     if (tid < Cs) {
@@ -308,22 +291,17 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
       else if (p.cs1) atomicAdd(p.cs1 + (size_t)n * (C - p.dc0) + (c - p.dc0), tot[tid]);
     }
   }
-  TLF(7);
 }
 
 }  // namespace
-#ifdef PULSE_MB
-void mb_timeline_gnf(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tlf, sizeof(unsigned long long) * 16); }
-#endif
 
 static int gcd_(int a, int b) { while (b) { const int t = a % b; a = b; b = t; } return a; }
 
 // One launch, or 0 when the shape is not covered (the caller then runs the two-kernel form).
 int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* gamma, const void* beta, const float* mr,
                  const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta,
-                 float* cs0, float* cs1, cudaStream_t st) {
-  static int enabled = -1;
-  if (enabled < 0) { const char* e = getenv("PULSE_NO_GN_FUSED"); enabled = (e && e[0] == '1') ? 0 : 1; }
+                 float* cs0, float* cs1, cudaStream_t st, bool fwd_data_ready) {
+  static bool enabled = !toggles().no_gn_fused;
   if (!enabled) return 0;
   const int C = x.c();
   if (groups <= 0 || C % groups) return 0;
@@ -376,7 +354,7 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
   if (!attr) {
     if (cudaFuncSetAttribute(gn_bwd_fused_k, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048) != cudaSuccess) {
       cudaGetLastError();
-      enabled = 0;
+      enabled = false;
       return 0;
     }
     attr = true;
@@ -388,7 +366,7 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
   at[0].id = cudaLaunchAttributeClusterDimension;
   at[0].val.clusterDim.x = CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[1].val.programmaticStreamSerializationAllowed = pdl_enabled() ? 1 : 0;
+  at[1].val.programmaticStreamSerializationAllowed = (pdl_enabled() && fwd_data_ready) ? 1 : 0;
   cfg.attrs = at; cfg.numAttrs = 2;
   if (cudaLaunchKernelEx(&cfg, gn_bwd_fused_k, mx0, mx1, mg, p) != cudaSuccess) { cudaGetLastError(); return 0; }
   return 1;

@@ -37,18 +37,7 @@ constexpr int STAGES = 5;
 constexpr int FLUSH_BYTES = 8 * 2 * 2048;             // per epilogue warp: 2 x [16 co][32 c] fp32 boxes
 constexpr int SMEM = STAGES * STAGE + FLUSH_BYTES + 1024;
 
-#ifdef PULSE_MB
-__device__ unsigned long long g_tlw[64];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TL(i) do { if (blockIdx.x == 0) { g_tlw[i] = gtime(); g_tlw[32 + i] = clock64(); } } while (0)
-#define DBGW(p) ((p).dbg)
-#else
-#define TL(i) do {} while (0)
-#define DBGW(p) 0
-#endif
-
 struct Wg2Params {
-  int dbg;
   int units, c_blocks, c0_blocks, c0, ctot, ktot, s2;
   Tap taps[9];
   int bw, bh, bn, tiles_w, tiles_h;
@@ -80,7 +69,6 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
     wb = p.work * pair / npairs; we = p.work * (pair + 1) / npairs;
   }
 
-  if (threadIdx.x == 0) TL(0);
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapG); prefetch_tmap(&mapG32); prefetch_tmap(&mapW);
     for (int i = 0; i < STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
@@ -123,9 +111,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
         }
         const int x0 = tx * p.bw, y0 = ty * p.bh, n0 = tn * p.bn;
         mbar_wait(&empty_bar[stage], phase ^ 1);
-        if (DBGW(p) & 2) {
-          if (rank == 0) mbar_arrive(&full_bar[stage]);
-        } else {
+        {
           if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * STAGE);
           const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
           uint8_t* sa = smem + stage * STAGE;
@@ -162,12 +148,10 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
         }
         mbar_wait(&full_bar[stage], phase);
         tc_fence_after();
-        if (it == 0) TL(2);
-        if (it == n_items - 1) TL(3);
         const uint32_t a16 = base16 + stage * (STAGE >> 4);
         const bool last = (++pt == p.pix_tiles || it == n_items - 1);
         if (elect_one_sync()) {
-          if (!(DBGW(p) & 1)) {
+          {
 #pragma unroll
             for (int k = 0; k < PIX / 16; ++k) {
               const uint32_t acc = (!fresh || k != 0);
@@ -211,7 +195,6 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       mbar_wait(&tfull_bar, tphase);
       tphase ^= 1;
       tc_fence_after();
-      if (warp == 2 && lane == 0 && seg_end == we) TL(4);
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
       constexpr int NIT = N_TOT / 32;          // 20 chunks of 16 columns, 10 per warp
       uint32_t rr[2][16];
@@ -228,7 +211,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty_bar), 0));
         }
-        if (valid && !(DBGW(p) & 4)) {
+        if (valid) {
           if (lane == 0) bulk_wait_read<1>();
           __syncwarp();
           const uint32_t dst = stg_lane + buf * 2048;
@@ -247,20 +230,15 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
     }
     if (lane == 0) bulk_wait_read<0>();       // the staging boxes have been read; the reductions complete before the grid does
   }
-  if (warp == 2 && lane == 0) TL(5);
   tc_fence_before();
   cluster_sync_all();
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc2(tmem_base, 512);
   }
-  if (threadIdx.x == 32) TL(6);
 }
 
 }  // namespace
-#ifdef PULSE_MB
-void mb_timeline_w(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_tlw, sizeof(unsigned long long) * 64); }
-#endif
 
 bool wgrad_tc2_supported(const WgradArgs& a) {
   if (a.dt != DT_BF16) return false;
@@ -294,9 +272,6 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   p.pix_tiles = p.tiles_w * p.tiles_h * ((a.n + p.bn - 1) / p.bn);
   p.m_tiles = (p.units + 3) / 4; p.n_tiles = a.cout / N_TOT;
   p.dw = a.dw;
-#ifdef PULSE_MB
-  { const char* e = getenv("PULSE_DBG"); p.dbg = e ? atoi(e) : 0; }
-#endif
   CUtensorMap m0, m1, mg, mg32, mw;
   bool ok;
   if (s2) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
@@ -328,11 +303,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   return 1;
 }
 
-static bool force_1cta_wgrad() {
-  static int v = -1;
-  if (v < 0) { const char* e = getenv("PULSE_WGRAD_1CTA"); v = (e && e[0] == '1') ? 1 : 0; }
-  return v == 1;
-}
+static bool force_1cta_wgrad() { return toggles().wgrad_1cta; }
 bool wgrad_tc_any_supported(const WgradArgs& a) { return wgrad_tc2_supported(a) || wgrad_tc_supported(a); }
 int wgrad_tc_any(const WgradArgs& a, cudaStream_t st) {
   if (!force_1cta_wgrad() && wgrad_tc2_supported(a)) return wgrad_tc2(a, st);

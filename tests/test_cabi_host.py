@@ -116,7 +116,7 @@ def test_groupnorm_entry_points_validate_before_any_launch(B):
     assert fwd(7, p, 64, None, 0, 2, 8) == INVALID
     assert fwd(B.BF16, p, 64, None, 0, 2, 7) == SHAPE                 # 64 % 7
     assert fwd(B.BF16, p, 60, None, 0, 2, 4) == SHAPE                 # 60 channels: not a multiple of 8 bf16
-    bwd = lambda g_a, c0, g: L.pulse_groupnorm_silu_backward(B.BF16, 0, g_a, p, c0, None, 0, 2, 8, 8, g, 1e-5, p, p, p, p,
+    bwd = lambda g_a, c0, g: L.pulse_groupnorm_silu_backward(B.BF16, 0, 0, g_a, p, c0, None, 0, 2, 8, 8, g, 1e-5, p, p, p, p,
                                                              None, p, 0, None, 0, p, p, None)
     assert bwd(None, 64, 8) == INVALID
     assert bwd(p, 64, 7) == SHAPE

@@ -49,12 +49,27 @@ FPROP_CASES = [
     (1, 64, 64, 64, 0, 320, 3, 1, False),
     (1, 8, 128, 64, 0, 160, 3, 1, False),      # W = 128: one row per tile
     (5, 8, 8, 320, 0, 128, 3, 1, False),       # BN = 128 path, odd image count
+    (5, 16, 16, 64, 64, 320, 3, 1, True),      # 10 M tiles = 5 pair tiles, 1280 pixels: even pairs, every epilogue input
+    (3, 16, 16, 64, 0, 320, 3, 1, True),       # 6 M tiles: 3 pair tiles
+    (1, 24, 16, 128, 0, 160, 3, 1, True),      # 3 M tiles: the last pair has no second tile (mt >= tiles_m on rank 1)
+    (3, 8, 16, 64, 0, 640, 3, 1, False),       # 3 M tiles x 2 N tiles, image boxes (bn > 1 is 8x8 only; here bh = 8)
+    (3, 16, 16, 64, 0, 160, 3, 2, True),       # stride 2: 8x8 outputs, 192 pixels, image box beyond N on the pair's rank 1
 ]
+KERNELS = ["pair", "1cta", "simt"]
 
 
-@pytest.mark.parametrize("simt", [False, True])
+def _or_skip(B, fn):
+    try:
+        return fn()
+    except B.PulseError as e:
+        if e.status == 3:
+            pytest.skip("this tcgen05 kernel does not cover the shape")
+        raise
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("case", FPROP_CASES)
-def test_conv_fprop(case, simt):
+def test_conv_fprop(case, kernel):
     B = _B()
     n, h, w, c0, c1, cout, k, stride, extras = case
     rng = np.random.default_rng(hash(case) % 2 ** 31)
@@ -67,37 +82,47 @@ def test_conv_fprop(case, simt):
     ref = O.conv_fwd(xin, torch.as_tensor(wt).double(), None if bias is None else torch.as_tensor(bias).double(), stride)
     if extras:
         ref = ref + torch.as_tensor(pn).double()[:, :, None, None] + torch.as_tensor(res).double()
-    got = B.conv2d(dev_nhwc(x0), dev_w(wt), None if x1 is None else dev_nhwc(x1),
-                   None if bias is None else torch.as_tensor(bias).to("cuda", torch.bfloat16),
-                   None if pn is None else torch.as_tensor(pn).cuda(), None if res is None else dev_nhwc(res),
-                   stride=stride, force_simt=simt)
+    cst = torch.zeros((n, 2, cout), dtype=torch.float32, device="cuda")
+    got = _or_skip(B, lambda: B.conv2d(dev_nhwc(x0), dev_w(wt), None if x1 is None else dev_nhwc(x1),
+                                       None if bias is None else torch.as_tensor(bias).to("cuda", torch.bfloat16),
+                                       None if pn is None else torch.as_tensor(pn).cuda(),
+                                       None if res is None else dev_nhwc(res), stride=stride, kernel=kernel,
+                                       chan_stats=cst))
     torch.cuda.synchronize()
-    assert_bf16_close(B.nchw(got), ref, f"fprop {case} simt={simt}")
+    assert_bf16_close(B.nchw(got), ref, f"fprop {case} kernel={kernel}")
+    # statistics hand-off (fused into the pair kernel's epilogue, masked on ragged tiles): sums of the STORED values
+    stored = got.double()                                         # [n, h, w, cout]
+    want = torch.stack([stored.sum((1, 2)), stored.pow(2).sum((1, 2))], 1).cpu()
+    tol = 1e-4 * float(want[:, 1].abs().max()) + 1e-3
+    assert float((cst.double().cpu() - want).abs().max()) <= tol, f"chan stats {case} kernel={kernel}"
 
 
 DGRAD_CASES = [
     (3, 8, 8, 128, 160, 3, 1), (2, 16, 16, 320, 64, 3, 1), (1, 32, 32, 160, 128, 1, 1),
     (2, 16, 16, 160, 128, 3, 2), (3, 32, 32, 320, 64, 3, 2),
+    (3, 16, 16, 320, 128, 3, 1),               # 6 M tiles = 3 pair tiles
+    (1, 24, 16, 160, 64, 3, 1),                # 3 M tiles: odd count
+    (3, 16, 16, 160, 64, 3, 2),                # stride-2 dgrad phases on 8x8 grids of 3 images (1.5 tiles per phase)
 ]
 
 
-@pytest.mark.parametrize("simt", [False, True])
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("case", DGRAD_CASES)
-def test_conv_dgrad(case, simt):
+def test_conv_dgrad(case, kernel):
     B = _B()
     n, h, w, cin, cout, k, stride = case       # h, w: input (g_in) size
     rng = np.random.default_rng(hash(case) % 2 ** 31)
     g = grid(rng, n, cout, h // stride, w // stride)
     wt = grid(rng, cout, cin, k, k, scale=(2.0 / (cin * k * k)) ** 0.5)
     ref = O.conv_dgrad(torch.as_tensor(g).double(), torch.as_tensor(wt).double(), (h, w), stride)
-    got = B.conv2d_dgrad(dev_nhwc(g), dev_w(wt), (h, w), stride=stride, force_simt=simt)
+    got = _or_skip(B, lambda: B.conv2d_dgrad(dev_nhwc(g), dev_w(wt), (h, w), stride=stride, kernel=kernel))
     torch.cuda.synchronize()
-    assert_bf16_close(B.nchw(got), ref, f"dgrad {case} simt={simt}")
+    assert_bf16_close(B.nchw(got), ref, f"dgrad {case} kernel={kernel}")
     # accumulate: g_in += ... on top of a seeded tensor
     base = grid(rng, n, cin, h, w)
-    acc = B.conv2d_dgrad(dev_nhwc(g), dev_w(wt), (h, w), stride=stride, force_simt=simt, g_in=dev_nhwc(base))
+    acc = B.conv2d_dgrad(dev_nhwc(g), dev_w(wt), (h, w), stride=stride, kernel=kernel, g_in=dev_nhwc(base))
     torch.cuda.synchronize()
-    assert_bf16_close(B.nchw(acc), ref + torch.as_tensor(base).double(), f"dgrad+= {case} simt={simt}")
+    assert_bf16_close(B.nchw(acc), ref + torch.as_tensor(base).double(), f"dgrad+= {case} kernel={kernel}")
 
 
 WGRAD_CASES = [

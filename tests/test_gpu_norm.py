@@ -55,12 +55,12 @@ CASES = [
 ]
 
 
-def _run_case(case, dtype, two_pass=False, with_add=False, accumulate=False, seed=0):
+def _run_case(case, dtype, two_pass=False, with_add=False, accumulate=False, seed=0, shift=0.3, scale=1.5):
     B = _B()
     n, h, w, c0, c1, groups = case
     C = c0 + c1
     rng = np.random.default_rng(abs(hash((case, seed))) % 2 ** 31)
-    x = grid(rng, n, C, h, w, scale=1.5, shift=0.3)
+    x = grid(rng, n, C, h, w, scale=scale, shift=shift)
     gamma, beta = grid(rng, C, scale=0.5, shift=1.0), grid(rng, C, scale=0.3)
     g_a = grid(rng, n, C, h, w)
     add = grid(rng, n, C, h, w) if with_add else None
@@ -110,6 +110,14 @@ def test_groupnorm_silu_fp32(case):
 def test_groupnorm_silu_backward_add_and_accumulate(case, two_pass):
     _run_case(case, torch.bfloat16, two_pass=two_pass, with_add=True, seed=1)
     _run_case(case, torch.bfloat16, two_pass=two_pass, with_add=True, accumulate=True, seed=2)
+
+
+@pytest.mark.parametrize("dtype", [torch.bfloat16, torch.float32])
+@pytest.mark.parametrize("case", [CASES[1], CASES[6]])
+def test_groupnorm_silu_large_mean(case, dtype):
+    """|mean| = 20 sigma: the statistics travel as per-channel sums of x and x^2 (variance = E[x^2] - E[x]^2, reading
+    R22), which cancels 400:1 here; the bars of the other cases must still hold."""
+    _run_case(case, dtype, seed=3, shift=20.0, scale=1.0)
 
 
 @pytest.mark.parametrize("case", [(4, 64, 64, 320, 0, 32), (4, 64, 64, 320, 320, 32)])

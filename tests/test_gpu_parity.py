@@ -1,6 +1,13 @@
 """GPU parity: libpulse.so (through the C-ABI binding) vs the CPU oracle, element by
 element on the same seeded inputs.  Bars (BASELINE.json north_star): fp32 debug path
-max|err| <= 1e-4 * RMS(ref); bf16 max|err| <= 2e-2 * RMS(ref), per tensor."""
+max|err| <= 1e-4 * RMS(ref); bf16 max|err| <= 2e-2 * RMS(ref), per tensor.
+
+The bf16 bar is the PLAIN 2e-2 for every tensor except those named in tests/golden/bf16_floor.json (written by
+tests/golden/make_bf16_floor.py from the oracle alone): tensors for which the plain definition evaluated with bf16
+storage (oracle.stored_in) is itself more than 1e-2 away from the exact result.  Those
+may reach 2 x their storage floor (never more than CAP) and must then stay within 1.5 x the floor in rms.  A tensor that
+is not on the committed list and exceeds 2e-2 fails the test."""
+import json
 import os
 
 import numpy as np
@@ -34,16 +41,38 @@ def rms_err(got, ref):
 
 
 REPORT = os.environ.get("PULSE_PARITY_REPORT")
+with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "bf16_floor.json")) as _f:
+    GOLD = json.load(_f)
+CAP = 0.15          # no tensor may be further than this from the exact oracle, whatever its storage floor
 
 
-def run_gpu(desc, data, flags=0, with_g_e_out=False):
+def run_gpu(desc, data, flags=0, with_g_e_out=False, order=None, max_inflight=None):
+    """order: list of ("F", m) / ("B", m) events (default: one step, or the wave F0..F{M-1}, B{M-1}..B0)."""
     B = _binding()
-    st = B.Stage(desc, flags=flags)
+    st = B.Stage(desc, flags=flags, max_inflight=max_inflight)
     st.load_params(data["params"])
     M = desc["microbatches"]
     outs = []
     devs = [st.to_device(mb) for mb in data["microbatches"]]
-    if M == 1:
+    if order is not None:
+        fw, done, first = {}, {}, True
+        for ev, m in order:
+            if ev == "F":
+                emb, tst = st.temb_forward(devs[m]["t"])
+                fw[m] = (emb, tst) + st.forward(m, devs[m]["x_in"], devs[m].get("h_in"), emb)
+                assert st.cache_stats()["live_slots"] <= st.max_inflight
+            else:
+                emb, tst, e_out, d_out = fw.pop(m)
+                loss, g_d = st.mse(d_out, devs[m]["target"], 1.0 / M)
+                g_temb = torch.zeros_like(emb)
+                g_x_in, g_h_in = st.backward(m, g_d, devs[m].get("g_e_out"), True, g_temb, accumulate=not first)
+                st.temb_backward(g_temb, tst, accumulate=not first)
+                first = False
+                done[m] = {"loss": loss, "e_out": e_out, "d_out": d_out, "g_x_in": g_x_in, "g_h_in": g_h_in,
+                           "g_emb": g_temb, "emb": emb}
+        outs = [done[m] for m in range(M)]
+        assert st.cache_stats()["live_slots"] == 0
+    elif M == 1:
         r = st.step(0, devs[0], 1.0, accumulate=False)
         outs.append(r)
     else:       # wave: F0..F{M-1}, B{M-1}..B0 (configs[4])
@@ -98,52 +127,45 @@ def flatten(per_mb, grads):
     return out
 
 
-def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, floor=True):
-    """fp32: every tensor within tol (1e-4) of the exact oracle, north_star's metric.
-    bf16: north_star's bar (2e-2) where it is reachable, else the rounding floor of the bf16 protocol:
-    the oracle is run a second time with bf16 rounding at the method's store points
-    (oracle.stored_in); its own distance e_q to the exact oracle is what storing activations and
-    gradients in bf16 costs, and the CUDA path must stay within max(tol, 2 e_q) in max-abs and, where it uses
-    that allowance (max-abs above tol), within 1.5 x in rms (reading R18)."""
+def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, gold=None, order=None,
+          max_inflight=None):
+    """fp32: every tensor within 1e-4 of the exact oracle.  bf16: every tensor within the plain 2e-2, except the
+    tensors named in tests/golden/bf16_floor.json[gold] (see the module docstring)."""
     data = W.draw(desc, seed, with_g_e_out=with_g_e_out)
-    got_raw = run_gpu(desc, data, flags, with_g_e_out)
+    got_raw = run_gpu(desc, data, flags, with_g_e_out, order, max_inflight)
     got = flatten(got_raw["per_mb"], got_raw["param_grads"])
     ref = flatten(*oracle_run(desc, data, oracle_dtype))
     bf16 = desc["dtype"] == "bf16"
     tol = tol or TOL[desc["dtype"]]
-    refq = None
-    if bf16 and floor:
-        with O.stored_in(torch.bfloat16):
-            refq = flatten(*oracle_run(desc, data, oracle_dtype))
+    exc = {}
+    if bf16:
+        g = GOLD[gold or desc["name"]]              # KeyError: run tests/golden/make_bf16_floor.py for this structure
+        assert g["seed"] == seed and g["tensors"] == len(ref) and g["oracle_dtype"] == str(oracle_dtype).split(".")[1], g
+        exc = g["exceptions"]
     rows, bad = {}, []
     for k, r in ref.items():
-        if k not in got:
-            continue
         e, er = rel_err(got[k], r), rms_err(got[k], r)
-        row = {"max": e, "rms": er}
-        limit, rlimit = tol, None
-        if refq is not None:
-            row["floor_max"], row["floor_rms"] = rel_err(refq[k], r), rms_err(refq[k], r)
-            row["vs_q_max"] = rel_err(got[k], refq[k])
-            limit = max(tol, 2.0 * row["floor_max"])
+        row = {"max": e, "rms": er, "limit": tol}
+        rlimit = None
+        if k in exc:
+            fmax, frms = exc[k]
+            row.update(floor_max=fmax, floor_rms=frms, limit=min(max(tol, 2.0 * fmax), CAP))
             # the rms bound needs elements to average over: a scalar (the loss) has rms == max
-            rlimit = 1.5 * row["floor_rms"] + 1e-4 if r.numel() >= 1024 else None
-        row["limit"] = limit
+            rlimit = 1.5 * frms + 1e-4 if r.numel() >= 1024 else None
         rows[k] = row
-        # north_star's bar is the max bar: a tensor inside the plain tol has met it.  The rms bound guards the tensors
-        # that are admitted under the floor allowance (tol < e <= 2 x floor) against a systematic error hiding there.
-        if not (e <= limit) or (e > tol and rlimit is not None and not (er <= rlimit)):
+        # a listed tensor that uses its allowance (max above the plain bar) must not hide a systematic error there
+        if not (e <= row["limit"]) or (e > tol and rlimit is not None and not (er <= rlimit)):
             bad.append((k, row))
     top = sorted(rows.items(), key=lambda kv: -kv[1]["max"] / kv[1]["limit"])[:4]
     print(f"[parity] {desc['name']} flags={flags} tol={tol:g}: " +
           "; ".join(f"{k} max={v['max']:.2e} (limit {v['limit']:.2e}) rms={v['rms']:.2e}" for k, v in top), flush=True)
     n_plain = sum(1 for v in rows.values() if v["max"] <= tol)
-    print(f"[parity] {desc['name']}: {n_plain}/{len(rows)} tensors within north_star's plain {tol:g} bar", flush=True)
+    print(f"[parity] {desc['name']}: {n_plain}/{len(rows)} tensors within north_star's plain {tol:g} bar, "
+          f"{len(exc)} on the committed exception list", flush=True)
     if REPORT:
-        import json
         with open(REPORT, "a") as f:
             f.write(json.dumps({"config": desc["name"], "flags": flags, "tol": tol, "within_plain_tol": n_plain,
-                                "tensors": len(rows), "rows": rows}) + "\n")
+                                "tensors": len(rows), "listed": len(exc), "rows": rows}) + "\n")
     assert not bad, f"{desc['name']}: {len(bad)} tensors out of tolerance: {bad[:6]}"
     return got_raw
 
@@ -161,15 +183,27 @@ def test_config1_fp32():
 # ------------------------------------------------------------------ bf16, small shapes (CUDA-core convs)
 @pytest.mark.parametrize("kind", ["level", "updown", "unet", "wave"])
 def test_mini_bf16(kind):
-    # 8-16 channel, 4x4 tensors: reductions of 32-100 terms do not average bf16 store rounding, so these sit
-    # above 2e-2 and are bounded by the rounding floor instead (see check()).
+    # 8-16 channel, 4x4 tensors: reductions of 32-100 terms do not average bf16 store rounding, so most of their
+    # tensors are on the exception list (storage floor above 1e-2).
     check(W.mini(kind, "bf16"), seed=1, with_g_e_out=True)
 
 
 # ------------------------------------------------------------------ bf16, tensor-core shapes with ragged tiles
+@pytest.mark.parametrize("flags", [0, 4, 8], ids=["auto", "pair", "1cta"])
 @pytest.mark.parametrize("kind", ["level", "updown", "unet"])
-def test_mid_bf16(kind):
-    check(W.gpu_mid(kind), seed=2, with_g_e_out=(kind != "unet"))
+def test_mid_bf16(kind, flags):
+    """flags 4 / 8: every tcgen05 conv through the CTA-pair kernel (ragged pair tiles, odd tile counts, image boxes,
+    stride-2 phases, 1x1 on the concat, masked statistics epilogue) / through the single-CTA kernel."""
+    check(W.gpu_mid(kind), seed=2, flags=flags, with_g_e_out=(kind != "unet"))
+
+
+def test_mid_bf16_1f1b_order():
+    """Interleaved 1F1B order F0 F1 B0 F2 B1 B2 on two slots with weight-gradient accumulation: slot reuse (FIFO
+    release), transposed-weight reuse across the backwards of a step, shared gradient work buffers; against the
+    oracle's wave result (order-free: mean loss, summed weight gradients)."""
+    desc = W.scaled(W.gpu_mid("level"), microbatches=3, name="mid_level_1f1b")
+    order = [("F", 0), ("F", 1), ("B", 0), ("F", 2), ("B", 1), ("B", 2)]
+    check(desc, seed=4, order=order, max_inflight=2)
 
 
 @pytest.mark.parametrize("kind", ["level", "updown"])
@@ -183,7 +217,7 @@ def test_bf16_gn_two_pass_crosscheck(kind):
     """GroupNorm backward as reduction pass + apply pass (PULSE_FLAG_GN_TWO_PASS): the form that runs where a
     slice of an image does not fit a cluster's shared memory; the default runs cover the one-pass cluster kernel."""
     desc = W.mini("updown", "bf16") if kind == "mini_updown" else W.gpu_mid(kind[4:])
-    check(desc, seed=2, flags=2, with_g_e_out=(kind != "mid_unet"))
+    check(desc, seed=2, flags=2, with_g_e_out=(kind != "mid_unet"), gold="mini_updown@2" if kind == "mini_updown" else None)
 
 
 # ------------------------------------------------------------------ full configs
@@ -200,9 +234,10 @@ def test_config4_bf16():
     check(W.config(4), seed=0, oracle_dtype=torch.float32)
 
 
-@pytest.mark.skipif(os.environ.get("PULSE_BIG_WAVE") != "1", reason="config 5's full wave costs the oracle ~80 TFLOP; "
-                    "set PULSE_BIG_WAVE=1 (test_config5_wave_reduced covers the same path at 2 microbatches)")
+@pytest.mark.skipif(os.environ.get("PULSE_SKIP_BIG") == "1", reason="PULSE_SKIP_BIG=1")
 def test_config5_wave_full():
+    """configs[4] at full size: wave of 8 microbatches, all 8 skip sets resident; the float32 oracle
+    takes about a minute on the GPU box's host cores."""
     got = check(W.config(5), seed=0, oracle_dtype=torch.float32)
     assert got["stage"].cache_stats()["peak_bytes"] == 780 * 2 ** 20
 

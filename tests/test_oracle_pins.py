@@ -409,3 +409,19 @@ def test_float32_instantiation_matches_float64(kind):
         assert b[k].dtype == torch.float32, k
         rms = max(float(v.pow(2).mean().sqrt()), 1e-30)
         assert float((b[k].to(D) - v).abs().max()) <= 3e-5 * rms, (k, float((b[k].to(D) - v).abs().max()) / rms)
+
+
+def test_one_bf16_store_of_a_config2_tensor_is_at_the_bar():
+    """Why tests/golden/bf16_floor.json exists: north_star's bf16 bar is max|err| <= 2e-2 x RMS per
+    tensor.  ONE round-to-nearest bf16 store of an N(0,1) tensor of configs[1]'s size (4 x 320 x 64 x 64 = 5.2 M
+    elements, max |x| = 5.9 sigma) already has max|err| = 1.6e-2 x RMS: 2^-9..2^-8 relative at the largest element.
+    Two stores in series pass the bar; a stage output has 20-100 in series."""
+    g = torch.Generator().manual_seed(0)
+    x = torch.randn(4 * 320 * 64 * 64, generator=g, dtype=D)
+    rms = float(x.pow(2).mean().sqrt())
+    with O.stored_in(torch.bfloat16):
+        e1 = float((O.st(x) - x).abs().max()) / rms
+        y = O.st(O.st(x) * 1.3371) / 1.3371            # a second store after any operator that moves the grid
+        e2 = float((y - x).abs().max()) / rms
+    assert 1.4e-2 < e1 <= 2.0 ** -8 * float(x.abs().max()) / rms
+    assert e2 > 2e-2
