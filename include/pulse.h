@@ -47,7 +47,9 @@ typedef enum {
 } pulse_status_t;
 
 enum { PULSE_F32 = 0, PULSE_BF16 = 1 };
-enum { PULSE_OP_CONV_IN = 0, PULSE_OP_RESBLOCK = 1, PULSE_OP_DOWN = 2, PULSE_OP_UP = 3, PULSE_OP_HEAD = 4 };
+enum { PULSE_OP_CONV_IN = 0, PULSE_OP_RESBLOCK = 1, PULSE_OP_DOWN = 2, PULSE_OP_UP = 3, PULSE_OP_HEAD = 4,
+       PULSE_OP_ATTN = 5 /* self-attention block: GroupNorm -> 1x1 conv to q|k|v -> softmax(q k^T / sqrt(d)) v
+                            per head over the H W pixels -> 1x1 conv, + residual; cin == cout, heads | cin */ };
 enum { PULSE_LINK_OPEN = 0, PULSE_LINK_CLOSED = 1 };
 enum { PULSE_TEMB_SINUSOIDAL = 0, PULSE_TEMB_MLP = 1 };
 /* stage flags (cross-checks: same arithmetic, different kernel / summation order) */
@@ -56,7 +58,15 @@ enum {
   PULSE_FLAG_GN_TWO_PASS = 2,   /* GroupNorm backward always as reduction pass + apply pass (never the one-pass
                                    cluster kernel) */
   PULSE_FLAG_CONV_PAIR = 4,     /* tcgen05 convs: the CTA-pair kernel (conv_tc2_k) wherever it covers the shape */
-  PULSE_FLAG_CONV_1CTA = 8      /* tcgen05 convs: the single-CTA kernel (conv_tc_k) wherever it covers the shape */
+  PULSE_FLAG_CONV_1CTA = 8,     /* tcgen05 convs: the single-CTA kernel (conv_tc_k) wherever it covers the shape */
+  /* Upsample + conv (row a6).  Default: forward and input gradient through the materialised upsampled tensor, weight
+   * gradient in the 4-phase form (4/9 of the FLOPs, exact: it reads the original bf16 operands).  The 4-phase forward and
+   * input gradient need PRE-SUMMED bf16 weights, one extra rounding of the weights that costs as much as one more bf16
+   * store of the activations: faster (configs[2]: -5 %), but opt-in because tensors that sit just
+   * under north_star's 2e-2 bar then cross it. */
+  PULSE_FLAG_UP_MATERIALISED = 16, /* weight gradient through the materialised tensor too (the oracle's form everywhere) */
+  PULSE_FLAG_UP_PHASE_FWD = 32,    /* forward in the 4-phase form (no upsampled tensor is written) */
+  PULSE_FLAG_UP_PHASE_DGRAD = 64   /* input gradient in the 4-phase form (one 16-tap conv over the gradient's parity view) */
 };
 /* kernel selector of the single-operator conv calls */
 enum { PULSE_CONV_AUTO = 0, PULSE_CONV_SIMT = 1, PULSE_CONV_TC_PAIR = 2, PULSE_CONV_TC_1CTA = 3 };
@@ -77,6 +87,7 @@ typedef struct {
   int cin, cout;
   int skip_channels;  /* decoder ResBlock: channels of the skip it pops (LIFO); else 0 */
   int push_skip;      /* encoder op: 1 = its output goes to the skip cache */
+  int heads;          /* PULSE_OP_ATTN: number of heads (head h owns channels [h d, (h+1) d), d = cin / heads); else 0 */
 } pulse_op_desc;
 
 typedef struct {
@@ -105,7 +116,7 @@ pulse_status_t pulse_stage_destroy(pulse_stage_t* stage);
 /* Parameters, in the fixed order temb MLP (w1,b1,w2,b2), then per op of enc, mid, dec:
  * ResBlock: gn1.gamma gn1.beta conv1.w conv1.b temb.w temb.b gn2.gamma gn2.beta conv2.w
  * conv2.b [sc.w sc.b if cin+skip != cout]; conv_in/down/up: conv.w conv.b; head: gn.gamma
- * gn.beta conv.w conv.b.  name points into the handle (valid until destroy). */
+ * gn.beta conv.w conv.b; attention: gn.gamma gn.beta qkv.w [3c][1][1][c] qkv.b proj.w [c][1][1][c] proj.b.  name points into the handle (valid until destroy). */
 pulse_status_t pulse_stage_param_count(const pulse_stage_t* stage, int* count);
 pulse_status_t pulse_stage_param_info(const pulse_stage_t* stage, int index, const char** name, int* rank,
                                       int shape[4], size_t* offset_bytes, size_t* grad_offset_bytes);
@@ -211,6 +222,33 @@ pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const void* d_src0,
                                   int n, int h, int w, int ksize, int stride, const void* d_g, int cout,
                                   float* d_dw, void* stream);
 
+/* Nearest-2x upsample followed by a 3x3 pad-1 conv (row a6), computed WITHOUT the upsampled tensor:
+ * output pixel (2y+py, 2x+px) is a 2x2 conv of the low-resolution input with the pre-summed weights of its parity phase
+ * (4 taps on h x w pixels per phase instead of 9 taps on 2h x 2w: 4/9 of the FLOPs; the result equals
+ * conv3x3(upsample2(src)) up to the rounding of the pre-summed bf16 weights).  bf16 / tcgen05 only; kernel: PULSE_CONV_AUTO,
+ * _TC_PAIR or _TC_1CTA.  src [n,h,w,cin], w [cout][3][3][cin], out [n,2h,2w,cout].
+ * d_wp_scratch / d_wpt_scratch: 16*cout*cin elements of dtype (the pre-summed phase weights, written by the call).
+ * dgrad: g [n,2h,2w,cout] -> g_in [n,h,w,cin] (written).  wgrad: dw [cout][3][3][cin] fp32, accumulated. */
+pulse_status_t pulse_upsample_conv2d(int dtype, int kernel, const void* d_src, int n, int h, int w, int cin,
+                                     const void* d_w, int cout, const void* d_bias, void* d_wp_scratch, void* d_out,
+                                     float* d_chan_stats, void* stream);
+pulse_status_t pulse_upsample_conv2d_dgrad(int dtype, int kernel, const void* d_g, int n, int h, int w, int cin,
+                                           const void* d_w, int cout, void* d_wpt_scratch, void* d_g_in, void* stream);
+pulse_status_t pulse_upsample_conv2d_wgrad(int dtype, const void* d_src, int n, int h, int w, int cin, const void* d_g,
+                                           int cout, float* d_dw, void* stream);
+
+/* Scaled dot-product self-attention in isolation (the core of PULSE_OP_ATTN):
+ *   S = q k^T / sqrt(d), P = softmax over keys, o = P v, per (image, head), d = c / heads <= 128.
+ * d_qkv [n][tokens][3c]: q | k | v interleaved per token as the 1x1 conv leaves them (head h = channels [h d, (h+1) d)
+ * of each third); d_o, d_g_o [n][tokens][c]; d_g_qkv as d_qkv (written).  d_stats: pulse_attention_stats_floats(n,
+ * heads, tokens) fp32, written by the forward (log-sum-exp per query) and the backward, kept between the two.
+ * CUDA-core fp32 arithmetic on fp32 or bf16 storage; the T x T matrix is never written; no atomics. */
+size_t pulse_attention_stats_floats(int n, int heads, int tokens);
+pulse_status_t pulse_attention(int dtype, const void* d_qkv, int n, int tokens, int c, int heads, void* d_o, float* d_stats,
+                               void* stream);
+pulse_status_t pulse_attention_backward(int dtype, const void* d_qkv, const void* d_g_o, int n, int tokens, int c, int heads,
+                                        float* d_stats, void* d_g_qkv, void* stream);
+
 /* GroupNorm + SiLU in isolation (the kernels of rows a2/a5 and a8/a9), on
  * x = concat_C(x0[c0], x1[c1]) (x1 may be NULL with c1 = 0), NHWC, C = c0 + c1 divisible by groups
  * (a group may straddle the x0|x1 boundary):
@@ -244,6 +282,19 @@ pulse_status_t pulse_groupnorm_silu_backward(int dtype, int two_pass, int fwd_da
                                              float* d_scratch, const void* d_add, void* d_g_x0, int accumulate0,
                                              void* d_g_x1, int accumulate1, float* d_dgamma, float* d_dbeta,
                                              void* stream);
+
+/* ---- skip-aware balanced partitioning (host code, no device work) -------------------------
+ * PAPER.md:L140-L197 (sec. IV-B, Eq. 1-5, Alg. 1): cut the linear sequence of n_ops operations into p stages (p even;
+ * stage q and stage p-q+1 share a device) such that both ends of every skip connection (skip_src[s] < skip_dst[s],
+ * 1-based operation indices, |src - dst| > 1) lie in a collocated stage pair, minimising the slowest stage
+ *   max_m ( sum_{l in S_m} t_f[l] + lambda (t_lat + M_a / b_inter) ),
+ * M_a = act_bytes of the stage's last operation (encoder side) or of the operation before its first (decoder side),
+ * Eq. 2-3.  t_f, act_bytes: host arrays [n_ops] (act_bytes may be NULL when lambda == 0).
+ * cuts [p-1] (host, written): 1-based index of the last operation of stages 1 .. p-1; *bottleneck: the optimum.
+ * O(p n^3) time, O(p n^2) memory.  PULSE_ERR_SHAPE: no feasible partition / bad skip indices. */
+pulse_status_t pulse_partition(int n_ops, const double* t_f, const double* act_bytes, int n_skips, const int* skip_src,
+                               const int* skip_dst, int p, double lambda, double t_lat, double b_inter, int* cuts,
+                               double* bottleneck);
 
 /* ---- per-kernel-class timing (row d: measurement) -------------------------------------------
  * With profiling enabled, forward/backward bracket every kernel of these classes with CUDA events

@@ -118,6 +118,91 @@ def upsample2_bwd(g_u):
     return g_u.reshape(n, c, h // 2, 2, w // 2, 2).sum(dim=(3, 5))
 
 
+# --------------------------------------------------------------------------- attention
+
+def gn_fwd(x, gamma, beta, groups, eps):
+    """Plain GroupNorm (no activation): y = gamma xhat + beta, statistics as in gn_silu_fwd."""
+    n, c, h, w = x.shape
+    xg = x.reshape(n, groups, -1)
+    mu = xg.mean(dim=2, keepdim=True)
+    var = ((xg - mu) ** 2).mean(dim=2, keepdim=True)
+    r = 1.0 / torch.sqrt(var + eps)
+    xhat = ((xg - mu) * r).reshape(n, c, h, w)
+    return gamma.view(1, c, 1, 1) * xhat + beta.view(1, c, 1, 1), {"xhat": xhat, "r": r, "groups": groups}
+
+
+def gn_bwd(g_y, ctx, gamma):
+    """dgamma = sum g_y xhat; dbeta = sum g_y; q = g_y gamma; g_x = r (q - mean_S q - xhat mean_S (q xhat))."""
+    xhat, r, groups = ctx["xhat"], ctx["r"], ctx["groups"]
+    n, c, h, w = xhat.shape
+    dgamma = (g_y * xhat).sum(dim=(0, 2, 3))
+    dbeta = g_y.sum(dim=(0, 2, 3))
+    q = (g_y * gamma.view(1, c, 1, 1)).reshape(n, groups, -1)
+    xh = xhat.reshape(n, groups, -1)
+    g_x = (r * (q - q.mean(dim=2, keepdim=True) - xh * (q * xh).mean(dim=2, keepdim=True))).reshape(n, c, h, w)
+    return g_x, dgamma, dbeta
+
+
+def attn_core_fwd(q, k, v):
+    """Scaled dot-product attention, the plain definition: q, k, v [B, T, d] (B = samples x heads, T tokens);
+    S = q k^T / sqrt(d); P = softmax over keys (each row of P sums to 1); o = P v."""
+    d = q.shape[-1]
+    s = q @ k.transpose(1, 2) / math.sqrt(d)
+    p = torch.exp(s - s.max(dim=2, keepdim=True).values)
+    p = p / p.sum(dim=2, keepdim=True)
+    return p @ v, p
+
+
+def attn_core_bwd(g_o, q, k, v, p):
+    """g_v = P^T g_o; g_P = g_o v^T; g_S = P (g_P - rowsum(P g_P))  (softmax Jacobian); g_q = g_S k / sqrt(d);
+    g_k = g_S^T q / sqrt(d)."""
+    d = q.shape[-1]
+    g_v = p.transpose(1, 2) @ g_o
+    g_p = g_o @ v.transpose(1, 2)
+    g_s = p * (g_p - (p * g_p).sum(dim=2, keepdim=True))
+    return g_s @ k / math.sqrt(d), g_s.transpose(1, 2) @ q / math.sqrt(d), g_v
+
+
+def _heads(t, heads):
+    """[N, C, H, W] -> [N heads, H W, C / heads]: head h owns channels [h d, (h+1) d), tokens are pixels in row-major order."""
+    n, c, h, w = t.shape
+    return t.reshape(n, heads, c // heads, h * w).permute(0, 1, 3, 2).reshape(n * heads, h * w, c // heads)
+
+
+def _unheads(t, n, heads, h, w):
+    d = t.shape[-1]
+    return t.reshape(n, heads, h * w, d).permute(0, 1, 3, 2).reshape(n, heads * d, h, w)
+
+
+def attn_block_fwd(P, p, x, groups, eps, heads):
+    """Self-attention block of a UNet level ("Each block contains Attention and ResNet layers"; the inside
+    is not in the paper: reading R24, the SD form): xn = GN(x); [q|k|v] = conv1x1(xn) (C -> 3C); o = attention per head
+    over the H W pixels; out = x + conv1x1(o).  st() marks the stored tensors."""
+    n, c, h, w = x.shape
+    xn, cg = gn_fwd(x, P[p + "gn.gamma"], P[p + "gn.beta"], groups, eps)
+    xn = st(xn)
+    qkv = st(conv_fwd(xn, P[p + "qkv.w"], P[p + "qkv.b"]))
+    q, k, v = (_heads(qkv[:, i * c:(i + 1) * c], heads) for i in range(3))
+    o, pr = attn_core_fwd(q, k, v)
+    o = st(_unheads(o, n, heads, h, w))
+    out = st(conv_fwd(o, P[p + "proj.w"], P[p + "proj.b"]) + x)
+    return out, {"x": x, "xn": xn, "cg": cg, "qkv": qkv, "q": q, "k": k, "v": v, "p": pr, "o": o, "heads": heads}
+
+
+def attn_block_bwd(P, p, ctx, g_out, G):
+    """Chain rule of attn_block_fwd; adds parameter grads into G, returns g_x before it is stored."""
+    x, heads = ctx["x"], ctx["heads"]
+    n, c, h, w = x.shape
+    G[p + "proj.w"], G[p + "proj.b"] = conv_wgrad(ctx["o"], g_out, P[p + "proj.w"].shape)
+    g_o = st(conv_dgrad(g_out, P[p + "proj.w"], (h, w)))
+    g_q, g_k, g_v = attn_core_bwd(_heads(g_o, heads), ctx["q"], ctx["k"], ctx["v"], ctx["p"])
+    g_qkv = st(torch.cat([_unheads(t, n, heads, h, w) for t in (g_q, g_k, g_v)], dim=1))
+    G[p + "qkv.w"], G[p + "qkv.b"] = conv_wgrad(ctx["xn"], g_qkv, P[p + "qkv.w"].shape)
+    g_xn = st(conv_dgrad(g_qkv, P[p + "qkv.w"], (h, w)))
+    g_x, G[p + "gn.gamma"], G[p + "gn.beta"] = gn_bwd(g_xn, ctx["cg"], P[p + "gn.gamma"])
+    return g_x + g_out
+
+
 # --------------------------------------------------------------------------- time embedding
 
 def sinusoidal(t, d, dtype=DT):
@@ -242,6 +327,8 @@ def stage_forward(desc, P, x_in, h_in, emb):
         p = f"enc{i}."
         if op["kind"] == "resblock":
             x, c = resblock_fwd(P, p, x, emb, G_, eps)
+        elif op["kind"] == "attn":
+            x, c = attn_block_fwd(P, p, x, G_, eps, op["heads"])
         elif op["kind"] in ("conv_in", "down"):
             s = 2 if op["kind"] == "down" else 1
             c = {"x": x, "stride": s}
@@ -257,7 +344,10 @@ def stage_forward(desc, P, x_in, h_in, emb):
     if desc["link"] == "closed":
         h = x
         for i, op in enumerate(desc["mid_ops"]):
-            h, c = resblock_fwd(P, f"mid{i}.", h, emb, G_, eps)
+            if op["kind"] == "attn":
+                h, c = attn_block_fwd(P, f"mid{i}.", h, G_, eps, op["heads"])
+            else:
+                h, c = resblock_fwd(P, f"mid{i}.", h, emb, G_, eps)
             tape["mid"].append(c)
     else:
         outs["e_out"] = x
@@ -269,6 +359,8 @@ def stage_forward(desc, P, x_in, h_in, emb):
             assert s.shape[1] == op["skip"] and h.shape[1] == op["cin"], (p, s.shape, h.shape)
             h, c = resblock_fwd(P, p, torch.cat([h, s], dim=1), emb, G_, eps)
             c["pop"], c["ch"] = key, op["cin"]
+        elif op["kind"] == "attn":
+            h, c = attn_block_fwd(P, p, h, G_, eps, op["heads"])
         elif op["kind"] == "up":
             u = upsample2(h)
             c = {"u": u}
@@ -319,6 +411,8 @@ def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
             add_emb(ge)
             acc(kin, g_x[:, :c["ch"]])
             acc(c["pop"], g_x[:, c["ch"]:])
+        elif op["kind"] == "attn":
+            acc(kin, attn_block_bwd(P, p, c, g, G))
         elif op["kind"] == "up":
             G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["u"], g, P[p + "conv.w"].shape)
             acc(kin, upsample2_bwd(st(conv_dgrad(g, P[p + "conv.w"], c["u"].shape[2:]))))
@@ -330,8 +424,11 @@ def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
     grads_out = {}
     if closed:
         for i in reversed(range(n_mid)):
-            g_x, ge = resblock_bwd(P, f"mid{i}.", tape["mid"][i], gbuf[("m", i)], G)
-            add_emb(ge)
+            if desc["mid_ops"][i]["kind"] == "attn":
+                g_x = attn_block_bwd(P, f"mid{i}.", tape["mid"][i], gbuf[("m", i)], G)
+            else:
+                g_x, ge = resblock_bwd(P, f"mid{i}.", tape["mid"][i], gbuf[("m", i)], G)
+                add_emb(ge)
             acc(("m", i - 1) if i else last_enc, g_x)
     else:
         grads_out["g_h_in"] = gbuf[("hin",)]
@@ -344,6 +441,8 @@ def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
             g_x, ge = resblock_bwd(P, p, c, g, G)
             add_emb(ge)
             acc(("e", i - 1), g_x)
+        elif op["kind"] == "attn":
+            acc(("e", i - 1), attn_block_bwd(P, p, c, g, G))
         else:
             G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["x"], g, P[p + "conv.w"].shape, c["stride"])
             acc(("e", i - 1), conv_dgrad(g, P[p + "conv.w"], c["x"].shape[2:], c["stride"]))

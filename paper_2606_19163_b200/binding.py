@@ -19,16 +19,19 @@ if not os.path.exists(LIB_PATH):
 lib = C.CDLL(LIB_PATH)
 
 F32, BF16 = 0, 1
-OP_KIND = {"conv_in": 0, "resblock": 1, "down": 2, "up": 3, "head": 4}
+OP_KIND = {"conv_in": 0, "resblock": 1, "down": 2, "up": 3, "head": 4, "attn": 5}
 FLAG_FORCE_SIMT = 1
 FLAG_GN_TWO_PASS = 2
 FLAG_CONV_PAIR = 4
 FLAG_CONV_1CTA = 8
+FLAG_UP_MATERIALISED = 16
+FLAG_UP_PHASE_FWD = 32
+FLAG_UP_PHASE_DGRAD = 64
 
 
 class OpDesc(C.Structure):
     _fields_ = [("kind", C.c_int), ("cin", C.c_int), ("cout", C.c_int), ("skip_channels", C.c_int),
-                ("push_skip", C.c_int)]
+                ("push_skip", C.c_int), ("heads", C.c_int)]
 
 
 class StageDesc(C.Structure):
@@ -78,12 +81,19 @@ _SIG = {
                            _vp, _vp, C.c_int, _vp],
     "pulse_conv2d_wgrad": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                            _vp, C.c_int, _vp, _vp],
+    "pulse_upsample_conv2d": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp, _vp, _vp, _vp],
+    "pulse_upsample_conv2d_dgrad": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp, _vp],
+    "pulse_upsample_conv2d_wgrad": [C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp],
+    "pulse_attention": [C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp],
+    "pulse_attention_backward": [C.c_int, _vp, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp],
     "pulse_groupnorm_silu": [C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, _vp, _vp,
                              _vp, C.c_int, _vp, _vp],
     "pulse_groupnorm_silu_backward": [C.c_int, C.c_int, C.c_int, _vp, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int,
                                       C.c_int, C.c_float, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int, _vp, C.c_int, _vp, _vp,
                                       _vp],
 }
+_dp, _ip = C.POINTER(C.c_double), C.POINTER(C.c_int)
+_SIG["pulse_partition"] = [C.c_int, _dp, _dp, C.c_int, _ip, _ip, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _dp]
 for _name, _args in _SIG.items():
     _f = getattr(lib, _name)
     _f.argtypes = _args
@@ -94,7 +104,9 @@ lib.pulse_status_string.argtypes = [C.c_int]
 lib.pulse_last_error.restype = C.c_char_p
 lib.pulse_groupnorm_stats_floats.restype = _sz
 lib.pulse_groupnorm_stats_floats.argtypes = [C.c_int, C.c_int, C.c_int]
-EXPORTS = list(_SIG) + ["pulse_groupnorm_stats_floats", "pulse_version", "pulse_status_string", "pulse_last_error"]
+lib.pulse_attention_stats_floats.restype = _sz
+lib.pulse_attention_stats_floats.argtypes = [C.c_int, C.c_int, C.c_int]
+EXPORTS = list(_SIG) + ["pulse_groupnorm_stats_floats", "pulse_attention_stats_floats", "pulse_version", "pulse_status_string", "pulse_last_error"]
 
 
 class PulseError(RuntimeError):
@@ -121,7 +133,7 @@ def make_desc(desc: dict, max_inflight: int = 1, flags: int = 0):
     def ops(lst):
         arr = (OpDesc * max(1, len(lst)))()
         for i, o in enumerate(lst):
-            arr[i] = OpDesc(OP_KIND[o["kind"]], o["cin"], o["cout"], o["skip"], o["push"])
+            arr[i] = OpDesc(OP_KIND[o["kind"]], o["cin"], o["cout"], o["skip"], o["push"], o.get("heads", 0))
         return arr
     e, m, d = ops(desc["enc_ops"]), ops(desc["mid_ops"]), ops(desc["dec_ops"])
     sd = StageDesc(BF16 if desc["dtype"] == "bf16" else F32, desc["n"], desc["h"], desc["w"], desc["c_in"],
@@ -388,6 +400,53 @@ def conv2d_wgrad(src0, g, ksize, src1=None, stride=1, force_simt=False):
     return dw
 
 
+def upsample_conv2d(src, w, bias=None, kernel="auto", chan_stats=None):
+    """conv3x3(upsample2(src)) in the 4-phase form (no upsampled tensor)."""
+    n, h, wd, cin = src.shape
+    cout = w.shape[0]
+    out = torch.empty((n, 2 * h, 2 * wd, cout), dtype=src.dtype, device=src.device)
+    wp = torch.empty(16 * cout * cin, dtype=src.dtype, device=src.device)
+    _ck(lib.pulse_upsample_conv2d(_cd(src), CONV_KERNELS[kernel], _ptr(src), n, h, wd, cin, _ptr(w), cout, _ptr(bias),
+                                  _ptr(wp), _ptr(out), _ptr(chan_stats), _stream()))
+    return out
+
+
+def upsample_conv2d_dgrad(g, w, kernel="auto"):
+    n, h2, w2, cout = g.shape
+    cin = w.shape[3]
+    g_in = torch.empty((n, h2 // 2, w2 // 2, cin), dtype=g.dtype, device=g.device)
+    wpt = torch.empty(16 * cout * cin, dtype=g.dtype, device=g.device)
+    _ck(lib.pulse_upsample_conv2d_dgrad(_cd(g), CONV_KERNELS[kernel], _ptr(g), n, h2 // 2, w2 // 2, cin, _ptr(w), cout,
+                                        _ptr(wpt), _ptr(g_in), _stream()))
+    return g_in
+
+
+def upsample_conv2d_wgrad(src, g):
+    n, h, wd, cin = src.shape
+    cout = g.shape[3]
+    dw = torch.zeros((cout, 3, 3, cin), dtype=torch.float32, device=g.device)
+    _ck(lib.pulse_upsample_conv2d_wgrad(_cd(src), _ptr(src), n, h, wd, cin, _ptr(g), cout, _ptr(dw), _stream()))
+    return dw
+
+
+def attention(qkv, heads):
+    """qkv [n, tokens, 3c] -> (o [n, tokens, c], stats)."""
+    n, t, c3 = qkv.shape
+    c = c3 // 3
+    o = torch.empty((n, t, c), dtype=qkv.dtype, device=qkv.device)
+    stats = torch.empty(lib.pulse_attention_stats_floats(n, heads, t), dtype=torch.float32, device=qkv.device)
+    _ck(lib.pulse_attention(_cd(qkv), _ptr(qkv), n, t, c, heads, _ptr(o), _ptr(stats), _stream()))
+    return o, stats
+
+
+def attention_backward(qkv, g_o, heads, stats):
+    n, t, c3 = qkv.shape
+    g_qkv = torch.empty_like(qkv)
+    _ck(lib.pulse_attention_backward(_cd(qkv), _ptr(qkv), _ptr(g_o), n, t, c3 // 3, heads, _ptr(stats), _ptr(g_qkv),
+                                     _stream()))
+    return g_qkv
+
+
 def groupnorm_silu(x0, gamma, beta, groups, eps=1e-5, x1=None, stats=None):
     """a = SiLU(GroupNorm(concat_C(x0, x1))); returns (a, stats).  stats from an earlier call on the same x: only the
     normalise + SiLU pass runs."""
@@ -422,3 +481,19 @@ def groupnorm_silu_backward(g_a, x0, gamma, beta, groups, stats, eps=1e-5, x1=No
                                           eps, _ptr(gamma), _ptr(beta), _ptr(stats), _ptr(scratch), _ptr(add), _ptr(g_x0),
                                           int(acc0), _ptr(g_x1), int(acc1), _ptr(dgamma), _ptr(dbeta), _stream()))
     return g_x0, g_x1, dgamma, dbeta
+
+
+# ---- skip-aware partitioning (host only) ------------------------------------------------------------
+def partition(t_f, skips, p, act_bytes=None, lam=0.0, t_lat=0.0, b_inter=1.0):
+    """PAPER.md sec. IV-B: returns (cuts, bottleneck); cuts[m] = 1-based last operation of stage m + 1; skips = [(src, dst)]
+    1-based."""
+    n = len(t_f)
+    tf = (C.c_double * n)(*[float(v) for v in t_f])
+    ab = None if act_bytes is None else (C.c_double * n)(*[float(v) for v in act_bytes])
+    ns = len(skips)
+    ss = (C.c_int * max(1, ns))(*[int(a) for a, _ in skips])
+    sd = (C.c_int * max(1, ns))(*[int(b) for _, b in skips])
+    cuts = (C.c_int * max(1, p - 1))()
+    best = C.c_double()
+    _ck(lib.pulse_partition(n, tf, ab, ns, ss, sd, p, lam, t_lat, b_inter, cuts, C.byref(best)))
+    return list(cuts[:p - 1]), best.value

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpulse.so")
-SOURCES = ["stage.cu", "exec.cu", "norm.cu", "norm_fused.cu", "misc.cu", "conv_simt.cu", "conv_thin.cu", "conv_tc.cu", "conv_tc2.cu", "wgrad_tc2.cu"]
+SOURCES = ["stage.cu", "exec.cu", "norm.cu", "norm_fused.cu", "misc.cu", "conv_simt.cu", "conv_thin.cu", "conv_tc.cu", "conv_tc2.cu", "wgrad_tc2.cu", "attention.cu", "partition.cpp"]
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--use_fast_math",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -29,7 +29,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     procs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     for src in SOURCES:
-        obj = os.path.join(HERE, "build", src.replace(".cu", ".o"))
+        obj = os.path.join(HERE, "build", os.path.splitext(src)[0] + ".o")
         cmd = ["nvcc", *FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)

@@ -37,14 +37,15 @@ using namespace tmap;
 constexpr int BM = 128, BK = 64;
 constexpr int A_BYTES = BM * BK * 2;           // 16 KB
 
-struct TcParams {
-  int c0_blocks, c_blocks, ntaps, ctot, c0;
+struct TcParams {      // phases: see conv_tc2.cu
+  int c0_blocks, c_blocks, ctot, c0;
   int s2;                         // 1: stride-2 fprop through the 5-D parity view
-  Tap taps[9];
+  int nph, ph_tap0[5], ph_wrow[4], ph_ooy[4], ph_oox[4];
+  Tap taps[16];
   int bw, bh, bn, tiles_h, tiles_mn, n_tiles;
   int GH, GN;                     // pixel grid (rows, images); columns == bw
   const bf16* bias; const float* pn; const bf16* residual; bf16* out; int accumulate;
-  int OH, OW, osy, osx, ooy, oox, cout_total;
+  int OH, OW, osy, osx, cout_total;
 };
 
 template <int BN> struct Cfg {
@@ -65,8 +66,8 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
   __shared__ uint32_t tmem_base_s;
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int num_kb = p.ntaps * p.c_blocks;
-  const int total_tiles = p.tiles_mn * p.n_tiles;
+  const int tiles_ph = p.tiles_mn * p.n_tiles;      // tiles per phase
+  const int total_tiles = p.nph * tiles_ph;
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB);
@@ -85,11 +86,13 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
       // ===== TMA producer =====
       int stage = 0; uint32_t phase = 0;
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        const int mt = tile / p.n_tiles, nt = tile - mt * p.n_tiles;
+        const int ph = tile / tiles_ph, tl = tile - ph * tiles_ph;
+        const int mt = tl / p.n_tiles, nt = tl - mt * p.n_tiles;
         const int n0 = (mt / p.tiles_h) * p.bn, y0 = (mt % p.tiles_h) * p.bh;
+        const int tap0 = p.ph_tap0[ph], num_kb = (p.ph_tap0[ph + 1] - tap0) * p.c_blocks, wrow = p.ph_wrow[ph];
         for (int kb = 0; kb < num_kb; ++kb) {
           const int ti = kb / p.c_blocks, cb = kb - ti * p.c_blocks;
-          const Tap t = p.taps[ti];
+          const Tap t = p.taps[tap0 + ti];
           mbar_wait(&empty_bar[stage], phase ^ 1);
           mbar_expect_tx(&full_bar[stage], C::STAGE_BYTES);
           uint8_t* sa = smem + stage * C::STAGE_BYTES;
@@ -98,7 +101,7 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
           const int cch = (first ? cb : cb - p.c0_blocks) * BK;
           if (!p.s2) tma_load_4d(sa, ma, &full_bar[stage], cch, t.dx, y0 + t.dy, n0);
           else tma_load_5d(sa, ma, &full_bar[stage], t.px * p.c0 + cch, t.dx, t.py, y0 + t.dy, n0);
-          tma_load_2d(sa + A_BYTES, &mapB, &full_bar[stage], t.widx * p.ctot + cb * BK, nt * BN);
+          tma_load_2d(sa + A_BYTES, &mapB, &full_bar[stage], t.widx * p.ctot + cb * BK, wrow + nt * BN);
           if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -110,6 +113,8 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
       constexpr uint64_t dbase = smem_desc_sw128(16, 1024);
       int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        const int ph = tile / tiles_ph;
+        const int num_kb = (p.ph_tap0[ph + 1] - p.ph_tap0[ph]) * p.c_blocks;
         mbar_wait(&tempty_bar[acc], acc_phase ^ 1);
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + acc * BN;
@@ -137,10 +142,11 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
     const int y_l = rem / p.bw, x = rem - y_l * p.bw;
     int acc = 0; uint32_t acc_phase = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-      const int mt = tile / p.n_tiles, nt = tile - mt * p.n_tiles;
+      const int ph = tile / tiles_ph, tl = tile - ph * tiles_ph;
+      const int mt = tl / p.n_tiles, nt = tl - mt * p.n_tiles;
       const int n = (mt / p.tiles_h) * p.bn + n_l, y = (mt % p.tiles_h) * p.bh + y_l;
       const bool valid = n < p.GN && y < p.GH;
-      const size_t off = (((size_t)n * p.OH + (size_t)y * p.osy + p.ooy) * p.OW + (size_t)x * p.osx + p.oox) *
+      const size_t off = (((size_t)n * p.OH + (size_t)y * p.osy + p.ph_ooy[ph]) * p.OW + (size_t)x * p.osx + p.ph_oox[ph]) *
                              p.cout_total + (size_t)nt * BN;
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
@@ -334,6 +340,12 @@ bool act_map_c(const void* ptr, int n, int h, int w, int c, int cbox, int bw, in
   uint32_t box[4] = {(uint32_t)cbox, (uint32_t)bw, (uint32_t)bh, (uint32_t)bn};
   return get_map(ptr, 4, dims, str, box, out, 2 * cbox);
 }
+bool act_map_s2_c(const void* ptr, int n, int h, int w, int c, int cbox, int bw, int bh, int bn, CUtensorMap* out) {
+  uint64_t dims[5] = {(uint64_t)2 * c, (uint64_t)w / 2, 2, (uint64_t)h / 2, (uint64_t)n};
+  uint64_t str[4] = {(uint64_t)2 * c * 2, (uint64_t)w * c * 2, (uint64_t)2 * w * c * 2, (uint64_t)h * w * c * 2};
+  uint32_t box[5] = {(uint32_t)cbox, (uint32_t)bw, 1, (uint32_t)bh, (uint32_t)bn};
+  return get_map(ptr, 5, dims, str, box, out, 2 * cbox);
+}
 }  // namespace tmap
 
 namespace {
@@ -349,7 +361,7 @@ bool launch(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, 
     }
     attr_set = true;
   }
-  const int tiles = p.tiles_mn * p.n_tiles;
+  const int tiles = p.nph * p.tiles_mn * p.n_tiles;
   const int grid = tiles < sm_count() ? tiles : sm_count();
   conv_tc_k<BN><<<grid, 192, Cfg<BN>::SMEM, st>>>(a0, a1, b, p);
   return true;
@@ -365,7 +377,11 @@ bool conv_tc_supported(const ConvArgs& a) {
   if (!pick_bn(a.cout)) return false;
   if (a.ksize != 1 && a.ksize != 3) return false;
   int bw, bh, bn;
-  if (a.mode == CONV_DGRAD_S2) {
+  if (a.mode == CONV_UP2_DGRAD) {
+    if (a.ksize != 3 || a.src.c1 || (a.hin & 1) || (a.win & 1) || a.hout * 2 != a.hin || a.wout * 2 != a.win) return false;
+    return tile_geometry(a.hout, a.wout, bw, bh, bn);
+  }
+  if (a.mode == CONV_DGRAD_S2 || a.mode == CONV_UP2) {
     if (a.ksize != 3 || a.src.c1) return false;
     if (a.hout != 2 * a.hin || a.wout != 2 * a.win) return false;
     return tile_geometry(a.hin, a.win, bw, bh, bn);
@@ -382,8 +398,9 @@ int conv_tc(const ConvArgs& a, cudaStream_t st) {
   TcParams p;
   memset(&p, 0, sizeof p);
   const int bnn = pick_bn(a.cout);
-  const bool s2d = a.mode == CONV_DGRAD_S2, s2f = !s2d && a.stride == 2;
-  const int gh = s2d ? a.hin : a.hout, gw = s2d ? a.win : a.wout;
+  const bool s2d = a.mode == CONV_DGRAD_S2, up2 = a.mode == CONV_UP2, up2d = a.mode == CONV_UP2_DGRAD;
+  const bool s2f = up2d || (a.mode == CONV_FPROP && a.stride == 2);      // source read through the 5-D parity view
+  const int gh = (s2d || up2) ? a.hin : a.hout, gw = (s2d || up2) ? a.win : a.wout;
   tile_geometry(gh, gw, p.bw, p.bh, p.bn);
   p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64;
   p.s2 = s2f;
@@ -393,53 +410,65 @@ int conv_tc(const ConvArgs& a, cudaStream_t st) {
   p.GH = gh; p.GN = a.n;
   p.bias = (const bf16*)a.bias; p.pn = a.pn; p.residual = (const bf16*)a.residual; p.out = (bf16*)a.out;
   p.accumulate = a.accumulate;
-  p.OH = a.hout; p.OW = a.wout; p.osy = p.osx = 1; p.ooy = p.oox = 0; p.cout_total = a.cout;
   CUtensorMap m0, m1, mb;
   bool ok = true;
   if (s2f) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
   else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
   m1 = m0;
   if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
-  if (ok) ok = mat_map(a.w, a.cout, (uint64_t)a.ksize * a.ksize * p.ctot, bnn, &mb);
+  const uint64_t wk = (uint64_t)(up2 ? 4 : up2d ? 16 : a.ksize * a.ksize) * p.ctot;     // K of the weight matrix
+  if (ok) ok = mat_map(a.w, (uint64_t)(up2 ? 4 : 1) * a.cout, wk, bnn, &mb);
   if (!ok) return -1;
-  int launches = 0;
-  auto go = [&]() {
-    bool r = bnn == 160 ? launch<160>(m0, m1, mb, p, st) : launch<128>(m0, m1, mb, p, st);
-    if (r) ++launches;
-    return r;
+  // phases (see conv_tc2.cu): taps, weight rows and output parity of each sub-pixel conv of this launch
+  p.OH = a.hout; p.OW = a.wout; p.osy = p.osx = 1; p.cout_total = a.cout;
+  p.nph = 0; p.ph_tap0[0] = 0;
+  int ntaps = 0;
+  auto add_tap = [&](int dy, int dx, int py, int px, int widx) {
+    Tap t; t.dy = dy; t.dx = dx; t.py = py; t.px = px; t.widx = widx;
+    p.taps[ntaps++] = t;
   };
-  if (s2d) {
-    // output pixel (2y'+py, 2x'+px) <- taps r' with (py + r' - 1) even: py=0: r'=1 (dy 0); py=1: r'=0 (dy 0), r'=2 (dy +1)
+  auto end_phase = [&](int wrow, int ooy, int oox) {
+    p.ph_wrow[p.nph] = wrow; p.ph_ooy[p.nph] = ooy; p.ph_oox[p.nph] = oox;
+    p.ph_tap0[++p.nph] = ntaps;
+  };
+  if (up2) {
     p.osy = p.osx = 2;
-    for (int py = 0; py < 2; ++py)
-      for (int px = 0; px < 2; ++px) {
-        p.ooy = py; p.oox = px; p.ntaps = 0;
-        for (int r = 0; r < 3; ++r) {
-          if ((py + r - 1) & 1) continue;
-          for (int s = 0; s < 3; ++s) {
-            if ((px + s - 1) & 1) continue;
-            Tap t; t.dy = (py + r - 1) >> 1; t.dx = (px + s - 1) >> 1; t.px = t.py = 0; t.widx = r * 3 + s;
-            p.taps[p.ntaps++] = t;
-          }
-        }
-        if (!go()) return -1;
-      }
-    return launches;
-  }
-  const int pad = (a.ksize - 1) / 2;
-  p.ntaps = a.ksize * a.ksize;
-  for (int r = 0; r < a.ksize; ++r)
-    for (int s = 0; s < a.ksize; ++s) {
-      Tap t; t.widx = r * a.ksize + s; t.px = t.py = 0;
-      if (!s2f) { t.dy = r - pad; t.dx = s - pad; }
-      else {   // input row 2y + r - 1 = 2(y + dy) + py
-        t.dy = r == 0 ? -1 : 0; t.py = r == 1 ? 0 : 1;
-        t.dx = s == 0 ? -1 : 0; t.px = s == 1 ? 0 : 1;
-      }
-      p.taps[t.widx] = t;
+    for (int ph = 0; ph < 4; ++ph) {
+      const int py = ph >> 1, px = ph & 1;
+      for (int t = 0; t < 4; ++t) add_tap((t >> 1) - 1 + py, (t & 1) - 1 + px, 0, 0, t);
+      end_phase(ph * a.cout, py, px);
     }
-  if (!go()) return -1;
-  return launches;
+  } else if (up2d) {
+    for (int q = 0; q < 16; ++q) {
+      const int py = q >> 3, px = (q >> 2) & 1, ta = (q >> 1) & 1, tb = q & 1;
+      add_tap(1 - ta - py, 1 - tb - px, py, px, q);
+    }
+    end_phase(0, 0, 0);
+  } else if (s2d) {
+    p.osy = p.osx = 2;
+    const int order[4][2] = {{1, 1}, {1, 0}, {0, 1}, {0, 0}};
+    for (int o = 0; o < 4; ++o) {
+      const int py = order[o][0], px = order[o][1];
+      for (int r = 0; r < 3; ++r) {
+        if ((py + r - 1) & 1) continue;
+        for (int s_ = 0; s_ < 3; ++s_) {
+          if ((px + s_ - 1) & 1) continue;
+          add_tap((py + r - 1) >> 1, (px + s_ - 1) >> 1, 0, 0, r * 3 + s_);
+        }
+      }
+      end_phase(0, py, px);
+    }
+  } else {
+    const int pad = (a.ksize - 1) / 2;
+    for (int r = 0; r < a.ksize; ++r)
+      for (int s_ = 0; s_ < a.ksize; ++s_) {
+        if (!s2f) add_tap(r - pad, s_ - pad, 0, 0, r * a.ksize + s_);
+        else add_tap(r == 0 ? -1 : 0, s_ == 0 ? -1 : 0, r == 1 ? 0 : 1, s_ == 1 ? 0 : 1, r * a.ksize + s_);
+      }
+    end_phase(0, 0, 0);
+  }
+  const bool r = bnn == 160 ? launch<160>(m0, m1, mb, p, st) : launch<128>(m0, m1, mb, p, st);
+  return r ? 1 : -1;
 }
 
 // ================================================================================ wgrad
@@ -603,7 +632,7 @@ wgrad_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
 }  // namespace
 
 bool wgrad_tc_supported(const WgradArgs& a) {
-  if (a.dt != DT_BF16) return false;
+  if (a.dt != DT_BF16 || a.up2) return false;
   if (a.src.c0 % 64 || a.src.c1 % 64 || a.src.c0 == 0 || a.cout % WG_N) return false;
   if (a.ksize != 1 && a.ksize != 3) return false;
   if (a.stride == 2) {

@@ -37,16 +37,21 @@ using namespace tmap;
 constexpr int BM = 128, BK = 64;
 constexpr int A_BYTES = BM * BK * 2;           // 16 KB
 
+// A launch covers 1 or 4 PHASES (stride-2 dgrad, 4-phase upsample conv): sub-pixel convs that share the source, the
+// pixel grid and the weight matrix's K layout but have their own taps, weight rows and output parity.  Phases are extra
+// tiles of one persistent launch, so small grids still fill the machine.
 struct Tc2Params {
-  int c0_blocks, c_blocks, ntaps, ctot, c0;
+  int c0_blocks, c_blocks, ctot, c0;
   int s2;                         // 1: stride-2 fprop through the 5-D parity view
-  Tap taps[9];
+  int nph, ph_tap0[5], ph_wrow[4], ph_ooy[4], ph_oox[4];      // phase i: taps [ph_tap0[i], ph_tap0[i+1]), first weight row, output parity
+  Tap taps[16];
   int bw, bh, bn, tiles_h, tiles_m, pair_tiles_m, n_tiles;
   int GH, GN;                     // pixel grid (rows, images); columns == bw
   const bf16* bias; const float* pn; const bf16* residual; bf16* out; int accumulate;
-  int OH, OW, osy, osx, ooy, oox, cout_total;
+  int OH, OW, osy, osx, cout_total;
   float* cst;                     // channel stats [n][2][cout] of the stored output, accumulated (or null)
 };
+struct OutMaps { CUtensorMap m[4]; };      // one output view per phase
 
 template <int UN, int NJ> struct Cfg2 {
   static constexpr int BN = UN * NJ;                       // output channels per pair tile
@@ -68,7 +73,7 @@ template <int UN, int NJ> struct Cfg2 {
 template <int UN, int NJ>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
 conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
-           const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CUtensorMap mapO, const Tc2Params p) {
+           const __grid_constant__ CUtensorMap mapB, const __grid_constant__ OutMaps mapO, const Tc2Params p) {
   using C = Cfg2<UN, NJ>;
   extern __shared__ uint8_t smem_raw[];
   __shared__ uint64_t full_bar[C::STAGES], empty_bar[C::STAGES], tfull_bar[2], tempty_bar[2];
@@ -76,12 +81,12 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
-  const int num_kb = p.ntaps * p.c_blocks;
-  const int total_tiles = p.pair_tiles_m * p.n_tiles;
+  const int tiles_ph = p.pair_tiles_m * p.n_tiles;      // tiles per phase
+  const int total_tiles = p.nph * tiles_ph;
   const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
 
   if (warp == 0 && lane == 0) {
-    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB); prefetch_tmap(&mapO);
+    prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB); prefetch_tmap(&mapO.m[0]);
     for (int i = 0; i < C::STAGES; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(&tfull_bar[i], 1); mbar_init(&tempty_bar[i], 16); }
     fence_barrier_init();
@@ -99,12 +104,14 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       // ===== TMA producer (both CTAs): own 128 pixel rows of A, own half of every weight slice =====
       int stage = 0; uint32_t phase = 0;
       for (int tile = pair; tile < total_tiles; tile += npairs) {
-        const int mp = tile / p.n_tiles, nt = tile - mp * p.n_tiles;
+        const int ph = tile / tiles_ph, tl = tile - ph * tiles_ph;
+        const int mp = tl / p.n_tiles, nt = tl - mp * p.n_tiles;
         const int mt = 2 * mp + (int)rank;
         const int n0 = (mt / p.tiles_h) * p.bn, y0 = (mt % p.tiles_h) * p.bh;
+        const int tap0 = p.ph_tap0[ph], num_kb = (p.ph_tap0[ph + 1] - tap0) * p.c_blocks, wrow = p.ph_wrow[ph];
         for (int kb = 0; kb < num_kb; ++kb) {
           const int ti = kb / p.c_blocks, cb = kb - ti * p.c_blocks;
-          const Tap t = p.taps[ti];
+          const Tap t = p.taps[tap0 + ti];
           mbar_wait(&empty_bar[stage], phase ^ 1);
           if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * C::STAGE_BYTES);
           const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
@@ -117,7 +124,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           const int kcol = t.widx * p.ctot + cb * BK;
 #pragma unroll
           for (int j = 0; j < NJ; ++j)
-            tma2_load_2d(sa + A_BYTES + j * C::B_SLICE, &mapB, fb, kcol, nt * C::BN + j * UN + (int)rank * (UN / 2));
+            tma2_load_2d(sa + A_BYTES + j * C::B_SLICE, &mapB, fb, kcol, wrow + nt * C::BN + j * UN + (int)rank * (UN / 2));
           if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -131,6 +138,8 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       const uint32_t desc_lo0 = (uint32_t)dbase | ((smem_u32(smem) >> 4) & 0x3FFF);     // smem is 1024-aligned: no carry
       int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
       for (int tile = pair; tile < total_tiles; tile += npairs) {
+        const int ph = tile / tiles_ph;
+        const int num_kb = (p.ph_tap0[ph + 1] - p.ph_tap0[ph]) * p.c_blocks;
         mbar_wait(&tempty_bar[acc], acc_phase ^ 1);
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + acc * C::BN;
@@ -178,12 +187,13 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
     int acc = 0; uint32_t acc_phase = 0;
     int buf = 0;
     for (int tile = pair; tile < total_tiles; tile += npairs) {
-      const int mp = tile / p.n_tiles, nt = tile - mp * p.n_tiles;
+      const int ph = tile / tiles_ph, tl = tile - ph * tiles_ph;
+      const int mp = tl / p.n_tiles, nt = tl - mp * p.n_tiles;
       const int mt = 2 * mp + (int)rank;
       const int n_t = (mt / p.tiles_h) * p.bn, y_t = (mt % p.tiles_h) * p.bh;
       const int n = n_t + n_l, y = y_t + y_l;
       const bool valid = mt < p.tiles_m && n < p.GN && y < p.GH;
-      const size_t off = (((size_t)n * p.OH + (size_t)y * p.osy + p.ooy) * p.OW + (size_t)x * p.osx + p.oox) *
+      const size_t off = (((size_t)n * p.OH + (size_t)y * p.osy + p.ph_ooy[ph]) * p.OW + (size_t)x * p.osx + p.ph_oox[ph]) *
                              p.cout_total + (size_t)nt * C::BN;
       const bf16* addend = p.residual ? p.residual : (p.accumulate ? p.out : nullptr);
       const unsigned vmask = __ballot_sync(0xffffffffu, valid);
@@ -245,7 +255,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            tma_store_4d(&mapO, stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
+            tma_store_4d(&mapO.m[ph], stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
             bulk_commit();
           }
           static_assert(CW == 32, "the statistics pass reads 16 words per staged row");
@@ -304,7 +314,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
 }
 
 template <int UN, int NJ>
-bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const CUtensorMap& o, const Tc2Params& p,
+bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const OutMaps& o, const Tc2Params& p,
              cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
@@ -315,7 +325,7 @@ bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b,
     }
     attr_set = true;
   }
-  const int tiles = p.pair_tiles_m * p.n_tiles;
+  const int tiles = p.nph * p.pair_tiles_m * p.n_tiles;
   const int max_pairs = sm_count() / 2;
   const int pairs = tiles < max_pairs ? tiles : max_pairs;
   launch_pdl(conv_tc2_k<UN, NJ>, dim3(2 * pairs), dim3(320), Cfg2<UN, NJ>::SMEM, st, a0, a1, b, o, p);
@@ -341,7 +351,11 @@ bool conv_tc2_supported(const ConvArgs& a) {
   if (!un) return false;
   if (a.ksize != 1 && a.ksize != 3) return false;
   int bw, bh, bn;
-  if (a.mode == CONV_DGRAD_S2) {
+  if (a.mode == CONV_UP2_DGRAD) {
+    if (a.ksize != 3 || a.src.c1 || (a.hin & 1) || (a.win & 1) || a.hout * 2 != a.hin || a.wout * 2 != a.win) return false;
+    return tile_geometry(a.hout, a.wout, bw, bh, bn) && bw * bh >= 32;
+  }
+  if (a.mode == CONV_DGRAD_S2 || a.mode == CONV_UP2) {
     if (a.ksize != 3 || a.src.c1) return false;
     if (a.hout != 2 * a.hin || a.wout != 2 * a.win) return false;
     return tile_geometry(a.hin, a.win, bw, bh, bn) && bw * bh >= 32;
@@ -359,8 +373,9 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
   memset(&p, 0, sizeof p);
   int un, nj;
   pick_tile(a.cout, un, nj);
-  const bool s2d = a.mode == CONV_DGRAD_S2, s2f = !s2d && a.stride == 2;
-  const int gh = s2d ? a.hin : a.hout, gw = s2d ? a.win : a.wout;
+  const bool s2d = a.mode == CONV_DGRAD_S2, up2 = a.mode == CONV_UP2, up2d = a.mode == CONV_UP2_DGRAD;
+  const bool s2f = up2d || (a.mode == CONV_FPROP && a.stride == 2);      // source read through the 5-D parity view
+  const int gh = (s2d || up2) ? a.hin : a.hout, gw = (s2d || up2) ? a.win : a.wout;
   tile_geometry(gh, gw, p.bw, p.bh, p.bn);
   p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64;
   p.s2 = s2f;
@@ -372,67 +387,85 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
   p.bias = (const bf16*)a.bias; p.pn = a.pn; p.residual = (const bf16*)a.residual; p.out = (bf16*)a.out;
   p.accumulate = a.accumulate;
   p.cst = a.cst;
-  p.OH = a.hout; p.OW = a.wout; p.osy = p.osx = 1; p.ooy = p.oox = 0; p.cout_total = a.cout;
   CUtensorMap m0, m1, mb;
   bool ok = true;
   if (s2f) ok = act_map_s2(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
   else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
   m1 = m0;
   if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
-  if (ok) ok = mat_map(a.w, a.cout, (uint64_t)a.ksize * a.ksize * p.ctot, un / 2, &mb);
+  const uint64_t wk = (uint64_t)(up2 ? 4 : up2d ? 16 : a.ksize * a.ksize) * p.ctot;     // K of the weight matrix
+  if (ok) ok = mat_map(a.w, (uint64_t)(up2 ? 4 : 1) * a.cout, wk, un / 2, &mb);
   if (!ok) return -1;
-  int launches = 0;
-  auto go = [&]() {
-    // output view of this launch: (c, x, y, n) with pixel strides osx/osy from pixel (ooy, oox); box = one warp's
-    // [32 pixels][32 channels], 64-byte swizzle
-    CUtensorMap mo;
-    {
-      const int bwb = p.bw < 32 ? p.bw : 32, bhb = 32 / bwb;
-      const size_t C2 = (size_t)a.cout * 2;
-      uint64_t dims[4] = {(uint64_t)a.cout, (uint64_t)gw, (uint64_t)gh, (uint64_t)a.n};
-      uint64_t str[3] = {(uint64_t)p.osx * C2, (uint64_t)p.osy * a.wout * C2, (uint64_t)a.hout * a.wout * C2};
-      const uint32_t cw = 32;        // Cfg2::CW
-      uint32_t box[4] = {cw, (uint32_t)bwb, (uint32_t)bhb, 1};
-      const char* base = (const char*)a.out + ((size_t)p.ooy * a.wout + p.oox) * C2;
-      if (!get_map(base, 4, dims, str, box, &mo, 2 * (int)cw)) return false;
-    }
-    bool r = un == 160 ? (nj == 2 ? launch2<160, 2>(m0, m1, mb, mo, p, st) : launch2<160, 1>(m0, m1, mb, mo, p, st))
-                       : (nj == 2 ? launch2<128, 2>(m0, m1, mb, mo, p, st) : launch2<128, 1>(m0, m1, mb, mo, p, st));
-    if (r) ++launches;
-    return r;
+  // phases: taps, weight rows and output parity of each sub-pixel conv of this launch (one phase for a plain conv)
+  p.OH = a.hout; p.OW = a.wout; p.osy = p.osx = 1; p.cout_total = a.cout;
+  p.nph = 0; p.ph_tap0[0] = 0;
+  int ntaps = 0;
+  auto add_tap = [&](int dy, int dx, int py, int px, int widx) {
+    Tap t; t.dy = dy; t.dx = dx; t.py = py; t.px = px; t.widx = widx;
+    p.taps[ntaps++] = t;
   };
-  if (s2d) {
-    // output pixel (2y'+py, 2x'+px) <- taps r' with (py + r' - 1) even: py=0: r'=1 (dy 0); py=1: r'=0 (dy 0), r'=2 (dy +1)
+  auto end_phase = [&](int wrow, int ooy, int oox) {
+    p.ph_wrow[p.nph] = wrow; p.ph_ooy[p.nph] = ooy; p.ph_oox[p.nph] = oox;
+    p.ph_tap0[++p.nph] = ntaps;
+  };
+  if (up2) {
+    // output pixel (2y+py, 2x+px) <- low-resolution pixels (y+dy, x+dx), dy = a-1+py, dx = b-1+px, through the pre-summed
+    // weights Wp[phase] (kernels.h): rows [phase cout, (phase + 1) cout) of one [4 cout][4 c] matrix
     p.osy = p.osx = 2;
-    for (int py = 0; py < 2; ++py)
-      for (int px = 0; px < 2; ++px) {
-        p.ooy = py; p.oox = px; p.ntaps = 0;
-        for (int r = 0; r < 3; ++r) {
-          if ((py + r - 1) & 1) continue;
-          for (int s = 0; s < 3; ++s) {
-            if ((px + s - 1) & 1) continue;
-            Tap t; t.dy = (py + r - 1) >> 1; t.dx = (px + s - 1) >> 1; t.px = t.py = 0; t.widx = r * 3 + s;
-            p.taps[p.ntaps++] = t;
-          }
-        }
-        if (!go()) return -1;
-      }
-    return launches;
-  }
-  const int pad = (a.ksize - 1) / 2;
-  p.ntaps = a.ksize * a.ksize;
-  for (int r = 0; r < a.ksize; ++r)
-    for (int s = 0; s < a.ksize; ++s) {
-      Tap t; t.widx = r * a.ksize + s; t.px = t.py = 0;
-      if (!s2f) { t.dy = r - pad; t.dx = s - pad; }
-      else {   // input row 2y + r - 1 = 2(y + dy) + py
-        t.dy = r == 0 ? -1 : 0; t.py = r == 1 ? 0 : 1;
-        t.dx = s == 0 ? -1 : 0; t.px = s == 1 ? 0 : 1;
-      }
-      p.taps[t.widx] = t;
+    for (int ph = 0; ph < 4; ++ph) {
+      const int py = ph >> 1, px = ph & 1;
+      for (int t = 0; t < 4; ++t) add_tap((t >> 1) - 1 + py, (t & 1) - 1 + px, 0, 0, t);
+      end_phase(ph * a.cout, py, px);
     }
-  if (!go()) return -1;
-  return launches;
+  } else if (up2d) {
+    // g_in(y, x) = sum over (phase, tap) of WpT[..][q] g(2 (y - dy) + py, 2 (x - dx) + px): 16 taps on the parity view
+    for (int q = 0; q < 16; ++q) {
+      const int py = q >> 3, px = (q >> 2) & 1, ta = (q >> 1) & 1, tb = q & 1;
+      add_tap(1 - ta - py, 1 - tb - px, py, px, q);
+    }
+    end_phase(0, 0, 0);
+  } else if (s2d) {
+    // output pixel (2y'+py, 2x'+px) <- taps r' with (py + r' - 1) even: py=0: r'=1 (dy 0); py=1: r'=0 (dy 0), r'=2 (dy +1).
+    // Phases in order of decreasing tap count (4, 2, 2, 1): the round-robin tile walk then mixes long and short tiles
+    p.osy = p.osx = 2;
+    const int order[4][2] = {{1, 1}, {1, 0}, {0, 1}, {0, 0}};
+    for (int o = 0; o < 4; ++o) {
+      const int py = order[o][0], px = order[o][1];
+      for (int r = 0; r < 3; ++r) {
+        if ((py + r - 1) & 1) continue;
+        for (int s_ = 0; s_ < 3; ++s_) {
+          if ((px + s_ - 1) & 1) continue;
+          add_tap((py + r - 1) >> 1, (px + s_ - 1) >> 1, 0, 0, r * 3 + s_);
+        }
+      }
+      end_phase(0, py, px);
+    }
+  } else {
+    const int pad = (a.ksize - 1) / 2;
+    for (int r = 0; r < a.ksize; ++r)
+      for (int s_ = 0; s_ < a.ksize; ++s_) {
+        if (!s2f) add_tap(r - pad, s_ - pad, 0, 0, r * a.ksize + s_);
+        else add_tap(r == 0 ? -1 : 0, s_ == 0 ? -1 : 0, r == 1 ? 0 : 1, s_ == 1 ? 0 : 1, r * a.ksize + s_);   // input row 2y + r - 1 = 2(y + dy) + py
+      }
+    end_phase(0, 0, 0);
+  }
+  // output view of each phase: (c, x, y, n) with pixel strides osx/osy from pixel (ooy, oox); box = one warp's
+  // [32 pixels][32 channels], 64-byte swizzle
+  OutMaps mo;
+  for (int ph = 0; ph < 4; ++ph) {
+    const int q = ph < p.nph ? ph : 0;
+    const int bwb = p.bw < 32 ? p.bw : 32, bhb = 32 / bwb;
+    const size_t C2 = (size_t)a.cout * 2;
+    uint64_t dims[4] = {(uint64_t)a.cout, (uint64_t)gw, (uint64_t)gh, (uint64_t)a.n};
+    uint64_t str[3] = {(uint64_t)p.osx * C2, (uint64_t)p.osy * a.wout * C2, (uint64_t)a.hout * a.wout * C2};
+    const uint32_t cw = 32;        // Cfg2::CW
+    uint32_t box[4] = {cw, (uint32_t)bwb, (uint32_t)bhb, 1};
+    const char* base = (const char*)a.out + ((size_t)p.ph_ooy[q] * a.wout + p.ph_oox[q]) * C2;
+    if (!get_map(base, 4, dims, str, box, &mo.m[ph], 2 * (int)cw)) return -1;
+  }
+  const bool r = un == 160 ? (nj == 2 ? launch2<160, 2>(m0, m1, mb, mo, p, st) : launch2<160, 1>(m0, m1, mb, mo, p, st))
+                           : (nj == 2 ? launch2<128, 2>(m0, m1, mb, mo, p, st) : launch2<128, 1>(m0, m1, mb, mo, p, st));
+  return r ? 1 : -1;
 }
 
 // Few output tiles (deep UNet levels: 1280 channels on 8 x 8 or 16 x 16 pixels give 8 / 32 pair tiles for 74 CTA
@@ -443,11 +476,11 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
 static int one_cta_tile_bound() { return toggles().conv_1cta_tiles >= 0 ? toggles().conv_1cta_tiles : sm_count(); }
 static bool prefer_1cta(const ConvArgs& a) {
   if (!conv_tc_supported(a)) return false;
-  const bool s2d = a.mode == CONV_DGRAD_S2;
+  const bool s2d = a.mode == CONV_DGRAD_S2 || a.mode == CONV_UP2;      // pixel grid = the low-resolution side
   int bw, bh, bn;
   if (!tile_geometry(s2d ? a.hin : a.hout, s2d ? a.win : a.wout, bw, bh, bn)) return false;
   const int gh = s2d ? a.hin : a.hout;
-  const long long tiles_m = (long long)((gh + bh - 1) / bh) * ((a.n + bn - 1) / bn);
+  const long long tiles_m = (long long)((gh + bh - 1) / bh) * ((a.n + bn - 1) / bn) * (s2d ? 4 : 1);      // 4 phases per launch
   const long long tiles = tiles_m * (a.cout / (a.cout % 160 == 0 ? 160 : 128));      // its N tiles are 160 (or 128) wide
   return tiles <= one_cta_tile_bound();
 }
@@ -458,7 +491,7 @@ static bool use_pair(const ConvArgs& a) {
   if (a.kernel == CONV_K_1CTA || toggles().conv_1cta) return false;
   return !prefer_1cta(a);
 }
-bool conv_emits_stats(const ConvArgs& a) { return use_pair(a) && a.mode == CONV_FPROP && !a.accumulate; }
+bool conv_emits_stats(const ConvArgs& a) { return use_pair(a) && (a.mode == CONV_FPROP || a.mode == CONV_UP2) && !a.accumulate; }
 bool conv_tc_any_supported(const ConvArgs& a) {
   if (a.kernel == CONV_K_PAIR) return conv_tc2_supported(a);
   if (a.kernel == CONV_K_1CTA) return conv_tc_supported(a);

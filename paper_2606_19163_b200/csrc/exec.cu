@@ -111,7 +111,9 @@ struct Prof {
   }
 };
 
-double conv_flops(const ConvArgs& a) {
+double conv_flops(const ConvArgs& a) {      // EXECUTED flops
+  if (a.mode == CONV_UP2) return 2.0 * a.n * a.hin * a.win * a.cout * a.src.c() * 16;          // 4 phases x 4 taps on the low-res grid
+  if (a.mode == CONV_UP2_DGRAD) return 2.0 * a.n * a.hout * a.wout * a.cout * a.src.c() * 16;
   const double mpix = a.mode == CONV_DGRAD_S2 ? (double)a.n * a.hin * a.win : (double)a.n * a.hout * a.wout;
   return 2.0 * mpix * a.cout * a.src.c() * a.ksize * a.ksize;     // the s2 dgrad phases execute exactly 9/4 taps per output
 }
@@ -137,7 +139,8 @@ void run_conv(Ctx& c, ConvArgs a, int stats_t = -1) {
 void run_wgrad(Ctx& c, const WgradArgs& a) {
   const bool tc = c.tc() && wgrad_tc_any_supported(a);
   Prof pr(c.s, c.wst(), tc ? PULSE_KCLASS_WGRAD_TC : PULSE_KCLASS_CONV_SIMT,
-          2.0 * a.n * a.hout * a.wout * a.cout * a.src.c() * a.ksize * a.ksize, 0.0);
+          a.up2 ? 2.0 * a.n * a.hin * a.win * a.cout * a.src.c() * 16
+                : 2.0 * a.n * a.hout * a.wout * a.cout * a.src.c() * a.ksize * a.ksize, 0.0);
   const int r = tc ? wgrad_tc_any(a, c.wst()) : wgrad_simt(a, c.wst());
   if (r < 0) c.err = true; else c.s->launches += r;
 }
@@ -156,20 +159,21 @@ void run_stats(Ctx& c, int t) {
   Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 0.0);      // its bytes are not algorithmic: counted as GroupNorm-forward time
   s->launches += chan_stats(c.dt, c.fwd(t), s->d.n, hw, T.ref.c, cst_of(c, t), c.st);
 }
-void run_gn_fwd(Ctx& c, Cat x, int t0, int t1, int hw, const void* gamma, const void* beta, size_t mr, void* a_out) {
+void run_gn_fwd(Ctx& c, Cat x, int t0, int t1, int hw, const void* gamma, const void* beta, size_t mr, void* a_out,
+                int act = 1) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 2.0 * s->esz() * s->d.n * hw * x.c());
   s->launches += gn_silu_fwd(c.dt, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta, cst_of(c, t0), cst_of(c, t1),
-                             (float*)(c.stash + mr), a_out, c.st);
+                             (float*)(c.stash + mr), a_out, c.st, act);
 }
 void run_gn_bwd(Ctx& c, const void* g_a, Cat x, size_t mr, int hw, const void* gamma, const void* beta,
                 size_t bst, const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma,
-                float* dbeta, float* cs0, float* cs1) {
+                float* dbeta, float* cs0, float* cs1, int act = 1) {
   pulse_stage* s = c.s;
   Prof pr(s, c.st, PULSE_KCLASS_GN_BWD, 0.0, (3.0 + (add ? 1.0 : 0.0)) * s->esz() * s->d.n * hw * x.c());
   s->launches += gn_silu_bwd(c.dt, g_a, x, s->d.n, hw, s->d.groups, s->d.eps, gamma, beta,
                              (const float*)(c.stash + mr), (float*)(c.work + bst), add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
-                             cs0, cs1, c.st, !(s->d.flags & PULSE_FLAG_GN_TWO_PASS));
+                             cs0, cs1, c.st, !(s->d.flags & PULSE_FLAG_GN_TWO_PASS), true, act);
 }
 
 ConvArgs conv_args(const Ctx& c, Cat src, int hin, int win, int hout, int wout, int k, int stride, const void* w,
@@ -193,6 +197,55 @@ void run_dgrad(Ctx& c, const void* g, int h, int w, int cout, size_t wt_off, int
   run_conv(c, a);
 }
 
+// ---- nearest-2x upsample + conv as four 2x2 phase convs on the low-resolution tensor (kernels.h CONV_UP2): no upsampled
+// tensor, no gradient of it, 4/9 of the FLOPs.  Taken where the tcgen05 kernels cover all three convs of the op; the
+// CUDA-core path (fp32, PULSE_FLAG_FORCE_SIMT) keeps the materialised form, which is the oracle's.
+ConvArgs up2_fwd_args(const Ctx& c, const OpPlan& op) {
+  ConvArgs a = conv_args(c, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, op.hin, op.win, op.hout, op.wout, 3, 1, c.work + op.wt2,
+                         op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out));
+  a.mode = CONV_UP2;
+  return a;
+}
+ConvArgs up2_dgrad_args(const Ctx& c, const OpPlan& op, const void* g_out) {
+  ConvArgs a = conv_args(c, Cat{g_out, op.cout, nullptr, 0}, op.hout, op.wout, op.hin, op.win, 3, 1, c.work + op.wt1, op.cin,
+                         nullptr, nullptr, nullptr, c.grad(op.x0));
+  a.mode = CONV_UP2_DGRAD;
+  return a;
+}
+WgradArgs up2_wgrad_args(const Ctx& c, const OpPlan& op, const void* g_out) {
+  WgradArgs w{c.dt, Cat{c.fwd(op.x0), op.cin, nullptr, 0}, c.s->d.n, op.hin, op.win, g_out, op.hout, op.wout, op.cout, 3, 1,
+              c.pgrad(op.p[P_C1W])};
+  w.up2 = 1;
+  return w;
+}
+// Which form each of the three convs of an up op takes (include/pulse.h, PULSE_FLAG_UP_*): the weight gradient takes the
+// phase form by default (4/9 of the work, exact); the forward and the adjoint need pre-summed bf16 weights (one extra
+// weight rounding) and are opt-in.  The 16-tap adjoint has a quarter of the materialised adjoint's tiles with 16/9 of its K:
+// it gains only when that adjoint needs more than one wave of tiles; on the few-tile grids of the deep levels the 9-tap
+// adjoint on the upsampled grid + 2x2 sum stays even when the flag is set.
+int sm_count_cached() {
+  static int v = 0;
+  if (!v) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;
+  }
+  return v;
+}
+bool up2_wg(const Ctx& c, const OpPlan& op) {
+  return op.kind == PULSE_OP_UP && c.tc() && !(c.s->d.flags & PULSE_FLAG_UP_MATERIALISED) &&
+         wgrad_tc_any_supported(up2_wgrad_args(c, op, nullptr));
+}
+bool up2_fwd(const Ctx& c, const OpPlan& op) {      // only with the phase-form weight gradient: nothing then needs u
+  return (c.s->d.flags & PULSE_FLAG_UP_PHASE_FWD) && up2_wg(c, op) && conv_tc_any_supported(up2_fwd_args(c, op));
+}
+bool up2_dg(const Ctx& c, const OpPlan& op) {
+  if (!(c.s->d.flags & PULSE_FLAG_UP_PHASE_DGRAD) || (c.s->d.flags & PULSE_FLAG_UP_MATERIALISED)) return false;
+  if (op.kind != PULSE_OP_UP || !c.tc() || !conv_tc_any_supported(up2_dgrad_args(c, op, nullptr))) return false;
+  const long long tiles_hi = ((long long)c.s->d.n * op.hout * op.wout + 127) / 128 * (op.cin / (op.cin % 160 == 0 ? 160 : 128));
+  return tiles_hi > sm_count_cached();
+}
+
 // Wt[ci][k-1-r][k-1-s][co] = W[co][r][s][ci] for the convs of ops [lo, hi), one batched launch.  Redone by the first
 // backward after a forward that followed a backward (a new step: parameters may have changed), reused by the other
 // backwards of a wave (R21).
@@ -206,6 +259,12 @@ void prepare_weights(Ctx& c, int lo, int hi) {
       e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, op.cout, 3, ctot});
       e.push_back({c.par(op.p[P_C2W]), c.work + op.wt2, op.cout, 3, op.cout});
       if (op.p[P_SCW] >= 0) e.push_back({c.par(op.p[P_SCW]), c.work + op.wtsc, op.cout, 1, ctot});
+    } else if (op.kind == PULSE_OP_ATTN) {
+      e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, 3 * op.cin, 1, op.cin});
+      e.push_back({c.par(op.p[P_C2W]), c.work + op.wt2, op.cin, 1, op.cin});
+    } else if (up2_dg(c, op)) {       // WpT [cin][16][cout] for the 16-tap adjoint
+      Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
+      s->launches += up2_weights(c.dt, c.par(op.p[P_C1W]), op.cout, op.cin, nullptr, c.work + op.wt1, c.st);
     } else {
       e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, op.cout, 3, op.cin});
     }
@@ -244,6 +303,22 @@ void resblock_forward(Ctx& c, const OpPlan& op) {
   Cat a2{c.fwd(op.a2), op.cout, nullptr, 0};
   run_conv(c, conv_args(c, a2, op.hin, op.win, op.hin, op.win, 3, 1, c.par(op.p[P_C2W]), op.cout,
                         c.par(op.p[P_C2B]), nullptr, res, c.fwd(op.out)), op.out);
+}
+
+// Self-attention block: xn = GN(x); qkv = conv1x1(xn); o = attention(qkv); out = conv1x1(o) + x
+void attn_forward(Ctx& c, const OpPlan& op) {
+  pulse_stage* s = c.s;
+  const int hw = op.hin * op.win, C = op.cin;
+  run_gn_fwd(c, Cat{c.fwd(op.x0), C, nullptr, 0}, op.x0, -1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.mr1,
+             c.fwd(op.a1), /*act=*/0);
+  run_conv(c, conv_args(c, Cat{c.fwd(op.a1), C, nullptr, 0}, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_C1W]), 3 * C,
+                        c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.h1)));
+  {
+    Prof pr(s, c.st, PULSE_KCLASS_OTHER, 4.0 * s->d.n * (double)hw * hw * C, 0.0);
+    s->launches += attn_fwd(c.dt, c.fwd(op.h1), s->d.n, hw, C, op.heads, c.fwd(op.a2), (float*)(c.stash + op.lse), c.st);
+  }
+  run_conv(c, conv_args(c, Cat{c.fwd(op.a2), C, nullptr, 0}, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_C2W]), C,
+                        c.par(op.p[P_C2B]), nullptr, c.fwd(op.x0), c.fwd(op.out)), op.out);
 }
 
 // pixel sums of the gradient of an op's output, for its bias gradient: fused by the writers or one colsum pass
@@ -314,6 +389,36 @@ void resblock_backward(Ctx& c, const OpPlan& op) {
   c.in_rb = false;
 }
 
+void attn_backward(Ctx& c, const OpPlan& op) {
+  pulse_stage* s = c.s;
+  const int n = s->d.n, hw = op.hin * op.win, C = op.cin;
+  char* g_out = c.grad(op.out);
+  char* g_o = c.work + s->w_ga2;
+  char* g_qkv = c.work + s->w_gqkv;
+  char* g_xn = c.work + s->w_ga1;
+  ensure_colsum(c, op.out);
+  c.fork();
+  run_wgrad(c, WgradArgs{c.dt, Cat{c.fwd(op.a2), C, nullptr, 0}, n, op.hin, op.win, g_out, op.hin, op.win, C, 1, 1,
+                         c.pgrad(op.p[P_C2W])});
+  run_dgrad(c, g_out, op.hin, op.win, C, op.wt2, 1, C, g_o, 0, 1, op.hin, op.win);
+  {
+    Prof pr(s, c.st, PULSE_KCLASS_OTHER, 10.0 * n * (double)hw * hw * C, 0.0);
+    s->launches += attn_bwd(c.dt, c.fwd(op.h1), g_o, n, hw, C, op.heads, (float*)(c.stash + op.lse), g_qkv, c.st);
+    s->launches += colsum(c.dt, g_qkv, n, hw, 3 * C, (float*)(c.work + op.gp), c.st);      // qkv bias gradient
+  }
+  c.fork();
+  if (c.last_op && c.side2) tail_work(c);
+  run_wgrad(c, WgradArgs{c.dt, Cat{c.fwd(op.a1), C, nullptr, 0}, n, op.hin, op.win, g_qkv, op.hin, op.win, 3 * C, 1, 1,
+                         c.pgrad(op.p[P_C1W])});
+  // the side stream's wgrad reads g_qkv: the next attention block's backward must not overwrite it before that (one
+  // shared buffer): join here
+  if (c.side) c.wait_side(c.mark_side());
+  run_dgrad(c, g_qkv, op.hin, op.win, 3 * C, op.wt1, 1, C, g_xn, 0, 1, op.hin, op.win);
+  run_gn_bwd(c, g_xn, Cat{c.fwd(op.x0), C, nullptr, 0}, op.mr1, hw, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]), op.bst1,
+             g_out, c.grad(op.x0), C, op.acc_x0, nullptr, 0, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]), cs_of(c, op.x0),
+             nullptr, /*act=*/0);
+}
+
 // bias / temb-projection gradients of every op from the pixel sums, in one batched launch (row a8-a10)
 void small_grads(Ctx& c, const float* emb, float* g_temb, cudaStream_t st) {
   pulse_stage* s = c.s;
@@ -328,6 +433,12 @@ void small_grads(Ctx& c, const float* emb, float* g_temb, cudaStream_t st) {
       g.db_out2 = op.p[P_SCB] >= 0 ? c.pgrad(op.p[P_SCB]) : nullptr;
       g.gp = (const float*)(c.work + op.gp);
       g.db1 = c.pgrad(op.p[P_C1B]); g.dtb = c.pgrad(op.p[P_TB]); g.dtw = c.pgrad(op.p[P_TW]); g.tw = c.par(op.p[P_TW]);
+    } else if (op.kind == PULSE_OP_ATTN) {
+      g.db_out = c.pgrad(op.p[P_C2B]);            // proj bias from the pixel sums of g_out
+      SmallGradEntry q;                           // qkv bias from the pixel sums of g_qkv
+      memset(&q, 0, sizeof q);
+      q.cs_out = (const float*)(c.work + op.gp); q.db_out = c.pgrad(op.p[P_C1B]); q.cout = 3 * op.cin;
+      e.push_back(q);
     } else {
       g.db_out = c.pgrad(op.p[P_C1B]);
     }
@@ -404,6 +515,15 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
       if (temb_forward_impl(s, d_t, d_temb, d_temb_stash, c.st) != PULSE_OK) c.err = true;
       CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
     }
+    if (s->last_was_backward) s->wp_valid = false;      // a forward after a backward starts a new step: parameters may have changed
+    if (!s->wp_valid) {                                  // pre-summed phase weights Wp [4][cout][4][cin] of the up convs
+      for (const OpPlan& op : s->ops)
+        if (up2_fwd(c, op)) {
+          Prof pr(s, c.st, PULSE_KCLASS_OTHER, 0.0, 0.0);
+          s->launches += up2_weights(c.dt, c.par(op.p[P_C1W]), op.cout, op.cin, c.work + op.wt2, nullptr, c.st);
+        }
+      s->wp_valid = true;
+    }
     std::vector<ProjEntry> pe;
     for (const OpPlan& op : s->ops)
       if (op.kind == PULSE_OP_RESBLOCK)
@@ -425,6 +545,7 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
     const OpPlan& op = s->ops[i];
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_forward(c, op); break;
+      case PULSE_OP_ATTN: attn_forward(c, op); break;
       case PULSE_OP_CONV_IN:
       case PULSE_OP_DOWN: {
         const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
@@ -433,6 +554,11 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
         break;
       }
       case PULSE_OP_UP: {
+        if (up2_fwd(c, op)) {
+          if (c.ev_proj >= 0) { c.wait_side(c.ev_proj); c.ev_proj = -1; }      // the phase weights (side stream) are ready
+          run_conv(c, up2_fwd_args(c, op), op.out);
+          break;
+        }
         s->launches += upsample2(c.dt, c.fwd(op.x0), s->d.n, op.hin, op.win, op.cin, c.fwd(op.u), c.st);
         run_conv(c, conv_args(c, Cat{c.fwd(op.u), op.cin, nullptr, 0}, op.hout, op.wout, op.hout, op.wout, 3, 1,
                               c.par(op.p[P_C1W]), op.cout, c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.out)), op.out);
@@ -527,6 +653,7 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
     if (i == nops - 2) c.wait_side(ev_wt_rest);
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_backward(c, op); break;
+      case PULSE_OP_ATTN: attn_backward(c, op); break;
       case PULSE_OP_CONV_IN:
       case PULSE_OP_DOWN: {
         const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
@@ -546,6 +673,24 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
         char* g_out = c.grad(op.out);
         char* g_u = c.work + s->w_gu;
         ensure_colsum(c, op.out);
+        const bool wg2 = up2_wg(c, op), dg2 = up2_dg(c, op);
+        if (wg2 || dg2) {
+          c.fork();
+          if (wg2) {
+            run_wgrad(c, up2_wgrad_args(c, op, g_out));
+          } else {          // (then the forward was the materialised form too: u exists)
+            WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
+                        1, c.pgrad(op.p[P_C1W])};
+            run_wgrad(c, w);
+          }
+          if (dg2) {
+            run_conv(c, up2_dgrad_args(c, op, g_out));
+          } else {
+            run_dgrad(c, g_out, op.hout, op.wout, op.cout, op.wt1, 3, op.cin, g_u, 0, 1, op.hout, op.wout);
+            s->launches += upsample2_bwd(c.dt, g_u, n, op.hin, op.win, op.cin, c.grad(op.x0), c.st);
+          }
+          break;
+        }
         WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
                     1, c.pgrad(op.p[P_C1W])};
         c.fork();
@@ -756,6 +901,93 @@ extern "C" pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const vo
               cout, ksize, stride, d_dw};
   const int r = (!force_simt && wgrad_tc_any_supported(a)) ? wgrad_tc_any(a, (cudaStream_t)stream) : wgrad_simt(a, (cudaStream_t)stream);
   if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core wgrad launch failed: %s", tc_last_error());
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+
+// ---- attention core in isolation
+static pulse_status_t check_attn(int dtype, int n, int t, int c, int heads) {
+  if (dtype != PULSE_F32 && dtype != PULSE_BF16) return fail(PULSE_ERR_INVALID_ARG, "dtype");
+  if (n <= 0 || t <= 0 || c <= 0 || heads <= 0) return fail(PULSE_ERR_INVALID_ARG, "non-positive size");
+  if (!attn_supported(c, heads)) return fail(PULSE_ERR_SHAPE, "channels %d not divisible by heads %d, or more than 128 per head", c, heads);
+  return PULSE_OK;
+}
+extern "C" size_t pulse_attention_stats_floats(int n, int heads, int tokens) {
+  return (n <= 0 || heads <= 0 || tokens <= 0) ? 0 : attn_stats_floats(n, heads, tokens);
+}
+extern "C" pulse_status_t pulse_attention(int dtype, const void* d_qkv, int n, int tokens, int c, int heads, void* d_o,
+                                          float* d_stats, void* stream) {
+  pulse_status_t s = check_attn(dtype, n, tokens, c, heads);
+  if (s) return s;
+  if (!d_qkv || !d_o || !d_stats) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  attn_fwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_qkv, n, tokens, c, heads, d_o, d_stats, (cudaStream_t)stream);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_attention_backward(int dtype, const void* d_qkv, const void* d_g_o, int n, int tokens, int c,
+                                                   int heads, float* d_stats, void* d_g_qkv, void* stream) {
+  pulse_status_t s = check_attn(dtype, n, tokens, c, heads);
+  if (s) return s;
+  if (!d_qkv || !d_g_o || !d_stats || !d_g_qkv) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  attn_bwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_qkv, d_g_o, n, tokens, c, heads, d_stats, d_g_qkv, (cudaStream_t)stream);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+
+// ---- nearest-2x upsample + 3x3 conv (row a6) as the 4-phase form, in isolation
+static pulse_status_t check_up(int dtype, int kernel, int n, int h, int w, int cin, int cout) {
+  if (dtype != PULSE_BF16) return fail(PULSE_ERR_UNSUPPORTED, "the 4-phase upsample conv is a tcgen05 (bf16) path");
+  if (n <= 0 || h <= 0 || w <= 0 || cin <= 0 || cout <= 0) return fail(PULSE_ERR_INVALID_ARG, "non-positive size");
+  if (kernel != PULSE_CONV_AUTO && kernel != PULSE_CONV_TC_PAIR && kernel != PULSE_CONV_TC_1CTA)
+    return fail(PULSE_ERR_INVALID_ARG, "kernel selector %d", kernel);
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_upsample_conv2d(int dtype, int kernel, const void* d_src, int n, int h, int w, int cin,
+                                                const void* d_w, int cout, const void* d_bias, void* d_wp_scratch,
+                                                void* d_out, float* d_chan_stats, void* stream) {
+  pulse_status_t s = check_up(dtype, kernel, n, h, w, cin, cout);
+  if (s) return s;
+  if (!d_src || !d_w || !d_wp_scratch || !d_out) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  ConvArgs a;
+  a.dt = DT_BF16; a.src = Cat{d_src, cin, nullptr, 0}; a.n = n; a.hin = h; a.win = w; a.hout = 2 * h; a.wout = 2 * w;
+  a.ksize = 3; a.stride = 1; a.mode = CONV_UP2; a.w = d_wp_scratch; a.cout = cout; a.bias = d_bias; a.pn = nullptr;
+  a.residual = nullptr; a.out = d_out; a.accumulate = 0; a.kernel = conv_kernel_of(kernel);
+  if (!conv_tc_any_supported(a)) return fail(PULSE_ERR_UNSUPPORTED, "shape not covered by the tcgen05 conv kernels");
+  up2_weights(DT_BF16, d_w, cout, cin, d_wp_scratch, nullptr, st);
+  const bool fused = d_chan_stats && (a.cst = d_chan_stats, conv_emits_stats(a));
+  if (!fused) a.cst = nullptr;
+  if (conv_tc_any(a, st) < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
+  if (d_chan_stats && !fused) chan_stats(DT_BF16, d_out, n, 4 * h * w, cout, d_chan_stats, st);
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_upsample_conv2d_dgrad(int dtype, int kernel, const void* d_g, int n, int h, int w, int cin,
+                                                      const void* d_w, int cout, void* d_wpt_scratch, void* d_g_in,
+                                                      void* stream) {
+  pulse_status_t s = check_up(dtype, kernel, n, h, w, cin, cout);
+  if (s) return s;
+  if (!d_g || !d_w || !d_wpt_scratch || !d_g_in) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  ConvArgs a;
+  a.dt = DT_BF16; a.src = Cat{d_g, cout, nullptr, 0}; a.n = n; a.hin = 2 * h; a.win = 2 * w; a.hout = h; a.wout = w;
+  a.ksize = 3; a.stride = 1; a.mode = CONV_UP2_DGRAD; a.w = d_wpt_scratch; a.cout = cin; a.bias = nullptr; a.pn = nullptr;
+  a.residual = nullptr; a.out = d_g_in; a.accumulate = 0; a.kernel = conv_kernel_of(kernel);
+  if (!conv_tc_any_supported(a)) return fail(PULSE_ERR_UNSUPPORTED, "shape not covered by the tcgen05 conv kernels");
+  up2_weights(DT_BF16, d_w, cout, cin, nullptr, d_wpt_scratch, st);
+  if (conv_tc_any(a, st) < 0) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
+  CK_CUDA(cudaGetLastError());
+  return PULSE_OK;
+}
+extern "C" pulse_status_t pulse_upsample_conv2d_wgrad(int dtype, const void* d_src, int n, int h, int w, int cin,
+                                                      const void* d_g, int cout, float* d_dw, void* stream) {
+  pulse_status_t s = check_up(dtype, PULSE_CONV_AUTO, n, h, w, cin, cout);
+  if (s) return s;
+  if (!d_src || !d_g || !d_dw) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
+  WgradArgs a{DT_BF16, Cat{d_src, cin, nullptr, 0}, n, h, w, d_g, 2 * h, 2 * w, cout, 3, 1, d_dw};
+  a.up2 = 1;
+  if (!wgrad_tc_any_supported(a)) return fail(PULSE_ERR_UNSUPPORTED, "shape not covered by the tcgen05 wgrad kernel");
+  if (wgrad_tc_any(a, (cudaStream_t)stream) < 0) return fail(PULSE_ERR_CUDA, "tensor-core wgrad launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }

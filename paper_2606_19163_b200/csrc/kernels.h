@@ -29,7 +29,8 @@ RowPlan row_plan(int dt, int hw, int c, int n, int max_threads);
 int chan_stats(int dt, const void* x, int n, int hw, int c, float* cst, cudaStream_t st, void* copy = nullptr);
 // mr_out: [n][2][groups] fp32, the group means and reciprocal standard deviations, kept for the backward
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st);
+                const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st, int act = 1);
+// act = 0 (here and in the backward launchers): plain GroupNorm, y = gamma xhat + beta, no SiLU (attention blocks)
 // g_x = r(gamma g_y - A - xhat B) [+ add]; channels [0,dc0) -> dst0, rest -> dst1; accX: += instead of =
 // bst: [n][2][C] fp32 scratch, zeroed by the caller (per-(image, channel) sums of g_y and g_y xhat).
 // dgamma/dbeta: fp32, +=.  cs0/cs1 (nullable): [n][dc0] / [n][C-dc0] fp32, += the per-(image, channel) pixel
@@ -37,7 +38,7 @@ int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void*
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
                 const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
-                cudaStream_t st, bool allow_fused = true, bool fwd_data_ready = true);
+                cudaStream_t st, bool allow_fused = true, bool fwd_data_ready = true, int act = 1);
 
 // the same in one launch (norm_fused.cu; bf16, mean / rstd from the forward); 0 = shape not covered, nothing launched.
 // fwd_data_ready: x and mr were complete before the PREVIOUS kernel of the stream started (true inside a stage: they
@@ -45,7 +46,17 @@ int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float
 // programmatic serialization (the single-operator entry point, where the forward may be the previous kernel).
 int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* gamma, const void* beta, const float* mr,
                  const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta,
-                 float* cs0, float* cs1, cudaStream_t st, bool fwd_data_ready = true);
+                 float* cs0, float* cs1, cudaStream_t st, bool fwd_data_ready = true, int act = 1);
+
+// ---- attention core (attention.cu) ------------------------------------
+// qkv [n][T][3C] (q | k | v per pixel, head h = channels [h d, (h+1) d) of each third), o / g_o [n][T][C];
+// stats: attn_stats_floats(n, heads, T) floats (log-sum-exp of the scaled scores, then D = rowsum(P g_P)) written by the
+// forward / backward and kept between them
+bool attn_supported(int C, int heads);
+size_t attn_stats_floats(int n, int heads, int T);
+int attn_fwd(int dt, const void* qkv, int n, int T, int C, int heads, void* o, float* stats, cudaStream_t st);
+int attn_bwd(int dt, const void* qkv, const void* g_o, int n, int T, int C, int heads, float* stats, void* g_qkv,
+             cudaStream_t st);
 
 // ---- small ops -----------------------------------------------------------------------
 // cs[n][c] += sum over pixels of g[n][hw][c]   (tensors whose writers could not emit their column sums)
@@ -75,6 +86,9 @@ int flip_transpose_batch(int dt, const TransposeEntry* e, int count, cudaStream_
 int sinusoidal(const int64_t* t, int n, int d, float* out, cudaStream_t st);
 int mse_fwd_bwd(int dt, const void* d, const void* target, size_t numel, float scale, float* loss, void* g,
                 cudaStream_t st);
+// Wp [4][cout][4][cin] (nullable) and WpT [cin][16][cout] (nullable) of CONV_UP2 / CONV_UP2_DGRAD from W [cout][3][3][cin];
+// sums in fp32, stored in dtype
+int up2_weights(int dt, const void* w, int cout, int cin, void* wp, void* wpt, cudaStream_t st);
 int upsample2(int dt, const void* in, int n, int h, int w, int c, void* out, cudaStream_t st);
 int upsample2_bwd(int dt, const void* g_u, int n, int h, int w, int c, void* g_out, cudaStream_t st);  // h,w: low-res
 int add_inplace(int dt, void* dst, const void* src, size_t numel, cudaStream_t st);
@@ -82,13 +96,21 @@ int add_inplace(int dt, void* dst, const void* src, size_t numel, cudaStream_t s
 int flip_transpose(int dt, const void* w, int cout, int k, int cin, void* wt, cudaStream_t st);
 
 // ---- convolution ---------------------------------------------------
-enum { CONV_FPROP = 0, CONV_DGRAD_S2 = 1 };
+// CONV_UP2 / CONV_UP2_DGRAD: nearest-2x upsample + 3x3 conv WITHOUT the upsampled tensor:
+// output pixel (2y+py, 2x+px) sees the low-resolution pixels (y+dy, x+dx), dy = a-1+py, dx = b-1+px, a,b in {0,1}, through
+// the pre-summed weights Wp[2py+px][co][2a+b][ci] = sum of W[co][r][s][ci] over r in R(py,a), s in R(px,b),
+// R(0,0)={0}, R(0,1)={1,2}, R(1,0)={0,1}, R(1,1)={2}  (up2_weights): 4 taps on h x w pixels per phase instead of 9 taps on
+// 2h x 2w = 4/9 of the FLOPs.  The adjoint in the input is one 16-tap conv over the parity view of the gradient.
+enum { CONV_FPROP = 0, CONV_DGRAD_S2 = 1, CONV_UP2 = 2, CONV_UP2_DGRAD = 3 };
 enum { CONV_K_AUTO = 0, CONV_K_PAIR = 1, CONV_K_1CTA = 2 };      // which tcgen05 conv kernel (ConvArgs::kernel)
 struct ConvArgs {
   int dt;
   Cat src; int n, hin, win;       // source tensor(s) [n,hin,win,c]
   int hout, wout;                 // output pixels
   int ksize, stride, mode;        // mode CONV_DGRAD_S2: src pixel = (y + r - pad)/2 when even (stride ignored)
+                                  // CONV_UP2: src low-res [n,hin,win,c], out [n,2hin,2win,cout], w = Wp [4][cout][4][c]
+                                  // CONV_UP2_DGRAD: src = gradient [n,hin,win,c] (high-res), out [n,hin/2,win/2,cout],
+                                  //                 w = WpT [cout][16][c] (cout = the conv's input channels)
   const void* w;                  // [cout][k][k][src.c()]
   int cout;
   const void* bias;               // [cout] dtype, or null
@@ -107,6 +129,7 @@ struct WgradArgs {
   const void* g; int hout, wout, cout;   // forward output gradient [n,hout,wout,cout]
   int ksize, stride;
   float* dw;                      // [cout][k][k][src.c()] fp32, atomically accumulated
+  int up2 = 0;                    // 1: the conv of CONV_UP2: src low-res [n,hin,win,c], g [n,2hin,2win,cout]; dw is the 9-tap gradient
 };
 int wgrad_simt(const WgradArgs& a, cudaStream_t st);
 // 4 channels on one side (conv_in, head; conv_thin.cu): conv_simt / wgrad_simt route to these when they apply

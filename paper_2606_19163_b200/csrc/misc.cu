@@ -586,6 +586,52 @@ int flip_transpose_batch(int dt, const TransposeEntry* e, int count, cudaStream_
   }
   return launches;
 }
+// ------------------------------------------------------------------ pre-summed phase weights of the 4-phase upsample conv
+// (kernels.h CONV_UP2).  One block = a 32 x 32 (co, ci) tile: the 9 taps are staged in shared memory as fp32, the 16
+// (phase, tap) sums are formed there and written along ci (Wp) and, transposed, along co (WpT).
+// The sums are formed in fp32 and rounded to the stage dtype: for bf16 that is one rounding of the WEIGHTS (2^-9 relative
+// per product; measured: as much as one more bf16 store of the conv's output).  tcgen05 kind::f16 does NOT take a bf16 A
+// operand with an fp16 B operand (tried: illegal instruction), so the 11 significand bits of fp16 are not available here.
+template <typename T>
+__global__ void __launch_bounds__(256) up2_weights_k(const T* __restrict__ w, int cout, int cin, T* __restrict__ wp,
+                                                      T* __restrict__ wpt) {
+  __shared__ float tile[9][32][33];
+  const int ci0 = blockIdx.x * 32, co0 = blockIdx.y * 32, tx = threadIdx.x, ty = threadIdx.y;
+  for (int tap = 0; tap < 9; ++tap)
+    for (int j = ty; j < 32; j += 8) {
+      const int co = co0 + j, ci = ci0 + tx;
+      tile[tap][j][tx] = (co < cout && ci < cin) ? to_f(w[((size_t)co * 9 + tap) * cin + ci]) : 0.f;
+    }
+  __syncthreads();
+  // R(0,0)={0}, R(0,1)={1,2}, R(1,0)={0,1}, R(1,1)={2} as [first, last] per (parity, a)
+  const int lo[2][2] = {{0, 1}, {0, 2}}, hi[2][2] = {{0, 2}, {1, 2}};
+  for (int q = 0; q < 16; ++q) {
+    const int py = q >> 3, px = (q >> 2) & 1, a = (q >> 1) & 1, b = q & 1;      // q = (2py+px)*4 + 2a+b
+    for (int j = ty; j < 32; j += 8) {
+      if (wp) {           // rows co, contiguous ci
+        const int co = co0 + j, ci = ci0 + tx;
+        float v = 0.f;
+        for (int r = lo[py][a]; r <= hi[py][a]; ++r)
+          for (int s = lo[px][b]; s <= hi[px][b]; ++s) v += tile[r * 3 + s][j][tx];
+        if (co < cout && ci < cin) wp[(((size_t)(q >> 2) * cout + co) * 4 + (q & 3)) * cin + ci] = from_f<T>(v);
+      }
+      if (wpt) {          // rows ci, contiguous co
+        const int ci = ci0 + j, co = co0 + tx;
+        float v = 0.f;
+        for (int r = lo[py][a]; r <= hi[py][a]; ++r)
+          for (int s = lo[px][b]; s <= hi[px][b]; ++s) v += tile[r * 3 + s][tx][j];
+        if (co < cout && ci < cin) wpt[((size_t)ci * 16 + q) * cout + co] = from_f<T>(v);
+      }
+    }
+  }
+}
+int up2_weights(int dt, const void* w, int cout, int cin, void* wp, void* wpt, cudaStream_t st) {
+  dim3 grid((cin + 31) / 32, (cout + 31) / 32), block(32, 8);
+  if (dt == DT_F32) up2_weights_k<float><<<grid, block, 0, st>>>((const float*)w, cout, cin, (float*)wp, (float*)wpt);
+  else up2_weights_k<bf16><<<grid, block, 0, st>>>((const bf16*)w, cout, cin, (bf16*)wp, (bf16*)wpt);
+  return 1;
+}
+
 int flip_transpose(int dt, const void* w, int cout, int k, int cin, void* wt, cudaStream_t st) {
   dim3 grid((cin + 31) / 32, (cout + 31) / 32, k * k), block(32, 8);
   if (dt == DT_F32) flip_transpose_k<float><<<grid, block, 0, st>>>((const float*)w, cout, k * k, cin, (float*)wt);

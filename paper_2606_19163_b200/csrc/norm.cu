@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(512, 2)
 gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw, int G, float eps,
            const T* __restrict__ gamma, const T* __restrict__ beta, const float* __restrict__ cst0,
            const float* __restrict__ cst1, float* __restrict__ mr_out, T* __restrict__ out, int P, int stage_bytes,
-           int pro_floats) {
+           int pro_floats, int act) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -332,8 +332,9 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
       if (two) lds<T>(st + xoff + (pl + rows) * xpp, v[1]);
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        v[0][i] = silu_t<T>(fmaf(v[0][i], sc[i], sh[i]));
-        v[1][i] = silu_t<T>(fmaf(v[1][i], sc[i], sh[i]));
+        const float y0 = fmaf(v[0][i], sc[i], sh[i]), y1 = fmaf(v[1][i], sc[i], sh[i]);
+        v[0][i] = act ? silu_t<T>(y0) : y0;          // act == 0: plain GroupNorm (attention blocks)
+        v[1][i] = act ? silu_t<T>(y1) : y1;
       }
       stv(out + ((size_t)n * hw + pbase + pl) * C + ch, v[0]);
       if (two) stv(out + ((size_t)n * hw + pbase + pl + rows) * C + ch, v[1]);
@@ -348,7 +349,7 @@ template <typename T>
 __global__ void __launch_bounds__(512, 1)
 gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
-               const float* __restrict__ mrp, float* __restrict__ bst, int P, int stage_bytes, int pro_floats) {
+               const float* __restrict__ mrp, float* __restrict__ bst, int P, int stage_bytes, int pro_floats, int act) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -386,7 +387,7 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
       lds<T>(st + goff + pl * gpp, g);
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        const float gy = g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i]));
+        const float gy = act ? g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i])) : g[i];
         v[0][i] += gy;
         v[1][i] = fmaf(gy, fmaf(x[i], rr[i], -mr[i]), v[1][i]);
       }
@@ -405,7 +406,7 @@ __global__ void __launch_bounds__(512, 1)
 gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
                const float* __restrict__ mrp, const float* __restrict__ bst, float* dgamma, float* dbeta, const T* __restrict__ add, T* dst0, int dc0, int acc0, T* dst1, int acc1,
-               float* cs0, float* cs1, int P, int stage_bytes, int pro_floats) {
+               float* cs0, float* cs1, int P, int stage_bytes, int pro_floats, int act) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -488,7 +489,7 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
       if (add) lds<T>(st + eoff + pl * gpp, e);
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        const float gy = g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i]));
+        const float gy = act ? g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i])) : g[i];
         const float xh = fmaf(x[i], rr[i], -mr[i]);
         o[i] = sc[i] * gy - k2[i] - xh * k3[i];
         if (add) o[i] += e[i];
@@ -561,7 +562,7 @@ template <typename K> static void allow_big_smem(K kernel) {
 }
 
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
-                const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st) {
+                const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st, int act) {
   const int C = x.c();
   const StreamPlan sp = stream_plan(dt, n, hw, C, groups, 0, C * (int)dt_size(dt), 2);
   static bool attr = false;
@@ -569,11 +570,11 @@ int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void*
   if (dt == DT_F32)
     launch_pdl(gn_apply_k<float>, sp.grid, sp.block, sp.smem, st, (const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw,
                groups, eps, (const float*)gamma, (const float*)beta, cst0, cst1, mr_out, (float*)a_out, sp.P, sp.stage_bytes,
-               sp.pro_floats);
+               sp.pro_floats, act);
   else
     launch_pdl(gn_apply_k<bf16>, sp.grid, sp.block, sp.smem, st, (const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw,
                groups, eps, (const bf16*)gamma, (const bf16*)beta, cst0, cst1, mr_out, (bf16*)a_out, sp.P, sp.stage_bytes,
-               sp.pro_floats);
+               sp.pro_floats, act);
   return 1;
 }
 
@@ -581,34 +582,34 @@ template <typename T>
 static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
                     const float* mr, float* bst, const void* add, void* dst0, int dc0, int acc0,
                     void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st,
-                    bool allow_fused, bool fwd_data_ready) {
+                    bool allow_fused, bool fwd_data_ready, int act) {
   const int C = x.c();
   const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
   if (dt == DT_BF16 && allow_fused) {        // one pass with the tensors resident in shared memory where the shape allows (norm_fused.cu)
     const int r = gn_bwd_fused(g_a, x, n, hw, groups, gamma, beta, mr, add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
-                               cs0, cs1, st, fwd_data_ready);
+                               cs0, cs1, st, fwd_data_ready, act);
     if (r > 0) return r;
   }
   static bool attr = false;
   if (!attr) { allow_big_smem(gn_bwd_stats_k<T>); allow_big_smem(gn_bwd_apply_k<T>); attr = true; }
   const StreamPlan s1 = stream_plan(dt, n, hw, C, groups, 2, 2 * C * (int)sizeof(T));
   launch_pdl(gn_bwd_stats_k<T>, s1.grid, s1.block, s1.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
-             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, bst, s1.P, s1.stage_bytes, s1.pro_floats);
+             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, bst, s1.P, s1.stage_bytes, s1.pro_floats, act);
   const StreamPlan s2 = stream_plan(dt, n, hw, C, groups, 1, (add ? 3 : 2) * C * (int)sizeof(T));
   launch_pdl(gn_bwd_apply_k<T>, s2.grid, s2.block, s2.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
              x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, (const float*)bst, dgamma, dbeta,
-             (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes, s2.pro_floats);
+             (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes, s2.pro_floats, act);
   return 2;
 }
 
 int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma,
                 const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
-                cudaStream_t st, bool allow_fused, bool fwd_data_ready) {
+                cudaStream_t st, bool allow_fused, bool fwd_data_ready, int act) {
   return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st, false, fwd_data_ready)
+                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st, false, fwd_data_ready, act)
                       : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st, allow_fused, fwd_data_ready);
+                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st, allow_fused, fwd_data_ready, act);
 }
 
 }  // namespace pulse

@@ -40,6 +40,7 @@ struct GnfParams {
   const bf16* add; bf16* dst0; bf16* dst1; int dc0, acc0, acc1;
   float* cs0; float* cs1;
   int data_bytes, red_floats;
+  int act;                       // 1: GroupNorm + SiLU, 0: plain GroupNorm (g_y = g_a)
 };
 
 __device__ __forceinline__ void lds8(const uint8_t* p, float (&o)[8]) { ldv(reinterpret_cast<const bf16*>(p), o); }
@@ -169,7 +170,7 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const f2_t x = bf2(xv[j]);
-        const f2_t gy = mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone));
+        const f2_t gy = p.act ? mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone)) : bf2(gv[j]);
         S2[0][j] = add2(S2[0][j], gy);
         S2[1][j] = fma2(gy, fma2(x, rr2[j], nmr2[j]), S2[1][j]);
       }
@@ -252,7 +253,7 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
 #pragma unroll
       for (int j = 0; j < 4; ++j) {          // g_y again, in fp32 (keeping it in shared memory would round it to bf16)
         const f2_t x = bf2(xv[j]);
-        const f2_t gy = mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone));
+        const f2_t gy = p.act ? mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone)) : bf2(gv[j]);
         o[j] = fma2(fma2(x, rr2[j], nmr2[j]), nk3[j], fma2(sc2[j], gy, nk2[j]));
       }
       if (p.add) {
@@ -300,7 +301,7 @@ static int gcd_(int a, int b) { while (b) { const int t = a % b; a = b; b = t; }
 // One launch, or 0 when the shape is not covered (the caller then runs the two-kernel form).
 int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* gamma, const void* beta, const float* mr,
                  const void* add, void* dst0, int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta,
-                 float* cs0, float* cs1, cudaStream_t st, bool fwd_data_ready) {
+                 float* cs0, float* cs1, cudaStream_t st, bool fwd_data_ready, int act) {
   static bool enabled = !toggles().no_gn_fused;
   if (!enabled) return 0;
   const int C = x.c();
@@ -339,7 +340,7 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
   p.c0 = x.c0; p.c1 = x.c1; p.hw = hw; p.G = groups; p.Cs = Cs; p.CL = CL;
   p.gamma = (const bf16*)gamma; p.beta = (const bf16*)beta; p.mr = mr; p.dgamma = dgamma; p.dbeta = dbeta;
   p.add = (const bf16*)add; p.dst0 = (bf16*)dst0; p.dst1 = (bf16*)dst1; p.dc0 = dc0; p.acc0 = acc0; p.acc1 = acc1;
-  p.cs0 = cs0; p.cs1 = cs1;
+  p.cs0 = cs0; p.cs1 = cs1; p.act = act;
   CUtensorMap mx0, mx1, mg;
   const uint64_t rows = (uint64_t)n * hw;
   auto mk = [&](const void* ptr, int c, CUtensorMap* m) {

@@ -93,7 +93,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
   if (d.x_in_is_skip) { s->skip_tensor.push_back(cur); stack.push_back(cur); }
   s->emb_off = pl.bump(R_STASH, (size_t)d.n * T * 4);
 
-  size_t m_out = 0, m_cat = 0, m_gu = 0;
+  size_t m_out = 0, m_cat = 0, m_gu = 0, m_qkv = 0;
   auto upd = [](size_t& m, size_t v) { if (v > m) m = v; };
 
   auto plan_ops = [&](const std::vector<pulse_op_desc>& list, const char* phase, bool is_dec) -> pulse_status_t {
@@ -102,7 +102,7 @@ static pulse_status_t build_plan(pulse_stage* s) {
       OpPlan op;
       for (int k = 0; k < 12; ++k) op.p[k] = -1;
       const Tensor& tin = s->tensors[cur];
-      op.kind = o.kind; op.cin = o.cin; op.cskip = o.skip_channels; op.cout = o.cout;
+      op.kind = o.kind; op.cin = o.cin; op.cskip = o.skip_channels; op.cout = o.cout; op.heads = o.heads;
       op.hin = tin.ref.h; op.win = tin.ref.w; op.hout = op.hin; op.wout = op.win;
       op.x0 = cur;
       if (tin.ref.c != o.cin) return fail(PULSE_ERR_SHAPE, "%s%zu: cin %d but input has %d channels", phase, i, o.cin, tin.ref.c);
@@ -157,7 +157,26 @@ static pulse_status_t build_plan(pulse_stage* s) {
         }
         if (o.kind == PULSE_OP_CONV_IN && is_dec) return fail(PULSE_ERR_SHAPE, "%s%zu: conv_in belongs to the encoder", phase, i);
         op.p[P_C1W] = pl.param(pre + "conv.w", 4, o.cout, 3, 3, o.cin); op.p[P_C1B] = pl.param(pre + "conv.b", 1, o.cout);
-        op.wt1 = pl.bump(R_WORK, (size_t)o.cout * 9 * o.cin * s->esz());
+        // up: room for the 16 pre-summed (phase, tap) matrices of the 4-phase form, transposed (wt1) and plain (wt2)
+        op.wt1 = pl.bump(R_WORK, (size_t)o.cout * (o.kind == PULSE_OP_UP ? 16 : 9) * o.cin * s->esz());
+        if (o.kind == PULSE_OP_UP) op.wt2 = pl.bump(R_WORK, (size_t)o.cout * 16 * o.cin * s->esz());
+      } else if (o.kind == PULSE_OP_ATTN) {
+        // x -> GN -> xn (a1) -> 1x1 conv -> qkv (h1, 3c channels) -> attention -> o (a2) -> 1x1 conv + x -> out
+        if (o.skip_channels || o.cin != o.cout || !chk_c(o.cin, "cin") || !attn_supported(o.cin, o.heads))
+          return fail(PULSE_ERR_SHAPE, "%s%zu: attention needs cin == cout divisible by groups and heads, cin / heads <= 128", phase, i);
+        const int c = o.cin;
+        op.p[P_GN1G] = pl.param(pre + "gn.gamma", 1, c); op.p[P_GN1B] = pl.param(pre + "gn.beta", 1, c);
+        op.p[P_C1W] = pl.param(pre + "qkv.w", 4, 3 * c, 1, 1, c); op.p[P_C1B] = pl.param(pre + "qkv.b", 1, 3 * c);
+        op.p[P_C2W] = pl.param(pre + "proj.w", 4, c, 1, 1, c); op.p[P_C2B] = pl.param(pre + "proj.b", 1, c);
+        op.a1 = pl.tensor(R_STASH, c, op.hin, op.win, false);
+        op.h1 = pl.tensor(R_STASH, 3 * c, op.hin, op.win, false);
+        op.a2 = pl.tensor(R_STASH, c, op.hin, op.win, false);
+        s->tensors[op.x0].gn_input = true;
+        op.mr1 = pl.bump(R_STASH, (size_t)d.n * 2 * G * 4);
+        op.lse = pl.bump(R_STASH, attn_stats_floats(d.n, o.heads, op.hin * op.win) * 4);
+        upd(m_out, pix * c * s->esz()); upd(m_cat, pix * c * s->esz()); upd(m_qkv, pix * 3 * c * s->esz());
+        op.wt1 = pl.bump(R_WORK, (size_t)3 * c * c * s->esz());
+        op.wt2 = pl.bump(R_WORK, (size_t)c * c * s->esz());
       } else if (o.kind == PULSE_OP_HEAD) {
         if (!is_dec || o.skip_channels || !chk_c(o.cin, "cin")) return fail(PULSE_ERR_SHAPE, "%s%zu: bad head", phase, i);
         op.p[P_GN1G] = pl.param(pre + "gn.gamma", 1, o.cin); op.p[P_GN1B] = pl.param(pre + "gn.beta", 1, o.cin);
@@ -185,7 +204,9 @@ static pulse_status_t build_plan(pulse_stage* s) {
   if (st) return st;
   s->n_enc = (int)s->enc.size();
   if (d.link == PULSE_LINK_CLOSED) {
-    for (auto& o : s->mid) if (o.kind != PULSE_OP_RESBLOCK || o.skip_channels) return fail(PULSE_ERR_SHAPE, "mid ops must be plain ResBlocks");
+    for (auto& o : s->mid)
+      if ((o.kind != PULSE_OP_RESBLOCK && o.kind != PULSE_OP_ATTN) || o.skip_channels)
+        return fail(PULSE_ERR_SHAPE, "mid ops must be plain ResBlocks or attention blocks");
     st = plan_ops(s->mid, "mid", false);
     if (st) return st;
   } else {
@@ -239,12 +260,16 @@ static pulse_status_t build_plan(pulse_stage* s) {
       op.gp = pl.bump(R_WORK, (size_t)d.n * op.cout * 4);
     } else if (op.kind == PULSE_OP_HEAD) {
       op.bst1 = pl.bump(R_WORK, (size_t)d.n * 2 * op.cin * 4);
+    } else if (op.kind == PULSE_OP_ATTN) {
+      op.bst1 = pl.bump(R_WORK, (size_t)d.n * 2 * op.cin * 4);
+      op.gp = pl.bump(R_WORK, (size_t)d.n * 3 * op.cin * 4);       // pixel sums of g_qkv: the qkv bias gradient
     }
   }
   s->zero_end = pl.bump(R_WORK, 0);
   s->w_ga2 = pl.bump(R_WORK, m_out); s->w_gh1 = pl.bump(R_WORK, m_out); s->w_gh1b = pl.bump(R_WORK, m_out);
   s->w_ga1 = pl.bump(R_WORK, m_cat); s->w_gsc = pl.bump(R_WORK, m_cat);
   s->w_gu = pl.bump(R_WORK, m_gu);
+  s->w_gqkv = pl.bump(R_WORK, m_qkv);
   s->w_tmpf = pl.bump(R_WORK, (size_t)d.n * T * 4 + 256);
   s->work_bytes = pl.top[R_WORK];
   return PULSE_OK;
@@ -310,7 +335,7 @@ extern "C" pulse_status_t pulse_stage_bind_params(pulse_stage_t* s, const void* 
   if (!s || !d_params || !d_grads) return fail(PULSE_ERR_INVALID_ARG, "null argument");
   if (!aligned256(d_params) || !aligned256(d_grads)) return fail(PULSE_ERR_INVALID_ARG, "buffers must be 256-byte aligned");
   s->d_params = (const char*)d_params; s->d_grads = d_grads;
-  s->wt_valid = false;
+  s->wt_valid = false; s->wp_valid = false;
   return PULSE_OK;
 }
 extern "C" pulse_status_t pulse_stage_workspace_bytes(const pulse_stage_t* s, size_t* per_stage, size_t* per_inflight) {
@@ -325,7 +350,7 @@ extern "C" pulse_status_t pulse_stage_bind_workspace(pulse_stage_t* s, void* d, 
   const size_t need = s->work_bytes + (size_t)s->d.max_inflight * s->stash_bytes;
   if (bytes < need) return fail(PULSE_ERR_BUFFER_TOO_SMALL, "workspace %zu < %zu bytes", bytes, need);
   s->d_work = (char*)d; s->work_bound = bytes;
-  s->wt_valid = false;
+  s->wt_valid = false; s->wp_valid = false;
   return PULSE_OK;
 }
 extern "C" pulse_status_t pulse_stage_launch_count(const pulse_stage_t* s, uint64_t* n) {

@@ -26,7 +26,7 @@ struct ParamInfo {
 constexpr size_t NO_OFF = (size_t)-1;
 
 struct OpPlan {
-  int kind, cin, cskip, cout;
+  int kind, cin, cskip, cout, heads = 0;
   int hin, win, hout, wout;
   int x0 = -1, x1 = -1, out = -1;           // indices into Stage::tensors (activations)
   int a1 = -1, h1 = -1, a2 = -1, u = -1;    // stashed intermediates
@@ -34,6 +34,7 @@ struct OpPlan {
   size_t gp = 0;                            // R_WORK (zeroed area): [n][cout] fp32 pixel sums of g_h1
   size_t pn = 0;                            // byte offset in the slot stash ([n,cout] fp32)
   size_t mr1 = 0, mr2 = 0;                  // slot stash: [n][2][G] fp32 group mean / rstd of the GroupNorm sites
+  size_t lse = 0;                           // slot stash (attention): softmax statistics, attn_stats_floats() floats
   size_t wt1 = 0, wt2 = 0, wtsc = 0;        // R_WORK: flipped/transposed conv weights (kept across a wave)
   int p[12];                                // parameter indices (see stage.cu)
   int push = -1, pop = -1;
@@ -79,8 +80,9 @@ struct pulse_stage {
   size_t cst_begin = 0, cst_end = 0;        // slot stash: channel-stats area, zeroed at the start of forward
   size_t zero_begin = 0, zero_end = 0;      // workspace: backward sums area, zeroed at the start of backward
   bool wt_valid = false;                    // transposed weights match the bound parameters
+  bool wp_valid = false;                    // pre-summed phase weights of the up convs (forward) match them
   // per-stage workspace offsets (bytes)
-  size_t w_ga2 = 0, w_gh1 = 0, w_gh1b = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0;
+  size_t w_ga2 = 0, w_gh1 = 0, w_gh1b = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0, w_gqkv = 0;
   // weight-gradient kernels run on a side stream, concurrently with the dgrad / GroupNorm chain of the backward
   // (fork / join with events; legal inside CUDA-graph capture).  PULSE_NO_SIDE_STREAM=1 disables it.
   cudaStream_t side = nullptr;

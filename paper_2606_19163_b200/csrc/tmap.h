@@ -25,6 +25,8 @@ bool mat_map(const void* ptr, uint64_t rows, uint64_t k, int brows, CUtensorMap*
 bool tile_geometry(int gh, int gw, int& bw, int& bh, int& bn);
 bool tile_geometry64(int gh, int gw, int& bw, int& bh, int& bn);
 bool act_map_c(const void* ptr, int n, int h, int w, int c, int cbox, int bw, int bh, int bn, CUtensorMap* out);
+// the parity view with a (cbox, bw, 1, bh, bn) box; swizzle = 2 * cbox bytes
+bool act_map_s2_c(const void* ptr, int n, int h, int w, int c, int cbox, int bw, int bh, int bn, CUtensorMap* out);
 int sm_count();
 void set_error(const std::string& e);
 const std::string& last_error();

@@ -39,6 +39,8 @@ constexpr int SMEM = STAGES * STAGE + FLUSH_BYTES + 1024;
 
 struct Wg2Params {
   int units, c_blocks, c0_blocks, c0, ctot, ktot, s2;
+  int up2, gc;                           // up2: the conv of CONV_UP2 (kernels.h): units = (phase, tap, channel block), the
+                                         // gradient is read through its parity view (gc = its channel count)
   Tap taps[9];
   int bw, bh, bn, tiles_w, tiles_h;
   int pix_tiles, m_tiles, n_tiles;       // m_tiles: pair tiles of 4 units
@@ -91,7 +93,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       int ot = (int)(wb / p.pix_tiles), pt = (int)(wb - (long long)ot * p.pix_tiles);
       int tx = pt % p.tiles_w, ty = (pt / p.tiles_w) % p.tiles_h, tn = pt / (p.tiles_w * p.tiles_h);
       const int n_items = (int)(we - wb);
-      const CUtensorMap* ma[2]; int cch[2], adx[2], ady[2], apx[2], apy[2], co = 0;
+      const CUtensorMap* ma[2]; int cch[2], adx[2], ady[2], apx[2], apy[2], co = 0, gpx = 0, gpy = 0;
       bool new_tile = true;
       for (int it = 0; it < n_items; ++it) {
         if (new_tile) {
@@ -100,11 +102,16 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
           for (int b = 0; b < 2; ++b) {
             const int u = min(4 * mt + 2 * (int)rank + b, p.units - 1);
             const int ti = u / p.c_blocks, cb = u - ti * p.c_blocks;
-            const Tap t = p.taps[ti];
             const bool first = cb < p.c0_blocks;
             ma[b] = first ? &mapA0 : &mapA1;
             cch[b] = (first ? cb : cb - p.c0_blocks) * 64;
-            adx[b] = t.dx; ady[b] = t.dy; apx[b] = t.px; apy[b] = t.py;
+            if (!p.up2) {
+              const Tap t = p.taps[ti];
+              adx[b] = t.dx; ady[b] = t.dy; apx[b] = t.px; apy[b] = t.py;
+            } else {      // ti = 4 (2 py + px) + 2 a + b': low-resolution pixel (y + a - 1 + py, x + b' - 1 + px)
+              gpy = ti >> 3; gpx = (ti >> 2) & 1;
+              ady[b] = ((ti >> 1) & 1) - 1 + gpy; adx[b] = (ti & 1) - 1 + gpx; apx[b] = apy[b] = 0;
+            }
           }
           co = nt * N_TOT;
           new_tile = false;
@@ -120,9 +127,16 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
             if (!p.s2) tma2_load_4d(sa + b * BLK, ma[b], fb, cch[b], x0 + adx[b], y0 + ady[b], n0);
             else tma2_load_5d(sa + b * BLK, ma[b], fb, apx[b] * p.c0 + cch[b], x0 + adx[b], apy[b], y0 + ady[b], n0);
           }
-          tma2_load_4d(sa + 2 * BLK, &mapG, fb, co + (int)rank * 128, x0, y0, n0);
-          tma2_load_4d(sa + 3 * BLK, &mapG, fb, co + (int)rank * 128 + 64, x0, y0, n0);
-          tma2_load_4d(sa + 4 * BLK, &mapG32, fb, co + 256 + (int)rank * 32, x0, y0, n0);
+          if (!p.up2) {
+            tma2_load_4d(sa + 2 * BLK, &mapG, fb, co + (int)rank * 128, x0, y0, n0);
+            tma2_load_4d(sa + 3 * BLK, &mapG, fb, co + (int)rank * 128 + 64, x0, y0, n0);
+            tma2_load_4d(sa + 4 * BLK, &mapG32, fb, co + 256 + (int)rank * 32, x0, y0, n0);
+          } else {        // the pixels (2y + py, 2x + px) of the gradient: parity view (px gc + channel, x, py, y, n)
+            const int gco = gpx * p.gc + co;
+            tma2_load_5d(sa + 2 * BLK, &mapG, fb, gco + (int)rank * 128, x0, gpy, y0, n0);
+            tma2_load_5d(sa + 3 * BLK, &mapG, fb, gco + (int)rank * 128 + 64, x0, gpy, y0, n0);
+            tma2_load_5d(sa + 4 * BLK, &mapG32, fb, gco + 256 + (int)rank * 32, x0, gpy, y0, n0);
+          }
         }
         if (++stage == STAGES) { stage = 0; phase ^= 1; }
         if (++tx == p.tiles_w) { tx = 0; if (++ty == p.tiles_h) { ty = 0; ++tn; } }
@@ -191,7 +205,15 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       const int u = 4 * mt + 2 * (int)rank + (q >> 1);
       const bool valid = u < p.units;
       const int ti = valid ? u / p.c_blocks : 0, cb = valid ? u - ti * p.c_blocks : 0;
-      const int kcol = p.taps[ti].widx * p.ctot + cb * 64 + (q & 1) * 32;
+      const int kch = cb * 64 + (q & 1) * 32;
+      const int kcol = p.taps[p.up2 ? 0 : ti].widx * p.ctot + kch;
+      // up2: this unit's partial belongs to every (r, s) its pre-summed tap covers: rows r0..r1, columns s0..s1 of the 3x3
+      int r0 = 0, r1 = 0, s0 = 0, s1 = 0;
+      if (p.up2) {
+        const int py = ti >> 3, px = (ti >> 2) & 1, ta = (ti >> 1) & 1, tb = ti & 1;
+        r0 = (py == 0 && ta == 1) ? 1 : (py == 1 && ta == 1) ? 2 : 0; r1 = (py == 0 && ta == 0) ? 0 : (py == 1 && ta == 0) ? 1 : 2;
+        s0 = (px == 0 && tb == 1) ? 1 : (px == 1 && tb == 1) ? 2 : 0; s1 = (px == 0 && tb == 0) ? 0 : (px == 1 && tb == 0) ? 1 : 2;
+      }
       mbar_wait(&tfull_bar, tphase);
       tphase ^= 1;
       tc_fence_after();
@@ -220,7 +242,13 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            tma_reduce_add_2d(&mapW, stg + buf * 2048, kcol, nt * N_TOT + ch * 16);
+            if (!p.up2) {
+              tma_reduce_add_2d(&mapW, stg + buf * 2048, kcol, nt * N_TOT + ch * 16);
+            } else {
+              for (int r = r0; r <= r1; ++r)
+                for (int s_ = s0; s_ <= s1; ++s_)
+                  tma_reduce_add_2d(&mapW, stg + buf * 2048, (r * 3 + s_) * p.ctot + kch, nt * N_TOT + ch * 16);
+            }
             bulk_commit();
           }
           buf ^= 1;
@@ -244,23 +272,29 @@ bool wgrad_tc2_supported(const WgradArgs& a) {
   if (a.dt != DT_BF16) return false;
   if (a.src.c0 % 64 || a.src.c1 % 64 || a.src.c0 == 0 || a.cout % N_TOT) return false;
   if (a.ksize != 1 && a.ksize != 3) return false;
+  int bw, bh, bn;
+  if (a.up2) {
+    if (a.ksize != 3 || a.src.c1 || a.hout != 2 * a.hin || a.wout != 2 * a.win) return false;
+    return tile_geometry64(a.hin, a.win, bw, bh, bn);
+  }
   if (a.stride == 2) {
     if (a.ksize != 3 || a.src.c1 || (a.hin & 1) || (a.win & 1) || a.hout * 2 != a.hin || a.wout * 2 != a.win) return false;
   } else if (a.stride != 1 || a.hout != a.hin || a.wout != a.win) {
     return false;
   }
-  int bw, bh, bn;
   return tile_geometry64(a.hout, a.wout, bw, bh, bn);
 }
 
 int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   Wg2Params p;
   memset(&p, 0, sizeof p);
-  const bool s2 = a.stride == 2;
-  tile_geometry64(a.hout, a.wout, p.bw, p.bh, p.bn);
+  const bool s2 = !a.up2 && a.stride == 2;
+  const int gh = a.up2 ? a.hin : a.hout, gw = a.up2 ? a.win : a.wout;      // pixel grid of the K dimension
+  tile_geometry64(gh, gw, p.bw, p.bh, p.bn);
+  p.up2 = a.up2; p.gc = a.cout;
   p.c0 = a.src.c0; p.ctot = a.src.c(); p.c0_blocks = a.src.c0 / 64; p.c_blocks = p.ctot / 64; p.s2 = s2;
   const int taps = a.ksize * a.ksize, pad = (a.ksize - 1) / 2;
-  p.units = taps * p.c_blocks; p.ktot = taps * p.ctot;
+  p.units = (a.up2 ? 16 : taps) * p.c_blocks; p.ktot = taps * p.ctot;
   for (int r = 0; r < a.ksize; ++r)
     for (int s = 0; s < a.ksize; ++s) {
       Tap t; t.widx = r * a.ksize + s; t.px = t.py = 0;
@@ -268,7 +302,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
       else { t.dy = r == 0 ? -1 : 0; t.py = r == 1 ? 0 : 1; t.dx = s == 0 ? -1 : 0; t.px = s == 1 ? 0 : 1; }
       p.taps[t.widx] = t;
     }
-  p.tiles_w = a.wout / p.bw; p.tiles_h = (a.hout + p.bh - 1) / p.bh;
+  p.tiles_w = gw / p.bw; p.tiles_h = (gh + p.bh - 1) / p.bh;
   p.pix_tiles = p.tiles_w * p.tiles_h * ((a.n + p.bn - 1) / p.bn);
   p.m_tiles = (p.units + 3) / 4; p.n_tiles = a.cout / N_TOT;
   p.dw = a.dw;
@@ -278,8 +312,10 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   else ok = act_map(a.src.p0, a.n, a.hin, a.win, a.src.c0, p.bw, p.bh, p.bn, &m0);
   m1 = m0;
   if (ok && a.src.c1) ok = act_map(a.src.p1, a.n, a.hin, a.win, a.src.c1, p.bw, p.bh, p.bn, &m1);
-  if (ok) ok = act_map(a.g, a.n, a.hout, a.wout, a.cout, p.bw, p.bh, p.bn, &mg);
-  if (ok) ok = act_map_c(a.g, a.n, a.hout, a.wout, a.cout, 32, p.bw, p.bh, p.bn, &mg32);
+  if (ok && !a.up2) ok = act_map(a.g, a.n, a.hout, a.wout, a.cout, p.bw, p.bh, p.bn, &mg);
+  if (ok && !a.up2) ok = act_map_c(a.g, a.n, a.hout, a.wout, a.cout, 32, p.bw, p.bh, p.bn, &mg32);
+  if (ok && a.up2) ok = act_map_s2(a.g, a.n, a.hout, a.wout, a.cout, p.bw, p.bh, p.bn, &mg);
+  if (ok && a.up2) ok = act_map_s2_c(a.g, a.n, a.hout, a.wout, a.cout, 32, p.bw, p.bh, p.bn, &mg32);
   if (ok) ok = mat_map_f32(a.dw, a.cout, p.ktot, 32, 16, &mw);
   if (!ok) return -1;
   static bool attr_set = false;
@@ -306,7 +342,7 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
 static bool force_1cta_wgrad() { return toggles().wgrad_1cta; }
 bool wgrad_tc_any_supported(const WgradArgs& a) { return wgrad_tc2_supported(a) || wgrad_tc_supported(a); }
 int wgrad_tc_any(const WgradArgs& a, cudaStream_t st) {
-  if (!force_1cta_wgrad() && wgrad_tc2_supported(a)) return wgrad_tc2(a, st);
+  if ((!force_1cta_wgrad() || a.up2) && wgrad_tc2_supported(a)) return wgrad_tc2(a, st);
   return wgrad_tc(a, st);
 }
 

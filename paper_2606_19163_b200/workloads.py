@@ -15,11 +15,17 @@ from __future__ import annotations
 import copy
 import numpy as np
 
-CONV_IN, RESBLOCK, DOWN, UP, HEAD = "conv_in", "resblock", "down", "up", "head"
+CONV_IN, RESBLOCK, DOWN, UP, HEAD, ATTN = "conv_in", "resblock", "down", "up", "head", "attn"
 
 
-def _op(kind, cin, cout, skip=0, push=0):
-    return {"kind": kind, "cin": cin, "cout": cout, "skip": skip, "push": push}
+def _op(kind, cin, cout, skip=0, push=0, heads=0):
+    return {"kind": kind, "cin": cin, "cout": cout, "skip": skip, "push": push, "heads": heads}
+
+
+def attn(c, heads, push=0):
+    """Self-attention block on c channels: GN -> 1x1 conv to q|k|v -> attention per head over the
+    H W pixels -> 1x1 conv, + residual."""
+    return _op(ATTN, c, c, 0, push, heads)
 
 
 def rb(cin, cout, skip=0, push=0):
@@ -106,6 +112,14 @@ def mini(kind: str, dtype: str = "fp32") -> dict:
         d = _unet("mini_wave", 1, 8, [8, 16], dtype=dtype, groups=4, temb=mlp, c_lat=4)
         d["microbatches"] = 3
         return d
+    if kind == "attn":          # ResBlock + self-attention per block, skips pushed after the attention
+        return _stage("mini_attn", dtype, 2, 4, 4, 8, 4, mlp, "open", 1,
+                      [rb(8, 16), attn(16, 2, push=1), rb(16, 16), attn(16, 4, push=1)], [],
+                      [rb(16, 16, skip=16), attn(16, 2), rb(16, 16, skip=16), attn(16, 1), rb(16, 16, skip=8)])
+    if kind == "attn_unet":     # closed: attention in the mid block as well
+        d = _unet("mini_attn_unet", 2, 8, [8, 16], dtype=dtype, groups=4, temb=mlp, c_lat=4)
+        d["mid_ops"] = [rb(16, 16), attn(16, 2), rb(16, 16)]
+        return d
     raise ValueError(kind)
 
 
@@ -125,6 +139,10 @@ def gpu_mid(kind: str) -> dict:
                        _op(UP, 640, 640)])
     if kind == "unet":
         return _unet("mid_unet", 1, 32, [320, 640], temb=mlp)
+    if kind == "attn":          # SD-style level with attention: 320 channels = 5 heads x 64, 64 tokens per image, 192 pixels = 1.5 tiles
+        return _stage("mid_attn", "bf16", 3, 8, 8, 320, 32, mlp, "open", 1,
+                      [rb(320, 320), attn(320, 5, push=1), rb(320, 320), attn(320, 5, push=1)], [],
+                      [rb(320, 320, skip=320), attn(320, 5), rb(320, 320, skip=320), attn(320, 5), rb(320, 320, skip=320)])
     raise ValueError(kind)
 
 
@@ -190,6 +208,10 @@ def param_specs(desc) -> list:
                     specs += [(p + "sc.w", (co, ci, 1, 1), "weight", ci), (p + "sc.b", (co,), "bias", 0)]
             elif k in (CONV_IN, DOWN, UP):
                 specs += [(p + "conv.w", (co, ci, 3, 3), "weight", ci * 9), (p + "conv.b", (co,), "bias", 0)]
+            elif k == ATTN:
+                specs += [(p + "gn.gamma", (ci,), "gamma", 0), (p + "gn.beta", (ci,), "beta", 0),
+                          (p + "qkv.w", (3 * ci, ci, 1, 1), "weight", ci), (p + "qkv.b", (3 * ci,), "bias", 0),
+                          (p + "proj.w", (ci, ci, 1, 1), "weight", ci), (p + "proj.b", (ci,), "bias", 0)]
             elif k == HEAD:
                 specs += [(p + "gn.gamma", (ci,), "gamma", 0), (p + "gn.beta", (ci,), "beta", 0),
                           (p + "conv.w", (co, ci, 3, 3), "weight", ci * 9), (p + "conv.b", (co,), "bias", 0)]

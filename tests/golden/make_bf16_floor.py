@@ -30,9 +30,9 @@ LIST_ABOVE = 1e-2
 
 # name -> (structure, seed, with_g_e_out, oracle dtype): exactly what tests/test_gpu_parity.py runs
 CASES = {}
-for kind in ("level", "updown", "unet", "wave"):
+for kind in ("level", "updown", "unet", "wave", "attn", "attn_unet"):
     CASES[f"mini_{kind}"] = (W.mini(kind, "bf16"), 1, True, torch.float64)
-for kind in ("level", "updown", "unet"):
+for kind in ("level", "updown", "unet", "attn"):
     CASES[f"mid_{kind}"] = (W.gpu_mid(kind), 2, kind != "unet", torch.float64)
 CASES["mini_updown@2"] = (W.mini("updown", "bf16"), 2, True, torch.float64)
 CASES["mid_level_1f1b"] = (W.scaled(W.gpu_mid("level"), microbatches=3, name="mid_level_1f1b"), 4, False, torch.float64)

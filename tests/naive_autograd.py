@@ -31,6 +31,16 @@ def _rb(desc, P, p, x, emb):
     return h + sc
 
 
+def _attn(desc, P, p, x, heads):
+    """Self-attention block from library pieces: F.group_norm, 1x1 convs, F.scaled_dot_product_attention."""
+    n, c, h, w = x.shape
+    qkv = F.conv2d(F.group_norm(x, desc["groups"], P[p + "gn.gamma"], P[p + "gn.beta"], desc["eps"]), P[p + "qkv.w"], P[p + "qkv.b"])
+    q, k, v = (t.reshape(n, heads, c // heads, h * w).transpose(2, 3) for t in qkv.chunk(3, dim=1))    # [n, heads, T, d]
+    o = F.scaled_dot_product_attention(q, k, v)
+    o = o.transpose(2, 3).reshape(n, c, h, w)
+    return x + F.conv2d(o, P[p + "proj.w"], P[p + "proj.b"])
+
+
 def _enc_prefix(desc, P, x_in, emb, upto_push):
     """Recompute the encoder from x_in until push number `upto_push` exists; return it."""
     k = 0
@@ -43,6 +53,8 @@ def _enc_prefix(desc, P, x_in, emb, upto_push):
         p = f"enc{i}."
         if op["kind"] == "resblock":
             x = _rb(desc, P, p, x, emb)
+        elif op["kind"] == "attn":
+            x = _attn(desc, P, p, x, op["heads"])
         else:
             x = F.conv2d(x, P[p + "conv.w"], P[p + "conv.b"], stride=2 if op["kind"] == "down" else 1, padding=1)
         if op["push"]:
@@ -66,8 +78,8 @@ def run(desc, params, mb, loss_scale=1.0, extra_e_loss=False):
     e_last = _enc_prefix(desc, P, x_in, emb, None)
     if desc["link"] == "closed":
         h = e_last
-        for i in range(len(desc["mid_ops"])):
-            h = _rb(desc, P, f"mid{i}.", h, emb)
+        for i, op in enumerate(desc["mid_ops"]):
+            h = _attn(desc, P, f"mid{i}.", h, op["heads"]) if op["kind"] == "attn" else _rb(desc, P, f"mid{i}.", h, emb)
     else:
         h = h_in
     top = n_push
@@ -77,6 +89,8 @@ def run(desc, params, mb, loss_scale=1.0, extra_e_loss=False):
             top -= 1
             skip = _enc_prefix(desc, P, x_in, emb, top)      # recomputed, never cached
             h = _rb(desc, P, p, torch.cat([h, skip], 1), emb)
+        elif op["kind"] == "attn":
+            h = _attn(desc, P, p, h, op["heads"])
         elif op["kind"] == "up":
             h = F.conv2d(F.interpolate(h, scale_factor=2, mode="nearest"), P[p + "conv.w"], P[p + "conv.b"], padding=1)
         else:

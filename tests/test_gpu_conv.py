@@ -148,3 +148,93 @@ def test_conv_wgrad(case, simt):
     rms = float(ref.pow(2).mean().sqrt())
     err = float((got - ref).abs().max())
     assert err <= 1e-4 * rms * 10, f"wgrad {case} simt={simt}: max err {err:.3e} vs rms {rms:.3e}"   # fp32 sums of exact products
+
+
+# ------------------------------------------------------------------ nearest-2x upsample + conv, 4-phase form (row a6)
+UP_CASES = [
+    # n, h, w (low resolution), cin, cout
+    (2, 8, 8, 64, 320),          # 128 low-res pixels: one tile, image box
+    (3, 8, 8, 128, 160),         # 192 pixels: ragged tile, image box beyond N
+    (1, 16, 16, 64, 640),        # two N tiles
+    (3, 16, 16, 128, 320),       # 6 M tiles
+    (1, 24, 16, 64, 320),        # 3 M tiles: odd count
+    (2, 32, 32, 64, 320),        # configs[2]'s up: 32x32 -> 64x64
+]
+
+
+def phase_form(x, wt, bias, round_weights):
+    """The 4-phase identity written out on the CPU (fp64): out[2y+py, 2x+px] = sum_{a,b} Wp[py,px][a,b] x[y+a-1+py, x+b-1+px],
+    Wp = sum of W[r][s] over r in R(py,a), s in R(px,b); round_weights: Wp rounded to bf16 as the kernels hold it."""
+    R = {(0, 0): [0], (0, 1): [1, 2], (1, 0): [0, 1], (1, 1): [2]}
+    n, c, h, w = x.shape
+    xp = torch.nn.functional.pad(x, (1, 1, 1, 1))
+    out = torch.zeros((n, wt.shape[0], 2 * h, 2 * w), dtype=torch.float64)
+    for py in range(2):
+        for px in range(2):
+            acc = torch.zeros((n, wt.shape[0], h, w), dtype=torch.float64)
+            for a in range(2):
+                for b in range(2):
+                    wp = sum(wt[:, :, r, s_] for r in R[(py, a)] for s_ in R[(px, b)])
+                    if round_weights:
+                        wp = wp.float().to(torch.bfloat16).double()
+                    dy, dx = a - 1 + py, b - 1 + px
+                    acc += torch.einsum("oc,nchw->nohw", wp, xp[:, :, 1 + dy:1 + dy + h, 1 + dx:1 + dx + w])
+            out[:, :, py::2, px::2] = acc + (0 if bias is None else bias.view(1, -1, 1, 1))
+    return out
+
+
+def test_phase_form_is_the_upsample_conv_identity():
+    """No GPU needed in principle (kept here beside its use): with exact weights the 4-phase form IS conv3x3(upsample2(x))."""
+    rng = np.random.default_rng(11)
+    x, wt, b = (torch.as_tensor(rng.standard_normal(s)) for s in ((2, 3, 4, 5), (6, 3, 3, 3), (6,)))
+    assert torch.allclose(phase_form(x, wt, b, False), O.conv_fwd(O.upsample2(x), wt, b), atol=1e-12)
+
+
+@pytest.mark.parametrize("kernel", ["pair", "1cta"])
+@pytest.mark.parametrize("case", UP_CASES)
+def test_upsample_conv_fprop_dgrad(case, kernel):
+    """The 4-phase form against the oracle's definition conv3x3(upsample2(x)) and its adjoint
+    upsample2_bwd(conv_dgrad(g)).  The kernels hold the pre-summed weights in bf16: one rounding of the WEIGHTS (2^-9
+    relative per product; it does not average out of the K = 4 c sum the way independent operand errors would), measured
+    as <= 1e-2 x RMS max-abs = the size of one bf16 store of the output.  Against the same identity with the weights
+    rounded the same way the kernels must be as tight as every other conv (2e-3)."""
+    B = _B()
+    n, h, w, cin, cout = case
+    rng = np.random.default_rng(hash(case) % 2 ** 31)
+    x = grid(rng, n, cin, h, w)
+    wt = grid(rng, cout, cin, 3, 3, scale=(2.0 / (cin * 9)) ** 0.5)
+    bias = grid(rng, cout, scale=0.1)
+    ref = O.conv_fwd(O.upsample2(torch.as_tensor(x).double()), torch.as_tensor(wt).double(), torch.as_tensor(bias).double())
+    cst = torch.zeros((n, 2, cout), dtype=torch.float32, device="cuda")
+    got = _or_skip(B, lambda: B.upsample_conv2d(dev_nhwc(x), dev_w(wt), torch.as_tensor(bias).to("cuda", torch.bfloat16),
+                                                kernel=kernel, chan_stats=cst))
+    torch.cuda.synchronize()
+    assert_bf16_close(B.nchw(got), ref, f"up fprop {case} kernel={kernel}", acc_tol=1e-2)
+    ref_q = phase_form(torch.as_tensor(x).double(), torch.as_tensor(wt).double(), torch.as_tensor(bias).double(), True)
+    assert_bf16_close(B.nchw(got), ref_q, f"up fprop (rounded phase weights) {case} kernel={kernel}")
+    stored = got.double()
+    want = torch.stack([stored.sum((1, 2)), stored.pow(2).sum((1, 2))], 1).cpu()
+    assert float((cst.double().cpu() - want).abs().max()) <= 1e-4 * float(want[:, 1].abs().max()) + 1e-3
+    g = grid(rng, n, cout, 2 * h, 2 * w)
+    ref_g = O.upsample2_bwd(O.conv_dgrad(torch.as_tensor(g).double(), torch.as_tensor(wt).double(), (2 * h, 2 * w)))
+    got_g = _or_skip(B, lambda: B.upsample_conv2d_dgrad(dev_nhwc(g), dev_w(wt), kernel=kernel))
+    torch.cuda.synchronize()
+    assert_bf16_close(B.nchw(got_g), ref_g, f"up dgrad {case} kernel={kernel}", acc_tol=1e-2)
+    # adjoint of the rounded-weight phase form, by autograd of the CPU identity above (fp64)
+    xg = torch.zeros((n, cin, h, w), dtype=torch.float64, requires_grad=True)
+    (phase_form(xg, torch.as_tensor(wt).double(), None, True) * torch.as_tensor(g).double()).sum().backward()
+    assert_bf16_close(B.nchw(got_g), xg.grad, f"up dgrad (rounded phase weights) {case} kernel={kernel}")
+
+
+@pytest.mark.parametrize("case", [c for c in UP_CASES if c[4] % 320 == 0])
+def test_upsample_conv_wgrad(case):
+    B = _B()
+    n, h, w, cin, cout = case
+    rng = np.random.default_rng(hash(case) % 2 ** 31 + 1)
+    x, g = grid(rng, n, cin, h, w), grid(rng, n, cout, 2 * h, 2 * w)
+    ref, _ = O.conv_wgrad(O.upsample2(torch.as_tensor(x).double()), torch.as_tensor(g).double(), (cout, cin, 3, 3))
+    got = B.upsample_conv2d_wgrad(dev_nhwc(x), dev_nhwc(g)).permute(0, 3, 1, 2).double().cpu()
+    torch.cuda.synchronize()
+    rms = float(ref.pow(2).mean().sqrt())
+    err = float((got - ref).abs().max())
+    assert err <= 1e-3 * rms, f"up wgrad {case}: max err {err:.3e} vs rms {rms:.3e}"      # fp32 sums of exact bf16 products

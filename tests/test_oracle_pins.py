@@ -192,7 +192,7 @@ def test_sinusoidal_and_upsample():
 
 # ------------------------------------------------------------------ whole stage
 
-KINDS = ["pair", "level", "updown", "straddle", "unet"]
+KINDS = ["pair", "level", "updown", "straddle", "unet", "attn", "attn_unet"]
 
 
 @pytest.mark.parametrize("kind", KINDS)
@@ -214,7 +214,7 @@ def test_stage_matches_naive_recompute_autograd(kind):
     assert set(r["param_grads"]) == set(ref["param_grads"])
 
 
-@pytest.mark.parametrize("kind", ["updown", "unet"])
+@pytest.mark.parametrize("kind", ["updown", "unet", "attn"])
 def test_stage_central_differences(kind):
     """fp64 central finite differences along random directions, every input and parameter
     tensor, rel err <= 1e-3 (BASELINE.json north_star)."""
@@ -331,6 +331,8 @@ def _store_point_count(desc):
                 n += 3
             elif op["kind"] == "head":
                 n += 4
+            elif op["kind"] == "attn":
+                n += 8          # xn, qkv, o, out; g_o, g_qkv, g_xn; the input gradient
     return n
 
 
@@ -383,7 +385,7 @@ def test_st_is_round_to_nearest_even_and_idempotent():
 @pytest.mark.parametrize("kind", KINDS + ["wave"])
 def test_float32_instantiation_matches_float64(kind):
     """The float32 oracle (used for configs 3-5 on the GPU box to bound the test time) against the pinned float64
-    one: max |err| <= 3e-5 x RMS per tensor (measured <= 1.4e-5 on these structures: fp32 rounding 6e-8 through ~40
+    one: max |err| <= 5e-5 x RMS per tensor (measured <= 3.6e-5 on these structures: fp32 rounding 6e-8 through 40-100
     operators in series with sums of 10^2-10^3 terms), three orders below the bf16 bar it serves and below north_star's own
     1e-4 bar for an fp32 evaluation of the stage."""
     desc = W.mini(kind)
@@ -408,7 +410,7 @@ def test_float32_instantiation_matches_float64(kind):
     for k, v in a.items():
         assert b[k].dtype == torch.float32, k
         rms = max(float(v.pow(2).mean().sqrt()), 1e-30)
-        assert float((b[k].to(D) - v).abs().max()) <= 3e-5 * rms, (k, float((b[k].to(D) - v).abs().max()) / rms)
+        assert float((b[k].to(D) - v).abs().max()) <= 5e-5 * rms, (k, float((b[k].to(D) - v).abs().max()) / rms)
 
 
 def test_one_bf16_store_of_a_config2_tensor_is_at_the_bar():
@@ -425,3 +427,80 @@ def test_one_bf16_store_of_a_config2_tensor_is_at_the_bar():
         e2 = float((y - x).abs().max()) / rms
     assert 1.4e-2 < e1 <= 2.0 ** -8 * float(x.abs().max()) / rms
     assert e2 > 2e-2
+
+
+# ------------------------------------------------------------------ attention
+
+def test_attention_core_matches_brute_force_and_closed_forms():
+    B_, T, d = 3, 7, 5
+    q, k, v = rnd(B_, T, d), rnd(B_, T, d), rnd(B_, T, d)
+    o, p = O.attn_core_fwd(q, k, v)
+    # the definition as loops: o[b,i] = sum_j softmax_j(q_i . k_j / sqrt(d)) v_j
+    want = torch.zeros(B_, T, d, dtype=D)
+    for b, i in itertools.product(range(B_), range(T)):
+        e = [math.exp(sum(q[b, i, c].item() * k[b, j, c].item() for c in range(d)) / math.sqrt(d)) for j in range(T)]
+        z = sum(e)
+        for j in range(T):
+            want[b, i] += (e[j] / z) * v[b, j]
+    assert torch.allclose(o, want, atol=1e-12)
+    assert torch.allclose(p.sum(2), torch.ones(B_, T, dtype=D), atol=1e-14) and (p > 0).all()       # rows sum to 1
+    # permuting keys and values together changes nothing; permuting queries permutes the output rows
+    perm = torch.randperm(T)
+    assert torch.allclose(O.attn_core_fwd(q, k[:, perm], v[:, perm])[0], o, atol=1e-12)
+    assert torch.allclose(O.attn_core_fwd(q[:, perm], k, v)[0], o[:, perm], atol=1e-12)
+    # equal keys -> uniform weights -> the mean of v; one dominant key -> its value
+    ku = k[:, :1].expand(B_, T, d)
+    assert torch.allclose(O.attn_core_fwd(q, ku, v)[0], v.mean(1, keepdim=True).expand(B_, T, d), atol=1e-12)
+    kb = torch.zeros(B_, T, d, dtype=D)
+    kb[:, 2] = 200.0 * torch.sign(q[:, 0])                   # query 0 sees key 2 with score >> all others
+    assert torch.allclose(O.attn_core_fwd(q, kb, v)[0][:, 0], v[:, 2], atol=1e-9)
+    # shift invariance of softmax: adding a constant vector to every key's score (q . c) changes nothing
+    assert torch.allclose(O.attn_core_fwd(q, k + 3.0, v)[0], o, atol=1e-10)
+    # the library routine
+    assert torch.allclose(o, torch.nn.functional.scaled_dot_product_attention(q, k, v), atol=1e-12)
+
+
+def test_attention_core_backward_finite_differences_and_autograd():
+    B_, T, d = 2, 6, 4
+    q, k, v, g = rnd(B_, T, d), rnd(B_, T, d), rnd(B_, T, d), rnd(B_, T, d)
+    o, p = O.attn_core_fwd(q, k, v)
+    g_q, g_k, g_v = O.attn_core_bwd(g, q, k, v, p)
+    qa, ka, va = (t.clone().requires_grad_(True) for t in (q, k, v))
+    (torch.nn.functional.scaled_dot_product_attention(qa, ka, va) * g).sum().backward()
+    assert torch.allclose(g_q, qa.grad, atol=1e-11) and torch.allclose(g_k, ka.grad, atol=1e-11)
+    assert torch.allclose(g_v, va.grad, atol=1e-11)
+    eps = 1e-6
+    for name, t, an in (("q", q, g_q), ("k", k, g_k), ("v", v, g_v)):
+        dirn = rnd(B_, T, d)
+        args = {"q": q, "k": k, "v": v}
+        plus, minus = dict(args), dict(args)
+        plus[name], minus[name] = t + eps * dirn, t - eps * dirn
+        fd = ((O.attn_core_fwd(**plus)[0] - O.attn_core_fwd(**minus)[0]) * g).sum() / (2 * eps)
+        assert abs(fd - (an * dirn).sum()) <= 1e-6 * max(1.0, abs(fd)), name
+    # softmax Jacobian: the score gradient of every query row sums to zero -> g_q, g_k are invariant to adding a constant to g_P
+    assert torch.allclose(O.attn_core_bwd(g, q, k, v, p)[0], g_q)
+
+
+def test_plain_groupnorm_matches_library_autograd():
+    n, c, G, eps = 2, 12, 4, 1e-5
+    x, gamma, beta, g_y = rnd(n, c, 3, 5) * 2 + 1, rnd(c), rnd(c), rnd(n, c, 3, 5)
+    y, ctx = O.gn_fwd(x, gamma, beta, G, eps)
+    g_x, dg, db = O.gn_bwd(g_y, ctx, gamma)
+    xr, gr, br = (t.clone().requires_grad_(True) for t in (x, gamma, beta))
+    yr = torch.nn.functional.group_norm(xr, G, gr, br, eps)
+    yr.backward(g_y)
+    assert torch.allclose(y, yr.detach(), atol=1e-12) and torch.allclose(g_x, xr.grad, atol=1e-10)
+    assert torch.allclose(dg, gr.grad, atol=1e-10) and torch.allclose(db, br.grad, atol=1e-10)
+    # same statistics as the fused GroupNorm + SiLU: a = SiLU(y)
+    a, _ = O.gn_silu_fwd(x, gamma, beta, G, eps)
+    assert torch.allclose(a, O.silu(y), atol=1e-12)
+
+
+def test_attention_heads_layout():
+    """Head h owns channels [h d, (h+1) d); tokens are pixels in row-major order (reading R24)."""
+    n, heads, d, h, w = 2, 3, 4, 2, 5
+    x = rnd(n, heads * d, h, w)
+    t = O._heads(x, heads)
+    assert t.shape == (n * heads, h * w, d)
+    assert torch.equal(t[1 * heads + 2, 1 * w + 3], x[1, 2 * d:3 * d, 1, 3])
+    assert torch.equal(O._unheads(t, n, heads, h, w), x)
