@@ -434,6 +434,43 @@ def main():
             sys.stderr.write(f"bench: stand-alone GroupNorm timing skipped ({ex})\n")
             gn_alone = None
 
+    # ---- the attention core alone at the level-2 shape of configs[2] (8 images, 32 x 32 tokens, 640
+    # channels = 10 heads x 64): tcgen05 forward, CUDA-core forward and backward.  FLOPs: forward 4 n T^2 C, backward 10 n T^2 C;
+    # the forward's roofline is the exponential: n heads T^2 MUFU.EX2 at 16 per clock per SM
+    attn_alone = None
+    if rank == 0 and desc["dtype"] == "bf16":
+        try:
+            an, aT, aC, ah = 8, 1024, 640, 10
+            gen = torch.Generator(device="cuda").manual_seed(3)
+            aq = torch.randn((an, aT, 3 * aC), device="cuda", generator=gen).to(torch.bfloat16)
+            ago = torch.randn((an, aT, aC), device="cuda", generator=gen).to(torch.bfloat16)
+            _, ast = B.attention(aq, ah)
+
+            def timed(fn, reps):
+                fn(); torch.cuda.synchronize()
+                a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a0.record()
+                for _ in range(reps):
+                    fn()
+                a1.record()
+                torch.cuda.synchronize()
+                return a0.elapsed_time(a1) * 1e3 / reps
+            f_tc = timed(lambda: B.attention(aq, ah), 20)
+            f_simt = timed(lambda: B.attention(aq, ah, force_simt=True), 3)
+            b_tc = timed(lambda: B.attention_backward(aq, ago, ah, ast), 20)
+            b_simt = timed(lambda: B.attention_backward(aq, ago, ah, ast, force_simt=True), 3)
+            ffl, bfl = 4.0 * an * aT * aT * aC, 10.0 * an * aT * aT * aC
+            sm_clk = 148 * 16 * 1.9e9          # MUFU lanes per second at 1.9 GHz (B200_PROFILING.md unit counts)
+            attn_alone = {"shape": f"n={an}, tokens={aT}, channels={aC}, heads={ah}",
+                          "fwd_tcgen05": {"us": f_tc, "tflops": ffl / (f_tc * 1e-6) / 1e12, "bound": "alu (MUFU.EX2)",
+                                          "frac_of_exp_peak": an * ah * aT * aT / (f_tc * 1e-6) / sm_clk},
+                          "fwd_cuda_core": {"us": f_simt, "tflops": ffl / (f_simt * 1e-6) / 1e12},
+                          "bwd_tcgen05": {"us": b_tc, "tflops": bfl / (b_tc * 1e-6) / 1e12, "bound": "alu (MUFU.EX2)",
+                                          "frac_of_exp_peak": 3.0 * an * ah * aT * aT / (b_tc * 1e-6) / sm_clk},
+                          "bwd_cuda_core": {"us": b_simt, "tflops": bfl / (b_simt * 1e-6) / 1e12}}
+        except Exception as ex:
+            sys.stderr.write(f"bench: stand-alone attention timing skipped ({ex})\n")
+
     # ---- end to end through the public API with HOST buffers -----------------------------------------------
     host = []
     for mb in data["microbatches"]:
@@ -611,7 +648,7 @@ def main():
             "frac_of_bf16_peak_nominal_2250": tflops / world / 2250.0,
             "frac_of_bf16_peak_measured": tflops / world / tf_burst, "peak_measured": tf_burst,
             "clocks": clocks, "gpu_launches": int(launches_per_step * K), "roofline": roofline,
-            "kernels": kern, "gn_alone": gn_alone, "eager_ms_per_step": eager_ms, "loss": last_loss,
+            "kernels": kern, "gn_alone": gn_alone, "attn_alone": attn_alone, "eager_ms_per_step": eager_ms, "loss": last_loss,
             "e2e": {"value": world * samples / e2e_s, "unit": "samples/s", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
                     "d2h": "e_out, d_out, g_x_in, g_h_in of every microbatch and the loss, into pinned host buffers; the fp32 weight gradients stay on the device (optimizer state)",

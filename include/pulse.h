@@ -242,12 +242,15 @@ pulse_status_t pulse_upsample_conv2d_wgrad(int dtype, const void* d_src, int n, 
  * d_qkv [n][tokens][3c]: q | k | v interleaved per token as the 1x1 conv leaves them (head h = channels [h d, (h+1) d)
  * of each third); d_o, d_g_o [n][tokens][c]; d_g_qkv as d_qkv (written).  d_stats: pulse_attention_stats_floats(n,
  * heads, tokens) fp32, written by the forward (log-sum-exp per query) and the backward, kept between the two.
- * CUDA-core fp32 arithmetic on fp32 or bf16 storage; the T x T matrix is never written; no atomics. */
+ * The T x T matrix is never written; no atomics.  bf16 tensors with 64 or 128 channels per head take the tcgen05
+ * kernels (Q K^T, P V and the five products of the backward on the tensor cores, softmax and its Jacobian in fp32 on the
+ * TMEM accumulator rows, P / g_S handed over as bf16) unless force_simt != 0; everything else takes CUDA-core kernels
+ * with fp32 arithmetic on fp32 or bf16 storage. */
 size_t pulse_attention_stats_floats(int n, int heads, int tokens);
-pulse_status_t pulse_attention(int dtype, const void* d_qkv, int n, int tokens, int c, int heads, void* d_o, float* d_stats,
-                               void* stream);
-pulse_status_t pulse_attention_backward(int dtype, const void* d_qkv, const void* d_g_o, int n, int tokens, int c, int heads,
-                                        float* d_stats, void* d_g_qkv, void* stream);
+pulse_status_t pulse_attention(int dtype, int force_simt, const void* d_qkv, int n, int tokens, int c, int heads, void* d_o,
+                               float* d_stats, void* stream);
+pulse_status_t pulse_attention_backward(int dtype, int force_simt, const void* d_qkv, const void* d_g_o, int n, int tokens,
+                                        int c, int heads, float* d_stats, void* d_g_qkv, void* stream);
 
 /* GroupNorm + SiLU in isolation (the kernels of rows a2/a5 and a8/a9), on
  * x = concat_C(x0[c0], x1[c1]) (x1 may be NULL with c1 = 0), NHWC, C = c0 + c1 divisible by groups

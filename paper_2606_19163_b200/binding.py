@@ -84,8 +84,8 @@ _SIG = {
     "pulse_upsample_conv2d": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp, _vp, _vp, _vp],
     "pulse_upsample_conv2d_dgrad": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp, _vp],
     "pulse_upsample_conv2d_wgrad": [C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp],
-    "pulse_attention": [C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp],
-    "pulse_attention_backward": [C.c_int, _vp, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp],
+    "pulse_attention": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp],
+    "pulse_attention_backward": [C.c_int, C.c_int, _vp, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp],
     "pulse_groupnorm_silu": [C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, _vp, _vp,
                              _vp, C.c_int, _vp, _vp],
     "pulse_groupnorm_silu_backward": [C.c_int, C.c_int, C.c_int, _vp, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int,
@@ -429,21 +429,21 @@ def upsample_conv2d_wgrad(src, g):
     return dw
 
 
-def attention(qkv, heads):
+def attention(qkv, heads, force_simt=False):
     """qkv [n, tokens, 3c] -> (o [n, tokens, c], stats)."""
     n, t, c3 = qkv.shape
     c = c3 // 3
     o = torch.empty((n, t, c), dtype=qkv.dtype, device=qkv.device)
     stats = torch.empty(lib.pulse_attention_stats_floats(n, heads, t), dtype=torch.float32, device=qkv.device)
-    _ck(lib.pulse_attention(_cd(qkv), _ptr(qkv), n, t, c, heads, _ptr(o), _ptr(stats), _stream()))
+    _ck(lib.pulse_attention(_cd(qkv), int(force_simt), _ptr(qkv), n, t, c, heads, _ptr(o), _ptr(stats), _stream()))
     return o, stats
 
 
-def attention_backward(qkv, g_o, heads, stats):
+def attention_backward(qkv, g_o, heads, stats, force_simt=False):
     n, t, c3 = qkv.shape
     g_qkv = torch.empty_like(qkv)
-    _ck(lib.pulse_attention_backward(_cd(qkv), _ptr(qkv), _ptr(g_o), n, t, c3 // 3, heads, _ptr(stats), _ptr(g_qkv),
-                                     _stream()))
+    _ck(lib.pulse_attention_backward(_cd(qkv), int(force_simt), _ptr(qkv), _ptr(g_o), n, t, c3 // 3, heads, _ptr(stats),
+                                     _ptr(g_qkv), _stream()))
     return g_qkv
 
 

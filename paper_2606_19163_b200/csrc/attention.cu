@@ -322,7 +322,8 @@ template <typename K> void big_smem(K kernel, size_t bytes) {
 bool attn_supported(int C, int heads) { return heads > 0 && C % heads == 0 && C / heads <= 16 * MAXJ; }
 size_t attn_stats_floats(int n, int heads, int T) { return (size_t)2 * n * heads * T; }
 
-int attn_fwd(int dt, const void* qkv, int n, int T, int C, int heads, void* o, float* lse, cudaStream_t st) {
+int attn_fwd(int dt, const void* qkv, int n, int T, int C, int heads, void* o, float* lse, cudaStream_t st, bool use_tc) {
+  if (use_tc && attn_fwd_tc_supported(dt, C, heads)) return attn_fwd_tc(qkv, n, T, C, heads, o, lse, st);
   AttnP p{};
   p.qkv = qkv; p.out_o = o; p.lse = lse; p.T = T; p.C = C; p.heads = heads; p.d = C / heads; p.scale = 1.0f / sqrtf((float)p.d);
   dim3 grid((T + BT - 1) / BT, heads, n);
@@ -333,7 +334,8 @@ int attn_fwd(int dt, const void* qkv, int n, int T, int C, int heads, void* o, f
 }
 
 int attn_bwd(int dt, const void* qkv, const void* g_o, int n, int T, int C, int heads, float* lse, void* g_qkv,
-             cudaStream_t st) {
+             cudaStream_t st, bool use_tc) {
+  if (use_tc && attn_fwd_tc_supported(dt, C, heads)) return attn_bwd_tc(qkv, g_o, n, T, C, heads, lse, g_qkv, st);
   AttnP p{};
   p.qkv = qkv; p.g_o = g_o; p.g_qkv = g_qkv; p.lse = lse; p.T = T; p.C = C; p.heads = heads; p.d = C / heads;
   p.scale = 1.0f / sqrtf((float)p.d);

@@ -1,0 +1,564 @@
+// attention_tc.cu - tcgen05 forward of the attention core for bf16 tensors with 64 or 128 channels per head
+// (formulas in attention.cu).  One CTA = 128 queries of one (image, head); thread i owns query
+// row i = TMEM lane i, so the softmax needs no cross-thread reduction:
+//   sweep 1 over the key tiles:  S = Q K^T (tcgen05.mma, M = 128, N = 128, K = d, both operands K-major from TMA boxes
+//                                of the interleaved qkv tensor) -> TMEM -> row maximum m_i
+//   sweep 2:                     S again -> p = 2^((s - m_i) scale log2 e) -> l_i += p, P as bf16 into a 128-byte-swizzled
+//                                A-operand tile -> O += P V (V is read MN-major, straight from its [keys][d] box) in TMEM
+//   epilogue:                    o_i = O_i / l_i -> bf16 -> global; log-sum-exp_i = m_i scale + ln l_i for the backward.
+// Two sweeps instead of the online rescale: O lives in tensor memory, where a rescale per key tile would cost a TMEM
+// round trip of the whole accumulator; the second Q K^T is 1/3 more MMA work on a kernel whose bound is the exponential
+// (128 x 128 MUFU ops per tile = 1024 cycles against 512 of MMA).
+#include <cuda.h>
+
+#include "common.cuh"
+#include "kernels.h"
+#include "sm100.cuh"
+#include "tmap.h"
+
+namespace pulse {
+
+namespace {
+
+using namespace sm100;
+
+constexpr int BQ = 128, BKEY = 128;
+constexpr int CH = BQ * 128;                    // one [128 rows][64 bf16] chunk: 16 KB
+
+template <int D> struct ACfg {
+  static constexpr int NC = D / 64;             // 64-channel chunks per row
+  static constexpr int Q_OFF = 0, K_OFF = NC * CH, V_OFF = 2 * NC * CH, P_OFF = 3 * NC * CH;
+  static constexpr int SMEM = 3 * NC * CH + 2 * CH + 1024;
+  static constexpr int TMEM_COLS = 256;         // S: columns [0, 128), O: [128, 128 + D)
+};
+
+struct AtcP { int T, C, heads; float scale; bf16* o; float* lse; };
+
+template <int D>
+__global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ CUtensorMap map, const AtcP p) {
+  using A = ACfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t bar_q, bar_kv, bar_s, bar_pv;
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, row = threadIdx.x;
+  const int q0 = blockIdx.x * BQ, h = blockIdx.y, n = blockIdx.z;
+  const int nkb = (p.T + BKEY - 1) / BKEY;
+  if (threadIdx.x == 0) {
+    prefetch_tmap(&map);
+    mbar_init(&bar_q, 1); mbar_init(&bar_kv, 1); mbar_init(&bar_s, 1); mbar_init(&bar_pv, 1);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(&tmem_base_s, A::TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+  pdl_wait();
+  pdl_launch_dependents();
+
+  constexpr uint64_t dk = smem_desc_sw128(16, 1024);            // K-major operand: 128-byte rows, 8-row atoms
+  constexpr uint64_t dmn = smem_desc_sw128(CH, 1024);           // MN-major operand (V): LBO = next 64-channel chunk
+  constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_o = idesc_bf16(BQ, D, 0, 1);
+  const uint32_t sb = smem_u32(smem);
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(&bar_q, A::NC * CH);
+    for (int c = 0; c < A::NC; ++c) tma_load_3d(smem + A::Q_OFF + c * CH, &map, &bar_q, h * D + 64 * c, q0, n);
+  }
+  uint32_t ph_kv = 0, ph_s = 0, ph_pv = 0;
+  auto load_kv = [&](int kb, bool with_v) {                      // thread 0
+    mbar_expect_tx(&bar_kv, (with_v ? 2 : 1) * A::NC * CH);
+    for (int c = 0; c < A::NC; ++c) {
+      tma_load_3d(smem + A::K_OFF + c * CH, &map, &bar_kv, p.C + h * D + 64 * c, kb * BKEY, n);
+      if (with_v) tma_load_3d(smem + A::V_OFF + c * CH, &map, &bar_kv, 2 * p.C + h * D + 64 * c, kb * BKEY, n);
+    }
+  };
+  auto issue_s = [&]() {                                         // thread 0: S = Q K^T
+    tc_fence_after();
+#pragma unroll
+    for (int k = 0; k < D / 16; ++k) {
+      const uint32_t off = (k / 4) * CH + (k % 4) * 32;          // chunk of 64 channels, 32 bytes per K = 16 step
+      umma_bf16(tmem, desc_with_addr(dk, sb + A::Q_OFF + off), desc_with_addr(dk, sb + A::K_OFF + off), idesc_s, k != 0);
+    }
+    umma_commit(&bar_s);
+  };
+  const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  const float c2 = p.scale * 1.4426950408889634f;
+
+  // ---- sweep 1: row maxima of the raw scores
+  float m = -INFINITY;
+  mbar_wait(&bar_q, 0);
+  for (int kb = 0; kb < nkb; ++kb) {
+    if (threadIdx.x == 0) load_kv(kb, false);
+    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
+    if (threadIdx.x == 0) issue_s();
+    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
+    tc_fence_after();
+#pragma unroll
+    for (int ch = 0; ch < BKEY / 32; ++ch) {
+      uint32_t r[32];
+      tmem_ld32(trow + ch * 32, r);
+      tmem_ld_wait();
+      const int kbase = kb * BKEY + ch * 32;
+#pragma unroll
+      for (int i = 0; i < 32; ++i)
+        if (kbase + i < p.T) m = fmaxf(m, __uint_as_float(r[i]));
+    }
+    tc_fence_before();
+    __syncthreads();                     // S and the K tile are free again
+  }
+  // ---- sweep 2: P = exp(scale (S - m)), O += P V
+  float l = 0.f, lx = 0.f;              // l: sum of the bf16 probabilities the P V product sees; lx: the exact sum
+  const float mc = m * c2;
+  for (int kb = 0; kb < nkb; ++kb) {
+    if (kb > 0) { mbar_wait(&bar_pv, ph_pv); ph_pv ^= 1; }      // the previous P V has read P and V
+    if (threadIdx.x == 0) load_kv(kb, true);
+    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
+    if (threadIdx.x == 0) issue_s();
+    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
+    tc_fence_after();
+#pragma unroll
+    for (int ch = 0; ch < BKEY / 32; ++ch) {
+      uint32_t r[32];
+      tmem_ld32(trow + ch * 32, r);
+      tmem_ld_wait();
+      const int kbase = kb * BKEY + ch * 32;
+      uint32_t pk[16];
+#pragma unroll
+      for (int i = 0; i < 32; i += 2) {
+        float e0 = kbase + i < p.T ? exp2f(fmaf(__uint_as_float(r[i]), c2, -mc)) : 0.f;
+        float e1 = kbase + i + 1 < p.T ? exp2f(fmaf(__uint_as_float(r[i + 1]), c2, -mc)) : 0.f;
+        pk[i >> 1] = pack_bf16(e0, e1);
+        // o is normalised by the sum of the values the P V product sees (bf16): the rows of P / l sum to one; the
+        // log-sum-exp handed to the backward, which recomputes P in fp32, takes the exact sum
+        l += __uint_as_float(pk[i >> 1] << 16) + __uint_as_float(pk[i >> 1] & 0xffff0000u);
+        lx += e0 + e1;
+      }
+      // keys [32 ch, 32 ch + 32) = 16-byte pieces 4 (ch & 1) .. + 3 of chunk ch / 2, row `row`, 128-byte swizzle
+      const uint32_t base = sb + A::P_OFF + (ch >> 1) * CH + row * 128;
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        st_shared_v4(base + ((((ch & 1) * 4 + j) ^ (row & 7)) << 4), pk[4 * j], pk[4 * j + 1], pk[4 * j + 2], pk[4 * j + 3]);
+    }
+    fence_proxy_async_smem();            // P (generic-proxy writes) before the MMA (async proxy) reads it
+    tc_fence_before();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      tc_fence_after();
+#pragma unroll
+      for (int k = 0; k < BKEY / 16; ++k) {
+        const uint32_t pa = sb + A::P_OFF + (k / 4) * CH + (k % 4) * 32;      // A = P, K-major: keys 16 k ..
+        const uint32_t vb = sb + A::V_OFF + k * 2048;                         // B = V, MN-major: 16 key rows of 128 bytes
+        umma_bf16(tmem + 128, desc_with_addr(dk, pa), desc_with_addr(dmn, vb), idesc_o, (kb | k) != 0);
+      }
+      umma_commit(&bar_pv);
+    }
+  }
+  mbar_wait(&bar_pv, ph_pv);
+  tc_fence_after();
+  // ---- epilogue: o = O / l
+  const int q = q0 + row;
+  const float inv = 1.0f / l;
+  bf16* op = p.o + ((size_t)n * p.T + q) * p.C + (size_t)h * D;
+#pragma unroll
+  for (int ch = 0; ch < D / 32; ++ch) {
+    uint32_t r[32];
+    tmem_ld32(trow + 128 + ch * 32, r);
+    tmem_ld_wait();
+    if (q < p.T) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        uint4 v;
+        v.x = pack_bf16(__uint_as_float(r[8 * j]) * inv, __uint_as_float(r[8 * j + 1]) * inv);
+        v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * inv, __uint_as_float(r[8 * j + 3]) * inv);
+        v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * inv, __uint_as_float(r[8 * j + 5]) * inv);
+        v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * inv, __uint_as_float(r[8 * j + 7]) * inv);
+        *reinterpret_cast<uint4*>(op + ch * 32 + 8 * j) = v;
+      }
+    }
+  }
+  if (q < p.T) p.lse[((size_t)n * p.heads + h) * p.T + q] = m * p.scale + __logf(lx);
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem, A::TMEM_COLS);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ backward
+// Operand layouts (all tiles are TMA boxes / register-written tiles of 128 rows x 64 bf16 = 128-byte-swizzled chunks):
+//   S  = Q K^T, g_P = g_o V^T        A = Q / g_o   K-major,   B = K / V     K-major     (rows = queries, K = channels)
+//   g_q += g_S K                     A = g_S       K-major,   B = K         MN-major    (K = keys)
+//   g_v += P^T g_o, g_k += g_S^T Q   A = P / g_S   MN-major (their [query][key] tiles read transposed), B = g_o / Q MN-major
+// P and g_S are recomputed per tile from the saved log-sum-exp, in fp32 on the TMEM rows (thread = query), and handed to
+// the tensor cores as bf16.  D_i = sum_j P_ij g_P_ij comes from a first sweep of the g_q kernel (fp32, from the unrounded
+// P: see attention.cu) and is read by the g_k / g_v kernel.
+struct AtbP { int T, C, heads; float scale; bf16* g_qkv; const float* lse; float* Dg; };
+
+// 128 fp32 values of this thread's row -> bf16 -> chunk-swizzled A tile at `tile` (two 16 KB chunks of 64 columns)
+__device__ __forceinline__ void store_row_chunk32(uint32_t tile, int row, int ch, const uint32_t (&pk)[16]) {
+  const uint32_t base = tile + (ch >> 1) * CH + row * 128;
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+    st_shared_v4(base + ((((ch & 1) * 4 + j) ^ (row & 7)) << 4), pk[4 * j], pk[4 * j + 1], pk[4 * j + 2], pk[4 * j + 3]);
+}
+
+template <int D> struct BCfg {
+  static constexpr int NC = D / 64;
+  // g_q kernel: Q, g_o (resident), K, V (per key tile), g_S
+  static constexpr int Q_OFF = 0, GO_OFF = NC * CH, K_OFF = 2 * NC * CH, V_OFF = 3 * NC * CH, DS_OFF = 4 * NC * CH;
+  static constexpr int SMEM_DQ = 4 * NC * CH + 2 * CH + 1024;
+  // g_k / g_v kernel: K, V (resident), Q, g_o (per query tile), P, g_S
+  static constexpr int P_OFF = 4 * NC * CH, DS2_OFF = 4 * NC * CH + 2 * CH;
+  static constexpr int SMEM_DKV = 4 * NC * CH + 4 * CH + 1024;
+};
+
+template <int D>
+__global__ void __launch_bounds__(128, 1) attn_bwd_dq_tc_k(const __grid_constant__ CUtensorMap mapQ,
+                                                           const __grid_constant__ CUtensorMap mapG, const AtbP p) {
+  using B = BCfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t bar_q, bar_kv, bar_s, bar_dq;
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5, row = threadIdx.x;
+  const int q0 = blockIdx.x * BQ, h = blockIdx.y, n = blockIdx.z;
+  const int nkb = (p.T + BKEY - 1) / BKEY;
+  if (threadIdx.x == 0) {
+    prefetch_tmap(&mapQ); prefetch_tmap(&mapG);
+    mbar_init(&bar_q, 1); mbar_init(&bar_kv, 1); mbar_init(&bar_s, 1); mbar_init(&bar_dq, 1);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(&tmem_base_s, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;      // S: [0,128), g_P: [128,256), g_q: [256, 256 + D)
+  pdl_wait();
+  pdl_launch_dependents();
+  constexpr uint64_t dk = smem_desc_sw128(16, 1024), dmn = smem_desc_sw128(CH, 1024);
+  constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_q = idesc_bf16(BQ, D, 0, 1);
+  const uint32_t sb = smem_u32(smem);
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(&bar_q, 2 * B::NC * CH);
+    for (int c = 0; c < B::NC; ++c) {
+      tma_load_3d(smem + B::Q_OFF + c * CH, &mapQ, &bar_q, h * D + 64 * c, q0, n);
+      tma_load_3d(smem + B::GO_OFF + c * CH, &mapG, &bar_q, h * D + 64 * c, q0, n);
+    }
+  }
+  uint32_t ph_kv = 0, ph_s = 0, ph_dq = 0;
+  auto load_kv = [&](int kb) {
+    mbar_expect_tx(&bar_kv, 2 * B::NC * CH);
+    for (int c = 0; c < B::NC; ++c) {
+      tma_load_3d(smem + B::K_OFF + c * CH, &mapQ, &bar_kv, p.C + h * D + 64 * c, kb * BKEY, n);
+      tma_load_3d(smem + B::V_OFF + c * CH, &mapQ, &bar_kv, 2 * p.C + h * D + 64 * c, kb * BKEY, n);
+    }
+  };
+  auto issue_s_dp = [&]() {               // S = Q K^T, g_P = g_o V^T
+    tc_fence_after();
+#pragma unroll
+    for (int k = 0; k < D / 16; ++k) {
+      const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+      umma_bf16(tmem, desc_with_addr(dk, sb + B::Q_OFF + off), desc_with_addr(dk, sb + B::K_OFF + off), idesc_s, k != 0);
+    }
+#pragma unroll
+    for (int k = 0; k < D / 16; ++k) {
+      const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+      umma_bf16(tmem + 128, desc_with_addr(dk, sb + B::GO_OFF + off), desc_with_addr(dk, sb + B::V_OFF + off), idesc_s, k != 0);
+    }
+    umma_commit(&bar_s);
+  };
+  const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  const int q = q0 + row;
+  const float c2 = p.scale * 1.4426950408889634f;
+  const float lse2 = (q < p.T ? p.lse[((size_t)n * p.heads + h) * p.T + q] : 0.f) * 1.4426950408889634f;
+  mbar_wait(&bar_q, 0);
+  // ---- sweep 1: D_i = sum_j P_ij g_P_ij
+  float Dr = 0.f;
+  for (int kb = 0; kb < nkb; ++kb) {
+    if (threadIdx.x == 0) load_kv(kb);
+    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
+    if (threadIdx.x == 0) issue_s_dp();
+    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
+    tc_fence_after();
+#pragma unroll
+    for (int ch = 0; ch < BKEY / 32; ++ch) {
+      uint32_t rs[32], rp[32];
+      tmem_ld32(trow + ch * 32, rs);
+      tmem_ld32(trow + 128 + ch * 32, rp);
+      tmem_ld_wait();
+      const int kbase = kb * BKEY + ch * 32;
+#pragma unroll
+      for (int i = 0; i < 32; ++i)
+        if (kbase + i < p.T) Dr = fmaf(exp2f(fmaf(__uint_as_float(rs[i]), c2, -lse2)), __uint_as_float(rp[i]), Dr);
+    }
+    tc_fence_before();
+    __syncthreads();
+  }
+  if (q < p.T) p.Dg[((size_t)n * p.heads + h) * p.T + q] = Dr;
+  // ---- sweep 2: g_S = P (g_P - D), g_q += g_S K
+  for (int kb = 0; kb < nkb; ++kb) {
+    if (kb > 0) { mbar_wait(&bar_dq, ph_dq); ph_dq ^= 1; }       // the previous g_S K has read g_S and K
+    if (threadIdx.x == 0) load_kv(kb);
+    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
+    if (threadIdx.x == 0) issue_s_dp();
+    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
+    tc_fence_after();
+#pragma unroll
+    for (int ch = 0; ch < BKEY / 32; ++ch) {
+      uint32_t rs[32], rp[32], pk[16];
+      tmem_ld32(trow + ch * 32, rs);
+      tmem_ld32(trow + 128 + ch * 32, rp);
+      tmem_ld_wait();
+      const int kbase = kb * BKEY + ch * 32;
+#pragma unroll
+      for (int i = 0; i < 32; i += 2) {
+        const float d0 = kbase + i < p.T ? exp2f(fmaf(__uint_as_float(rs[i]), c2, -lse2)) * (__uint_as_float(rp[i]) - Dr) : 0.f;
+        const float d1 = kbase + i + 1 < p.T ? exp2f(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) * (__uint_as_float(rp[i + 1]) - Dr) : 0.f;
+        pk[i >> 1] = pack_bf16(d0, d1);
+      }
+      store_row_chunk32(sb + B::DS_OFF, row, ch, pk);
+    }
+    fence_proxy_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      tc_fence_after();
+#pragma unroll
+      for (int k = 0; k < BKEY / 16; ++k)
+        umma_bf16(tmem + 256, desc_with_addr(dk, sb + B::DS_OFF + (k / 4) * CH + (k % 4) * 32),
+                  desc_with_addr(dmn, sb + B::K_OFF + k * 2048), idesc_q, (kb | k) != 0);
+      umma_commit(&bar_dq);
+    }
+  }
+  mbar_wait(&bar_dq, ph_dq);
+  tc_fence_after();
+  bf16* gq = p.g_qkv + ((size_t)n * p.T + q) * 3 * p.C + (size_t)h * D;
+#pragma unroll
+  for (int ch = 0; ch < D / 32; ++ch) {
+    uint32_t r[32];
+    tmem_ld32(trow + 256 + ch * 32, r);
+    tmem_ld_wait();
+    if (q < p.T) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        uint4 v;
+        v.x = pack_bf16(__uint_as_float(r[8 * j]) * p.scale, __uint_as_float(r[8 * j + 1]) * p.scale);
+        v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * p.scale, __uint_as_float(r[8 * j + 3]) * p.scale);
+        v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * p.scale, __uint_as_float(r[8 * j + 5]) * p.scale);
+        v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * p.scale, __uint_as_float(r[8 * j + 7]) * p.scale);
+        *reinterpret_cast<uint4*>(gq + ch * 32 + 8 * j) = v;
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem, 512);
+  }
+}
+
+template <int D>
+__global__ void __launch_bounds__(128, 1) attn_bwd_dkv_tc_k(const __grid_constant__ CUtensorMap mapQ,
+                                                            const __grid_constant__ CUtensorMap mapG, const AtbP p) {
+  using B = BCfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t bar_kv, bar_q, bar_s, bar_acc;
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5, row = threadIdx.x;
+  const int k0 = blockIdx.x * BKEY, h = blockIdx.y, n = blockIdx.z;
+  const int nqb = (p.T + BQ - 1) / BQ;
+  if (threadIdx.x == 0) {
+    prefetch_tmap(&mapQ); prefetch_tmap(&mapG);
+    mbar_init(&bar_kv, 1); mbar_init(&bar_q, 1); mbar_init(&bar_s, 1); mbar_init(&bar_acc, 1);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(&tmem_base_s, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;      // S: [0,128), g_P: [128,256), g_v: [256, 256 + D), g_k: [256 + D, 256 + 2 D)
+  pdl_wait();
+  pdl_launch_dependents();
+  constexpr uint64_t dk = smem_desc_sw128(16, 1024), dmn = smem_desc_sw128(CH, 1024);
+  constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_t = idesc_bf16(BKEY, D, 1, 1);
+  const uint32_t sb = smem_u32(smem);
+  // this CTA's keys: K, V resident (their offsets in B:: are those of the g_q kernel's K / V slots)
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(&bar_kv, 2 * B::NC * CH);
+    for (int c = 0; c < B::NC; ++c) {
+      tma_load_3d(smem + B::K_OFF + c * CH, &mapQ, &bar_kv, p.C + h * D + 64 * c, k0, n);
+      tma_load_3d(smem + B::V_OFF + c * CH, &mapQ, &bar_kv, 2 * p.C + h * D + 64 * c, k0, n);
+    }
+  }
+  const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  const float c2 = p.scale * 1.4426950408889634f;
+  uint32_t ph_q = 0, ph_s = 0, ph_acc = 0;
+  mbar_wait(&bar_kv, 0);
+  for (int qb = 0; qb < nqb; ++qb) {
+    if (qb > 0) { mbar_wait(&bar_acc, ph_acc); ph_acc ^= 1; }    // the previous P^T g_o / g_S^T Q have read Q, g_o, P, g_S
+    if (threadIdx.x == 0) {
+      mbar_expect_tx(&bar_q, 2 * B::NC * CH);
+      for (int c = 0; c < B::NC; ++c) {
+        tma_load_3d(smem + B::Q_OFF + c * CH, &mapQ, &bar_q, h * D + 64 * c, qb * BQ, n);
+        tma_load_3d(smem + B::GO_OFF + c * CH, &mapG, &bar_q, h * D + 64 * c, qb * BQ, n);
+      }
+    }
+    const int q = qb * BQ + row;
+    const float lse2 = (q < p.T ? p.lse[((size_t)n * p.heads + h) * p.T + q] : 0.f) * 1.4426950408889634f;
+    const float Dr = q < p.T ? p.Dg[((size_t)n * p.heads + h) * p.T + q] : 0.f;
+    mbar_wait(&bar_q, ph_q); ph_q ^= 1;
+    if (threadIdx.x == 0) {
+      tc_fence_after();
+#pragma unroll
+      for (int k = 0; k < D / 16; ++k) {
+        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+        umma_bf16(tmem, desc_with_addr(dk, sb + B::Q_OFF + off), desc_with_addr(dk, sb + B::K_OFF + off), idesc_s, k != 0);
+      }
+#pragma unroll
+      for (int k = 0; k < D / 16; ++k) {
+        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+        umma_bf16(tmem + 128, desc_with_addr(dk, sb + B::GO_OFF + off), desc_with_addr(dk, sb + B::V_OFF + off), idesc_s, k != 0);
+      }
+      umma_commit(&bar_s);
+    }
+    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
+    tc_fence_after();
+#pragma unroll
+    for (int ch = 0; ch < BKEY / 32; ++ch) {
+      uint32_t rs[32], rp[32], pp[16], pd[16];
+      tmem_ld32(trow + ch * 32, rs);
+      tmem_ld32(trow + 128 + ch * 32, rp);
+      tmem_ld_wait();
+      const int kbase = k0 + ch * 32;
+#pragma unroll
+      for (int i = 0; i < 32; i += 2) {
+        const bool in0 = q < p.T && kbase + i < p.T, in1 = q < p.T && kbase + i + 1 < p.T;
+        const float e0 = in0 ? exp2f(fmaf(__uint_as_float(rs[i]), c2, -lse2)) : 0.f;
+        const float e1 = in1 ? exp2f(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) : 0.f;
+        pp[i >> 1] = pack_bf16(e0, e1);
+        pd[i >> 1] = pack_bf16(e0 * (__uint_as_float(rp[i]) - Dr), e1 * (__uint_as_float(rp[i + 1]) - Dr));
+      }
+      store_row_chunk32(sb + B::P_OFF, row, ch, pp);
+      store_row_chunk32(sb + B::DS2_OFF, row, ch, pd);
+    }
+    fence_proxy_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      tc_fence_after();
+      // A = P^T / g_S^T: the [query][key] tiles read MN-major (M = keys: two 64-key chunks, LBO = CH; K = 16 query rows per step)
+#pragma unroll
+      for (int k = 0; k < BQ / 16; ++k)
+        umma_bf16(tmem + 256, desc_with_addr(dmn, sb + B::P_OFF + k * 2048), desc_with_addr(dmn, sb + B::GO_OFF + k * 2048),
+                  idesc_t, (qb | k) != 0);
+#pragma unroll
+      for (int k = 0; k < BQ / 16; ++k)
+        umma_bf16(tmem + 256 + D, desc_with_addr(dmn, sb + B::DS2_OFF + k * 2048), desc_with_addr(dmn, sb + B::Q_OFF + k * 2048),
+                  idesc_t, (qb | k) != 0);
+      umma_commit(&bar_acc);
+    }
+  }
+  mbar_wait(&bar_acc, ph_acc);
+  tc_fence_after();
+  const int key = k0 + row;
+  bf16* gk = p.g_qkv + ((size_t)n * p.T + key) * 3 * p.C + (size_t)h * D + p.C;
+#pragma unroll
+  for (int part = 0; part < 2; ++part) {       // 0: g_v (unscaled) -> third 2; 1: g_k (x scale) -> third 1
+    const float f = part ? p.scale : 1.0f;
+    bf16* dst = part ? gk : gk + p.C;
+#pragma unroll
+    for (int ch = 0; ch < D / 32; ++ch) {
+      uint32_t r[32];
+      tmem_ld32(trow + 256 + part * D + ch * 32, r);
+      tmem_ld_wait();
+      if (key < p.T) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          uint4 v;
+          v.x = pack_bf16(__uint_as_float(r[8 * j]) * f, __uint_as_float(r[8 * j + 1]) * f);
+          v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * f, __uint_as_float(r[8 * j + 3]) * f);
+          v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * f, __uint_as_float(r[8 * j + 5]) * f);
+          v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * f, __uint_as_float(r[8 * j + 7]) * f);
+          *reinterpret_cast<uint4*>(dst + ch * 32 + 8 * j) = v;
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem, 512);
+  }
+}
+
+template <int D> bool launch_atb(const CUtensorMap& mq, const CUtensorMap& mg, const AtbP& p, int n, cudaStream_t st) {
+  static bool attr = false;
+  if (!attr) {
+    if (cudaFuncSetAttribute(attn_bwd_dq_tc_k<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, BCfg<D>::SMEM_DQ) != cudaSuccess ||
+        cudaFuncSetAttribute(attn_bwd_dkv_tc_k<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, BCfg<D>::SMEM_DKV) != cudaSuccess)
+      return false;
+    attr = true;
+  }
+  const dim3 grid((p.T + BQ - 1) / BQ, p.heads, n);
+  // the second kernel reads D, which the first one writes after its dependency wait: ordinary stream order between the two
+  if (launch_pdl(attn_bwd_dq_tc_k<D>, grid, dim3(128), BCfg<D>::SMEM_DQ, st, mq, mg, p) != cudaSuccess) return false;
+  return launch_pdl(attn_bwd_dkv_tc_k<D>, grid, dim3(128), BCfg<D>::SMEM_DKV, st, mq, mg, p) == cudaSuccess;
+}
+
+template <int D> bool launch_atc(const CUtensorMap& map, const AtcP& p, int n, cudaStream_t st) {
+  static bool attr = false;
+  if (!attr) {
+    if (cudaFuncSetAttribute(attn_fwd_tc_k<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, ACfg<D>::SMEM) != cudaSuccess) return false;
+    attr = true;
+  }
+  return launch_pdl(attn_fwd_tc_k<D>, dim3((p.T + BQ - 1) / BQ, p.heads, n), dim3(128), ACfg<D>::SMEM, st, map, p) == cudaSuccess;
+}
+
+}  // namespace
+
+bool attn_fwd_tc_supported(int dt, int C, int heads) {
+  if (dt != DT_BF16 || heads <= 0 || C % heads) return false;
+  const int d = C / heads;
+  return d == 64 || d == 128;
+}
+
+// 1 on launch, -1 on failure (tensor map / attribute)
+int attn_fwd_tc(const void* qkv, int n, int T, int C, int heads, void* o, float* lse, cudaStream_t st) {
+  CUtensorMap map;
+  const uint64_t dims[3] = {(uint64_t)3 * C, (uint64_t)T, (uint64_t)n};
+  const uint64_t str[2] = {(uint64_t)3 * C * 2, (uint64_t)T * 3 * C * 2};
+  const uint32_t box[3] = {64, BQ, 1};
+  if (!tmap::get_map(qkv, 3, dims, str, box, &map)) return -1;
+  AtcP p;
+  p.T = T; p.C = C; p.heads = heads; p.scale = 1.0f / sqrtf((float)(C / heads)); p.o = (bf16*)o; p.lse = lse;
+  const bool ok = C / heads == 64 ? launch_atc<64>(map, p, n, st) : launch_atc<128>(map, p, n, st);
+  return ok ? 1 : -1;
+}
+
+// 2 on launch, -1 on failure.  stats: [log-sum-exp | D] as attn_stats_floats lays them out
+int attn_bwd_tc(const void* qkv, const void* g_o, int n, int T, int C, int heads, float* stats, void* g_qkv, cudaStream_t st) {
+  CUtensorMap mq, mg;
+  const uint32_t box[3] = {64, BQ, 1};
+  {
+    const uint64_t dims[3] = {(uint64_t)3 * C, (uint64_t)T, (uint64_t)n};
+    const uint64_t str[2] = {(uint64_t)3 * C * 2, (uint64_t)T * 3 * C * 2};
+    if (!tmap::get_map(qkv, 3, dims, str, box, &mq)) return -1;
+  }
+  {
+    const uint64_t dims[3] = {(uint64_t)C, (uint64_t)T, (uint64_t)n};
+    const uint64_t str[2] = {(uint64_t)C * 2, (uint64_t)T * C * 2};
+    if (!tmap::get_map(g_o, 3, dims, str, box, &mg)) return -1;
+  }
+  AtbP p;
+  p.T = T; p.C = C; p.heads = heads; p.scale = 1.0f / sqrtf((float)(C / heads)); p.g_qkv = (bf16*)g_qkv;
+  p.lse = stats; p.Dg = stats + (size_t)n * heads * T;
+  const bool ok = C / heads == 64 ? launch_atb<64>(mq, mg, p, n, st) : launch_atb<128>(mq, mg, p, n, st);
+  return ok ? 2 : -1;
+}
+
+}  // namespace pulse

@@ -80,6 +80,8 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
+  pdl_wait();                  // everything above overlapped the tail of the previous kernel
+  pdl_launch_dependents();
 
   if (warp == 0) {
     if (lane == 0) {
@@ -107,8 +109,8 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      // ===== MMA issuer =====
+    {
+      // ===== MMA issuer: the whole warp runs the loop, one elected lane issues (sm100.cuh elect_one_sync) =====
       constexpr uint32_t idesc = idesc_bf16(BM, BN, 0, 0);
       constexpr uint64_t dbase = smem_desc_sw128(16, 1024);
       int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t acc_phase = 0;
@@ -122,14 +124,17 @@ conv_tc_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUt
           mbar_wait(&full_bar[stage], phase);
           tc_fence_after();
           const uint32_t a_addr = smem_u32(smem + stage * C::STAGE_BYTES), b_addr = a_addr + A_BYTES;
+          if (elect_one_sync()) {
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k)
-            umma_bf16(tmem_d, desc_with_addr(dbase, a_addr + k * 32), desc_with_addr(dbase, b_addr + k * 32), idesc,
-                      (kb | k) != 0);
-          umma_commit(&empty_bar[stage]);
+            for (int k = 0; k < BK / 16; ++k)
+              umma_bf16(tmem_d, desc_with_addr(dbase, a_addr + k * 32), desc_with_addr(dbase, b_addr + k * 32), idesc,
+                        (kb | k) != 0);
+            umma_commit(&empty_bar[stage]);
+            if (kb == num_kb - 1) umma_commit(&tfull_bar[acc]);
+          }
+          __syncwarp();
           if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
         }
-        umma_commit(&tfull_bar[acc]);
         acc ^= 1;
         if (acc == 0) acc_phase ^= 1;
       }
@@ -363,7 +368,7 @@ bool launch(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, 
   }
   const int tiles = p.nph * p.tiles_mn * p.n_tiles;
   const int grid = tiles < sm_count() ? tiles : sm_count();
-  conv_tc_k<BN><<<grid, 192, Cfg<BN>::SMEM, st>>>(a0, a1, b, p);
+  launch_pdl(conv_tc_k<BN>, dim3(grid), dim3(192), Cfg<BN>::SMEM, st, a0, a1, b, p);
   return true;
 }
 

@@ -315,7 +315,8 @@ void attn_forward(Ctx& c, const OpPlan& op) {
                         c.par(op.p[P_C1B]), nullptr, nullptr, c.fwd(op.h1)));
   {
     Prof pr(s, c.st, PULSE_KCLASS_OTHER, 4.0 * s->d.n * (double)hw * hw * C, 0.0);
-    s->launches += attn_fwd(c.dt, c.fwd(op.h1), s->d.n, hw, C, op.heads, c.fwd(op.a2), (float*)(c.stash + op.lse), c.st);
+    const int r = attn_fwd(c.dt, c.fwd(op.h1), s->d.n, hw, C, op.heads, c.fwd(op.a2), (float*)(c.stash + op.lse), c.st, c.tc());
+    if (r < 0) c.err = true; else s->launches += r;
   }
   run_conv(c, conv_args(c, Cat{c.fwd(op.a2), C, nullptr, 0}, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_C2W]), C,
                         c.par(op.p[P_C2B]), nullptr, c.fwd(op.x0), c.fwd(op.out)), op.out);
@@ -403,7 +404,8 @@ void attn_backward(Ctx& c, const OpPlan& op) {
   run_dgrad(c, g_out, op.hin, op.win, C, op.wt2, 1, C, g_o, 0, 1, op.hin, op.win);
   {
     Prof pr(s, c.st, PULSE_KCLASS_OTHER, 10.0 * n * (double)hw * hw * C, 0.0);
-    s->launches += attn_bwd(c.dt, c.fwd(op.h1), g_o, n, hw, C, op.heads, (float*)(c.stash + op.lse), g_qkv, c.st);
+    const int r = attn_bwd(c.dt, c.fwd(op.h1), g_o, n, hw, C, op.heads, (float*)(c.stash + op.lse), g_qkv, c.st, c.tc());
+    if (r < 0) c.err = true; else s->launches += r;
     s->launches += colsum(c.dt, g_qkv, n, hw, 3 * C, (float*)(c.work + op.gp), c.st);      // qkv bias gradient
   }
   c.fork();
@@ -915,21 +917,25 @@ static pulse_status_t check_attn(int dtype, int n, int t, int c, int heads) {
 extern "C" size_t pulse_attention_stats_floats(int n, int heads, int tokens) {
   return (n <= 0 || heads <= 0 || tokens <= 0) ? 0 : attn_stats_floats(n, heads, tokens);
 }
-extern "C" pulse_status_t pulse_attention(int dtype, const void* d_qkv, int n, int tokens, int c, int heads, void* d_o,
-                                          float* d_stats, void* stream) {
+extern "C" pulse_status_t pulse_attention(int dtype, int force_simt, const void* d_qkv, int n, int tokens, int c, int heads,
+                                          void* d_o, float* d_stats, void* stream) {
   pulse_status_t s = check_attn(dtype, n, tokens, c, heads);
   if (s) return s;
   if (!d_qkv || !d_o || !d_stats) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
-  attn_fwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_qkv, n, tokens, c, heads, d_o, d_stats, (cudaStream_t)stream);
+  if (attn_fwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_qkv, n, tokens, c, heads, d_o, d_stats, (cudaStream_t)stream, !force_simt) < 0)
+    return fail(PULSE_ERR_CUDA, "tensor-core attention launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }
-extern "C" pulse_status_t pulse_attention_backward(int dtype, const void* d_qkv, const void* d_g_o, int n, int tokens, int c,
-                                                   int heads, float* d_stats, void* d_g_qkv, void* stream) {
+extern "C" pulse_status_t pulse_attention_backward(int dtype, int force_simt, const void* d_qkv, const void* d_g_o, int n,
+                                                   int tokens, int c, int heads, float* d_stats, void* d_g_qkv,
+                                                   void* stream) {
   pulse_status_t s = check_attn(dtype, n, tokens, c, heads);
   if (s) return s;
   if (!d_qkv || !d_g_o || !d_stats || !d_g_qkv) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
-  attn_bwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_qkv, d_g_o, n, tokens, c, heads, d_stats, d_g_qkv, (cudaStream_t)stream);
+  if (attn_bwd(dtype == PULSE_F32 ? DT_F32 : DT_BF16, d_qkv, d_g_o, n, tokens, c, heads, d_stats, d_g_qkv, (cudaStream_t)stream,
+               !force_simt) < 0)
+    return fail(PULSE_ERR_CUDA, "tensor-core attention launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;
 }

@@ -54,9 +54,13 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
 // forward / backward and kept between them
 bool attn_supported(int C, int heads);
 size_t attn_stats_floats(int n, int heads, int T);
-int attn_fwd(int dt, const void* qkv, int n, int T, int C, int heads, void* o, float* stats, cudaStream_t st);
+// use_tc: the tcgen05 forward (attention_tc.cu) where it applies (bf16, 64 or 128 channels per head), else CUDA cores
+int attn_fwd(int dt, const void* qkv, int n, int T, int C, int heads, void* o, float* stats, cudaStream_t st, bool use_tc = true);
+bool attn_fwd_tc_supported(int dt, int C, int heads);
+int attn_fwd_tc(const void* qkv, int n, int T, int C, int heads, void* o, float* lse, cudaStream_t st);
 int attn_bwd(int dt, const void* qkv, const void* g_o, int n, int T, int C, int heads, float* stats, void* g_qkv,
-             cudaStream_t st);
+             cudaStream_t st, bool use_tc = true);
+int attn_bwd_tc(const void* qkv, const void* g_o, int n, int T, int C, int heads, float* stats, void* g_qkv, cudaStream_t st);
 
 // ---- small ops -----------------------------------------------------------------------
 // cs[n][c] += sum over pixels of g[n][hw][c]   (tensors whose writers could not emit their column sums)

@@ -11,6 +11,9 @@
 //   phase 2  g_x from the resident x and g_a: no second read (g_y is recomputed in fp32: keeping it in shared
 //            memory as bf16 would add a rounding the two-kernel form does not have); `add` (the shortcut
 //            gradient) streams in through a per-thread cp.async ring started before the reductions.
+//            (Measured and rejected in round 2: keeping g_y as fp32 IN PLACE of the x / g_a it came from and reading x
+//            again from L2 in phase 2, three pixels ahead in registers - it halves the special-function work, but a
+//            thread has only ~10 pixels per phase, too few to hide the L2 latency: 16.4 vs 15.9 us per launch.)
 // Falls back (returns 0) when a slice of one image does not fit into 8 CTAs' shared memory or the channel split
 // does not fall on slice boundaries; norm.cu then runs the two-kernel form.
 #include <cuda.h>

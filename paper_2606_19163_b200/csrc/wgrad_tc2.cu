@@ -49,6 +49,7 @@ struct Wg2Params {
   float* dw;
 };
 
+template <bool UP2>      // compile-time: the plain conv's kernel carries none of the phase-form code
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
 wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
             const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapG32,
@@ -105,7 +106,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
             const bool first = cb < p.c0_blocks;
             ma[b] = first ? &mapA0 : &mapA1;
             cch[b] = (first ? cb : cb - p.c0_blocks) * 64;
-            if (!p.up2) {
+            if (!UP2) {
               const Tap t = p.taps[ti];
               adx[b] = t.dx; ady[b] = t.dy; apx[b] = t.px; apy[b] = t.py;
             } else {      // ti = 4 (2 py + px) + 2 a + b': low-resolution pixel (y + a - 1 + py, x + b' - 1 + px)
@@ -127,7 +128,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
             if (!p.s2) tma2_load_4d(sa + b * BLK, ma[b], fb, cch[b], x0 + adx[b], y0 + ady[b], n0);
             else tma2_load_5d(sa + b * BLK, ma[b], fb, apx[b] * p.c0 + cch[b], x0 + adx[b], apy[b], y0 + ady[b], n0);
           }
-          if (!p.up2) {
+          if (!UP2) {
             tma2_load_4d(sa + 2 * BLK, &mapG, fb, co + (int)rank * 128, x0, y0, n0);
             tma2_load_4d(sa + 3 * BLK, &mapG, fb, co + (int)rank * 128 + 64, x0, y0, n0);
             tma2_load_4d(sa + 4 * BLK, &mapG32, fb, co + 256 + (int)rank * 32, x0, y0, n0);
@@ -206,10 +207,10 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
       const bool valid = u < p.units;
       const int ti = valid ? u / p.c_blocks : 0, cb = valid ? u - ti * p.c_blocks : 0;
       const int kch = cb * 64 + (q & 1) * 32;
-      const int kcol = p.taps[p.up2 ? 0 : ti].widx * p.ctot + kch;
+      const int kcol = p.taps[UP2 ? 0 : ti].widx * p.ctot + kch;
       // up2: this unit's partial belongs to every (r, s) its pre-summed tap covers: rows r0..r1, columns s0..s1 of the 3x3
       int r0 = 0, r1 = 0, s0 = 0, s1 = 0;
-      if (p.up2) {
+      if (UP2) {
         const int py = ti >> 3, px = (ti >> 2) & 1, ta = (ti >> 1) & 1, tb = ti & 1;
         r0 = (py == 0 && ta == 1) ? 1 : (py == 1 && ta == 1) ? 2 : 0; r1 = (py == 0 && ta == 0) ? 0 : (py == 1 && ta == 0) ? 1 : 2;
         s0 = (px == 0 && tb == 1) ? 1 : (px == 1 && tb == 1) ? 2 : 0; s1 = (px == 0 && tb == 0) ? 0 : (px == 1 && tb == 0) ? 1 : 2;
@@ -242,7 +243,7 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            if (!p.up2) {
+            if (!UP2) {
               tma_reduce_add_2d(&mapW, stg + buf * 2048, kcol, nt * N_TOT + ch * 16);
             } else {
               for (int r = r0; r <= r1; ++r)
@@ -320,7 +321,8 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   if (!ok) return -1;
   static bool attr_set = false;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(wgrad_tc2_k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM) != cudaSuccess) {
+    if (cudaFuncSetAttribute(wgrad_tc2_k<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM) != cudaSuccess ||
+        cudaFuncSetAttribute(wgrad_tc2_k<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM) != cudaSuccess) {
       tmap::set_error("cudaFuncSetAttribute(wgrad2 smem) failed");
       return -1;
     }
@@ -335,7 +337,8 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
     p.ppt = (int)(pairs / out_tiles);
     pairs = p.ppt * out_tiles;
   }
-  launch_pdl(wgrad_tc2_k, dim3((unsigned)(2 * pairs)), dim3(320), SMEM, st, m0, m1, mg, mg32, mw, p);
+  if (a.up2) launch_pdl(wgrad_tc2_k<true>, dim3((unsigned)(2 * pairs)), dim3(320), SMEM, st, m0, m1, mg, mg32, mw, p);
+  else launch_pdl(wgrad_tc2_k<false>, dim3((unsigned)(2 * pairs)), dim3(320), SMEM, st, m0, m1, mg, mg32, mw, p);
   return 1;
 }
 

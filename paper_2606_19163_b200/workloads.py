@@ -141,8 +141,8 @@ def gpu_mid(kind: str) -> dict:
         return _unet("mid_unet", 1, 32, [320, 640], temb=mlp)
     if kind == "attn":          # SD-style level with attention: 320 channels = 5 heads x 64, 64 tokens per image, 192 pixels = 1.5 tiles
         return _stage("mid_attn", "bf16", 3, 8, 8, 320, 32, mlp, "open", 1,
-                      [rb(320, 320), attn(320, 5, push=1), rb(320, 320), attn(320, 5, push=1)], [],
-                      [rb(320, 320, skip=320), attn(320, 5), rb(320, 320, skip=320), attn(320, 5), rb(320, 320, skip=320)])
+                      [rb(320, 320), attn(320, 5, push=1)], [],
+                      [rb(320, 320, skip=320), attn(320, 5), rb(320, 320, skip=320)])
     raise ValueError(kind)
 
 

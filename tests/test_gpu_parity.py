@@ -128,7 +128,7 @@ def flatten(per_mb, grads):
 
 
 def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, gold=None, order=None,
-          max_inflight=None):
+          max_inflight=None, slack=1.0):
     """fp32: every tensor within 1e-4 of the exact oracle.  bf16: every tensor within the plain 2e-2, except the
     tensors named in tests/golden/bf16_floor.json[gold] (see the module docstring)."""
     data = W.draw(desc, seed, with_g_e_out=with_g_e_out)
@@ -149,7 +149,7 @@ def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False,
         rlimit = None
         if k in exc:
             fmax, frms = exc[k]
-            row.update(floor_max=fmax, floor_rms=frms, limit=min(max(tol, 2.0 * fmax), CAP))
+            row.update(floor_max=fmax, floor_rms=frms, limit=min(max(tol, 2.0 * slack * fmax), CAP))
             # the rms bound needs elements to average over: a scalar (the loss) has rms == max
             rlimit = 1.5 * frms + 1e-4 if r.numel() >= 1024 else None
         rows[k] = row
@@ -162,7 +162,19 @@ def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False,
     n_plain = sum(1 for v in rows.values() if v["max"] <= tol)
     print(f"[parity] {desc['name']}: {n_plain}/{len(rows)} tensors within north_star's plain {tol:g} bar, "
           f"{len(exc)} on the committed exception list", flush=True)
-    if REPORT:
+    if REPORT and REPORT.endswith(".md"):      # the per-tensor report kept under profiles/ (markdown, appended per structure)
+        with open(REPORT, "a") as f:
+            rest = [v["max"] for k, v in rows.items() if k not in exc and v["max"] <= 0.5 * tol]
+            f.write(f"\n### {desc['name']} (flags {flags}, seed {seed}, oracle {str(oracle_dtype).split('.')[1]}): "
+                    f"{n_plain}/{len(rows)} tensors within the plain {tol:g} bar; {len(exc)} on the exception list; "
+                    f"{len(bad)} out of tolerance\n\n")
+            f.write("| tensor | max err / RMS | rms err / RMS | storage floor (max) | limit | listed |\n|---|---|---|---|---|---|\n")
+            for k, v in sorted(rows.items(), key=lambda kv: -kv[1]["max"]):
+                if k in exc or v["max"] > 0.5 * tol:
+                    f.write(f"| {k} | {v['max']:.3e} | {v['rms']:.3e} | {v.get('floor_max', float('nan')):.3e} | "
+                            f"{v['limit']:.3e} | {'yes' if k in exc else 'no'} |\n")
+            f.write(f"\n{len(rest)} further unlisted tensors, all below half the bar (worst {max(rest, default=0.0):.3e}).\n")
+    elif REPORT:
         with open(REPORT, "a") as f:
             f.write(json.dumps({"config": desc["name"], "flags": flags, "tol": tol, "within_plain_tol": n_plain,
                                 "tensors": len(rows), "listed": len(exc), "rows": rows}) + "\n")
@@ -208,8 +220,11 @@ def test_mid_bf16_attention_stage():
 @pytest.mark.parametrize("kind", ["updown", "unet"])
 def test_mid_bf16_upsample_forms(kind, flags):
     """Row a6 in its other forms (include/pulse.h PULSE_FLAG_UP_*): everything through the materialised upsampled tensor,
-    and the 4-phase forward / input gradient with pre-summed bf16 weights.  Same bar as the default form."""
-    check(W.gpu_mid(kind), seed=2, flags=flags, with_g_e_out=(kind != "unet"))
+    and the 4-phase forward / input gradient with pre-summed bf16 weights.  The materialised form has the default bar;
+    the opt-in phase forms carry one extra rounding of the weights per up conv and direction, which
+    the oracle's storage floor does not contain: listed tensors get 2.5 x (not 2 x) their floor, unlisted ones still
+    the plain 2e-2."""
+    check(W.gpu_mid(kind), seed=2, flags=flags, with_g_e_out=(kind != "unet"), slack=1.0 if flags == 16 else 1.25)
 
 
 def test_mid_bf16_1f1b_order():
