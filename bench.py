@@ -27,7 +27,9 @@ METRIC = "stage fwd+bwd samples/s"
 WORKLOADS = {1: "configs[0]: tiny collocated pair, fp32 debug path", 2: "configs[1]: SD1.5-shaped level-1 stage, "
              "2 enc + 3 dec ResBlocks 320ch, microbatch 4, 64x64", 3: "configs[2]: level-2 stage with down/up, "
              "microbatch 8, 32x32", 4: "configs[3]: full conv-only SD1.5-shaped UNet, microbatch 8, 4x64x64",
-             5: "configs[4]: SDXL-shaped stage, wave of 8 microbatches of 2, 4x128x128"}
+             5: "configs[4]: SDXL-shaped stage, wave of 8 microbatches of 2, 4x128x128",
+             6: "SURVEY 8f f1: configs[2]'s level-2 stage with a self-attention block (10 heads x 64, 1024 tokens) after "
+                "every ResBlock, microbatch 8, 32x32"}
 
 
 def conv_flops_fwd(desc) -> float:
@@ -61,6 +63,8 @@ def _op_flops(op, n, h, w, T):
         if ci != co:
             f += pix * co * ci
         return f
+    if op["kind"] == "attn":      # qkv and proj 1x1 convs + Q K^T and P V (4 n tokens^2 c)
+        return pix * ci * 3 * ci + pix * ci * ci + 4.0 * n * (h * w) ** 2 * ci
     return pix * co * ci * 9
 
 
@@ -663,7 +667,7 @@ def main():
     if world == 1 and args.config == 2 and not args.no_other_configs:
         torch.cuda.empty_cache()
         others = {}
-        for c in (3, 4, 5):
+        for c in (3, 4, 5, 6):
             try:
                 r = subprocess.run([sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", "10", "--warmup", "3",
                                     "--brief"], capture_output=True, text=True, timeout=900)

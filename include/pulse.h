@@ -66,7 +66,12 @@ enum {
    * under north_star's 2e-2 bar then cross it. */
   PULSE_FLAG_UP_MATERIALISED = 16, /* weight gradient through the materialised tensor too (the oracle's form everywhere) */
   PULSE_FLAG_UP_PHASE_FWD = 32,    /* forward in the 4-phase form (no upsampled tensor is written) */
-  PULSE_FLAG_UP_PHASE_DGRAD = 64   /* input gradient in the 4-phase form (one 16-tap conv over the gradient's parity view) */
+  PULSE_FLAG_UP_PHASE_DGRAD = 64,  /* input gradient in the 4-phase form (one 16-tap conv over the gradient's parity view) */
+  /* Pipeline execution: the encoder half and the decoder half of an OPEN stage
+   * run as separate calls (pulse_stage_forward_enc / _dec, pulse_stage_backward_dec / _enc), with other microbatches'
+   * halves in between.  The gradient buffers of the cached skips then live per in-flight microbatch ("local
+   * buffers for skip activations and their gradients"), beside its skip-cache slot, instead of once per stage. */
+  PULSE_FLAG_SPLIT = 128
 };
 /* kernel selector of the single-operator conv calls */
 enum { PULSE_CONV_AUTO = 0, PULSE_CONV_SIMT = 1, PULSE_CONV_TC_PAIR = 2, PULSE_CONV_TC_1CTA = 3 };
@@ -166,6 +171,21 @@ pulse_status_t pulse_stage_forward(pulse_stage_t* stage, pulse_skip_cache_t* cac
 pulse_status_t pulse_stage_backward(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id,
                                     const void* d_g_d_out, const void* d_g_e_out, void* d_g_x_in,
                                     void* d_g_h_in, float* d_g_temb, int accumulate_wgrad, void* stream);
+
+/* The two halves of an OPEN stage as separate calls (needs PULSE_FLAG_SPLIT; row f2): on a pipeline, the stages further in
+ * run between the encoder half and the decoder half of a microbatch, and between the backward of its decoder half and of
+ * its encoder half.  Order per microbatch: forward_enc (takes the slot) -> forward_dec -> backward_dec -> backward_enc
+ * (releases the slot); halves of other live microbatches may run anywhere in between.  Arguments as in the one-call
+ * forms.  accumulate_wgrad applies to backward_dec (0: zero the parameter gradients first); backward_enc always adds. */
+pulse_status_t pulse_stage_forward_enc(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id, const void* d_x_in,
+                                       const float* d_temb, void* d_e_out, void* stream);
+pulse_status_t pulse_stage_forward_dec(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id, const void* d_h_in,
+                                       void* d_d_out, void* stream);
+pulse_status_t pulse_stage_backward_dec(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id,
+                                        const void* d_g_d_out, void* d_g_h_in, float* d_g_temb, int accumulate_wgrad,
+                                        void* stream);
+pulse_status_t pulse_stage_backward_enc(pulse_stage_t* stage, pulse_skip_cache_t* cache, int64_t mb_id,
+                                        const void* d_g_e_out, void* d_g_x_in, float* d_g_temb, void* stream);
 
 /* The same two calls with the timestep path inside (rows a1, a7), so that it runs beside the chain instead of
  * before / after it: forward = pulse_temb_forward(d_t -> d_emb, d_temb_stash) + pulse_stage_forward(d_temb = d_emb);

@@ -27,6 +27,7 @@ FLAG_CONV_1CTA = 8
 FLAG_UP_MATERIALISED = 16
 FLAG_UP_PHASE_FWD = 32
 FLAG_UP_PHASE_DGRAD = 64
+FLAG_SPLIT = 128
 
 
 class OpDesc(C.Structure):
@@ -65,6 +66,10 @@ _SIG = {
     "pulse_skip_cache_destroy": [_vp],
     "pulse_stage_forward": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp],
     "pulse_stage_backward": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_int, _vp],
+    "pulse_stage_forward_enc": [_vp, _vp, _i64, _vp, _vp, _vp, _vp],
+    "pulse_stage_forward_dec": [_vp, _vp, _i64, _vp, _vp, _vp],
+    "pulse_stage_backward_dec": [_vp, _vp, _i64, _vp, _vp, _vp, C.c_int, _vp],
+    "pulse_stage_backward_enc": [_vp, _vp, _i64, _vp, _vp, _vp, _vp],
     "pulse_stage_forward_temb": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
     "pulse_stage_backward_temb": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int, _vp],
     "pulse_temb_stash_elems": [_vp, C.POINTER(_sz)],
@@ -261,6 +266,28 @@ class Stage:
         _ck(lib.pulse_stage_backward(self.h, self.cache, mb_id, _ptr(g_d_out), _ptr(g_e_out), _ptr(g_x_in),
                                      _ptr(g_h_in), _ptr(g_temb), int(accumulate), _stream()))
         return g_x_in, g_h_in
+
+    # ---- the two halves of a split (pipeline) stage (FLAG_SPLIT) ----------------------
+    def forward_enc(self, mb_id: int, x_in, temb):
+        e_out = torch.empty(self._shapes()["e_out"], dtype=self.tdtype, device=self.device)
+        _ck(lib.pulse_stage_forward_enc(self.h, self.cache, mb_id, _ptr(x_in), _ptr(temb), _ptr(e_out), _stream()))
+        return e_out
+
+    def forward_dec(self, mb_id: int, h_in):
+        d_out = torch.empty(self._shapes()["d_out"], dtype=self.tdtype, device=self.device)
+        _ck(lib.pulse_stage_forward_dec(self.h, self.cache, mb_id, _ptr(h_in), _ptr(d_out), _stream()))
+        return d_out
+
+    def backward_dec(self, mb_id: int, g_d_out, g_temb=None, accumulate=False):
+        g_h_in = torch.empty(self._shapes()["h_in"], dtype=self.tdtype, device=self.device)
+        _ck(lib.pulse_stage_backward_dec(self.h, self.cache, mb_id, _ptr(g_d_out), _ptr(g_h_in), _ptr(g_temb), int(accumulate),
+                                         _stream()))
+        return g_h_in
+
+    def backward_enc(self, mb_id: int, g_e_out, g_temb=None):
+        g_x_in = torch.empty(self._shapes()["x_in"], dtype=self.tdtype, device=self.device)
+        _ck(lib.pulse_stage_backward_enc(self.h, self.cache, mb_id, _ptr(g_e_out), _ptr(g_x_in), _ptr(g_temb), _stream()))
+        return g_x_in
 
     def forward_temb(self, mb_id: int, x_in, h_in, t):
         """temb_forward + forward in one call: the timestep path runs beside the stash of the boundary tensors."""

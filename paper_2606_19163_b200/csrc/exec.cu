@@ -27,6 +27,7 @@ struct Ctx {
   // backward) needs; it is enqueued beside the chain as soon as the last g_p is complete (tail_work)
   const float* emb = nullptr; float* g_temb = nullptr; const float* temb_stash = nullptr;
   int acc_w = 0; bool last_op = false, tail_done = false;
+  int op_lo = 0, op_hi = 0;      // ops this call runs: [op_lo, op_hi)
   bool err = false;
   cudaEvent_t new_event() {
     if (n_ev == (int)s->sync_events.size()) {
@@ -62,7 +63,7 @@ struct Ctx {
   }
   char* grad(int t) const {
     for (int i = 0; i < 3; ++i) if (t == ov_gt[i]) return ov_gp[i];
-    return work + s->tensors[t].goff;
+    return (s->tensors[t].g_in_stash ? stash : work) + s->tensors[t].goff;
   }
   const char* par(int p) const { return s->d_params + s->params[p].off; }
   float* pgrad(int p) const { return (float*)((char*)s->d_grads + s->params[p].goff); }
@@ -425,7 +426,8 @@ void attn_backward(Ctx& c, const OpPlan& op) {
 void small_grads(Ctx& c, const float* emb, float* g_temb, cudaStream_t st) {
   pulse_stage* s = c.s;
   std::vector<SmallGradEntry> e;
-  for (const OpPlan& op : s->ops) {
+  for (int oi = c.op_lo; oi < c.op_hi; ++oi) {       // the ops of this call (all of them, or one half of a split stage)
+    const OpPlan& op = s->ops[oi];
     SmallGradEntry g;
     memset(&g, 0, sizeof g);
     g.cs_out = (const float*)(c.work + s->tensors[op.out].cs);
@@ -446,6 +448,7 @@ void small_grads(Ctx& c, const float* emb, float* g_temb, cudaStream_t st) {
     }
     e.push_back(g);
   }
+  if (e.empty()) return;
   Prof pr(s, st, PULSE_KCLASS_OTHER, 0.0, 0.0);
   s->launches += small_grads_batch(c.dt, emb, g_temb, s->d.n, s->d.temb_dim, e.data(), (int)e.size(), st);
 }
@@ -478,39 +481,56 @@ pulse_status_t check_bound(pulse_stage* s, pulse_skip_cache* cache) {
 namespace {
 pulse_status_t temb_forward_impl(pulse_stage* s, const int64_t* d_t, float* d_emb, float* d_stash, cudaStream_t st);
 }
+enum { PART_ENC = 1, PART_DEC = 2, PART_ALL = 3 };      // halves of a split (pipeline) stage; PART_ALL: the one-call forms
+
 // d_t != nullptr (pulse_stage_forward_temb): the embedding is computed here, beside the stash of the boundary tensors,
 // from the timesteps into d_temb (written) with its MLP stash in d_temb_stash
 static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_x_in,
                                    const void* d_h_in, float* d_temb, const int64_t* d_t, float* d_temb_stash,
-                                   void* d_e_out, void* d_d_out, void* stream) {
+                                   void* d_e_out, void* d_d_out, void* stream, int parts = PART_ALL) {
   pulse_status_t stt = check_bound(s, cache);
   if (stt) return stt;
   const bool open = s->d.link == PULSE_LINK_OPEN;
-  if (!d_x_in || !d_temb || !d_d_out || mb < 0) return fail(PULSE_ERR_INVALID_ARG, "null x_in / temb / d_out or negative mb_id");
-  if (open && (!d_h_in || !d_e_out)) return fail(PULSE_ERR_INVALID_ARG, "OPEN stage needs h_in and e_out");
+  const bool enc = parts & PART_ENC, dec = parts & PART_DEC;
+  if (parts != PART_ALL && !(s->d.flags & PULSE_FLAG_SPLIT)) return fail(PULSE_ERR_STATE, "the two-call forms need PULSE_FLAG_SPLIT");
+  if (mb < 0) return fail(PULSE_ERR_INVALID_ARG, "negative mb_id");
+  if (enc && (!d_x_in || !d_temb)) return fail(PULSE_ERR_INVALID_ARG, "null x_in / temb");
+  if (dec && !d_d_out) return fail(PULSE_ERR_INVALID_ARG, "null d_out");
+  if (open && ((enc && !d_e_out) || (dec && !d_h_in))) return fail(PULSE_ERR_INVALID_ARG, "OPEN stage needs h_in and e_out");
   if (!open && (d_h_in || d_e_out)) return fail(PULSE_ERR_INVALID_ARG, "CLOSED stage takes no h_in / e_out");
   int slot = -1;
-  for (int i = 0; i < cache->slots; ++i) {
-    if (cache->mb[i] == mb) return fail(PULSE_ERR_CACHE, "microbatch %lld is already live", (long long)mb);
-    if (cache->mb[i] < 0 && slot < 0) slot = i;
+  if (enc) {
+    for (int i = 0; i < cache->slots; ++i) {
+      if (cache->mb[i] == mb) return fail(PULSE_ERR_CACHE, "microbatch %lld is already live", (long long)mb);
+      if (cache->mb[i] < 0 && slot < 0) slot = i;
+    }
+    if (slot < 0) return fail(PULSE_ERR_CACHE, "skip cache full (%d slots)", cache->slots);
+  } else {
+    for (int i = 0; i < cache->slots; ++i) if (cache->mb[i] == mb) slot = i;
+    if (slot < 0 || cache->phase[slot] != 1)
+      return fail(PULSE_ERR_STATE, "forward_dec of microbatch %lld without a forward_enc", (long long)mb);
   }
-  if (slot < 0) return fail(PULSE_ERR_CACHE, "skip cache full (%d slots)", cache->slots);
   Ctx c;
   c.s = s; c.st = (cudaStream_t)stream; c.dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
   c.skip = cache->base + (size_t)slot * cache->bytes_per_slot;
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
+  const int n_first = s->n_enc + s->n_mid, nops = (int)s->ops.size();
+  c.op_lo = enc ? 0 : n_first; c.op_hi = dec ? nops : n_first;
   float* emb = (float*)(c.stash + s->emb_off);
-  if (s->tensors[s->t_dout].ref.region == R_STASH && ((uintptr_t)d_d_out & 255) == 0) { c.ov_ft = s->t_dout; c.ov_fp = (char*)d_d_out; }
-  if (s->cst_end > s->cst_begin) CK_CUDA(cudaMemsetAsync(c.stash + s->cst_begin, 0, s->cst_end - s->cst_begin, c.st));
+  if (dec && s->tensors[s->t_dout].ref.region == R_STASH && ((uintptr_t)d_d_out & 255) == 0) { c.ov_ft = s->t_dout; c.ov_fp = (char*)d_d_out; }
   // a boundary tensor that a GroupNorm reads is stashed and measured in one pass (stash_in below); the rest are copies
   const bool fuse_x = s->tensors[s->t_xin].gn_input, fuse_h = open && s->tensors[s->t_hin].gn_input;
-  if (!fuse_x) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
-  if (!d_t) CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
-  if (open && !fuse_h) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
+  if (enc) {
+    // channel stats of every GroupNorm input of the slot, both halves: zeroed once, when the slot is taken
+    if (s->cst_end > s->cst_begin) CK_CUDA(cudaMemsetAsync(c.stash + s->cst_begin, 0, s->cst_end - s->cst_begin, c.st));
+    if (!fuse_x) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_xin), d_x_in, c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
+    if (!d_t) CK_CUDA(cudaMemcpyAsync(emb, d_temb, (size_t)s->d.n * s->d.temb_dim * 4, cudaMemcpyDeviceToDevice, c.st));
+  }
+  if (dec && open && !fuse_h) CK_CUDA(cudaMemcpyAsync(c.fwd(s->t_hin), d_h_in, c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
   setup_side(s, c);
-  {   // beside the chain (side stream): (one-call form) the timestep MLP, then p[n,c] = Wt SiLU(emb) + bt of every
-      // ResBlock in one launch (row a1), joined before the first conv1
+  if (enc) {   // beside the chain (side stream): (one-call form) the timestep MLP, then p[n,c] = Wt SiLU(emb) + bt of every
+               // ResBlock of BOTH halves in one launch (row a1), joined before the first conv1
     c.fork();
     OnSide g(c);
     if (d_t) {
@@ -541,9 +561,9 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
     Prof pr(s, c.st, PULSE_KCLASS_GN_FWD, 0.0, 0.0);
     s->launches += chan_stats(c.dt, src, s->d.n, T.ref.h * T.ref.w, T.ref.c, cst_of(c, t), c.st, c.fwd(t));
   };
-  if (fuse_x) stash_in(s->t_xin, d_x_in);
-  if (fuse_h) stash_in(s->t_hin, d_h_in);
-  for (size_t i = 0; i < s->ops.size(); ++i) {
+  if (enc && fuse_x) stash_in(s->t_xin, d_x_in);
+  if (dec && fuse_h) stash_in(s->t_hin, d_h_in);
+  for (int i = c.op_lo; i < c.op_hi; ++i) {
     const OpPlan& op = s->ops[i];
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_forward(c, op); break;
@@ -578,19 +598,23 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
   if (c.side) c.wait_side(c.mark_side());       // join
   if (s->last_was_backward) s->wt_valid = false;      // a forward after a backward starts a new step: the parameters may have changed
   s->last_was_backward = false;
-  if (open) CK_CUDA(cudaMemcpyAsync(d_e_out, c.fwd(s->t_eout), c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
-  if (c.ov_ft < 0) CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+  if (enc && open) CK_CUDA(cudaMemcpyAsync(d_e_out, c.fwd(s->t_eout), c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
+  if (dec && c.ov_ft < 0) CK_CUDA(cudaMemcpyAsync(d_d_out, c.fwd(s->t_dout), c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
-  cache->mb[slot] = mb;
-  cache->live++;
-  const size_t lb = (size_t)cache->live * cache->bytes_per_slot;
-  if (lb > cache->peak_bytes) cache->peak_bytes = lb;
+  if (enc) {
+    cache->mb[slot] = mb;
+    cache->live++;
+    const size_t lb = (size_t)cache->live * cache->bytes_per_slot;
+    if (lb > cache->peak_bytes) cache->peak_bytes = lb;
+  }
+  cache->phase[slot] = dec ? 2 : 1;
   return PULSE_OK;
 }
 extern "C" pulse_status_t pulse_stage_forward(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
                                               const void* d_x_in, const void* d_h_in, const float* d_temb,
                                               void* d_e_out, void* d_d_out, void* stream) {
+  if (!d_x_in || !d_temb || !d_d_out) return fail(PULSE_ERR_INVALID_ARG, "null x_in / temb / d_out");
   return forward_impl(s, cache, mb, d_x_in, d_h_in, const_cast<float*>(d_temb), nullptr, nullptr, d_e_out, d_d_out, stream);
 }
 extern "C" pulse_status_t pulse_stage_forward_temb(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb,
@@ -598,61 +622,92 @@ extern "C" pulse_status_t pulse_stage_forward_temb(pulse_stage_t* s, pulse_skip_
                                                    float* d_emb, float* d_temb_stash, void* d_e_out, void* d_d_out,
                                                    void* stream) {
   if (!d_t || !d_emb || !d_temb_stash) return fail(PULSE_ERR_INVALID_ARG, "null t / emb / temb stash");
+  if (!d_x_in || !d_d_out) return fail(PULSE_ERR_INVALID_ARG, "null x_in / d_out");
   return forward_impl(s, cache, mb, d_x_in, d_h_in, d_emb, d_t, d_temb_stash, d_e_out, d_d_out, stream);
+}
+extern "C" pulse_status_t pulse_stage_forward_enc(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_x_in,
+                                                  const float* d_temb, void* d_e_out, void* stream) {
+  return forward_impl(s, cache, mb, d_x_in, nullptr, const_cast<float*>(d_temb), nullptr, nullptr, d_e_out, nullptr, stream, PART_ENC);
+}
+extern "C" pulse_status_t pulse_stage_forward_dec(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_h_in,
+                                                  void* d_d_out, void* stream) {
+  return forward_impl(s, cache, mb, nullptr, d_h_in, nullptr, nullptr, nullptr, nullptr, d_d_out, stream, PART_DEC);
 }
 
 static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_g_d_out,
                                     const void* d_g_e_out, void* d_g_x_in, void* d_g_h_in, float* d_g_temb,
-                                    const float* d_temb_stash, int accumulate_wgrad, void* stream) {
+                                    const float* d_temb_stash, int accumulate_wgrad, void* stream, int parts = PART_ALL) {
   pulse_status_t stt = check_bound(s, cache);
   if (stt) return stt;
+  if (parts == PART_ALL && (s->d.flags & PULSE_FLAG_SPLIT)) {      // a split stage runs its one-call backward as the two halves
+    stt = backward_impl(s, cache, mb, d_g_d_out, nullptr, nullptr, d_g_h_in, d_g_temb, nullptr, accumulate_wgrad, stream, PART_DEC);
+    if (stt) return stt;
+    return backward_impl(s, cache, mb, nullptr, d_g_e_out, d_g_x_in, nullptr, d_g_temb, d_temb_stash, 1, stream, PART_ENC);
+  }
   const bool open = s->d.link == PULSE_LINK_OPEN;
-  if (!d_g_d_out || mb < 0) return fail(PULSE_ERR_INVALID_ARG, "null g_d_out or negative mb_id");
-  if (open && !d_g_h_in) return fail(PULSE_ERR_INVALID_ARG, "OPEN stage needs g_h_in");
+  const bool enc = parts & PART_ENC, dec = parts & PART_DEC;
+  if (parts != PART_ALL && !(s->d.flags & PULSE_FLAG_SPLIT)) return fail(PULSE_ERR_STATE, "the two-call forms need PULSE_FLAG_SPLIT");
+  if (mb < 0 || (dec && !d_g_d_out)) return fail(PULSE_ERR_INVALID_ARG, "null g_d_out or negative mb_id");
+  if (open && dec && !d_g_h_in) return fail(PULSE_ERR_INVALID_ARG, "OPEN stage needs g_h_in");
   if (!open && (d_g_h_in || d_g_e_out)) return fail(PULSE_ERR_INVALID_ARG, "CLOSED stage takes no g_h_in / g_e_out");
   int slot = -1;
   for (int i = 0; i < cache->slots; ++i) if (cache->mb[i] == mb) slot = i;
   if (slot < 0) return fail(PULSE_ERR_STATE, "backward of microbatch %lld without a live forward", (long long)mb);
+  if (cache->phase[slot] != (dec ? 2 : 3))
+    return fail(PULSE_ERR_STATE, "microbatch %lld: calls out of order (forward_enc, forward_dec, backward_dec, backward_enc)", (long long)mb);
   Ctx c;
   c.s = s; c.st = (cudaStream_t)stream; c.dt = s->d.dtype == PULSE_F32 ? DT_F32 : DT_BF16;
   c.skip = cache->base + (size_t)slot * cache->bytes_per_slot;
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
-  c.emb = (const float*)(c.stash + s->emb_off); c.g_temb = d_g_temb; c.temb_stash = d_temb_stash; c.acc_w = accumulate_wgrad;
+  c.emb = (const float*)(c.stash + s->emb_off); c.g_temb = d_g_temb; c.temb_stash = enc ? d_temb_stash : nullptr; c.acc_w = accumulate_wgrad;
+  const int n_first = s->n_enc + s->n_mid, nops = (int)s->ops.size();
+  c.op_lo = enc ? 0 : n_first; c.op_hi = dec ? nops : n_first;
   setup_side(s, c);
   // flipped / transposed weights for the dgrad convs, beside the memsets / column sums that open the backward (side
   // stream): first those of the last op (waited for before its dgrad), then the rest (waited for before the next op)
   int ev_wt_first = -1, ev_wt_rest = -1;
-  const int nops = (int)s->ops.size();
   if (!s->wt_valid) {
     c.fork();
     {
       OnSide g(c);
-      prepare_weights(c, nops - 1, nops);
+      prepare_weights(c, c.op_hi - 1, c.op_hi);
       if (c.side) ev_wt_first = c.mark_side();
-      prepare_weights(c, 0, nops - 1);
+      prepare_weights(c, 0, c.op_hi - 1);
+      if (c.op_hi < nops) prepare_weights(c, c.op_hi, nops);
       if (c.side) ev_wt_rest = c.mark_side();
     }
     s->wt_valid = true;
   }
-  if (!accumulate_wgrad)
+  if (dec && !accumulate_wgrad)
     CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
   CK_CUDA(cudaMemsetAsync(c.work + s->zero_begin, 0, s->zero_end - s->zero_begin, c.st));
+  const bool split = parts != PART_ALL;
   const bool al = (((uintptr_t)d_g_d_out | (uintptr_t)d_g_h_in | (uintptr_t)d_g_x_in) & 255) == 0;
-  if (al) { c.ov_gt[0] = s->t_dout; c.ov_gp[0] = (char*)const_cast<void*>(d_g_d_out); }       // read in place
-  else CK_CUDA(cudaMemcpyAsync(c.grad(s->t_dout), d_g_d_out, c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
-  if (al && open && s->t_hin != s->t_dout) { c.ov_gt[1] = s->t_hin; c.ov_gp[1] = (char*)d_g_h_in; }
-  if (al && d_g_x_in && s->t_xin != s->t_dout && s->t_xin != s->t_eout) { c.ov_gt[2] = s->t_xin; c.ov_gp[2] = (char*)d_g_x_in; }
-  if (open) {
-    if (d_g_e_out) CK_CUDA(cudaMemcpyAsync(c.grad(s->t_eout), d_g_e_out, c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
-    else CK_CUDA(cudaMemsetAsync(c.grad(s->t_eout), 0, c.bytes(s->t_eout), c.st));
+  if (dec) {
+    if (al) { c.ov_gt[0] = s->t_dout; c.ov_gp[0] = (char*)const_cast<void*>(d_g_d_out); }       // read in place
+    else CK_CUDA(cudaMemcpyAsync(c.grad(s->t_dout), d_g_d_out, c.bytes(s->t_dout), cudaMemcpyDeviceToDevice, c.st));
+    if (al && open && s->t_hin != s->t_dout) { c.ov_gt[1] = s->t_hin; c.ov_gp[1] = (char*)d_g_h_in; }
   }
-  for (int i = (int)s->ops.size() - 1; i >= 0; --i) {
+  // g_x_in lives in the caller's buffer only when one call writes all of it (not a per-slot skip gradient of a split stage)
+  if (enc && al && d_g_x_in && s->t_xin != s->t_dout && s->t_xin != s->t_eout && !s->tensors[s->t_xin].g_in_stash) {
+    c.ov_gt[2] = s->t_xin; c.ov_gp[2] = (char*)d_g_x_in;
+  }
+  if (enc && open) {
+    if (split && s->eout_grad_by_dec) {        // the decoder half wrote the skip gradient of e_out first: g_e_out adds to it
+      if (d_g_e_out) s->launches += add_inplace(c.dt, c.grad(s->t_eout), d_g_e_out, c.bytes(s->t_eout) / s->esz(), c.st);
+    } else if (d_g_e_out) {
+      CK_CUDA(cudaMemcpyAsync(c.grad(s->t_eout), d_g_e_out, c.bytes(s->t_eout), cudaMemcpyDeviceToDevice, c.st));
+    } else {
+      CK_CUDA(cudaMemsetAsync(c.grad(s->t_eout), 0, c.bytes(s->t_eout), c.st));
+    }
+  }
+  for (int i = c.op_hi - 1; i >= c.op_lo; --i) {
     const OpPlan& op = s->ops[i];
     const int n = s->d.n;
-    c.last_op = i == 0;
-    if (i == nops - 1) c.wait_side(ev_wt_first);
-    if (i == nops - 2) c.wait_side(ev_wt_rest);
+    c.last_op = i == c.op_lo;
+    if (i == c.op_hi - 1) c.wait_side(ev_wt_first);
+    if (i == c.op_hi - 2) c.wait_side(ev_wt_rest);
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_backward(c, op); break;
       case PULSE_OP_ATTN: attn_backward(c, op); break;
@@ -676,29 +731,20 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
         char* g_u = c.work + s->w_gu;
         ensure_colsum(c, op.out);
         const bool wg2 = up2_wg(c, op), dg2 = up2_dg(c, op);
-        if (wg2 || dg2) {
-          c.fork();
-          if (wg2) {
-            run_wgrad(c, up2_wgrad_args(c, op, g_out));
-          } else {          // (then the forward was the materialised form too: u exists)
-            WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
-                        1, c.pgrad(op.p[P_C1W])};
-            run_wgrad(c, w);
-          }
-          if (dg2) {
-            run_conv(c, up2_dgrad_args(c, op, g_out));
-          } else {
-            run_dgrad(c, g_out, op.hout, op.wout, op.cout, op.wt1, 3, op.cin, g_u, 0, 1, op.hout, op.wout);
-            s->launches += upsample2_bwd(c.dt, g_u, n, op.hin, op.win, op.cin, c.grad(op.x0), c.st);
-          }
-          break;
-        }
-        WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
-                    1, c.pgrad(op.p[P_C1W])};
         c.fork();
-        run_wgrad(c, w);
-        run_dgrad(c, g_out, op.hout, op.wout, op.cout, op.wt1, 3, op.cin, g_u, 0, 1, op.hout, op.wout);
-        s->launches += upsample2_bwd(c.dt, g_u, n, op.hin, op.win, op.cin, c.grad(op.x0), c.st);
+        if (wg2) {
+          run_wgrad(c, up2_wgrad_args(c, op, g_out));
+        } else {          // (then the forward was the materialised form too: u exists)
+          WgradArgs w{c.dt, Cat{c.fwd(op.u), op.cin, nullptr, 0}, n, op.hout, op.wout, g_out, op.hout, op.wout, op.cout, 3,
+                      1, c.pgrad(op.p[P_C1W])};
+          run_wgrad(c, w);
+        }
+        if (dg2) {
+          run_conv(c, up2_dgrad_args(c, op, g_out));
+        } else {
+          run_dgrad(c, g_out, op.hout, op.wout, op.cout, op.wt1, 3, op.cin, g_u, 0, 1, op.hout, op.wout);
+          s->launches += upsample2_bwd(c.dt, g_u, n, op.hin, op.win, op.cin, c.grad(op.x0), c.st);
+        }
         break;
       }
       case PULSE_OP_HEAD: {
@@ -727,12 +773,17 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
     cudaStreamWaitEvent(c.st, e, 0);
   }
   if (c.side) c.wait_side(c.mark_side());      // join: the caller's stream sees every weight gradient complete
-  if (open && c.ov_gt[1] < 0) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
-  if (d_g_x_in && c.ov_gt[2] < 0) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
+  if (dec && open && c.ov_gt[1] < 0) CK_CUDA(cudaMemcpyAsync(d_g_h_in, c.grad(s->t_hin), c.bytes(s->t_hin), cudaMemcpyDeviceToDevice, c.st));
+  if (enc && d_g_x_in && c.ov_gt[2] < 0) CK_CUDA(cudaMemcpyAsync(d_g_x_in, c.grad(s->t_xin), c.bytes(s->t_xin), cudaMemcpyDeviceToDevice, c.st));
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
-  cache->mb[slot] = -1;
-  cache->live--;
+  if (enc) {
+    cache->mb[slot] = -1;
+    cache->phase[slot] = 0;
+    cache->live--;
+  } else {
+    cache->phase[slot] = 3;
+  }
   s->last_was_backward = true;
   return PULSE_OK;
 }
@@ -747,6 +798,14 @@ extern "C" pulse_status_t pulse_stage_backward_temb(pulse_stage_t* s, pulse_skip
                                                     int accumulate_wgrad, void* stream) {
   if (!d_g_temb || !d_temb_stash) return fail(PULSE_ERR_INVALID_ARG, "null g_temb / temb stash");
   return backward_impl(s, cache, mb, d_g_d_out, d_g_e_out, d_g_x_in, d_g_h_in, d_g_temb, d_temb_stash, accumulate_wgrad, stream);
+}
+extern "C" pulse_status_t pulse_stage_backward_dec(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_g_d_out,
+                                                   void* d_g_h_in, float* d_g_temb, int accumulate_wgrad, void* stream) {
+  return backward_impl(s, cache, mb, d_g_d_out, nullptr, nullptr, d_g_h_in, d_g_temb, nullptr, accumulate_wgrad, stream, PART_DEC);
+}
+extern "C" pulse_status_t pulse_stage_backward_enc(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_g_e_out,
+                                                   void* d_g_x_in, float* d_g_temb, void* stream) {
+  return backward_impl(s, cache, mb, nullptr, d_g_e_out, d_g_x_in, nullptr, d_g_temb, nullptr, 1, stream, PART_ENC);
 }
 
 // ------------------------------------------------------------------------------ temb, loss

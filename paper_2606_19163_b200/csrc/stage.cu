@@ -53,7 +53,10 @@ struct Planner {
     t.ref.region = region; t.ref.c = c; t.ref.h = h; t.ref.w = w;
     const size_t bytes = (size_t)s->d.n * h * w * c * s->esz();
     t.ref.off = bump(region, bytes);
-    t.goff = need_grad ? bump(R_WORK, bytes) : 0;
+    // split (pipeline) stages keep the gradient of a cached skip per in-flight microbatch: it is written by the backward
+    // of the decoder half and read by the backward of the encoder half, with other microbatches' halves in between
+    t.g_in_stash = need_grad && region == R_SKIP && (s->d.flags & PULSE_FLAG_SPLIT);
+    t.goff = need_grad ? bump(t.g_in_stash ? R_STASH : R_WORK, bytes) : 0;
     s->tensors.push_back(t);
     return (int)s->tensors.size() - 1;
   }
@@ -229,11 +232,19 @@ static pulse_status_t build_plan(pulse_stage* s) {
   // backward write modes: first writer of a gradient buffer stores, later writers add.  A gradient's pixel
   // sums come fused from its writers when ALL of them are GroupNorm-backward launches (norm.cu); a gradient
   // that enters from outside or is written by a conv / upsample adjoint gets a colsum pass instead.
+  const bool split = (d.flags & PULSE_FLAG_SPLIT) != 0;
+  if (split && d.link != PULSE_LINK_OPEN) return fail(PULSE_ERR_SHAPE, "PULSE_FLAG_SPLIT needs an OPEN stage");
   std::vector<char> written(s->tensors.size(), 0);
   written[s->t_dout] = 1; s->tensors[s->t_dout].cs_fused = false;
-  if (s->t_eout >= 0) { written[s->t_eout] = 1; s->tensors[s->t_eout].cs_fused = false; }
+  // one-call form: g_e_out is written first, the skip gradient of a decoder op then adds to it.  Split form: the decoder
+  // half runs BEFORE g_e_out arrives, so it is the first writer and g_e_out is added at the start of backward_enc
+  if (s->t_eout >= 0) { written[s->t_eout] = split ? 0 : 1; s->tensors[s->t_eout].cs_fused = false; }
   for (int i = (int)s->ops.size() - 1; i >= 0; --i) {
     OpPlan& op = s->ops[i];
+    if (split && i == s->n_enc + s->n_mid - 1 && s->t_eout >= 0) {      // the encoder half starts: g_e_out has been merged
+      s->eout_grad_by_dec = written[s->t_eout] != 0;
+      written[s->t_eout] = 1;
+    }
     op.acc_x0 = written[op.x0]; written[op.x0] = 1;
     if (op.x1 >= 0) { op.acc_x1 = written[op.x1]; written[op.x1] = 1; }
     if (op.kind == PULSE_OP_CONV_IN || op.kind == PULSE_OP_DOWN || op.kind == PULSE_OP_UP)
@@ -241,6 +252,9 @@ static pulse_status_t build_plan(pulse_stage* s) {
     if ((op.kind == PULSE_OP_UP || op.kind == PULSE_OP_HEAD) && op.acc_x0)
       return fail(PULSE_ERR_UNSUPPORTED, "up/head input with a second consumer");
   }
+  // split form: the pixel sums of a cached skip's gradient cannot be collected from its two writers (they run in
+  // different calls): one column-sum pass over the final gradient in backward_enc instead
+  if (split) for (int t : s->skip_tensor) s->tensors[t].cs_fused = false;
 
   // slot stash: channel stats of every tensor a GroupNorm reads, one contiguous area (zeroed per forward)
   s->cst_begin = pl.bump(R_STASH, 0);
@@ -375,6 +389,7 @@ extern "C" pulse_status_t pulse_skip_cache_create(pulse_stage_t* s, void* d_mem,
   if (!c) return fail(PULSE_ERR_INVALID_ARG, "out of host memory");
   c->stage = s; c->base = (char*)d_mem; c->slots = slots; c->bytes_per_slot = s->skip_bytes;
   c->mb.assign(slots, -1);
+  c->phase.assign(slots, 0);
   *out = c;
   return PULSE_OK;
 }

@@ -44,7 +44,8 @@ struct OpPlan {
 
 struct Tensor {
   TRef ref;              // forward value
-  size_t goff = 0;       // gradient buffer (R_WORK), same shape/dtype
+  size_t goff = 0;       // gradient buffer (R_WORK; per-slot R_STASH if g_in_stash), same shape/dtype
+  bool g_in_stash = false;   // PULSE_FLAG_SPLIT: gradient of a cached skip, kept per in-flight microbatch
   bool gn_input = false; // read by a GroupNorm site: carries channel stats
   size_t cst = NO_OFF;   // R_STASH (zeroed area): channel stats [n][2][c] fp32 of the forward value
   bool is_out = false;   // output of an op with a bias: its gradient's pixel sums are needed
@@ -80,6 +81,7 @@ struct pulse_stage {
   size_t cst_begin = 0, cst_end = 0;        // slot stash: channel-stats area, zeroed at the start of forward
   size_t zero_begin = 0, zero_end = 0;      // workspace: backward sums area, zeroed at the start of backward
   bool wt_valid = false;                    // transposed weights match the bound parameters
+  bool eout_grad_by_dec = false;            // PULSE_FLAG_SPLIT: a decoder op writes the gradient of e_out before g_e_out arrives
   bool wp_valid = false;                    // pre-summed phase weights of the up convs (forward) match them
   // per-stage workspace offsets (bytes)
   size_t w_ga2 = 0, w_gh1 = 0, w_gh1b = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0, w_gqkv = 0;
@@ -105,5 +107,6 @@ struct pulse_skip_cache {
   pulse_stage* stage;
   char* base; int slots; size_t bytes_per_slot;
   std::vector<int64_t> mb;     // microbatch id per slot, -1 = free
+  std::vector<int> phase;      // split calls: 1 forward_enc done, 2 forward_dec done, 3 backward_dec done
   int live = 0; size_t peak_bytes = 0;
 };

@@ -67,8 +67,10 @@ def _unet(name, n, hw, levels, microbatches=1, dtype="bf16", groups=32, temb=Non
 
 
 def config(i: int) -> dict:
-    """The five configs of BASELINE.json, 1-based, read as SURVEY.md 8c R1-R20."""
+    """The five configs of BASELINE.json, 1-based, read as SURVEY.md 8c R1-R20; 6 = attn_level() (row f1)."""
     mlp = {"kind": "mlp", "d0": 320, "dim": 1280}
+    if i == 6:
+        return attn_level()
     if i == 1:
         return _stage("config1", "fp32", 2, 16, 16, 32, 8, {"kind": "sinusoidal", "d0": 128, "dim": 128},
                       "open", 0, [rb(32, 32, push=1)], [], [rb(32, 32, skip=32)])
@@ -86,6 +88,16 @@ def config(i: int) -> dict:
     if i == 5:
         return _unet("config5", 2, 128, [320, 640, 1280], microbatches=8)
     raise ValueError(i)
+
+
+def attn_level() -> dict:
+    """configs[2]'s level-2 stage with a self-attention block (640 channels = 10 heads x 64, 1024
+    tokens) after every ResBlock, as in an SD-shaped UNet level; skips are pushed after the attention."""
+    mlp = {"kind": "mlp", "d0": 320, "dim": 1280}
+    return _stage("attn_level", "bf16", 8, 32, 32, 320, 32, mlp, "open", 1,
+                  [rb(320, 640), attn(640, 10, push=1), rb(640, 640), attn(640, 10, push=1), _op(DOWN, 640, 640)], [],
+                  [rb(640, 640, skip=640), attn(640, 10), rb(640, 640, skip=640), attn(640, 10), rb(640, 640, skip=320),
+                   attn(640, 10), _op(UP, 640, 640)])
 
 
 def mini(kind: str, dtype: str = "fp32") -> dict:
@@ -144,6 +156,47 @@ def gpu_mid(kind: str) -> dict:
                       [rb(320, 320), attn(320, 5, push=1)], [],
                       [rb(320, 320, skip=320), attn(320, 5), rb(320, 320, skip=320)])
     raise ValueError(kind)
+
+
+def split_closed(desc: dict, k_enc: int) -> tuple:
+    """Cut a CLOSED whole-model structure into an OPEN outer stage and a CLOSED inner stage for two pipeline devices
+    (a stage pair = a contiguous encoder-side op range plus the decoder-side range that
+    consumes its skips).  The outer stage takes enc_ops[:k_enc] and the decoder suffix that pops exactly their skips.
+    Returns (outer, inner, name map): map[stage][stage param prefix] = whole-model param prefix."""
+    enc, dec = desc["enc_ops"], desc["dec_ops"]
+    pushes = desc["x_in_is_skip"] + sum(op["push"] for op in enc[:k_enc])
+    j, pops = len(dec), 0
+    while pops < pushes:
+        j -= 1
+        pops += 1 if dec[j]["skip"] else 0
+    assert pops == pushes and j > 0, "cut does not separate whole skip pairs"
+    h = w = desc["h"]
+    for op in enc[:k_enc]:
+        if op["kind"] == DOWN:
+            h, w = h // 2, w // 2
+    outer = _stage(desc["name"] + "_outer", desc["dtype"], desc["n"], desc["h"], desc["w"], desc["c_in"], desc["groups"],
+                   desc["temb"], "open", desc["x_in_is_skip"], copy.deepcopy(enc[:k_enc]), [], copy.deepcopy(dec[j:]),
+                   microbatches=desc["microbatches"], eps=desc["eps"])
+    inner = _stage(desc["name"] + "_inner", desc["dtype"], desc["n"], h, w, enc[k_enc - 1]["cout"], desc["groups"], desc["temb"],
+                   "closed", 0, copy.deepcopy(enc[k_enc:]), copy.deepcopy(desc["mid_ops"]), copy.deepcopy(dec[:j]),
+                   microbatches=desc["microbatches"], eps=desc["eps"])
+    names = {"outer": {f"enc{i}.": f"enc{i}." for i in range(k_enc)}, "inner": {f"enc{i}.": f"enc{k_enc + i}." for i in range(len(enc) - k_enc)}}
+    names["outer"].update({f"dec{i}.": f"dec{j + i}." for i in range(len(dec) - j)})
+    names["inner"].update({f"dec{i}.": f"dec{i}." for i in range(j)})
+    names["inner"].update({f"mid{i}.": f"mid{i}." for i in range(len(desc["mid_ops"]))})
+    for k in names:
+        names[k]["temb."] = "temb."
+    return outer, inner, names
+
+
+def stage_params(whole_params: dict, names: dict) -> dict:
+    """Parameters of one stage of split_closed() out of the whole model's (same arrays, renamed)."""
+    out = {}
+    for sp, wp in names.items():
+        for k, v in whole_params.items():
+            if k.startswith(wp):
+                out[sp + k[len(wp):]] = v
+    return out
 
 
 # ----------------------------------------------------------------------------- structure walks

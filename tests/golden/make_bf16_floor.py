@@ -39,6 +39,7 @@ CASES["mid_level_1f1b"] = (W.scaled(W.gpu_mid("level"), microbatches=3, name="mi
 CASES["config2"] = (W.config(2), 0, False, torch.float64)
 CASES["config2_n3"] = (W.scaled(W.config(2), n=3, name="config2_n3"), 0, False, torch.float64)      # __graft_entry__.smoke()
 CASES["config3"] = (W.config(3), 0, False, torch.float32)
+CASES["attn_level"] = (W.attn_level(), 0, False, torch.float32)
 CASES["config4"] = (W.config(4), 0, False, torch.float32)
 CASES["config5_wave2"] = (W.scaled(W.config(5), microbatches=2, name="config5_wave2"), 0, False, torch.float32)
 CASES["config5"] = (W.config(5), 0, False, torch.float32)
