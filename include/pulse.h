@@ -49,7 +49,11 @@ typedef enum {
 enum { PULSE_F32 = 0, PULSE_BF16 = 1 };
 enum { PULSE_OP_CONV_IN = 0, PULSE_OP_RESBLOCK = 1, PULSE_OP_DOWN = 2, PULSE_OP_UP = 3, PULSE_OP_HEAD = 4,
        PULSE_OP_ATTN = 5 /* self-attention block: GroupNorm -> 1x1 conv to q|k|v -> softmax(q k^T / sqrt(d)) v
-                            per head over the H W pixels -> 1x1 conv, + residual; cin == cout, heads | cin */ };
+                            per head over the H W pixels -> 1x1 conv, + residual; cin == cout, heads | cin */,
+       PULSE_OP_TBLOCK = 6 /* transformer block with an optional long skip:
+                              [x = Linear(concat_C(x, skip)) where skip_channels > 0 ("concat + Linear")];
+                              x = x + proj(attention(qkv(LayerNorm(x)))); x = x + fc2(GELU(fc1(LayerNorm(x)))), fc1: c -> 4c;
+                              tokens = the H W pixels, Linear = 1x1 conv; cin == cout, heads | cin; takes no timestep input */ };
 enum { PULSE_LINK_OPEN = 0, PULSE_LINK_CLOSED = 1 };
 enum { PULSE_TEMB_SINUSOIDAL = 0, PULSE_TEMB_MLP = 1 };
 /* stage flags (cross-checks: same arithmetic, different kernel / summation order) */
@@ -121,7 +125,9 @@ pulse_status_t pulse_stage_destroy(pulse_stage_t* stage);
 /* Parameters, in the fixed order temb MLP (w1,b1,w2,b2), then per op of enc, mid, dec:
  * ResBlock: gn1.gamma gn1.beta conv1.w conv1.b temb.w temb.b gn2.gamma gn2.beta conv2.w
  * conv2.b [sc.w sc.b if cin+skip != cout]; conv_in/down/up: conv.w conv.b; head: gn.gamma
- * gn.beta conv.w conv.b; attention: gn.gamma gn.beta qkv.w [3c][1][1][c] qkv.b proj.w [c][1][1][c] proj.b.  name points into the handle (valid until destroy). */
+ * gn.beta conv.w conv.b; attention: gn.gamma gn.beta qkv.w [3c][1][1][c] qkv.b proj.w [c][1][1][c] proj.b;
+ * transformer block: [skip.w [c][1][1][c+skip] skip.b] ln1.gamma ln1.beta qkv.w qkv.b proj.w proj.b ln2.gamma ln2.beta
+ * fc1.w [4c][1][1][c] fc1.b fc2.w [c][1][1][4c] fc2.b.  name points into the handle (valid until destroy). */
 pulse_status_t pulse_stage_param_count(const pulse_stage_t* stage, int* count);
 pulse_status_t pulse_stage_param_info(const pulse_stage_t* stage, int index, const char** name, int* rank,
                                       int shape[4], size_t* offset_bytes, size_t* grad_offset_bytes);

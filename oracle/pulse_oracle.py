@@ -203,6 +203,92 @@ def attn_block_bwd(P, p, ctx, g_out, G):
     return g_x + g_out
 
 
+# --------------------------------------------------------------------------- transformer block with a long skip
+
+def ln_fwd(x, gamma, beta, eps):
+    """LayerNorm over the channels of every token (pixel): y = gamma xhat + beta, biased variance, eps inside the sqrt."""
+    c = x.shape[1]
+    mu = x.mean(dim=1, keepdim=True)
+    var = ((x - mu) ** 2).mean(dim=1, keepdim=True)
+    r = 1.0 / torch.sqrt(var + eps)
+    xhat = (x - mu) * r
+    return gamma.view(1, c, 1, 1) * xhat + beta.view(1, c, 1, 1), {"xhat": xhat, "r": r}
+
+
+def ln_bwd(g_y, ctx, gamma):
+    """dgamma = sum g_y xhat; dbeta = sum g_y; q = g_y gamma; g_x = r (q - mean_c q - xhat mean_c (q xhat))."""
+    xhat, r = ctx["xhat"], ctx["r"]
+    c = xhat.shape[1]
+    q = g_y * gamma.view(1, c, 1, 1)
+    g_x = r * (q - q.mean(dim=1, keepdim=True) - xhat * (q * xhat).mean(dim=1, keepdim=True))
+    return g_x, (g_y * xhat).sum(dim=(0, 2, 3)), g_y.sum(dim=(0, 2, 3))
+
+
+def gelu(x):
+    """GELU(x) = x Phi(x), Phi the standard normal CDF (the exact erf form)."""
+    return 0.5 * x * (1.0 + torch.erf(x / math.sqrt(2.0)))
+
+
+def gelu_grad(x):
+    """Phi(x) + x phi(x)."""
+    return 0.5 * (1.0 + torch.erf(x / math.sqrt(2.0))) + x * torch.exp(-0.5 * x * x) / math.sqrt(2.0 * math.pi)
+
+
+def tblock_fwd(P, p, x, skip, eps, heads):
+    """Transformer block of a U-ViT / Hunyuan-DiT style stage (long skips between early and late
+    transformer blocks; reading R26): tokens are the H W pixels, Linear layers are 1x1 convs.
+      xs  = Linear_skip(concat_C(x, skip))      only where a cached skip is consumed ("concat + Linear")
+      x1  = xs + proj(attention(qkv(LN1(xs))))
+      out = x1 + fc2(GELU(fc1(LN2(x1))))        fc1: C -> 4C
+    st() marks the stored tensors."""
+    n, _, h, w = x.shape
+    xin = x if skip is None else torch.cat([x, skip], dim=1)
+    xs = x if skip is None else st(conv_fwd(xin, P[p + "skip.w"], P[p + "skip.b"]))
+    c = xs.shape[1]
+    l1, c1 = ln_fwd(xs, P[p + "ln1.gamma"], P[p + "ln1.beta"], eps)
+    l1 = st(l1)
+    qkv = st(conv_fwd(l1, P[p + "qkv.w"], P[p + "qkv.b"]))
+    q, k, v = (_heads(qkv[:, i * c:(i + 1) * c], heads) for i in range(3))
+    o, pr = attn_core_fwd(q, k, v)
+    o = st(_unheads(o, n, heads, h, w))
+    x1 = st(conv_fwd(o, P[p + "proj.w"], P[p + "proj.b"]) + xs)
+    l2, c2 = ln_fwd(x1, P[p + "ln2.gamma"], P[p + "ln2.beta"], eps)
+    l2 = st(l2)
+    f1 = st(conv_fwd(l2, P[p + "fc1.w"], P[p + "fc1.b"]))
+    g = st(gelu(f1))
+    out = st(conv_fwd(g, P[p + "fc2.w"], P[p + "fc2.b"]) + x1)
+    return out, {"xin": xin, "has_skip": skip is not None, "xs": xs, "c1": c1, "l1": l1, "q": q, "k": k, "v": v, "p": pr,
+                 "o": o, "x1": x1, "c2": c2, "l2": l2, "f1": f1, "g": g, "heads": heads, "ch": x.shape[1]}
+
+
+def tblock_bwd(P, p, ctx, g_out, G):
+    """Chain rule of tblock_fwd; adds parameter grads into G; returns the gradient of the block's input before it is
+    stored (of concat_C(x, skip) where a skip was consumed)."""
+    heads = ctx["heads"]
+    n, c, h, w = ctx["xs"].shape
+    hw = (h, w)
+    G[p + "fc2.w"], G[p + "fc2.b"] = conv_wgrad(ctx["g"], g_out, P[p + "fc2.w"].shape)
+    g_g = st(conv_dgrad(g_out, P[p + "fc2.w"], hw))
+    g_f1 = st(g_g * gelu_grad(ctx["f1"]))
+    G[p + "fc1.w"], G[p + "fc1.b"] = conv_wgrad(ctx["l2"], g_f1, P[p + "fc1.w"].shape)
+    g_l2 = st(conv_dgrad(g_f1, P[p + "fc1.w"], hw))
+    g_x1, G[p + "ln2.gamma"], G[p + "ln2.beta"] = ln_bwd(g_l2, ctx["c2"], P[p + "ln2.gamma"])
+    g_x1 = st(g_x1 + g_out)
+    G[p + "proj.w"], G[p + "proj.b"] = conv_wgrad(ctx["o"], g_x1, P[p + "proj.w"].shape)
+    g_o = st(conv_dgrad(g_x1, P[p + "proj.w"], hw))
+    g_q, g_k, g_v = attn_core_bwd(_heads(g_o, heads), ctx["q"], ctx["k"], ctx["v"], ctx["p"])
+    g_qkv = st(torch.cat([_unheads(t, n, heads, h, w) for t in (g_q, g_k, g_v)], dim=1))
+    G[p + "qkv.w"], G[p + "qkv.b"] = conv_wgrad(ctx["l1"], g_qkv, P[p + "qkv.w"].shape)
+    g_l1 = st(conv_dgrad(g_qkv, P[p + "qkv.w"], hw))
+    g_xs, G[p + "ln1.gamma"], G[p + "ln1.beta"] = ln_bwd(g_l1, ctx["c1"], P[p + "ln1.gamma"])
+    g_xs = g_xs + g_x1
+    if not ctx["has_skip"]:
+        return g_xs
+    g_xs = st(g_xs)
+    G[p + "skip.w"], G[p + "skip.b"] = conv_wgrad(ctx["xin"], g_xs, P[p + "skip.w"].shape)
+    return conv_dgrad(g_xs, P[p + "skip.w"], hw)
+
+
 # --------------------------------------------------------------------------- time embedding
 
 def sinusoidal(t, d, dtype=DT):
@@ -329,6 +415,8 @@ def stage_forward(desc, P, x_in, h_in, emb):
             x, c = resblock_fwd(P, p, x, emb, G_, eps)
         elif op["kind"] == "attn":
             x, c = attn_block_fwd(P, p, x, G_, eps, op["heads"])
+        elif op["kind"] == "tblock":
+            x, c = tblock_fwd(P, p, x, None, eps, op["heads"])
         elif op["kind"] in ("conv_in", "down"):
             s = 2 if op["kind"] == "down" else 1
             c = {"x": x, "stride": s}
@@ -361,6 +449,14 @@ def stage_forward(desc, P, x_in, h_in, emb):
             c["pop"], c["ch"] = key, op["cin"]
         elif op["kind"] == "attn":
             h, c = attn_block_fwd(P, p, h, G_, eps, op["heads"])
+        elif op["kind"] == "tblock":
+            sk = None
+            if op["skip"]:
+                key, sk = skips.pop()
+                assert sk.shape[1] == op["skip"] and h.shape[1] == op["cin"], (p, sk.shape, h.shape)
+            h, c = tblock_fwd(P, p, h, sk, eps, op["heads"])
+            if op["skip"]:
+                c["pop"] = key
         elif op["kind"] == "up":
             u = upsample2(h)
             c = {"u": u}
@@ -413,6 +509,11 @@ def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
             acc(c["pop"], g_x[:, c["ch"]:])
         elif op["kind"] == "attn":
             acc(kin, attn_block_bwd(P, p, c, g, G))
+        elif op["kind"] == "tblock":
+            g_x = tblock_bwd(P, p, c, g, G)
+            acc(kin, g_x[:, :c["ch"]])
+            if c["has_skip"]:
+                acc(c["pop"], g_x[:, c["ch"]:])
         elif op["kind"] == "up":
             G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["u"], g, P[p + "conv.w"].shape)
             acc(kin, upsample2_bwd(st(conv_dgrad(g, P[p + "conv.w"], c["u"].shape[2:]))))
@@ -443,6 +544,8 @@ def stage_backward(desc, P, ctx, g_d_out, g_e_out=None):
             acc(("e", i - 1), g_x)
         elif op["kind"] == "attn":
             acc(("e", i - 1), attn_block_bwd(P, p, c, g, G))
+        elif op["kind"] == "tblock":
+            acc(("e", i - 1), tblock_bwd(P, p, c, g, G))
         else:
             G[p + "conv.w"], G[p + "conv.b"] = conv_wgrad(c["x"], g, P[p + "conv.w"].shape, c["stride"])
             acc(("e", i - 1), conv_dgrad(g, P[p + "conv.w"], c["x"].shape[2:], c["stride"]))

@@ -19,7 +19,7 @@ if not os.path.exists(LIB_PATH):
 lib = C.CDLL(LIB_PATH)
 
 F32, BF16 = 0, 1
-OP_KIND = {"conv_in": 0, "resblock": 1, "down": 2, "up": 3, "head": 4, "attn": 5}
+OP_KIND = {"conv_in": 0, "resblock": 1, "down": 2, "up": 3, "head": 4, "attn": 5, "tblock": 6}
 FLAG_FORCE_SIMT = 1
 FLAG_GN_TWO_PASS = 2
 FLAG_CONV_PAIR = 4

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpulse.so")
-SOURCES = ["stage.cu", "exec.cu", "norm.cu", "norm_fused.cu", "misc.cu", "conv_simt.cu", "conv_thin.cu", "conv_tc.cu", "conv_tc2.cu", "wgrad_tc2.cu", "attention.cu", "attention_tc.cu", "partition.cpp"]
+SOURCES = ["stage.cu", "exec.cu", "norm.cu", "norm_fused.cu", "misc.cu", "conv_simt.cu", "conv_thin.cu", "conv_tc.cu", "conv_tc2.cu", "wgrad_tc2.cu", "attention.cu", "attention_tc.cu", "tblock.cu", "partition.cpp"]
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--use_fast_math",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

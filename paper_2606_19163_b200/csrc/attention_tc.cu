@@ -1,6 +1,7 @@
 // attention_tc.cu - tcgen05 forward of the attention core for bf16 tensors with 64 or 128 channels per head
-// (formulas in attention.cu).  One CTA = 128 queries of one (image, head); thread i owns query
-// row i = TMEM lane i, so the softmax needs no cross-thread reduction:
+// (formulas in attention.cu).  One CTA = 128 queries of one (image, head); query row i = TMEM lane i
+// is shared by the two threads i and 128 + i (warps w and w + 4 reach the same lane quadrant), each taking half of the
+// columns, so the softmax needs one exchange of the row maximum / sum per sweep and no shuffles:
 //   sweep 1 over the key tiles:  S = Q K^T (tcgen05.mma, M = 128, N = 128, K = d, both operands K-major from TMA boxes
 //                                of the interleaved qkv tensor) -> TMEM -> row maximum m_i
 //   sweep 2:                     S again -> p = 2^((s - m_i) scale log2 e) -> l_i += p, P as bf16 into a 128-byte-swizzled
@@ -35,13 +36,14 @@ template <int D> struct ACfg {
 struct AtcP { int T, C, heads; float scale; bf16* o; float* lse; };
 
 template <int D>
-__global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ CUtensorMap map, const AtcP p) {
+__global__ void __launch_bounds__(256, 2) attn_fwd_tc_k(const __grid_constant__ CUtensorMap map, const AtcP p) {
   using A = ACfg<D>;
   extern __shared__ uint8_t smem_raw[];
   __shared__ uint64_t bar_q, bar_kv, bar_s, bar_pv;
   __shared__ uint32_t tmem_base_s;
+  __shared__ float xch[2][2][BQ];            // [m | l, lx][column half][row]
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, row = threadIdx.x;
+  const int warp = threadIdx.x >> 5, row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;      // half: which 64 columns
   const int q0 = blockIdx.x * BQ, h = blockIdx.y, n = blockIdx.z;
   const int nkb = (p.T + BKEY - 1) / BKEY;
   if (threadIdx.x == 0) {
@@ -82,7 +84,7 @@ __global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ 
     }
     umma_commit(&bar_s);
   };
-  const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
   const float c2 = p.scale * 1.4426950408889634f;
 
   // ---- sweep 1: row maxima of the raw scores
@@ -95,7 +97,8 @@ __global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ 
     mbar_wait(&bar_s, ph_s); ph_s ^= 1;
     tc_fence_after();
 #pragma unroll
-    for (int ch = 0; ch < BKEY / 32; ++ch) {
+    for (int c = 0; c < 2; ++c) {
+      const int ch = 2 * half + c;
       uint32_t r[32];
       tmem_ld32(trow + ch * 32, r);
       tmem_ld_wait();
@@ -107,6 +110,9 @@ __global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ 
     tc_fence_before();
     __syncthreads();                     // S and the K tile are free again
   }
+  xch[0][half][row] = m;
+  __syncthreads();
+  m = fmaxf(xch[0][0][row], xch[0][1][row]);
   // ---- sweep 2: P = exp(scale (S - m)), O += P V
   float l = 0.f, lx = 0.f;              // l: sum of the bf16 probabilities the P V product sees; lx: the exact sum
   const float mc = m * c2;
@@ -118,7 +124,8 @@ __global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ 
     mbar_wait(&bar_s, ph_s); ph_s ^= 1;
     tc_fence_after();
 #pragma unroll
-    for (int ch = 0; ch < BKEY / 32; ++ch) {
+    for (int c = 0; c < 2; ++c) {
+      const int ch = 2 * half + c;
       uint32_t r[32];
       tmem_ld32(trow + ch * 32, r);
       tmem_ld_wait();
@@ -154,14 +161,20 @@ __global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ 
       umma_commit(&bar_pv);
     }
   }
+  xch[1][half][row] = l;
+  xch[0][half][row] = lx;               // (the maxima have been consumed)
   mbar_wait(&bar_pv, ph_pv);
   tc_fence_after();
-  // ---- epilogue: o = O / l
+  __syncthreads();
+  l = xch[1][0][row] + xch[1][1][row];
+  lx = xch[0][0][row] + xch[0][1][row];
+  // ---- epilogue: o = O / l; each of the row's two threads stores half of the D channels
   const int q = q0 + row;
   const float inv = 1.0f / l;
   bf16* op = p.o + ((size_t)n * p.T + q) * p.C + (size_t)h * D;
 #pragma unroll
-  for (int ch = 0; ch < D / 32; ++ch) {
+  for (int cc = 0; cc < D / 64; ++cc) {
+    const int ch = half * (D / 64) + cc;
     uint32_t r[32];
     tmem_ld32(trow + 128 + ch * 32, r);
     tmem_ld_wait();
@@ -177,7 +190,7 @@ __global__ void __launch_bounds__(128, 1) attn_fwd_tc_k(const __grid_constant__ 
       }
     }
   }
-  if (q < p.T) p.lse[((size_t)n * p.heads + h) * p.T + q] = m * p.scale + __logf(lx);
+  if (q < p.T && half == 0) p.lse[((size_t)n * p.heads + h) * p.T + q] = m * p.scale + __logf(lx);
   tc_fence_before();
   __syncthreads();
   if (warp == 1) {
@@ -516,7 +529,7 @@ template <int D> bool launch_atc(const CUtensorMap& map, const AtcP& p, int n, c
     if (cudaFuncSetAttribute(attn_fwd_tc_k<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, ACfg<D>::SMEM) != cudaSuccess) return false;
     attr = true;
   }
-  return launch_pdl(attn_fwd_tc_k<D>, dim3((p.T + BQ - 1) / BQ, p.heads, n), dim3(128), ACfg<D>::SMEM, st, map, p) == cudaSuccess;
+  return launch_pdl(attn_fwd_tc_k<D>, dim3((p.T + BQ - 1) / BQ, p.heads, n), dim3(256), ACfg<D>::SMEM, st, map, p) == cudaSuccess;
 }
 
 }  // namespace

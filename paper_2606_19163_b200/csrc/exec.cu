@@ -260,6 +260,12 @@ void prepare_weights(Ctx& c, int lo, int hi) {
       e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, op.cout, 3, ctot});
       e.push_back({c.par(op.p[P_C2W]), c.work + op.wt2, op.cout, 3, op.cout});
       if (op.p[P_SCW] >= 0) e.push_back({c.par(op.p[P_SCW]), c.work + op.wtsc, op.cout, 1, ctot});
+    } else if (op.kind == PULSE_OP_TBLOCK) {
+      e.push_back({c.par(op.p[P_F2W]), c.work + op.wt4, op.cin, 1, 4 * op.cin});
+      e.push_back({c.par(op.p[P_TW]), c.work + op.wt3, 4 * op.cin, 1, op.cin});
+      e.push_back({c.par(op.p[P_C2W]), c.work + op.wt2, op.cin, 1, op.cin});
+      e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, 3 * op.cin, 1, op.cin});
+      if (op.x1 >= 0) e.push_back({c.par(op.p[P_SCW]), c.work + op.wtsc, op.cin, 1, ctot});
     } else if (op.kind == PULSE_OP_ATTN) {
       e.push_back({c.par(op.p[P_C1W]), c.work + op.wt1, 3 * op.cin, 1, op.cin});
       e.push_back({c.par(op.p[P_C2W]), c.work + op.wt2, op.cin, 1, op.cin});
@@ -321,6 +327,38 @@ void attn_forward(Ctx& c, const OpPlan& op) {
   }
   run_conv(c, conv_args(c, Cat{c.fwd(op.a2), C, nullptr, 0}, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_C2W]), C,
                         c.par(op.p[P_C2B]), nullptr, c.fwd(op.x0), c.fwd(op.out)), op.out);
+}
+
+// Transformer block with an optional long skip: see stage.cu for the tensor names
+void conv1x1(Ctx& c, Cat src, int h, int w, const void* wgt, int cout, const void* bias, const void* res, void* out) {
+  run_conv(c, conv_args(c, src, h, w, h, w, 1, 1, wgt, cout, bias, nullptr, res, out));
+}
+void tblock_forward(Ctx& c, const OpPlan& op) {
+  pulse_stage* s = c.s;
+  const int hw = op.hin * op.win, C = op.cin, n = s->d.n;
+  const size_t tokens = (size_t)n * hw;
+  const char* xs = c.fwd(op.x0);
+  if (op.x1 >= 0) {          // the long skip: Linear on the virtual concat [x | skip]
+    conv1x1(c, Cat{c.fwd(op.x0), C, c.fwd(op.x1), op.cskip}, op.hin, op.win, c.par(op.p[P_SCW]), C, c.par(op.p[P_SCB]), nullptr,
+            c.fwd(op.u));
+    xs = c.fwd(op.u);
+  }
+  s->launches += layernorm_fwd(c.dt, xs, tokens, C, s->d.eps, c.par(op.p[P_GN1G]), c.par(op.p[P_GN1B]),
+                               (float*)(c.stash + op.ln1), c.fwd(op.a1), c.st);
+  conv1x1(c, Cat{c.fwd(op.a1), C, nullptr, 0}, op.hin, op.win, c.par(op.p[P_C1W]), 3 * C, c.par(op.p[P_C1B]), nullptr, c.fwd(op.h1));
+  {
+    Prof pr(s, c.st, PULSE_KCLASS_OTHER, 4.0 * n * (double)hw * hw * C, 0.0);
+    const int r = attn_fwd(c.dt, c.fwd(op.h1), n, hw, C, op.heads, c.fwd(op.a2), (float*)(c.stash + op.lse), c.st, c.tc());
+    if (r < 0) c.err = true; else s->launches += r;
+  }
+  conv1x1(c, Cat{c.fwd(op.a2), C, nullptr, 0}, op.hin, op.win, c.par(op.p[P_C2W]), C, c.par(op.p[P_C2B]), xs, c.fwd(op.tx1));
+  s->launches += layernorm_fwd(c.dt, c.fwd(op.tx1), tokens, C, s->d.eps, c.par(op.p[P_GN2G]), c.par(op.p[P_GN2B]),
+                               (float*)(c.stash + op.ln2), c.fwd(op.tl2), c.st);
+  conv1x1(c, Cat{c.fwd(op.tl2), C, nullptr, 0}, op.hin, op.win, c.par(op.p[P_TW]), 4 * C, c.par(op.p[P_TB]), nullptr, c.fwd(op.tf1));
+  s->launches += gelu_fwd(c.dt, c.fwd(op.tf1), c.fwd(op.tg), tokens * 4 * C, c.st);
+  // a GroupNorm never reads a transformer block's output (stats_t = -1 unless a later ResBlock / attention block does)
+  run_conv(c, conv_args(c, Cat{c.fwd(op.tg), 4 * C, nullptr, 0}, op.hin, op.win, op.hin, op.win, 1, 1, c.par(op.p[P_F2W]), C,
+                        c.par(op.p[P_F2B]), nullptr, c.fwd(op.tx1), c.fwd(op.out)), op.out);
 }
 
 // pixel sums of the gradient of an op's output, for its bias gradient: fused by the writers or one colsum pass
@@ -422,6 +460,68 @@ void attn_backward(Ctx& c, const OpPlan& op) {
              nullptr, /*act=*/0);
 }
 
+void tblock_backward(Ctx& c, const OpPlan& op) {
+  pulse_stage* s = c.s;
+  const int n = s->d.n, hw = op.hin * op.win, C = op.cin, H = op.hin, Wd = op.win, ctot = C + op.cskip;
+  const size_t tokens = (size_t)n * hw;
+  const bool skip = op.x1 >= 0;
+  const char* xs = skip ? c.fwd(op.u) : c.fwd(op.x0);
+  char* g_out = c.grad(op.out);
+  char* g_g = c.work + s->w_t4a;  char* g_f1 = c.work + s->w_t4b;
+  char* g_l2 = c.work + s->w_tca; char* g_x1 = c.work + s->w_tcb;
+  char* g_o = c.work + s->w_tca;  char* g_l1 = c.work + s->w_tca;      // g_l2, g_o, g_l1 are never live together
+  char* g_qkv = c.work + s->w_gqkv; char* g_xs = c.work + s->w_ga1;
+  float* gp = (float*)(c.work + op.gp);                                // [n][c] | [n][3c] | [n][c] | [n][4c]
+  float* gp_xs = gp; float* gp_qkv = gp + (size_t)n * C; float* gp_x1 = gp + (size_t)n * 4 * C; float* gp_f1 = gp + (size_t)n * 5 * C;
+  auto wg = [&](const void* src, int cs, const void* src1, int cs1, const void* g, int cout, int pidx) {
+    run_wgrad(c, WgradArgs{c.dt, Cat{src, cs, src1, cs1}, n, H, Wd, g, H, Wd, cout, 1, 1, c.pgrad(op.p[pidx])});
+  };
+  ensure_colsum(c, op.out);                                            // fc2 bias
+  c.fork();
+  wg(c.fwd(op.tg), 4 * C, nullptr, 0, g_out, C, P_F2W);
+  run_dgrad(c, g_out, H, Wd, C, op.wt4, 1, 4 * C, g_g, 0, 1, H, Wd);
+  s->launches += gelu_bwd(c.dt, c.fwd(op.tf1), g_g, g_f1, tokens * 4 * C, c.st);
+  s->launches += colsum(c.dt, g_f1, n, hw, 4 * C, gp_f1, c.st);       // fc1 bias
+  c.fork();
+  wg(c.fwd(op.tl2), C, nullptr, 0, g_f1, 4 * C, P_TW);
+  run_dgrad(c, g_f1, H, Wd, 4 * C, op.wt3, 1, C, g_l2, 0, 1, H, Wd);
+  // g_x1 = LN2'(g_l2) + g_out
+  s->launches += layernorm_bwd(c.dt, g_l2, c.fwd(op.tx1), tokens, C, c.par(op.p[P_GN2G]), (const float*)(c.stash + op.ln2), g_out,
+                               g_x1, 0, c.pgrad(op.p[P_GN2G]), c.pgrad(op.p[P_GN2B]), c.st);
+  s->launches += colsum(c.dt, g_x1, n, hw, C, gp_x1, c.st);           // proj bias
+  c.fork();
+  wg(c.fwd(op.a2), C, nullptr, 0, g_x1, C, P_C2W);
+  run_dgrad(c, g_x1, H, Wd, C, op.wt2, 1, C, g_o, 0, 1, H, Wd);
+  {
+    Prof pr(s, c.st, PULSE_KCLASS_OTHER, 10.0 * n * (double)hw * hw * C, 0.0);
+    const int r = attn_bwd(c.dt, c.fwd(op.h1), g_o, n, hw, C, op.heads, (float*)(c.stash + op.lse), g_qkv, c.st, c.tc());
+    if (r < 0) c.err = true; else s->launches += r;
+    s->launches += colsum(c.dt, g_qkv, n, hw, 3 * C, gp_qkv, c.st);   // qkv bias
+  }
+  c.fork();
+  wg(c.fwd(op.a1), C, nullptr, 0, g_qkv, 3 * C, P_C1W);
+  run_dgrad(c, g_qkv, H, Wd, 3 * C, op.wt1, 1, C, g_l1, 0, 1, H, Wd);
+  // g_xs = LN1'(g_l1) + g_x1: the block's input gradient, or (long skip) the gradient of the Linear's output
+  if (!skip) {
+    s->launches += layernorm_bwd(c.dt, g_l1, xs, tokens, C, c.par(op.p[P_GN1G]), (const float*)(c.stash + op.ln1), g_x1,
+                                 c.grad(op.x0), op.acc_x0, c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]), c.st);
+  } else {
+    s->launches += layernorm_bwd(c.dt, g_l1, xs, tokens, C, c.par(op.p[P_GN1G]), (const float*)(c.stash + op.ln1), g_x1, g_xs, 0,
+                                 c.pgrad(op.p[P_GN1G]), c.pgrad(op.p[P_GN1B]), c.st);
+    s->launches += colsum(c.dt, g_xs, n, hw, C, gp_xs, c.st);         // skip Linear bias
+    c.fork();
+    wg(c.fwd(op.x0), C, c.fwd(op.x1), op.cskip, g_xs, C, P_SCW);
+    // the Linear's adjoint, one 1x1 conv per source: rows [0, C) / [C, C + skip) of the transposed weight [C + skip][C]
+    const size_t esz = s->esz();
+    run_dgrad(c, g_xs, H, Wd, C, op.wtsc, 1, C, c.grad(op.x0), op.acc_x0, 1, H, Wd);
+    run_dgrad(c, g_xs, H, Wd, C, op.wtsc + (size_t)C * C * esz, 1, op.cskip, c.grad(op.x1), op.acc_x1, 1, H, Wd);
+    (void)ctot;
+  }
+  // the side stream's weight gradients read the shared gradient buffers of this block: join before the next block reuses them
+  if (c.side) c.wait_side(c.mark_side());
+  if (c.last_op && c.side2) tail_work(c);
+}
+
 // bias / temb-projection gradients of every op from the pixel sums, in one batched launch (row a8-a10)
 void small_grads(Ctx& c, const float* emb, float* g_temb, cudaStream_t st) {
   pulse_stage* s = c.s;
@@ -437,6 +537,20 @@ void small_grads(Ctx& c, const float* emb, float* g_temb, cudaStream_t st) {
       g.db_out2 = op.p[P_SCB] >= 0 ? c.pgrad(op.p[P_SCB]) : nullptr;
       g.gp = (const float*)(c.work + op.gp);
       g.db1 = c.pgrad(op.p[P_C1B]); g.dtb = c.pgrad(op.p[P_TB]); g.dtw = c.pgrad(op.p[P_TW]); g.tw = c.par(op.p[P_TW]);
+    } else if (op.kind == PULSE_OP_TBLOCK) {
+      g.db_out = c.pgrad(op.p[P_F2B]);            // fc2 bias from the pixel sums of g_out
+      const float* gp = (const float*)(c.work + op.gp);
+      const int C = op.cin, n = s->d.n;
+      auto extra = [&](const float* sums, int width, int pidx) {
+        SmallGradEntry q;
+        memset(&q, 0, sizeof q);
+        q.cs_out = sums; q.db_out = c.pgrad(op.p[pidx]); q.cout = width;
+        e.push_back(q);
+      };
+      if (op.x1 >= 0) extra(gp, C, P_SCB);
+      extra(gp + (size_t)n * C, 3 * C, P_C1B);
+      extra(gp + (size_t)n * 4 * C, C, P_C2B);
+      extra(gp + (size_t)n * 5 * C, 4 * C, P_TB);
     } else if (op.kind == PULSE_OP_ATTN) {
       g.db_out = c.pgrad(op.p[P_C2B]);            // proj bias from the pixel sums of g_out
       SmallGradEntry q;                           // qkv bias from the pixel sums of g_qkv
@@ -568,6 +682,7 @@ static pulse_status_t forward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, 
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_forward(c, op); break;
       case PULSE_OP_ATTN: attn_forward(c, op); break;
+      case PULSE_OP_TBLOCK: tblock_forward(c, op); break;
       case PULSE_OP_CONV_IN:
       case PULSE_OP_DOWN: {
         const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;
@@ -711,6 +826,7 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
     switch (op.kind) {
       case PULSE_OP_RESBLOCK: resblock_backward(c, op); break;
       case PULSE_OP_ATTN: attn_backward(c, op); break;
+      case PULSE_OP_TBLOCK: tblock_backward(c, op); break;
       case PULSE_OP_CONV_IN:
       case PULSE_OP_DOWN: {
         const int stride = op.kind == PULSE_OP_DOWN ? 2 : 1;

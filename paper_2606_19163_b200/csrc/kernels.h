@@ -62,6 +62,16 @@ int attn_bwd(int dt, const void* qkv, const void* g_o, int n, int T, int C, int 
              cudaStream_t st, bool use_tc = true);
 int attn_bwd_tc(const void* qkv, const void* g_o, int n, int T, int C, int heads, float* stats, void* g_qkv, cudaStream_t st);
 
+// ---- transformer-block pointwise kernels (tblock.cu) ------------------------
+// LayerNorm over the C channels of each of `tokens` rows; stat [tokens][2] fp32 = mean, rstd (written by the forward)
+int layernorm_fwd(int dt, const void* x, size_t tokens, int C, float eps, const void* gamma, const void* beta, float* stat,
+                  void* y, cudaStream_t st);
+// g_x (+)= r (q - mean q - xhat mean(q xhat)) [+ add], q = g_y gamma; dgamma / dbeta: fp32, +=
+int layernorm_bwd(int dt, const void* g_y, const void* x, size_t tokens, int C, const void* gamma, const float* stat,
+                  const void* add, void* g_x, int acc, float* dgamma, float* dbeta, cudaStream_t st);
+int gelu_fwd(int dt, const void* x, void* y, size_t numel, cudaStream_t st);
+int gelu_bwd(int dt, const void* x, const void* g, void* g_x, size_t numel, cudaStream_t st);     // g_x = g GELU'(x)
+
 // ---- small ops -----------------------------------------------------------------------
 // cs[n][c] += sum over pixels of g[n][hw][c]   (tensors whose writers could not emit their column sums)
 int colsum(int dt, const void* g, int n, int hw, int c, float* cs, cudaStream_t st);

@@ -96,14 +96,14 @@ static pulse_status_t build_plan(pulse_stage* s) {
   if (d.x_in_is_skip) { s->skip_tensor.push_back(cur); stack.push_back(cur); }
   s->emb_off = pl.bump(R_STASH, (size_t)d.n * T * 4);
 
-  size_t m_out = 0, m_cat = 0, m_gu = 0, m_qkv = 0;
+  size_t m_out = 0, m_cat = 0, m_gu = 0, m_qkv = 0, m_t4 = 0, m_tc = 0;
   auto upd = [](size_t& m, size_t v) { if (v > m) m = v; };
 
   auto plan_ops = [&](const std::vector<pulse_op_desc>& list, const char* phase, bool is_dec) -> pulse_status_t {
     for (size_t i = 0; i < list.size(); ++i) {
       const pulse_op_desc& o = list[i];
       OpPlan op;
-      for (int k = 0; k < 12; ++k) op.p[k] = -1;
+      for (int k = 0; k < 16; ++k) op.p[k] = -1;
       const Tensor& tin = s->tensors[cur];
       op.kind = o.kind; op.cin = o.cin; op.cskip = o.skip_channels; op.cout = o.cout; op.heads = o.heads;
       op.hin = tin.ref.h; op.win = tin.ref.w; op.hout = op.hin; op.wout = op.win;
@@ -180,6 +180,46 @@ static pulse_status_t build_plan(pulse_stage* s) {
         upd(m_out, pix * c * s->esz()); upd(m_cat, pix * c * s->esz()); upd(m_qkv, pix * 3 * c * s->esz());
         op.wt1 = pl.bump(R_WORK, (size_t)3 * c * c * s->esz());
         op.wt2 = pl.bump(R_WORK, (size_t)c * c * s->esz());
+      } else if (o.kind == PULSE_OP_TBLOCK) {
+        // [x0 | x1 -> Linear -> xs (u)] -> LN1 -> l1 (a1) -> qkv (h1) -> attention -> o (a2) -> proj + xs -> x1 (tx1)
+        //   -> LN2 -> l2 (tl2) -> fc1 -> f1 (tf1) -> GELU -> g (tg) -> fc2 + x1 -> out
+        const int c = o.cin;
+        if (o.cin != o.cout || c % vec || !attn_supported(c, o.heads) || c > (d.dtype == PULSE_F32 ? 640 * 2 : 1280))
+          return fail(PULSE_ERR_SHAPE, "%s%zu: transformer block needs cin == cout <= 1280, divisible by the vector and by heads", phase, i);
+        if (o.skip_channels > 0) {
+          if (!is_dec) return fail(PULSE_ERR_SHAPE, "%s%zu: only decoder-side blocks consume skips", phase, i);
+          if (stack.empty()) return fail(PULSE_ERR_SHAPE, "%s%zu pops a skip but none is cached", phase, i);
+          op.x1 = stack.back(); stack.pop_back();
+          const Tensor& ts = s->tensors[op.x1];
+          if (ts.ref.c != o.skip_channels || ts.ref.h != op.hin || ts.ref.w != op.win || o.skip_channels % vec)
+            return fail(PULSE_ERR_SHAPE, "%s%zu: popped skip is [%d,%d,%d], expected [%d,%d,%d]", phase, i, ts.ref.h, ts.ref.w,
+                        ts.ref.c, op.hin, op.win, o.skip_channels);
+          for (size_t k = 0; k < s->skip_tensor.size(); ++k) if (s->skip_tensor[k] == op.x1) op.pop = (int)k;
+          op.p[P_SCW] = pl.param(pre + "skip.w", 4, c, 1, 1, ctot); op.p[P_SCB] = pl.param(pre + "skip.b", 1, c);
+          op.u = pl.tensor(R_STASH, c, op.hin, op.win, false);
+          op.wtsc = pl.bump(R_WORK, (size_t)c * ctot * s->esz());
+        }
+        op.p[P_GN1G] = pl.param(pre + "ln1.gamma", 1, c); op.p[P_GN1B] = pl.param(pre + "ln1.beta", 1, c);
+        op.p[P_C1W] = pl.param(pre + "qkv.w", 4, 3 * c, 1, 1, c); op.p[P_C1B] = pl.param(pre + "qkv.b", 1, 3 * c);
+        op.p[P_C2W] = pl.param(pre + "proj.w", 4, c, 1, 1, c); op.p[P_C2B] = pl.param(pre + "proj.b", 1, c);
+        op.p[P_GN2G] = pl.param(pre + "ln2.gamma", 1, c); op.p[P_GN2B] = pl.param(pre + "ln2.beta", 1, c);
+        op.p[P_TW] = pl.param(pre + "fc1.w", 4, 4 * c, 1, 1, c); op.p[P_TB] = pl.param(pre + "fc1.b", 1, 4 * c);
+        op.p[P_F2W] = pl.param(pre + "fc2.w", 4, c, 1, 1, 4 * c); op.p[P_F2B] = pl.param(pre + "fc2.b", 1, c);
+        op.a1 = pl.tensor(R_STASH, c, op.hin, op.win, false);
+        op.h1 = pl.tensor(R_STASH, 3 * c, op.hin, op.win, false);
+        op.a2 = pl.tensor(R_STASH, c, op.hin, op.win, false);
+        op.tx1 = pl.tensor(R_STASH, c, op.hin, op.win, false);
+        op.tl2 = pl.tensor(R_STASH, c, op.hin, op.win, false);
+        op.tf1 = pl.tensor(R_STASH, 4 * c, op.hin, op.win, false);
+        op.tg = pl.tensor(R_STASH, 4 * c, op.hin, op.win, false);
+        op.ln1 = pl.bump(R_STASH, pix * 2 * 4); op.ln2 = pl.bump(R_STASH, pix * 2 * 4);
+        op.lse = pl.bump(R_STASH, attn_stats_floats(d.n, o.heads, op.hin * op.win) * 4);
+        upd(m_qkv, pix * 3 * c * s->esz()); upd(m_t4, pix * 4 * c * s->esz()); upd(m_tc, pix * c * s->esz());
+        upd(m_cat, pix * ctot * s->esz());
+        op.wt1 = pl.bump(R_WORK, (size_t)3 * c * c * s->esz());
+        op.wt2 = pl.bump(R_WORK, (size_t)c * c * s->esz());
+        op.wt3 = pl.bump(R_WORK, (size_t)4 * c * c * s->esz());
+        op.wt4 = pl.bump(R_WORK, (size_t)4 * c * c * s->esz());
       } else if (o.kind == PULSE_OP_HEAD) {
         if (!is_dec || o.skip_channels || !chk_c(o.cin, "cin")) return fail(PULSE_ERR_SHAPE, "%s%zu: bad head", phase, i);
         op.p[P_GN1G] = pl.param(pre + "gn.gamma", 1, o.cin); op.p[P_GN1B] = pl.param(pre + "gn.beta", 1, o.cin);
@@ -208,8 +248,8 @@ static pulse_status_t build_plan(pulse_stage* s) {
   s->n_enc = (int)s->enc.size();
   if (d.link == PULSE_LINK_CLOSED) {
     for (auto& o : s->mid)
-      if ((o.kind != PULSE_OP_RESBLOCK && o.kind != PULSE_OP_ATTN) || o.skip_channels)
-        return fail(PULSE_ERR_SHAPE, "mid ops must be plain ResBlocks or attention blocks");
+      if ((o.kind != PULSE_OP_RESBLOCK && o.kind != PULSE_OP_ATTN && o.kind != PULSE_OP_TBLOCK) || o.skip_channels)
+        return fail(PULSE_ERR_SHAPE, "mid ops must be plain ResBlocks, attention or transformer blocks");
     st = plan_ops(s->mid, "mid", false);
     if (st) return st;
   } else {
@@ -247,8 +287,9 @@ static pulse_status_t build_plan(pulse_stage* s) {
     }
     op.acc_x0 = written[op.x0]; written[op.x0] = 1;
     if (op.x1 >= 0) { op.acc_x1 = written[op.x1]; written[op.x1] = 1; }
-    if (op.kind == PULSE_OP_CONV_IN || op.kind == PULSE_OP_DOWN || op.kind == PULSE_OP_UP)
+    if (op.kind == PULSE_OP_CONV_IN || op.kind == PULSE_OP_DOWN || op.kind == PULSE_OP_UP || op.kind == PULSE_OP_TBLOCK)
       s->tensors[op.x0].cs_fused = false;
+    if (op.kind == PULSE_OP_TBLOCK && op.x1 >= 0) s->tensors[op.x1].cs_fused = false;
     if ((op.kind == PULSE_OP_UP || op.kind == PULSE_OP_HEAD) && op.acc_x0)
       return fail(PULSE_ERR_UNSUPPORTED, "up/head input with a second consumer");
   }
@@ -277,6 +318,9 @@ static pulse_status_t build_plan(pulse_stage* s) {
     } else if (op.kind == PULSE_OP_ATTN) {
       op.bst1 = pl.bump(R_WORK, (size_t)d.n * 2 * op.cin * 4);
       op.gp = pl.bump(R_WORK, (size_t)d.n * 3 * op.cin * 4);       // pixel sums of g_qkv: the qkv bias gradient
+    } else if (op.kind == PULSE_OP_TBLOCK) {
+      // pixel sums for the bias gradients: g_xs [c] | g_qkv [3c] | g_x1 [c] | g_f1 [4c], per image
+      op.gp = pl.bump(R_WORK, (size_t)d.n * 9 * op.cin * 4);
     }
   }
   s->zero_end = pl.bump(R_WORK, 0);
@@ -284,6 +328,8 @@ static pulse_status_t build_plan(pulse_stage* s) {
   s->w_ga1 = pl.bump(R_WORK, m_cat); s->w_gsc = pl.bump(R_WORK, m_cat);
   s->w_gu = pl.bump(R_WORK, m_gu);
   s->w_gqkv = pl.bump(R_WORK, m_qkv);
+  s->w_t4a = pl.bump(R_WORK, m_t4); s->w_t4b = pl.bump(R_WORK, m_t4);
+  s->w_tca = pl.bump(R_WORK, m_tc); s->w_tcb = pl.bump(R_WORK, m_tc);
   s->w_tmpf = pl.bump(R_WORK, (size_t)d.n * T * 4 + 256);
   s->work_bytes = pl.top[R_WORK];
   return PULSE_OK;

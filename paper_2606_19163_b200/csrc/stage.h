@@ -30,13 +30,17 @@ struct OpPlan {
   int hin, win, hout, wout;
   int x0 = -1, x1 = -1, out = -1;           // indices into Stage::tensors (activations)
   int a1 = -1, h1 = -1, a2 = -1, u = -1;    // stashed intermediates
+  int tx1 = -1, tl2 = -1, tf1 = -1, tg = -1; // transformer block: x1, LN2 output, fc1 output, GELU output (a1 = LN1 output,
+                                            // h1 = qkv, a2 = attention output, u = Linear(concat) output)
+  size_t ln1 = 0, ln2 = 0;                  // slot stash: [tokens][2] fp32 mean / rstd of the LayerNorm sites
+  size_t wt3 = 0, wt4 = 0;                  // R_WORK: transposed fc1 / fc2 weights
   size_t bst1 = 0, bst2 = 0;                // R_WORK (zeroed area): GroupNorm backward sums [n][2][C] fp32 per site
   size_t gp = 0;                            // R_WORK (zeroed area): [n][cout] fp32 pixel sums of g_h1
   size_t pn = 0;                            // byte offset in the slot stash ([n,cout] fp32)
   size_t mr1 = 0, mr2 = 0;                  // slot stash: [n][2][G] fp32 group mean / rstd of the GroupNorm sites
   size_t lse = 0;                           // slot stash (attention): softmax statistics, attn_stats_floats() floats
   size_t wt1 = 0, wt2 = 0, wtsc = 0;        // R_WORK: flipped/transposed conv weights (kept across a wave)
-  int p[12];                                // parameter indices (see stage.cu)
+  int p[16];                                // parameter indices (see stage.cu)
   int push = -1, pop = -1;
   // backward write modes decided at plan time (0: '=', 1: '+=')
   int acc_x0 = 0, acc_x1 = 0;
@@ -63,7 +67,8 @@ pulse_status_t pulse_set_error(pulse_status_t s, const char* fmt, ...);
     if (e_ != cudaSuccess) return fail(PULSE_ERR_CUDA, "%s: %s", #x, cudaGetErrorString(e_)); \
   } while (0)
 // parameter slots of OpPlan::p
-enum { P_GN1G = 0, P_GN1B, P_C1W, P_C1B, P_TW, P_TB, P_GN2G, P_GN2B, P_C2W, P_C2B, P_SCW, P_SCB };
+enum { P_GN1G = 0, P_GN1B, P_C1W, P_C1B, P_TW, P_TB, P_GN2G, P_GN2B, P_C2W, P_C2B, P_SCW, P_SCB, P_F2W, P_F2B };
+// transformer block: GN1 = ln1, C1 = qkv, C2 = proj, GN2 = ln2, T = fc1, F2 = fc2, SC = the long skip's Linear
 
 struct pulse_stage {
   pulse_stage_desc d;
@@ -84,7 +89,7 @@ struct pulse_stage {
   bool eout_grad_by_dec = false;            // PULSE_FLAG_SPLIT: a decoder op writes the gradient of e_out before g_e_out arrives
   bool wp_valid = false;                    // pre-summed phase weights of the up convs (forward) match them
   // per-stage workspace offsets (bytes)
-  size_t w_ga2 = 0, w_gh1 = 0, w_gh1b = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0, w_gqkv = 0;
+  size_t w_ga2 = 0, w_gh1 = 0, w_gh1b = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0, w_gqkv = 0, w_t4a = 0, w_t4b = 0, w_tca = 0, w_tcb = 0;
   // weight-gradient kernels run on a side stream, concurrently with the dgrad / GroupNorm chain of the backward
   // (fork / join with events; legal inside CUDA-graph capture).  PULSE_NO_SIDE_STREAM=1 disables it.
   cudaStream_t side = nullptr;

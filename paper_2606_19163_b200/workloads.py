@@ -15,7 +15,7 @@ from __future__ import annotations
 import copy
 import numpy as np
 
-CONV_IN, RESBLOCK, DOWN, UP, HEAD, ATTN = "conv_in", "resblock", "down", "up", "head", "attn"
+CONV_IN, RESBLOCK, DOWN, UP, HEAD, ATTN, TBLOCK = "conv_in", "resblock", "down", "up", "head", "attn", "tblock"
 
 
 def _op(kind, cin, cout, skip=0, push=0, heads=0):
@@ -90,6 +90,20 @@ def config(i: int) -> dict:
     raise ValueError(i)
 
 
+def tblock(c, heads, skip=0, push=0):
+    """Transformer block on c channels: [Linear on concat(x, skip) where a skip is consumed ->]
+    LN -> qkv -> attention -> proj + residual -> LN -> fc1 (c -> 4c) -> GELU -> fc2 + residual."""
+    return _op(TBLOCK, c, c, skip, push, heads)
+
+
+def uvit_stage(name, n, hw, c, heads, depth, dtype="bf16") -> dict:
+    """U-ViT style stage: `depth` early blocks whose outputs are cached, `depth` late blocks that each
+    consume one of them through concat + Linear (LIFO); OPEN (tokens in, tokens out on both sides)."""
+    temb = {"kind": "sinusoidal", "d0": 16, "dim": 16}      # the blocks take no timestep input (reading R26)
+    return _stage(name, dtype, n, hw, hw, c, 1, temb, "open", 0, [tblock(c, heads, push=1) for _ in range(depth)], [],
+                  [tblock(c, heads, skip=c) for _ in range(depth)])
+
+
 def attn_level() -> dict:
     """configs[2]'s level-2 stage with a self-attention block (640 channels = 10 heads x 64, 1024
     tokens) after every ResBlock, as in an SD-shaped UNet level; skips are pushed after the attention."""
@@ -128,6 +142,8 @@ def mini(kind: str, dtype: str = "fp32") -> dict:
         return _stage("mini_attn", dtype, 2, 4, 4, 8, 4, mlp, "open", 1,
                       [rb(8, 16), attn(16, 2, push=1), rb(16, 16), attn(16, 4, push=1)], [],
                       [rb(16, 16, skip=16), attn(16, 2), rb(16, 16, skip=16), attn(16, 1), rb(16, 16, skip=8)])
+    if kind == "uvit":          # transformer blocks with long skips (concat + Linear)
+        return uvit_stage("mini_uvit", 2, 4, 16, 2, 2, dtype=dtype)
     if kind == "attn_unet":     # closed: attention in the mid block as well
         d = _unet("mini_attn_unet", 2, 8, [8, 16], dtype=dtype, groups=4, temb=mlp, c_lat=4)
         d["mid_ops"] = [rb(16, 16), attn(16, 2), rb(16, 16)]
@@ -151,6 +167,8 @@ def gpu_mid(kind: str) -> dict:
                        _op(UP, 640, 640)])
     if kind == "unet":
         return _unet("mid_unet", 1, 32, [320, 640], temb=mlp)
+    if kind == "uvit":          # 320 channels = 5 heads x 64, 3 images of 64 tokens (192 pixels = 1.5 tiles), 2 + 2 blocks
+        return uvit_stage("mid_uvit", 3, 8, 320, 5, 2)
     if kind == "attn":          # SD-style level with attention: 320 channels = 5 heads x 64, 64 tokens per image, 192 pixels = 1.5 tiles
         return _stage("mid_attn", "bf16", 3, 8, 8, 320, 32, mlp, "open", 1,
                       [rb(320, 320), attn(320, 5, push=1)], [],
@@ -261,6 +279,16 @@ def param_specs(desc) -> list:
                     specs += [(p + "sc.w", (co, ci, 1, 1), "weight", ci), (p + "sc.b", (co,), "bias", 0)]
             elif k in (CONV_IN, DOWN, UP):
                 specs += [(p + "conv.w", (co, ci, 3, 3), "weight", ci * 9), (p + "conv.b", (co,), "bias", 0)]
+            elif k == TBLOCK:
+                c = co
+                if op["skip"]:
+                    specs += [(p + "skip.w", (c, ci, 1, 1), "weight", ci), (p + "skip.b", (c,), "bias", 0)]
+                specs += [(p + "ln1.gamma", (c,), "gamma", 0), (p + "ln1.beta", (c,), "beta", 0),
+                          (p + "qkv.w", (3 * c, c, 1, 1), "weight", c), (p + "qkv.b", (3 * c,), "bias", 0),
+                          (p + "proj.w", (c, c, 1, 1), "weight", c), (p + "proj.b", (c,), "bias", 0),
+                          (p + "ln2.gamma", (c,), "gamma", 0), (p + "ln2.beta", (c,), "beta", 0),
+                          (p + "fc1.w", (4 * c, c, 1, 1), "weight", c), (p + "fc1.b", (4 * c,), "bias", 0),
+                          (p + "fc2.w", (c, 4 * c, 1, 1), "weight", 4 * c), (p + "fc2.b", (c,), "bias", 0)]
             elif k == ATTN:
                 specs += [(p + "gn.gamma", (ci,), "gamma", 0), (p + "gn.beta", (ci,), "beta", 0),
                           (p + "qkv.w", (3 * ci, ci, 1, 1), "weight", ci), (p + "qkv.b", (3 * ci,), "bias", 0),

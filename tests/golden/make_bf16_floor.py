@@ -32,7 +32,7 @@ LIST_ABOVE = 1e-2
 CASES = {}
 for kind in ("level", "updown", "unet", "wave", "attn", "attn_unet"):
     CASES[f"mini_{kind}"] = (W.mini(kind, "bf16"), 1, True, torch.float64)
-for kind in ("level", "updown", "unet", "attn"):
+for kind in ("level", "updown", "unet", "attn", "uvit"):
     CASES[f"mid_{kind}"] = (W.gpu_mid(kind), 2, kind != "unet", torch.float64)
 CASES["mini_updown@2"] = (W.mini("updown", "bf16"), 2, True, torch.float64)
 CASES["mid_level_1f1b"] = (W.scaled(W.gpu_mid("level"), microbatches=3, name="mid_level_1f1b"), 4, False, torch.float64)

@@ -41,6 +41,24 @@ def _attn(desc, P, p, x, heads):
     return x + F.conv2d(o, P[p + "proj.w"], P[p + "proj.b"])
 
 
+def _tblock(desc, P, p, x, skip, heads):
+    """Transformer block with an optional long skip from library pieces (F.layer_norm on channels-last tokens, F.gelu,
+    F.scaled_dot_product_attention, F.linear)."""
+    n, _, h, w = x.shape
+    tok = lambda t: t.flatten(2).transpose(1, 2)                  # [n, T, c]
+    lin = lambda t, name: F.linear(t, P[p + name + ".w"][:, :, 0, 0], P[p + name + ".b"])
+    z = tok(x)
+    if skip is not None:
+        z = lin(torch.cat([z, tok(skip)], dim=2), "skip")
+    c = z.shape[2]
+    qkv = lin(F.layer_norm(z, (c,), P[p + "ln1.gamma"], P[p + "ln1.beta"], desc["eps"]), "qkv")
+    q, k, v = (t.reshape(n, h * w, heads, c // heads).transpose(1, 2) for t in qkv.chunk(3, dim=2))
+    o = F.scaled_dot_product_attention(q, k, v).transpose(1, 2).reshape(n, h * w, c)
+    z = z + lin(o, "proj")
+    z = z + lin(F.gelu(lin(F.layer_norm(z, (c,), P[p + "ln2.gamma"], P[p + "ln2.beta"], desc["eps"]), "fc1")), "fc2")
+    return z.transpose(1, 2).reshape(n, c, h, w)
+
+
 def _enc_prefix(desc, P, x_in, emb, upto_push):
     """Recompute the encoder from x_in until push number `upto_push` exists; return it."""
     k = 0
@@ -55,6 +73,8 @@ def _enc_prefix(desc, P, x_in, emb, upto_push):
             x = _rb(desc, P, p, x, emb)
         elif op["kind"] == "attn":
             x = _attn(desc, P, p, x, op["heads"])
+        elif op["kind"] == "tblock":
+            x = _tblock(desc, P, p, x, None, op["heads"])
         else:
             x = F.conv2d(x, P[p + "conv.w"], P[p + "conv.b"], stride=2 if op["kind"] == "down" else 1, padding=1)
         if op["push"]:
@@ -91,6 +111,12 @@ def run(desc, params, mb, loss_scale=1.0, extra_e_loss=False):
             h = _rb(desc, P, p, torch.cat([h, skip], 1), emb)
         elif op["kind"] == "attn":
             h = _attn(desc, P, p, h, op["heads"])
+        elif op["kind"] == "tblock":
+            sk = None
+            if op["skip"]:
+                top -= 1
+                sk = _enc_prefix(desc, P, x_in, emb, top)      # recomputed, never cached
+            h = _tblock(desc, P, p, h, sk, op["heads"])
         elif op["kind"] == "up":
             h = F.conv2d(F.interpolate(h, scale_factor=2, mode="nearest"), P[p + "conv.w"], P[p + "conv.b"], padding=1)
         else:

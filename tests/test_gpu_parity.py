@@ -203,7 +203,7 @@ def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False,
 
 
 # ------------------------------------------------------------------ fp32 debug path
-@pytest.mark.parametrize("kind", ["pair", "level", "updown", "straddle", "unet", "wave", "attn", "attn_unet"])
+@pytest.mark.parametrize("kind", ["pair", "level", "updown", "straddle", "unet", "wave", "attn", "attn_unet", "uvit"])
 def test_mini_fp32(kind):
     check(W.mini(kind, "fp32"), seed=1, with_g_e_out=True)
 
@@ -338,6 +338,12 @@ def test_pipeline_two_stages_bf16():
     for k, r in ref.items():
         limit = min(max(2e-2, 2.0 * exc[k][0]), CAP) if k in exc else 2e-2
         assert rel_err(got[k], r) <= limit, (k, rel_err(got[k], r), limit)
+
+
+def test_mid_bf16_transformer_skip_stage():
+    """transformer blocks with long skips (concat + Linear as a 1x1 conv on the virtual concat), 320
+    channels = 5 heads x 64: LayerNorm / GELU kernels, Linear layers on the tcgen05 conv path, tcgen05 attention."""
+    check(W.gpu_mid("uvit"), seed=2, with_g_e_out=True)
 
 
 def test_mid_bf16_1f1b_order():

@@ -192,7 +192,7 @@ def test_sinusoidal_and_upsample():
 
 # ------------------------------------------------------------------ whole stage
 
-KINDS = ["pair", "level", "updown", "straddle", "unet", "attn", "attn_unet"]
+KINDS = ["pair", "level", "updown", "straddle", "unet", "attn", "attn_unet", "uvit"]
 
 
 @pytest.mark.parametrize("kind", KINDS)
@@ -205,16 +205,14 @@ def test_stage_matches_naive_recompute_autograd(kind):
     r = O.run_stage(desc, data["params"], mb)
     ref = NA.run(desc, data["params"], mb)
     for k in ["loss", "d_out", "g_x_in", "g_h_in", "e_out", "g_emb"]:
-        if k in ref:
+        if k in ref and not (ref[k] is None and r[k] is None):      # g_emb: None on both sides where no block takes the embedding
             assert torch.allclose(r[k], ref[k], rtol=1e-9, atol=1e-11), k
-    if desc["temb"]["kind"] == "mlp":
-        pass
     for k, v in ref["param_grads"].items():
         assert torch.allclose(r["param_grads"][k], v, rtol=1e-8, atol=1e-11), k
     assert set(r["param_grads"]) == set(ref["param_grads"])
 
 
-@pytest.mark.parametrize("kind", ["updown", "unet", "attn"])
+@pytest.mark.parametrize("kind", ["updown", "unet", "attn", "uvit"])
 def test_stage_central_differences(kind):
     """fp64 central finite differences along random directions, every input and parameter
     tensor, rel err <= 1e-3 (BASELINE.json north_star)."""
@@ -333,6 +331,10 @@ def _store_point_count(desc):
                 n += 4
             elif op["kind"] == "attn":
                 n += 8          # xn, qkv, o, out; g_o, g_qkv, g_xn; the input gradient
+            elif op["kind"] == "tblock":
+                # l1, qkv, o, x1, l2, f1, g, out; g_g, g_f1, g_l2, g_x1, g_o, g_qkv, g_l1; the input gradient
+                # with a long skip: xs forward, g_xs backward, and a second input-gradient write (g_skip)
+                n += 16 + (3 if op["skip"] else 0)
     return n
 
 
@@ -363,7 +365,7 @@ def test_stored_in_store_points(kind, monkeypatch):
             assert torch.equal(q[k].to(torch.bfloat16).to(D), q[k]), k
     # statistics, weight gradients and the timestep path are NOT stored in bf16 (fp32 accumulate, north_star)
     assert any(not torch.equal(v.to(torch.bfloat16).to(D), v) for v in q["param_grads"].values())
-    assert not torch.equal(q["g_emb"].to(torch.bfloat16).to(D), q["g_emb"])
+    assert q["g_emb"] is None or not torch.equal(q["g_emb"].to(torch.bfloat16).to(D), q["g_emb"])
     # and the rounded run stays a small perturbation of the exact one (<= 2^-8 relative per store point)
     rms = float(exact["d_out"].pow(2).mean().sqrt())
     assert 0 < float((q["d_out"] - exact["d_out"]).abs().max()) < 0.05 * rms
@@ -504,3 +506,45 @@ def test_attention_heads_layout():
     assert t.shape == (n * heads, h * w, d)
     assert torch.equal(t[1 * heads + 2, 1 * w + 3], x[1, 2 * d:3 * d, 1, 3])
     assert torch.equal(O._unheads(t, n, heads, h, w), x)
+
+
+# ------------------------------------------------------------------ transformer block pieces
+
+def test_layernorm_and_gelu_match_library_and_closed_forms():
+    n, c = 2, 10
+    x, gamma, beta, g_y = rnd(n, c, 3, 4) * 2 + 1, rnd(c), rnd(c), rnd(n, c, 3, 4)
+    y, ctx = O.ln_fwd(x, gamma, beta, 1e-5)
+    g_x, dg, db = O.ln_bwd(g_y, ctx, gamma)
+    xr, gr, br = (t.clone().requires_grad_(True) for t in (x, gamma, beta))
+    yr = torch.nn.functional.layer_norm(xr.permute(0, 2, 3, 1), (c,), gr, br, 1e-5).permute(0, 3, 1, 2)
+    yr.backward(g_y)
+    assert torch.allclose(y, yr.detach(), atol=1e-12) and torch.allclose(g_x, xr.grad, atol=1e-10)
+    assert torch.allclose(dg, gr.grad, atol=1e-10) and torch.allclose(db, br.grad, atol=1e-10)
+    # per token: mean 0, variance var / (var + eps) before the affine; the input gradient sums to zero over the channels
+    assert ctx["xhat"].mean(1).abs().max() < 1e-12 and g_x.sum(1).abs().max() < 1e-10
+    # GELU: x Phi(x); GELU(0) = 0, GELU'(0) = 1/2, GELU(x) -> x, GELU(-x) -> 0; the library's erf form; finite differences
+    z = torch.zeros(1, dtype=D)
+    assert O.gelu(z).item() == 0.0 and O.gelu_grad(z).item() == 0.5
+    big = torch.tensor([12.0], dtype=D)
+    assert abs(O.gelu(big).item() - 12.0) < 1e-12 and abs(O.gelu(-big).item()) < 1e-12
+    assert abs(O.gelu(torch.tensor([1.0], dtype=D)).item() - 0.8413447460685429) < 1e-12      # Phi(1)
+    t = rnd(50)
+    assert torch.allclose(O.gelu(t), torch.nn.functional.gelu(t), atol=1e-12)
+    assert torch.allclose(O.gelu_grad(t), (O.gelu(t + 1e-6) - O.gelu(t - 1e-6)) / 2e-6, atol=1e-8)
+
+
+def test_long_skip_is_concat_then_linear():
+    """the long skip of a transformer stage is concat + Linear: with the Linear = [I | 0] the block ignores
+    the skip, with [0 | I] it runs on the skip instead of on h."""
+    desc = W.mini("uvit")
+    data = W.draw(desc, seed=8)
+    P = {k: torch.as_tensor(v, dtype=D) for k, v in data["params"].items()}
+    x, sk = rnd(2, 16, 4, 4), rnd(2, 16, 4, 4)
+    eye = torch.eye(16, dtype=D)
+    Pa = dict(P); Pa["dec0.skip.w"] = torch.cat([eye, torch.zeros(16, 16, dtype=D)], 1)[:, :, None, None]; Pa["dec0.skip.b"] = torch.zeros(16, dtype=D)
+    Pb = dict(P); Pb["dec0.skip.w"] = torch.cat([torch.zeros(16, 16, dtype=D), eye], 1)[:, :, None, None]; Pb["dec0.skip.b"] = torch.zeros(16, dtype=D)
+    Pn = {k.replace("dec0.", "enc0."): v for k, v in P.items() if k.startswith("dec0.") and "skip" not in k}
+    base_x, _ = O.tblock_fwd(Pn, "enc0.", x, None, 1e-5, 2)
+    base_s, _ = O.tblock_fwd(Pn, "enc0.", sk, None, 1e-5, 2)
+    assert torch.allclose(O.tblock_fwd(Pa, "dec0.", x, sk, 1e-5, 2)[0], base_x, atol=1e-12)
+    assert torch.allclose(O.tblock_fwd(Pb, "dec0.", x, sk, 1e-5, 2)[0], base_s, atol=1e-12)
