@@ -28,8 +28,10 @@ constexpr int CH = BQ * 128;                    // one [128 rows][64 bf16] chunk
 
 template <int D> struct ACfg {
   static constexpr int NC = D / 64;             // 64-channel chunks per row
-  static constexpr int Q_OFF = 0, K_OFF = NC * CH, V_OFF = 2 * NC * CH, P_OFF = 3 * NC * CH;
-  static constexpr int SMEM = 3 * NC * CH + 2 * CH + 1024;
+  static constexpr int KV_BYTES = NC * CH;                      // one K tile
+  // Q | K double-buffered | V | P: 96 KB at d = 64, so that two CTAs share an SM
+  static constexpr int Q_OFF = 0, KV_OFF = NC * CH, V_OFF = 3 * NC * CH, P_OFF = 4 * NC * CH;
+  static constexpr int SMEM = 4 * NC * CH + 2 * CH + 1024;
   static constexpr int TMEM_COLS = 256;         // S: columns [0, 128), O: [128, 128 + D)
 };
 
@@ -39,7 +41,7 @@ template <int D>
 __global__ void __launch_bounds__(256, 2) attn_fwd_tc_k(const __grid_constant__ CUtensorMap map, const AtcP p) {
   using A = ACfg<D>;
   extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t bar_q, bar_kv, bar_s, bar_pv;
+  __shared__ uint64_t bar_q, bar_kv[2], bar_v, bar_s, bar_pv;
   __shared__ uint32_t tmem_base_s;
   __shared__ float xch[2][2][BQ];            // [m | l, lx][column half][row]
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
@@ -48,7 +50,7 @@ __global__ void __launch_bounds__(256, 2) attn_fwd_tc_k(const __grid_constant__ 
   const int nkb = (p.T + BKEY - 1) / BKEY;
   if (threadIdx.x == 0) {
     prefetch_tmap(&map);
-    mbar_init(&bar_q, 1); mbar_init(&bar_kv, 1); mbar_init(&bar_s, 1); mbar_init(&bar_pv, 1);
+    mbar_init(&bar_q, 1); mbar_init(&bar_kv[0], 1); mbar_init(&bar_kv[1], 1); mbar_init(&bar_v, 1); mbar_init(&bar_s, 1); mbar_init(&bar_pv, 1);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(&tmem_base_s, A::TMEM_COLS);
@@ -67,62 +69,72 @@ __global__ void __launch_bounds__(256, 2) attn_fwd_tc_k(const __grid_constant__ 
     mbar_expect_tx(&bar_q, A::NC * CH);
     for (int c = 0; c < A::NC; ++c) tma_load_3d(smem + A::Q_OFF + c * CH, &map, &bar_q, h * D + 64 * c, q0, n);
   }
-  uint32_t ph_kv = 0, ph_s = 0, ph_pv = 0;
-  auto load_kv = [&](int kb, bool with_v) {                      // thread 0
-    mbar_expect_tx(&bar_kv, (with_v ? 2 : 1) * A::NC * CH);
-    for (int c = 0; c < A::NC; ++c) {
-      tma_load_3d(smem + A::K_OFF + c * CH, &map, &bar_kv, p.C + h * D + 64 * c, kb * BKEY, n);
-      if (with_v) tma_load_3d(smem + A::V_OFF + c * CH, &map, &bar_kv, 2 * p.C + h * D + 64 * c, kb * BKEY, n);
-    }
+  uint32_t ph_s = 0, ph_pv = 0, ph_v = 0;
+  // K tiles are double-buffered: the tile of iteration it + 1 (the two sweeps form one sequence of 2 nkb iterations) is
+  // requested at the top of iteration it, so its L2 / DRAM latency hides behind this iteration's MMA and softmax.  V has
+  // one buffer: it is requested at the top of its own iteration and first needed after that iteration's softmax.
+  auto load_kv = [&](int it) {                                   // thread 0
+    const int b = it & 1, kb = it % nkb;
+    mbar_expect_tx(&bar_kv[b], A::NC * CH);
+    for (int c = 0; c < A::NC; ++c)
+      tma_load_3d(smem + A::KV_OFF + b * A::KV_BYTES + c * CH, &map, &bar_kv[b], p.C + h * D + 64 * c, kb * BKEY, n);
   };
-  auto issue_s = [&]() {                                         // thread 0: S = Q K^T
+  auto load_v = [&](int kb) {                                    // thread 0
+    mbar_expect_tx(&bar_v, A::NC * CH);
+    for (int c = 0; c < A::NC; ++c)
+      tma_load_3d(smem + A::V_OFF + c * CH, &map, &bar_v, 2 * p.C + h * D + 64 * c, kb * BKEY, n);
+  };
+  auto issue_s = [&](int b) {                                    // thread 0: S = Q K^T
     tc_fence_after();
 #pragma unroll
     for (int k = 0; k < D / 16; ++k) {
       const uint32_t off = (k / 4) * CH + (k % 4) * 32;          // chunk of 64 channels, 32 bytes per K = 16 step
-      umma_bf16(tmem, desc_with_addr(dk, sb + A::Q_OFF + off), desc_with_addr(dk, sb + A::K_OFF + off), idesc_s, k != 0);
+      umma_bf16(tmem, desc_with_addr(dk, sb + A::Q_OFF + off), desc_with_addr(dk, sb + A::KV_OFF + b * A::KV_BYTES + off), idesc_s, k != 0);
     }
     umma_commit(&bar_s);
   };
   const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
   const float c2 = p.scale * 1.4426950408889634f;
 
-  // ---- sweep 1: row maxima of the raw scores
-  float m = -INFINITY;
+  float m = -INFINITY, l = 0.f, lx = 0.f, mc = 0.f;      // l: sum of the bf16 probabilities the P V product sees; lx: the exact sum
+  if (threadIdx.x == 0) load_kv(0);
   mbar_wait(&bar_q, 0);
-  for (int kb = 0; kb < nkb; ++kb) {
-    if (threadIdx.x == 0) load_kv(kb, false);
-    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
-    if (threadIdx.x == 0) issue_s();
-    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
-    tc_fence_after();
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const int ch = 2 * half + c;
-      uint32_t r[32];
-      tmem_ld32(trow + ch * 32, r);
-      tmem_ld_wait();
-      const int kbase = kb * BKEY + ch * 32;
-#pragma unroll
-      for (int i = 0; i < 32; ++i)
-        if (kbase + i < p.T) m = fmaxf(m, __uint_as_float(r[i]));
+  for (int it = 0; it < 2 * nkb; ++it) {
+    const int b = it & 1, kb = it % nkb;
+    const bool sweep2 = it >= nkb;
+    if (it == nkb) {                     // between the sweeps: the row maximum of the two column halves
+      xch[0][half][row] = m;
+      __syncthreads();
+      m = fmaxf(xch[0][0][row], xch[0][1][row]);
+      mc = m * c2;
     }
-    tc_fence_before();
-    __syncthreads();                     // S and the K tile are free again
-  }
-  xch[0][half][row] = m;
-  __syncthreads();
-  m = fmaxf(xch[0][0][row], xch[0][1][row]);
-  // ---- sweep 2: P = exp(scale (S - m)), O += P V
-  float l = 0.f, lx = 0.f;              // l: sum of the bf16 probabilities the P V product sees; lx: the exact sum
-  const float mc = m * c2;
-  for (int kb = 0; kb < nkb; ++kb) {
-    if (kb > 0) { mbar_wait(&bar_pv, ph_pv); ph_pv ^= 1; }      // the previous P V has read P and V
-    if (threadIdx.x == 0) load_kv(kb, true);
-    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
-    if (threadIdx.x == 0) issue_s();
+    if (it > nkb) { mbar_wait(&bar_pv, ph_pv); ph_pv ^= 1; }     // the previous P V has read P and its V tile
+    if (threadIdx.x == 0) {
+      if (it + 1 < 2 * nkb) load_kv(it + 1);                     // that tile's buffer (iteration it - 1's) is free now
+      if (sweep2) load_v(kb);                                    // the previous P V (waited for above) was V's last reader
+    }
+    mbar_wait(&bar_kv[b], (it >> 1) & 1);
+    if (threadIdx.x == 0) issue_s(b);
     mbar_wait(&bar_s, ph_s); ph_s ^= 1;
     tc_fence_after();
+    if (!sweep2) {
+      // ---- sweep 1: row maxima of the raw scores
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        const int ch = 2 * half + c;
+        uint32_t r[32];
+        tmem_ld32(trow + ch * 32, r);
+        tmem_ld_wait();
+        const int kbase = kb * BKEY + ch * 32;
+#pragma unroll
+        for (int i = 0; i < 32; ++i)
+          if (kbase + i < p.T) m = fmaxf(m, __uint_as_float(r[i]));
+      }
+      tc_fence_before();
+      __syncthreads();                   // S is free again
+      continue;
+    }
+    // ---- sweep 2: P = exp(scale (S - m)), O += P V
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
       const int ch = 2 * half + c;
@@ -151,6 +163,7 @@ __global__ void __launch_bounds__(256, 2) attn_fwd_tc_k(const __grid_constant__ 
     tc_fence_before();
     __syncthreads();
     if (threadIdx.x == 0) {
+      mbar_wait(&bar_v, ph_v); ph_v ^= 1;
       tc_fence_after();
 #pragma unroll
       for (int k = 0; k < BKEY / 16; ++k) {
@@ -219,28 +232,31 @@ __device__ __forceinline__ void store_row_chunk32(uint32_t tile, int row, int ch
 
 template <int D> struct BCfg {
   static constexpr int NC = D / 64;
-  // g_q kernel: Q, g_o (resident), K, V (per key tile), g_S
-  static constexpr int Q_OFF = 0, GO_OFF = NC * CH, K_OFF = 2 * NC * CH, V_OFF = 3 * NC * CH, DS_OFF = 4 * NC * CH;
-  static constexpr int SMEM_DQ = 4 * NC * CH + 2 * CH + 1024;
-  // g_k / g_v kernel: K, V (resident), Q, g_o (per query tile), P, g_S
-  static constexpr int P_OFF = 4 * NC * CH, DS2_OFF = 4 * NC * CH + 2 * CH;
-  static constexpr int SMEM_DKV = 4 * NC * CH + 4 * CH + 1024;
+  static constexpr int PAIR = 2 * NC * CH;                      // two operand tiles (K + V, or Q + g_o)
+  // g_q kernel: Q, g_o (resident) | K, V per key tile, double-buffered | g_S
+  static constexpr int Q_OFF = 0, GO_OFF = NC * CH, KV_OFF = PAIR, DS_OFF = 3 * PAIR;
+  static constexpr int SMEM_DQ = 3 * PAIR + 2 * CH + 1024;
+  // g_k / g_v kernel: K, V (resident) | Q, g_o per query tile, double-buffered where it fits (d = 64) | P, g_S
+  static constexpr int NQB = D == 64 ? 2 : 1;
+  static constexpr int K_OFF = 0, V_OFF = NC * CH, QG_OFF = PAIR, P_OFF = (1 + NQB) * PAIR, DS2_OFF = (1 + NQB) * PAIR + 2 * CH;
+  static constexpr int SMEM_DKV = (1 + NQB) * PAIR + 4 * CH + 1024;
 };
 
 template <int D>
-__global__ void __launch_bounds__(128, 1) attn_bwd_dq_tc_k(const __grid_constant__ CUtensorMap mapQ,
+__global__ void __launch_bounds__(256, 1) attn_bwd_dq_tc_k(const __grid_constant__ CUtensorMap mapQ,
                                                            const __grid_constant__ CUtensorMap mapG, const AtbP p) {
   using B = BCfg<D>;
   extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t bar_q, bar_kv, bar_s, bar_dq;
+  __shared__ uint64_t bar_q, bar_kv[2], bar_s, bar_dq;
   __shared__ uint32_t tmem_base_s;
+  __shared__ float xch[2][BQ];
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
-  const int warp = threadIdx.x >> 5, row = threadIdx.x;
+  const int warp = threadIdx.x >> 5, row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;      // two threads per query row
   const int q0 = blockIdx.x * BQ, h = blockIdx.y, n = blockIdx.z;
   const int nkb = (p.T + BKEY - 1) / BKEY;
   if (threadIdx.x == 0) {
     prefetch_tmap(&mapQ); prefetch_tmap(&mapG);
-    mbar_init(&bar_q, 1); mbar_init(&bar_kv, 1); mbar_init(&bar_s, 1); mbar_init(&bar_dq, 1);
+    mbar_init(&bar_q, 1); mbar_init(&bar_kv[0], 1); mbar_init(&bar_kv[1], 1); mbar_init(&bar_s, 1); mbar_init(&bar_dq, 1);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(&tmem_base_s, 512);
@@ -260,43 +276,50 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dq_tc_k(const __grid_constant
       tma_load_3d(smem + B::GO_OFF + c * CH, &mapG, &bar_q, h * D + 64 * c, q0, n);
     }
   }
-  uint32_t ph_kv = 0, ph_s = 0, ph_dq = 0;
-  auto load_kv = [&](int kb) {
-    mbar_expect_tx(&bar_kv, 2 * B::NC * CH);
+  uint32_t ph_s = 0, ph_dq = 0;
+  // the K / V tiles of the 2 nkb iterations (two sweeps) are double-buffered: tile it + 1 is requested at the top of
+  // iteration it
+  auto load_kv = [&](int it) {
+    const int b = it & 1, kb = it % nkb;
+    mbar_expect_tx(&bar_kv[b], B::PAIR);
     for (int c = 0; c < B::NC; ++c) {
-      tma_load_3d(smem + B::K_OFF + c * CH, &mapQ, &bar_kv, p.C + h * D + 64 * c, kb * BKEY, n);
-      tma_load_3d(smem + B::V_OFF + c * CH, &mapQ, &bar_kv, 2 * p.C + h * D + 64 * c, kb * BKEY, n);
+      tma_load_3d(smem + B::KV_OFF + b * B::PAIR + c * CH, &mapQ, &bar_kv[b], p.C + h * D + 64 * c, kb * BKEY, n);
+      tma_load_3d(smem + B::KV_OFF + b * B::PAIR + B::NC * CH + c * CH, &mapQ, &bar_kv[b], 2 * p.C + h * D + 64 * c, kb * BKEY, n);
     }
   };
-  auto issue_s_dp = [&]() {               // S = Q K^T, g_P = g_o V^T
+  auto issue_s_dp = [&](int b) {          // S = Q K^T, g_P = g_o V^T
     tc_fence_after();
+    const uint32_t kv = sb + B::KV_OFF + b * B::PAIR;
 #pragma unroll
     for (int k = 0; k < D / 16; ++k) {
       const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-      umma_bf16(tmem, desc_with_addr(dk, sb + B::Q_OFF + off), desc_with_addr(dk, sb + B::K_OFF + off), idesc_s, k != 0);
+      umma_bf16(tmem, desc_with_addr(dk, sb + B::Q_OFF + off), desc_with_addr(dk, kv + off), idesc_s, k != 0);
     }
 #pragma unroll
     for (int k = 0; k < D / 16; ++k) {
       const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-      umma_bf16(tmem + 128, desc_with_addr(dk, sb + B::GO_OFF + off), desc_with_addr(dk, sb + B::V_OFF + off), idesc_s, k != 0);
+      umma_bf16(tmem + 128, desc_with_addr(dk, sb + B::GO_OFF + off), desc_with_addr(dk, kv + B::NC * CH + off), idesc_s, k != 0);
     }
     umma_commit(&bar_s);
   };
-  const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
   const int q = q0 + row;
   const float c2 = p.scale * 1.4426950408889634f;
   const float lse2 = (q < p.T ? p.lse[((size_t)n * p.heads + h) * p.T + q] : 0.f) * 1.4426950408889634f;
   mbar_wait(&bar_q, 0);
   // ---- sweep 1: D_i = sum_j P_ij g_P_ij
   float Dr = 0.f;
+  if (threadIdx.x == 0) load_kv(0);
   for (int kb = 0; kb < nkb; ++kb) {
-    if (threadIdx.x == 0) load_kv(kb);
-    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
-    if (threadIdx.x == 0) issue_s_dp();
+    const int it = kb, b = it & 1;
+    if (threadIdx.x == 0) load_kv(it + 1);        // (iteration nkb, the first of sweep 2, always exists)
+    mbar_wait(&bar_kv[b], (it >> 1) & 1);
+    if (threadIdx.x == 0) issue_s_dp(b);
     mbar_wait(&bar_s, ph_s); ph_s ^= 1;
     tc_fence_after();
 #pragma unroll
-    for (int ch = 0; ch < BKEY / 32; ++ch) {
+    for (int c = 0; c < 2; ++c) {
+      const int ch = 2 * half + c;
       uint32_t rs[32], rp[32];
       tmem_ld32(trow + ch * 32, rs);
       tmem_ld32(trow + 128 + ch * 32, rp);
@@ -309,17 +332,22 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dq_tc_k(const __grid_constant
     tc_fence_before();
     __syncthreads();
   }
-  if (q < p.T) p.Dg[((size_t)n * p.heads + h) * p.T + q] = Dr;
+  xch[half][row] = Dr;
+  __syncthreads();
+  Dr = xch[0][row] + xch[1][row];
+  if (q < p.T && half == 0) p.Dg[((size_t)n * p.heads + h) * p.T + q] = Dr;
   // ---- sweep 2: g_S = P (g_P - D), g_q += g_S K
   for (int kb = 0; kb < nkb; ++kb) {
-    if (kb > 0) { mbar_wait(&bar_dq, ph_dq); ph_dq ^= 1; }       // the previous g_S K has read g_S and K
-    if (threadIdx.x == 0) load_kv(kb);
-    mbar_wait(&bar_kv, ph_kv); ph_kv ^= 1;
-    if (threadIdx.x == 0) issue_s_dp();
+    const int it = nkb + kb, b = it & 1;
+    if (kb > 0) { mbar_wait(&bar_dq, ph_dq); ph_dq ^= 1; }       // the previous g_S K has read g_S and its K tile
+    if (threadIdx.x == 0 && kb + 1 < nkb) load_kv(it + 1);
+    mbar_wait(&bar_kv[b], (it >> 1) & 1);
+    if (threadIdx.x == 0) issue_s_dp(b);
     mbar_wait(&bar_s, ph_s); ph_s ^= 1;
     tc_fence_after();
 #pragma unroll
-    for (int ch = 0; ch < BKEY / 32; ++ch) {
+    for (int c = 0; c < 2; ++c) {
+      const int ch = 2 * half + c;
       uint32_t rs[32], rp[32], pk[16];
       tmem_ld32(trow + ch * 32, rs);
       tmem_ld32(trow + 128 + ch * 32, rp);
@@ -341,7 +369,7 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dq_tc_k(const __grid_constant
 #pragma unroll
       for (int k = 0; k < BKEY / 16; ++k)
         umma_bf16(tmem + 256, desc_with_addr(dk, sb + B::DS_OFF + (k / 4) * CH + (k % 4) * 32),
-                  desc_with_addr(dmn, sb + B::K_OFF + k * 2048), idesc_q, (kb | k) != 0);
+                  desc_with_addr(dmn, sb + B::KV_OFF + b * B::PAIR + k * 2048), idesc_q, (kb | k) != 0);
       umma_commit(&bar_dq);
     }
   }
@@ -349,7 +377,8 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dq_tc_k(const __grid_constant
   tc_fence_after();
   bf16* gq = p.g_qkv + ((size_t)n * p.T + q) * 3 * p.C + (size_t)h * D;
 #pragma unroll
-  for (int ch = 0; ch < D / 32; ++ch) {
+  for (int cc = 0; cc < D / 64; ++cc) {
+    const int ch = half * (D / 64) + cc;
     uint32_t r[32];
     tmem_ld32(trow + 256 + ch * 32, r);
     tmem_ld_wait();
@@ -374,19 +403,19 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dq_tc_k(const __grid_constant
 }
 
 template <int D>
-__global__ void __launch_bounds__(128, 1) attn_bwd_dkv_tc_k(const __grid_constant__ CUtensorMap mapQ,
+__global__ void __launch_bounds__(256, 1) attn_bwd_dkv_tc_k(const __grid_constant__ CUtensorMap mapQ,
                                                             const __grid_constant__ CUtensorMap mapG, const AtbP p) {
   using B = BCfg<D>;
   extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t bar_kv, bar_q, bar_s, bar_acc;
+  __shared__ uint64_t bar_kv, bar_q[2], bar_s, bar_acc;
   __shared__ uint32_t tmem_base_s;
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
-  const int warp = threadIdx.x >> 5, row = threadIdx.x;
+  const int warp = threadIdx.x >> 5, row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;      // two threads per row
   const int k0 = blockIdx.x * BKEY, h = blockIdx.y, n = blockIdx.z;
   const int nqb = (p.T + BQ - 1) / BQ;
   if (threadIdx.x == 0) {
     prefetch_tmap(&mapQ); prefetch_tmap(&mapG);
-    mbar_init(&bar_kv, 1); mbar_init(&bar_q, 1); mbar_init(&bar_s, 1); mbar_init(&bar_acc, 1);
+    mbar_init(&bar_kv, 1); mbar_init(&bar_q[0], 1); mbar_init(&bar_q[1], 1); mbar_init(&bar_s, 1); mbar_init(&bar_acc, 1);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(&tmem_base_s, 512);
@@ -399,7 +428,7 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dkv_tc_k(const __grid_constan
   constexpr uint64_t dk = smem_desc_sw128(16, 1024), dmn = smem_desc_sw128(CH, 1024);
   constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_t = idesc_bf16(BKEY, D, 1, 1);
   const uint32_t sb = smem_u32(smem);
-  // this CTA's keys: K, V resident (their offsets in B:: are those of the g_q kernel's K / V slots)
+  // this CTA's keys: K, V resident
   if (threadIdx.x == 0) {
     mbar_expect_tx(&bar_kv, 2 * B::NC * CH);
     for (int c = 0; c < B::NC; ++c) {
@@ -407,41 +436,51 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dkv_tc_k(const __grid_constan
       tma_load_3d(smem + B::V_OFF + c * CH, &mapQ, &bar_kv, 2 * p.C + h * D + 64 * c, k0, n);
     }
   }
-  const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+  const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
   const float c2 = p.scale * 1.4426950408889634f;
-  uint32_t ph_q = 0, ph_s = 0, ph_acc = 0;
+  uint32_t ph_s = 0, ph_acc = 0;
+  // the Q / g_o tiles of the query blocks: double-buffered where shared memory allows (d = 64), requested one block ahead
+  auto load_q = [&](int qb) {
+    const int b = B::NQB == 2 ? (qb & 1) : 0;
+    mbar_expect_tx(&bar_q[b], B::PAIR);
+    for (int c = 0; c < B::NC; ++c) {
+      tma_load_3d(smem + B::QG_OFF + b * B::PAIR + c * CH, &mapQ, &bar_q[b], h * D + 64 * c, qb * BQ, n);
+      tma_load_3d(smem + B::QG_OFF + b * B::PAIR + B::NC * CH + c * CH, &mapG, &bar_q[b], h * D + 64 * c, qb * BQ, n);
+    }
+  };
+  if (threadIdx.x == 0 && B::NQB == 2) load_q(0);
   mbar_wait(&bar_kv, 0);
   for (int qb = 0; qb < nqb; ++qb) {
+    const int b = B::NQB == 2 ? (qb & 1) : 0;
+    const uint32_t qg = sb + B::QG_OFF + b * B::PAIR;
     if (qb > 0) { mbar_wait(&bar_acc, ph_acc); ph_acc ^= 1; }    // the previous P^T g_o / g_S^T Q have read Q, g_o, P, g_S
     if (threadIdx.x == 0) {
-      mbar_expect_tx(&bar_q, 2 * B::NC * CH);
-      for (int c = 0; c < B::NC; ++c) {
-        tma_load_3d(smem + B::Q_OFF + c * CH, &mapQ, &bar_q, h * D + 64 * c, qb * BQ, n);
-        tma_load_3d(smem + B::GO_OFF + c * CH, &mapG, &bar_q, h * D + 64 * c, qb * BQ, n);
-      }
+      if (B::NQB == 2) { if (qb + 1 < nqb) load_q(qb + 1); }
+      else load_q(qb);
     }
     const int q = qb * BQ + row;
     const float lse2 = (q < p.T ? p.lse[((size_t)n * p.heads + h) * p.T + q] : 0.f) * 1.4426950408889634f;
     const float Dr = q < p.T ? p.Dg[((size_t)n * p.heads + h) * p.T + q] : 0.f;
-    mbar_wait(&bar_q, ph_q); ph_q ^= 1;
+    mbar_wait(&bar_q[b], B::NQB == 2 ? ((qb >> 1) & 1) : (qb & 1));
     if (threadIdx.x == 0) {
       tc_fence_after();
 #pragma unroll
       for (int k = 0; k < D / 16; ++k) {
         const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-        umma_bf16(tmem, desc_with_addr(dk, sb + B::Q_OFF + off), desc_with_addr(dk, sb + B::K_OFF + off), idesc_s, k != 0);
+        umma_bf16(tmem, desc_with_addr(dk, qg + off), desc_with_addr(dk, sb + B::K_OFF + off), idesc_s, k != 0);
       }
 #pragma unroll
       for (int k = 0; k < D / 16; ++k) {
         const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-        umma_bf16(tmem + 128, desc_with_addr(dk, sb + B::GO_OFF + off), desc_with_addr(dk, sb + B::V_OFF + off), idesc_s, k != 0);
+        umma_bf16(tmem + 128, desc_with_addr(dk, qg + B::NC * CH + off), desc_with_addr(dk, sb + B::V_OFF + off), idesc_s, k != 0);
       }
       umma_commit(&bar_s);
     }
     mbar_wait(&bar_s, ph_s); ph_s ^= 1;
     tc_fence_after();
 #pragma unroll
-    for (int ch = 0; ch < BKEY / 32; ++ch) {
+    for (int c = 0; c < 2; ++c) {
+      const int ch = 2 * half + c;
       uint32_t rs[32], rp[32], pp[16], pd[16];
       tmem_ld32(trow + ch * 32, rs);
       tmem_ld32(trow + 128 + ch * 32, rp);
@@ -466,11 +505,11 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dkv_tc_k(const __grid_constan
       // A = P^T / g_S^T: the [query][key] tiles read MN-major (M = keys: two 64-key chunks, LBO = CH; K = 16 query rows per step)
 #pragma unroll
       for (int k = 0; k < BQ / 16; ++k)
-        umma_bf16(tmem + 256, desc_with_addr(dmn, sb + B::P_OFF + k * 2048), desc_with_addr(dmn, sb + B::GO_OFF + k * 2048),
+        umma_bf16(tmem + 256, desc_with_addr(dmn, sb + B::P_OFF + k * 2048), desc_with_addr(dmn, qg + B::NC * CH + k * 2048),
                   idesc_t, (qb | k) != 0);
 #pragma unroll
       for (int k = 0; k < BQ / 16; ++k)
-        umma_bf16(tmem + 256 + D, desc_with_addr(dmn, sb + B::DS2_OFF + k * 2048), desc_with_addr(dmn, sb + B::Q_OFF + k * 2048),
+        umma_bf16(tmem + 256 + D, desc_with_addr(dmn, sb + B::DS2_OFF + k * 2048), desc_with_addr(dmn, qg + k * 2048),
                   idesc_t, (qb | k) != 0);
       umma_commit(&bar_acc);
     }
@@ -484,7 +523,8 @@ __global__ void __launch_bounds__(128, 1) attn_bwd_dkv_tc_k(const __grid_constan
     const float f = part ? p.scale : 1.0f;
     bf16* dst = part ? gk : gk + p.C;
 #pragma unroll
-    for (int ch = 0; ch < D / 32; ++ch) {
+    for (int cc = 0; cc < D / 64; ++cc) {
+      const int ch = half * (D / 64) + cc;
       uint32_t r[32];
       tmem_ld32(trow + 256 + part * D + ch * 32, r);
       tmem_ld_wait();
@@ -519,8 +559,8 @@ template <int D> bool launch_atb(const CUtensorMap& mq, const CUtensorMap& mg, c
   }
   const dim3 grid((p.T + BQ - 1) / BQ, p.heads, n);
   // the second kernel reads D, which the first one writes after its dependency wait: ordinary stream order between the two
-  if (launch_pdl(attn_bwd_dq_tc_k<D>, grid, dim3(128), BCfg<D>::SMEM_DQ, st, mq, mg, p) != cudaSuccess) return false;
-  return launch_pdl(attn_bwd_dkv_tc_k<D>, grid, dim3(128), BCfg<D>::SMEM_DKV, st, mq, mg, p) == cudaSuccess;
+  if (launch_pdl(attn_bwd_dq_tc_k<D>, grid, dim3(256), BCfg<D>::SMEM_DQ, st, mq, mg, p) != cudaSuccess) return false;
+  return launch_pdl(attn_bwd_dkv_tc_k<D>, grid, dim3(256), BCfg<D>::SMEM_DKV, st, mq, mg, p) == cudaSuccess;
 }
 
 template <int D> bool launch_atc(const CUtensorMap& map, const AtcP& p, int n, cudaStream_t st) {
