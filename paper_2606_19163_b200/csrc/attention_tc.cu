@@ -7,6 +7,10 @@
 //   sweep 2:                     S again -> p = 2^((s - m_i) scale log2 e) -> l_i += p, P as bf16 into a 128-byte-swizzled
 //                                A-operand tile -> O += P V (V is read MN-major, straight from its [keys][d] box) in TMEM
 //   epilogue:                    o_i = O_i / l_i -> bf16 -> global; log-sum-exp_i = m_i scale + ln l_i for the backward.
+// Roles: warps 0-7 are the softmax threads; warp 8 issues every TMA load and MMA.  The S columns are copied to registers
+// in one go and released (bar_sfree), so the Q K^T of the NEXT key tile runs on the tensor pipe while the exponentials of
+// this one are computed; P V of this tile is queued behind it.  K tiles are double-buffered, V is refilled as soon as its
+// P V has completed.  96 KB of shared memory and 256 TMEM columns: two CTAs per SM.
 // Two sweeps instead of the online rescale: O lives in tensor memory, where a rescale per key tile would cost a TMEM
 // round trip of the whole accumulator; the second Q K^T is 1/3 more MMA work on a kernel whose bound is the exponential
 // (128 x 128 MUFU ops per tile = 1024 cycles against 512 of MMA).
@@ -37,176 +41,227 @@ template <int D> struct ACfg {
 
 struct AtcP { int T, C, heads; float scale; bf16* o; float* lse; };
 
+// 2^x for x <= 0 (scores minus their row maximum / log-sum-exp): one MUFU.EX2; results below 2^-126 flush to zero, which
+// exp2f() would pay a compare and two multiplies per element to keep
+__device__ __forceinline__ float ex2a(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// forward: warps 0-7 = softmax (two per TMEM lane quadrant), warp 8 = TMA + MMA issue
+constexpr int SOFTMAX_THREADS = 256, ISSUER_WARP = 8, FWD_THREADS = SOFTMAX_THREADS + 32;
+__device__ __forceinline__ void softmax_sync() { asm volatile("bar.sync 1, %0;" ::"n"(SOFTMAX_THREADS) : "memory"); }
+
 template <int D>
-__global__ void __launch_bounds__(256, 2) attn_fwd_tc_k(const __grid_constant__ CUtensorMap map, const AtcP p) {
+__global__ void __launch_bounds__(FWD_THREADS, 2) attn_fwd_tc_k(const __grid_constant__ CUtensorMap map, const AtcP p) {
   using A = ACfg<D>;
   extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t bar_q, bar_kv[2], bar_v, bar_s, bar_pv;
+  // bar_s: S = Q K^T complete | bar_sfree: all softmax threads hold their S columns in registers | bar_p: P written |
+  // bar_pv: O += P V complete (P and the V tile are free)
+  __shared__ uint64_t bar_q, bar_k[2], bar_v, bar_s, bar_sfree, bar_p, bar_pv;
   __shared__ uint32_t tmem_base_s;
   __shared__ float xch[2][2][BQ];            // [m | l, lx][column half][row]
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
-  const int warp = threadIdx.x >> 5, row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;      // half: which 64 columns
+  const int warp = threadIdx.x >> 5;
   const int q0 = blockIdx.x * BQ, h = blockIdx.y, n = blockIdx.z;
-  const int nkb = (p.T + BKEY - 1) / BKEY;
+  const int nkb = (p.T + BKEY - 1) / BKEY, nit = 2 * nkb;
   if (threadIdx.x == 0) {
     prefetch_tmap(&map);
-    mbar_init(&bar_q, 1); mbar_init(&bar_kv[0], 1); mbar_init(&bar_kv[1], 1); mbar_init(&bar_v, 1); mbar_init(&bar_s, 1); mbar_init(&bar_pv, 1);
+    mbar_init(&bar_q, 1); mbar_init(&bar_k[0], 1); mbar_init(&bar_k[1], 1); mbar_init(&bar_v, 1);
+    mbar_init(&bar_s, 1); mbar_init(&bar_sfree, SOFTMAX_THREADS); mbar_init(&bar_p, SOFTMAX_THREADS); mbar_init(&bar_pv, 1);
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc(&tmem_base_s, A::TMEM_COLS);
+  if (warp == ISSUER_WARP) tmem_alloc(&tmem_base_s, A::TMEM_COLS);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
   pdl_wait();
   pdl_launch_dependents();
-
-  constexpr uint64_t dk = smem_desc_sw128(16, 1024);            // K-major operand: 128-byte rows, 8-row atoms
-  constexpr uint64_t dmn = smem_desc_sw128(CH, 1024);           // MN-major operand (V): LBO = next 64-channel chunk
-  constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_o = idesc_bf16(BQ, D, 0, 1);
   const uint32_t sb = smem_u32(smem);
-  if (threadIdx.x == 0) {
-    mbar_expect_tx(&bar_q, A::NC * CH);
-    for (int c = 0; c < A::NC; ++c) tma_load_3d(smem + A::Q_OFF + c * CH, &map, &bar_q, h * D + 64 * c, q0, n);
-  }
-  uint32_t ph_s = 0, ph_pv = 0, ph_v = 0;
-  // K tiles are double-buffered: the tile of iteration it + 1 (the two sweeps form one sequence of 2 nkb iterations) is
-  // requested at the top of iteration it, so its L2 / DRAM latency hides behind this iteration's MMA and softmax.  V has
-  // one buffer: it is requested at the top of its own iteration and first needed after that iteration's softmax.
-  auto load_kv = [&](int it) {                                   // thread 0
-    const int b = it & 1, kb = it % nkb;
-    mbar_expect_tx(&bar_kv[b], A::NC * CH);
-    for (int c = 0; c < A::NC; ++c)
-      tma_load_3d(smem + A::KV_OFF + b * A::KV_BYTES + c * CH, &map, &bar_kv[b], p.C + h * D + 64 * c, kb * BKEY, n);
-  };
-  auto load_v = [&](int kb) {                                    // thread 0
-    mbar_expect_tx(&bar_v, A::NC * CH);
-    for (int c = 0; c < A::NC; ++c)
-      tma_load_3d(smem + A::V_OFF + c * CH, &map, &bar_v, 2 * p.C + h * D + 64 * c, kb * BKEY, n);
-  };
-  auto issue_s = [&](int b) {                                    // thread 0: S = Q K^T
-    tc_fence_after();
-#pragma unroll
-    for (int k = 0; k < D / 16; ++k) {
-      const uint32_t off = (k / 4) * CH + (k % 4) * 32;          // chunk of 64 channels, 32 bytes per K = 16 step
-      umma_bf16(tmem, desc_with_addr(dk, sb + A::Q_OFF + off), desc_with_addr(dk, sb + A::KV_OFF + b * A::KV_BYTES + off), idesc_s, k != 0);
-    }
-    umma_commit(&bar_s);
-  };
-  const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-  const float c2 = p.scale * 1.4426950408889634f;
 
-  float m = -INFINITY, l = 0.f, lx = 0.f, mc = 0.f;      // l: sum of the bf16 probabilities the P V product sees; lx: the exact sum
-  if (threadIdx.x == 0) load_kv(0);
-  mbar_wait(&bar_q, 0);
-  for (int it = 0; it < 2 * nkb; ++it) {
-    const int b = it & 1, kb = it % nkb;
-    const bool sweep2 = it >= nkb;
-    if (it == nkb) {                     // between the sweeps: the row maximum of the two column halves
-      xch[0][half][row] = m;
-      __syncthreads();
-      m = fmaxf(xch[0][0][row], xch[0][1][row]);
-      mc = m * c2;
-    }
-    if (it > nkb) { mbar_wait(&bar_pv, ph_pv); ph_pv ^= 1; }     // the previous P V has read P and its V tile
-    if (threadIdx.x == 0) {
-      if (it + 1 < 2 * nkb) load_kv(it + 1);                     // that tile's buffer (iteration it - 1's) is free now
-      if (sweep2) load_v(kb);                                    // the previous P V (waited for above) was V's last reader
-    }
-    mbar_wait(&bar_kv[b], (it >> 1) & 1);
-    if (threadIdx.x == 0) issue_s(b);
-    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
-    tc_fence_after();
-    if (!sweep2) {
-      // ---- sweep 1: row maxima of the raw scores
-#pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        const int ch = 2 * half + c;
-        uint32_t r[32];
-        tmem_ld32(trow + ch * 32, r);
-        tmem_ld_wait();
-        const int kbase = kb * BKEY + ch * 32;
-#pragma unroll
-        for (int i = 0; i < 32; ++i)
-          if (kbase + i < p.T) m = fmaxf(m, __uint_as_float(r[i]));
+  if (warp == ISSUER_WARP) {
+    // ---------------------------------------------------------------- TMA + MMA issue (whole warp runs the loop, one lane issues)
+    constexpr uint64_t dk = smem_desc_sw128(16, 1024);            // K-major operand: 128-byte rows, 8-row atoms
+    constexpr uint64_t dmn = smem_desc_sw128(CH, 1024);           // MN-major operand (V): LBO = next 64-channel chunk
+    constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_o = idesc_bf16(BQ, D, 0, 1);
+    // K tiles are double-buffered over the 2 nkb iterations of the two sweeps; V has one buffer, refilled as soon as the
+    // P V product that read it has completed
+    auto load_k = [&](int it) {
+      const int b = it & 1, kb = it % nkb;
+      if (elect_one_sync()) {
+        mbar_expect_tx(&bar_k[b], A::NC * CH);
+        for (int c = 0; c < A::NC; ++c)
+          tma_load_3d(smem + A::KV_OFF + b * A::KV_BYTES + c * CH, &map, &bar_k[b], p.C + h * D + 64 * c, kb * BKEY, n);
       }
-      tc_fence_before();
-      __syncthreads();                   // S is free again
-      continue;
-    }
-    // ---- sweep 2: P = exp(scale (S - m)), O += P V
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const int ch = 2 * half + c;
-      uint32_t r[32];
-      tmem_ld32(trow + ch * 32, r);
-      tmem_ld_wait();
-      const int kbase = kb * BKEY + ch * 32;
-      uint32_t pk[16];
-#pragma unroll
-      for (int i = 0; i < 32; i += 2) {
-        float e0 = kbase + i < p.T ? exp2f(fmaf(__uint_as_float(r[i]), c2, -mc)) : 0.f;
-        float e1 = kbase + i + 1 < p.T ? exp2f(fmaf(__uint_as_float(r[i + 1]), c2, -mc)) : 0.f;
-        pk[i >> 1] = pack_bf16(e0, e1);
-        // o is normalised by the sum of the values the P V product sees (bf16): the rows of P / l sum to one; the
-        // log-sum-exp handed to the backward, which recomputes P in fp32, takes the exact sum
-        l += __uint_as_float(pk[i >> 1] << 16) + __uint_as_float(pk[i >> 1] & 0xffff0000u);
-        lx += e0 + e1;
+    };
+    auto load_v = [&](int kb) {
+      if (elect_one_sync()) {
+        mbar_expect_tx(&bar_v, A::NC * CH);
+        for (int c = 0; c < A::NC; ++c)
+          tma_load_3d(smem + A::V_OFF + c * CH, &map, &bar_v, 2 * p.C + h * D + 64 * c, kb * BKEY, n);
       }
-      // keys [32 ch, 32 ch + 32) = 16-byte pieces 4 (ch & 1) .. + 3 of chunk ch / 2, row `row`, 128-byte swizzle
-      const uint32_t base = sb + A::P_OFF + (ch >> 1) * CH + row * 128;
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-        st_shared_v4(base + ((((ch & 1) * 4 + j) ^ (row & 7)) << 4), pk[4 * j], pk[4 * j + 1], pk[4 * j + 2], pk[4 * j + 3]);
-    }
-    fence_proxy_async_smem();            // P (generic-proxy writes) before the MMA (async proxy) reads it
-    tc_fence_before();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      mbar_wait(&bar_v, ph_v); ph_v ^= 1;
+    };
+    auto issue_pv = [&](int j) {                                  // j: key tile of sweep 2
+      mbar_wait(&bar_p, j & 1);
+      mbar_wait(&bar_v, j & 1);
       tc_fence_after();
 #pragma unroll
       for (int k = 0; k < BKEY / 16; ++k) {
         const uint32_t pa = sb + A::P_OFF + (k / 4) * CH + (k % 4) * 32;      // A = P, K-major: keys 16 k ..
         const uint32_t vb = sb + A::V_OFF + k * 2048;                         // B = V, MN-major: 16 key rows of 128 bytes
-        umma_bf16(tmem + 128, desc_with_addr(dk, pa), desc_with_addr(dmn, vb), idesc_o, (kb | k) != 0);
+        if (elect_one_sync()) umma_bf16(tmem + 128, desc_with_addr(dk, pa), desc_with_addr(dmn, vb), idesc_o, (j | k) != 0);
       }
-      umma_commit(&bar_pv);
+      if (elect_one_sync()) umma_commit(&bar_pv);
+      __syncwarp();
+    };
+    if (elect_one_sync()) {
+      mbar_expect_tx(&bar_q, A::NC * CH);
+      for (int c = 0; c < A::NC; ++c) tma_load_3d(smem + A::Q_OFF + c * CH, &map, &bar_q, h * D + 64 * c, q0, n);
     }
-  }
-  xch[1][half][row] = l;
-  xch[0][half][row] = lx;               // (the maxima have been consumed)
-  mbar_wait(&bar_pv, ph_pv);
-  tc_fence_after();
-  __syncthreads();
-  l = xch[1][0][row] + xch[1][1][row];
-  lx = xch[0][0][row] + xch[0][1][row];
-  // ---- epilogue: o = O / l; each of the row's two threads stores half of the D channels
-  const int q = q0 + row;
-  const float inv = 1.0f / l;
-  bf16* op = p.o + ((size_t)n * p.T + q) * p.C + (size_t)h * D;
+    load_k(0);
+    mbar_wait(&bar_q, 0);
+    for (int it = 0; it < nit; ++it) {
+      const int b = it & 1;
+      mbar_wait(&bar_k[b], (it >> 1) & 1);
+      if (it > 0) mbar_wait(&bar_sfree, (it - 1) & 1);           // S(it - 1) is in registers (and its MMA done: K buffer b ^ 1 free)
+      tc_fence_after();
 #pragma unroll
-  for (int cc = 0; cc < D / 64; ++cc) {
-    const int ch = half * (D / 64) + cc;
-    uint32_t r[32];
-    tmem_ld32(trow + 128 + ch * 32, r);
-    tmem_ld_wait();
-    if (q < p.T) {
+      for (int k = 0; k < D / 16; ++k) {                          // S = Q K^T: runs while the softmax threads work on S(it - 1)
+        const uint32_t off = (k / 4) * CH + (k % 4) * 32;        // chunk of 64 channels, 32 bytes per K = 16 step
+        if (elect_one_sync())
+          umma_bf16(tmem, desc_with_addr(dk, sb + A::Q_OFF + off), desc_with_addr(dk, sb + A::KV_OFF + b * A::KV_BYTES + off), idesc_s, k != 0);
+      }
+      if (elect_one_sync()) umma_commit(&bar_s);
+      __syncwarp();
+      if (it + 1 < nit) load_k(it + 1);
+      if (it > nkb) issue_pv(it - 1 - nkb);                       // O += P V of the previous sweep-2 tile, behind S(it) in the pipe
+      if (it >= nkb) {
+        if (it > nkb) mbar_wait(&bar_pv, (it - 1 - nkb) & 1);    // V's reader has completed
+        load_v(it - nkb);
+      }
+    }
+    issue_pv(nkb - 1);
+  } else {
+    // ---------------------------------------------------------------- softmax: thread = (query row, half of the key columns)
+    const int row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;
+    const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const float c2 = p.scale * 1.4426950408889634f;
+    float m = -INFINITY, l = 0.f, lx = 0.f, mc = 0.f;    // l: sum of the bf16 probabilities the P V product sees; lx: the exact sum
+    for (int it = 0; it < nit; ++it) {
+      const int kb = it % nkb;
+      if (it == nkb) {                     // between the sweeps: the row maximum of the two column halves
+        xch[0][half][row] = m;
+        softmax_sync();
+        m = fmaxf(xch[0][0][row], xch[0][1][row]);
+        mc = m * c2;
+      }
+      mbar_wait(&bar_s, it & 1);
+      tc_fence_after();
+      uint32_t r0[32], r1[32];
+      tmem_ld32(trow + (2 * half) * 32, r0);
+      tmem_ld32(trow + (2 * half + 1) * 32, r1);
+      tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(&bar_sfree);             // the next S may overwrite the columns
+      const int kbase = kb * BKEY + 2 * half * 32;
+      const bool ragged = (kb + 1) * BKEY > p.T;                 // only the last key tile masks its columns
+      if (it < nkb) {
+        // ---- sweep 1: row maxima of the raw scores
+        if (!ragged) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) m = fmaxf(m, fmaxf(__uint_as_float(r0[i]), __uint_as_float(r1[i])));
+        } else {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            if (kbase + i < p.T) m = fmaxf(m, __uint_as_float(r0[i]));
+            if (kbase + 32 + i < p.T) m = fmaxf(m, __uint_as_float(r1[i]));
+          }
+        }
+        continue;
+      }
+      // ---- sweep 2: P = exp(scale (S - m)) as bf16 into the A tile
+      // o is normalised by the sum of the values the P V product sees (bf16): the rows of P / l sum to one; the
+      // log-sum-exp handed to the backward, which recomputes P in fp32, takes the exact sum
+      uint32_t pk0[16], pk1[16];
+      if (!ragged) {
+        // packed fp32 pairs (FFMA2 / FADD2: one issue slot per two keys) around the per-lane MUFU.EX2
+        const f2_t c22 = pk2(c2, c2), mc2 = pk2(-mc, -mc);
+        f2_t l2 = pk2(l, 0.f), lx2 = pk2(lx, 0.f);
+#pragma unroll
+        for (int i = 0; i < 32; i += 2) {
+          float a0, a1;
+          upk2(fma2(pk2(__uint_as_float(r0[i]), __uint_as_float(r0[i + 1])), c22, mc2), a0, a1);
+          float e0 = ex2a(a0), e1 = ex2a(a1);
+          pk0[i >> 1] = pack_bf16(e0, e1);
+          l2 = add2(l2, bf2(pk0[i >> 1]));
+          lx2 = add2(lx2, pk2(e0, e1));
+          upk2(fma2(pk2(__uint_as_float(r1[i]), __uint_as_float(r1[i + 1])), c22, mc2), a0, a1);
+          e0 = ex2a(a0), e1 = ex2a(a1);
+          pk1[i >> 1] = pack_bf16(e0, e1);
+          l2 = add2(l2, bf2(pk1[i >> 1]));
+          lx2 = add2(lx2, pk2(e0, e1));
+        }
+        float t0, t1;
+        upk2(l2, t0, t1); l = t0 + t1;
+        upk2(lx2, t0, t1); lx = t0 + t1;
+      } else {
+#pragma unroll
+        for (int i = 0; i < 32; i += 2) {
+          float e0 = kbase + i < p.T ? ex2a(fmaf(__uint_as_float(r0[i]), c2, -mc)) : 0.f;
+          float e1 = kbase + i + 1 < p.T ? ex2a(fmaf(__uint_as_float(r0[i + 1]), c2, -mc)) : 0.f;
+          pk0[i >> 1] = pack_bf16(e0, e1);
+          l += __uint_as_float(pk0[i >> 1] << 16) + __uint_as_float(pk0[i >> 1] & 0xffff0000u);
+          lx += e0 + e1;
+          e0 = kbase + 32 + i < p.T ? ex2a(fmaf(__uint_as_float(r1[i]), c2, -mc)) : 0.f;
+          e1 = kbase + 32 + i + 1 < p.T ? ex2a(fmaf(__uint_as_float(r1[i + 1]), c2, -mc)) : 0.f;
+          pk1[i >> 1] = pack_bf16(e0, e1);
+          l += __uint_as_float(pk1[i >> 1] << 16) + __uint_as_float(pk1[i >> 1] & 0xffff0000u);
+          lx += e0 + e1;
+        }
+      }
+      if (it > nkb) mbar_wait(&bar_pv, (it - 1 - nkb) & 1);      // the previous P V has read P
+      // keys [32 ch, 32 ch + 32) = 16-byte pieces 4 (ch & 1) .. + 3 of chunk ch / 2 (= half), row `row`, 128-byte swizzle
+      const uint32_t base = sb + A::P_OFF + half * CH + row * 128;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        uint4 v;
-        v.x = pack_bf16(__uint_as_float(r[8 * j]) * inv, __uint_as_float(r[8 * j + 1]) * inv);
-        v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * inv, __uint_as_float(r[8 * j + 3]) * inv);
-        v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * inv, __uint_as_float(r[8 * j + 5]) * inv);
-        v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * inv, __uint_as_float(r[8 * j + 7]) * inv);
-        *reinterpret_cast<uint4*>(op + ch * 32 + 8 * j) = v;
+        st_shared_v4(base + ((j ^ (row & 7)) << 4), pk0[4 * j], pk0[4 * j + 1], pk0[4 * j + 2], pk0[4 * j + 3]);
+        st_shared_v4(base + (((4 + j) ^ (row & 7)) << 4), pk1[4 * j], pk1[4 * j + 1], pk1[4 * j + 2], pk1[4 * j + 3]);
+      }
+      fence_proxy_async_smem();            // P (generic-proxy writes) before the MMA (async proxy) reads it
+      mbar_arrive(&bar_p);
+    }
+    xch[1][half][row] = l;
+    xch[0][half][row] = lx;               // (the maxima have been consumed)
+    softmax_sync();
+    l = xch[1][0][row] + xch[1][1][row];
+    lx = xch[0][0][row] + xch[0][1][row];
+    mbar_wait(&bar_pv, (nkb - 1) & 1);
+    tc_fence_after();
+    // ---- epilogue: o = O / l; each of the row's two threads stores half of the D channels
+    const int q = q0 + row;
+    const float inv = 1.0f / l;
+    bf16* op = p.o + ((size_t)n * p.T + q) * p.C + (size_t)h * D;
+#pragma unroll
+    for (int cc = 0; cc < D / 64; ++cc) {
+      const int ch = half * (D / 64) + cc;
+      uint32_t r[32];
+      tmem_ld32(trow + 128 + ch * 32, r);
+      tmem_ld_wait();
+      if (q < p.T) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          uint4 v;
+          v.x = pack_bf16(__uint_as_float(r[8 * j]) * inv, __uint_as_float(r[8 * j + 1]) * inv);
+          v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * inv, __uint_as_float(r[8 * j + 3]) * inv);
+          v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * inv, __uint_as_float(r[8 * j + 5]) * inv);
+          v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * inv, __uint_as_float(r[8 * j + 7]) * inv);
+          *reinterpret_cast<uint4*>(op + ch * 32 + 8 * j) = v;
+        }
       }
     }
+    if (q < p.T && half == 0) p.lse[((size_t)n * p.heads + h) * p.T + q] = m * p.scale + __logf(lx);
   }
-  if (q < p.T && half == 0) p.lse[((size_t)n * p.heads + h) * p.T + q] = m * p.scale + __logf(lx);
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) {
+  if (warp == ISSUER_WARP) {
     tc_fence_after();
     tmem_dealloc(tmem, A::TMEM_COLS);
   }
@@ -327,7 +382,7 @@ __global__ void __launch_bounds__(256, 1) attn_bwd_dq_tc_k(const __grid_constant
       const int kbase = kb * BKEY + ch * 32;
 #pragma unroll
       for (int i = 0; i < 32; ++i)
-        if (kbase + i < p.T) Dr = fmaf(exp2f(fmaf(__uint_as_float(rs[i]), c2, -lse2)), __uint_as_float(rp[i]), Dr);
+        if (kbase + i < p.T) Dr = fmaf(ex2a(fmaf(__uint_as_float(rs[i]), c2, -lse2)), __uint_as_float(rp[i]), Dr);
     }
     tc_fence_before();
     __syncthreads();
@@ -355,8 +410,8 @@ __global__ void __launch_bounds__(256, 1) attn_bwd_dq_tc_k(const __grid_constant
       const int kbase = kb * BKEY + ch * 32;
 #pragma unroll
       for (int i = 0; i < 32; i += 2) {
-        const float d0 = kbase + i < p.T ? exp2f(fmaf(__uint_as_float(rs[i]), c2, -lse2)) * (__uint_as_float(rp[i]) - Dr) : 0.f;
-        const float d1 = kbase + i + 1 < p.T ? exp2f(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) * (__uint_as_float(rp[i + 1]) - Dr) : 0.f;
+        const float d0 = kbase + i < p.T ? ex2a(fmaf(__uint_as_float(rs[i]), c2, -lse2)) * (__uint_as_float(rp[i]) - Dr) : 0.f;
+        const float d1 = kbase + i + 1 < p.T ? ex2a(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) * (__uint_as_float(rp[i + 1]) - Dr) : 0.f;
         pk[i >> 1] = pack_bf16(d0, d1);
       }
       store_row_chunk32(sb + B::DS_OFF, row, ch, pk);
@@ -489,8 +544,8 @@ __global__ void __launch_bounds__(256, 1) attn_bwd_dkv_tc_k(const __grid_constan
 #pragma unroll
       for (int i = 0; i < 32; i += 2) {
         const bool in0 = q < p.T && kbase + i < p.T, in1 = q < p.T && kbase + i + 1 < p.T;
-        const float e0 = in0 ? exp2f(fmaf(__uint_as_float(rs[i]), c2, -lse2)) : 0.f;
-        const float e1 = in1 ? exp2f(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) : 0.f;
+        const float e0 = in0 ? ex2a(fmaf(__uint_as_float(rs[i]), c2, -lse2)) : 0.f;
+        const float e1 = in1 ? ex2a(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) : 0.f;
         pp[i >> 1] = pack_bf16(e0, e1);
         pd[i >> 1] = pack_bf16(e0 * (__uint_as_float(rp[i]) - Dr), e1 * (__uint_as_float(rp[i + 1]) - Dr));
       }
@@ -569,7 +624,7 @@ template <int D> bool launch_atc(const CUtensorMap& map, const AtcP& p, int n, c
     if (cudaFuncSetAttribute(attn_fwd_tc_k<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, ACfg<D>::SMEM) != cudaSuccess) return false;
     attr = true;
   }
-  return launch_pdl(attn_fwd_tc_k<D>, dim3((p.T + BQ - 1) / BQ, p.heads, n), dim3(256), ACfg<D>::SMEM, st, map, p) == cudaSuccess;
+  return launch_pdl(attn_fwd_tc_k<D>, dim3((p.T + BQ - 1) / BQ, p.heads, n), dim3(FWD_THREADS), ACfg<D>::SMEM, st, map, p) == cudaSuccess;
 }
 
 }  // namespace
