@@ -51,7 +51,8 @@ struct Tc2Params {
   int OH, OW, osy, osx, cout_total;
   float* cst;                     // channel stats [n][2][cout] of the stored output, accumulated (or null)
 };
-struct OutMaps { CUtensorMap m[4]; };      // one output view per phase
+// one output view per phase; MP = false: the one-phase launch's kernel carries one map (0.5 KB less of kernel parameters)
+template <bool MP> struct OutMaps { CUtensorMap m[MP ? 4 : 1]; };
 
 template <int UN, int NJ> struct Cfg2 {
   static constexpr int BN = UN * NJ;                       // output channels per pair tile
@@ -70,10 +71,10 @@ template <int UN, int NJ> struct Cfg2 {
   static_assert(UN % 16 == 0 && UN <= 256, "UMMA N for M = 256");
 };
 
-template <int UN, int NJ>
+template <int UN, int NJ, bool MP>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
 conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
-           const __grid_constant__ CUtensorMap mapB, const __grid_constant__ OutMaps mapO, const Tc2Params p) {
+           const __grid_constant__ CUtensorMap mapB, const __grid_constant__ OutMaps<MP> mapO, const Tc2Params p) {
   using C = Cfg2<UN, NJ>;
   extern __shared__ uint8_t smem_raw[];
   __shared__ uint64_t full_bar[C::STAGES], empty_bar[C::STAGES], tfull_bar[2], tempty_bar[2];
@@ -255,7 +256,7 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            tma_store_4d(&mapO.m[ph], stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
+            tma_store_4d(&mapO.m[MP ? ph : 0], stg + buf * C::BOX_BYTES, co, x_w, y_t + y_w, n_t + n_w);
             bulk_commit();
           }
           static_assert(CW == 32, "the statistics pass reads 16 words per staged row");
@@ -313,12 +314,12 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   }
 }
 
-template <int UN, int NJ>
-bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const OutMaps& o, const Tc2Params& p,
+template <int UN, int NJ, bool MP>
+bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const OutMaps<MP>& o, const Tc2Params& p,
              cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(conv_tc2_k<UN, NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg2<UN, NJ>::SMEM) !=
+    if (cudaFuncSetAttribute(conv_tc2_k<UN, NJ, MP>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg2<UN, NJ>::SMEM) !=
         cudaSuccess) {
       tmap::set_error("cudaFuncSetAttribute(max dynamic smem) failed for conv_tc2_k");
       return false;
@@ -328,7 +329,7 @@ bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b,
   const int tiles = p.nph * p.pair_tiles_m * p.n_tiles;
   const int max_pairs = sm_count() / 2;
   const int pairs = tiles < max_pairs ? tiles : max_pairs;
-  launch_pdl(conv_tc2_k<UN, NJ>, dim3(2 * pairs), dim3(320), Cfg2<UN, NJ>::SMEM, st, a0, a1, b, o, p);
+  launch_pdl(conv_tc2_k<UN, NJ, MP>, dim3(2 * pairs), dim3(320), Cfg2<UN, NJ>::SMEM, st, a0, a1, b, o, p);
   return true;
 }
 
@@ -451,20 +452,28 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
   }
   // output view of each phase: (c, x, y, n) with pixel strides osx/osy from pixel (ooy, oox); box = one warp's
   // [32 pixels][32 channels], 64-byte swizzle
-  OutMaps mo;
-  for (int ph = 0; ph < 4; ++ph) {
-    const int q = ph < p.nph ? ph : 0;
+  OutMaps<true> mo;
+  for (int ph = 0; ph < p.nph; ++ph) {
     const int bwb = p.bw < 32 ? p.bw : 32, bhb = 32 / bwb;
     const size_t C2 = (size_t)a.cout * 2;
     uint64_t dims[4] = {(uint64_t)a.cout, (uint64_t)gw, (uint64_t)gh, (uint64_t)a.n};
     uint64_t str[3] = {(uint64_t)p.osx * C2, (uint64_t)p.osy * a.wout * C2, (uint64_t)a.hout * a.wout * C2};
     const uint32_t cw = 32;        // Cfg2::CW
     uint32_t box[4] = {cw, (uint32_t)bwb, (uint32_t)bhb, 1};
-    const char* base = (const char*)a.out + ((size_t)p.ph_ooy[q] * a.wout + p.ph_oox[q]) * C2;
+    const char* base = (const char*)a.out + ((size_t)p.ph_ooy[ph] * a.wout + p.ph_oox[ph]) * C2;
     if (!get_map(base, 4, dims, str, box, &mo.m[ph], 2 * (int)cw)) return -1;
   }
-  const bool r = un == 160 ? (nj == 2 ? launch2<160, 2>(m0, m1, mb, mo, p, st) : launch2<160, 1>(m0, m1, mb, mo, p, st))
-                           : (nj == 2 ? launch2<128, 2>(m0, m1, mb, mo, p, st) : launch2<128, 1>(m0, m1, mb, mo, p, st));
+  bool r;
+  if (p.nph == 1) {
+    OutMaps<false> m1p;
+    m1p.m[0] = mo.m[0];
+    r = un == 160 ? (nj == 2 ? launch2<160, 2, false>(m0, m1, mb, m1p, p, st) : launch2<160, 1, false>(m0, m1, mb, m1p, p, st))
+                  : (nj == 2 ? launch2<128, 2, false>(m0, m1, mb, m1p, p, st) : launch2<128, 1, false>(m0, m1, mb, m1p, p, st));
+  } else {
+    for (int ph = p.nph; ph < 4; ++ph) mo.m[ph] = mo.m[0];
+    r = un == 160 ? (nj == 2 ? launch2<160, 2, true>(m0, m1, mb, mo, p, st) : launch2<160, 1, true>(m0, m1, mb, mo, p, st))
+                  : (nj == 2 ? launch2<128, 2, true>(m0, m1, mb, mo, p, st) : launch2<128, 1, true>(m0, m1, mb, mo, p, st));
+  }
   return r ? 1 : -1;
 }
 

@@ -289,12 +289,14 @@ __device__ __forceinline__ uint8_t* ring_base(float* sm, int pro_floats) {
 }
 
 // ------------------------------------------------------------------------------ forward apply (one pass)
-template <typename T>
+// ACT (here and in the backward kernels): 1 = GroupNorm + SiLU, 0 = plain GroupNorm (attention blocks); a template parameter
+// because the pixel loops are bound by instruction issue
+template <typename T, int ACT>
 __global__ void __launch_bounds__(512, 2)
 gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw, int G, float eps,
            const T* __restrict__ gamma, const T* __restrict__ beta, const float* __restrict__ cst0,
            const float* __restrict__ cst1, float* __restrict__ mr_out, T* __restrict__ out, int P, int stage_bytes,
-           int pro_floats, int act) {
+           int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -333,8 +335,8 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
 #pragma unroll
       for (int i = 0; i < V; ++i) {
         const float y0 = fmaf(v[0][i], sc[i], sh[i]), y1 = fmaf(v[1][i], sc[i], sh[i]);
-        v[0][i] = act ? silu_t<T>(y0) : y0;          // act == 0: plain GroupNorm (attention blocks)
-        v[1][i] = act ? silu_t<T>(y1) : y1;
+        v[0][i] = ACT ? silu_t<T>(y0) : y0;          // act == 0: plain GroupNorm (attention blocks)
+        v[1][i] = ACT ? silu_t<T>(y1) : y1;
       }
       stv(out + ((size_t)n * hw + pbase + pl) * C + ch, v[0]);
       if (two) stv(out + ((size_t)n * hw + pbase + pl + rows) * C + ch, v[1]);
@@ -345,11 +347,11 @@ gn_apply_k(const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, i
 
 // ------------------------------------------------------------------------------ backward: reduction pass
 // bst[n][0][c] += sum_pix g_y, bst[n][1][c] += sum_pix g_y xhat
-template <typename T>
+template <typename T, int ACT>
 __global__ void __launch_bounds__(512, 1)
 gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
-               const float* __restrict__ mrp, float* __restrict__ bst, int P, int stage_bytes, int pro_floats, int act) {
+               const float* __restrict__ mrp, float* __restrict__ bst, int P, int stage_bytes, int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -387,7 +389,7 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
       lds<T>(st + goff + pl * gpp, g);
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        const float gy = act ? g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i])) : g[i];
+        const float gy = ACT ? g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i])) : g[i];
         v[0][i] += gy;
         v[1][i] = fmaf(gy, fmaf(x[i], rr[i], -mr[i]), v[1][i]);
       }
@@ -401,12 +403,12 @@ gn_bwd_stats_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
 // g_x = r (gamma g_y - A - xhat B) [+ add]; channels [0,dc0) -> dst0, the rest -> dst1 (skip gradient,
 // PAPER.md:L91); acc: += instead of =.  cs0/cs1: per-(image, channel) sums of what this launch ADDS to
 // dst0/dst1 (before bf16 rounding), accumulated.  dgamma/dbeta: += sum_n bst (CTA chunk 0 of each image).
-template <typename T>
+template <typename T, int ACT>
 __global__ void __launch_bounds__(512, 1)
 gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const T* __restrict__ p1, int c1, int hw,
                int G, float eps, const T* __restrict__ gamma, const T* __restrict__ beta,
                const float* __restrict__ mrp, const float* __restrict__ bst, float* dgamma, float* dbeta, const T* __restrict__ add, T* dst0, int dc0, int acc0, T* dst1, int acc1,
-               float* cs0, float* cs1, int P, int stage_bytes, int pro_floats, int act) {
+               float* cs0, float* cs1, int P, int stage_bytes, int pro_floats) {
   constexpr int V = Vec<T>::N;
   extern __shared__ float sm_[];
   __shared__ uint64_t full[RS];
@@ -489,7 +491,7 @@ gn_bwd_apply_k(const T* __restrict__ ga, const T* __restrict__ p0, int c0, const
       if (add) lds<T>(st + eoff + pl * gpp, e);
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        const float gy = act ? g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i])) : g[i];
+        const float gy = ACT ? g[i] * silu_grad_t<T>(fmaf(x[i], sc[i], sh[i])) : g[i];
         const float xh = fmaf(x[i], rr[i], -mr[i]);
         o[i] = sc[i] * gy - k2[i] - xh * k3[i];
         if (add) o[i] += e[i];
@@ -561,44 +563,50 @@ template <typename K> static void allow_big_smem(K kernel) {
   cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
 }
 
+template <typename T, int ACT>
+static void gn_fwd_t(Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta, const float* cst0,
+                     const float* cst1, float* mr_out, void* a_out, cudaStream_t st) {
+  const int C = x.c();
+  const StreamPlan sp = stream_plan(sizeof(T) == 4 ? DT_F32 : DT_BF16, n, hw, C, groups, 0, C * (int)sizeof(T), 2);
+  static bool attr = false;
+  if (!attr) { allow_big_smem(gn_apply_k<T, ACT>); attr = true; }
+  launch_pdl(gn_apply_k<T, ACT>, sp.grid, sp.block, sp.smem, st, (const T*)x.p0, x.c0, (const T*)x.p1, x.c1, hw, groups, eps,
+             (const T*)gamma, (const T*)beta, cst0, cst1, mr_out, (T*)a_out, sp.P, sp.stage_bytes, sp.pro_floats);
+}
+
 int gn_silu_fwd(int dt, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
                 const float* cst0, const float* cst1, float* mr_out, void* a_out, cudaStream_t st, int act) {
-  const int C = x.c();
-  const StreamPlan sp = stream_plan(dt, n, hw, C, groups, 0, C * (int)dt_size(dt), 2);
-  static bool attr = false;
-  if (!attr) { allow_big_smem(gn_apply_k<float>); allow_big_smem(gn_apply_k<bf16>); attr = true; }
-  if (dt == DT_F32)
-    launch_pdl(gn_apply_k<float>, sp.grid, sp.block, sp.smem, st, (const float*)x.p0, x.c0, (const float*)x.p1, x.c1, hw,
-               groups, eps, (const float*)gamma, (const float*)beta, cst0, cst1, mr_out, (float*)a_out, sp.P, sp.stage_bytes,
-               sp.pro_floats, act);
-  else
-    launch_pdl(gn_apply_k<bf16>, sp.grid, sp.block, sp.smem, st, (const bf16*)x.p0, x.c0, (const bf16*)x.p1, x.c1, hw,
-               groups, eps, (const bf16*)gamma, (const bf16*)beta, cst0, cst1, mr_out, (bf16*)a_out, sp.P, sp.stage_bytes,
-               sp.pro_floats, act);
+  if (dt == DT_F32) {
+    if (act) gn_fwd_t<float, 1>(x, n, hw, groups, eps, gamma, beta, cst0, cst1, mr_out, a_out, st);
+    else gn_fwd_t<float, 0>(x, n, hw, groups, eps, gamma, beta, cst0, cst1, mr_out, a_out, st);
+  } else {
+    if (act) gn_fwd_t<bf16, 1>(x, n, hw, groups, eps, gamma, beta, cst0, cst1, mr_out, a_out, st);
+    else gn_fwd_t<bf16, 0>(x, n, hw, groups, eps, gamma, beta, cst0, cst1, mr_out, a_out, st);
+  }
   return 1;
 }
 
-template <typename T>
+template <typename T, int ACT>
 static int gn_bwd_t(const void* g_a, Cat x, int n, int hw, int groups, float eps, const void* gamma, const void* beta,
                     const float* mr, float* bst, const void* add, void* dst0, int dc0, int acc0,
                     void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1, cudaStream_t st,
-                    bool allow_fused, bool fwd_data_ready, int act) {
+                    bool allow_fused, bool fwd_data_ready) {
   const int C = x.c();
   const int dt = sizeof(T) == 4 ? DT_F32 : DT_BF16;
   if (dt == DT_BF16 && allow_fused) {        // one pass with the tensors resident in shared memory where the shape allows (norm_fused.cu)
     const int r = gn_bwd_fused(g_a, x, n, hw, groups, gamma, beta, mr, add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta,
-                               cs0, cs1, st, fwd_data_ready, act);
+                               cs0, cs1, st, fwd_data_ready, ACT);
     if (r > 0) return r;
   }
   static bool attr = false;
-  if (!attr) { allow_big_smem(gn_bwd_stats_k<T>); allow_big_smem(gn_bwd_apply_k<T>); attr = true; }
+  if (!attr) { allow_big_smem(gn_bwd_stats_k<T, ACT>); allow_big_smem(gn_bwd_apply_k<T, ACT>); attr = true; }
   const StreamPlan s1 = stream_plan(dt, n, hw, C, groups, 2, 2 * C * (int)sizeof(T));
-  launch_pdl(gn_bwd_stats_k<T>, s1.grid, s1.block, s1.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
-             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, bst, s1.P, s1.stage_bytes, s1.pro_floats, act);
+  launch_pdl(gn_bwd_stats_k<T, ACT>, s1.grid, s1.block, s1.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
+             x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, bst, s1.P, s1.stage_bytes, s1.pro_floats);
   const StreamPlan s2 = stream_plan(dt, n, hw, C, groups, 1, (add ? 3 : 2) * C * (int)sizeof(T));
-  launch_pdl(gn_bwd_apply_k<T>, s2.grid, s2.block, s2.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
+  launch_pdl(gn_bwd_apply_k<T, ACT>, s2.grid, s2.block, s2.smem, st, (const T*)g_a, (const T*)x.p0, x.c0, (const T*)x.p1,
              x.c1, hw, groups, eps, (const T*)gamma, (const T*)beta, mr, (const float*)bst, dgamma, dbeta,
-             (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes, s2.pro_floats, act);
+             (const T*)add, (T*)dst0, dc0, acc0, (T*)dst1, acc1, cs0, cs1, s2.P, s2.stage_bytes, s2.pro_floats);
   return 2;
 }
 
@@ -606,10 +614,12 @@ int gn_silu_bwd(int dt, const void* g_a, Cat x, int n, int hw, int groups, float
                 const void* beta, const float* mr, float* bst, const void* add, void* dst0,
                 int dc0, int acc0, void* dst1, int acc1, float* dgamma, float* dbeta, float* cs0, float* cs1,
                 cudaStream_t st, bool allow_fused, bool fwd_data_ready, int act) {
-  return dt == DT_F32 ? gn_bwd_t<float>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                        dst1, acc1, dgamma, dbeta, cs0, cs1, st, false, fwd_data_ready, act)
-                      : gn_bwd_t<bf16>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0,
-                                       dst1, acc1, dgamma, dbeta, cs0, cs1, st, allow_fused, fwd_data_ready, act);
+#define PULSE_GN_BWD(T, A, FUSED)                                                                                       \
+  gn_bwd_t<T, A>(g_a, x, n, hw, groups, eps, gamma, beta, mr, bst, add, dst0, dc0, acc0, dst1, acc1, dgamma, dbeta, cs0, \
+                 cs1, st, FUSED, fwd_data_ready)
+  if (dt == DT_F32) return act ? PULSE_GN_BWD(float, 1, false) : PULSE_GN_BWD(float, 0, false);
+  return act ? PULSE_GN_BWD(bf16, 1, allow_fused) : PULSE_GN_BWD(bf16, 0, allow_fused);
+#undef PULSE_GN_BWD
 }
 
 }  // namespace pulse

@@ -95,6 +95,9 @@ __device__ __forceinline__ void cta_reduce(const float (&v)[K][8], bool active, 
   __syncthreads();
 }
 
+// ACT: 1 = GroupNorm + SiLU, 0 = plain GroupNorm (g_y = g_a); a template parameter because the phase loops are bound by
+// instruction issue (a run-time select in them cost 2 % of the kernel)
+template <int ACT>
 __global__ void __launch_bounds__(512, 1)
 gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant__ CUtensorMap mapX1,
                const __grid_constant__ CUtensorMap mapG, const GnfParams p) {
@@ -173,7 +176,7 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const f2_t x = bf2(xv[j]);
-        const f2_t gy = p.act ? mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone)) : bf2(gv[j]);
+        const f2_t gy = ACT ? mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone)) : bf2(gv[j]);
         S2[0][j] = add2(S2[0][j], gy);
         S2[1][j] = fma2(gy, fma2(x, rr2[j], nmr2[j]), S2[1][j]);
       }
@@ -256,7 +259,7 @@ gn_bwd_fused_k(const __grid_constant__ CUtensorMap mapX0, const __grid_constant_
 #pragma unroll
       for (int j = 0; j < 4; ++j) {          // g_y again, in fp32 (keeping it in shared memory would round it to bf16)
         const f2_t x = bf2(xv[j]);
-        const f2_t gy = p.act ? mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone)) : bf2(gv[j]);
+        const f2_t gy = ACT ? mul2(bf2(gv[j]), silu_grad2(fma2(x, sc2[j], sh2[j]), nl2e, one, mone)) : bf2(gv[j]);
         o[j] = fma2(fma2(x, rr2[j], nmr2[j]), nk3[j], fma2(sc2[j], gy, nk2[j]));
       }
       if (p.add) {
@@ -356,7 +359,8 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
   if (!mk(g_a, C, &mg)) return 0;
   static bool attr = false;
   if (!attr) {
-    if (cudaFuncSetAttribute(gn_bwd_fused_k, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048) != cudaSuccess) {
+    if (cudaFuncSetAttribute(gn_bwd_fused_k<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048) != cudaSuccess ||
+        cudaFuncSetAttribute(gn_bwd_fused_k<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048) != cudaSuccess) {
       cudaGetLastError();
       enabled = false;
       return 0;
@@ -372,7 +376,9 @@ int gn_bwd_fused(const void* g_a, Cat x, int n, int hw, int groups, const void* 
   at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[1].val.programmaticStreamSerializationAllowed = (pdl_enabled() && fwd_data_ready) ? 1 : 0;
   cfg.attrs = at; cfg.numAttrs = 2;
-  if (cudaLaunchKernelEx(&cfg, gn_bwd_fused_k, mx0, mx1, mg, p) != cudaSuccess) { cudaGetLastError(); return 0; }
+  const cudaError_t e = act ? cudaLaunchKernelEx(&cfg, gn_bwd_fused_k<1>, mx0, mx1, mg, p)
+                            : cudaLaunchKernelEx(&cfg, gn_bwd_fused_k<0>, mx0, mx1, mg, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return 0; }
   return 1;
 }
 
