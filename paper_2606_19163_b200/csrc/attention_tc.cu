@@ -45,7 +45,7 @@ struct AtcP { int T, C, heads; float scale; bf16* o; float* lse; };
 // exp2f() would pay a compare and two multiplies per element to keep
 __device__ __forceinline__ float ex2a(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
-// forward: warps 0-7 = softmax (two per TMEM lane quadrant), warp 8 = TMA + MMA issue
+// all three kernels: warps 0-7 = softmax (two per TMEM lane quadrant), warp 8 = TMA + MMA issue
 constexpr int SOFTMAX_THREADS = 256, ISSUER_WARP = 8, FWD_THREADS = SOFTMAX_THREADS + 32;
 __device__ __forceinline__ void softmax_sync() { asm volatile("bar.sync 1, %0;" ::"n"(SOFTMAX_THREADS) : "memory"); }
 
@@ -275,6 +275,12 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) attn_fwd_tc_k(const __grid_con
 // P and g_S are recomputed per tile from the saved log-sum-exp, in fp32 on the TMEM rows (thread = query), and handed to
 // the tensor cores as bf16.  D_i = sum_j P_ij g_P_ij comes from a first sweep of the g_q kernel (fp32, from the unrounded
 // P: see attention.cu) and is read by the g_k / g_v kernel.
+// Roles as in the forward: warps 0-7 recompute P / g_S on the TMEM rows, warp 8 issues every TMA load and MMA.  S and g_P
+// go to registers in one pass (4 x tcgen05.ld of 32 columns) and are released at once, so the next tile's S / g_P products
+// run while this tile's exponentials are computed, and this tile's accumulating products are queued behind them.  The
+// streamed operand tiles go round three buffers at d = 64 (the refill then waits for a product issued one iteration
+// earlier, never for one just issued).  Rows / keys past the end need no masks in the g_k / g_v kernel: TMA zero-fills
+// them and a zero row of Q, g_o, K or V contributes nothing to any product.
 struct AtbP { int T, C, heads; float scale; bf16* g_qkv; const float* lse; float* Dg; };
 
 // 128 fp32 values of this thread's row -> bf16 -> chunk-swizzled A tile at `tile` (two 16 KB chunks of 64 columns)
@@ -288,317 +294,408 @@ __device__ __forceinline__ void store_row_chunk32(uint32_t tile, int row, int ch
 template <int D> struct BCfg {
   static constexpr int NC = D / 64;
   static constexpr int PAIR = 2 * NC * CH;                      // two operand tiles (K + V, or Q + g_o)
-  // g_q kernel: Q, g_o (resident) | K, V per key tile, double-buffered | g_S
-  static constexpr int Q_OFF = 0, GO_OFF = NC * CH, KV_OFF = PAIR, DS_OFF = 3 * PAIR;
-  static constexpr int SMEM_DQ = 3 * PAIR + 2 * CH + 1024;
-  // g_k / g_v kernel: K, V (resident) | Q, g_o per query tile, double-buffered where it fits (d = 64) | P, g_S
-  static constexpr int NQB = D == 64 ? 2 : 1;
+  // g_q kernel: Q, g_o (resident) | K, V per key tile in NKV buffers | g_S
+  static constexpr int NKV = D == 64 ? 3 : 2;
+  static constexpr int Q_OFF = 0, GO_OFF = NC * CH, KV_OFF = PAIR, DS_OFF = (1 + NKV) * PAIR;
+  static constexpr int SMEM_DQ = (1 + NKV) * PAIR + 2 * CH + 1024;
+  // g_k / g_v kernel: K, V (resident) | Q, g_o per query tile in NQB buffers | P, g_S
+  static constexpr int NQB = D == 64 ? 3 : 1;
   static constexpr int K_OFF = 0, V_OFF = NC * CH, QG_OFF = PAIR, P_OFF = (1 + NQB) * PAIR, DS2_OFF = (1 + NQB) * PAIR + 2 * CH;
   static constexpr int SMEM_DKV = (1 + NQB) * PAIR + 4 * CH + 1024;
 };
 
 template <int D>
-__global__ void __launch_bounds__(256, 1) attn_bwd_dq_tc_k(const __grid_constant__ CUtensorMap mapQ,
-                                                           const __grid_constant__ CUtensorMap mapG, const AtbP p) {
+__global__ void __launch_bounds__(FWD_THREADS, 1) attn_bwd_dq_tc_k(const __grid_constant__ CUtensorMap mapQ,
+                                                                   const __grid_constant__ CUtensorMap mapG, const AtbP p) {
   using B = BCfg<D>;
   extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t bar_q, bar_kv[2], bar_s, bar_dq;
+  // bar_s: S and g_P complete | bar_sfree: both are in the softmax threads' registers | bar_ds: g_S written |
+  // bar_dq: g_q += g_S K complete (g_S and that K tile are free)
+  __shared__ uint64_t bar_q, bar_kv[B::NKV], bar_s, bar_sfree, bar_ds, bar_dq;
   __shared__ uint32_t tmem_base_s;
   __shared__ float xch[2][BQ];
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
-  const int warp = threadIdx.x >> 5, row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;      // two threads per query row
+  const int warp = threadIdx.x >> 5;
   const int q0 = blockIdx.x * BQ, h = blockIdx.y, n = blockIdx.z;
-  const int nkb = (p.T + BKEY - 1) / BKEY;
+  const int nkb = (p.T + BKEY - 1) / BKEY, nit = 2 * nkb;
   if (threadIdx.x == 0) {
     prefetch_tmap(&mapQ); prefetch_tmap(&mapG);
-    mbar_init(&bar_q, 1); mbar_init(&bar_kv[0], 1); mbar_init(&bar_kv[1], 1); mbar_init(&bar_s, 1); mbar_init(&bar_dq, 1);
+    mbar_init(&bar_q, 1);
+    for (int b = 0; b < B::NKV; ++b) mbar_init(&bar_kv[b], 1);
+    mbar_init(&bar_s, 1); mbar_init(&bar_sfree, SOFTMAX_THREADS); mbar_init(&bar_ds, SOFTMAX_THREADS); mbar_init(&bar_dq, 1);
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc(&tmem_base_s, 512);
+  if (warp == ISSUER_WARP) tmem_alloc(&tmem_base_s, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;      // S: [0,128), g_P: [128,256), g_q: [256, 256 + D)
   pdl_wait();
   pdl_launch_dependents();
-  constexpr uint64_t dk = smem_desc_sw128(16, 1024), dmn = smem_desc_sw128(CH, 1024);
-  constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_q = idesc_bf16(BQ, D, 0, 1);
   const uint32_t sb = smem_u32(smem);
-  if (threadIdx.x == 0) {
-    mbar_expect_tx(&bar_q, 2 * B::NC * CH);
-    for (int c = 0; c < B::NC; ++c) {
-      tma_load_3d(smem + B::Q_OFF + c * CH, &mapQ, &bar_q, h * D + 64 * c, q0, n);
-      tma_load_3d(smem + B::GO_OFF + c * CH, &mapG, &bar_q, h * D + 64 * c, q0, n);
-    }
-  }
-  uint32_t ph_s = 0, ph_dq = 0;
-  // the K / V tiles of the 2 nkb iterations (two sweeps) are double-buffered: tile it + 1 is requested at the top of
-  // iteration it
-  auto load_kv = [&](int it) {
-    const int b = it & 1, kb = it % nkb;
-    mbar_expect_tx(&bar_kv[b], B::PAIR);
-    for (int c = 0; c < B::NC; ++c) {
-      tma_load_3d(smem + B::KV_OFF + b * B::PAIR + c * CH, &mapQ, &bar_kv[b], p.C + h * D + 64 * c, kb * BKEY, n);
-      tma_load_3d(smem + B::KV_OFF + b * B::PAIR + B::NC * CH + c * CH, &mapQ, &bar_kv[b], 2 * p.C + h * D + 64 * c, kb * BKEY, n);
-    }
-  };
-  auto issue_s_dp = [&](int b) {          // S = Q K^T, g_P = g_o V^T
-    tc_fence_after();
-    const uint32_t kv = sb + B::KV_OFF + b * B::PAIR;
-#pragma unroll
-    for (int k = 0; k < D / 16; ++k) {
-      const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-      umma_bf16(tmem, desc_with_addr(dk, sb + B::Q_OFF + off), desc_with_addr(dk, kv + off), idesc_s, k != 0);
-    }
-#pragma unroll
-    for (int k = 0; k < D / 16; ++k) {
-      const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-      umma_bf16(tmem + 128, desc_with_addr(dk, sb + B::GO_OFF + off), desc_with_addr(dk, kv + B::NC * CH + off), idesc_s, k != 0);
-    }
-    umma_commit(&bar_s);
-  };
-  const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-  const int q = q0 + row;
-  const float c2 = p.scale * 1.4426950408889634f;
-  const float lse2 = (q < p.T ? p.lse[((size_t)n * p.heads + h) * p.T + q] : 0.f) * 1.4426950408889634f;
-  mbar_wait(&bar_q, 0);
-  // ---- sweep 1: D_i = sum_j P_ij g_P_ij
-  float Dr = 0.f;
-  if (threadIdx.x == 0) load_kv(0);
-  for (int kb = 0; kb < nkb; ++kb) {
-    const int it = kb, b = it & 1;
-    if (threadIdx.x == 0) load_kv(it + 1);        // (iteration nkb, the first of sweep 2, always exists)
-    mbar_wait(&bar_kv[b], (it >> 1) & 1);
-    if (threadIdx.x == 0) issue_s_dp(b);
-    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
-    tc_fence_after();
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const int ch = 2 * half + c;
-      uint32_t rs[32], rp[32];
-      tmem_ld32(trow + ch * 32, rs);
-      tmem_ld32(trow + 128 + ch * 32, rp);
-      tmem_ld_wait();
-      const int kbase = kb * BKEY + ch * 32;
-#pragma unroll
-      for (int i = 0; i < 32; ++i)
-        if (kbase + i < p.T) Dr = fmaf(ex2a(fmaf(__uint_as_float(rs[i]), c2, -lse2)), __uint_as_float(rp[i]), Dr);
-    }
-    tc_fence_before();
-    __syncthreads();
-  }
-  xch[half][row] = Dr;
-  __syncthreads();
-  Dr = xch[0][row] + xch[1][row];
-  if (q < p.T && half == 0) p.Dg[((size_t)n * p.heads + h) * p.T + q] = Dr;
-  // ---- sweep 2: g_S = P (g_P - D), g_q += g_S K
-  for (int kb = 0; kb < nkb; ++kb) {
-    const int it = nkb + kb, b = it & 1;
-    if (kb > 0) { mbar_wait(&bar_dq, ph_dq); ph_dq ^= 1; }       // the previous g_S K has read g_S and its K tile
-    if (threadIdx.x == 0 && kb + 1 < nkb) load_kv(it + 1);
-    mbar_wait(&bar_kv[b], (it >> 1) & 1);
-    if (threadIdx.x == 0) issue_s_dp(b);
-    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
-    tc_fence_after();
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const int ch = 2 * half + c;
-      uint32_t rs[32], rp[32], pk[16];
-      tmem_ld32(trow + ch * 32, rs);
-      tmem_ld32(trow + 128 + ch * 32, rp);
-      tmem_ld_wait();
-      const int kbase = kb * BKEY + ch * 32;
-#pragma unroll
-      for (int i = 0; i < 32; i += 2) {
-        const float d0 = kbase + i < p.T ? ex2a(fmaf(__uint_as_float(rs[i]), c2, -lse2)) * (__uint_as_float(rp[i]) - Dr) : 0.f;
-        const float d1 = kbase + i + 1 < p.T ? ex2a(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) * (__uint_as_float(rp[i + 1]) - Dr) : 0.f;
-        pk[i >> 1] = pack_bf16(d0, d1);
+
+  if (warp == ISSUER_WARP) {
+    // ---------------------------------------------------------------- TMA + MMA issue
+    constexpr uint64_t dk = smem_desc_sw128(16, 1024), dmn = smem_desc_sw128(CH, 1024);
+    constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_q = idesc_bf16(BQ, D, 0, 1);
+    // the K / V tiles of the 2 nkb iterations (two sweeps) go round NKV buffers
+    auto load_kv = [&](int it) {
+      const int b = it % B::NKV, kb = it % nkb;
+      if (elect_one_sync()) {
+        mbar_expect_tx(&bar_kv[b], B::PAIR);
+        for (int c = 0; c < B::NC; ++c) {
+          tma_load_3d(smem + B::KV_OFF + b * B::PAIR + c * CH, &mapQ, &bar_kv[b], p.C + h * D + 64 * c, kb * BKEY, n);
+          tma_load_3d(smem + B::KV_OFF + b * B::PAIR + B::NC * CH + c * CH, &mapQ, &bar_kv[b], 2 * p.C + h * D + 64 * c, kb * BKEY, n);
+        }
       }
-      store_row_chunk32(sb + B::DS_OFF, row, ch, pk);
-    }
-    fence_proxy_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (threadIdx.x == 0) {
+    };
+    auto issue_dq = [&](int j) {            // j: key tile of sweep 2; its K tile is the one of iteration nkb + j
+      mbar_wait(&bar_ds, j & 1);
       tc_fence_after();
+      const uint32_t kt = sb + B::KV_OFF + ((nkb + j) % B::NKV) * B::PAIR;
 #pragma unroll
       for (int k = 0; k < BKEY / 16; ++k)
-        umma_bf16(tmem + 256, desc_with_addr(dk, sb + B::DS_OFF + (k / 4) * CH + (k % 4) * 32),
-                  desc_with_addr(dmn, sb + B::KV_OFF + b * B::PAIR + k * 2048), idesc_q, (kb | k) != 0);
-      umma_commit(&bar_dq);
-    }
-  }
-  mbar_wait(&bar_dq, ph_dq);
-  tc_fence_after();
-  bf16* gq = p.g_qkv + ((size_t)n * p.T + q) * 3 * p.C + (size_t)h * D;
-#pragma unroll
-  for (int cc = 0; cc < D / 64; ++cc) {
-    const int ch = half * (D / 64) + cc;
-    uint32_t r[32];
-    tmem_ld32(trow + 256 + ch * 32, r);
-    tmem_ld_wait();
-    if (q < p.T) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        uint4 v;
-        v.x = pack_bf16(__uint_as_float(r[8 * j]) * p.scale, __uint_as_float(r[8 * j + 1]) * p.scale);
-        v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * p.scale, __uint_as_float(r[8 * j + 3]) * p.scale);
-        v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * p.scale, __uint_as_float(r[8 * j + 5]) * p.scale);
-        v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * p.scale, __uint_as_float(r[8 * j + 7]) * p.scale);
-        *reinterpret_cast<uint4*>(gq + ch * 32 + 8 * j) = v;
+        if (elect_one_sync())
+          umma_bf16(tmem + 256, desc_with_addr(dk, sb + B::DS_OFF + (k / 4) * CH + (k % 4) * 32), desc_with_addr(dmn, kt + k * 2048),
+                    idesc_q, (j | k) != 0);
+      if (elect_one_sync()) umma_commit(&bar_dq);
+      __syncwarp();
+    };
+    if (elect_one_sync()) {
+      mbar_expect_tx(&bar_q, 2 * B::NC * CH);
+      for (int c = 0; c < B::NC; ++c) {
+        tma_load_3d(smem + B::Q_OFF + c * CH, &mapQ, &bar_q, h * D + 64 * c, q0, n);
+        tma_load_3d(smem + B::GO_OFF + c * CH, &mapG, &bar_q, h * D + 64 * c, q0, n);
       }
     }
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 1) {
-    tc_fence_after();
-    tmem_dealloc(tmem, 512);
-  }
-}
-
-template <int D>
-__global__ void __launch_bounds__(256, 1) attn_bwd_dkv_tc_k(const __grid_constant__ CUtensorMap mapQ,
-                                                            const __grid_constant__ CUtensorMap mapG, const AtbP p) {
-  using B = BCfg<D>;
-  extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t bar_kv, bar_q[2], bar_s, bar_acc;
-  __shared__ uint32_t tmem_base_s;
-  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
-  const int warp = threadIdx.x >> 5, row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;      // two threads per row
-  const int k0 = blockIdx.x * BKEY, h = blockIdx.y, n = blockIdx.z;
-  const int nqb = (p.T + BQ - 1) / BQ;
-  if (threadIdx.x == 0) {
-    prefetch_tmap(&mapQ); prefetch_tmap(&mapG);
-    mbar_init(&bar_kv, 1); mbar_init(&bar_q[0], 1); mbar_init(&bar_q[1], 1); mbar_init(&bar_s, 1); mbar_init(&bar_acc, 1);
-    fence_barrier_init();
-  }
-  if (warp == 1) tmem_alloc(&tmem_base_s, 512);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = tmem_base_s;      // S: [0,128), g_P: [128,256), g_v: [256, 256 + D), g_k: [256 + D, 256 + 2 D)
-  pdl_wait();
-  pdl_launch_dependents();
-  constexpr uint64_t dk = smem_desc_sw128(16, 1024), dmn = smem_desc_sw128(CH, 1024);
-  constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_t = idesc_bf16(BKEY, D, 1, 1);
-  const uint32_t sb = smem_u32(smem);
-  // this CTA's keys: K, V resident
-  if (threadIdx.x == 0) {
-    mbar_expect_tx(&bar_kv, 2 * B::NC * CH);
-    for (int c = 0; c < B::NC; ++c) {
-      tma_load_3d(smem + B::K_OFF + c * CH, &mapQ, &bar_kv, p.C + h * D + 64 * c, k0, n);
-      tma_load_3d(smem + B::V_OFF + c * CH, &mapQ, &bar_kv, 2 * p.C + h * D + 64 * c, k0, n);
+    load_kv(0);
+    mbar_wait(&bar_q, 0);
+    for (int it = 0; it < nit; ++it) {
+      const int b = it % B::NKV;
+      mbar_wait(&bar_kv[b], (it / B::NKV) & 1);
+      if (it > 0) mbar_wait(&bar_sfree, (it - 1) & 1);
+      tc_fence_after();
+      const uint32_t kv = sb + B::KV_OFF + b * B::PAIR;
+#pragma unroll
+      for (int k = 0; k < D / 16; ++k) {      // S = Q K^T
+        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+        if (elect_one_sync()) umma_bf16(tmem, desc_with_addr(dk, sb + B::Q_OFF + off), desc_with_addr(dk, kv + off), idesc_s, k != 0);
+      }
+#pragma unroll
+      for (int k = 0; k < D / 16; ++k) {      // g_P = g_o V^T
+        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+        if (elect_one_sync())
+          umma_bf16(tmem + 128, desc_with_addr(dk, sb + B::GO_OFF + off), desc_with_addr(dk, kv + B::NC * CH + off), idesc_s, k != 0);
+      }
+      if (elect_one_sync()) umma_commit(&bar_s);
+      __syncwarp();
+      // The tile of iteration it + 1 goes into the buffer that iteration it + 1 - NKV used.  Its S / g_P are complete
+      // (bar_sfree); in sweep 2 its g_S K must be, too.  Three buffers (d = 64): that is the product of iteration it - 2,
+      // issued one iteration ago, and it is waited for BEFORE the next one is issued (bar_dq must not run two phases ahead
+      // of a parity wait).  Two buffers (d = 128): the product issued in this iteration.
+      if (B::NKV == 3) {
+        if (it - 2 >= nkb) mbar_wait(&bar_dq, (it - 2 - nkb) & 1);
+        if (it + 1 < nit) load_kv(it + 1);
+      }
+      if (it > nkb) issue_dq(it - 1 - nkb);
+      if (B::NKV == 2) {
+        if (it - 1 >= nkb) mbar_wait(&bar_dq, (it - 1 - nkb) & 1);
+        if (it + 1 < nit) load_kv(it + 1);
+      }
     }
-  }
-  const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-  const float c2 = p.scale * 1.4426950408889634f;
-  uint32_t ph_s = 0, ph_acc = 0;
-  // the Q / g_o tiles of the query blocks: double-buffered where shared memory allows (d = 64), requested one block ahead
-  auto load_q = [&](int qb) {
-    const int b = B::NQB == 2 ? (qb & 1) : 0;
-    mbar_expect_tx(&bar_q[b], B::PAIR);
-    for (int c = 0; c < B::NC; ++c) {
-      tma_load_3d(smem + B::QG_OFF + b * B::PAIR + c * CH, &mapQ, &bar_q[b], h * D + 64 * c, qb * BQ, n);
-      tma_load_3d(smem + B::QG_OFF + b * B::PAIR + B::NC * CH + c * CH, &mapG, &bar_q[b], h * D + 64 * c, qb * BQ, n);
-    }
-  };
-  if (threadIdx.x == 0 && B::NQB == 2) load_q(0);
-  mbar_wait(&bar_kv, 0);
-  for (int qb = 0; qb < nqb; ++qb) {
-    const int b = B::NQB == 2 ? (qb & 1) : 0;
-    const uint32_t qg = sb + B::QG_OFF + b * B::PAIR;
-    if (qb > 0) { mbar_wait(&bar_acc, ph_acc); ph_acc ^= 1; }    // the previous P^T g_o / g_S^T Q have read Q, g_o, P, g_S
-    if (threadIdx.x == 0) {
-      if (B::NQB == 2) { if (qb + 1 < nqb) load_q(qb + 1); }
-      else load_q(qb);
-    }
-    const int q = qb * BQ + row;
+    issue_dq(nkb - 1);
+  } else {
+    // ---------------------------------------------------------------- softmax threads: (query row, half of the key columns)
+    const int row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;
+    const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const int q = q0 + row;
+    const float c2 = p.scale * 1.4426950408889634f;
     const float lse2 = (q < p.T ? p.lse[((size_t)n * p.heads + h) * p.T + q] : 0.f) * 1.4426950408889634f;
-    const float Dr = q < p.T ? p.Dg[((size_t)n * p.heads + h) * p.T + q] : 0.f;
-    mbar_wait(&bar_q[b], B::NQB == 2 ? ((qb >> 1) & 1) : (qb & 1));
-    if (threadIdx.x == 0) {
+    const f2_t c22 = pk2(c2, c2), ml2 = pk2(-lse2, -lse2);
+    float Dr = 0.f;
+    f2_t D2 = pk2(0.f, 0.f), mD2 = D2;
+    for (int it = 0; it < nit; ++it) {
+      const int kb = it % nkb;
+      if (it == nkb) {                     // between the sweeps: D_i of the two column halves
+        float t0, t1;
+        upk2(D2, t0, t1);
+        xch[half][row] = Dr + t0 + t1;
+        softmax_sync();
+        Dr = xch[0][row] + xch[1][row];
+        if (q < p.T && half == 0) p.Dg[((size_t)n * p.heads + h) * p.T + q] = Dr;
+        mD2 = pk2(-Dr, -Dr);
+      }
+      mbar_wait(&bar_s, it & 1);
       tc_fence_after();
-#pragma unroll
-      for (int k = 0; k < D / 16; ++k) {
-        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-        umma_bf16(tmem, desc_with_addr(dk, qg + off), desc_with_addr(dk, sb + B::K_OFF + off), idesc_s, k != 0);
-      }
-#pragma unroll
-      for (int k = 0; k < D / 16; ++k) {
-        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
-        umma_bf16(tmem + 128, desc_with_addr(dk, qg + B::NC * CH + off), desc_with_addr(dk, sb + B::V_OFF + off), idesc_s, k != 0);
-      }
-      umma_commit(&bar_s);
-    }
-    mbar_wait(&bar_s, ph_s); ph_s ^= 1;
-    tc_fence_after();
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const int ch = 2 * half + c;
-      uint32_t rs[32], rp[32], pp[16], pd[16];
-      tmem_ld32(trow + ch * 32, rs);
-      tmem_ld32(trow + 128 + ch * 32, rp);
+      uint32_t rs0[32], rs1[32], rp0[32], rp1[32];
+      tmem_ld32(trow + (2 * half) * 32, rs0);
+      tmem_ld32(trow + (2 * half + 1) * 32, rs1);
+      tmem_ld32(trow + 128 + (2 * half) * 32, rp0);
+      tmem_ld32(trow + 128 + (2 * half + 1) * 32, rp1);
       tmem_ld_wait();
-      const int kbase = k0 + ch * 32;
+      tc_fence_before();
+      mbar_arrive(&bar_sfree);
+      const int kbase = kb * BKEY + 2 * half * 32;
+      const bool ragged = (kb + 1) * BKEY > p.T;
+      if (it < nkb) {
+        // ---- sweep 1: D_i = sum_j P_ij g_P_ij
+        if (!ragged) {
 #pragma unroll
-      for (int i = 0; i < 32; i += 2) {
-        const bool in0 = q < p.T && kbase + i < p.T, in1 = q < p.T && kbase + i + 1 < p.T;
-        const float e0 = in0 ? ex2a(fmaf(__uint_as_float(rs[i]), c2, -lse2)) : 0.f;
-        const float e1 = in1 ? ex2a(fmaf(__uint_as_float(rs[i + 1]), c2, -lse2)) : 0.f;
-        pp[i >> 1] = pack_bf16(e0, e1);
-        pd[i >> 1] = pack_bf16(e0 * (__uint_as_float(rp[i]) - Dr), e1 * (__uint_as_float(rp[i + 1]) - Dr));
+          for (int i = 0; i < 32; i += 2) {
+            float a0, a1;
+            upk2(fma2(pk2(__uint_as_float(rs0[i]), __uint_as_float(rs0[i + 1])), c22, ml2), a0, a1);
+            D2 = fma2(pk2(ex2a(a0), ex2a(a1)), pk2(__uint_as_float(rp0[i]), __uint_as_float(rp0[i + 1])), D2);
+            upk2(fma2(pk2(__uint_as_float(rs1[i]), __uint_as_float(rs1[i + 1])), c22, ml2), a0, a1);
+            D2 = fma2(pk2(ex2a(a0), ex2a(a1)), pk2(__uint_as_float(rp1[i]), __uint_as_float(rp1[i + 1])), D2);
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            if (kbase + i < p.T) Dr = fmaf(ex2a(fmaf(__uint_as_float(rs0[i]), c2, -lse2)), __uint_as_float(rp0[i]), Dr);
+            if (kbase + 32 + i < p.T) Dr = fmaf(ex2a(fmaf(__uint_as_float(rs1[i]), c2, -lse2)), __uint_as_float(rp1[i]), Dr);
+          }
+        }
+        continue;
       }
-      store_row_chunk32(sb + B::P_OFF, row, ch, pp);
-      store_row_chunk32(sb + B::DS2_OFF, row, ch, pd);
+      // ---- sweep 2: g_S = P (g_P - D) as bf16 into the A tile
+      uint32_t pk0[16], pk1[16];
+      if (!ragged) {
+#pragma unroll
+        for (int i = 0; i < 32; i += 2) {
+          float a0, a1, d0, d1;
+          upk2(fma2(pk2(__uint_as_float(rs0[i]), __uint_as_float(rs0[i + 1])), c22, ml2), a0, a1);
+          upk2(mul2(pk2(ex2a(a0), ex2a(a1)), add2(pk2(__uint_as_float(rp0[i]), __uint_as_float(rp0[i + 1])), mD2)), d0, d1);
+          pk0[i >> 1] = pack_bf16(d0, d1);
+          upk2(fma2(pk2(__uint_as_float(rs1[i]), __uint_as_float(rs1[i + 1])), c22, ml2), a0, a1);
+          upk2(mul2(pk2(ex2a(a0), ex2a(a1)), add2(pk2(__uint_as_float(rp1[i]), __uint_as_float(rp1[i + 1])), mD2)), d0, d1);
+          pk1[i >> 1] = pack_bf16(d0, d1);
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < 32; i += 2) {
+          float d0 = kbase + i < p.T ? ex2a(fmaf(__uint_as_float(rs0[i]), c2, -lse2)) * (__uint_as_float(rp0[i]) - Dr) : 0.f;
+          float d1 = kbase + i + 1 < p.T ? ex2a(fmaf(__uint_as_float(rs0[i + 1]), c2, -lse2)) * (__uint_as_float(rp0[i + 1]) - Dr) : 0.f;
+          pk0[i >> 1] = pack_bf16(d0, d1);
+          d0 = kbase + 32 + i < p.T ? ex2a(fmaf(__uint_as_float(rs1[i]), c2, -lse2)) * (__uint_as_float(rp1[i]) - Dr) : 0.f;
+          d1 = kbase + 32 + i + 1 < p.T ? ex2a(fmaf(__uint_as_float(rs1[i + 1]), c2, -lse2)) * (__uint_as_float(rp1[i + 1]) - Dr) : 0.f;
+          pk1[i >> 1] = pack_bf16(d0, d1);
+        }
+      }
+      if (it > nkb) mbar_wait(&bar_dq, (it - 1 - nkb) & 1);      // the previous g_S K has read g_S
+      store_row_chunk32(sb + B::DS_OFF, row, 2 * half, pk0);
+      store_row_chunk32(sb + B::DS_OFF, row, 2 * half + 1, pk1);
+      fence_proxy_async_smem();
+      mbar_arrive(&bar_ds);
     }
-    fence_proxy_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      tc_fence_after();
-      // A = P^T / g_S^T: the [query][key] tiles read MN-major (M = keys: two 64-key chunks, LBO = CH; K = 16 query rows per step)
-#pragma unroll
-      for (int k = 0; k < BQ / 16; ++k)
-        umma_bf16(tmem + 256, desc_with_addr(dmn, sb + B::P_OFF + k * 2048), desc_with_addr(dmn, qg + B::NC * CH + k * 2048),
-                  idesc_t, (qb | k) != 0);
-#pragma unroll
-      for (int k = 0; k < BQ / 16; ++k)
-        umma_bf16(tmem + 256 + D, desc_with_addr(dmn, sb + B::DS2_OFF + k * 2048), desc_with_addr(dmn, qg + k * 2048),
-                  idesc_t, (qb | k) != 0);
-      umma_commit(&bar_acc);
-    }
-  }
-  mbar_wait(&bar_acc, ph_acc);
-  tc_fence_after();
-  const int key = k0 + row;
-  bf16* gk = p.g_qkv + ((size_t)n * p.T + key) * 3 * p.C + (size_t)h * D + p.C;
-#pragma unroll
-  for (int part = 0; part < 2; ++part) {       // 0: g_v (unscaled) -> third 2; 1: g_k (x scale) -> third 1
-    const float f = part ? p.scale : 1.0f;
-    bf16* dst = part ? gk : gk + p.C;
+    mbar_wait(&bar_dq, (nkb - 1) & 1);
+    tc_fence_after();
+    bf16* gq = p.g_qkv + ((size_t)n * p.T + q) * 3 * p.C + (size_t)h * D;
 #pragma unroll
     for (int cc = 0; cc < D / 64; ++cc) {
       const int ch = half * (D / 64) + cc;
       uint32_t r[32];
-      tmem_ld32(trow + 256 + part * D + ch * 32, r);
+      tmem_ld32(trow + 256 + ch * 32, r);
       tmem_ld_wait();
-      if (key < p.T) {
+      if (q < p.T) {
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           uint4 v;
-          v.x = pack_bf16(__uint_as_float(r[8 * j]) * f, __uint_as_float(r[8 * j + 1]) * f);
-          v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * f, __uint_as_float(r[8 * j + 3]) * f);
-          v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * f, __uint_as_float(r[8 * j + 5]) * f);
-          v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * f, __uint_as_float(r[8 * j + 7]) * f);
-          *reinterpret_cast<uint4*>(dst + ch * 32 + 8 * j) = v;
+          v.x = pack_bf16(__uint_as_float(r[8 * j]) * p.scale, __uint_as_float(r[8 * j + 1]) * p.scale);
+          v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * p.scale, __uint_as_float(r[8 * j + 3]) * p.scale);
+          v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * p.scale, __uint_as_float(r[8 * j + 5]) * p.scale);
+          v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * p.scale, __uint_as_float(r[8 * j + 7]) * p.scale);
+          *reinterpret_cast<uint4*>(gq + ch * 32 + 8 * j) = v;
         }
       }
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) {
+  if (warp == ISSUER_WARP) {
+    tc_fence_after();
+    tmem_dealloc(tmem, 512);
+  }
+}
+
+template <int D>
+__global__ void __launch_bounds__(FWD_THREADS, 1) attn_bwd_dkv_tc_k(const __grid_constant__ CUtensorMap mapQ,
+                                                                    const __grid_constant__ CUtensorMap mapG, const AtbP p) {
+  using B = BCfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  // bar_s: S and g_P complete | bar_sfree: both are in registers | bar_p: P and g_S written | bar_acc: g_v += P^T g_o and
+  // g_k += g_S^T Q complete (P, g_S and that Q / g_o tile are free)
+  __shared__ uint64_t bar_kv, bar_q[B::NQB], bar_s, bar_sfree, bar_p, bar_acc;
+  __shared__ uint32_t tmem_base_s;
+  uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
+  const int warp = threadIdx.x >> 5;
+  const int k0 = blockIdx.x * BKEY, h = blockIdx.y, n = blockIdx.z;
+  const int nqb = (p.T + BQ - 1) / BQ;
+  if (threadIdx.x == 0) {
+    prefetch_tmap(&mapQ); prefetch_tmap(&mapG);
+    mbar_init(&bar_kv, 1);
+    for (int b = 0; b < B::NQB; ++b) mbar_init(&bar_q[b], 1);
+    mbar_init(&bar_s, 1); mbar_init(&bar_sfree, SOFTMAX_THREADS); mbar_init(&bar_p, SOFTMAX_THREADS); mbar_init(&bar_acc, 1);
+    fence_barrier_init();
+  }
+  if (warp == ISSUER_WARP) tmem_alloc(&tmem_base_s, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;      // S: [0,128), g_P: [128,256), g_v: [256, 256 + D), g_k: [256 + D, 256 + 2 D)
+  pdl_wait();
+  pdl_launch_dependents();
+  const uint32_t sb = smem_u32(smem);
+
+  if (warp == ISSUER_WARP) {
+    // ---------------------------------------------------------------- TMA + MMA issue
+    constexpr uint64_t dk = smem_desc_sw128(16, 1024), dmn = smem_desc_sw128(CH, 1024);
+    constexpr uint32_t idesc_s = idesc_bf16(BQ, BKEY, 0, 0), idesc_t = idesc_bf16(BKEY, D, 1, 1);
+    if (elect_one_sync()) {                 // this CTA's keys: K, V resident
+      mbar_expect_tx(&bar_kv, 2 * B::NC * CH);
+      for (int c = 0; c < B::NC; ++c) {
+        tma_load_3d(smem + B::K_OFF + c * CH, &mapQ, &bar_kv, p.C + h * D + 64 * c, k0, n);
+        tma_load_3d(smem + B::V_OFF + c * CH, &mapQ, &bar_kv, 2 * p.C + h * D + 64 * c, k0, n);
+      }
+    }
+    auto load_q = [&](int qb) {             // Q and g_o of a query block
+      const int b = qb % B::NQB;
+      if (elect_one_sync()) {
+        mbar_expect_tx(&bar_q[b], B::PAIR);
+        for (int c = 0; c < B::NC; ++c) {
+          tma_load_3d(smem + B::QG_OFF + b * B::PAIR + c * CH, &mapQ, &bar_q[b], h * D + 64 * c, qb * BQ, n);
+          tma_load_3d(smem + B::QG_OFF + b * B::PAIR + B::NC * CH + c * CH, &mapG, &bar_q[b], h * D + 64 * c, qb * BQ, n);
+        }
+      }
+    };
+    auto issue_acc = [&](int j) {           // g_v += P^T g_o, g_k += g_S^T Q of query block j
+      mbar_wait(&bar_p, j & 1);
+      tc_fence_after();
+      const uint32_t qg = sb + B::QG_OFF + (j % B::NQB) * B::PAIR;
+      // A = P^T / g_S^T: the [query][key] tiles read MN-major (M = keys: two 64-key chunks, LBO = CH; K = 16 query rows per step)
+#pragma unroll
+      for (int k = 0; k < BQ / 16; ++k)
+        if (elect_one_sync())
+          umma_bf16(tmem + 256, desc_with_addr(dmn, sb + B::P_OFF + k * 2048), desc_with_addr(dmn, qg + B::NC * CH + k * 2048),
+                    idesc_t, (j | k) != 0);
+#pragma unroll
+      for (int k = 0; k < BQ / 16; ++k)
+        if (elect_one_sync())
+          umma_bf16(tmem + 256 + D, desc_with_addr(dmn, sb + B::DS2_OFF + k * 2048), desc_with_addr(dmn, qg + k * 2048),
+                    idesc_t, (j | k) != 0);
+      if (elect_one_sync()) umma_commit(&bar_acc);
+      __syncwarp();
+    };
+    if (B::NQB == 3) load_q(0);
+    mbar_wait(&bar_kv, 0);
+    for (int qb = 0; qb < nqb; ++qb) {
+      const int b = qb % B::NQB;
+      if (B::NQB == 1) {                    // one Q / g_o buffer (d = 128): the previous block's products first
+        if (qb > 0) { issue_acc(qb - 1); mbar_wait(&bar_acc, (qb - 1) & 1); }
+        load_q(qb);
+      }
+      mbar_wait(&bar_q[b], (qb / B::NQB) & 1);
+      if (qb > 0) mbar_wait(&bar_sfree, (qb - 1) & 1);
+      tc_fence_after();
+      const uint32_t qg = sb + B::QG_OFF + b * B::PAIR;
+#pragma unroll
+      for (int k = 0; k < D / 16; ++k) {
+        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+        if (elect_one_sync()) umma_bf16(tmem, desc_with_addr(dk, qg + off), desc_with_addr(dk, sb + B::K_OFF + off), idesc_s, k != 0);
+      }
+#pragma unroll
+      for (int k = 0; k < D / 16; ++k) {
+        const uint32_t off = (k / 4) * CH + (k % 4) * 32;
+        if (elect_one_sync())
+          umma_bf16(tmem + 128, desc_with_addr(dk, qg + B::NC * CH + off), desc_with_addr(dk, sb + B::V_OFF + off), idesc_s, k != 0);
+      }
+      if (elect_one_sync()) umma_commit(&bar_s);
+      __syncwarp();
+      if (B::NQB == 3) {
+        // block qb + 1 goes into the buffer block qb - 2 used: its products (issued one iteration ago) are waited for
+        // BEFORE the next ones are issued (bar_acc must not run two phases ahead of a parity wait)
+        if (qb >= 2) mbar_wait(&bar_acc, (qb - 2) & 1);
+        if (qb + 1 < nqb) load_q(qb + 1);
+        if (qb > 0) issue_acc(qb - 1);
+      }
+    }
+    issue_acc(nqb - 1);
+  } else {
+    // ---------------------------------------------------------------- softmax threads: (query row, half of this CTA's keys)
+    const int row = threadIdx.x & (BQ - 1), half = threadIdx.x >> 7;
+    const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const float c2 = p.scale * 1.4426950408889634f;
+    const f2_t c22 = pk2(c2, c2);
+    for (int qb = 0; qb < nqb; ++qb) {
+      const int q = qb * BQ + row;
+      // rows past the end: Q and g_o are zero-filled by TMA, so with lse = D = 0 their P = 1 and g_S = 0 meet zero rows of
+      // g_o / Q in the products: no masks
+      const float lse2 = (q < p.T ? p.lse[((size_t)n * p.heads + h) * p.T + q] : 0.f) * 1.4426950408889634f;
+      const float Dr = q < p.T ? p.Dg[((size_t)n * p.heads + h) * p.T + q] : 0.f;
+      const f2_t ml2 = pk2(-lse2, -lse2), mD2 = pk2(-Dr, -Dr);
+      mbar_wait(&bar_s, qb & 1);
+      tc_fence_after();
+      uint32_t rs0[32], rs1[32], rp0[32], rp1[32];
+      tmem_ld32(trow + (2 * half) * 32, rs0);
+      tmem_ld32(trow + (2 * half + 1) * 32, rs1);
+      tmem_ld32(trow + 128 + (2 * half) * 32, rp0);
+      tmem_ld32(trow + 128 + (2 * half + 1) * 32, rp1);
+      tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(&bar_sfree);
+      uint32_t pp0[16], pp1[16], pd0[16], pd1[16];
+#pragma unroll
+      for (int i = 0; i < 32; i += 2) {
+        float a0, a1, d0, d1;
+        upk2(fma2(pk2(__uint_as_float(rs0[i]), __uint_as_float(rs0[i + 1])), c22, ml2), a0, a1);
+        a0 = ex2a(a0); a1 = ex2a(a1);
+        pp0[i >> 1] = pack_bf16(a0, a1);
+        upk2(mul2(pk2(a0, a1), add2(pk2(__uint_as_float(rp0[i]), __uint_as_float(rp0[i + 1])), mD2)), d0, d1);
+        pd0[i >> 1] = pack_bf16(d0, d1);
+        upk2(fma2(pk2(__uint_as_float(rs1[i]), __uint_as_float(rs1[i + 1])), c22, ml2), a0, a1);
+        a0 = ex2a(a0); a1 = ex2a(a1);
+        pp1[i >> 1] = pack_bf16(a0, a1);
+        upk2(mul2(pk2(a0, a1), add2(pk2(__uint_as_float(rp1[i]), __uint_as_float(rp1[i + 1])), mD2)), d0, d1);
+        pd1[i >> 1] = pack_bf16(d0, d1);
+      }
+      if (qb > 0) mbar_wait(&bar_acc, (qb - 1) & 1);      // the previous products have read P and g_S
+      store_row_chunk32(sb + B::P_OFF, row, 2 * half, pp0);
+      store_row_chunk32(sb + B::P_OFF, row, 2 * half + 1, pp1);
+      store_row_chunk32(sb + B::DS2_OFF, row, 2 * half, pd0);
+      store_row_chunk32(sb + B::DS2_OFF, row, 2 * half + 1, pd1);
+      fence_proxy_async_smem();
+      mbar_arrive(&bar_p);
+    }
+    mbar_wait(&bar_acc, (nqb - 1) & 1);
+    tc_fence_after();
+    const int key = k0 + row;
+    bf16* gk = p.g_qkv + ((size_t)n * p.T + key) * 3 * p.C + (size_t)h * D + p.C;
+#pragma unroll
+    for (int part = 0; part < 2; ++part) {       // 0: g_v (unscaled) -> third 2; 1: g_k (x scale) -> third 1
+      const float f = part ? p.scale : 1.0f;
+      bf16* dst = part ? gk : gk + p.C;
+#pragma unroll
+      for (int cc = 0; cc < D / 64; ++cc) {
+        const int ch = half * (D / 64) + cc;
+        uint32_t r[32];
+        tmem_ld32(trow + 256 + part * D + ch * 32, r);
+        tmem_ld_wait();
+        if (key < p.T) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            uint4 v;
+            v.x = pack_bf16(__uint_as_float(r[8 * j]) * f, __uint_as_float(r[8 * j + 1]) * f);
+            v.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * f, __uint_as_float(r[8 * j + 3]) * f);
+            v.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * f, __uint_as_float(r[8 * j + 5]) * f);
+            v.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * f, __uint_as_float(r[8 * j + 7]) * f);
+            *reinterpret_cast<uint4*>(dst + ch * 32 + 8 * j) = v;
+          }
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == ISSUER_WARP) {
     tc_fence_after();
     tmem_dealloc(tmem, 512);
   }
@@ -614,8 +711,8 @@ template <int D> bool launch_atb(const CUtensorMap& mq, const CUtensorMap& mg, c
   }
   const dim3 grid((p.T + BQ - 1) / BQ, p.heads, n);
   // the second kernel reads D, which the first one writes after its dependency wait: ordinary stream order between the two
-  if (launch_pdl(attn_bwd_dq_tc_k<D>, grid, dim3(256), BCfg<D>::SMEM_DQ, st, mq, mg, p) != cudaSuccess) return false;
-  return launch_pdl(attn_bwd_dkv_tc_k<D>, grid, dim3(256), BCfg<D>::SMEM_DKV, st, mq, mg, p) == cudaSuccess;
+  if (launch_pdl(attn_bwd_dq_tc_k<D>, grid, dim3(FWD_THREADS), BCfg<D>::SMEM_DQ, st, mq, mg, p) != cudaSuccess) return false;
+  return launch_pdl(attn_bwd_dkv_tc_k<D>, grid, dim3(FWD_THREADS), BCfg<D>::SMEM_DKV, st, mq, mg, p) == cudaSuccess;
 }
 
 template <int D> bool launch_atc(const CUtensorMap& map, const AtcP& p, int n, cudaStream_t st) {
