@@ -87,7 +87,8 @@ enum { PULSE_CONV_AUTO = 0, PULSE_CONV_SIMT = 1, PULSE_CONV_TC_PAIR = 2, PULSE_C
  *   PULSE_NO_GN_FUSED=1      as PULSE_FLAG_GN_TWO_PASS, for every stage of the process
  *   PULSE_CONV_1CTA=1        as PULSE_FLAG_CONV_1CTA, for every conv of the process without an explicit selector
  *   PULSE_CONV_1CTA_TILES=k  convs with at most k single-CTA tiles take the single-CTA kernel (default: the SM count)
- *   PULSE_WGRAD_1CTA=1       single-CTA tcgen05 weight-gradient kernel everywhere */
+ *   PULSE_WGRAD_1CTA=1       single-CTA tcgen05 weight-gradient kernel everywhere
+ *   PULSE_NO_SPLIT_K=1       no cluster split-K in the CTA-pair conv kernel (few-tile convs then take the single-CTA kernel) */
 
 /* One operation of the linearised model.  cin excludes the popped skip:
  * a decoder ResBlock runs on concat_C(h[cin], skip[skip_channels]), h first. */

@@ -17,6 +17,13 @@
 //   empty[s]  (own copy)       tcgen05.commit multicast to both CTAs when the MMAs reading stage s are done,
 //   tfull[a]  (own copy)       tcgen05.commit multicast when a tile's accumulator is complete,
 //   tempty[a] (leader's copy)  8 arrivals: the 4 epilogue warps of both CTAs (remote arrive from the peer).
+//
+// Split-K over a cluster (SK = 2 or 4 pairs, cluster of 2 SK CTAs) for convs with few tiles and a long K (1280 channels on
+// 8x8 / 16x16 pixels: 8 / 32 pair tiles for 74 pairs): the SK pairs of a cluster take the SAME output tile and 1/SK of the
+// K blocks each.  The partial accumulators meet through distributed shared memory: the tile's 32-channel chunks are dealt
+// round-robin to the SK pairs; every CTA writes the chunks it does not own into the owner's (by then idle) operand ring
+// (st.shared::cluster, 16 KB per chunk and sender), the owner adds them to its TMEM chunk and runs the ordinary epilogue on
+// it.  Two cluster barriers: all rings idle / all partials delivered.  One tile per cluster.
 #include <cuda.h>
 
 #include <cstdlib>
@@ -71,8 +78,8 @@ template <int UN, int NJ> struct Cfg2 {
   static_assert(UN % 16 == 0 && UN <= 256, "UMMA N for M = 256");
 };
 
-template <int UN, int NJ, bool MP>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
+template <int UN, int NJ, bool MP, int SK>
+__global__ void __cluster_dims__(2 * SK, 1, 1) __launch_bounds__(320, 1)
 conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
            const __grid_constant__ CUtensorMap mapB, const __grid_constant__ OutMaps<MP> mapO, const Tc2Params p) {
   using C = Cfg2<UN, NJ>;
@@ -81,10 +88,14 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   __shared__ uint32_t tmem_base_s;
   uint8_t* smem = smem_raw + ((1024 - (smem_u32(smem_raw) & 1023)) & 1023);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();
+  // rank: this CTA inside its pair; lead: cluster rank of the pair's leader; ks: which share of the K blocks (split-K)
+  const uint32_t crank = cluster_ctarank();
+  const uint32_t rank = SK == 1 ? crank : (crank & 1u), lead = SK == 1 ? 0u : (crank & ~1u);
+  const int ks = SK == 1 ? 0 : (int)(crank >> 1);
+  const uint16_t pair_mask = (uint16_t)(3u << lead);
   const int tiles_ph = p.pair_tiles_m * p.n_tiles;      // tiles per phase
   const int total_tiles = p.nph * tiles_ph;
-  const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+  const int pair = blockIdx.x / (2 * SK), npairs = gridDim.x / (2 * SK);      // tile walkers: pairs, or clusters of SK pairs
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&mapA0); prefetch_tmap(&mapA1); prefetch_tmap(&mapB); prefetch_tmap(&mapO.m[0]);
@@ -110,12 +121,13 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
         const int mt = 2 * mp + (int)rank;
         const int n0 = (mt / p.tiles_h) * p.bn, y0 = (mt % p.tiles_h) * p.bh;
         const int tap0 = p.ph_tap0[ph], num_kb = (p.ph_tap0[ph + 1] - tap0) * p.c_blocks, wrow = p.ph_wrow[ph];
-        for (int kb = 0; kb < num_kb; ++kb) {
+        const int kb0 = SK == 1 ? 0 : ks * num_kb / SK, kb1 = SK == 1 ? num_kb : (ks + 1) * num_kb / SK;
+        for (int kb = kb0; kb < kb1; ++kb) {
           const int ti = kb / p.c_blocks, cb = kb - ti * p.c_blocks;
           const Tap t = p.taps[tap0 + ti];
           mbar_wait(&empty_bar[stage], phase ^ 1);
           if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * C::STAGE_BYTES);
-          const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
+          const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), lead);
           uint8_t* sa = smem + stage * C::STAGE_BYTES;
           const bool first = cb < p.c0_blocks;
           const CUtensorMap* ma = first ? &mapA0 : &mapA1;
@@ -144,7 +156,8 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
         mbar_wait(&tempty_bar[acc], acc_phase ^ 1);
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + acc * C::BN;
-        for (int kb = 0; kb < num_kb; ++kb) {
+        const int kb0 = SK == 1 ? 0 : ks * num_kb / SK, kb1 = SK == 1 ? num_kb : (ks + 1) * num_kb / SK;
+        for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(&full_bar[stage], phase);
           tc_fence_after();
           const uint32_t a_lo = desc_lo0 + stage * (C::STAGE_BYTES >> 4), b_lo = a_lo + (A_BYTES >> 4);
@@ -154,9 +167,9 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
 #pragma unroll
               for (int j = 0; j < NJ; ++j)
                 umma2_bf16(tmem_d + j * UN, ((uint64_t)desc_hi << 32) | (a_lo + 2 * k),
-                           ((uint64_t)desc_hi << 32) | (b_lo + j * (C::B_SLICE >> 4) + 2 * k), idesc, (kb | k) != 0);
-            umma2_commit_mc(&empty_bar[stage], 3);
-            if (kb == num_kb - 1) umma2_commit_mc(&tfull_bar[acc], 3);
+                           ((uint64_t)desc_hi << 32) | (b_lo + j * (C::B_SLICE >> 4) + 2 * k), idesc, ((kb - kb0) | k) != 0);
+            umma2_commit_mc(&empty_bar[stage], pair_mask);
+            if (kb == kb1 - 1) umma2_commit_mc(&tfull_bar[acc], pair_mask);
           }
           __syncwarp();
           if (++stage == C::STAGES) { stage = 0; phase ^= 1; }
@@ -213,25 +226,10 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
       mbar_wait(&tfull_bar[acc], acc_phase);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * C::BN;
-      // software pipeline: the TMEM load of this warp's next chunk is issued before the current chunk is converted
-      // and stored (tcgen05.wait::ld waits for every outstanding load, so the next one is issued right after it)
-      constexpr int NCH = C::BN / CW, NIT = (NCH + 1) / 2;
-      uint32_t rr[2][32];
-      tmem_ld32(taddr + grp * CW, rr[0]);
-#pragma unroll
-      for (int it = 0; it < NIT; ++it) {
-        const int ch = grp + 2 * it;
-        if (ch >= NCH) break;
-        uint32_t (&r)[32] = rr[it & 1];
+      // one 32-channel chunk of this warp's 32 pixels, accumulator values in r: + bias / temb / residual -> bf16 -> staging
+      // box -> TMA store; channel statistics of the stored values
+      auto finish_chunk = [&](const int ch, uint32_t (&r)[32]) {
         const int co = nt * C::BN + ch * CW;
-        tmem_ld_wait();
-        if (ch + 2 < NCH) {
-          tmem_ld32(taddr + (ch + 2) * CW, rr[(it + 1) & 1]);
-        } else {                                    // that was this warp's last TMEM read of the tile
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty_bar[acc]), 0));
-        }
         {
           if (lane == 0) bulk_wait_read<C::NBUF - 1>();   // the store that last used this box has read it
           __syncwarp();
@@ -300,11 +298,81 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
           }
           buf ^= 1;
         }
+      };
+      constexpr int NCH = C::BN / CW;
+      if constexpr (SK == 1) {
+        // software pipeline: the TMEM load of this warp's next chunk is issued before the current chunk is converted
+        // and stored (tcgen05.wait::ld waits for every outstanding load, so the next one is issued right after it)
+        constexpr int NIT = (NCH + 1) / 2;
+        uint32_t rr[2][32];
+        tmem_ld32(taddr + grp * CW, rr[0]);
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+          const int ch = grp + 2 * it;
+          if (ch >= NCH) break;
+          uint32_t (&r)[32] = rr[it & 1];
+          tmem_ld_wait();
+          if (ch + 2 < NCH) {
+            tmem_ld32(taddr + (ch + 2) * CW, rr[(it + 1) & 1]);
+          } else {                                    // that was this warp's last TMEM read of the tile
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty_bar[acc]), lead));
+          }
+          finish_chunk(ch, r);
+        }
+      } else {
+        // split-K: this warp's chunks are [ch_lo, ch_hi); chunk ch belongs to pair ch % SK of the cluster
+        constexpr int PER = (NCH + 1) / 2;
+        const int ch_lo = grp * PER, ch_hi = ch_lo + PER < NCH ? ch_lo + PER : NCH;
+        const uint32_t ring = smem_u32(smem);
+        const uint32_t rsw = (uint32_t)(row & 7);
+        cluster_arrive(); cluster_wait();             // every CTA of the cluster has seen its accumulator complete: all rings idle
+        for (int ch = ch_lo; ch < ch_hi; ++ch) {
+          const int owner = ch % SK;
+          if (owner == ks) continue;
+          uint32_t r[32];
+          tmem_ld32(taddr + ch * CW, r);
+          tmem_ld_wait();
+          // slot (owned-chunk ordinal, sender ordinal) of the owner's ring: [128 rows][32 fp32], 16-byte pieces swizzled by row
+          const int slot = (ch / SK) * (SK - 1) + (ks < owner ? ks : ks - 1);
+          const uint32_t dst = mapa_u32(ring + (uint32_t)((slot * 128 + row) * 128), (uint32_t)(owner * 2) + rank);
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst + ((i ^ rsw) << 4)), "r"(r[4 * i]),
+                         "r"(r[4 * i + 1]), "r"(r[4 * i + 2]), "r"(r[4 * i + 3]) : "memory");
+        }
+        cluster_arrive(); cluster_wait();             // all partials delivered
+        for (int ch = ch_lo; ch < ch_hi; ++ch) {
+          if (ch % SK != ks) continue;
+          uint32_t r[32];
+          tmem_ld32(taddr + ch * CW, r);
+          tmem_ld_wait();
+#pragma unroll
+          for (int s_ = 0; s_ < SK - 1; ++s_) {
+            const uint32_t src = ring + (uint32_t)((((ch / SK) * (SK - 1) + s_) * 128 + row) * 128);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              uint32_t v0, v1, v2, v3;
+              asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3) : "r"(src + ((i ^ rsw) << 4)));
+              r[4 * i] = __float_as_uint(__uint_as_float(r[4 * i]) + __uint_as_float(v0));
+              r[4 * i + 1] = __float_as_uint(__uint_as_float(r[4 * i + 1]) + __uint_as_float(v1));
+              r[4 * i + 2] = __float_as_uint(__uint_as_float(r[4 * i + 2]) + __uint_as_float(v2));
+              r[4 * i + 3] = __float_as_uint(__uint_as_float(r[4 * i + 3]) + __uint_as_float(v3));
+            }
+          }
+          finish_chunk(ch, r);
+        }
       }
       if (C::ACC == 2) { acc ^= 1; if (acc == 0) acc_phase ^= 1; }
       else acc_phase ^= 1;
     }
     if (lane == 0) bulk_wait_read<0>();       // the staging boxes have been read; the global writes complete before the grid does
+  }
+  if (SK > 1 && warp < 2) {      // the split-K exchange's two cluster barriers count every thread of the cluster
+    __syncwarp();
+    cluster_arrive(); cluster_wait();
+    cluster_arrive(); cluster_wait();
   }
   tc_fence_before();
   cluster_sync_all();          // nobody leaves (or frees TMEM) while the peer may still read its shared memory / TMEM
@@ -314,12 +382,12 @@ conv_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CU
   }
 }
 
-template <int UN, int NJ, bool MP>
+template <int UN, int NJ, bool MP, int SK>
 bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b, const OutMaps<MP>& o, const Tc2Params& p,
              cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(conv_tc2_k<UN, NJ, MP>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg2<UN, NJ>::SMEM) !=
+    if (cudaFuncSetAttribute(conv_tc2_k<UN, NJ, MP, SK>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg2<UN, NJ>::SMEM) !=
         cudaSuccess) {
       tmap::set_error("cudaFuncSetAttribute(max dynamic smem) failed for conv_tc2_k");
       return false;
@@ -328,9 +396,20 @@ bool launch2(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& b,
   }
   const int tiles = p.nph * p.pair_tiles_m * p.n_tiles;
   const int max_pairs = sm_count() / 2;
-  const int pairs = tiles < max_pairs ? tiles : max_pairs;
-  launch_pdl(conv_tc2_k<UN, NJ, MP>, dim3(2 * pairs), dim3(320), Cfg2<UN, NJ>::SMEM, st, a0, a1, b, o, p);
+  // split-K: one tile per cluster of SK pairs (the exchange's cluster barriers are counted once per CTA)
+  const int pairs = SK > 1 ? tiles : (tiles < max_pairs ? tiles : max_pairs);
+  launch_pdl(conv_tc2_k<UN, NJ, MP, SK>, dim3(2 * SK * pairs), dim3(320), Cfg2<UN, NJ>::SMEM, st, a0, a1, b, o, p);
   return true;
+}
+
+// Split-K factor for a one-phase conv (conv_tc2.cu header): the largest of 4, 2 whose clusters all run in one wave and
+// that leaves every pair at least 8 K blocks; 1 = no split.  Only the 320-channel tile (UN = 160, NJ = 2) is instantiated.
+int split_k(int tiles, int num_kb, int un, int nj) {
+  if (un != 160 || nj != 2 || toggles().no_split_k) return 1;
+  const int max_pairs = sm_count() / 2;
+  for (int sk = 4; sk >= 2; sk /= 2)
+    if (tiles * sk <= max_pairs - max_pairs % sk && num_kb / sk >= 8) return sk;
+  return 1;
 }
 
 // (UN, NJ) for a channel count: 320 k -> 2 x 160; 160 k -> 1 x 160; 256 k -> 2 x 128; 128 k -> 1 x 128
@@ -467,12 +546,16 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
   if (p.nph == 1) {
     OutMaps<false> m1p;
     m1p.m[0] = mo.m[0];
-    r = un == 160 ? (nj == 2 ? launch2<160, 2, false>(m0, m1, mb, m1p, p, st) : launch2<160, 1, false>(m0, m1, mb, m1p, p, st))
-                  : (nj == 2 ? launch2<128, 2, false>(m0, m1, mb, m1p, p, st) : launch2<128, 1, false>(m0, m1, mb, m1p, p, st));
+    const int sk = (a.mode == CONV_FPROP && a.stride == 1) ? split_k(p.pair_tiles_m * p.n_tiles, ntaps * p.c_blocks, un, nj) : 1;
+    if (sk == 4) r = launch2<160, 2, false, 4>(m0, m1, mb, m1p, p, st);
+    else if (sk == 2) r = launch2<160, 2, false, 2>(m0, m1, mb, m1p, p, st);
+    else
+      r = un == 160 ? (nj == 2 ? launch2<160, 2, false, 1>(m0, m1, mb, m1p, p, st) : launch2<160, 1, false, 1>(m0, m1, mb, m1p, p, st))
+                    : (nj == 2 ? launch2<128, 2, false, 1>(m0, m1, mb, m1p, p, st) : launch2<128, 1, false, 1>(m0, m1, mb, m1p, p, st));
   } else {
     for (int ph = p.nph; ph < 4; ++ph) mo.m[ph] = mo.m[0];
-    r = un == 160 ? (nj == 2 ? launch2<160, 2, true>(m0, m1, mb, mo, p, st) : launch2<160, 1, true>(m0, m1, mb, mo, p, st))
-                  : (nj == 2 ? launch2<128, 2, true>(m0, m1, mb, mo, p, st) : launch2<128, 1, true>(m0, m1, mb, mo, p, st));
+    r = un == 160 ? (nj == 2 ? launch2<160, 2, true, 1>(m0, m1, mb, mo, p, st) : launch2<160, 1, true, 1>(m0, m1, mb, mo, p, st))
+                  : (nj == 2 ? launch2<128, 2, true, 1>(m0, m1, mb, mo, p, st) : launch2<128, 1, true, 1>(m0, m1, mb, mo, p, st));
   }
   return r ? 1 : -1;
 }
@@ -483,8 +566,18 @@ int conv_tc2(const ConvArgs& a, cudaStream_t st) {
 // kernel is preferred while all of its tiles still fit one wave.  PULSE_CONV_1CTA_TILES overrides the bound
 // (single-CTA tiles; 0 = never).
 static int one_cta_tile_bound() { return toggles().conv_1cta_tiles >= 0 ? toggles().conv_1cta_tiles : sm_count(); }
+// split-K factor conv_tc2 would use for this conv (1: none)
+static int split_k_of(const ConvArgs& a) {
+  if (a.mode != CONV_FPROP || a.stride != 1 || !conv_tc2_supported(a)) return 1;
+  int un, nj, bw, bh, bn;
+  pick_tile(a.cout, un, nj);
+  if (!tile_geometry(a.hout, a.wout, bw, bh, bn)) return 1;
+  const int tiles_m = ((a.hout + bh - 1) / bh) * ((a.n + bn - 1) / bn);
+  return split_k(((tiles_m + 1) / 2) * (a.cout / (un * nj)), a.ksize * a.ksize * (a.src.c() / 64), un, nj);
+}
 static bool prefer_1cta(const ConvArgs& a) {
   if (!conv_tc_supported(a)) return false;
+  if (split_k_of(a) > 1) return false;       // few tiles and a long K: the pair kernel splits K over a cluster instead
   const bool s2d = a.mode == CONV_DGRAD_S2 || a.mode == CONV_UP2;      // pixel grid = the low-resolution side
   int bw, bh, bn;
   if (!tile_geometry(s2d ? a.hin : a.hout, s2d ? a.win : a.wout, bw, bh, bn)) return false;
