@@ -244,10 +244,13 @@ pulse_status_t pulse_conv2d(int dtype, int kernel, const void* d_src0, int c0, c
 pulse_status_t pulse_conv2d_dgrad(int dtype, int kernel, const void* d_g, int n, int h, int w, int cin,
                                   int ksize, int stride, const void* d_w, int cout, void* d_wt_scratch,
                                   void* d_g_in, int accumulate, void* stream);
-/* dw[cout][k][k][c0+c1] += sum_{n,y,x} g[n,y,x,co] in[n, y st+r-pad, x st+s-pad, c]  (fp32, accumulated) */
+/* dw[cout][k][k][c0+c1] (+)= sum_{n,y,x} g[n,y,x,co] in[n, y st+r-pad, x st+s-pad, c]  (fp32).
+ * accumulate = 1: added to what d_dw holds.  accumulate = 0: d_dw is overwritten, whatever it held - stored directly
+ * where the tcgen05 kernel owns whole output tiles (many tiles, few pixels: the deep UNet levels), zeroed by the call
+ * and added into otherwise. */
 pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1, int c1,
                                   int n, int h, int w, int ksize, int stride, const void* d_g, int cout,
-                                  float* d_dw, void* stream);
+                                  float* d_dw, int accumulate, void* stream);
 
 /* Nearest-2x upsample followed by a 3x3 pad-1 conv (row a6), computed WITHOUT the upsampled tensor:
  * output pixel (2y+py, 2x+px) is a 2x2 conv of the low-resolution input with the pre-summed weights of its parity phase

@@ -85,7 +85,7 @@ _SIG = {
     "pulse_conv2d_dgrad": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int,
                            _vp, _vp, C.c_int, _vp],
     "pulse_conv2d_wgrad": [C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
-                           _vp, C.c_int, _vp, _vp],
+                           _vp, C.c_int, _vp, C.c_int, _vp],
     "pulse_upsample_conv2d": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp, _vp, _vp, _vp],
     "pulse_upsample_conv2d_dgrad": [C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp, _vp],
     "pulse_upsample_conv2d_wgrad": [C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_int, _vp, _vp],
@@ -417,13 +417,16 @@ def conv2d_dgrad(g, w, in_hw, stride=1, kernel="auto", g_in=None):
     return g_in
 
 
-def conv2d_wgrad(src0, g, ksize, src1=None, stride=1, force_simt=False):
+def conv2d_wgrad(src0, g, ksize, src1=None, stride=1, force_simt=False, dw=None):
+    """dw given: += into it; else a fresh gradient (written into a NaN-filled buffer: accumulate = 0 must overwrite)."""
     n, h, wd, c0 = src0.shape
     c1 = 0 if src1 is None else src1.shape[3]
     cout = g.shape[3]
-    dw = torch.zeros((cout, ksize, ksize, c0 + c1), dtype=torch.float32, device=g.device)
+    acc = dw is not None
+    if dw is None:
+        dw = torch.full((cout, ksize, ksize, c0 + c1), float("nan"), dtype=torch.float32, device=g.device)
     _ck(lib.pulse_conv2d_wgrad(_cd(src0), int(force_simt), _ptr(src0), c0, _ptr(src1), c1, n, h, wd, ksize, stride,
-                               _ptr(g), cout, _ptr(dw), _stream()))
+                               _ptr(g), cout, _ptr(dw), int(acc), _stream()))
     return dw
 
 

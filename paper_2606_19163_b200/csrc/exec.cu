@@ -1,3 +1,4 @@
+#include <algorithm>
 // exec.cu - pulse_stage_forward / pulse_stage_backward / temb and loss helpers:
 // walks the op plan and enqueues kernels.  Rows a1-a11 of SURVEY.md 8a.
 #include "stage.h"
@@ -26,7 +27,8 @@ struct Ctx {
   // backward: what the tail (bias / temb-projection gradients of every op, then optionally the timestep-MLP
   // backward) needs; it is enqueued beside the chain as soon as the last g_p is complete (tail_work)
   const float* emb = nullptr; float* g_temb = nullptr; const float* temb_stash = nullptr;
-  int acc_w = 0; bool last_op = false, tail_done = false;
+  int acc_w = 0, acc_temb = 0; bool last_op = false, tail_done = false;
+  bool own_ok = true;      // this call also zeroes the gradient buffer (not the encoder half of a split stage): see run_wgrad
   int op_lo = 0, op_hi = 0;      // ops this call runs: [op_lo, op_hi)
   bool err = false;
   cudaEvent_t new_event() {
@@ -142,7 +144,13 @@ void run_wgrad(Ctx& c, const WgradArgs& a) {
   Prof pr(c.s, c.wst(), tc ? PULSE_KCLASS_WGRAD_TC : PULSE_KCLASS_CONV_SIMT,
           a.up2 ? 2.0 * a.n * a.hin * a.win * a.cout * a.src.c() * 16
                 : 2.0 * a.n * a.hout * a.wout * a.cout * a.src.c() * a.ksize * a.ksize, 0.0);
-  const int r = tc ? wgrad_tc_any(a, c.wst()) : wgrad_simt(a, c.wst());
+  WgradArgs b = a;
+  if (tc && c.own_ok && wgrad_whole_tiles(a)) {
+    const size_t off = (size_t)((const char*)a.dw - (const char*)c.s->d_grads);
+    if (c.s->own_valid) b.overwrite = !c.acc_w;       // (its range was left out of the zeroing: backward_impl)
+    else c.s->own_runs.push_back({off, (size_t)a.cout * a.ksize * a.ksize * a.src.c() * sizeof(float)});
+  }
+  const int r = tc ? wgrad_tc_any(b, c.wst()) : wgrad_simt(b, c.wst());
   if (r < 0) c.err = true; else c.s->launches += r;
 }
 // GroupNorm+SiLU wrappers: algorithmic bytes 2 x esz per element forward, 3 x esz backward
@@ -578,7 +586,7 @@ void tail_work(Ctx& c) {
     cudaStreamWaitEvent(c.side2, e, 0);
   }
   small_grads(c, c.emb, c.g_temb, st);
-  if (c.temb_stash && temb_backward_impl(c.s, c.g_temb, c.temb_stash, c.acc_w, st) != PULSE_OK) c.err = true;
+  if (c.temb_stash && temb_backward_impl(c.s, c.g_temb, c.temb_stash, c.acc_temb, st) != PULSE_OK) c.err = true;
   c.tail_done = true;
 }
 
@@ -751,13 +759,18 @@ extern "C" pulse_status_t pulse_stage_forward_dec(pulse_stage_t* s, pulse_skip_c
 
 static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache, int64_t mb, const void* d_g_d_out,
                                     const void* d_g_e_out, void* d_g_x_in, void* d_g_h_in, float* d_g_temb,
-                                    const float* d_temb_stash, int accumulate_wgrad, void* stream, int parts = PART_ALL) {
+                                    const float* d_temb_stash, int accumulate_wgrad, void* stream, int parts = PART_ALL,
+                                    int accumulate_temb = -1) {
   pulse_status_t stt = check_bound(s, cache);
   if (stt) return stt;
+  if (accumulate_temb < 0) accumulate_temb = accumulate_wgrad;
   if (parts == PART_ALL && (s->d.flags & PULSE_FLAG_SPLIT)) {      // a split stage runs its one-call backward as the two halves
     stt = backward_impl(s, cache, mb, d_g_d_out, nullptr, nullptr, d_g_h_in, d_g_temb, nullptr, accumulate_wgrad, stream, PART_DEC);
     if (stt) return stt;
-    return backward_impl(s, cache, mb, nullptr, d_g_e_out, d_g_x_in, nullptr, d_g_temb, d_temb_stash, 1, stream, PART_ENC);
+    // the encoder half adds to what the decoder half (which zeroed the buffer) wrote; the timestep MLP's own gradients
+    // are written by this half only and follow the caller's flag
+    return backward_impl(s, cache, mb, nullptr, d_g_e_out, d_g_x_in, nullptr, d_g_temb, d_temb_stash, 1, stream, PART_ENC,
+                         accumulate_wgrad);
   }
   const bool open = s->d.link == PULSE_LINK_OPEN;
   const bool enc = parts & PART_ENC, dec = parts & PART_DEC;
@@ -776,6 +789,7 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
   c.work = s->d_work;
   c.stash = s->d_work + s->work_bytes + (size_t)slot * s->stash_bytes;
   c.emb = (const float*)(c.stash + s->emb_off); c.g_temb = d_g_temb; c.temb_stash = enc ? d_temb_stash : nullptr; c.acc_w = accumulate_wgrad;
+  c.acc_temb = accumulate_temb; c.own_ok = dec;
   const int n_first = s->n_enc + s->n_mid, nops = (int)s->ops.size();
   c.op_lo = enc ? 0 : n_first; c.op_hi = dec ? nops : n_first;
   setup_side(s, c);
@@ -794,8 +808,13 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
     }
     s->wt_valid = true;
   }
-  if (dec && !accumulate_wgrad)
-    CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
+  if (dec && !accumulate_wgrad) {
+    if (!s->own_valid) {
+      CK_CUDA(cudaMemsetAsync((char*)s->d_grads + s->temb_grad_bytes, 0, s->grad_bytes - s->temb_grad_bytes, c.st));
+    } else {                      // everything but the weight gradients that are stored whole
+      for (const auto& r : s->zero_runs) CK_CUDA(cudaMemsetAsync((char*)s->d_grads + r.first, 0, r.second, c.st));
+    }
+  }
   CK_CUDA(cudaMemsetAsync(c.work + s->zero_begin, 0, s->zero_end - s->zero_begin, c.st));
   const bool split = parts != PART_ALL;
   const bool al = (((uintptr_t)d_g_d_out | (uintptr_t)d_g_h_in | (uintptr_t)d_g_x_in) & 255) == 0;
@@ -894,6 +913,17 @@ static pulse_status_t backward_impl(pulse_stage_t* s, pulse_skip_cache_t* cache,
   if (c.err) return fail(PULSE_ERR_CUDA, "tensor-core conv launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   if (enc) {
+    if (!s->own_valid) {          // every conv of the stage has been seen once: what is left to zero at the start of a step
+      std::sort(s->own_runs.begin(), s->own_runs.end());
+      s->own_runs.erase(std::unique(s->own_runs.begin(), s->own_runs.end()), s->own_runs.end());
+      size_t at = s->temb_grad_bytes;
+      for (const auto& r : s->own_runs) {
+        if (r.first > at) s->zero_runs.push_back({at, r.first - at});
+        at = r.first + r.second;
+      }
+      if (s->grad_bytes > at) s->zero_runs.push_back({at, s->grad_bytes - at});
+      s->own_valid = true;
+    }
     cache->mb[slot] = -1;
     cache->phase[slot] = 0;
     cache->live--;
@@ -1070,13 +1100,18 @@ extern "C" pulse_status_t pulse_conv2d_dgrad(int dtype, int kernel, const void* 
 }
 extern "C" pulse_status_t pulse_conv2d_wgrad(int dtype, int force_simt, const void* d_src0, int c0, const void* d_src1,
                                              int c1, int n, int h, int w, int ksize, int stride, const void* d_g, int cout,
-                                             float* d_dw, void* stream) {
+                                             float* d_dw, int accumulate, void* stream) {
   pulse_status_t s = check_conv(dtype, c0, c1, n, h, w, ksize, stride, cout);
   if (s) return s;
   if (!d_src0 || !d_g || !d_dw || (c1 && !d_src1)) return fail(PULSE_ERR_INVALID_ARG, "null pointer");
   WgradArgs a{dtype == PULSE_F32 ? DT_F32 : DT_BF16, Cat{d_src0, c0, d_src1, c1}, n, h, w, d_g, h / stride, w / stride,
               cout, ksize, stride, d_dw};
-  const int r = (!force_simt && wgrad_tc_any_supported(a)) ? wgrad_tc_any(a, (cudaStream_t)stream) : wgrad_simt(a, (cudaStream_t)stream);
+  const bool tc = !force_simt && wgrad_tc_any_supported(a);
+  if (!accumulate) {
+    if (tc && wgrad_whole_tiles(a)) a.overwrite = 1;
+    else CK_CUDA(cudaMemsetAsync(d_dw, 0, (size_t)cout * ksize * ksize * (c0 + c1) * sizeof(float), (cudaStream_t)stream));
+  }
+  const int r = tc ? wgrad_tc_any(a, (cudaStream_t)stream) : wgrad_simt(a, (cudaStream_t)stream);
   if (r < 0) return fail(PULSE_ERR_CUDA, "tensor-core wgrad launch failed: %s", tc_last_error());
   CK_CUDA(cudaGetLastError());
   return PULSE_OK;

@@ -144,7 +144,11 @@ struct WgradArgs {
   int ksize, stride;
   float* dw;                      // [cout][k][k][src.c()] fp32, atomically accumulated
   int up2 = 0;                    // 1: the conv of CONV_UP2: src low-res [n,hin,win,c], g [n,2hin,2win,cout]; dw is the 9-tap gradient
+  int overwrite = 0;              // 1: dw = (not +=); honoured only where wgrad_whole_tiles(a) holds (the caller zeroes otherwise)
 };
+// the tcgen05 pair kernel gives every output tile of dw to ONE CTA pair (many output tiles, few pixels: the deep UNet
+// levels), so that it can store instead of reduce-add and dw needs no zeroing
+bool wgrad_whole_tiles(const WgradArgs& a);
 int wgrad_simt(const WgradArgs& a, cudaStream_t st);
 // 4 channels on one side (conv_in, head; conv_thin.cu): conv_simt / wgrad_simt route to these when they apply
 bool conv_thin_supported(const ConvArgs& a);

@@ -2,6 +2,7 @@
 #pragma once
 #include <map>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/pulse.h"
@@ -87,6 +88,10 @@ struct pulse_stage {
   size_t zero_begin = 0, zero_end = 0;      // workspace: backward sums area, zeroed at the start of backward
   bool wt_valid = false;                    // transposed weights match the bound parameters
   bool eout_grad_by_dec = false;            // PULSE_FLAG_SPLIT: a decoder op writes the gradient of e_out before g_e_out arrives
+  // weight-gradient tensors whose tcgen05 kernel owns whole output tiles (kernels.h wgrad_whole_tiles): byte ranges of
+  // d_grads, recorded by the first backward; later first-of-a-step backwards store into them and zero only the rest
+  std::vector<std::pair<size_t, size_t>> own_runs, zero_runs;
+  bool own_valid = false;
   bool wp_valid = false;                    // pre-summed phase weights of the up convs (forward) match them
   // per-stage workspace offsets (bytes)
   size_t w_ga2 = 0, w_gh1 = 0, w_gh1b = 0, w_ga1 = 0, w_gsc = 0, w_gu = 0, w_tmpf = 0, w_gqkv = 0, w_t4a = 0, w_t4b = 0, w_tca = 0, w_tcb = 0;

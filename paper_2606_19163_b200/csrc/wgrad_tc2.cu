@@ -46,6 +46,7 @@ struct Wg2Params {
   int pix_tiles, m_tiles, n_tiles;       // m_tiles: pair tiles of 4 units
   long long work;
   int ppt;                               // pairs per output tile (aligned split) or 0 (stream-K)
+  int whole, store;                      // whole: every output tile belongs to one pair (contiguous runs of tiles); store: plain stores
   float* dw;
 };
 
@@ -68,6 +69,9 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
     const int ot = pair / p.ppt, k = pair - ot * p.ppt;
     wb = (long long)ot * p.pix_tiles + (long long)p.pix_tiles * k / p.ppt;
     we = (long long)ot * p.pix_tiles + (long long)p.pix_tiles * (k + 1) / p.ppt;
+  } else if (p.whole) {
+    const long long tiles = (long long)p.m_tiles * p.n_tiles;
+    wb = tiles * pair / npairs * p.pix_tiles; we = tiles * (pair + 1) / npairs * p.pix_tiles;
   } else {
     wb = p.work * pair / npairs; we = p.work * (pair + 1) / npairs;
   }
@@ -244,7 +248,8 @@ wgrad_tc2_k(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ C
           __syncwarp();
           if (lane == 0) {
             if (!UP2) {
-              tma_reduce_add_2d(&mapW, stg + buf * 2048, kcol, nt * N_TOT + ch * 16);
+              if (p.store) tma_store_2d(&mapW, stg + buf * 2048, kcol, nt * N_TOT + ch * 16);
+              else tma_reduce_add_2d(&mapW, stg + buf * 2048, kcol, nt * N_TOT + ch * 16);
             } else {
               for (int r = r0; r <= r1; ++r)
                 for (int s_ = s0; s_ <= s1; ++s_)
@@ -284,6 +289,16 @@ bool wgrad_tc2_supported(const WgradArgs& a) {
     return false;
   }
   return tile_geometry64(a.hout, a.wout, bw, bh, bn);
+}
+
+// Whole-tile ownership: at least as many output tiles as pairs, and runs of ceil(tiles / pairs) tiles waste at most a
+// quarter of the machine.  Then a tile's pixel range is never shared, the flush may STORE (first backward of a step) and
+// the 59 - 118 MB gradient of a 1280-channel conv is written once instead of zeroed, read and written.
+bool wgrad_whole_tiles(const WgradArgs& a) {
+  if (a.up2 || !wgrad_tc2_supported(a) || toggles().wgrad_1cta) return false;
+  const long long units = (long long)a.ksize * a.ksize * (a.src.c() / 64);
+  const long long tiles = (units + 3) / 4 * (a.cout / N_TOT), pairs = sm_count() / 2;
+  return tiles >= pairs && ((tiles + pairs - 1) / pairs) * pairs * 4 <= 5 * tiles;
 }
 
 int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
@@ -333,6 +348,8 @@ int wgrad_tc2(const WgradArgs& a, cudaStream_t st) {
   if (p.work / 4 < pairs) pairs = p.work / 4 > 0 ? p.work / 4 : 1;
   const long long out_tiles = (long long)p.m_tiles * p.n_tiles;
   p.ppt = 0;
+  p.whole = wgrad_whole_tiles(a); p.store = p.whole && a.overwrite;
+  if (p.whole) pairs = sm_count() / 2;
   if (out_tiles <= pairs && p.pix_tiles >= 4 * (pairs / out_tiles)) {       // aligned split: one flush per pair
     p.ppt = (int)(pairs / out_tiles);
     pairs = p.ppt * out_tiles;

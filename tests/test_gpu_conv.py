@@ -143,6 +143,10 @@ def test_conv_dgrad(case, kernel):
 WGRAD_CASES = [
     (3, 8, 8, 64, 0, 320, 3, 1), (2, 16, 16, 128, 64, 320, 3, 1), (1, 32, 32, 64, 0, 320, 1, 1),
     (2, 16, 16, 128, 0, 320, 3, 2), (1, 64, 64, 128, 0, 640, 3, 1), (2, 16, 16, 192, 128, 320, 1, 1),
+    # whole-tile ownership (at least as many output tiles as CTA pairs: stores instead of reduce-adds)
+    (2, 8, 8, 1280, 0, 1280, 3, 1),            # 180 output tiles: runs of 2 - 3 tiles per pair
+    (2, 8, 8, 1280, 640, 640, 3, 1),           # virtual concat, 68 x 2 = 136 tiles, last unit block ragged (270 units)
+    (3, 8, 8, 1280, 0, 1280, 1, 1),            # 1x1: 20 units x 4 = 20 tiles < pairs: the shared-tile (reduce-add) path
 ]
 
 
@@ -163,6 +167,13 @@ def test_conv_wgrad(case, simt):
     rms = float(ref.pow(2).mean().sqrt())
     err = float((got - ref).abs().max())
     assert err <= 1e-4 * rms * 10, f"wgrad {case} simt={simt}: max err {err:.3e} vs rms {rms:.3e}"   # fp32 sums of exact products
+    # += on top of a seeded gradient (the accumulating backwards of a wave)
+    base = torch.as_tensor(rng.standard_normal((cout, k, k, c0 + c1)).astype(np.float32))
+    acc = B.conv2d_wgrad(dev_nhwc(x0), dev_nhwc(g), k, None if x1 is None else dev_nhwc(x1), stride=stride,
+                         force_simt=simt, dw=base.cuda())
+    torch.cuda.synchronize()
+    err = float((acc.permute(0, 3, 1, 2).double().cpu() - ref - base.permute(0, 3, 1, 2).double()).abs().max())
+    assert err <= 1e-4 * rms * 10 + 1e-6, f"wgrad += {case} simt={simt}: max err {err:.3e} vs rms {rms:.3e}"
 
 
 # ------------------------------------------------------------------ nearest-2x upsample + conv, 4-phase form (row a6)

@@ -47,7 +47,7 @@ with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "bf
 CAP = 0.15          # allowance cap for tensors whose own storage floor is below CAP / 2
 
 
-def run_gpu(desc, data, flags=0, with_g_e_out=False, order=None, max_inflight=None):
+def run_gpu(desc, data, flags=0, with_g_e_out=False, order=None, max_inflight=None, steps=1):
     """order: list of ("F", m) / ("B", m) events (default: one step, or the wave F0..F{M-1}, B{M-1}..B0)."""
     B = _binding()
     st = B.Stage(desc, flags=flags, max_inflight=max_inflight)
@@ -92,27 +92,34 @@ def run_gpu(desc, data, flags=0, with_g_e_out=False, order=None, max_inflight=No
         outs = [done[m] for m in range(M)]
         assert st.cache_stats()["live_slots"] == 0
     elif M == 1:
-        r = st.step(0, devs[0], 1.0, accumulate=False)
+        for rep in range(steps):       # steps > 1: the later steps run what the first backward of a stage prepares
+            if rep:                    # (weight gradients stored whole into a buffer that is no longer zeroed): poison it
+                st.d_grads.fill_(255)
+            r = st.step(0, devs[0], 1.0, accumulate=False)
         outs.append(r)
     else:       # wave: F0..F{M-1}, B{M-1}..B0 (configs[4])
-        fw = []
-        for m, dev in enumerate(devs):
-            emb, tst = st.temb_forward(dev["t"])
-            e_out, d_out = st.forward(m, dev["x_in"], dev.get("h_in"), emb)
-            fw.append((emb, tst, e_out, d_out))
-        peak = st.cache_stats()
-        assert peak["live_slots"] == M and peak["peak_bytes"] == M * st.skip_bytes
-        for m in reversed(range(M)):
-            emb, tst, e_out, d_out = fw[m]
-            loss, g_d = st.mse(d_out, devs[m]["target"], 1.0 / M)
-            g_temb = torch.zeros_like(emb)
-            first = m == M - 1
-            g_x_in, g_h_in = st.backward(m, g_d, None, True, g_temb, accumulate=not first)
-            st.temb_backward(g_temb, tst, accumulate=not first)
-            outs.append({"loss": loss, "e_out": e_out, "d_out": d_out, "g_x_in": g_x_in, "g_h_in": g_h_in,
-                         "g_emb": g_temb, "emb": emb})
-        outs.reverse()
-        assert st.cache_stats()["live_slots"] == 0
+        for rep in range(steps):
+            if rep:
+                st.d_grads.fill_(255)
+                outs = []
+            fw = []
+            for m, dev in enumerate(devs):
+                emb, tst = st.temb_forward(dev["t"])
+                e_out, d_out = st.forward(m, dev["x_in"], dev.get("h_in"), emb)
+                fw.append((emb, tst, e_out, d_out))
+            peak = st.cache_stats()
+            assert peak["live_slots"] == M and peak["peak_bytes"] == M * st.skip_bytes
+            for m in reversed(range(M)):
+                emb, tst, e_out, d_out = fw[m]
+                loss, g_d = st.mse(d_out, devs[m]["target"], 1.0 / M)
+                g_temb = torch.zeros_like(emb)
+                first = m == M - 1
+                g_x_in, g_h_in = st.backward(m, g_d, None, True, g_temb, accumulate=not first)
+                st.temb_backward(g_temb, tst, accumulate=not first)
+                outs.append({"loss": loss, "e_out": e_out, "d_out": d_out, "g_x_in": g_x_in, "g_h_in": g_h_in,
+                             "g_emb": g_temb, "emb": emb})
+            outs.reverse()
+            assert st.cache_stats()["live_slots"] == 0
     torch.cuda.synchronize()
     res = {"per_mb": [], "param_grads": st.grads(), "stage": st}
     for r in outs:
@@ -146,12 +153,16 @@ def flatten(per_mb, grads):
     return out
 
 
-def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, gold=None, order=None,
+def check(desc, seed=0, flags=0, oracle_dtype=torch.float64, with_g_e_out=False, tol=None, gold=None, order=None, steps=2,
           max_inflight=None, slack=1.0):
     """fp32: every tensor within 1e-4 of the exact oracle.  bf16: every tensor within the plain 2e-2, except the
-    tensors named in tests/golden/bf16_floor.json[gold] (see the module docstring)."""
+    tensors named in tests/golden/bf16_floor.json[gold] (see the module docstring).
+    steps = 2 (where the calls are not given by `order`): the step is run twice on the same inputs, the gradient buffer
+    filled with NaN patterns in between, and the SECOND step is compared - the steady state a training loop and bench.py
+    see (the first backward of a stage also records which weight gradients later steps store whole instead of adding
+    into a zeroed buffer)."""
     data = W.draw(desc, seed, with_g_e_out=with_g_e_out)
-    got_raw = run_gpu(desc, data, flags, with_g_e_out, order, max_inflight)
+    got_raw = run_gpu(desc, data, flags, with_g_e_out, order, max_inflight, steps)
     got = flatten(got_raw["per_mb"], got_raw["param_grads"])
     ref = flatten(*oracle_run(desc, data, oracle_dtype))
     bf16 = desc["dtype"] == "bf16"
